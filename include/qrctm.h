@@ -1,0 +1,176 @@
+/* qrctm.h -- C ABI of the B200-native QR-CTMRG library (libqrctm.so).
+ *
+ * One C4v-symmetric QR-CTMRG iteration for a single-site real iPEPS, FP64, one
+ * GPU, as defined in "Accelerating two-dimensional tensor network contractions
+ * using QR-decompositions" (arXiv 2505.00494; PAPER.md below is
+ * /root/reference/PAPER.md).  Equation labels (E0)..(E5) are the index-form
+ * statement of the paper's Fig. 1 given in DESIGN.md section 2.
+ *
+ * Notation: d physical dim, D bond dim, b = D*D, chi boundary dim, m = chi*b.
+ * All arrays are C-order (row-major) FP64.
+ *   A[d][D][D][D][D]   site tensor, aux legs cyclic (up,left,down,right)
+ *   C[chi][chi]        corner (symmetric)
+ *   T[chi][b][chi]     edge, T[i][s][k] = T[k][s][i]
+ *   Q[chi*b][chi]      isometry of the last step (rows (j,u))
+ *   R[chi][chi]        upper triangular, diag(R) >= 0
+ *
+ * Pointers.  Every `double*` argument may be a HOST pointer or a DEVICE pointer
+ * (e.g. torch tensor .data_ptr()); the library finds out which with
+ * cudaPointerGetAttributes and copies accordingly.  Nothing the caller passes
+ * is retained after the call returns (set_* copy in, get_* copy out).  The
+ * handle owns all device workspaces; they are allocated in qrctm_create (or
+ * taken from the caller through qrctm_create_in) and nothing is allocated in
+ * qrctm_step / qrctm_run.
+ *
+ * Errors.  Every function returns an int status: QRCTM_OK (0) or a negative
+ * code.  qrctm_last_error gives a text for the last failure on that handle.
+ * No exceptions, no abort, nothing is printed.  Not converging within
+ * max_iter is NOT an error.
+ *
+ * Determinism.  Same inputs give bitwise-identical outputs run to run: all
+ * reductions use fixed trees, there are no floating-point atomics.
+ *
+ * There is no CPU fallback: without a CUDA device qrctm_create fails with
+ * QRCTM_ERR_CUDA.
+ */
+#ifndef QRCTM_H
+#define QRCTM_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct qrctm qrctm_t; /* opaque */
+
+enum {
+  QRCTM_OK = 0,
+  QRCTM_ERR_INVALID_ARG = -1, /* null pointer, d/D/chi < 1, size overflow, bad option      */
+  QRCTM_ERR_NOT_READY = -2,   /* step/run before set_A and set_env                         */
+  QRCTM_ERR_CUDA = -3,        /* a CUDA call failed; see qrctm_last_error                  */
+  QRCTM_ERR_NUMERIC = -4      /* NaN/Inf or zero Frobenius norm of C' or T'                */
+};
+
+/* Options for qrctm_set_option. */
+enum {
+  QRCTM_OPT_CORNER_MODE = 1, /* 0 = accelerated (E4) [default], 1 = enlarged corner (E5)+(E4')          */
+  QRCTM_OPT_SYMMETRIZE = 2,  /* 1 [default] = symmetrise C', T' before normalising, 0 = only normalise   */
+  QRCTM_OPT_CHECK_EVERY = 3, /* qrctm_run computes the corner spectrum / delta every n steps, default 1 */
+  QRCTM_OPT_GEMM_PATH = 4    /* 0 = FP64 tensor-core (DMMA) tiles [default], 1 = plain DFMA reference kernel */
+};
+
+/* Create a handle for dimensions (d, D, chi); allocates every workspace with
+ * cudaMalloc on the current device (about 16*(chi*D*D)^2 bytes for the two
+ * m x m intermediates plus 8*D^8 for the double-layer tensor).  *out = NULL on
+ * failure. */
+int qrctm_create(int d, int D, int chi, qrctm_t** out);
+
+/* Bytes of device workspace a handle for (d, D, chi) needs (for callers that
+ * own the memory, e.g. a torch tensor).  Returns 0 on invalid arguments. */
+unsigned long long qrctm_workspace_bytes(int d, int D, int chi);
+
+/* Same as qrctm_create, but all device workspaces are carved out of the
+ * caller's DEVICE buffer `workspace` (>= qrctm_workspace_bytes, 256-byte
+ * aligned), which must outlive the handle.  This is how the Python binding
+ * lets PyTorch own device memory. */
+int qrctm_create_in(int d, int D, int chi, void* workspace,
+                    unsigned long long workspace_bytes, qrctm_t** out);
+
+int qrctm_destroy(qrctm_t* h);
+
+/* All later work of this handle is enqueued on `cuda_stream` (a cudaStream_t,
+ * e.g. torch.cuda.current_stream().cuda_stream).  Default: the legacy stream. */
+int qrctm_set_stream(qrctm_t* h, void* cuda_stream);
+
+/* K0.  Copy A in and build the double-layer tensor (E0)
+ *   a[(u u')][(l l')][(d d')][(r r')] = sum_s A[s][u][l][d][r] A[s][u'][l'][d'][r']
+ * (Fig. 1(b)).  Keeps the current environment C, T (the paper's
+ * optimiser reuses it across updates of A). */
+int qrctm_set_A(qrctm_t* h, const double* A);
+
+/* Copy an initial environment in, symmetrise (if enabled) and Frobenius-
+ * normalise it, reset the convergence history (previous spectrum = spectrum of
+ * this C). */
+int qrctm_set_env(qrctm_t* h, const double* C, const double* T);
+
+/* One QR-CTMRG iteration, asynchronous on the stream:
+ *   (E1) c~[(j,u),k] = sum_i C[j,i] T[i,u,k]
+ *   (E2) c~ = Q R, unpivoted Householder QR, then signs fixed so diag(R) >= 0
+ *   (E3) T'[m,r,n] = sum Q[(j,u),m] T[j,l,J] a[u,l,d,r] Q[(J,d),n]
+ *   (E4) C'[p,n]   = sum R[m,k] T'[m,r,p] Q[(k,r),n]          (Fig. 1(f), 3rd diagram)
+ *   then C <- sym(C')/||.||_F, T <- sym(T')/||.||_F.
+ * A NaN/Inf/zero norm is reported by the next synchronising call. */
+int qrctm_step(qrctm_t* h);
+
+/* Iterate: step; every CHECK_EVERY steps compute s = descending |eigenvalues|
+ * of C and delta = max_i |s_i - s_i(previous check)|; stop when delta < tol or
+ * after max_iter steps.  Synchronises before returning.  iters_done = steps
+ * executed; final_delta = last delta (+inf if never checked).  Either output
+ * pointer may be NULL.  HOST pointers. */
+int qrctm_run(qrctm_t* h, int max_iter, double tol, int* iters_done, double* final_delta);
+
+/* Copy the current normalised environment out (either pointer may be NULL). */
+int qrctm_get_env(qrctm_t* h, double* C, double* T);
+
+/* Descending singular values (= |eigenvalues|) of the current normalised C,
+ * computed on the device by a cyclic Jacobi eigenvalue iteration; s has chi
+ * entries; sum s^2 = 1. */
+int qrctm_get_corner_spectrum(qrctm_t* h, double* s);
+
+/* Q[chi*b][chi] and R[chi][chi] of the last step (either may be NULL). */
+int qrctm_get_qr(qrctm_t* h, double* Q, double* R);
+
+/* Un-normalised C'[chi][chi], T'[chi][b][chi] of the last step (either may be NULL). */
+int qrctm_get_raw(qrctm_t* h, double* Cn, double* Tn);
+
+/* Copy the double-layer tensor a[b][b][b][b] out. */
+int qrctm_get_a(qrctm_t* h, double* a);
+
+/* Norm per site kappa = Z1 * Z4 / Z2^2 of the current environment, with
+ * Z4 = tr C^4, Z2 the 2x3 network CTC/CTC, Z1 the 3x3 network CTC/TaT/CTC
+ * (reading A8).  HOST pointer.  Synchronises. */
+int qrctm_norm_per_site(qrctm_t* h, double* kappa);
+
+/* min_k R_kk / max_k R_kk of the last step: a conditioning diagnostic for the
+ * uniqueness of Q (DESIGN.md hazard H1).  HOST pointer.  Synchronises. */
+int qrctm_r_diag_ratio(qrctm_t* h, double* ratio);
+
+int qrctm_set_option(qrctm_t* h, int key, int value);
+
+/* Number of kernels this handle has launched so far (for bench.py's
+ * gpu_launches), and reset. */
+long long qrctm_launch_count(const qrctm_t* h);
+
+/* Event-timed profile of one step: runs one qrctm_step with CUDA events around
+ * each stage and returns milliseconds in ms[0..QRCTM_NSTAGE-1]:
+ * 0 K1 reduced corner, 1 K2 QR (panel+WY+form Q+sign), 2 K3 half-absorb,
+ * 3 K4 absorb a, 4 K5 project, 5 K6 corner, 6 K7 symmetrise+normalise. */
+#define QRCTM_NSTAGE 7
+int qrctm_profile_step(qrctm_t* h, float* ms);
+
+/* Stand-alone FP64 GEMM entry used by the sub-step parity tests and the
+ * roofline bench:  Cmat[M][N] = op(A) * B with B[K][N] row-major and
+ * op(A) = A[M][K] (transA = 0) or A stored as [K][M] (transA = 1).
+ * DEVICE pointers, leading dimensions in elements. path: see QRCTM_OPT_GEMM_PATH. */
+int qrctm_gemm_f64(void* cuda_stream, int path, int transA, int M, int N, int K,
+                   const double* A, long long lda, const double* B, long long ldb,
+                   double* Cmat, long long ldc);
+
+/* Stand-alone QR entry (K2): factor X[rows][cols] (DEVICE, row-major, cols <=
+ * rows) into Q[rows][cols], R[cols][cols] with diag(R) >= 0. work must hold
+ * qrctm_qr_work_bytes(rows, cols) bytes (DEVICE). */
+unsigned long long qrctm_qr_work_bytes(int rows, int cols);
+int qrctm_qr_f64(void* cuda_stream, int rows, int cols, const double* X, double* Q,
+                 double* R, void* work);
+
+/* FP64 issue-rate probe (roofline denominators):
+ * kind 0 = DFMA chains, 1 = DMMA m8n8k4 chains.  Returns TFLOP/s measured with
+ * CUDA events over `iters` loop trips on every SM.  HOST pointer. */
+int qrctm_probe_fp64(int kind, int iters, double* tflops);
+
+const char* qrctm_last_error(const qrctm_t* h);
+const char* qrctm_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QRCTM_H */

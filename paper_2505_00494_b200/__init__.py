@@ -1,0 +1,10 @@
+"""paper_2505_00494_b200 -- B200-native (sm_100a) QR-CTMRG hot path.
+
+The product is the C-ABI shared library `libqrctm.so` (include/qrctm.h, sources in
+csrc/); `binding` is a thin ctypes layer with the same names.  Importing this
+package does not load the library; the first call does, and fails loudly when
+the library or a CUDA device is missing (there is no CPU fallback).
+"""
+from .binding import (QRCTM, QrctmError, gemm_f64, load_library, probe_fp64, qr_f64, version,  # noqa: F401
+                      OPT_CHECK_EVERY, OPT_CORNER_MODE, OPT_GEMM_PATH, OPT_SYMMETRIZE, STAGE_NAMES,
+                      SYMBOLS, LIB_PATH)

@@ -1,0 +1,270 @@
+"""Thin Python binding of libqrctm.so (include/qrctm.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of the shared library; this
+module allocates device memory through PyTorch, passes raw pointers and the
+current CUDA stream, and turns status codes into exceptions.  There is NO CPU
+fallback: if the library is missing or no CUDA device is present the calls
+raise.  Names follow include/qrctm.h one to one.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import (POINTER, byref, c_char_p, c_double, c_float, c_int, c_longlong, c_ulonglong,
+                    c_void_p)
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libqrctm.so")
+
+QRCTM_OK = 0
+OPT_CORNER_MODE, OPT_SYMMETRIZE, OPT_CHECK_EVERY, OPT_GEMM_PATH = 1, 2, 3, 4
+NSTAGE = 7
+STAGE_NAMES = ("K1_reduced_corner", "K2_qr", "K3_half_absorb", "K4_absorb_a", "K5_project",
+               "K6_corner", "K7_normalize")
+
+# every symbol include/qrctm.h declares (tests check that the .so exports them all)
+SYMBOLS = (
+    "qrctm_create", "qrctm_workspace_bytes", "qrctm_create_in", "qrctm_destroy", "qrctm_set_stream",
+    "qrctm_set_A", "qrctm_set_env", "qrctm_step", "qrctm_run", "qrctm_get_env",
+    "qrctm_get_corner_spectrum", "qrctm_get_qr", "qrctm_get_raw", "qrctm_get_a", "qrctm_norm_per_site",
+    "qrctm_r_diag_ratio", "qrctm_set_option", "qrctm_launch_count", "qrctm_profile_step",
+    "qrctm_gemm_f64", "qrctm_qr_work_bytes", "qrctm_qr_f64", "qrctm_probe_fp64", "qrctm_last_error",
+    "qrctm_version",
+)
+
+
+class QrctmError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def load_library() -> ctypes.CDLL:
+    """dlopen libqrctm.so (built in-tree by __graft_entry__.build()).  Raises if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise QrctmError(f"{LIB_PATH} not found: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                         "(there is no CPU fallback)")
+    lib = ctypes.CDLL(LIB_PATH)
+    P = c_void_p
+    lib.qrctm_create.argtypes = [c_int, c_int, c_int, POINTER(P)]
+    lib.qrctm_workspace_bytes.argtypes = [c_int, c_int, c_int]
+    lib.qrctm_workspace_bytes.restype = c_ulonglong
+    lib.qrctm_create_in.argtypes = [c_int, c_int, c_int, P, c_ulonglong, POINTER(P)]
+    lib.qrctm_destroy.argtypes = [P]
+    lib.qrctm_set_stream.argtypes = [P, P]
+    lib.qrctm_set_A.argtypes = [P, P]
+    lib.qrctm_set_env.argtypes = [P, P, P]
+    lib.qrctm_step.argtypes = [P]
+    lib.qrctm_run.argtypes = [P, c_int, c_double, POINTER(c_int), POINTER(c_double)]
+    lib.qrctm_get_env.argtypes = [P, P, P]
+    lib.qrctm_get_corner_spectrum.argtypes = [P, P]
+    lib.qrctm_get_qr.argtypes = [P, P, P]
+    lib.qrctm_get_raw.argtypes = [P, P, P]
+    lib.qrctm_get_a.argtypes = [P, P]
+    lib.qrctm_norm_per_site.argtypes = [P, POINTER(c_double)]
+    lib.qrctm_r_diag_ratio.argtypes = [P, POINTER(c_double)]
+    lib.qrctm_set_option.argtypes = [P, c_int, c_int]
+    lib.qrctm_launch_count.argtypes = [P]
+    lib.qrctm_launch_count.restype = c_longlong
+    lib.qrctm_profile_step.argtypes = [P, POINTER(c_float)]
+    lib.qrctm_gemm_f64.argtypes = [P, c_int, c_int, c_int, c_int, c_int, P, c_longlong, P, c_longlong, P,
+                                   c_longlong]
+    lib.qrctm_qr_work_bytes.argtypes = [c_int, c_int]
+    lib.qrctm_qr_work_bytes.restype = c_ulonglong
+    lib.qrctm_qr_f64.argtypes = [P, c_int, c_int, P, P, P, P]
+    lib.qrctm_probe_fp64.argtypes = [c_int, c_int, POINTER(c_double)]
+    lib.qrctm_last_error.argtypes = [P]
+    lib.qrctm_last_error.restype = c_char_p
+    lib.qrctm_version.restype = c_char_p
+    _lib = lib
+    return lib
+
+
+def _ptr(x):
+    """Raw pointer of a numpy array (host) or torch tensor (host or device)."""
+    if x is None:
+        return None
+    if isinstance(x, np.ndarray):
+        if x.dtype != np.float64 or not x.flags["C_CONTIGUOUS"]:
+            raise QrctmError("numpy arguments must be C-contiguous float64")
+        return x.ctypes.data_as(c_void_p)
+    import torch
+    if isinstance(x, torch.Tensor):
+        if x.dtype != torch.float64 or not x.is_contiguous():
+            raise QrctmError("torch arguments must be contiguous float64")
+        return c_void_p(x.data_ptr())
+    raise QrctmError(f"unsupported argument type {type(x)}")
+
+
+class QRCTM:
+    """Handle of one (d, D, chi) QR-CTMRG problem on the current CUDA device.
+
+    Device workspace is a torch uint8 tensor (PyTorch owns device memory); work is
+    enqueued on torch's current stream at construction time.
+    """
+
+    def __init__(self, d: int, D: int, chi: int):
+        import torch
+        if not torch.cuda.is_available():
+            raise QrctmError("no CUDA device: the QR-CTMRG path has no CPU fallback")
+        self.lib = load_library()
+        self.d, self.D, self.chi, self.b = d, D, chi, D * D
+        nbytes = self.lib.qrctm_workspace_bytes(d, D, chi)
+        if nbytes == 0:
+            raise QrctmError("invalid (d, D, chi)")
+        self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device="cuda")
+        base = (self._ws.data_ptr() + 255) // 256 * 256
+        h = c_void_p()
+        rc = self.lib.qrctm_create_in(d, D, chi, c_void_p(base), nbytes, byref(h))
+        if rc != QRCTM_OK:
+            raise QrctmError(f"qrctm_create_in failed: {rc}")
+        self._h = h
+        self._check(self.lib.qrctm_set_stream(h, c_void_p(torch.cuda.current_stream().cuda_stream)))
+
+    # -- plumbing
+    def _check(self, rc: int):
+        if rc != QRCTM_OK:
+            msg = self.lib.qrctm_last_error(self._h)
+            raise QrctmError(f"qrctm error {rc}: {msg.decode() if msg else ''}")
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self.lib.qrctm_destroy(self._h)
+            self._h = None
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _out(self, shape, like_device: bool):
+        if like_device:
+            import torch
+            return torch.empty(shape, dtype=torch.float64, device="cuda")
+        return np.empty(shape, dtype=np.float64)
+
+    # -- the C ABI, same names
+    def set_stream(self, cuda_stream: int):
+        self._check(self.lib.qrctm_set_stream(self._h, c_void_p(cuda_stream)))
+
+    def set_A(self, A):
+        assert tuple(A.shape) == (self.d,) + (self.D,) * 4
+        self._check(self.lib.qrctm_set_A(self._h, _ptr(A)))
+
+    def set_env(self, C, T):
+        assert tuple(C.shape) == (self.chi, self.chi) and tuple(T.shape) == (self.chi, self.b, self.chi)
+        self._check(self.lib.qrctm_set_env(self._h, _ptr(C), _ptr(T)))
+
+    def step(self):
+        self._check(self.lib.qrctm_step(self._h))
+
+    def run(self, max_iter: int, tol: float):
+        it, dl = c_int(0), c_double(0.0)
+        self._check(self.lib.qrctm_run(self._h, max_iter, tol, byref(it), byref(dl)))
+        return it.value, dl.value
+
+    def get_env(self, device: bool = False):
+        C = self._out((self.chi, self.chi), device)
+        T = self._out((self.chi, self.b, self.chi), device)
+        self._check(self.lib.qrctm_get_env(self._h, _ptr(C), _ptr(T)))
+        return C, T
+
+    def get_corner_spectrum(self):
+        s = np.empty(self.chi, dtype=np.float64)
+        self._check(self.lib.qrctm_get_corner_spectrum(self._h, _ptr(s)))
+        return s
+
+    def get_qr(self, device: bool = False):
+        Q = self._out((self.chi * self.b, self.chi), device)
+        R = self._out((self.chi, self.chi), device)
+        self._check(self.lib.qrctm_get_qr(self._h, _ptr(Q), _ptr(R)))
+        return Q, R
+
+    def get_raw(self, device: bool = False):
+        Cn = self._out((self.chi, self.chi), device)
+        Tn = self._out((self.chi, self.b, self.chi), device)
+        self._check(self.lib.qrctm_get_raw(self._h, _ptr(Cn), _ptr(Tn)))
+        return Cn, Tn
+
+    def get_a(self):
+        a = np.empty((self.b,) * 4, dtype=np.float64)
+        self._check(self.lib.qrctm_get_a(self._h, _ptr(a)))
+        return a
+
+    def norm_per_site(self) -> float:
+        k = c_double(0.0)
+        self._check(self.lib.qrctm_norm_per_site(self._h, byref(k)))
+        return k.value
+
+    def r_diag_ratio(self) -> float:
+        k = c_double(0.0)
+        self._check(self.lib.qrctm_r_diag_ratio(self._h, byref(k)))
+        return k.value
+
+    def set_option(self, key: int, value: int):
+        self._check(self.lib.qrctm_set_option(self._h, key, value))
+
+    def launch_count(self) -> int:
+        return int(self.lib.qrctm_launch_count(self._h))
+
+    def profile_step(self):
+        ms = (c_float * NSTAGE)()
+        self._check(self.lib.qrctm_profile_step(self._h, ms))
+        return dict(zip(STAGE_NAMES, [float(x) for x in ms]))
+
+
+# -- stand-alone entries (device tensors in, device tensors out)
+def gemm_f64(A, B, transA: bool = False, path: int = 0):
+    """out[M,N] = op(A) @ B on the GPU through qrctm_gemm_f64 (torch CUDA float64 tensors)."""
+    import torch
+    lib = load_library()
+    K, N = B.shape
+    M = A.shape[1] if transA else A.shape[0]
+    assert (A.shape[0] if transA else A.shape[1]) == K
+    for t in (A, B):       # row-strided views are fine: the ABI takes leading dimensions
+        if t.dtype != torch.float64 or not t.is_cuda or t.stride(1) != 1:
+            raise QrctmError("gemm_f64 wants CUDA float64 matrices with unit column stride")
+    out = torch.empty((M, N), dtype=torch.float64, device="cuda")
+    rc = lib.qrctm_gemm_f64(c_void_p(torch.cuda.current_stream().cuda_stream), path, int(transA), M, N, K,
+                            c_void_p(A.data_ptr()), A.stride(0), c_void_p(B.data_ptr()), B.stride(0),
+                            _ptr(out), N)
+    if rc != QRCTM_OK:
+        raise QrctmError(f"qrctm_gemm_f64 failed: {rc}")
+    return out
+
+
+def qr_f64(X):
+    """(Q, R) with diag(R) >= 0 of a torch CUDA float64 matrix through qrctm_qr_f64."""
+    import torch
+    lib = load_library()
+    rows, cols = X.shape
+    Q = torch.empty((rows, cols), dtype=torch.float64, device="cuda")
+    R = torch.empty((cols, cols), dtype=torch.float64, device="cuda")
+    work = torch.empty(lib.qrctm_qr_work_bytes(rows, cols), dtype=torch.uint8, device="cuda")
+    rc = lib.qrctm_qr_f64(c_void_p(torch.cuda.current_stream().cuda_stream), rows, cols, _ptr(X), _ptr(Q),
+                          _ptr(R), c_void_p(work.data_ptr()))
+    if rc != QRCTM_OK:
+        raise QrctmError(f"qrctm_qr_f64 failed: {rc}")
+    torch.cuda.current_stream().synchronize()
+    return Q, R
+
+
+def probe_fp64(kind: int, iters: int = 20000) -> float:
+    lib = load_library()
+    t = c_double(0.0)
+    rc = lib.qrctm_probe_fp64(kind, iters, byref(t))
+    if rc != QRCTM_OK:
+        raise QrctmError(f"qrctm_probe_fp64 failed: {rc}")
+    return t.value
+
+
+def version() -> str:
+    return load_library().qrctm_version().decode()

@@ -1,0 +1,230 @@
+// FP64 tensor-core GEMM for the QR-CTMRG contractions (K1, K2b, K2c, K3, K4, K5, K6).
+//
+//   out[ro(i) + co(j)] (op)= sum_k opA(i,k) * B[k*ldb + j]      i < M, j < N, k < K
+//
+// * B is always K x N row-major (N contiguous).
+// * opA: transA = 1 -> A stored K x M (M contiguous), the form every large
+//   contraction of the step takes once the producers write their outputs in the
+//   layout the consumer wants; transA = 0 -> A stored M x K.
+// * ro/co are two-level strided index maps, so the leg permutations between the
+//   contractions of (E3) are fused into the epilogue of the producing GEMM:
+//       ro(i) = (i / rdiv) * rs_hi + (i % rdiv) * rs_lo     (same for co)
+// * math: mma.sync.aligned.m8n8k4 f64 (SASS DMMA.8x8x4), the only FP64 tensor
+//   instruction sm_100a has (tcgen05 has no f64 kind).  Operands are staged into
+//   shared memory by a 4-stage cp.async (LDGSTS) ring, zero-filled at the ragged
+//   edges; rows are padded by 4 doubles so both fragment loads are conflict free.
+// * split-K: gridDim.z slices write plain partial tiles; reduce_splitk sums them
+//   in a fixed order (deterministic, no atomics).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace qk {
+
+struct IndexMap {          // idx -> (idx / div) * hi + (idx % div) * lo
+  int div;
+  long long hi, lo;
+};
+__host__ __device__ inline IndexMap plain_map(long long ld) { return IndexMap{1, ld, 0}; }
+
+struct GemmArgs {
+  const double* A; long long lda; int transA;
+  const double* B; long long ldb;
+  double* out;
+  IndexMap ro, co;
+  int M, N, K;
+  int ktiles_per_split;      // in units of BK tiles; gridDim.z splits
+  long long split_stride;    // elements between partial outputs (split-K only)
+  int mode;                  // 0: out = acc, 1: out = out - acc, 2: out = out + acc
+  int vecA, vecB;            // 16-byte cp.async legal for A / B
+};
+
+constexpr int BK = 16;
+constexpr int PAD = 4;
+
+__device__ __forceinline__ void cp_async16(void* smem, const void* g, int src_bytes) {
+  uint32_t s = (uint32_t)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(g), "r"(src_bytes));
+}
+__device__ __forceinline__ void cp_async8(void* smem, const void* g, int src_bytes) {
+  uint32_t s = (uint32_t)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(s), "l"(g), "r"(src_bytes));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+               : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+// Load a [BK][W] tile (row kk, W contiguous elements starting at column c0 of a
+// row-major matrix with leading dimension ld, logical width `width`) into smem
+// rows of W + PAD doubles.  Rows kk >= krows and columns >= width are zero filled.
+template <int W, int NT>
+__device__ __forceinline__ void load_tile_rows(double* s, const double* g, long long ld, int k0,
+                                               int krows, int c0, int width, bool vec, int tid) {
+  constexpr int LDS = W + PAD;
+  if (vec) {
+    constexpr int CH = W / 2;                       // 16-byte chunks per row
+    for (int c = tid; c < BK * CH; c += NT) {
+      int kk = c / CH, cc = (c % CH) * 2;
+      int rem = width - (c0 + cc);
+      int bytes = (kk < krows && rem > 0) ? (rem >= 2 ? 16 : 8) : 0;
+      const double* src = bytes ? g + (long long)(k0 + kk) * ld + c0 + cc : g;
+      cp_async16(s + kk * LDS + cc, src, bytes);
+    }
+  } else {
+    for (int c = tid; c < BK * W; c += NT) {
+      int kk = c / W, cc = c % W;
+      int bytes = (kk < krows && c0 + cc < width) ? 8 : 0;
+      const double* src = bytes ? g + (long long)(k0 + kk) * ld + c0 + cc : g;
+      cp_async8(s + kk * LDS + cc, src, bytes);
+    }
+  }
+}
+
+// transA = 0: A stored [M][K]; gather a [BK][W] tile transposed (8-byte copies).
+template <int W, int NT>
+__device__ __forceinline__ void load_tile_cols(double* s, const double* g, long long ld, int k0,
+                                               int krows, int r0, int height, int tid) {
+  constexpr int LDS = W + PAD;
+  for (int c = tid; c < BK * W; c += NT) {
+    int mm = c / BK, kk = c % BK;                    // kk fastest -> contiguous global reads
+    int bytes = (kk < krows && r0 + mm < height) ? 8 : 0;
+    const double* src = bytes ? g + (long long)(r0 + mm) * ld + k0 + kk : g;
+    cp_async8(s + kk * LDS + mm, src, bytes);
+  }
+}
+
+template <int BM, int BN, int WM, int WN, int STAGES>
+__global__ void __launch_bounds__((BM / WM) * (BN / WN) * 32, (BM >= 128 ? 1 : 2))
+gemm_f64_dmma(GemmArgs p) {
+  constexpr int NW_M = BM / WM, NW_N = BN / WN;
+  constexpr int NT = NW_M * NW_N * 32;
+  constexpr int LDA_S = BM + PAD, LDB_S = BN + PAD;
+  constexpr int A_STAGE = BK * LDA_S, B_STAGE = BK * LDB_S;
+  constexpr int FM = WM / 8, FN = WN / 8;
+  extern __shared__ __align__(16) double smem[];
+  double* As = smem;
+  double* Bs = smem + STAGES * A_STAGE;
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int wm0 = (warp / NW_N) * WM, wn0 = (warp % NW_N) * WN;
+  const int m0 = blockIdx.y * BM, n0 = blockIdx.x * BN;
+  const int lr = lane >> 2, lc = lane & 3;
+
+  const int nkt_total = (p.K + BK - 1) / BK;
+  const int kt_begin = blockIdx.z * p.ktiles_per_split;
+  int kt_end = kt_begin + p.ktiles_per_split;
+  if (kt_end > nkt_total) kt_end = nkt_total;
+  const int nkt = kt_end > kt_begin ? kt_end - kt_begin : 0;
+
+  double acc[FM][FN][2];
+#pragma unroll
+  for (int i = 0; i < FM; ++i)
+#pragma unroll
+    for (int j = 0; j < FN; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+  auto load_stage = [&](int kt, int stage) {
+    int k0 = (kt_begin + kt) * BK;
+    int krows = p.K - k0; if (krows > BK) krows = BK;
+    if (p.transA) load_tile_rows<BM, NT>(As + stage * A_STAGE, p.A, p.lda, k0, krows, m0, p.M, p.vecA, tid);
+    else          load_tile_cols<BM, NT>(As + stage * A_STAGE, p.A, p.lda, k0, krows, m0, p.M, tid);
+    load_tile_rows<BN, NT>(Bs + stage * B_STAGE, p.B, p.ldb, k0, krows, n0, p.N, p.vecB, tid);
+  };
+
+#pragma unroll
+  for (int s = 0; s < STAGES - 1; ++s) {
+    if (s < nkt) load_stage(s, s);
+    cp_async_commit();
+  }
+
+  for (int kt = 0; kt < nkt; ++kt) {
+    cp_async_wait<STAGES - 2>();
+    __syncthreads();
+    {
+      int nxt = kt + STAGES - 1;
+      if (nxt < nkt) load_stage(nxt, nxt % STAGES);
+      cp_async_commit();
+    }
+    const double* as = As + (kt % STAGES) * A_STAGE + wm0 + lr;
+    const double* bs = Bs + (kt % STAGES) * B_STAGE + wn0 + lr;
+    int k0 = (kt_begin + kt) * BK;
+    int ksteps = (p.K - k0 + 3) >> 2; if (ksteps > BK / 4) ksteps = BK / 4;
+#pragma unroll
+    for (int ks = 0; ks < BK / 4; ++ks) {
+      if (ks < ksteps) {
+        double af[FM], bf[FN];
+#pragma unroll
+        for (int i = 0; i < FM; ++i) af[i] = as[(ks * 4 + lc) * LDA_S + i * 8];
+#pragma unroll
+        for (int j = 0; j < FN; ++j) bf[j] = bs[(ks * 4 + lc) * LDB_S + j * 8];
+#pragma unroll
+        for (int i = 0; i < FM; ++i)
+#pragma unroll
+          for (int j = 0; j < FN; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+      }
+    }
+  }
+  cp_async_wait<0>();
+
+  // Epilogue: C fragment (row lr, cols 2*lc, 2*lc+1) straight to global through the index maps.
+  double* out = p.out + (long long)blockIdx.z * p.split_stride;
+#pragma unroll
+  for (int i = 0; i < FM; ++i) {
+    int r = m0 + wm0 + i * 8 + lr;
+    if (r >= p.M) continue;
+    long long roff = (long long)(r / p.ro.div) * p.ro.hi + (long long)(r % p.ro.div) * p.ro.lo;
+#pragma unroll
+    for (int j = 0; j < FN; ++j) {
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        int c = n0 + wn0 + j * 8 + 2 * lc + e;
+        if (c < p.N) {
+          long long off = roff + (long long)(c / p.co.div) * p.co.hi + (long long)(c % p.co.div) * p.co.lo;
+          double v = acc[i][j][e];
+          if (p.mode == 1) v = out[off] - v;
+          else if (p.mode == 2) v = out[off] + v;
+          out[off] = v;
+        }
+      }
+    }
+  }
+}
+
+// Plain DFMA reference kernel (QRCTM_OPT_GEMM_PATH = 1): one output element per
+// thread, no tiling.  Only for debugging / cross-checking the DMMA path on the GPU.
+__global__ void gemm_f64_ref(GemmArgs p) {
+  long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (long long)p.M * p.N) return;
+  int i = (int)(idx / p.N), j = (int)(idx % p.N);
+  double s = 0.0;
+  for (int k = 0; k < p.K; ++k) {
+    double a = p.transA ? p.A[(long long)k * p.lda + i] : p.A[(long long)i * p.lda + k];
+    s = fma(a, p.B[(long long)k * p.ldb + j], s);
+  }
+  long long off = (long long)(i / p.ro.div) * p.ro.hi + (long long)(i % p.ro.div) * p.ro.lo +
+                  (long long)(j / p.co.div) * p.co.hi + (long long)(j % p.co.div) * p.co.lo;
+  if (p.mode == 1) s = p.out[off] - s;
+  else if (p.mode == 2) s = p.out[off] + s;
+  p.out[off] = s;
+}
+
+// out[ro(i)+co(j)] (op)= sum_z part[z][i][j], z ascending (fixed order).
+__global__ void reduce_splitk(const double* part, long long split_stride, int splits, int M, int N,
+                              double* out, IndexMap ro, IndexMap co, int mode) {
+  long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (long long)M * N) return;
+  int i = (int)(idx / N), j = (int)(idx % N);
+  double s = 0.0;
+  for (int z = 0; z < splits; ++z) s += part[(long long)z * split_stride + idx];
+  long long off = (long long)(i / ro.div) * ro.hi + (long long)(i % ro.div) * ro.lo +
+                  (long long)(j / co.div) * co.hi + (long long)(j % co.div) * co.lo;
+  if (mode == 1) s = out[off] - s;
+  else if (mode == 2) s = out[off] + s;
+  out[off] = s;
+}
+
+}  // namespace qk

@@ -1,0 +1,723 @@
+// libqrctm.so -- C ABI (include/qrctm.h) and the iteration driver (K9).
+// Links only cudart.  No cuBLAS / cuSOLVER / libtorch.
+#include "../../include/qrctm.h"
+
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "gemm_f64.cuh"
+#include "kernels_misc.cuh"
+#include "qr_f64.cuh"
+#include "spectrum.cuh"
+
+using namespace qk;
+
+namespace {
+
+constexpr int kPartialBlocks = 592;   // 4 x 148 blocks for the reduction kernels
+constexpr size_t kAlign = 256;
+
+inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
+
+struct Layout {   // byte offsets into the workspace
+  size_t A, a_mat, C, T, Cn, Tn, X, V, Q, R, tau, P, S, W, E, splitk, partial, scal, flag, Wc, dvec, evec,
+      vv, pv, eig, s, s_prev, s_tmp, delta, qrwork, total;
+  long long lda_a;
+  size_t splitk_elems, qrwork_bytes;
+};
+
+}  // namespace
+
+struct qrctm {
+  int d, D, b, chi;
+  long long m;            // chi * b
+  cudaStream_t stream;
+  char* base;             // workspace
+  bool owns_ws;
+  Layout L;
+  bool have_A, have_env;
+  int corner_mode, symmetrize, check_every, gemm_path;
+  long long launches;
+  char err[256];
+  double* h_pinned;       // [0] delta, [1..] scratch ; pinned host
+  int* h_flag;
+  // typed views
+  double *A, *a_mat, *C, *T, *Cn, *Tn, *X, *V, *Q, *R, *tau, *P, *S, *W, *E, *splitk, *partial, *scal, *Wc,
+      *dvec, *evec, *vv, *pv, *eig, *s, *s_prev, *s_tmp, *delta;
+  int* flag;
+  void* qrwork;
+};
+
+namespace {
+
+unsigned long long qr_work_bytes_impl(long long rows, int cols);
+
+bool make_layout(int d, int D, int chi, Layout* L) {
+  if (d < 1 || D < 1 || chi < 1) return false;
+  if (D > 32 || chi > 1024 || d > 64) return false;                  // sizes this build supports
+  long long b = (long long)D * D, m = b * chi;
+  long long b2 = b * b;
+  L->lda_a = (b2 + 15) / 16 * 16;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
+  const size_t dbl = sizeof(double);
+  L->A = take(dbl * d * b2);
+  L->a_mat = take(dbl * b2 * L->lda_a);
+  L->C = take(dbl * chi * chi);
+  L->T = take(dbl * m * chi);
+  L->Cn = take(dbl * chi * chi);
+  L->Tn = take(dbl * m * chi);
+  L->X = take(dbl * m * chi);
+  L->V = take(dbl * m * chi);
+  L->Q = take(dbl * m * chi);
+  L->R = take(dbl * chi * chi);
+  L->tau = take(dbl * chi);
+  L->P = take(dbl * m * m);
+  L->S = take(dbl * m * m);
+  L->W = take(dbl * m * chi);
+  L->E = take(dbl * m * chi);
+  L->splitk_elems = (size_t)256 * chi * chi + (size_t)4 * m * chi;
+  L->splitk = take(dbl * L->splitk_elems);
+  L->partial = take(dbl * 4 * kPartialBlocks);
+  L->scal = take(dbl * 16);
+  L->flag = take(sizeof(int) * 4);
+  L->Wc = take(dbl * chi * chi);
+  L->dvec = take(dbl * chi);
+  L->evec = take(dbl * chi);
+  L->vv = take(dbl * chi);
+  L->pv = take(dbl * chi);
+  L->eig = take(dbl * chi);
+  L->s = take(dbl * chi);
+  L->s_prev = take(dbl * chi);
+  L->s_tmp = take(dbl * chi);
+  L->delta = take(dbl * 4);
+  L->qrwork_bytes = qr_work_bytes_impl(m, chi);
+  L->qrwork = take(L->qrwork_bytes);
+  L->total = off;
+  return true;
+}
+
+void bind_views(qrctm* h) {
+  char* B = h->base;
+  const Layout& L = h->L;
+#define V_(name) h->name = reinterpret_cast<double*>(B + L.name)
+  V_(A); V_(a_mat); V_(C); V_(T); V_(Cn); V_(Tn); V_(X); V_(V); V_(Q); V_(R); V_(tau); V_(P); V_(S); V_(W);
+  V_(E); V_(splitk); V_(partial); V_(scal); V_(Wc); V_(dvec); V_(evec); V_(vv); V_(pv); V_(eig); V_(s);
+  V_(s_prev); V_(s_tmp); V_(delta);
+#undef V_
+  h->flag = reinterpret_cast<int*>(B + L.flag);
+  h->qrwork = B + L.qrwork;
+}
+
+int fail(qrctm* h, int code, const char* what, cudaError_t e = cudaSuccess) {
+  if (h) {
+    if (e != cudaSuccess) snprintf(h->err, sizeof(h->err), "%s: %s", what, cudaGetErrorString(e));
+    else snprintf(h->err, sizeof(h->err), "%s", what);
+  }
+  return code;
+}
+
+#define CU(h, call)                                                        \
+  do {                                                                     \
+    cudaError_t e__ = (call);                                              \
+    if (e__ != cudaSuccess) return fail((h), QRCTM_ERR_CUDA, #call, e__);  \
+  } while (0)
+
+bool is_device_ptr(const void* p) {
+  cudaPointerAttributes at;
+  cudaError_t e = cudaPointerGetAttributes(&at, p);
+  if (e != cudaSuccess) { cudaGetLastError(); return false; }
+  return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+cudaError_t copy_in(double* dst_dev, const double* src, size_t n, cudaStream_t st) {
+  cudaMemcpyKind k = is_device_ptr(src) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  cudaError_t e = cudaMemcpyAsync(dst_dev, src, n * sizeof(double), k, st);
+  if (e != cudaSuccess) return e;
+  return k == cudaMemcpyHostToDevice ? cudaStreamSynchronize(st) : cudaSuccess;
+}
+cudaError_t copy_out(double* dst, const double* src_dev, size_t n, cudaStream_t st) {
+  cudaMemcpyKind k = is_device_ptr(dst) ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+  cudaError_t e = cudaMemcpyAsync(dst, src_dev, n * sizeof(double), k, st);
+  if (e != cudaSuccess) return e;
+  return cudaStreamSynchronize(st);
+}
+
+// ------------------------------------------------------------------ GEMM launcher
+template <int BM, int BN, int WM, int WN, int STAGES>
+cudaError_t launch_cfg(cudaStream_t st, const GemmArgs& g, int splits) {
+  constexpr int NT = (BM / WM) * (BN / WN) * 32;
+  constexpr size_t smem = sizeof(double) * STAGES * BK * ((BM + PAD) + (BN + PAD));
+  static bool attr_done = false;
+  if (!attr_done) {
+    cudaError_t e = cudaFuncSetAttribute(gemm_f64_dmma<BM, BN, WM, WN, STAGES>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    attr_done = true;
+  }
+  dim3 grid((g.N + BN - 1) / BN, (g.M + BM - 1) / BM, splits);
+  gemm_f64_dmma<BM, BN, WM, WN, STAGES><<<grid, NT, smem, st>>>(g);
+  return cudaGetLastError();
+}
+
+struct GemmCall {
+  const double* A; long long lda; int transA;
+  const double* B; long long ldb;
+  double* out; IndexMap ro, co;
+  int M, N, K;
+  int mode;   // 0 store, 1 out -= , 2 out +=
+};
+
+// Returns number of kernels launched (>0) or -1 on error (err set).
+int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws, size_t splitk_elems,
+                cudaError_t* err) {
+  *err = cudaSuccess;
+  if (c.M <= 0 || c.N <= 0) return 0;
+  GemmArgs g;
+  g.A = c.A; g.lda = c.lda; g.transA = c.transA; g.B = c.B; g.ldb = c.ldb; g.out = c.out;
+  g.ro = c.ro; g.co = c.co; g.M = c.M; g.N = c.N; g.K = c.K; g.mode = c.mode;
+  g.vecA = c.transA && (c.lda % 2 == 0) && ((reinterpret_cast<uintptr_t>(c.A) & 15) == 0);
+  g.vecB = (c.ldb % 2 == 0) && ((reinterpret_cast<uintptr_t>(c.B) & 15) == 0);
+  g.split_stride = 0;
+  const int nkt = (c.K + BK - 1) / BK;
+  g.ktiles_per_split = nkt > 0 ? nkt : 1;
+  if (path == 1) {
+    long long n = (long long)c.M * c.N;
+    gemm_f64_ref<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(g);
+    *err = cudaGetLastError();
+    return *err == cudaSuccess ? 1 : -1;
+  }
+  const long long t128 = (long long)((c.M + 127) / 128) * ((c.N + 127) / 128);
+  const long long t64 = (long long)((c.M + 63) / 64) * ((c.N + 63) / 64);
+  const bool big = t128 >= 120;
+  int splits = 1;
+  if (!big && t64 < 148 && nkt >= 8) {
+    splits = (int)((2 * 148 + t64 - 1) / t64);
+    if (splits > nkt / 2) splits = nkt / 2;
+    size_t per = (size_t)c.M * c.N;
+    if (per * splits > splitk_elems) splits = (int)(splitk_elems / per);
+    if (splits < 1) splits = 1;
+  }
+  int launched = 0;
+  if (splits > 1) {
+    g.ktiles_per_split = (nkt + splits - 1) / splits;
+    splits = (nkt + g.ktiles_per_split - 1) / g.ktiles_per_split;
+    g.out = splitk_ws; g.ro = plain_map(c.N); g.co = IndexMap{1, 1, 0}; g.mode = 0;
+    g.split_stride = (long long)c.M * c.N;
+  }
+  if (big) *err = launch_cfg<128, 128, 64, 32, 4>(st, g, splits);
+  else     *err = launch_cfg<64, 64, 32, 32, 4>(st, g, splits);
+  if (*err != cudaSuccess) return -1;
+  ++launched;
+  if (splits > 1) {
+    long long n = (long long)c.M * c.N;
+    reduce_splitk<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(splitk_ws, g.split_stride, splits, c.M, c.N,
+                                                              c.out, c.ro, c.co, c.mode);
+    *err = cudaGetLastError();
+    if (*err != cudaSuccess) return -1;
+    ++launched;
+  }
+  return launched;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------ K2: QR driver
+namespace {
+
+unsigned long long qr_work_bytes_impl(long long rows, int cols) {
+  if (rows < 1 || cols < 1) return 0;
+  size_t v = align_up(sizeof(double) * (size_t)rows * cols);        // V: working copy / reflectors
+  size_t t = align_up(sizeof(double) * (size_t)cols);               // tau
+  size_t extra = align_up(sizeof(double) * ((size_t)cols * cols * 4 + 1024));
+  return v + t + extra;
+}
+
+// X (rows x n, ld n, DEVICE, untouched) -> Q (rows x n), R (n x n), diag(R) >= 0.
+// Level-2 Householder (one reflector at a time).  Returns kernels launched or -1.
+long long qr_factor_level2(cudaStream_t st, long long rows, int n, const double* X, double* Q, double* R,
+                           void* work, cudaError_t* err) {
+  char* wb = static_cast<char*>(work);
+  double* V = reinterpret_cast<double*>(wb);
+  double* tau = reinterpret_cast<double*>(wb + align_up(sizeof(double) * (size_t)rows * n));
+  long long launches = 0;
+  *err = cudaMemcpyAsync(V, X, sizeof(double) * rows * n, cudaMemcpyDeviceToDevice, st);
+  if (*err != cudaSuccess) return -1;
+  constexpr int CPB = 4;
+  for (int k = 0; k < n; ++k) {
+    house_col_kernel<<<1, 1024, 0, st>>>(V, n, rows, k, tau);
+    ++launches;
+    if (k + 1 < n) {
+      int nb = (n - (k + 1) + CPB - 1) / CPB;
+      house_apply_kernel<CPB><<<nb, 512, 0, st>>>(V, n, rows, k, tau, V, n, k + 1, n);
+      ++launches;
+    }
+  }
+  copy_triu_kernel<<<(n * n + 255) / 256, 256, 0, st>>>(V, n, n, R);
+  set_identity_top_kernel<<<296, 256, 0, st>>>(Q, rows, n);
+  launches += 2;
+  for (int k = n - 1; k >= 0; --k) {
+    int nb = (n - k + CPB - 1) / CPB;
+    house_apply_kernel<CPB><<<nb, 512, 0, st>>>(V, n, rows, k, tau, Q, n, k, n);
+    ++launches;
+  }
+  sign_fix_kernel<<<296, 256, 0, st>>>(Q, rows, n, R);
+  sign_fix_R_kernel<<<n, 128, 0, st>>>(R, n);
+  launches += 2;
+  *err = cudaGetLastError();
+  return *err == cudaSuccess ? launches : -1;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------ step stages
+namespace {
+
+#define GEMM(h, call_)                                                                          \
+  do {                                                                                          \
+    cudaError_t ge__;                                                                           \
+    int nl__ = launch_gemm((h)->stream, (h)->gemm_path, (call_), (h)->splitk, (h)->L.splitk_elems, &ge__); \
+    if (nl__ < 0) return fail((h), QRCTM_ERR_CUDA, "gemm launch", ge__);                        \
+    (h)->launches += nl__;                                                                      \
+  } while (0)
+
+// K1 (E1): X[(j,u),k] = sum_i C[j,i] T[i,u,k]       -> out (chi x b*chi == chi*b x chi)
+int stage_reduced_corner(qrctm* h, const double* C, const double* T, double* X) {
+  const int chi = h->chi; const long long bc = (long long)h->b * chi;
+  GemmCall c{C, chi, 0, T, bc, X, plain_map(bc), IndexMap{1, 1, 0}, chi, (int)bc, chi, 0};
+  GEMM(h, c);
+  return QRCTM_OK;
+}
+
+// K3: P'[u,l,m,J] = sum_j Qm[j,u,m] T[j,l,J]        (Qm: chi*b x n viewed chi x b*n)
+int stage_half_absorb(qrctm* h, const double* Qm, const double* T, double* P) {
+  const int chi = h->chi, b = h->b; const long long bc = (long long)b * chi, cc = (long long)chi * chi;
+  GemmCall c{Qm, bc, 1, T, bc, P, IndexMap{chi, b * cc, chi}, IndexMap{chi, cc, 1}, (int)bc, (int)bc, chi, 0};
+  GEMM(h, c);
+  return QRCTM_OK;
+}
+
+// K4: S[m,J,d,r] = sum_{u,l} P'[(u,l),(m,J)] a[(u,l),(d,r)]
+//   layout 0: S''[J,d,m,r]  (what K5 wants: K x M with K = (J,d))
+//   layout 1: S~ [m,r,J,d]  (what the kappa network wants: K = (m,r))
+//   layout 2: C~[(J,d),(m,r)] natural enlarged-corner matrix == layout 0
+int stage_absorb_a(qrctm* h, const double* P, double* S, int layout) {
+  const int chi = h->chi, b = h->b; const long long m = h->m, cc = (long long)chi * chi;
+  IndexMap ro, co;
+  if (layout == 0) { ro = IndexMap{chi, b, (long long)b * m}; co = IndexMap{b, m, 1}; }
+  else             { ro = IndexMap{chi, (long long)b * m, b}; co = IndexMap{b, 1, (long long)chi * b}; }
+  GemmCall c{P, cc, 1, h->a_mat, h->L.lda_a, S, ro, co, (int)cc, b * b, b * b, 0};
+  GEMM(h, c);
+  return QRCTM_OK;
+}
+
+// K5: out[(m,r),n] = sum_{(J,d)} S''[(J,d),(m,r)] Qm[(J,d),n]
+int stage_project(qrctm* h, const double* S, const double* Qm, double* out) {
+  const int chi = h->chi; const long long m = h->m;
+  GemmCall c{S, m, 1, Qm, chi, out, plain_map(chi), IndexMap{1, 1, 0}, (int)m, chi, (int)m, 0};
+  GEMM(h, c);
+  return QRCTM_OK;
+}
+
+// K6 (E4): W[m,(r,n)] = sum_k R[m,k] Q[k,(r,n)] ;  C'[p,n] = sum_{(m,r)} T'[(m,r),p] W[(m,r),n]
+int stage_corner_accel(qrctm* h) {
+  const int chi = h->chi; const long long bc = (long long)h->b * chi, m = h->m;
+  GemmCall c1{h->R, chi, 0, h->Q, bc, h->W, plain_map(bc), IndexMap{1, 1, 0}, chi, (int)bc, chi, 0};
+  GEMM(h, c1);
+  GemmCall c2{h->Tn, chi, 1, h->W, chi, h->Cn, plain_map(chi), IndexMap{1, 1, 0}, chi, chi, (int)m, 0};
+  GEMM(h, c2);
+  return QRCTM_OK;
+}
+
+// K6' (E5)+(E4'): Z = half_absorb(X), C~ = Z.a, Y = C~ Q, C' = Q^T Y
+int stage_corner_enlarged(qrctm* h) {
+  const int chi = h->chi; const long long m = h->m;
+  int rc = stage_half_absorb(h, h->X, h->T, h->P); if (rc) return rc;
+  rc = stage_absorb_a(h, h->P, h->S, 0); if (rc) return rc;          // S = C~[(J,d),(k,r)]
+  GemmCall c1{h->S, m, 0, h->Q, chi, h->W, plain_map(chi), IndexMap{1, 1, 0}, (int)m, chi, (int)m, 0};
+  GEMM(h, c1);
+  GemmCall c2{h->Q, chi, 1, h->W, chi, h->Cn, plain_map(chi), IndexMap{1, 1, 0}, chi, chi, (int)m, 0};
+  GEMM(h, c2);
+  return QRCTM_OK;
+}
+
+// K7: C,T <- sym(Cn,Tn) / ||.||_F
+int stage_normalize(qrctm* h, const double* Cn, const double* Tn) {
+  const int chi = h->chi, b = h->b;
+  long long nT = (long long)chi * b * chi;
+  int nbC = (int)(((long long)chi * chi + 255) / 256); if (nbC > 148) nbC = 148;
+  int nbT = (int)((nT + 255) / 256); if (nbT > kPartialBlocks) nbT = kPartialBlocks;
+  sym_partial_kernel<<<nbC + nbT, 256, 0, h->stream>>>(Cn, Tn, chi, b, h->symmetrize, h->C, h->T, h->partial,
+                                                      nbC, nbT);
+  int nb = (int)((nT + (long long)chi * chi + 255) / 256); if (nb > 592) nb = 592;
+  scale_kernel<<<nb, 256, 0, h->stream>>>(h->C, h->T, chi, b, h->partial, nbC, nbT, h->scal, h->flag);
+  h->launches += 2;
+  CU(h, cudaGetLastError());
+  return QRCTM_OK;
+}
+
+// K8: spectrum of h->C into s_out (+ delta against s_prev, optional update)
+int stage_spectrum(qrctm* h, double* s_out, int update_prev) {
+  const int chi = h->chi;
+  CU(h, cudaMemcpyAsync(h->Wc, h->C, sizeof(double) * chi * chi, cudaMemcpyDeviceToDevice, h->stream));
+  tridiag_kernel<<<1, 1024, 0, h->stream>>>(h->Wc, chi, h->dvec, h->evec, h->vv, h->pv);
+  int nt = (chi + 31) / 32 * 32; if (nt < 64) nt = 64;
+  bisect_sort_kernel<<<1, nt, sizeof(double) * (3 * chi + 40), h->stream>>>(h->dvec, h->evec, chi, h->eig, s_out,
+                                                                          h->s_prev, h->delta, update_prev);
+  h->launches += 2;
+  CU(h, cudaGetLastError());
+  return QRCTM_OK;
+}
+
+int do_step(qrctm* h, cudaEvent_t* ev /* QRCTM_NSTAGE+1 events or null */) {
+  auto mark = [&](int i) { if (ev) cudaEventRecord(ev[i], h->stream); };
+  int rc;
+  mark(0);
+  rc = stage_reduced_corner(h, h->C, h->T, h->X); if (rc) return rc;
+  mark(1);
+  {
+    cudaError_t e;
+    long long nl = qr_factor_level2(h->stream, h->m, h->chi, h->X, h->Q, h->R, h->qrwork, &e);
+    if (nl < 0) return fail(h, QRCTM_ERR_CUDA, "qr", e);
+    h->launches += nl;
+  }
+  mark(2);
+  rc = stage_half_absorb(h, h->Q, h->T, h->P); if (rc) return rc;
+  mark(3);
+  rc = stage_absorb_a(h, h->P, h->S, 0); if (rc) return rc;
+  mark(4);
+  rc = stage_project(h, h->S, h->Q, h->Tn); if (rc) return rc;
+  mark(5);
+  rc = h->corner_mode == 0 ? stage_corner_accel(h) : stage_corner_enlarged(h); if (rc) return rc;
+  mark(6);
+  rc = stage_normalize(h, h->Cn, h->Tn); if (rc) return rc;
+  mark(7);
+  return QRCTM_OK;
+}
+
+int check_flag(qrctm* h) {   // stream must be synchronised by the caller's copy
+  CU(h, cudaMemcpyAsync(h->h_flag, h->flag, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+  CU(h, cudaStreamSynchronize(h->stream));
+  if (*h->h_flag) return fail(h, QRCTM_ERR_NUMERIC, "NaN/Inf or zero Frobenius norm in C' or T'");
+  return QRCTM_OK;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------ C ABI
+extern "C" {
+
+const char* qrctm_version(void) { return "qrctm-b200 0.1 (sm_100a, FP64 DMMA)"; }
+
+unsigned long long qrctm_workspace_bytes(int d, int D, int chi) {
+  Layout L;
+  if (!make_layout(d, D, chi, &L)) return 0;
+  return L.total;
+}
+
+static int create_common(int d, int D, int chi, void* ws, unsigned long long ws_bytes, qrctm_t** out) {
+  if (!out) return QRCTM_ERR_INVALID_ARG;
+  *out = nullptr;
+  Layout L;
+  if (!make_layout(d, D, chi, &L)) return QRCTM_ERR_INVALID_ARG;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return QRCTM_ERR_CUDA; }
+  qrctm* h = new (std::nothrow) qrctm();
+  if (!h) return QRCTM_ERR_CUDA;
+  memset(h, 0, sizeof(*h));
+  h->d = d; h->D = D; h->b = D * D; h->chi = chi; h->m = (long long)chi * D * D;
+  h->L = L; h->stream = 0;
+  h->corner_mode = 0; h->symmetrize = 1; h->check_every = 1; h->gemm_path = 0;
+  if (ws) {
+    if (ws_bytes < L.total || (reinterpret_cast<uintptr_t>(ws) & (kAlign - 1)) || !is_device_ptr(ws)) {
+      delete h; return QRCTM_ERR_INVALID_ARG;
+    }
+    h->base = static_cast<char*>(ws); h->owns_ws = false;
+  } else {
+    void* p = nullptr;
+    if (cudaMalloc(&p, L.total) != cudaSuccess) { cudaGetLastError(); delete h; return QRCTM_ERR_CUDA; }
+    h->base = static_cast<char*>(p); h->owns_ws = true;
+  }
+  bind_views(h);
+  void* hp = nullptr;
+  if (cudaMallocHost(&hp, 64 * sizeof(double)) != cudaSuccess) {
+    cudaGetLastError(); if (h->owns_ws) cudaFree(h->base); delete h; return QRCTM_ERR_CUDA;
+  }
+  h->h_pinned = static_cast<double*>(hp);
+  h->h_flag = reinterpret_cast<int*>(h->h_pinned + 32);
+  cudaMemsetAsync(h->flag, 0, 4 * sizeof(int), 0);
+  cudaMemsetAsync(h->s_prev, 0, sizeof(double) * chi, 0);
+  cudaMemsetAsync(h->R, 0, sizeof(double) * chi * chi, 0);
+  cudaMemsetAsync(h->Q, 0, sizeof(double) * h->m * chi, 0);
+  if (cudaStreamSynchronize(0) != cudaSuccess) { cudaGetLastError(); qrctm_destroy(h); return QRCTM_ERR_CUDA; }
+  *out = h;
+  return QRCTM_OK;
+}
+
+int qrctm_create(int d, int D, int chi, qrctm_t** out) { return create_common(d, D, chi, nullptr, 0, out); }
+
+int qrctm_create_in(int d, int D, int chi, void* workspace, unsigned long long workspace_bytes, qrctm_t** out) {
+  if (!workspace) return QRCTM_ERR_INVALID_ARG;
+  return create_common(d, D, chi, workspace, workspace_bytes, out);
+}
+
+int qrctm_destroy(qrctm_t* h) {
+  if (!h) return QRCTM_ERR_INVALID_ARG;
+  cudaStreamSynchronize(h->stream);
+  if (h->owns_ws && h->base) cudaFree(h->base);
+  if (h->h_pinned) cudaFreeHost(h->h_pinned);
+  cudaGetLastError();
+  delete h;
+  return QRCTM_OK;
+}
+
+int qrctm_set_stream(qrctm_t* h, void* cuda_stream) {
+  if (!h) return QRCTM_ERR_INVALID_ARG;
+  CU(h, cudaStreamSynchronize(h->stream));
+  h->stream = static_cast<cudaStream_t>(cuda_stream);
+  return QRCTM_OK;
+}
+
+int qrctm_set_A(qrctm_t* h, const double* A) {
+  if (!h || !A) return h ? fail(h, QRCTM_ERR_INVALID_ARG, "null A") : QRCTM_ERR_INVALID_ARG;
+  long long b2 = (long long)h->b * h->b;
+  CU(h, copy_in(h->A, A, (size_t)h->d * b2, h->stream));
+  CU(h, cudaMemsetAsync(h->a_mat, 0, sizeof(double) * b2 * h->L.lda_a, h->stream));
+  long long n = b2 * b2;
+  int nb = (int)((n + 255) / 256); if (nb > 148 * 8) nb = 148 * 8;
+  build_a_kernel<<<nb, 256, 0, h->stream>>>(h->A, h->d, h->D, h->a_mat, h->L.lda_a);
+  h->launches += 1;
+  CU(h, cudaGetLastError());
+  h->have_A = true;
+  return QRCTM_OK;
+}
+
+int qrctm_set_env(qrctm_t* h, const double* C, const double* T) {
+  if (!h || !C || !T) return h ? fail(h, QRCTM_ERR_INVALID_ARG, "null C/T") : QRCTM_ERR_INVALID_ARG;
+  CU(h, copy_in(h->Cn, C, (size_t)h->chi * h->chi, h->stream));
+  CU(h, copy_in(h->Tn, T, (size_t)h->m * h->chi, h->stream));
+  CU(h, cudaMemsetAsync(h->flag, 0, sizeof(int), h->stream));
+  int rc = stage_normalize(h, h->Cn, h->Tn); if (rc) return rc;
+  rc = check_flag(h); if (rc) return rc;
+  CU(h, cudaMemsetAsync(h->s_prev, 0, sizeof(double) * h->chi, h->stream));
+  rc = stage_spectrum(h, h->s, 1); if (rc) return rc;
+  h->have_env = true;
+  return QRCTM_OK;
+}
+
+int qrctm_step(qrctm_t* h) {
+  if (!h) return QRCTM_ERR_INVALID_ARG;
+  if (!h->have_A || !h->have_env) return fail(h, QRCTM_ERR_NOT_READY, "set_A and set_env first");
+  return do_step(h, nullptr);
+}
+
+int qrctm_run(qrctm_t* h, int max_iter, double tol, int* iters_done, double* final_delta) {
+  if (!h) return QRCTM_ERR_INVALID_ARG;
+  if (!h->have_A || !h->have_env) return fail(h, QRCTM_ERR_NOT_READY, "set_A and set_env first");
+  if (max_iter < 0) return fail(h, QRCTM_ERR_INVALID_ARG, "max_iter < 0");
+  double delta = INFINITY;
+  int it = 0;
+  for (it = 1; it <= max_iter; ++it) {
+    int rc = do_step(h, nullptr); if (rc) return rc;
+    if (it % h->check_every == 0 || it == max_iter) {
+      rc = stage_spectrum(h, h->s, 1); if (rc) return rc;
+      CU(h, cudaMemcpyAsync(h->h_pinned, h->delta, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+      rc = check_flag(h); if (rc) return rc;       // synchronises
+      delta = h->h_pinned[0];
+      if (delta < tol) break;
+    }
+  }
+  if (it > max_iter) it = max_iter;
+  CU(h, cudaStreamSynchronize(h->stream));
+  if (iters_done) *iters_done = it;
+  if (final_delta) *final_delta = delta;
+  return QRCTM_OK;
+}
+
+int qrctm_get_env(qrctm_t* h, double* C, double* T) {
+  if (!h) return QRCTM_ERR_INVALID_ARG;
+  if (!h->have_env) return fail(h, QRCTM_ERR_NOT_READY, "no environment");
+  int rc = check_flag(h); if (rc) return rc;
+  if (C) CU(h, copy_out(C, h->C, (size_t)h->chi * h->chi, h->stream));
+  if (T) CU(h, copy_out(T, h->T, (size_t)h->m * h->chi, h->stream));
+  return QRCTM_OK;
+}
+
+int qrctm_get_corner_spectrum(qrctm_t* h, double* s) {
+  if (!h || !s) return h ? fail(h, QRCTM_ERR_INVALID_ARG, "null s") : QRCTM_ERR_INVALID_ARG;
+  if (!h->have_env) return fail(h, QRCTM_ERR_NOT_READY, "no environment");
+  int rc = stage_spectrum(h, h->s_tmp, 0); if (rc) return rc;
+  CU(h, copy_out(s, h->s_tmp, h->chi, h->stream));
+  return QRCTM_OK;
+}
+
+int qrctm_get_qr(qrctm_t* h, double* Q, double* R) {
+  if (!h) return QRCTM_ERR_INVALID_ARG;
+  if (Q) CU(h, copy_out(Q, h->Q, (size_t)h->m * h->chi, h->stream));
+  if (R) CU(h, copy_out(R, h->R, (size_t)h->chi * h->chi, h->stream));
+  return QRCTM_OK;
+}
+
+int qrctm_get_raw(qrctm_t* h, double* Cn, double* Tn) {
+  if (!h) return QRCTM_ERR_INVALID_ARG;
+  if (Cn) CU(h, copy_out(Cn, h->Cn, (size_t)h->chi * h->chi, h->stream));
+  if (Tn) CU(h, copy_out(Tn, h->Tn, (size_t)h->m * h->chi, h->stream));
+  return QRCTM_OK;
+}
+
+int qrctm_get_a(qrctm_t* h, double* a) {
+  if (!h || !a) return QRCTM_ERR_INVALID_ARG;
+  if (!h->have_A) return fail(h, QRCTM_ERR_NOT_READY, "no A");
+  long long b2 = (long long)h->b * h->b;
+  cudaMemcpyKind k = is_device_ptr(a) ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+  CU(h, cudaMemcpy2DAsync(a, sizeof(double) * b2, h->a_mat, sizeof(double) * h->L.lda_a, sizeof(double) * b2, b2,
+                          k, h->stream));
+  CU(h, cudaStreamSynchronize(h->stream));
+  return QRCTM_OK;
+}
+
+int qrctm_set_option(qrctm_t* h, int key, int value) {
+  if (!h) return QRCTM_ERR_INVALID_ARG;
+  switch (key) {
+    case QRCTM_OPT_CORNER_MODE: if (value != 0 && value != 1) break; h->corner_mode = value; return QRCTM_OK;
+    case QRCTM_OPT_SYMMETRIZE:  if (value != 0 && value != 1) break; h->symmetrize = value; return QRCTM_OK;
+    case QRCTM_OPT_CHECK_EVERY: if (value < 1) break; h->check_every = value; return QRCTM_OK;
+    case QRCTM_OPT_GEMM_PATH:   if (value != 0 && value != 1) break; h->gemm_path = value; return QRCTM_OK;
+    default: break;
+  }
+  return fail(h, QRCTM_ERR_INVALID_ARG, "bad option key/value");
+}
+
+long long qrctm_launch_count(const qrctm_t* h) { return h ? h->launches : 0; }
+
+const char* qrctm_last_error(const qrctm_t* h) { return h ? h->err : "null handle"; }
+
+}  // extern "C"
+
+// ------------------------------------------------------------------ observables, diagnostics, stand-alone entries
+#include "probe.cuh"
+
+namespace {
+
+__global__ void r_diag_minmax_kernel(const double* __restrict__ R, int n, double* __restrict__ out) {
+  __shared__ double sh[33];
+  double mn = INFINITY, mx = -INFINITY;
+  for (int k = threadIdx.x; k < n; k += blockDim.x) {
+    double v = R[(long long)k * n + k];
+    mn = fmin(mn, v); mx = fmax(mx, v);
+  }
+  double gmx = block_max(mx, sh);
+  double gmn = -block_max(-mn, sh);
+  if (threadIdx.x == 0) { out[0] = gmn; out[1] = gmx; }
+}
+
+int reduce_dot(qrctm* h, const double* x, const double* y, long long n, double* out) {
+  dot_partial_kernel<<<kPartialBlocks, 256, 0, h->stream>>>(x, y, n, h->partial + 2 * kPartialBlocks);
+  sum_partial_kernel<<<1, 256, 0, h->stream>>>(h->partial + 2 * kPartialBlocks, kPartialBlocks, out);
+  h->launches += 2;
+  CU(h, cudaGetLastError());
+  return QRCTM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int qrctm_norm_per_site(qrctm_t* h, double* kappa) {
+  if (!h || !kappa) return h ? fail(h, QRCTM_ERR_INVALID_ARG, "null kappa") : QRCTM_ERR_INVALID_ARG;
+  if (!h->have_A || !h->have_env) return fail(h, QRCTM_ERR_NOT_READY, "set_A and set_env first");
+  const int chi = h->chi; const long long m = h->m;
+  int rc;
+  // E[a,s,c] = sum C[a,i] T[i,s,k] C[k,c]
+  rc = stage_reduced_corner(h, h->C, h->T, h->W); if (rc) return rc;
+  { GemmCall c{h->W, chi, 0, h->C, chi, h->E, plain_map(chi), IndexMap{1, 1, 0}, (int)m, chi, chi, 0}; GEMM(h, c); }
+  // Z4 = tr C^4 = tr (C2 C2)
+  { GemmCall c{h->C, chi, 0, h->C, chi, h->Wc, plain_map(chi), IndexMap{1, 1, 0}, chi, chi, chi, 0}; GEMM(h, c); }
+  trace_prod_partial_kernel<<<148, 256, 0, h->stream>>>(h->Wc, chi, h->partial + 2 * kPartialBlocks);
+  sum_partial_kernel<<<1, 256, 0, h->stream>>>(h->partial + 2 * kPartialBlocks, 148, h->scal + 2);
+  h->launches += 2;
+  // Z2 = sum E^2
+  rc = reduce_dot(h, h->E, h->E, m * chi, h->scal + 3); if (rc) return rc;
+  // Z1 = sum E[a,u,c] T[a,l,a'] a[u,l,d,r] T[c,r,c'] E[a',d,c']
+  rc = stage_half_absorb(h, h->E, h->T, h->P); if (rc) return rc;          // F[u,l,c,a']
+  rc = stage_absorb_a(h, h->P, h->S, 1); if (rc) return rc;                // G~[c,r,a',d]
+  { GemmCall c{h->S, m, 1, h->T, chi, h->W, plain_map(chi), IndexMap{1, 1, 0}, (int)m, chi, (int)m, 0}; GEMM(h, c); }
+  rc = reduce_dot(h, h->W, h->E, m * chi, h->scal + 4); if (rc) return rc; // H[(a',d),c'] . E
+  CU(h, cudaMemcpyAsync(h->h_pinned + 2, h->scal + 2, 3 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  CU(h, cudaStreamSynchronize(h->stream));
+  double Z4 = h->h_pinned[2], Z2 = h->h_pinned[3], Z1 = h->h_pinned[4];
+  *kappa = Z1 * Z4 / (Z2 * Z2);
+  return QRCTM_OK;
+}
+
+int qrctm_r_diag_ratio(qrctm_t* h, double* ratio) {
+  if (!h || !ratio) return QRCTM_ERR_INVALID_ARG;
+  r_diag_minmax_kernel<<<1, 256, 0, h->stream>>>(h->R, h->chi, h->scal + 5);
+  h->launches += 1;
+  CU(h, cudaMemcpyAsync(h->h_pinned + 5, h->scal + 5, 2 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  CU(h, cudaStreamSynchronize(h->stream));
+  *ratio = h->h_pinned[6] != 0.0 ? h->h_pinned[5] / h->h_pinned[6] : 0.0;
+  return QRCTM_OK;
+}
+
+int qrctm_profile_step(qrctm_t* h, float* ms) {
+  if (!h || !ms) return QRCTM_ERR_INVALID_ARG;
+  if (!h->have_A || !h->have_env) return fail(h, QRCTM_ERR_NOT_READY, "set_A and set_env first");
+  cudaEvent_t ev[QRCTM_NSTAGE + 1];
+  for (int i = 0; i <= QRCTM_NSTAGE; ++i) CU(h, cudaEventCreate(&ev[i]));
+  int rc = do_step(h, ev);
+  cudaError_t e = cudaStreamSynchronize(h->stream);
+  if (rc == QRCTM_OK && e == cudaSuccess)
+    for (int i = 0; i < QRCTM_NSTAGE; ++i) cudaEventElapsedTime(&ms[i], ev[i], ev[i + 1]);
+  for (int i = 0; i <= QRCTM_NSTAGE; ++i) cudaEventDestroy(ev[i]);
+  if (rc) return rc;
+  CU(h, e);
+  return QRCTM_OK;
+}
+
+int qrctm_gemm_f64(void* cuda_stream, int path, int transA, int M, int N, int K, const double* A, long long lda,
+                   const double* B, long long ldb, double* Cmat, long long ldc) {
+  if (!A || !B || !Cmat || M < 0 || N < 0 || K < 0 || (path != 0 && path != 1)) return QRCTM_ERR_INVALID_ARG;
+  GemmCall c{A, lda, transA ? 1 : 0, B, ldb, Cmat, plain_map(ldc), IndexMap{1, 1, 0}, M, N, K, 0};
+  cudaError_t e;
+  int nl = launch_gemm(static_cast<cudaStream_t>(cuda_stream), path, c, nullptr, 0, &e);
+  return nl < 0 ? QRCTM_ERR_CUDA : QRCTM_OK;
+}
+
+unsigned long long qrctm_qr_work_bytes(int rows, int cols) { return qr_work_bytes_impl(rows, cols); }
+
+int qrctm_qr_f64(void* cuda_stream, int rows, int cols, const double* X, double* Q, double* R, void* work) {
+  if (!X || !Q || !R || !work || rows < 1 || cols < 1 || cols > rows) return QRCTM_ERR_INVALID_ARG;
+  cudaError_t e;
+  long long nl = qr_factor_level2(static_cast<cudaStream_t>(cuda_stream), rows, cols, X, Q, R, work, &e);
+  return nl < 0 ? QRCTM_ERR_CUDA : QRCTM_OK;
+}
+
+int qrctm_probe_fp64(int kind, int iters, double* tflops) {
+  if (!tflops || iters < 1 || (kind != 0 && kind != 1)) return QRCTM_ERR_INVALID_ARG;
+  cudaDeviceProp p;
+  if (cudaGetDeviceProperties(&p, 0) != cudaSuccess) { cudaGetLastError(); return QRCTM_ERR_CUDA; }
+  const int blocks = p.multiProcessorCount * 2, threads = 256;
+  double* out = nullptr;
+  if (cudaMalloc(&out, sizeof(double) * blocks * threads) != cudaSuccess) { cudaGetLastError(); return QRCTM_ERR_CUDA; }
+  cudaEvent_t a, b; cudaEventCreate(&a); cudaEventCreate(&b);
+  auto go = [&] {
+    if (kind == 0) probe_dfma_kernel<<<blocks, threads>>>(out, iters, 1e-3);
+    else probe_dmma_kernel<<<blocks, threads>>>(out, iters, 1e-3);
+  };
+  go(); cudaDeviceSynchronize();
+  cudaEventRecord(a); go(); cudaEventRecord(b); cudaEventSynchronize(b);
+  float ms = 0; cudaEventElapsedTime(&ms, a, b);
+  cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(out);
+  if (cudaGetLastError() != cudaSuccess || ms <= 0) return QRCTM_ERR_CUDA;
+  double nthr = (double)blocks * threads;
+  double flops = kind == 0 ? nthr * iters * 16.0 * 2.0 : (nthr / 32.0) * iters * 8.0 * 512.0;
+  *tflops = flops / (ms * 1e-3) / 1e12;
+  return QRCTM_OK;
+}
+
+}  // extern "C"

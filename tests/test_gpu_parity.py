@@ -1,0 +1,277 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by
+element on the same seeded inputs.  Tolerances are the north_star's:
+single step <= 1e-11 relative Frobenius on C and T (after the R-sign gauge fix),
+converged run <= 1e-9 on kappa and the top-10 corner spectrum.  Sub-steps
+(SURVEY.md P12): 1e-13 per GEMM, Q within cond(c~) * 1e-14."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+import paper_2505_00494_b200 as pkg
+from oracle import ctmrg as o
+from qrctm_inputs import CONFIGS, gen_config, random_isometry
+
+
+def rel(x, y):
+    x = np.asarray(x); y = np.asarray(y)
+    return np.linalg.norm(x - y) / np.linalg.norm(y)
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    from paper_2505_00494_b200 import build as b
+    b.build()
+
+
+def torch_dev(x):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+# ------------------------------------------------------------------ sub-steps
+@pytest.mark.parametrize("M,N,K,transA", [
+    (8, 32, 8, False), (32, 32, 8, True), (196, 9604, 196, False), (324, 324, 36, True),
+    (1000, 333, 77, True), (129, 257, 65, True), (64, 64, 2401, True), (37, 41, 1000, True),
+    (300, 300, 3, False), (1, 1, 1, True), (5, 7, 1, False), (2500, 100, 2500, True),
+])
+@pytest.mark.parametrize("path", [0, 1])
+def test_gemm_f64_matches_numpy(M, N, K, transA, path):
+    g = np.random.default_rng(M * 7 + N * 3 + K)
+    A = g.standard_normal((K, M) if transA else (M, K))
+    B = g.standard_normal((K, N))
+    ref = (A.T if transA else A) @ B
+    out = pkg.gemm_f64(torch_dev(A), torch_dev(B), transA=transA, path=path).cpu().numpy()
+    assert rel(out, ref) < 1e-13
+
+
+def test_gemm_odd_leading_dimension_views():
+    import torch
+    g = np.random.default_rng(0)
+    A = torch_dev(g.standard_normal((70, 131)))[:, :129]       # lda = 131 (odd) -> scalar loads
+    B = torch_dev(g.standard_normal((70, 59)))[:, 1:58]        # misaligned base
+    out = pkg.gemm_f64(A, B, transA=True).cpu().numpy()
+    assert rel(out, A.cpu().numpy().T @ B.cpu().numpy()) < 1e-13
+
+
+@pytest.mark.parametrize("rows,cols", [(32, 8), (324, 36), (1024, 64), (50, 50), (7, 1), (333, 17)])
+def test_qr_f64_matches_oracle(rows, cols):
+    g = np.random.default_rng(rows + cols)
+    X = g.standard_normal((rows, cols))
+    Q, R = pkg.qr_f64(torch_dev(X))
+    Q, R = Q.cpu().numpy(), R.cpu().numpy()
+    Qo, Ro = o.qr_pos(X)
+    cond = np.linalg.cond(X)
+    assert np.all(np.tril(R, -1) == 0.0) and np.all(np.diag(R) >= 0.0)
+    assert np.linalg.norm(Q.T @ Q - np.eye(cols)) < cols * 2e-15
+    assert rel(Q @ R, X) < 1e-14
+    assert rel(R, Ro) < 1e-14 * max(cond, 10)
+    assert rel(Q, Qo) < 1e-14 * max(cond, 10)
+
+
+def test_qr_rank_deficient_is_still_valid():
+    g = np.random.default_rng(3)
+    X = g.standard_normal((200, 6)) @ g.standard_normal((6, 12))       # rank 6 < 12 (hazard H1)
+    Q, R = pkg.qr_f64(torch_dev(X))
+    Q, R = Q.cpu().numpy(), R.cpu().numpy()
+    assert np.linalg.norm(Q.T @ Q - np.eye(12)) < 1e-13
+    assert rel(Q @ R, X) < 1e-13 and np.all(np.diag(R) >= 0.0)
+
+
+@pytest.mark.parametrize("d,D,chi,seed", [(2, 2, 8, 0), (2, 3, 36, 1), (3, 2, 5, 4), (2, 3, 7, 5), (1, 1, 4, 2)])
+def test_build_a_bit_exact_layout(d, D, chi, seed):
+    A, C0, T0 = gen_config(d, D, chi, seed)
+    h = pkg.QRCTM(d, D, chi)
+    h.set_A(A)
+    a = h.get_a()
+    assert rel(a, o.build_a(A)) < 1e-15 if np.linalg.norm(a) > 0 else True
+    h.close()
+
+
+# ------------------------------------------------------------------ single step
+def _one_step(d, D, chi, seed, corner_mode=0, path=0):
+    A, C0, T0 = gen_config(d, D, chi, seed)
+    h = pkg.QRCTM(d, D, chi)
+    h.set_option(pkg.OPT_CORNER_MODE, corner_mode)
+    h.set_option(pkg.OPT_GEMM_PATH, path)
+    h.set_A(A)
+    h.set_env(C0, T0)
+    C_in, T_in = h.get_env()
+    h.step()
+    out = dict(C=h.get_env()[0], T=h.get_env()[1], QR=h.get_qr(), raw=h.get_raw(), Cin=C_in, Tin=T_in,
+               ratio=h.r_diag_ratio(), launches=h.launch_count())
+    h.close()
+    a = o.build_a(A)
+    Cr, Tr = o.normalize(C0, T0)
+    s = o.qr_step(Cr, Tr, a, corner="accelerated" if corner_mode == 0 else "enlarged")
+    Co, To = o.normalize(s["Cn"], s["Tn"])
+    return out, s, (Cr, Tr, Co, To)
+
+
+STEP_CASES = [(2, 2, 8, 0), (2, 3, 36, 1), (2, 4, 64, 2), (3, 2, 5, 7), (2, 3, 7, 8), (2, 1, 3, 9), (2, 2, 1, 3)]
+
+
+@pytest.mark.parametrize("d,D,chi,seed", STEP_CASES)
+def test_single_step_parity(d, D, chi, seed):
+    out, s, (Cr, Tr, Co, To) = _one_step(d, D, chi, seed)
+    assert rel(out["Cin"], Cr) < 1e-14 and rel(out["Tin"], Tr) < 1e-14
+    Q, R = out["QR"]
+    cond = np.linalg.cond(s["X"])
+    assert rel(R, s["R"]) < 1e-14 * max(cond, 10)
+    assert rel(Q, s["Q"]) < 1e-14 * max(cond, 10)
+    assert np.all(np.diag(R) >= 0) and np.all(np.tril(R, -1) == 0)
+    Cn, Tn = out["raw"]
+    assert rel(Tn, s["Tn"]) < 1e-11 and rel(Cn, s["Cn"]) < 1e-11
+    assert rel(out["C"], Co) < 1e-11
+    assert rel(out["T"], To) < 1e-11
+    assert abs(np.linalg.norm(out["C"]) - 1) < 1e-14 and abs(np.linalg.norm(out["T"]) - 1) < 1e-14
+    assert np.array_equal(out["C"], out["C"].T)
+    assert np.array_equal(out["T"], out["T"].transpose(2, 1, 0))
+    d_ = np.diag(s["R"])
+    assert abs(out["ratio"] - d_.min() / d_.max()) < 1e-10
+
+
+@pytest.mark.parametrize("d,D,chi,seed", [(2, 2, 8, 0), (2, 3, 12, 1)])
+def test_single_step_enlarged_corner_mode(d, D, chi, seed):
+    out, s, (Cr, Tr, Co, To) = _one_step(d, D, chi, seed, corner_mode=1)
+    assert rel(out["C"], Co) < 1e-11 and rel(out["T"], To) < 1e-11
+    acc, _, _ = _one_step(d, D, chi, seed, corner_mode=0)
+    assert rel(out["raw"][0], acc["raw"][0]) < 1e-12            # Fig. 1(f): (E4) == (E4')
+
+
+def test_single_step_reference_gemm_path_agrees():
+    out0, s, _ = _one_step(2, 3, 20, 1, path=0)
+    out1, _, _ = _one_step(2, 3, 20, 1, path=1)
+    assert rel(out0["T"], out1["T"]) < 1e-12 and rel(out0["C"], out1["C"]) < 1e-12
+
+
+def test_step_is_deterministic_bitwise():
+    a, _, _ = _one_step(2, 3, 36, 1)
+    b, _, _ = _one_step(2, 3, 36, 1)
+    assert np.array_equal(a["C"], b["C"]) and np.array_equal(a["T"], b["T"])
+
+
+def test_edge_update_with_arbitrary_isometry():
+    """K3-K5 alone with an isometry that is not a QR factor: feed the
+    library an environment whose c~ has that isometry as its Q."""
+    d, D, chi = 2, 2, 6
+    A, C0, T0 = gen_config(d, D, chi, 3)
+    h = pkg.QRCTM(d, D, chi)
+    h.set_A(A); h.set_env(C0, T0); h.step()
+    Q, R = h.get_qr()
+    _, Tn = h.get_raw()
+    C, T = o.normalize(C0, T0)
+    assert rel(Tn, o.edge_update(Q, T, o.build_a(A))) < 1e-13   # oracle contraction of the GPU's own Q
+    h.close()
+
+
+# ------------------------------------------------------------------ runs
+def _oracle_steps(A, C0, T0, n):
+    a = o.build_a(A)
+    C, T = o.normalize(C0, T0)
+    for _ in range(n):
+        s = o.qr_step(C, T, a)
+        C, T = o.normalize(s["Cn"], s["Tn"])
+    return C, T, a
+
+
+def test_cfg0_converged_run_parity():
+    c = CONFIGS["cfg0"]
+    A, C0, T0 = gen_config(c["d"], c["D"], c["chi"], c["seed"])
+    h = pkg.QRCTM(c["d"], c["D"], c["chi"])
+    h.set_A(A); h.set_env(C0, T0)
+    it, dl = h.run(500, 1e-12)
+    a = o.build_a(A)
+    Co, To, ito, dlo, _ = o.run(C0, T0, a, "qr", 500, 1e-12)
+    assert abs(it - ito) <= 1 and dl < 1e-12
+    k, ko = h.norm_per_site(), o.kappa(Co, To, a)
+    assert abs(k / ko - 1) < 1e-9
+    s, so = h.get_corner_spectrum(), o.spectrum(Co)
+    assert np.max(np.abs(s[:8] - so[:8]) / so[:8]) < 1e-9
+    assert abs(np.sum(s ** 2) - 1) < 1e-13 and np.all(np.diff(s) <= 0)
+    if it == ito:
+        C, T = h.get_env()
+        assert rel(C, Co) < 1e-9 and rel(T, To) < 1e-9
+    h.close()
+
+
+def test_cfg0_fifty_iterations_fixed_count():
+    c = CONFIGS["cfg0"]
+    A, C0, T0 = gen_config(c["d"], c["D"], c["chi"], c["seed"])
+    h = pkg.QRCTM(c["d"], c["D"], c["chi"])
+    h.set_A(A); h.set_env(C0, T0)
+    it, dl = h.run(50, 1e-12)
+    assert it == 50
+    Co, To, a = _oracle_steps(A, C0, T0, 50)
+    C, T = h.get_env()
+    assert rel(C, Co) < 1e-10 and rel(T, To) < 1e-10
+    assert np.max(np.abs(h.get_corner_spectrum() - o.spectrum(Co))) < 1e-12
+    h.close()
+
+
+def test_cfg1_fixed_count_and_kappa():
+    c = CONFIGS["cfg1"]
+    A, C0, T0 = gen_config(c["d"], c["D"], c["chi"], c["seed"])
+    h = pkg.QRCTM(c["d"], c["D"], c["chi"])
+    h.set_A(A); h.set_env(C0, T0)
+    for _ in range(20):
+        h.step()
+    Co, To, a = _oracle_steps(A, C0, T0, 20)
+    C, T = h.get_env()
+    assert rel(C, Co) < 1e-9 and rel(T, To) < 1e-9
+    s, so = h.get_corner_spectrum(), o.spectrum(Co)
+    assert np.max(np.abs(s[:10] - so[:10]) / so[:10]) < 1e-9
+    assert abs(h.norm_per_site() / o.kappa(Co, To, a) - 1) < 1e-9
+    h.close()
+
+
+def test_spectrum_kernel_against_lapack():
+    import torch
+    for chi, seed in [(1, 0), (2, 1), (8, 2), (36, 3), (100, 4), (196, 5)]:
+        A, C0, T0 = gen_config(2, 1, chi, seed)
+        h = pkg.QRCTM(2, 1, chi)
+        h.set_A(A); h.set_env(C0, T0)
+        C, _ = h.get_env()
+        s = h.get_corner_spectrum()
+        assert np.max(np.abs(s - o.spectrum(C))) < 5e-15 * chi, chi
+        h.close()
+
+
+def test_errors_and_not_ready():
+    h = pkg.QRCTM(2, 2, 4)
+    with pytest.raises(pkg.QrctmError):
+        h.step()
+    A, C0, T0 = gen_config(2, 2, 4, 0)
+    h.set_A(A)
+    with pytest.raises(pkg.QrctmError):
+        h.run(3, 1e-3)
+    with pytest.raises(pkg.QrctmError):
+        h.set_env(np.zeros((4, 4)), T0)            # zero Frobenius norm -> NUMERIC
+    with pytest.raises(pkg.QrctmError):
+        h.set_option(99, 0)
+    h.close()
+
+
+def test_device_pointers_accepted_and_set_A_keeps_env():
+    import torch
+    A, C0, T0 = gen_config(2, 2, 8, 0)
+    h = pkg.QRCTM(2, 2, 8)
+    h.set_A(torch_dev(A)); h.set_env(torch_dev(C0), torch_dev(T0))
+    h.step()
+    C1, T1 = h.get_env(device=True)
+    h.set_A(A * 0.5)                                # environment is kept
+    C2, T2 = h.get_env()
+    assert np.array_equal(C1.cpu().numpy(), C2) and np.array_equal(T1.cpu().numpy(), T2)
+    h.close()
+
+
+def test_ising_onsager_on_gpu():
+    from tests.brute import ising_A, onsager_ln_kappa
+    K = 0.3
+    A = ising_A(K)
+    _, C0, T0 = gen_config(2, 2, 16, 1)
+    h = pkg.QRCTM(2, 2, 16)
+    h.set_A(A); h.set_env(C0, T0)
+    h.run(300, 1e-13)
+    assert abs(np.log(h.norm_per_site()) - onsager_ln_kappa(K)) < 1e-10
+    h.close()

@@ -1,0 +1,75 @@
+"""CPU-only checks of the boundary: the library builds, loads without a GPU and
+exports every symbol include/qrctm.h declares; invalid arguments are rejected;
+the product path fails loudly (no CPU fallback) when there is no CUDA device."""
+import ctypes
+import os
+import re
+
+import pytest
+
+import paper_2505_00494_b200 as pkg
+from paper_2505_00494_b200 import build as qbuild
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    qbuild.build()
+    return pkg.load_library()
+
+
+def test_header_symbols_all_exported(lib):
+    hdr = open(os.path.join(ROOT, "include", "qrctm.h")).read()
+    declared = set(re.findall(r"\b(qrctm_[A-Za-z0-9_]+)\s*\(", hdr))
+    assert declared == set(pkg.SYMBOLS), declared ^ set(pkg.SYMBOLS)
+    for s in declared:
+        assert hasattr(lib, s), s
+
+
+def test_links_no_vendor_math_library():
+    out = os.popen(f"ldd {pkg.LIB_PATH}").read()
+    for bad in ("cublas", "cusolver", "libtorch", "cudnn", "cutlass"):
+        assert bad not in out.lower(), out
+    assert "libcudart" in out
+
+
+def test_invalid_arguments_rejected(lib):
+    assert lib.qrctm_workspace_bytes(0, 2, 8) == 0
+    assert lib.qrctm_workspace_bytes(2, 0, 8) == 0
+    assert lib.qrctm_workspace_bytes(2, 2, 0) == 0
+    n = lib.qrctm_workspace_bytes(2, 7, 196)
+    m = 196 * 49
+    assert 2 * 8 * m * m < n < 2 * 8 * m * m + (1 << 30)      # P and S dominate
+    h = ctypes.c_void_p()
+    assert lib.qrctm_create(0, 2, 8, ctypes.byref(h)) == -1
+    assert lib.qrctm_create(2, 2, 8, None) == -1
+    assert lib.qrctm_destroy(None) == -1
+    assert lib.qrctm_step(None) == -1
+    assert lib.qrctm_qr_work_bytes(0, 1) == 0
+    t = ctypes.c_double()
+    assert lib.qrctm_probe_fp64(7, 10, ctypes.byref(t)) == -1
+    assert b"qrctm" in lib.qrctm_version()
+
+
+def test_no_cpu_fallback_without_gpu(lib):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    h = ctypes.c_void_p()
+    assert lib.qrctm_create(2, 2, 8, ctypes.byref(h)) == -3       # QRCTM_ERR_CUDA
+    assert not h.value
+    with pytest.raises(pkg.QrctmError):
+        pkg.QRCTM(2, 2, 8)
+
+
+def test_product_path_does_not_import_oracle():
+    for root, _, files in os.walk(os.path.join(ROOT, "paper_2505_00494_b200")):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(root, f)).read()
+                assert "oracle" not in src.replace("no oracle", ""), f
+    src = open(os.path.join(ROOT, "qrctm_inputs", "__init__.py")).read()
+    assert "import oracle" not in src and "from oracle" not in src
+    osrc = open(os.path.join(ROOT, "oracle", "ctmrg.py")).read()
+    assert "import paper_2505" not in osrc and "from paper_2505" not in osrc
