@@ -1,0 +1,309 @@
+#!/usr/bin/env python
+"""bench.py -- QR-CTMRG iterations/s on one B200 (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path: K1..K7 (one QR-CTMRG iteration) plus
+K8 (corner spectrum + convergence delta), i.e. what qrctm_run does per
+iteration.  Default workload: BASELINE.json configs[4] (d=2, D=7, chi=196), the
+configuration the north_star's roofline target is quoted on; `--config` selects
+another one.  Inputs are the seeded synthetic tensors of qrctm_inputs.
+
+  value      iterations/s with A, C, T resident in HBM (CUDA events around qrctm_run)
+  e2e        iterations/s through the C ABI with HOST buffers: every step copies
+             A, C, T from pinned host memory, runs one iteration and copies C, T and
+             delta back (copies inside the timed region)
+  roofline   the dominant kernel (K4, P.a, FP64 DMMA GEMM): algorithmic flops
+             2 chi^2 D^8 per launch / its mean CUDA-event duration in the timed run,
+             against the FP64 tensor issue rate measured live by qrctm_probe_fp64
+  cpu_baseline  the oracle (NumPy) timed on the host cores, rank 0, bounded sample
+
+Multi-GPU: the path is one dependent chain on one GPU:
+"replicas only" -- each rank runs an independent instance, no collective.
+
+`--impl reference` times the oracle as it stands on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from qrctm_inputs import CONFIGS, gen_named  # noqa: E402
+
+METRIC = "QR-CTMRG iterations/s"
+UNIT = "iterations/s"
+
+
+def step_flops(D, chi):
+    b = D * D
+    m = chi * b
+    return dict(K1=2 * chi ** 3 * b, K2=4 * m * chi ** 2 - (4 / 3) * chi ** 3, K3=2 * m * m * chi,
+                K4=2 * chi ** 2 * b ** 4, K5=2 * m * m * chi, K6=4 * chi ** 3 * b)
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_time_steps(name, max_steps, budget_s):
+    """Time the oracle's QR-CTMRG iteration (qr_step + normalize + spectrum) as it stands."""
+    from oracle import ctmrg as o
+    try:
+        from threadpoolctl import threadpool_info
+        cores = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
+    except Exception:
+        cores = os.cpu_count()
+    A, C0, T0, c = gen_named(name)
+    a = o.build_a(A)
+    C, T = o.normalize(C0, T0)
+    times = []
+    t_all = time.perf_counter()
+    for _ in range(max_steps):
+        t0 = time.perf_counter()
+        s = o.qr_step(C, T, a)
+        C, T = o.normalize(s["Cn"], s["Tn"])
+        o.spectrum(C)
+        times.append(time.perf_counter() - t0)
+        if time.perf_counter() - t_all > budget_s:
+            break
+    return times, cores
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    name = args.config
+    c = CONFIGS[name]
+    total = args.steps + args.warmup
+    times, cores = oracle_time_steps(name, total, budget_s=150.0)
+    timed = times[args.warmup:] if len(times) > args.warmup else times[-1:]
+    ms = 1e3 * float(np.mean(timed))
+    val = 1e3 / ms
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": len(timed), "warmup": min(args.warmup, len(times) - len(timed)), "ms_per_step": ms,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{name}: d={c['d']} D={c['D']} chi={c['chi']} seed={c['seed']} (BASELINE.json configs)",
+                   "step": "oracle qr_step + normalize + spectrum (NumPy FP64, host BLAS)"},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": f"{len(timed)} full iterations of {name} after {len(times) - len(timed)} warm-up"},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="cfg4", choices=sorted(CONFIGS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+    if args.warmup < 3:
+        args.warmup = 3
+
+    import torch
+    import torch.distributed as dist
+    import paper_2505_00494_b200 as pkg
+    from paper_2505_00494_b200 import build as qbuild
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl")
+    if rank == 0:
+        qbuild.build()
+    if world > 1:
+        dist.barrier()
+
+    name = args.config
+    A, C0, T0, c = gen_named(name)
+    d, D, chi = c["d"], c["D"], c["chi"]
+    b = D * D
+    fl = step_flops(D, chi)
+
+    h = pkg.QRCTM(d, D, chi)
+    h.set_A(A)
+    h.set_env(C0, T0)
+    h.run(args.warmup, -1.0)                 # warm-up (tol < 0: never stops early)
+    peak_dmma = pkg.probe_fp64(1)
+    peak_dfma = pkg.probe_fp64(0)
+
+    # ---- device-resident timing: K steps, barrier + sync on both sides, CUDA events
+    h.set_option(pkg.OPT_TIME_STAGES, 1)
+    h.run(1, -1.0)
+    h.get_stage_ms(reset=True)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n0 = h.launch_count()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ev0.record()
+    it, delta = h.run(args.steps, -1.0)
+    ev1.record()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    ms_total = ev0.elapsed_time(ev1)
+    launches = h.launch_count() - n0
+    stage_ms, nst = h.get_stage_ms(reset=True)
+    clocks = sampler.stop() if rank == 0 else None
+    h.set_option(pkg.OPT_TIME_STAGES, 0)
+    assert it == args.steps and nst == args.steps
+
+    # ---- end to end through the C ABI with host buffers (pinned), copies inside the timed region
+    Ah = torch.from_numpy(A).pin_memory()
+    Ch, Th = torch.from_numpy(C0).pin_memory(), torch.from_numpy(T0).pin_memory()
+    Co = torch.empty((chi, chi), dtype=torch.float64).pin_memory()
+    To = torch.empty((chi, b, chi), dtype=torch.float64).pin_memory()
+    import ctypes
+    lib = h.lib
+    P = ctypes.c_void_p
+
+    bufs = {"in": (Ch, Th), "out": (Co, To)}
+
+    def e2e_step():
+        ci, ti = bufs["in"]
+        co, to = bufs["out"]
+        assert lib.qrctm_set_A(h._h, P(Ah.data_ptr())) == 0
+        assert lib.qrctm_set_env(h._h, P(ci.data_ptr()), P(ti.data_ptr())) == 0
+        its, dl = h.run(1, -1.0)
+        assert lib.qrctm_get_env(h._h, P(co.data_ptr()), P(to.data_ptr())) == 0
+        bufs["in"], bufs["out"] = (co, to), (ci, ti)   # next step continues from the returned environment
+        return dl
+
+    for _ in range(2):
+        e2e_step()
+    torch.cuda.synchronize()
+    e2e_n = max(3, min(args.steps, 10))
+    t0 = time.perf_counter()
+    for _ in range(e2e_n):
+        e2e_step()
+    torch.cuda.synchronize()
+    e2e_ms = 1e3 * (time.perf_counter() - t0) / e2e_n
+    h2d = 8 * (A.size + C0.size + T0.size)
+    d2h = 8 * (C0.size + T0.size) + 8
+
+    # ---- max over ranks
+    if world > 1:
+        t = torch.tensor([ms_total, e2e_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total, e2e_ms = float(t[0]), float(t[1])
+    ms_per_step = ms_total / args.steps
+    value = world * args.steps / (ms_total * 1e-3)
+    e2e_value = world * 1e3 / e2e_ms
+
+    if rank == 0:
+        k4_ms = stage_ms["K4_absorb_a"] / nst
+        ach = fl["K4"] / (k4_ms * 1e-3) / 1e12
+        traffic = None
+        tpath = os.path.join(ROOT, "profiles", "k4_traffic_bytes.json")
+        if os.path.exists(tpath):
+            try:
+                traffic = json.load(open(tpath)).get(name)
+            except Exception:
+                traffic = None
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{name}: d={d} D={D} chi={chi} seed={c['seed']} (BASELINE.json configs)",
+                       "step": "K1..K7 + K8 spectrum check (qrctm_run, check_every=1)",
+                       "l2": "inputs larger than L2 (P and S are %.0f MB each; L2 126 MB)" % (8e-6 * (chi * b) ** 2)
+                             if 8 * (chi * b) ** 2 > 126e6 else "working set smaller than L2: L2-resident by design, no flush",
+                       "multi_gpu": "replicas only"},
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "ms_per_step": e2e_ms},
+            "gpu_launches": int(launches),
+            "clocks": clocks,
+            "roofline": {"bound": "tensor", "kernel": "gemm_f64_dmma (K4: S = P.a)", "achieved": ach,
+                         "peak": peak_dmma, "unit": "TFLOP/s", "frac": ach / peak_dmma, "traffic": traffic,
+                         "peak_source": "FP64 DMMA issue rate measured live by qrctm_probe_fp64 "
+                                        "(MEASURED_PEAKS.json has no FP64 entry; nominal 148 SM x 64 FMA/clk x 1.965 GHz = 37.2)",
+                         "dfma_peak": peak_dfma, "algorithmic_flops_per_launch": fl["K4"], "ms_per_launch": k4_ms},
+            "stages_ms": {k: v / nst for k, v in stage_ms.items()},
+            "step_tflops": sum(fl.values()) / (ms_per_step * 1e-3) / 1e12,
+            "step_frac_of_fp64_peak": sum(fl.values()) / (ms_per_step * 1e-3) / 1e12 / peak_dmma,
+        }
+        if not args.no_cpu_baseline and world == 1:
+            budget = 20.0
+            times, cores = oracle_time_steps(name, 50, budget_s=budget)
+            tt = times[1:] if len(times) > 1 else times
+            cms = 1e3 * float(np.mean(tt))
+            line["cpu_baseline"] = {"value": 1e3 / cms, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                    "sample": f"{len(tt)} full iterations of {name} (oracle qr_step+normalize+spectrum, "
+                                              f"NumPy {np.__version__}), first one discarded" if len(times) > 1 else
+                                              f"1 iteration of {name}",
+                                    "ms_per_step": cms}
+        print(json.dumps(line), flush=True)
+    h.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -55,7 +55,8 @@ enum {
   QRCTM_OPT_CORNER_MODE = 1, /* 0 = accelerated (E4) [default], 1 = enlarged corner (E5)+(E4')          */
   QRCTM_OPT_SYMMETRIZE = 2,  /* 1 [default] = symmetrise C', T' before normalising, 0 = only normalise   */
   QRCTM_OPT_CHECK_EVERY = 3, /* qrctm_run computes the corner spectrum / delta every n steps, default 1 */
-  QRCTM_OPT_GEMM_PATH = 4    /* 0 = FP64 tensor-core (DMMA) tiles [default], 1 = plain DFMA reference kernel */
+  QRCTM_OPT_GEMM_PATH = 4,   /* 0 = FP64 tensor-core (DMMA) tiles [default], 1 = plain DFMA reference kernel */
+  QRCTM_OPT_TIME_STAGES = 5  /* 1 = qrctm_run records CUDA events around every stage of every step (default 0) */
 };
 
 /* Create a handle for dimensions (d, D, chi); allocates every workspace with
@@ -146,6 +147,11 @@ long long qrctm_launch_count(const qrctm_t* h);
  * 3 K4 absorb a, 4 K5 project, 5 K6 corner, 6 K7 symmetrise+normalise. */
 #define QRCTM_NSTAGE 7
 int qrctm_profile_step(qrctm_t* h, float* ms);
+
+/* Per-stage device time accumulated by qrctm_run while QRCTM_OPT_TIME_STAGES = 1:
+ * ms[0..6] as in qrctm_profile_step, ms[7] = K8 spectrum + delta; *steps = number
+ * of steps accumulated.  reset != 0 clears the accumulators.  HOST pointers. */
+int qrctm_get_stage_ms(qrctm_t* h, double* ms /* QRCTM_NSTAGE + 1 */, long long* steps, int reset);
 
 /* Stand-alone FP64 GEMM entry used by the sub-step parity tests and the
  * roofline bench:  Cmat[M][N] = op(A) * B with B[K][N] row-major and

@@ -19,17 +19,18 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libqrctm.so")
 
 QRCTM_OK = 0
-OPT_CORNER_MODE, OPT_SYMMETRIZE, OPT_CHECK_EVERY, OPT_GEMM_PATH = 1, 2, 3, 4
+OPT_CORNER_MODE, OPT_SYMMETRIZE, OPT_CHECK_EVERY, OPT_GEMM_PATH, OPT_TIME_STAGES = 1, 2, 3, 4, 5
 NSTAGE = 7
 STAGE_NAMES = ("K1_reduced_corner", "K2_qr", "K3_half_absorb", "K4_absorb_a", "K5_project",
                "K6_corner", "K7_normalize")
+STAGE_NAMES_RUN = STAGE_NAMES + ("K8_spectrum",)
 
 # every symbol include/qrctm.h declares (tests check that the .so exports them all)
 SYMBOLS = (
     "qrctm_create", "qrctm_workspace_bytes", "qrctm_create_in", "qrctm_destroy", "qrctm_set_stream",
     "qrctm_set_A", "qrctm_set_env", "qrctm_step", "qrctm_run", "qrctm_get_env",
     "qrctm_get_corner_spectrum", "qrctm_get_qr", "qrctm_get_raw", "qrctm_get_a", "qrctm_norm_per_site",
-    "qrctm_r_diag_ratio", "qrctm_set_option", "qrctm_launch_count", "qrctm_profile_step",
+    "qrctm_r_diag_ratio", "qrctm_set_option", "qrctm_launch_count", "qrctm_get_stage_ms", "qrctm_profile_step",
     "qrctm_gemm_f64", "qrctm_qr_work_bytes", "qrctm_qr_f64", "qrctm_probe_fp64", "qrctm_last_error",
     "qrctm_version",
 )
@@ -73,6 +74,7 @@ def load_library() -> ctypes.CDLL:
     lib.qrctm_launch_count.argtypes = [P]
     lib.qrctm_launch_count.restype = c_longlong
     lib.qrctm_profile_step.argtypes = [P, POINTER(c_float)]
+    lib.qrctm_get_stage_ms.argtypes = [P, POINTER(c_double), POINTER(c_longlong), c_int]
     lib.qrctm_gemm_f64.argtypes = [P, c_int, c_int, c_int, c_int, c_int, P, c_longlong, P, c_longlong, P,
                                    c_longlong]
     lib.qrctm_qr_work_bytes.argtypes = [c_int, c_int]
@@ -214,6 +216,13 @@ class QRCTM:
 
     def launch_count(self) -> int:
         return int(self.lib.qrctm_launch_count(self._h))
+
+    def get_stage_ms(self, reset: bool = False):
+        """(dict stage -> total ms, steps) accumulated by run() while OPT_TIME_STAGES = 1."""
+        ms = (c_double * (NSTAGE + 1))()
+        n = c_longlong(0)
+        self._check(self.lib.qrctm_get_stage_ms(self._h, ms, byref(n), int(reset)))
+        return dict(zip(STAGE_NAMES_RUN, [float(x) for x in ms])), int(n.value)
 
     def profile_step(self):
         ms = (c_float * NSTAGE)()

@@ -40,8 +40,12 @@ struct qrctm {
   bool owns_ws;
   Layout L;
   bool have_A, have_env;
-  int corner_mode, symmetrize, check_every, gemm_path;
+  int corner_mode, symmetrize, check_every, gemm_path, time_stages;
   long long launches;
+  cudaEvent_t ev[QRCTM_NSTAGE + 2];
+  bool have_ev;
+  double stage_ms[QRCTM_NSTAGE + 1];
+  long long stage_steps;
   char err[256];
   double* h_pinned;       // [0] delta, [1..] scratch ; pinned host
   int* h_flag;
@@ -470,6 +474,7 @@ int qrctm_destroy(qrctm_t* h) {
   cudaStreamSynchronize(h->stream);
   if (h->owns_ws && h->base) cudaFree(h->base);
   if (h->h_pinned) cudaFreeHost(h->h_pinned);
+  if (h->have_ev) for (int i = 0; i < QRCTM_NSTAGE + 2; ++i) cudaEventDestroy(h->ev[i]);
   cudaGetLastError();
   delete h;
   return QRCTM_OK;
@@ -521,12 +526,29 @@ int qrctm_run(qrctm_t* h, int max_iter, double tol, int* iters_done, double* fin
   if (max_iter < 0) return fail(h, QRCTM_ERR_INVALID_ARG, "max_iter < 0");
   double delta = INFINITY;
   int it = 0;
+  if (h->time_stages && !h->have_ev) {
+    for (int i = 0; i < QRCTM_NSTAGE + 2; ++i) CU(h, cudaEventCreate(&h->ev[i]));
+    h->have_ev = true;
+  }
   for (it = 1; it <= max_iter; ++it) {
-    int rc = do_step(h, nullptr); if (rc) return rc;
-    if (it % h->check_every == 0 || it == max_iter) {
+    int rc = do_step(h, h->time_stages ? h->ev : nullptr); if (rc) return rc;
+    const bool check = (it % h->check_every == 0 || it == max_iter);
+    if (check) {
       rc = stage_spectrum(h, h->s, 1); if (rc) return rc;
       CU(h, cudaMemcpyAsync(h->h_pinned, h->delta, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
-      rc = check_flag(h); if (rc) return rc;       // synchronises
+    }
+    if (h->time_stages) CU(h, cudaEventRecord(h->ev[QRCTM_NSTAGE + 1], h->stream));
+    if (check) { rc = check_flag(h); if (rc) return rc; }       // synchronises
+    else if (h->time_stages) CU(h, cudaStreamSynchronize(h->stream));
+    if (h->time_stages) {
+      for (int i = 0; i <= QRCTM_NSTAGE; ++i) {
+        float ms = 0.f;
+        CU(h, cudaEventElapsedTime(&ms, h->ev[i], h->ev[i + 1]));
+        h->stage_ms[i] += ms;
+      }
+      h->stage_steps += 1;
+    }
+    if (check) {
       delta = h->h_pinned[0];
       if (delta < tol) break;
     }
@@ -587,12 +609,21 @@ int qrctm_set_option(qrctm_t* h, int key, int value) {
     case QRCTM_OPT_SYMMETRIZE:  if (value != 0 && value != 1) break; h->symmetrize = value; return QRCTM_OK;
     case QRCTM_OPT_CHECK_EVERY: if (value < 1) break; h->check_every = value; return QRCTM_OK;
     case QRCTM_OPT_GEMM_PATH:   if (value != 0 && value != 1) break; h->gemm_path = value; return QRCTM_OK;
+    case QRCTM_OPT_TIME_STAGES: if (value != 0 && value != 1) break; h->time_stages = value; return QRCTM_OK;
     default: break;
   }
   return fail(h, QRCTM_ERR_INVALID_ARG, "bad option key/value");
 }
 
 long long qrctm_launch_count(const qrctm_t* h) { return h ? h->launches : 0; }
+
+int qrctm_get_stage_ms(qrctm_t* h, double* ms, long long* steps, int reset) {
+  if (!h) return QRCTM_ERR_INVALID_ARG;
+  if (ms) for (int i = 0; i <= QRCTM_NSTAGE; ++i) ms[i] = h->stage_ms[i];
+  if (steps) *steps = h->stage_steps;
+  if (reset) { for (int i = 0; i <= QRCTM_NSTAGE; ++i) h->stage_ms[i] = 0.0; h->stage_steps = 0; }
+  return QRCTM_OK;
+}
 
 const char* qrctm_last_error(const qrctm_t* h) { return h ? h->err : "null handle"; }
 
