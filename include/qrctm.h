@@ -56,7 +56,8 @@ enum {
   QRCTM_OPT_SYMMETRIZE = 2,  /* 1 [default] = symmetrise C', T' before normalising, 0 = only normalise   */
   QRCTM_OPT_CHECK_EVERY = 3, /* qrctm_run computes the corner spectrum / delta every n steps, default 1 */
   QRCTM_OPT_GEMM_PATH = 4,   /* 0 = FP64 tensor-core (DMMA) tiles [default], 1 = plain DFMA reference kernel */
-  QRCTM_OPT_TIME_STAGES = 5  /* 1 = qrctm_run records CUDA events around every stage of every step (default 0) */
+  QRCTM_OPT_TIME_STAGES = 5, /* 1 = qrctm_run records CUDA events around every stage of every step (default 0) */
+  QRCTM_OPT_QR_PATH = 6      /* 0 = blocked compact-WY QR, cluster panel kernel [default], 1 = level-2 column kernels */
 };
 
 /* Create a handle for dimensions (d, D, chi); allocates every workspace with
@@ -113,7 +114,7 @@ int qrctm_run(qrctm_t* h, int max_iter, double tol, int* iters_done, double* fin
 int qrctm_get_env(qrctm_t* h, double* C, double* T);
 
 /* Descending singular values (= |eigenvalues|) of the current normalised C,
- * computed on the device by a cyclic Jacobi eigenvalue iteration; s has chi
+ * computed on the device (Householder tridiagonalisation + Sturm bisection); s has chi
  * entries; sum s^2 = 1. */
 int qrctm_get_corner_spectrum(qrctm_t* h, double* s);
 
@@ -162,10 +163,11 @@ int qrctm_gemm_f64(void* cuda_stream, int path, int transA, int M, int N, int K,
                    double* Cmat, long long ldc);
 
 /* Stand-alone QR entry (K2): factor X[rows][cols] (DEVICE, row-major, cols <=
- * rows) into Q[rows][cols], R[cols][cols] with diag(R) >= 0. work must hold
+ * rows) into Q[rows][cols], R[cols][cols] with diag(R) >= 0 (path: see
+ * QRCTM_OPT_QR_PATH). work must hold
  * qrctm_qr_work_bytes(rows, cols) bytes (DEVICE). */
 unsigned long long qrctm_qr_work_bytes(int rows, int cols);
-int qrctm_qr_f64(void* cuda_stream, int rows, int cols, const double* X, double* Q,
+int qrctm_qr_f64(void* cuda_stream, int path, int rows, int cols, const double* X, double* Q,
                  double* R, void* work);
 
 /* FP64 issue-rate probe (roofline denominators):

@@ -19,7 +19,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libqrctm.so")
 
 QRCTM_OK = 0
-OPT_CORNER_MODE, OPT_SYMMETRIZE, OPT_CHECK_EVERY, OPT_GEMM_PATH, OPT_TIME_STAGES = 1, 2, 3, 4, 5
+OPT_CORNER_MODE, OPT_SYMMETRIZE, OPT_CHECK_EVERY, OPT_GEMM_PATH, OPT_TIME_STAGES, OPT_QR_PATH = 1, 2, 3, 4, 5, 6
 NSTAGE = 7
 STAGE_NAMES = ("K1_reduced_corner", "K2_qr", "K3_half_absorb", "K4_absorb_a", "K5_project",
                "K6_corner", "K7_normalize")
@@ -79,7 +79,7 @@ def load_library() -> ctypes.CDLL:
                                    c_longlong]
     lib.qrctm_qr_work_bytes.argtypes = [c_int, c_int]
     lib.qrctm_qr_work_bytes.restype = c_ulonglong
-    lib.qrctm_qr_f64.argtypes = [P, c_int, c_int, P, P, P, P]
+    lib.qrctm_qr_f64.argtypes = [P, c_int, c_int, c_int, P, P, P, P]
     lib.qrctm_probe_fp64.argtypes = [c_int, c_int, POINTER(c_double)]
     lib.qrctm_last_error.argtypes = [P]
     lib.qrctm_last_error.restype = c_char_p
@@ -250,7 +250,7 @@ def gemm_f64(A, B, transA: bool = False, path: int = 0):
     return out
 
 
-def qr_f64(X):
+def qr_f64(X, path: int = 0):
     """(Q, R) with diag(R) >= 0 of a torch CUDA float64 matrix through qrctm_qr_f64."""
     import torch
     lib = load_library()
@@ -258,7 +258,7 @@ def qr_f64(X):
     Q = torch.empty((rows, cols), dtype=torch.float64, device="cuda")
     R = torch.empty((cols, cols), dtype=torch.float64, device="cuda")
     work = torch.empty(lib.qrctm_qr_work_bytes(rows, cols), dtype=torch.uint8, device="cuda")
-    rc = lib.qrctm_qr_f64(c_void_p(torch.cuda.current_stream().cuda_stream), rows, cols, _ptr(X), _ptr(Q),
+    rc = lib.qrctm_qr_f64(c_void_p(torch.cuda.current_stream().cuda_stream), path, rows, cols, _ptr(X), _ptr(Q),
                           _ptr(R), c_void_p(work.data_ptr()))
     if rc != QRCTM_OK:
         raise QrctmError(f"qrctm_qr_f64 failed: {rc}")

@@ -40,7 +40,7 @@ struct qrctm {
   bool owns_ws;
   Layout L;
   bool have_A, have_env;
-  int corner_mode, symmetrize, check_every, gemm_path, time_stages;
+  int corner_mode, symmetrize, check_every, gemm_path, time_stages, qr_path;
   long long launches;
   cudaEvent_t ev[QRCTM_NSTAGE + 2];
   bool have_ev;
@@ -233,21 +233,43 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
 // ------------------------------------------------------------------ K2: QR driver
 namespace {
 
+constexpr int QR_NB = 16;
+
+struct QrWork {     // carved out of the caller's work buffer
+  double *V, *Vc, *tau, *Tfac, *W1, *W2, *splitk;
+  size_t splitk_elems;
+};
+
+size_t qr_layout(long long rows, int n, char* base, QrWork* w) {
+  size_t off = 0;
+  auto take = [&](size_t elems) { size_t o = off; off = align_up(off + sizeof(double) * elems); return o; };
+  size_t oV = take((size_t)rows * n), oVc = take((size_t)rows * n), otau = take(n);
+  size_t npan = (n + QR_NB - 1) / QR_NB;
+  size_t oT = take(npan * QR_NB * QR_NB), oW1 = take((size_t)QR_NB * n), oW2 = take((size_t)QR_NB * n);
+  size_t sk = (size_t)512 * QR_NB * n;
+  size_t oS = take(sk);
+  if (w) {
+    w->V = reinterpret_cast<double*>(base + oV); w->Vc = reinterpret_cast<double*>(base + oVc);
+    w->tau = reinterpret_cast<double*>(base + otau); w->Tfac = reinterpret_cast<double*>(base + oT);
+    w->W1 = reinterpret_cast<double*>(base + oW1); w->W2 = reinterpret_cast<double*>(base + oW2);
+    w->splitk = reinterpret_cast<double*>(base + oS); w->splitk_elems = sk;
+  }
+  return off;
+}
+
 unsigned long long qr_work_bytes_impl(long long rows, int cols) {
   if (rows < 1 || cols < 1) return 0;
-  size_t v = align_up(sizeof(double) * (size_t)rows * cols);        // V: working copy / reflectors
-  size_t t = align_up(sizeof(double) * (size_t)cols);               // tau
-  size_t extra = align_up(sizeof(double) * ((size_t)cols * cols * 4 + 1024));
-  return v + t + extra;
+  return qr_layout(rows, cols, nullptr, nullptr);
 }
 
 // X (rows x n, ld n, DEVICE, untouched) -> Q (rows x n), R (n x n), diag(R) >= 0.
 // Level-2 Householder (one reflector at a time).  Returns kernels launched or -1.
 long long qr_factor_level2(cudaStream_t st, long long rows, int n, const double* X, double* Q, double* R,
                            void* work, cudaError_t* err) {
-  char* wb = static_cast<char*>(work);
-  double* V = reinterpret_cast<double*>(wb);
-  double* tau = reinterpret_cast<double*>(wb + align_up(sizeof(double) * (size_t)rows * n));
+  QrWork wk;
+  qr_layout(rows, n, static_cast<char*>(work), &wk);
+  double* V = wk.V;
+  double* tau = wk.tau;
   long long launches = 0;
   *err = cudaMemcpyAsync(V, X, sizeof(double) * rows * n, cudaMemcpyDeviceToDevice, st);
   if (*err != cudaSuccess) return -1;
@@ -268,6 +290,99 @@ long long qr_factor_level2(cudaStream_t st, long long rows, int n, const double*
     int nb = (n - k + CPB - 1) / CPB;
     house_apply_kernel<CPB><<<nb, 512, 0, st>>>(V, n, rows, k, tau, Q, n, k, n);
     ++launches;
+  }
+  sign_fix_kernel<<<296, 256, 0, st>>>(Q, rows, n, R);
+  sign_fix_R_kernel<<<n, 128, 0, st>>>(R, n);
+  launches += 2;
+  *err = cudaGetLastError();
+  return *err == cudaSuccess ? launches : -1;
+}
+
+// Panel launch: one cluster of C CTAs x 1024 threads.
+cudaError_t launch_panel(cudaStream_t st, double* V, long long ld, long long m, int j0, int nbw, double* Vc,
+                         double* tau, double* Tp) {
+  constexpr int NB = QR_NB;
+  static int max_smem = -1, cluster16 = -1;
+  if (max_smem < 0) {
+    int dev = 0; cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    cudaError_t e = cudaFuncSetAttribute(qr_panel_cluster_kernel<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         max_smem);
+    if (e != cudaSuccess) return e;
+    cluster16 = cudaFuncSetAttribute(qr_panel_cluster_kernel<NB>, cudaFuncAttributeNonPortableClusterSizeAllowed,
+                                     1) == cudaSuccess ? 1 : 0;
+    cudaGetLastError();
+  }
+  const long long prow = m - j0;
+  const size_t fixed = sizeof(double) * (2 * 16 * NB + 2 * NB + 32 * NB + 3 * NB + NB * NB + 16 * NB * NB);
+  const size_t scratch = sizeof(double) * 1024;
+  int C = 8;
+  if (prow < 8 * 64) C = prow >= 256 ? 4 : (prow >= 64 ? 2 : 1);
+  long long rpc = (prow + C - 1) / C;
+  size_t slice = sizeof(double) * (size_t)rpc * NB;
+  int use_smem = 1;
+  if (fixed + scratch + slice > (size_t)max_smem) {
+    if (cluster16) {
+      C = 16; rpc = (prow + C - 1) / C; slice = sizeof(double) * (size_t)rpc * NB;
+    }
+    if (fixed + scratch + slice > (size_t)max_smem) { use_smem = 0; slice = 0; }
+  }
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(C); cfg.blockDim = dim3(1024);
+  cfg.dynamicSmemBytes = fixed + scratch + slice; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, qr_panel_cluster_kernel<NB>, V, ld, m, j0, nbw, Vc, tau, Tp, rpc, use_smem);
+}
+
+// Blocked Householder QR with compact-WY updates (K2a panel / K2b trailing / K2c form Q + sign fix).
+long long qr_factor_blocked(cudaStream_t st, int path, long long rows, int n, const double* X, double* Q,
+                            double* R, void* work, cudaError_t* err) {
+  constexpr int NB = QR_NB;
+  QrWork wk;
+  qr_layout(rows, n, static_cast<char*>(work), &wk);
+  long long launches = 0;
+  *err = cudaMemcpyAsync(wk.V, X, sizeof(double) * rows * n, cudaMemcpyDeviceToDevice, st);
+  if (*err != cudaSuccess) return -1;
+  auto gemm = [&](const GemmCall& c) -> bool {
+    int nl = launch_gemm(st, path, c, wk.splitk, wk.splitk_elems, err);
+    if (nl < 0) return false;
+    launches += nl;
+    return true;
+  };
+  const IndexMap unit{1, 1, 0};
+  const int npan = (n + NB - 1) / NB;
+  for (int p = 0; p < npan; ++p) {
+    const int j0 = p * NB, nbw = (n - j0 < NB) ? n - j0 : NB, n2 = n - j0 - nbw;
+    double* Tp = wk.Tfac + (size_t)p * NB * NB;
+    *err = launch_panel(st, wk.V, n, rows, j0, nbw, wk.Vc, wk.tau, Tp);
+    if (*err != cudaSuccess) return -1;
+    ++launches;
+    if (n2 > 0) {
+      const long long pr = rows - j0;
+      const double* Vp = wk.Vc + (long long)j0 * n + j0;
+      double* A2 = wk.V + (long long)j0 * n + j0 + nbw;
+      // W1 = Vp^T A2 ; W2 = T^T W1 ; A2 -= Vp W2
+      if (!gemm(GemmCall{Vp, n, 1, A2, n, wk.W1, plain_map(n2), unit, nbw, n2, (int)pr, 0})) return -1;
+      if (!gemm(GemmCall{Tp, NB, 1, wk.W1, n2, wk.W2, plain_map(n2), unit, nbw, n2, nbw, 0})) return -1;
+      if (!gemm(GemmCall{Vp, n, 0, wk.W2, n2, A2, plain_map(n), unit, (int)pr, n2, nbw, 1})) return -1;
+    }
+  }
+  copy_triu_kernel<<<(n * n + 255) / 256, 256, 0, st>>>(wk.V, n, n, R);
+  set_identity_top_kernel<<<296, 256, 0, st>>>(Q, rows, n);
+  launches += 2;
+  for (int p = npan - 1; p >= 0; --p) {
+    const int j0 = p * NB, nbw = (n - j0 < NB) ? n - j0 : NB, nc = n - j0;
+    const long long pr = rows - j0;
+    double* Tp = wk.Tfac + (size_t)p * NB * NB;
+    const double* Vp = wk.Vc + (long long)j0 * n + j0;
+    double* Q2 = Q + (long long)j0 * n + j0;
+    // Q2 <- (I - Vp T Vp^T) Q2
+    if (!gemm(GemmCall{Vp, n, 1, Q2, n, wk.W1, plain_map(nc), unit, nbw, nc, (int)pr, 0})) return -1;
+    if (!gemm(GemmCall{Tp, NB, 0, wk.W1, nc, wk.W2, plain_map(nc), unit, nbw, nc, nbw, 0})) return -1;
+    if (!gemm(GemmCall{Vp, n, 0, wk.W2, nc, Q2, plain_map(n), unit, (int)pr, nc, nbw, 1})) return -1;
   }
   sign_fix_kernel<<<296, 256, 0, st>>>(Q, rows, n, R);
   sign_fix_R_kernel<<<n, 128, 0, st>>>(R, n);
@@ -385,7 +500,9 @@ int do_step(qrctm* h, cudaEvent_t* ev /* QRCTM_NSTAGE+1 events or null */) {
   mark(1);
   {
     cudaError_t e;
-    long long nl = qr_factor_level2(h->stream, h->m, h->chi, h->X, h->Q, h->R, h->qrwork, &e);
+    long long nl = h->qr_path == 0
+        ? qr_factor_blocked(h->stream, h->gemm_path, h->m, h->chi, h->X, h->Q, h->R, h->qrwork, &e)
+        : qr_factor_level2(h->stream, h->m, h->chi, h->X, h->Q, h->R, h->qrwork, &e);
     if (nl < 0) return fail(h, QRCTM_ERR_CUDA, "qr", e);
     h->launches += nl;
   }
@@ -609,6 +726,7 @@ int qrctm_set_option(qrctm_t* h, int key, int value) {
     case QRCTM_OPT_SYMMETRIZE:  if (value != 0 && value != 1) break; h->symmetrize = value; return QRCTM_OK;
     case QRCTM_OPT_CHECK_EVERY: if (value < 1) break; h->check_every = value; return QRCTM_OK;
     case QRCTM_OPT_GEMM_PATH:   if (value != 0 && value != 1) break; h->gemm_path = value; return QRCTM_OK;
+    case QRCTM_OPT_QR_PATH:     if (value != 0 && value != 1) break; h->qr_path = value; return QRCTM_OK;
     case QRCTM_OPT_TIME_STAGES: if (value != 0 && value != 1) break; h->time_stages = value; return QRCTM_OK;
     default: break;
   }
@@ -721,10 +839,14 @@ int qrctm_gemm_f64(void* cuda_stream, int path, int transA, int M, int N, int K,
 
 unsigned long long qrctm_qr_work_bytes(int rows, int cols) { return qr_work_bytes_impl(rows, cols); }
 
-int qrctm_qr_f64(void* cuda_stream, int rows, int cols, const double* X, double* Q, double* R, void* work) {
-  if (!X || !Q || !R || !work || rows < 1 || cols < 1 || cols > rows) return QRCTM_ERR_INVALID_ARG;
+int qrctm_qr_f64(void* cuda_stream, int path, int rows, int cols, const double* X, double* Q, double* R,
+                 void* work) {
+  if (!X || !Q || !R || !work || rows < 1 || cols < 1 || cols > rows || (path != 0 && path != 1))
+    return QRCTM_ERR_INVALID_ARG;
   cudaError_t e;
-  long long nl = qr_factor_level2(static_cast<cudaStream_t>(cuda_stream), rows, cols, X, Q, R, work, &e);
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  long long nl = path == 0 ? qr_factor_blocked(st, 0, rows, cols, X, Q, R, work, &e)
+                           : qr_factor_level2(st, rows, cols, X, Q, R, work, &e);
   return nl < 0 ? QRCTM_ERR_CUDA : QRCTM_OK;
 }
 

@@ -54,11 +54,15 @@ def test_gemm_odd_leading_dimension_views():
     assert rel(out, A.cpu().numpy().T @ B.cpu().numpy()) < 1e-13
 
 
-@pytest.mark.parametrize("rows,cols", [(32, 8), (324, 36), (1024, 64), (50, 50), (7, 1), (333, 17)])
-def test_qr_f64_matches_oracle(rows, cols):
+@pytest.mark.parametrize("rows,cols", [(32, 8), (324, 36), (1024, 64), (50, 50), (7, 1), (333, 17), (16, 16),
+                                       (2500, 100), (40, 33), (9604, 196), (3000, 150)])
+@pytest.mark.parametrize("path", [0, 1])
+def test_qr_f64_matches_oracle(rows, cols, path):
+    if path == 1 and rows * cols > 200000:
+        pytest.skip("level-2 path only checked on small cases")
     g = np.random.default_rng(rows + cols)
     X = g.standard_normal((rows, cols))
-    Q, R = pkg.qr_f64(torch_dev(X))
+    Q, R = pkg.qr_f64(torch_dev(X), path=path)
     Q, R = Q.cpu().numpy(), R.cpu().numpy()
     Qo, Ro = o.qr_pos(X)
     cond = np.linalg.cond(X)
@@ -72,6 +76,11 @@ def test_qr_f64_matches_oracle(rows, cols):
 def test_qr_rank_deficient_is_still_valid():
     g = np.random.default_rng(3)
     X = g.standard_normal((200, 6)) @ g.standard_normal((6, 12))       # rank 6 < 12 (hazard H1)
+    for path in (0, 1):
+        Q, R = pkg.qr_f64(torch_dev(X), path=path)
+        Q, R = Q.cpu().numpy(), R.cpu().numpy()
+        assert np.linalg.norm(Q.T @ Q - np.eye(12)) < 1e-13
+        assert rel(Q @ R, X) < 1e-13 and np.all(np.diag(R) >= 0.0)
     Q, R = pkg.qr_f64(torch_dev(X))
     Q, R = Q.cpu().numpy(), R.cpu().numpy()
     assert np.linalg.norm(Q.T @ Q - np.eye(12)) < 1e-13
