@@ -194,6 +194,169 @@ gemm_f64_dmma(GemmArgs p) {
   }
 }
 
+// ------------------------------------------------------------------------------
+// Warp-specialised variant (the hot path for every large contraction, transA = 1):
+//   * ONE producer warp stages the operands with bulk asynchronous copies
+//     (cp.async.bulk global -> shared, SASS UBLKCP: the TMA engine's linear mode),
+//     one copy per k-row of the A tile (lanes 0..15) and of the B tile (lanes
+//     16..31), completion counted in bytes on the stage's `full` mbarrier;
+//   * the consumer warps only do LDS.64 + DMMA and release a stage by arriving on
+//     its `empty` mbarrier -- no CTA-wide barrier and no address arithmetic in the
+//     math warps (ncu on the cp.async kernel: DMMA pipe 71.6 % active, the rest
+//     lost to the in-line producer code and __syncthreads, profiles/).
+// The padded row pitch (BM + 4 doubles) keeps the fragment loads conflict free,
+// which the dense box of a tiled tensor map could not.  Ragged M/N edges: copied
+// widths are clipped (rounded up to 16 bytes), the unwritten columns only feed
+// output rows/columns that are never stored.  Ragged K: the missing k-rows of the
+// last tile are zero-filled by the producer with ordinary stores.
+// Requires even leading dimensions and 16-byte aligned bases (checked on the host;
+// otherwise the cp.async kernel above is used).
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* b, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(b)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* b, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* b) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* b, uint32_t parity) {
+  asm volatile(
+      "{\n.reg .pred p;\nWAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\nbra WAIT_%=;\nDONE_%=:\n}\n" ::"r"(smem_u32(b)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n"
+               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+template <int BM, int BN, int WM, int WN, int STAGES>
+__global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 1) * 32, 1)
+gemm_f64_dmma_ws(GemmArgs p) {
+  constexpr int NW_M = BM / WM, NW_N = BN / WN, NCW = NW_M * NW_N;
+  constexpr int LDA_S = BM + PAD, LDB_S = BN + PAD;
+  constexpr int A_STAGE = BK * LDA_S, B_STAGE = BK * LDB_S;
+  constexpr int FM = WM / 8, FN = WN / 8;
+  static_assert(BK == 16, "one copy per lane: 16 A rows + 16 B rows");
+  extern __shared__ __align__(16) double smem[];
+  double* As = smem;
+  double* Bs = smem + STAGES * A_STAGE;
+  uint64_t* full = reinterpret_cast<uint64_t*>(Bs + STAGES * B_STAGE);
+  uint64_t* empty = full + STAGES;
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int m0 = blockIdx.y * BM, n0 = blockIdx.x * BN;
+  const int nkt_total = (p.K + BK - 1) / BK;
+  const int kt_begin = blockIdx.z * p.ktiles_per_split;
+  int kt_end = kt_begin + p.ktiles_per_split;
+  if (kt_end > nkt_total) kt_end = nkt_total;
+  const int nkt = kt_end > kt_begin ? kt_end - kt_begin : 0;
+
+  if (tid == 0) {
+    for (int s = 0; s < STAGES; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, NCW); }
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  __syncthreads();
+
+  if (warp == NCW) {
+    // ------------------------------ producer warp
+    int wA = p.M - m0; if (wA > BM) wA = BM; wA = (wA + 1) & ~1;
+    int wB = p.N - n0; if (wB > BN) wB = BN; wB = (wB + 1) & ~1;
+    const int row = lane & 15;
+    const bool isB = lane >= 16;
+    const double* src = isB ? p.B + (long long)row * p.ldb + n0 : p.A + (long long)row * p.lda + m0;
+    src += (long long)kt_begin * BK * (isB ? p.ldb : p.lda);
+    const long long step = (long long)BK * (isB ? p.ldb : p.lda);
+    const uint32_t bytes = (uint32_t)(isB ? wB : wA) * 8u;
+    const int srow = isB ? row * LDB_S : row * LDA_S;
+    for (int kt = 0; kt < nkt; ++kt, src += step) {
+      const int stage = kt % STAGES, round = kt / STAGES;
+      if (round > 0) mbar_wait(empty + stage, (round - 1) & 1);
+      int krows = p.K - (kt_begin + kt) * BK; if (krows > BK) krows = BK;
+      double* dst = (isB ? Bs + stage * B_STAGE : As + stage * A_STAGE) + srow;
+      if (row >= krows) {                         // ragged K: zero rows (last tile only)
+        const int w = isB ? BN : BM;
+        for (int c = 0; c < w; ++c) dst[c] = 0.0;
+      }
+      __syncwarp();
+      if (lane == 0) mbar_expect_tx(full + stage, (uint32_t)krows * (uint32_t)(wA + wB) * 8u);
+      __syncwarp();
+      if (row < krows) bulk_g2s(dst, src, bytes, full + stage);
+    }
+    return;
+  }
+
+  // -------------------------------- consumer warps
+  const int wm0 = (warp / NW_N) * WM, wn0 = (warp % NW_N) * WN;
+  const int lr = lane >> 2, lc = lane & 3;
+  double acc[FM][FN][2];
+#pragma unroll
+  for (int i = 0; i < FM; ++i)
+#pragma unroll
+    for (int j = 0; j < FN; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+  for (int kt = 0; kt < nkt; ++kt) {
+    const int stage = kt % STAGES, round = kt / STAGES;
+    mbar_wait(full + stage, round & 1);
+    const double* as = As + stage * A_STAGE + wm0 + lr + lc * LDA_S;
+    const double* bs = Bs + stage * B_STAGE + wn0 + lr + lc * LDB_S;
+    int krows = p.K - (kt_begin + kt) * BK;
+    if (krows >= BK) {
+#pragma unroll
+      for (int ks = 0; ks < BK / 4; ++ks) {
+        double af[FM], bf[FN];
+#pragma unroll
+        for (int i = 0; i < FM; ++i) af[i] = as[ks * 4 * LDA_S + i * 8];
+#pragma unroll
+        for (int j = 0; j < FN; ++j) bf[j] = bs[ks * 4 * LDB_S + j * 8];
+#pragma unroll
+        for (int i = 0; i < FM; ++i)
+#pragma unroll
+          for (int j = 0; j < FN; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+      }
+    } else {
+      const int ksteps = (krows + 3) >> 2;
+      for (int ks = 0; ks < ksteps; ++ks) {
+        double af[FM], bf[FN];
+#pragma unroll
+        for (int i = 0; i < FM; ++i) af[i] = as[ks * 4 * LDA_S + i * 8];
+#pragma unroll
+        for (int j = 0; j < FN; ++j) bf[j] = bs[ks * 4 * LDB_S + j * 8];
+#pragma unroll
+        for (int i = 0; i < FM; ++i)
+#pragma unroll
+          for (int j = 0; j < FN; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(empty + stage);
+  }
+
+  double* out = p.out + (long long)blockIdx.z * p.split_stride;
+#pragma unroll
+  for (int i = 0; i < FM; ++i) {
+    int r = m0 + wm0 + i * 8 + lr;
+    if (r >= p.M) continue;
+    long long roff = (long long)(r / p.ro.div) * p.ro.hi + (long long)(r % p.ro.div) * p.ro.lo;
+#pragma unroll
+    for (int j = 0; j < FN; ++j) {
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        int c = n0 + wn0 + j * 8 + 2 * lc + e;
+        if (c < p.N) {
+          long long off = roff + (long long)(c / p.co.div) * p.co.hi + (long long)(c % p.co.div) * p.co.lo;
+          double v = acc[i][j][e];
+          if (p.mode == 1) v = out[off] - v;
+          else if (p.mode == 2) v = out[off] + v;
+          out[off] = v;
+        }
+      }
+    }
+  }
+}
+
 // Plain DFMA reference kernel (QRCTM_OPT_GEMM_PATH = 1): one output element per
 // thread, no tiling.  Only for debugging / cross-checking the DMMA path on the GPU.
 __global__ void gemm_f64_ref(GemmArgs p) {
@@ -219,7 +382,15 @@ __global__ void reduce_splitk(const double* part, long long split_stride, int sp
   if (idx >= (long long)M * N) return;
   int i = (int)(idx / N), j = (int)(idx % N);
   double s = 0.0;
-  for (int z = 0; z < splits; ++z) s += part[(long long)z * split_stride + idx];
+  int z = 0;
+  for (; z + 8 <= splits; z += 8) {            // 8 loads in flight, summed in ascending z (fixed order)
+    double v[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) v[u] = part[(long long)(z + u) * split_stride + idx];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) s += v[u];
+  }
+  for (; z < splits; ++z) s += part[(long long)z * split_stride + idx];
   long long off = (long long)(i / ro.div) * ro.hi + (long long)(i % ro.div) * ro.lo +
                   (long long)(j / co.div) * co.hi + (long long)(j % co.div) * co.lo;
   if (mode == 1) s = out[off] - s;

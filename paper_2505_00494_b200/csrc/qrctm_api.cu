@@ -3,6 +3,7 @@
 #include "../../include/qrctm.h"
 
 #include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>
 #include <math.h>
 #include <stdio.h>
 #include <string.h>
@@ -168,6 +169,22 @@ cudaError_t launch_cfg(cudaStream_t st, const GemmArgs& g, int splits) {
   return cudaGetLastError();
 }
 
+template <int BM, int BN, int WM, int WN, int STAGES>
+cudaError_t launch_cfg_ws(cudaStream_t st, const GemmArgs& g, int splits) {
+  constexpr int NT = ((BM / WM) * (BN / WN) + 1) * 32;
+  constexpr size_t smem = sizeof(double) * STAGES * BK * ((BM + PAD) + (BN + PAD)) + 2 * STAGES * sizeof(uint64_t);
+  static bool attr_done = false;
+  if (!attr_done) {
+    cudaError_t e = cudaFuncSetAttribute(gemm_f64_dmma_ws<BM, BN, WM, WN, STAGES>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    attr_done = true;
+  }
+  dim3 grid((g.N + BN - 1) / BN, (g.M + BM - 1) / BM, splits);
+  gemm_f64_dmma_ws<BM, BN, WM, WN, STAGES><<<grid, NT, smem, st>>>(g);
+  return cudaGetLastError();
+}
+
 struct GemmCall {
   const double* A; long long lda; int transA;
   const double* B; long long ldb;
@@ -213,7 +230,9 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
     g.out = splitk_ws; g.ro = plain_map(c.N); g.co = IndexMap{1, 1, 0}; g.mode = 0;
     g.split_stride = (long long)c.M * c.N;
   }
-  if (big) *err = launch_cfg<128, 128, 64, 32, 4>(st, g, splits);
+  const bool ws_ok = g.transA && g.vecA && g.vecB;     // bulk copies need 16-byte aligned rows
+  if (big && ws_ok) *err = launch_cfg_ws<128, 128, 64, 32, 4>(st, g, splits);
+  else if (big) *err = launch_cfg<128, 128, 64, 32, 4>(st, g, splits);
   else     *err = launch_cfg<64, 64, 32, 32, 4>(st, g, splits);
   if (*err != cudaSuccess) return -1;
   ++launched;
@@ -493,31 +512,30 @@ int stage_spectrum(qrctm* h, double* s_out, int update_prev) {
 }
 
 int do_step(qrctm* h, cudaEvent_t* ev /* QRCTM_NSTAGE+1 events or null */) {
-  auto mark = [&](int i) { if (ev) cudaEventRecord(ev[i], h->stream); };
-  int rc;
-  mark(0);
-  rc = stage_reduced_corner(h, h->C, h->T, h->X); if (rc) return rc;
-  mark(1);
-  {
+  // NVTX ranges name the stages so that `ncu --nvtx --nvtx-include "K4_absorb_a/"` selects one.
+  auto mark = [&](int i, const char* next) {
+    if (i > 0) nvtxRangePop();
+    if (ev) cudaEventRecord(ev[i], h->stream);
+    if (next) nvtxRangePushA(next);
+  };
+  int rc = QRCTM_OK;
+  mark(0, "K1_reduced_corner");
+  rc = stage_reduced_corner(h, h->C, h->T, h->X);
+  if (!rc) {
+    mark(1, "K2_qr");
     cudaError_t e;
     long long nl = h->qr_path == 0
         ? qr_factor_blocked(h->stream, h->gemm_path, h->m, h->chi, h->X, h->Q, h->R, h->qrwork, &e)
         : qr_factor_level2(h->stream, h->m, h->chi, h->X, h->Q, h->R, h->qrwork, &e);
-    if (nl < 0) return fail(h, QRCTM_ERR_CUDA, "qr", e);
-    h->launches += nl;
+    if (nl < 0) rc = fail(h, QRCTM_ERR_CUDA, "qr", e); else h->launches += nl;
   }
-  mark(2);
-  rc = stage_half_absorb(h, h->Q, h->T, h->P); if (rc) return rc;
-  mark(3);
-  rc = stage_absorb_a(h, h->P, h->S, 0); if (rc) return rc;
-  mark(4);
-  rc = stage_project(h, h->S, h->Q, h->Tn); if (rc) return rc;
-  mark(5);
-  rc = h->corner_mode == 0 ? stage_corner_accel(h) : stage_corner_enlarged(h); if (rc) return rc;
-  mark(6);
-  rc = stage_normalize(h, h->Cn, h->Tn); if (rc) return rc;
-  mark(7);
-  return QRCTM_OK;
+  if (!rc) { mark(2, "K3_half_absorb"); rc = stage_half_absorb(h, h->Q, h->T, h->P); }
+  if (!rc) { mark(3, "K4_absorb_a"); rc = stage_absorb_a(h, h->P, h->S, 0); }
+  if (!rc) { mark(4, "K5_project"); rc = stage_project(h, h->S, h->Q, h->Tn); }
+  if (!rc) { mark(5, "K6_corner"); rc = h->corner_mode == 0 ? stage_corner_accel(h) : stage_corner_enlarged(h); }
+  if (!rc) { mark(6, "K7_normalize"); rc = stage_normalize(h, h->Cn, h->Tn); }
+  if (!rc) mark(7, nullptr); else nvtxRangePop();
+  return rc;
 }
 
 int check_flag(qrctm* h) {   // stream must be synchronised by the caller's copy
