@@ -96,40 +96,42 @@ __global__ void house_apply_kernel(const double* __restrict__ V, long long ldv, 
 // Column k is left unscaled until write-back so nobody races on it.
 // Afterwards the Gram matrix of the unit-lower-trapezoidal reflectors gives the
 // compact-WY factor T (forward larft recurrence), written to Tp[NB][NB].
-template <int NB>
+template <int NB, bool SMEM>
 __global__ void __launch_bounds__(1024, 1)
 qr_panel_cluster_kernel(double* __restrict__ V, long long ld, long long m, int j0, int nbw,
                         double* __restrict__ Vc, double* __restrict__ tau, double* __restrict__ Tp,
-                        long long rpc, int use_smem) {
+                        long long rpc) {
   namespace cg = cooperative_groups;
   cg::cluster_group cluster = cg::this_cluster();
   const int C = (int)cluster.num_blocks();
   const int rank = (int)cluster.block_rank();
-  constexpr int NT = 1024, NRG = NT / NB, NW = NT / 32;
+  constexpr int NT = 1024, NRG = NT / NB, NW = NT / 32, NP = NB * NB, NQ = NT / NP > 0 ? NT / NP : 1;
   extern __shared__ __align__(16) double sm[];
-  // layout: exch[2][Cmax=16][NB] | rowv[2][NB] | red[NW][NB] | par[3][NB] (scale,beta,tau) | G[NB*NB] |
-  //         exchG[16][NB*NB] (rank 0 uses) | slice
+  // exch[2][16][NB] | rowv[2][NB] | red[NW][NB] | par[3][NB] (scale,beta,tau) | wv[NB+1] | G[NP] |
+  // exchG[16][NP] | scratch[NQ*NP] | slice
   double* exch = sm;
   double* rowv = exch + 2 * 16 * NB;
   double* red = rowv + 2 * NB;
   double* par = red + NW * NB;
-  double* Gs = par + 3 * NB;
-  double* exchG = Gs + NB * NB;
-  double* slice = exchG + 16 * NB * NB;
+  double* wv = par + 3 * NB;
+  double* Gs = wv + NB + 2;
+  double* exchG = Gs + NP;
+  double* scratch = exchG + 16 * NP;
+  double* slice = scratch + NQ * NP;
 
   const int tid = threadIdx.x, col = tid % NB, rg = tid / NB, warp = tid >> 5, lane = tid & 31;
   const long long row_lo = (long long)j0 + (long long)rank * rpc;
   long long row_hi = row_lo + rpc; if (row_hi > m) row_hi = m;
   const int nloc = row_hi > row_lo ? (int)(row_hi - row_lo) : 0;
-  double* pan; long long ldp;
-  if (use_smem) {
-    pan = slice; ldp = NB;
+  // pan(li, c): shared slice with pitch NB, or the matrix itself in global memory / L2
+  double* const gpan = V + row_lo * ld + j0;
+  const long long LD = SMEM ? NB : ld;
+  double* const pan = SMEM ? slice : gpan;
+  if (SMEM) {
     for (int idx = tid; idx < nloc * NB; idx += NT) {
       int li = idx / NB, c = idx % NB;
-      slice[idx] = c < nbw ? V[(row_lo + li) * ld + j0 + c] : 0.0;
+      slice[idx] = c < nbw ? gpan[(long long)li * ld + c] : 0.0;
     }
-  } else {
-    pan = V + row_lo * ld + j0; ldp = ld;
   }
   __syncthreads();
   cluster.sync();          // every CTA of the cluster is resident before the first DSMEM store
@@ -137,20 +139,31 @@ qr_panel_cluster_kernel(double* __restrict__ V, long long ld, long long m, int j
   int buf = 0;
   for (int k = 0; k < nbw; ++k) {
     const long long r = (long long)j0 + k;
+    long long lo64 = r + 1 - row_lo; if (lo64 < 0) lo64 = 0; if (lo64 > nloc) lo64 = nloc;
+    const int lo = (int)lo64;                                   // first local row strictly below the diagonal
+    const int li0 = lo <= rg ? rg : rg + ((lo - rg + NRG - 1) / NRG) * NRG;
+    const bool owner = (r >= row_lo && r < row_hi);
     double acc = 0.0;
     if (col >= k && col < nbw) {
-      for (int li = rg; li < nloc; li += NRG) {
-        if (row_lo + li > r) acc = fma(pan[li * ldp + k], pan[li * ldp + col], acc);
+      const double* pk = pan + (long long)li0 * LD + k;
+      const double* pc = pan + (long long)li0 * LD + col;
+      double a0 = 0.0, a1 = 0.0;
+      int li = li0;
+      for (; li + NRG < nloc; li += 2 * NRG, pk += 2 * NRG * LD, pc += 2 * NRG * LD) {
+        a0 = fma(pk[0], pc[0], a0);
+        a1 = fma(pk[NRG * LD], pc[NRG * LD], a1);
       }
+      if (li < nloc) a0 = fma(pk[0], pc[0], a0);
+      acc = a0 + a1;
     }
     if (NB == 16) acc += __shfl_xor_sync(0xffffffffu, acc, 16);
-    if (lane < NB) red[warp * NB + lane] = acc;      // NB == 32: every lane; NB == 16: lanes 0..15
+    if (lane < NB) red[warp * NB + lane] = acc;
     __syncthreads();
     if (tid < NB) {
       double g = 0.0;
+#pragma unroll
       for (int w = 0; w < NW; ++w) g += red[w * NB + tid];
-      const bool owner = (r >= row_lo && r < row_hi);
-      double rv = owner ? pan[(r - row_lo) * ldp + tid] : 0.0;
+      double rv = owner ? pan[(r - row_lo) * LD + tid] : 0.0;
       for (int q = 0; q < C; ++q) {
         double* rex = cluster.map_shared_rank(exch, q);
         rex[(buf * 16 + rank) * NB + tid] = g;
@@ -158,59 +171,65 @@ qr_panel_cluster_kernel(double* __restrict__ V, long long ld, long long m, int j
       }
     }
     cluster.sync();
-    double gk = 0.0, gj = 0.0;
-    for (int q = 0; q < C; ++q) { gk += exch[(buf * 16 + q) * NB + k]; gj += exch[(buf * 16 + q) * NB + col]; }
-    const double alpha = rowv[buf * NB + k], yrj = rowv[buf * NB + col];
-    double tk = 0.0, scale = 0.0, beta = alpha;
-    if (gk > 0.0) {
-      double sigma = sqrt(fma(alpha, alpha, gk));
-      beta = alpha >= 0.0 ? -sigma : sigma;
-      tk = (beta - alpha) / beta;
-      scale = 1.0 / (alpha - beta);
-    }
-    if (tid == 0) { par[k] = scale; par[NB + k] = beta; par[2 * NB + k] = tk; }
-    if (col > k && col < nbw && tk != 0.0) {
-      const double w = tk * fma(scale, gj, yrj);
-      for (int li = rg; li < nloc; li += NRG) {
-        long long gi = row_lo + li;
-        if (gi > r) pan[li * ldp + col] = fma(-(pan[li * ldp + k] * scale), w, pan[li * ldp + col]);
-        else if (gi == r) pan[li * ldp + col] -= w;
+    if (tid < NB) {
+      double gk = 0.0, gj = 0.0;
+      for (int q = 0; q < C; ++q) { gk += exch[(buf * 16 + q) * NB + k]; gj += exch[(buf * 16 + q) * NB + tid]; }
+      const double alpha = rowv[buf * NB + k], yrj = rowv[buf * NB + tid];
+      double tk = 0.0, scale = 0.0, beta = alpha;
+      if (gk > 0.0) {
+        double sigma = sqrt(fma(alpha, alpha, gk));
+        beta = alpha >= 0.0 ? -sigma : sigma;
+        tk = (beta - alpha) / beta;
+        scale = 1.0 / (alpha - beta);
       }
+      wv[tid] = tk * fma(scale, gj, yrj);
+      if (tid == 0) { par[k] = scale; par[NB + k] = beta; par[2 * NB + k] = tk; wv[NB] = scale; wv[NB + 1] = tk; }
+    }
+    __syncthreads();
+    const double tk = wv[NB + 1];
+    if (col > k && col < nbw && tk != 0.0) {
+      const double w = wv[col], scale = wv[NB];
+      const double* pk = pan + (long long)li0 * LD + k;
+      double* pc = pan + (long long)li0 * LD + col;
+      for (int li = li0; li < nloc; li += NRG, pk += NRG * LD, pc += NRG * LD)
+        pc[0] = fma(-(pk[0] * scale), w, pc[0]);
+      if (owner && rg == 0) pan[(r - row_lo) * LD + col] -= w;
     }
     __syncthreads();
     buf ^= 1;
   }
 
   // write-back: in-place factor (R above/on the diagonal, scaled v below), clean reflectors Vc
+  double* const gvc = Vc + row_lo * ld + j0;
   for (int idx = tid; idx < nloc * NB; idx += NT) {
     int li = idx / NB, c = idx % NB;
     if (c >= nbw) continue;
     long long gi = row_lo + li, rc = (long long)j0 + c;
-    double x = pan[li * ldp + c], vout, vclean;
+    double x = pan[(long long)li * LD + c], vout, vclean;
     if (gi > rc) { vclean = x * par[c]; vout = vclean; }
     else if (gi == rc) { vclean = 1.0; vout = par[NB + c]; }
     else { vclean = 0.0; vout = x; }
-    V[gi * ld + j0 + c] = vout;
-    Vc[gi * ld + j0 + c] = vclean;
-    if (use_smem) slice[idx] = vclean;
+    gpan[(long long)li * ld + c] = vout;
+    gvc[(long long)li * ld + c] = vclean;
+    if (SMEM) slice[idx] = vclean;
   }
   if (rank == 0 && tid < nbw) tau[j0 + tid] = par[2 * NB + tid];
   __syncthreads();
 
   // Gram of the clean reflectors (strict upper part is what larft needs)
   {
-    constexpr int NP = NB * NB, NQ = NT / NP > 0 ? NT / NP : 1;   // NB=16: 256 pairs x 4 row subsets
     const int pidx = tid % NP, a = pidx / NB, c = pidx % NB, qs = tid / NP;
-    double g = 0.0;
-    const double* gsrc = use_smem ? slice : Vc + row_lo * ld + j0;
-    const long long gld = use_smem ? NB : ld;
+    const double* gsrc = SMEM ? slice : gvc;
+    double g0 = 0.0, g1 = 0.0;
     if (tid < NP * NQ && a < c && c < nbw) {
-      for (int li = qs; li < nloc; li += NQ) g = fma(gsrc[li * gld + a], gsrc[li * gld + c], g);
+      int li = qs;
+      for (; li + NQ < nloc; li += 2 * NQ) {
+        g0 = fma(gsrc[(long long)li * LD + a], gsrc[(long long)li * LD + c], g0);
+        g1 = fma(gsrc[(long long)(li + NQ) * LD + a], gsrc[(long long)(li + NQ) * LD + c], g1);
+      }
+      if (li < nloc) g0 = fma(gsrc[(long long)li * LD + a], gsrc[(long long)li * LD + c], g0);
     }
-    // reduce the NQ row subsets through scratch behind the slice (exchG receives remote writes)
-    __syncthreads();
-    double* scratch = slice + (use_smem ? (size_t)rpc * NB : 0);    // NQ*NP doubles reserved by the host
-    if (tid < NP * NQ) scratch[qs * NP + pidx] = g;
+    if (tid < NP * NQ) scratch[qs * NP + pidx] = g0 + g1;
     __syncthreads();
     if (tid < NP) {
       double t = 0.0;
@@ -221,7 +240,6 @@ qr_panel_cluster_kernel(double* __restrict__ V, long long ld, long long m, int j
   }
   cluster.sync();
   if (rank == 0) {
-    constexpr int NP = NB * NB;
     if (tid < NP) {
       double t = 0.0;
       for (int q = 0; q < C; ++q) t += exchG[q * NP + tid];
@@ -249,6 +267,306 @@ qr_panel_cluster_kernel(double* __restrict__ V, long long ld, long long m, int j
       }
 #pragma unroll
       for (int i = 0; i < NB; ++i) Tp[a * NB + i] = Trow[i];
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------
+// Register-resident panel kernel (default path).  Same algorithm as above, but
+// every thread keeps its RPT rows of its column in REGISTERS and column k is
+// broadcast inside the (half-)warp with shuffles, so a column step costs no
+// shared-memory traffic for the panel itself (the shared-memory version is bound
+// by the 128 B/clk LDS bandwidth: ncu, profiles/).  All NB lanes take part in the
+// dot products: lanes j >= k give the reflector/update terms g_j, lanes a < k give
+// h_a = sum_{i>r} x_a[i] x_k[i], from which the Gram entries of the compact-WY
+// recurrence follow at no extra pass:
+//     G[a][k] = v_a^T v_k = scale_a (scale_k h_a + x_a[r]),
+//     T[a][k] = -tau_k sum_{c=a}^{k-1} T[a][c] G[c][k],  T[k][k] = tau_k.
+// Thread layout: col = tid % NB, row group rg = tid / NB, local rows rg + t*NRG.
+template <int NB, int NT, int RPT>
+__global__ void __launch_bounds__(NT, 1)
+qr_panel_reg_kernel(double* __restrict__ V, long long ld, long long m, int j0, int nbw,
+                    double* __restrict__ Vc, double* __restrict__ tau, double* __restrict__ Tp, long long rpc) {
+  namespace cg = cooperative_groups;
+  cg::cluster_group cluster = cg::this_cluster();
+  const int C = (int)cluster.num_blocks();
+  const int rank = (int)cluster.block_rank();
+  constexpr int NRG = NT / NB, NW = NT / 32;
+  __shared__ double exch[2 * 16 * NB];
+  __shared__ double rowv[2 * NB];
+  __shared__ double red[NW * NB];
+  __shared__ double par[3 * NB];          // scale, beta, tau per column
+  __shared__ double wv[NB + 2];
+  __shared__ double Gcol[NB];
+  __shared__ double Ts[NB * NB];
+
+  const int tid = threadIdx.x, col = tid % NB, rg = tid / NB, warp = tid >> 5, lane = tid & 31;
+  const int lane_base = lane & ~(NB - 1);
+  const long long row_lo = (long long)j0 + (long long)rank * rpc;
+  long long row_hi = row_lo + rpc; if (row_hi > m) row_hi = m;
+  const int nloc = row_hi > row_lo ? (int)(row_hi - row_lo) : 0;
+  double* const gpan = V + row_lo * ld + j0;
+
+  double val[RPT];
+#pragma unroll
+  for (int t = 0; t < RPT; ++t) {
+    const int li = rg + t * NRG;
+    val[t] = (li < nloc && col < nbw) ? gpan[(long long)li * ld + col] : 0.0;
+  }
+  for (int i = tid; i < NB * NB; i += NT) Ts[i] = 0.0;
+  __syncthreads();
+  cluster.sync();
+
+  int buf = 0;
+  for (int k = 0; k < nbw; ++k) {
+    const long long r = (long long)j0 + k;
+    long long lo64 = r + 1 - row_lo; if (lo64 < 0) lo64 = 0; if (lo64 > nloc) lo64 = nloc;
+    const int lo = (int)lo64;
+    const int t0 = lo <= rg ? 0 : (lo - rg + NRG - 1) / NRG;        // first t with row strictly below r
+    const bool owner = (r >= row_lo && r < row_hi);
+    const int lr_ = owner ? (int)(r - row_lo) : -1;
+    const bool mine = owner && (lr_ % NRG) == rg;                   // this thread holds row r of its column
+    const int tr = owner ? lr_ / NRG : -1;
+    double a0 = 0.0, a1 = 0.0, rvv = 0.0;
+    double xs[RPT];                                   // column k of my rows, broadcast once per step
+#pragma unroll
+    for (int t = 0; t < RPT; ++t) {
+      xs[t] = __shfl_sync(0xffffffffu, val[t], lane_base | k);
+      if (t >= t0) { if (t & 1) a1 = fma(xs[t], val[t], a1); else a0 = fma(xs[t], val[t], a0); }
+      if (mine && t == tr) rvv = val[t];
+    }
+    double acc = a0 + a1;
+    if (NB == 16) acc += __shfl_xor_sync(0xffffffffu, acc, 16);
+    if (lane < NB) red[warp * NB + lane] = acc;
+    __syncthreads();
+    if (tid < NB) {
+      double g = 0.0;
+#pragma unroll
+      for (int w = 0; w < NW; ++w) g += red[w * NB + tid];
+      for (int q = 0; q < C; ++q) {
+        double* rex = cluster.map_shared_rank(exch, q);
+        rex[(buf * 16 + rank) * NB + tid] = g;
+      }
+    }
+    if (mine) {
+      for (int q = 0; q < C; ++q) { double* rr = cluster.map_shared_rank(rowv, q); rr[buf * NB + col] = rvv; }
+    }
+    cluster.sync();
+    if (tid < NB) {
+      double gk = 0.0, gj = 0.0;
+      for (int q = 0; q < C; ++q) { gk += exch[(buf * 16 + q) * NB + k]; gj += exch[(buf * 16 + q) * NB + tid]; }
+      const double alpha = rowv[buf * NB + k], yrj = rowv[buf * NB + tid];
+      double tk = 0.0, scale = 0.0, beta = alpha;
+      if (gk > 0.0) {
+        double sigma = sqrt(fma(alpha, alpha, gk));
+        beta = alpha >= 0.0 ? -sigma : sigma;
+        tk = (beta - alpha) / beta;
+        scale = 1.0 / (alpha - beta);
+      }
+      if (tid > k) wv[tid] = tk * fma(scale, gj, yrj);
+      else if (tid < k) Gcol[tid] = par[tid] * fma(scale, gj, yrj);     // G[a][k], a = tid
+      if (tid == 0) { par[k] = scale; par[NB + k] = beta; par[2 * NB + k] = tk; wv[NB] = scale; wv[NB + 1] = tk; }
+    }
+    __syncthreads();
+    const double tk = wv[NB + 1];
+    if (tid < NB) {                                   // column k of T (every CTA keeps an identical copy)
+      if (tid == k) Ts[k * NB + k] = tk;
+      else if (tid < k) {
+        double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+        for (int c = 0; c < NB; c += 2) {
+          if (c >= tid && c < k) s0 = fma(Ts[tid * NB + c], Gcol[c], s0);
+          if (c + 1 >= tid && c + 1 < k) s1 = fma(Ts[tid * NB + c + 1], Gcol[c + 1], s1);
+        }
+        Ts[tid * NB + k] = -tk * (s0 + s1);
+      }
+    }
+    if (tk != 0.0) {
+      const bool upd = col > k && col < nbw;
+      const double w = upd ? wv[col] : 0.0, scale = wv[NB];
+      const double nsw = -scale * w;
+#pragma unroll
+      for (int t = 0; t < RPT; ++t) {
+        if (upd && t >= t0) val[t] = fma(xs[t], nsw, val[t]);
+        if (upd && mine && t == tr) val[t] -= w;
+      }
+    }
+    __syncthreads();
+    buf ^= 1;
+  }
+
+  double* const gvc = Vc + row_lo * ld + j0;
+  if (col < nbw) {
+    const double sc = par[col], be = par[NB + col];
+    const long long rc = (long long)j0 + col;
+#pragma unroll
+    for (int t = 0; t < RPT; ++t) {
+      const int li = rg + t * NRG;
+      if (li < nloc) {
+        const long long gi = row_lo + li;
+        double vout, vclean;
+        if (gi > rc) { vclean = val[t] * sc; vout = vclean; }
+        else if (gi == rc) { vclean = 1.0; vout = be; }
+        else { vclean = 0.0; vout = val[t]; }
+        gpan[(long long)li * ld + col] = vout;
+        gvc[(long long)li * ld + col] = vclean;
+      }
+    }
+  }
+  if (rank == 0) {
+    if (tid < nbw) tau[j0 + tid] = par[2 * NB + tid];
+    for (int i = tid; i < NB * NB; i += NT) Tp[i] = Ts[i];
+  }
+  cluster.sync();      // nobody exits while a peer may still address its shared memory
+}
+
+// ------------------------------------------------------------------------------
+// Applying a block reflector  Y <- (I - Vp op(T) Vp^T) Y  to Y = rows x nc (ld ldy):
+// three memory-bound kernels (intensity 2*NB flop per 16 bytes of Y, below the
+// FP64 ridge of ~5.7 flop/B even at NB = 32, so plain DFMA with coalesced row
+// streaming, not tensor tiles):
+//   wy_partial : part[cta][a][j] = sum_{i in chunk} Vp[i][a] Y[i][j]
+//   wy_reduce  : W2[a][j] = sum_k opT(a,k) sum_cta part[cta][k][j]      (fixed order)
+//   wy_update  : Y[i][j] -= sum_a Vp[i][a] W2[a][j]
+// One thread per column j (nc <= 4 * blockDim).
+template <int NB>
+__global__ void __launch_bounds__(256)
+wy_partial_kernel(const double* __restrict__ Vp, long long ldv, const double* __restrict__ Y, long long ldy,
+                  long long rows, int nc, int nbw, int chunk, double* __restrict__ part) {
+  __shared__ double vs[64 * NB];
+  const long long r0 = (long long)blockIdx.x * chunk;
+  long long r1 = r0 + chunk; if (r1 > rows) r1 = rows;
+  const int tid = threadIdx.x;
+  for (int j0c = 0; j0c < nc; j0c += 256) {
+    const int j = j0c + tid;
+    double acc[NB];
+#pragma unroll
+    for (int a = 0; a < NB; ++a) acc[a] = 0.0;
+    for (long long rb = r0; rb < r1; rb += 64) {
+      const int nr = (int)((r1 - rb) < 64 ? (r1 - rb) : 64);
+      __syncthreads();
+      for (int idx = tid; idx < nr * NB; idx += 256) {
+        int i = idx / NB, a = idx % NB;
+        vs[idx] = a < nbw ? Vp[(rb + i) * ldv + a] : 0.0;
+      }
+      __syncthreads();
+      if (j < nc) {
+        int i = 0;
+        for (; i + 4 <= nr; i += 4) {
+          double y0 = Y[(rb + i) * ldy + j], y1 = Y[(rb + i + 1) * ldy + j], y2 = Y[(rb + i + 2) * ldy + j],
+                 y3 = Y[(rb + i + 3) * ldy + j];
+#pragma unroll
+          for (int a = 0; a < NB; ++a) {
+            acc[a] = fma(vs[i * NB + a], y0, acc[a]);
+            acc[a] = fma(vs[(i + 1) * NB + a], y1, acc[a]);
+            acc[a] = fma(vs[(i + 2) * NB + a], y2, acc[a]);
+            acc[a] = fma(vs[(i + 3) * NB + a], y3, acc[a]);
+          }
+        }
+        for (; i < nr; ++i) {
+          double y0 = Y[(rb + i) * ldy + j];
+#pragma unroll
+          for (int a = 0; a < NB; ++a) acc[a] = fma(vs[i * NB + a], y0, acc[a]);
+        }
+      }
+    }
+    if (j < nc) {
+#pragma unroll
+      for (int a = 0; a < NB; ++a) part[((long long)blockIdx.x * NB + a) * nc + j] = acc[a];
+    }
+  }
+}
+
+// grid: ceil(nc / 4) blocks; block = 4 columns x NB rows k (= 4*NB elements) x NG part-groups.
+// Thread (e, g) sums the parts c == g (mod NG) of element e with coalesced loads, the NG
+// group sums are added in fixed order, then W2 = op(T) W1 for the block's 4 columns.
+template <int NB>
+__global__ void __launch_bounds__(1024)
+wy_reduce_kernel(const double* __restrict__ part, int nparts, int nc, int nbw, const double* __restrict__ Tp,
+                 int transT, double* __restrict__ W2) {
+  constexpr int NE = 4 * NB, NG = 1024 / NE;
+  __shared__ double gs[NG * NE];
+  __shared__ double w1[NE];
+  const int e = threadIdx.x % NE, g = threadIdx.x / NE;
+  const int k = e / 4, jj = e % 4, j = blockIdx.x * 4 + jj;
+  double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+  if (j < nc && k < nbw) {
+    const double* p = part + (long long)k * nc + j;
+    const long long st = (long long)NB * nc;
+    int c = g;
+    for (; c + 3 * NG < nparts; c += 4 * NG) {
+      double v0 = p[(long long)c * st], v1 = p[(long long)(c + NG) * st], v2 = p[(long long)(c + 2 * NG) * st],
+             v3 = p[(long long)(c + 3 * NG) * st];
+      s0 += v0; s1 += v1; s2 += v2; s3 += v3;
+    }
+    for (; c < nparts; c += NG) s0 += p[(long long)c * st];
+  }
+  gs[g * NE + e] = (s0 + s1) + (s2 + s3);
+  __syncthreads();
+  if (threadIdx.x < NE) {
+    double t = 0.0;
+#pragma unroll
+    for (int q = 0; q < NG; ++q) t += gs[q * NE + threadIdx.x];
+    w1[threadIdx.x] = t;
+  }
+  __syncthreads();
+  if (threadIdx.x < NE) {
+    const int a = k;                 // reuse the (k, jj) decomposition as (a, jj)
+    if (j < nc && a < nbw) {
+      double s = 0.0;
+      for (int kk = 0; kk < nbw; ++kk) {
+        const double t = transT ? Tp[kk * NB + a] : Tp[a * NB + kk];
+        s = fma(t, w1[kk * 4 + jj], s);
+      }
+      W2[(long long)a * nc + j] = s;
+    }
+  }
+}
+
+template <int NB>
+__global__ void __launch_bounds__(256)
+wy_update_kernel(const double* __restrict__ Vp, long long ldv, double* __restrict__ Y, long long ldy,
+                 long long rows, int nc, int nbw, int chunk, const double* __restrict__ W2) {
+  __shared__ double vs[64 * NB];
+  const long long r0 = (long long)blockIdx.x * chunk;
+  long long r1 = r0 + chunk; if (r1 > rows) r1 = rows;
+  const int tid = threadIdx.x;
+  for (int j0c = 0; j0c < nc; j0c += 256) {
+    const int j = j0c + tid;
+    double w[NB];
+#pragma unroll
+    for (int a = 0; a < NB; ++a) w[a] = (j < nc && a < nbw) ? W2[(long long)a * nc + j] : 0.0;
+    for (long long rb = r0; rb < r1; rb += 64) {
+      const int nr = (int)((r1 - rb) < 64 ? (r1 - rb) : 64);
+      __syncthreads();
+      for (int idx = tid; idx < nr * NB; idx += 256) {
+        int i = idx / NB, a = idx % NB;
+        vs[idx] = a < nbw ? Vp[(rb + i) * ldv + a] : 0.0;
+      }
+      __syncthreads();
+      if (j < nc) {
+        int i = 0;
+        for (; i + 4 <= nr; i += 4) {
+          double* y = Y + (rb + i) * ldy + j;
+          double y0 = y[0], y1 = y[ldy], y2 = y[2 * ldy], y3 = y[3 * ldy];
+          double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+#pragma unroll
+          for (int a = 0; a < NB; ++a) {
+            s0 = fma(vs[i * NB + a], w[a], s0);
+            s1 = fma(vs[(i + 1) * NB + a], w[a], s1);
+            s2 = fma(vs[(i + 2) * NB + a], w[a], s2);
+            s3 = fma(vs[(i + 3) * NB + a], w[a], s3);
+          }
+          y[0] = y0 - s0; y[ldy] = y1 - s1; y[2 * ldy] = y2 - s2; y[3 * ldy] = y3 - s3;
+        }
+        for (; i < nr; ++i) {
+          double* y = Y + (rb + i) * ldy + j;
+          double s0 = 0.0;
+#pragma unroll
+          for (int a = 0; a < NB; ++a) s0 = fma(vs[i * NB + a], w[a], s0);
+          y[0] -= s0;
+        }
+      }
     }
   }
 }

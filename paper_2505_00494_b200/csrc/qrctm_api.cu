@@ -252,10 +252,13 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
 // ------------------------------------------------------------------ K2: QR driver
 namespace {
 
-constexpr int QR_NB = 16;
+constexpr int QR_NB = 16;        // shared-memory / global panel kernel (fallback for very tall panels)
+constexpr int QR_NB_REG = 16;    // register-resident panel kernel (default)
+constexpr int QR_REG_NT = 512, QR_REG_RPT = 20;                       // 640 rows per CTA
+constexpr int QR_MAX_PARTS = 320;
 
 struct QrWork {     // carved out of the caller's work buffer
-  double *V, *Vc, *tau, *Tfac, *W1, *W2, *splitk;
+  double *V, *Vc, *tau, *Tfac, *W1, *W2, *splitk, *part;
   size_t splitk_elems;
 };
 
@@ -264,14 +267,16 @@ size_t qr_layout(long long rows, int n, char* base, QrWork* w) {
   auto take = [&](size_t elems) { size_t o = off; off = align_up(off + sizeof(double) * elems); return o; };
   size_t oV = take((size_t)rows * n), oVc = take((size_t)rows * n), otau = take(n);
   size_t npan = (n + QR_NB - 1) / QR_NB;
-  size_t oT = take(npan * QR_NB * QR_NB), oW1 = take((size_t)QR_NB * n), oW2 = take((size_t)QR_NB * n);
+  size_t oT = take(npan * QR_NB_REG * QR_NB_REG), oW1 = take((size_t)QR_NB_REG * n), oW2 = take((size_t)QR_NB_REG * n);
   size_t sk = (size_t)512 * QR_NB * n;
   size_t oS = take(sk);
+  size_t oP = take((size_t)QR_MAX_PARTS * QR_NB_REG * n);
   if (w) {
     w->V = reinterpret_cast<double*>(base + oV); w->Vc = reinterpret_cast<double*>(base + oVc);
     w->tau = reinterpret_cast<double*>(base + otau); w->Tfac = reinterpret_cast<double*>(base + oT);
     w->W1 = reinterpret_cast<double*>(base + oW1); w->W2 = reinterpret_cast<double*>(base + oW2);
     w->splitk = reinterpret_cast<double*>(base + oS); w->splitk_elems = sk;
+    w->part = reinterpret_cast<double*>(base + oP);
   }
   return off;
 }
@@ -325,89 +330,126 @@ cudaError_t launch_panel(cudaStream_t st, double* V, long long ld, long long m, 
   if (max_smem < 0) {
     int dev = 0; cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-    cudaError_t e = cudaFuncSetAttribute(qr_panel_cluster_kernel<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         max_smem);
+    cudaError_t e = cudaFuncSetAttribute(qr_panel_cluster_kernel<NB, true>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
     if (e != cudaSuccess) return e;
-    cluster16 = cudaFuncSetAttribute(qr_panel_cluster_kernel<NB>, cudaFuncAttributeNonPortableClusterSizeAllowed,
-                                     1) == cudaSuccess ? 1 : 0;
+    e = cudaFuncSetAttribute(qr_panel_cluster_kernel<NB, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             max_smem);
+    if (e != cudaSuccess) return e;
+    cluster16 = (cudaFuncSetAttribute(qr_panel_cluster_kernel<NB, true>,
+                                      cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess &&
+                 cudaFuncSetAttribute(qr_panel_cluster_kernel<NB, false>,
+                                      cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess) ? 1 : 0;
     cudaGetLastError();
   }
   const long long prow = m - j0;
-  const size_t fixed = sizeof(double) * (2 * 16 * NB + 2 * NB + 32 * NB + 3 * NB + NB * NB + 16 * NB * NB);
-  const size_t scratch = sizeof(double) * 1024;
+  constexpr int NP = NB * NB, NQ = 1024 / NP > 0 ? 1024 / NP : 1;
+  const size_t fixed = sizeof(double) * (2 * 16 * NB + 2 * NB + 32 * NB + 3 * NB + (NB + 2) + NP + 16 * NP + NQ * NP);
   int C = 8;
   if (prow < 8 * 64) C = prow >= 256 ? 4 : (prow >= 64 ? 2 : 1);
   long long rpc = (prow + C - 1) / C;
   size_t slice = sizeof(double) * (size_t)rpc * NB;
-  int use_smem = 1;
-  if (fixed + scratch + slice > (size_t)max_smem) {
-    if (cluster16) {
-      C = 16; rpc = (prow + C - 1) / C; slice = sizeof(double) * (size_t)rpc * NB;
-    }
-    if (fixed + scratch + slice > (size_t)max_smem) { use_smem = 0; slice = 0; }
+  bool use_smem = true;
+  if (fixed + slice > (size_t)max_smem) {
+    if (cluster16) { C = 16; rpc = (prow + C - 1) / C; slice = sizeof(double) * (size_t)rpc * NB; }
+    if (fixed + slice > (size_t)max_smem) { use_smem = false; slice = 0; }
   }
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(C); cfg.blockDim = dim3(1024);
-  cfg.dynamicSmemBytes = fixed + scratch + slice; cfg.stream = st;
+  cfg.dynamicSmemBytes = fixed + slice; cfg.stream = st;
   cudaLaunchAttribute at[1];
   at[0].id = cudaLaunchAttributeClusterDimension;
   at[0].val.clusterDim.x = C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
   cfg.attrs = at; cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, qr_panel_cluster_kernel<NB>, V, ld, m, j0, nbw, Vc, tau, Tp, rpc, use_smem);
+  return use_smem ? cudaLaunchKernelEx(&cfg, qr_panel_cluster_kernel<NB, true>, V, ld, m, j0, nbw, Vc, tau, Tp, rpc)
+                  : cudaLaunchKernelEx(&cfg, qr_panel_cluster_kernel<NB, false>, V, ld, m, j0, nbw, Vc, tau, Tp, rpc);
+}
+
+// Register-resident panel launch.  Returns cudaErrorInvalidValue if the panel is too tall for it.
+int reg_panel_max_cluster() {
+  static int maxc = -1;
+  if (maxc < 0) {
+    auto k = qr_panel_reg_kernel<QR_NB_REG, QR_REG_NT, QR_REG_RPT>;
+    maxc = cudaFuncSetAttribute(k, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess ? 16 : 8;
+    cudaGetLastError();
+  }
+  return maxc;
+}
+
+cudaError_t launch_panel_reg(cudaStream_t st, double* V, long long ld, long long m, int j0, int nbw, double* Vc,
+                             double* tau, double* Tp) {
+  constexpr int cap = QR_REG_RPT * (QR_REG_NT / QR_NB_REG);
+  const long long prow = m - j0;
+  const int maxc = reg_panel_max_cluster();
+  int C = 1;
+  while (C < maxc && (prow + C - 1) / C > cap) C *= 2;
+  const long long rpc = (prow + C - 1) / C;
+  if (rpc > cap) return cudaErrorInvalidValue;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(C); cfg.blockDim = dim3(QR_REG_NT); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, qr_panel_reg_kernel<QR_NB_REG, QR_REG_NT, QR_REG_RPT>, V, ld, m, j0, nbw, Vc, tau,
+                            Tp, rpc);
+}
+
+// Y <- (I - Vp op(T) Vp^T) Y with the three WY kernels.  Returns launches.
+template <int NB>
+int apply_block_reflector(cudaStream_t st, const double* Vp, long long ldv, double* Y, long long ldy, long long rows,
+                          int nc, int nbw, const double* Tp, int transT, const QrWork& wk) {
+  int chunk = 32;
+  long long nparts = (rows + chunk - 1) / chunk;
+  if (nparts > QR_MAX_PARTS) { chunk = (int)((rows + QR_MAX_PARTS - 1) / QR_MAX_PARTS); nparts = (rows + chunk - 1) / chunk; }
+  wy_partial_kernel<NB><<<(unsigned)nparts, 256, 0, st>>>(Vp, ldv, Y, ldy, rows, nc, nbw, chunk, wk.part);
+  wy_reduce_kernel<NB><<<(nc + 3) / 4, 1024, 0, st>>>(wk.part, (int)nparts, nc, nbw, Tp, transT, wk.W2);
+  wy_update_kernel<NB><<<(unsigned)nparts, 256, 0, st>>>(Vp, ldv, Y, ldy, rows, nc, nbw, chunk, wk.W2);
+  return 3;
 }
 
 // Blocked Householder QR with compact-WY updates (K2a panel / K2b trailing / K2c form Q + sign fix).
-long long qr_factor_blocked(cudaStream_t st, int path, long long rows, int n, const double* X, double* Q,
-                            double* R, void* work, cudaError_t* err) {
-  constexpr int NB = QR_NB;
+template <int NB, bool REG>
+long long qr_factor_blocked_t(cudaStream_t st, long long rows, int n, const double* X, double* Q, double* R,
+                              void* work, cudaError_t* err) {
   QrWork wk;
   qr_layout(rows, n, static_cast<char*>(work), &wk);
   long long launches = 0;
   *err = cudaMemcpyAsync(wk.V, X, sizeof(double) * rows * n, cudaMemcpyDeviceToDevice, st);
   if (*err != cudaSuccess) return -1;
-  auto gemm = [&](const GemmCall& c) -> bool {
-    int nl = launch_gemm(st, path, c, wk.splitk, wk.splitk_elems, err);
-    if (nl < 0) return false;
-    launches += nl;
-    return true;
-  };
-  const IndexMap unit{1, 1, 0};
   const int npan = (n + NB - 1) / NB;
   for (int p = 0; p < npan; ++p) {
     const int j0 = p * NB, nbw = (n - j0 < NB) ? n - j0 : NB, n2 = n - j0 - nbw;
     double* Tp = wk.Tfac + (size_t)p * NB * NB;
-    *err = launch_panel(st, wk.V, n, rows, j0, nbw, wk.Vc, wk.tau, Tp);
+    *err = REG ? launch_panel_reg(st, wk.V, n, rows, j0, nbw, wk.Vc, wk.tau, Tp)
+               : launch_panel(st, wk.V, n, rows, j0, nbw, wk.Vc, wk.tau, Tp);
     if (*err != cudaSuccess) return -1;
     ++launches;
-    if (n2 > 0) {
-      const long long pr = rows - j0;
-      const double* Vp = wk.Vc + (long long)j0 * n + j0;
-      double* A2 = wk.V + (long long)j0 * n + j0 + nbw;
-      // W1 = Vp^T A2 ; W2 = T^T W1 ; A2 -= Vp W2
-      if (!gemm(GemmCall{Vp, n, 1, A2, n, wk.W1, plain_map(n2), unit, nbw, n2, (int)pr, 0})) return -1;
-      if (!gemm(GemmCall{Tp, NB, 1, wk.W1, n2, wk.W2, plain_map(n2), unit, nbw, n2, nbw, 0})) return -1;
-      if (!gemm(GemmCall{Vp, n, 0, wk.W2, n2, A2, plain_map(n), unit, (int)pr, n2, nbw, 1})) return -1;
-    }
+    if (n2 > 0)      // trailing update: A2 <- (I - Vp T^T Vp^T) A2
+      launches += apply_block_reflector<NB>(st, wk.Vc + (long long)j0 * n + j0, n, wk.V + (long long)j0 * n + j0 + nbw,
+                                            n, rows - j0, n2, nbw, Tp, 1, wk);
   }
   copy_triu_kernel<<<(n * n + 255) / 256, 256, 0, st>>>(wk.V, n, n, R);
   set_identity_top_kernel<<<296, 256, 0, st>>>(Q, rows, n);
   launches += 2;
-  for (int p = npan - 1; p >= 0; --p) {
-    const int j0 = p * NB, nbw = (n - j0 < NB) ? n - j0 : NB, nc = n - j0;
-    const long long pr = rows - j0;
-    double* Tp = wk.Tfac + (size_t)p * NB * NB;
-    const double* Vp = wk.Vc + (long long)j0 * n + j0;
-    double* Q2 = Q + (long long)j0 * n + j0;
-    // Q2 <- (I - Vp T Vp^T) Q2
-    if (!gemm(GemmCall{Vp, n, 1, Q2, n, wk.W1, plain_map(nc), unit, nbw, nc, (int)pr, 0})) return -1;
-    if (!gemm(GemmCall{Tp, NB, 0, wk.W1, nc, wk.W2, plain_map(nc), unit, nbw, nc, nbw, 0})) return -1;
-    if (!gemm(GemmCall{Vp, n, 0, wk.W2, nc, Q2, plain_map(n), unit, (int)pr, nc, nbw, 1})) return -1;
+  for (int p = npan - 1; p >= 0; --p) {      // Q2 <- (I - Vp T Vp^T) Q2, back to front
+    const int j0 = p * NB, nbw = (n - j0 < NB) ? n - j0 : NB;
+    launches += apply_block_reflector<NB>(st, wk.Vc + (long long)j0 * n + j0, n, Q + (long long)j0 * n + j0, n,
+                                          rows - j0, n - j0, nbw, wk.Tfac + (size_t)p * NB * NB, 0, wk);
   }
   sign_fix_kernel<<<296, 256, 0, st>>>(Q, rows, n, R);
   sign_fix_R_kernel<<<n, 128, 0, st>>>(R, n);
   launches += 2;
   *err = cudaGetLastError();
   return *err == cudaSuccess ? launches : -1;
+}
+
+long long qr_factor_blocked(cudaStream_t st, int /*gemm_path*/, long long rows, int n, const double* X, double* Q,
+                            double* R, void* work, cudaError_t* err) {
+  constexpr long long cap = (long long)QR_REG_RPT * (QR_REG_NT / QR_NB_REG);
+  if (rows <= cap * reg_panel_max_cluster())
+    return qr_factor_blocked_t<QR_NB_REG, true>(st, rows, n, X, Q, R, work, err);
+  return qr_factor_blocked_t<QR_NB, false>(st, rows, n, X, Q, R, work, err);
 }
 
 }  // namespace

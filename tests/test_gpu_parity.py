@@ -55,7 +55,8 @@ def test_gemm_odd_leading_dimension_views():
 
 
 @pytest.mark.parametrize("rows,cols", [(32, 8), (324, 36), (1024, 64), (50, 50), (7, 1), (333, 17), (16, 16),
-                                       (2500, 100), (40, 33), (9604, 196), (3000, 150)])
+                                       (2500, 100), (40, 33), (9604, 196), (3000, 150),
+                                       (15000, 24), (40000, 40)])   # 16-CTA cluster; global-memory panel path
 @pytest.mark.parametrize("path", [0, 1])
 def test_qr_f64_matches_oracle(rows, cols, path):
     if path == 1 and rows * cols > 200000:
