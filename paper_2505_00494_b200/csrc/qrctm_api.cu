@@ -45,6 +45,9 @@ struct qrctm {
   long long launches;
   cudaEvent_t ev[QRCTM_NSTAGE + 2];
   bool have_ev;
+  cudaStream_t side;            // high-priority stream for the overlapped convergence check
+  cudaEvent_t ev_env, ev_spec;  // environment ready (main) / spectrum done (side)
+  int overlap;
   double stage_ms[QRCTM_NSTAGE + 1];
   long long stage_steps;
   char err[256];
@@ -541,19 +544,36 @@ int stage_normalize(qrctm* h, const double* Cn, const double* Tn) {
 }
 
 // K8: spectrum of h->C into s_out (+ delta against s_prev, optional update)
-int stage_spectrum(qrctm* h, double* s_out, int update_prev) {
+int stage_spectrum(qrctm* h, double* s_out, int update_prev, cudaStream_t st) {
   const int chi = h->chi;
-  CU(h, cudaMemcpyAsync(h->Wc, h->C, sizeof(double) * chi * chi, cudaMemcpyDeviceToDevice, h->stream));
-  tridiag_kernel<<<1, 1024, 0, h->stream>>>(h->Wc, chi, h->dvec, h->evec, h->vv, h->pv);
-  int nt = (chi + 31) / 32 * 32; if (nt < 64) nt = 64;
-  bisect_sort_kernel<<<1, nt, sizeof(double) * (3 * chi + 40), h->stream>>>(h->dvec, h->evec, chi, h->eig, s_out,
-                                                                          h->s_prev, h->delta, update_prev);
-  h->launches += 2;
+  static int max_smem = -1;
+  if (max_smem < 0) {
+    int dev = 0; cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    max_smem -= 1024;      // static shared memory of the kernel
+    CU(h, cudaFuncSetAttribute(tridiag_smem_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
+  }
+  const size_t tri_bytes = sizeof(double) * ((size_t)chi * (chi + 1) / 2 + 2 * (size_t)chi + 40);
+  const int nt = ((chi + 31) / 32 * 32) < 64 ? 64 : (chi + 31) / 32 * 32;
+  if (tri_bytes <= (size_t)max_smem && chi <= 1024) {
+    tridiag_smem_kernel<<<1, 1024, tri_bytes, st>>>(h->C, chi, h->dvec, h->evec);
+    multisect_kernel<<<(chi + 7) / 8, 256, sizeof(double) * (2 * chi + 40), st>>>(h->dvec, h->evec, chi,
+                                                                                         h->eig);
+    spectrum_finalize_kernel<<<1, nt, sizeof(double) * (chi + 40), st>>>(h->eig, chi, s_out, h->s_prev,
+                                                                                 h->delta, update_prev);
+    h->launches += 3;
+  } else {
+    CU(h, cudaMemcpyAsync(h->Wc, h->C, sizeof(double) * chi * chi, cudaMemcpyDeviceToDevice, st));
+    tridiag_kernel<<<1, 1024, 0, st>>>(h->Wc, chi, h->dvec, h->evec, h->vv, h->pv);
+    bisect_sort_kernel<<<1, nt, sizeof(double) * (3 * chi + 40), st>>>(h->dvec, h->evec, chi, h->eig, s_out,
+                                                                            h->s_prev, h->delta, update_prev);
+    h->launches += 2;
+  }
   CU(h, cudaGetLastError());
   return QRCTM_OK;
 }
 
-int do_step(qrctm* h, cudaEvent_t* ev /* QRCTM_NSTAGE+1 events or null */) {
+int do_step(qrctm* h, cudaEvent_t* ev /* QRCTM_NSTAGE+1 events or null */, bool with_k7 = true) {
   // NVTX ranges name the stages so that `ncu --nvtx --nvtx-include "K4_absorb_a/"` selects one.
   auto mark = [&](int i, const char* next) {
     if (i > 0) nvtxRangePop();
@@ -575,6 +595,7 @@ int do_step(qrctm* h, cudaEvent_t* ev /* QRCTM_NSTAGE+1 events or null */) {
   if (!rc) { mark(3, "K4_absorb_a"); rc = stage_absorb_a(h, h->P, h->S, 0); }
   if (!rc) { mark(4, "K5_project"); rc = stage_project(h, h->S, h->Q, h->Tn); }
   if (!rc) { mark(5, "K6_corner"); rc = h->corner_mode == 0 ? stage_corner_accel(h) : stage_corner_enlarged(h); }
+  if (!rc && !with_k7) { nvtxRangePop(); return rc; }
   if (!rc) { mark(6, "K7_normalize"); rc = stage_normalize(h, h->Cn, h->Tn); }
   if (!rc) mark(7, nullptr); else nvtxRangePop();
   return rc;
@@ -612,7 +633,7 @@ static int create_common(int d, int D, int chi, void* ws, unsigned long long ws_
   memset(h, 0, sizeof(*h));
   h->d = d; h->D = D; h->b = D * D; h->chi = chi; h->m = (long long)chi * D * D;
   h->L = L; h->stream = 0;
-  h->corner_mode = 0; h->symmetrize = 1; h->check_every = 1; h->gemm_path = 0;
+  h->corner_mode = 0; h->symmetrize = 1; h->check_every = 1; h->gemm_path = 0; h->overlap = 1;
   if (ws) {
     if (ws_bytes < L.total || (reinterpret_cast<uintptr_t>(ws) & (kAlign - 1)) || !is_device_ptr(ws)) {
       delete h; return QRCTM_ERR_INVALID_ARG;
@@ -629,6 +650,15 @@ static int create_common(int d, int D, int chi, void* ws, unsigned long long ws_
     cudaGetLastError(); if (h->owns_ws) cudaFree(h->base); delete h; return QRCTM_ERR_CUDA;
   }
   h->h_pinned = static_cast<double*>(hp);
+  {
+    int lo = 0, hi = 0;
+    cudaDeviceGetStreamPriorityRange(&lo, &hi);
+    if (cudaStreamCreateWithPriority(&h->side, cudaStreamNonBlocking, hi) != cudaSuccess ||
+        cudaEventCreateWithFlags(&h->ev_env, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&h->ev_spec, cudaEventDisableTiming) != cudaSuccess) {
+      cudaGetLastError(); h->side = nullptr; h->overlap = 0;
+    }
+  }
   h->h_flag = reinterpret_cast<int*>(h->h_pinned + 32);
   cudaMemsetAsync(h->flag, 0, 4 * sizeof(int), 0);
   cudaMemsetAsync(h->s_prev, 0, sizeof(double) * chi, 0);
@@ -651,6 +681,7 @@ int qrctm_destroy(qrctm_t* h) {
   cudaStreamSynchronize(h->stream);
   if (h->owns_ws && h->base) cudaFree(h->base);
   if (h->h_pinned) cudaFreeHost(h->h_pinned);
+  if (h->side) { cudaStreamSynchronize(h->side); cudaStreamDestroy(h->side); cudaEventDestroy(h->ev_env); cudaEventDestroy(h->ev_spec); }
   if (h->have_ev) for (int i = 0; i < QRCTM_NSTAGE + 2; ++i) cudaEventDestroy(h->ev[i]);
   cudaGetLastError();
   delete h;
@@ -686,7 +717,7 @@ int qrctm_set_env(qrctm_t* h, const double* C, const double* T) {
   int rc = stage_normalize(h, h->Cn, h->Tn); if (rc) return rc;
   rc = check_flag(h); if (rc) return rc;
   CU(h, cudaMemsetAsync(h->s_prev, 0, sizeof(double) * h->chi, h->stream));
-  rc = stage_spectrum(h, h->s, 1); if (rc) return rc;
+  rc = stage_spectrum(h, h->s, 1, h->stream); if (rc) return rc;
   h->have_env = true;
   return QRCTM_OK;
 }
@@ -701,6 +732,44 @@ int qrctm_run(qrctm_t* h, int max_iter, double tol, int* iters_done, double* fin
   if (!h) return QRCTM_ERR_INVALID_ARG;
   if (!h->have_A || !h->have_env) return fail(h, QRCTM_ERR_NOT_READY, "set_A and set_env first");
   if (max_iter < 0) return fail(h, QRCTM_ERR_INVALID_ARG, "max_iter < 0");
+  if (h->overlap && h->side && !h->time_stages) {
+    // Overlapped driver: K1..K6 of step it are queued before the host waits for the spectrum of
+    // step it-1 (side stream); K7 of step it (the only stage that overwrites C, T) waits for it.
+    double delta = INFINITY;
+    int done = 0;
+    bool pending = false;                       // a spectrum result is in flight on the side stream
+    for (int it = 1; it <= max_iter; ++it) {
+      int rc = do_step(h, nullptr, false); if (rc) return rc;
+      if (pending) {
+        CU(h, cudaEventSynchronize(h->ev_spec));
+        pending = false;
+        if (h->h_flag[0]) { cudaStreamSynchronize(h->stream); return fail(h, QRCTM_ERR_NUMERIC, "NaN/Inf or zero Frobenius norm in C' or T'"); }
+        delta = h->h_pinned[0];
+        if (delta < tol) break;                 // converged at step it-1: the half step in flight is discarded
+      }
+      rc = stage_normalize(h, h->Cn, h->Tn); if (rc) return rc;
+      done = it;
+      if (it % h->check_every == 0 || it == max_iter) {
+        CU(h, cudaEventRecord(h->ev_env, h->stream));
+        CU(h, cudaStreamWaitEvent(h->side, h->ev_env, 0));
+        rc = stage_spectrum(h, h->s, 1, h->side); if (rc) return rc;
+        CU(h, cudaMemcpyAsync(h->h_pinned, h->delta, sizeof(double), cudaMemcpyDeviceToHost, h->side));
+        CU(h, cudaMemcpyAsync(h->h_flag, h->flag, sizeof(int), cudaMemcpyDeviceToHost, h->side));
+        CU(h, cudaEventRecord(h->ev_spec, h->side));
+        // (the next K7, the only writer of C, is enqueued after the host has seen ev_spec complete)
+        pending = true;
+      }
+    }
+    if (pending) {
+      CU(h, cudaEventSynchronize(h->ev_spec));
+      if (h->h_flag[0]) { cudaStreamSynchronize(h->stream); return fail(h, QRCTM_ERR_NUMERIC, "NaN/Inf or zero Frobenius norm in C' or T'"); }
+      delta = h->h_pinned[0];
+    }
+    CU(h, cudaStreamSynchronize(h->stream));
+    if (iters_done) *iters_done = done;
+    if (final_delta) *final_delta = delta;
+    return QRCTM_OK;
+  }
   double delta = INFINITY;
   int it = 0;
   if (h->time_stages && !h->have_ev) {
@@ -711,7 +780,7 @@ int qrctm_run(qrctm_t* h, int max_iter, double tol, int* iters_done, double* fin
     int rc = do_step(h, h->time_stages ? h->ev : nullptr); if (rc) return rc;
     const bool check = (it % h->check_every == 0 || it == max_iter);
     if (check) {
-      rc = stage_spectrum(h, h->s, 1); if (rc) return rc;
+      rc = stage_spectrum(h, h->s, 1, h->stream); if (rc) return rc;
       CU(h, cudaMemcpyAsync(h->h_pinned, h->delta, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
     }
     if (h->time_stages) CU(h, cudaEventRecord(h->ev[QRCTM_NSTAGE + 1], h->stream));
@@ -749,7 +818,7 @@ int qrctm_get_env(qrctm_t* h, double* C, double* T) {
 int qrctm_get_corner_spectrum(qrctm_t* h, double* s) {
   if (!h || !s) return h ? fail(h, QRCTM_ERR_INVALID_ARG, "null s") : QRCTM_ERR_INVALID_ARG;
   if (!h->have_env) return fail(h, QRCTM_ERR_NOT_READY, "no environment");
-  int rc = stage_spectrum(h, h->s_tmp, 0); if (rc) return rc;
+  int rc = stage_spectrum(h, h->s_tmp, 0, h->stream); if (rc) return rc;
   CU(h, copy_out(s, h->s_tmp, h->chi, h->stream));
   return QRCTM_OK;
 }
@@ -787,6 +856,7 @@ int qrctm_set_option(qrctm_t* h, int key, int value) {
     case QRCTM_OPT_CHECK_EVERY: if (value < 1) break; h->check_every = value; return QRCTM_OK;
     case QRCTM_OPT_GEMM_PATH:   if (value != 0 && value != 1) break; h->gemm_path = value; return QRCTM_OK;
     case QRCTM_OPT_QR_PATH:     if (value != 0 && value != 1) break; h->qr_path = value; return QRCTM_OK;
+    case QRCTM_OPT_OVERLAP_CHECK: if (value != 0 && value != 1) break; h->overlap = value; return QRCTM_OK;
     case QRCTM_OPT_TIME_STAGES: if (value != 0 && value != 1) break; h->time_stages = value; return QRCTM_OK;
     default: break;
   }

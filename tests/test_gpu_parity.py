@@ -285,3 +285,38 @@ def test_ising_onsager_on_gpu():
     h.run(300, 1e-13)
     assert abs(np.log(h.norm_per_site()) - onsager_ln_kappa(K)) < 1e-10
     h.close()
+
+
+def test_overlapped_check_is_bitwise_identical_to_serial():
+    """qrctm_run with the convergence check overlapped on the side stream must give the same
+    iteration count, delta and environment as the strictly serial driver."""
+    A, C0, T0 = gen_config(2, 3, 24, 0)
+    res = []
+    for overlap in (1, 0):
+        h = pkg.QRCTM(2, 3, 24)
+        h.set_option(pkg.OPT_OVERLAP_CHECK, overlap)
+        h.set_A(A); h.set_env(C0, T0)
+        it, dl = h.run(400, 1e-9)
+        C, T = h.get_env()
+        it2, dl2 = h.run(7, -1.0)                  # fixed count afterwards
+        C2, T2 = h.get_env()
+        res.append((it, dl, C, T, it2, dl2, C2, T2, h.get_corner_spectrum()))
+        h.close()
+    a, b = res
+    assert a[0] == b[0] and a[1] == b[1] and a[4] == b[4] == 7 and a[5] == b[5]
+    assert a[0] < 400
+    for i in (2, 3, 6, 7, 8):
+        assert np.array_equal(a[i], b[i])
+
+
+def test_check_every_option():
+    A, C0, T0 = gen_config(2, 2, 8, 0)
+    h = pkg.QRCTM(2, 2, 8)
+    h.set_option(pkg.OPT_CHECK_EVERY, 5)
+    h.set_A(A); h.set_env(C0, T0)
+    it, dl = h.run(500, 1e-12)
+    assert it % 5 == 0 and it < 500
+    Co, To, a = _oracle_steps(A, C0, T0, it)
+    C, T = h.get_env()
+    assert rel(C, Co) < 1e-9 and rel(T, To) < 1e-9
+    h.close()
