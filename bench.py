@@ -266,12 +266,12 @@ def main():
         k4_ms = stage_ms["K4_absorb_a"] / nst
         ach = fl["K4"] / (k4_ms * 1e-3) / 1e12
         traffic = None
-        tpath = os.path.join(ROOT, "profiles", "k4_traffic_bytes.json")
+        tpath = os.path.join(ROOT, "profiles", "k4_traffic_bytes.txt")   # from the committed ncu --set full capture
         if os.path.exists(tpath):
-            try:
-                traffic = json.load(open(tpath)).get(name)
-            except Exception:
-                traffic = None
+            for ln in open(tpath):
+                f = ln.split()
+                if len(f) == 2 and f[0] == name:
+                    traffic = int(f[1])
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
