@@ -233,7 +233,7 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 }
 
 template <int BM, int BN, int WM, int WN, int STAGES>
-__global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 1) * 32, 1)
+__global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 1) * 32, ((BM / WM) * (BN / WN) <= 4 ? 2 : 1))
 gemm_f64_dmma_ws(GemmArgs p) {
   constexpr int NW_M = BM / WM, NW_N = BN / WN, NCW = NW_M * NW_N;
   constexpr int LDA_S = BM + PAD, LDB_S = BN + PAD;

@@ -421,6 +421,156 @@ qr_panel_reg_kernel(double* __restrict__ V, long long ld, long long m, int j0, i
 }
 
 // ------------------------------------------------------------------------------
+// Register-resident panel kernel, second version (the default).  Differences to
+// qr_panel_reg_kernel: (1) the diagonal row r of step k is taken out of the register
+// tile at the START of the step (its values travel through `rowv`, its final R / v
+// entries are written straight to global memory), so the register tile only ever
+// holds rows strictly below the current diagonal and the dot / update loops carry no
+// per-row predicates; (2) every thread finishes the reflector scalars (sqrt, two
+// divisions) redundantly from the exchanged partial sums, so a column step needs ONE
+// __syncthreads and (multi-CTA only) ONE cluster barrier; (3) the compact-WY column
+// of T is built by warp 0 with shuffles off the critical path of the other warps.
+// The panel's diagonal rows j0..j0+nbw-1 are the first local rows of rank 0 (t = 0).
+template <int NB, int NT, int RPT, bool CLUSTER>
+__global__ void __launch_bounds__(NT, 1)
+qr_panel_reg2_kernel(double* __restrict__ V, long long ld, long long m, int j0, int nbw,
+                     double* __restrict__ Vc, double* __restrict__ tau, double* __restrict__ Tp, long long rpc) {
+  namespace cg = cooperative_groups;
+  cg::cluster_group cluster = cg::this_cluster();
+  const int C = CLUSTER ? (int)cluster.num_blocks() : 1;
+  const int rank = CLUSTER ? (int)cluster.block_rank() : 0;
+  constexpr int NRG = NT / NB, NW = NT / 32;
+  static_assert(NRG >= NB, "diagonal rows must all sit at t = 0");
+  __shared__ double exch[2 * 16 * NB];
+  __shared__ double rowv[2 * NB];
+  __shared__ double red[2 * NW * NB];
+  __shared__ double Ts[NB * NB];
+
+  const int tid = threadIdx.x, col = tid % NB, rg = tid / NB, warp = tid >> 5, lane = tid & 31;
+  const int lane_base = lane & ~(NB - 1);
+  const long long row_lo = (long long)j0 + (long long)rank * rpc;
+  long long row_hi = row_lo + rpc; if (row_hi > m) row_hi = m;
+  const int nloc = row_hi > row_lo ? (int)(row_hi - row_lo) : 0;
+  double* const gpan = V + row_lo * ld + j0;
+  double* const gvc = Vc + row_lo * ld + j0;
+
+  double val[RPT];
+  {
+    const double* pl = gpan + (long long)rg * ld + col;
+#pragma unroll
+    for (int t = 0; t < RPT; ++t, pl += (long long)NRG * ld)
+      val[t] = (rg + t * NRG < nloc && col < nbw) ? *pl : 0.0;
+  }
+  if (tid < NB * NB) Ts[tid] = 0.0;
+  if (NT < NB * NB) for (int i = tid + NT; i < NB * NB; i += NT) Ts[i] = 0.0;
+  double my_scale = 0.0;                       // scale of this thread's column once it has been factored
+  __syncthreads();
+  if (CLUSTER) cluster.sync();
+
+  int buf = 0;
+  for (int k = 0; k < nbw; ++k) {
+    // A. take the diagonal row r = j0 + k out of the tile (rank 0, row group k, t = 0)
+    const bool mine = (rank == 0) && (rg == k);
+    double rvv = 0.0;
+    if (mine) {
+      rvv = val[0]; val[0] = 0.0;
+      if (CLUSTER) { for (int q = 0; q < C; ++q) { double* rr = cluster.map_shared_rank(rowv, q); rr[buf * NB + col] = rvv; } }
+      else rowv[buf * NB + col] = rvv;
+    }
+    // B. column k of my rows, dot with my column
+    double xs[RPT];
+    double a0 = 0.0, a1 = 0.0;
+#pragma unroll
+    for (int t = 0; t < RPT; ++t) {
+      xs[t] = __shfl_sync(0xffffffffu, val[t], lane_base | k);
+      if (t & 1) a1 = fma(xs[t], val[t], a1); else a0 = fma(xs[t], val[t], a0);
+    }
+    double acc = a0 + a1;
+    if (NB == 16) acc += __shfl_xor_sync(0xffffffffu, acc, 16);
+    if (lane < NB) red[(buf * NW + warp) * NB + lane] = acc;
+    __syncthreads();
+    double gk = 0.0, gj = 0.0;
+    if (CLUSTER) {
+      if (tid < NB) {
+        double g = 0.0;
+#pragma unroll
+        for (int w = 0; w < NW; ++w) g += red[(buf * NW + w) * NB + tid];
+        for (int q = 0; q < C; ++q) { double* rex = cluster.map_shared_rank(exch, q); rex[(buf * 16 + rank) * NB + tid] = g; }
+      }
+      cluster.sync();
+      for (int q = 0; q < C; ++q) { gk += exch[(buf * 16 + q) * NB + k]; gj += exch[(buf * 16 + q) * NB + col]; }
+    } else {
+#pragma unroll
+      for (int w = 0; w < NW; ++w) { gk += red[(buf * NW + w) * NB + k]; gj += red[(buf * NW + w) * NB + col]; }
+    }
+    // F. reflector scalars (identical in every thread)
+    const double alpha = rowv[buf * NB + k], yrj = rowv[buf * NB + col];
+    double tk = 0.0, scale = 0.0, beta = alpha;
+    if (gk > 0.0) {
+      const double sigma = sqrt(fma(alpha, alpha, gk));
+      beta = alpha >= 0.0 ? -sigma : sigma;
+      tk = (beta - alpha) / beta;
+      scale = 1.0 / (alpha - beta);
+    }
+    const double z = fma(scale, gj, yrj);          // v_k^T y_j (j > k)  or  (x_a[r] + scale h_a) (a < k)
+    const double w = tk * z;
+    // G. update the trailing panel columns
+    if (col > k && col < nbw && tk != 0.0) {
+      const double nsw = -scale * w;
+#pragma unroll
+      for (int t = 0; t < RPT; ++t) val[t] = fma(xs[t], nsw, val[t]);
+    }
+    // H. final entries of row r
+    if (mine && col < nbw) {
+      double vout, vclean;
+      if (col < k) { vclean = rvv * my_scale; vout = vclean; }
+      else if (col == k) { vclean = 1.0; vout = beta; }
+      else { vclean = 0.0; vout = (tk != 0.0) ? rvv - w : rvv; }
+      V[(long long)(j0 + k) * ld + j0 + col] = vout;
+      Vc[(long long)(j0 + k) * ld + j0 + col] = vclean;
+    }
+    // I. column k of T (warp 0, lanes a < NB hold col = a): T[a][k] = -tau_k sum_{c=a}^{k-1} T[a][c] G[c][k]
+    if (warp == 0) {
+      const double Gak = my_scale * z;                       // valid for lanes with col < k (rg = 0 half)
+      double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+      for (int c = 0; c < NB; c += 2) {
+        const double g0 = __shfl_sync(0xffffffffu, Gak, c), g1 = __shfl_sync(0xffffffffu, Gak, c + 1);
+        if (lane < NB && c >= lane && c < k) s0 = fma(Ts[lane * NB + c], g0, s0);
+        if (lane < NB && c + 1 >= lane && c + 1 < k) s1 = fma(Ts[lane * NB + c + 1], g1, s1);
+      }
+      if (lane < NB) {
+        if (lane == k) Ts[k * NB + k] = tk;
+        else if (lane < k) Ts[lane * NB + k] = -tk * (s0 + s1);
+      }
+      if (rank == 0 && lane == k) tau[j0 + k] = tk;
+    }
+    if (col == k) my_scale = scale;
+    buf ^= 1;
+  }
+
+  // write-back of the rows below the panel's diagonal block
+  if (col < nbw) {
+    double* po = gpan + (long long)rg * ld + col;
+    double* pc = gvc + (long long)rg * ld + col;
+#pragma unroll
+    for (int t = 0; t < RPT; ++t, po += (long long)NRG * ld, pc += (long long)NRG * ld) {
+      const int li = rg + t * NRG;
+      if (li < nloc && !(rank == 0 && li < nbw)) {
+        const double v = val[t] * my_scale;
+        *po = v; *pc = v;
+      }
+    }
+  }
+  __syncwarp();
+  if (rank == 0 && warp == 0) {
+    __syncwarp();
+    for (int i = lane; i < NB * NB; i += 32) Tp[i] = Ts[i];
+  }
+  if (CLUSTER) cluster.sync();      // nobody exits while a peer may still address its shared memory
+}
+
+// ------------------------------------------------------------------------------
 // Applying a block reflector  Y <- (I - Vp op(T) Vp^T) Y  to Y = rows x nc (ld ldy):
 // three memory-bound kernels (intensity 2*NB flop per 16 bytes of Y, below the
 // FP64 ridge of ~5.7 flop/B even at NB = 32, so plain DFMA with coalesced row

@@ -88,7 +88,7 @@ bool make_layout(int d, int D, int chi, Layout* L) {
   L->S = take(dbl * m * m);
   L->W = take(dbl * m * chi);
   L->E = take(dbl * m * chi);
-  L->splitk_elems = (size_t)256 * chi * chi + (size_t)4 * m * chi;
+  L->splitk_elems = (size_t)256 * chi * chi + (size_t)16 * m * chi;
   L->splitk = take(dbl * L->splitk_elems);
   L->partial = take(dbl * 4 * kPartialBlocks);
   L->scal = take(dbl * 16);
@@ -218,8 +218,33 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
   const long long t128 = (long long)((c.M + 127) / 128) * ((c.N + 127) / 128);
   const long long t64 = (long long)((c.M + 63) / 64) * ((c.N + 63) / 64);
   const bool big = t128 >= 120;
+  const bool ws_ok = g.transA && g.vecA && g.vecB;     // bulk copies need 16-byte aligned rows
   int splits = 1;
-  if (!big && t64 < 148 && nkt >= 8) {
+  int cfg = 0;          // 0: 64x64 cp.async, 1: 128x128 cp.async, 2: ws 128x128, 3: ws 128x104, 4: ws 128x64 (2 CTA/SM)
+  const bool ws_big = ws_ok && c.M >= 96 && c.N >= 96 && (double)c.M * c.N * c.K > 2.0e8;
+  if (ws_big) {
+    // pick the N tile with the least padding, then split K so that the CTAs fill whole waves
+    auto padded = [&](int bn) { return (long long)((c.N + bn - 1) / bn) * bn; };
+    int bn = 128; cfg = 2;
+    if (nkt <= 32 && c.N >= 1024) { bn = 64; cfg = 4; }        // short K: two CTAs per SM overlap epilogue and mainloop
+    else if (padded(104) * 100 < padded(128) * 97) { bn = 104; cfg = 3; }
+    const long long tiles = (long long)((c.M + 127) / 128) * ((c.N + bn - 1) / bn);
+    const int slots = cfg == 4 ? 296 : 148;
+    const double t_kt = 2.1e-6 * bn / 128.0 * (cfg == 4 ? 2.0 : 1.0), t_fix = 4e-6;
+    double best = 1e30;
+    for (int sp = 1; sp <= 64; ++sp) {
+      int per = (nkt + sp - 1) / sp;
+      if (sp > 1 && per < 8) break;
+      int sp_eff = (nkt + per - 1) / per;
+      if (sp_eff != sp) continue;
+      if (sp > 1 && (size_t)c.M * c.N * sp > splitk_elems) break;
+      long long waves = (tiles * sp + slots - 1) / slots;
+      double t = waves * (per * t_kt + t_fix) + (sp > 1 ? 2.0 * sp * c.M * (double)c.N * 8.0 / 4e12 + 4e-6 : 0.0);
+      if (t < best * 0.97) { best = t; splits = sp; }
+    }
+  } else if (big) {
+    cfg = 1;
+  } else if (t64 < 148 && nkt >= 8) {
     splits = (int)((2 * 148 + t64 - 1) / t64);
     if (splits > nkt / 2) splits = nkt / 2;
     size_t per = (size_t)c.M * c.N;
@@ -233,10 +258,13 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
     g.out = splitk_ws; g.ro = plain_map(c.N); g.co = IndexMap{1, 1, 0}; g.mode = 0;
     g.split_stride = (long long)c.M * c.N;
   }
-  const bool ws_ok = g.transA && g.vecA && g.vecB;     // bulk copies need 16-byte aligned rows
-  if (big && ws_ok) *err = launch_cfg_ws<128, 128, 64, 32, 4>(st, g, splits);
-  else if (big) *err = launch_cfg<128, 128, 64, 32, 4>(st, g, splits);
-  else     *err = launch_cfg<64, 64, 32, 32, 4>(st, g, splits);
+  switch (cfg) {
+    case 2: *err = launch_cfg_ws<128, 128, 64, 32, 4>(st, g, splits); break;
+    case 3: *err = launch_cfg_ws<128, 104, 16, 104, 4>(st, g, splits); break;
+    case 4: *err = launch_cfg_ws<128, 64, 64, 32, 4>(st, g, splits); break;
+    case 1: *err = launch_cfg<128, 128, 64, 32, 4>(st, g, splits); break;
+    default: *err = launch_cfg<64, 64, 32, 32, 4>(st, g, splits); break;
+  }
   if (*err != cudaSuccess) return -1;
   ++launched;
   if (splits > 1) {
@@ -257,7 +285,7 @@ namespace {
 
 constexpr int QR_NB = 16;        // shared-memory / global panel kernel (fallback for very tall panels)
 constexpr int QR_NB_REG = 16;    // register-resident panel kernel (default)
-constexpr int QR_REG_NT = 512, QR_REG_RPT = 20;                       // 640 rows per CTA
+constexpr int QR_REG_NT = 256, QR_REG_RPT = 40;                       // 640 rows per CTA
 constexpr int QR_MAX_PARTS = 320;
 
 struct QrWork {     // carved out of the caller's work buffer
@@ -372,7 +400,7 @@ cudaError_t launch_panel(cudaStream_t st, double* V, long long ld, long long m, 
 int reg_panel_max_cluster() {
   static int maxc = -1;
   if (maxc < 0) {
-    auto k = qr_panel_reg_kernel<QR_NB_REG, QR_REG_NT, QR_REG_RPT>;
+    auto k = qr_panel_reg2_kernel<QR_NB_REG, QR_REG_NT, QR_REG_RPT, true>;
     maxc = cudaFuncSetAttribute(k, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess ? 16 : 8;
     cudaGetLastError();
   }
@@ -388,14 +416,19 @@ cudaError_t launch_panel_reg(cudaStream_t st, double* V, long long ld, long long
   while (C < maxc && (prow + C - 1) / C > cap) C *= 2;
   const long long rpc = (prow + C - 1) / C;
   if (rpc > cap) return cudaErrorInvalidValue;
+  if (C == 1) {
+    qr_panel_reg2_kernel<QR_NB_REG, QR_REG_NT, QR_REG_RPT, false><<<1, QR_REG_NT, 0, st>>>(V, ld, m, j0, nbw, Vc, tau,
+                                                                                          Tp, rpc);
+    return cudaGetLastError();
+  }
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(C); cfg.blockDim = dim3(QR_REG_NT); cfg.dynamicSmemBytes = 0; cfg.stream = st;
   cudaLaunchAttribute at[1];
   at[0].id = cudaLaunchAttributeClusterDimension;
   at[0].val.clusterDim.x = C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
   cfg.attrs = at; cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, qr_panel_reg_kernel<QR_NB_REG, QR_REG_NT, QR_REG_RPT>, V, ld, m, j0, nbw, Vc, tau,
-                            Tp, rpc);
+  return cudaLaunchKernelEx(&cfg, qr_panel_reg2_kernel<QR_NB_REG, QR_REG_NT, QR_REG_RPT, true>, V, ld, m, j0, nbw, Vc,
+                            tau, Tp, rpc);
 }
 
 // Y <- (I - Vp op(T) Vp^T) Y with the three WY kernels.  Returns launches.

@@ -320,3 +320,35 @@ def test_check_every_option():
     C, T = h.get_env()
     assert rel(C, Co) < 1e-9 and rel(T, To) < 1e-9
     h.close()
+
+
+@pytest.mark.parametrize("name", ["cfg3a", "cfg3b", "cfg4"])
+def test_full_size_single_step_parity(name):
+    """North-star bar at BASELINE.json's full sizes, in the launch configuration bench.py times:
+    relative Frobenius error <= 1e-11 on C and T after one step (after the R-sign gauge fix)."""
+    c = CONFIGS[name]
+    out, s, (Cr, Tr, Co, To) = _one_step(c["d"], c["D"], c["chi"], c["seed"])
+    Q, R = out["QR"]
+    cond = np.linalg.cond(s["X"])
+    assert rel(R, s["R"]) < 1e-14 * max(cond, 10) and rel(Q, s["Q"]) < 1e-14 * max(cond, 10)
+    assert np.linalg.norm(Q.T @ Q - np.eye(c["chi"])) < c["chi"] * 2e-15
+    Cn, Tn = out["raw"]
+    assert rel(Tn, s["Tn"]) < 1e-11 and rel(Cn, s["Cn"]) < 1e-11
+    assert rel(out["C"], Co) < 1e-11 and rel(out["T"], To) < 1e-11
+    assert np.array_equal(out["C"], out["C"].T) and np.array_equal(out["T"], out["T"].transpose(2, 1, 0))
+
+
+def test_cfg3a_ten_steps_and_kappa_parity():
+    c = CONFIGS["cfg3a"]
+    A, C0, T0 = gen_config(c["d"], c["D"], c["chi"], c["seed"])
+    h = pkg.QRCTM(c["d"], c["D"], c["chi"])
+    h.set_A(A); h.set_env(C0, T0)
+    it, dl = h.run(10, -1.0)
+    assert it == 10
+    Co, To, a = _oracle_steps(A, C0, T0, 10)
+    C, T = h.get_env()
+    assert rel(C, Co) < 1e-9 and rel(T, To) < 1e-9
+    s, so = h.get_corner_spectrum(), o.spectrum(Co)
+    assert np.max(np.abs(s[:10] - so[:10]) / so[:10]) < 1e-9
+    assert abs(h.norm_per_site() / o.kappa(Co, To, a) - 1) < 1e-9
+    h.close()
