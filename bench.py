@@ -96,6 +96,20 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def aggregate_over_ranks(ms_total, e2e_ms, steps, world, device=None):
+    """Whole-job numbers from per-rank times ("replicas only": every rank ran `steps` independent
+    iterations): MAX over ranks of the elapsed times, then value = world * steps / max time.
+    Works on any torch.distributed backend (nccl on GPUs, gloo in the CPU tests)."""
+    if world > 1:
+        import torch
+        import torch.distributed as dist
+        t = torch.tensor([ms_total, e2e_ms], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total, e2e_ms = float(t[0]), float(t[1])
+    return dict(ms_total=ms_total, e2e_ms=e2e_ms, ms_per_step=ms_total / steps,
+                value=world * steps / (ms_total * 1e-3), e2e_value=world * 1e3 / e2e_ms)
+
+
 def oracle_time_steps(name, max_steps, budget_s):
     """Time the oracle's QR-CTMRG iteration (qr_step + normalize + spectrum) as it stands."""
     from oracle import ctmrg as o
@@ -200,9 +214,9 @@ def main():
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
-    ev0.record()
+    ev0.record(h.stream)                 # events on the stream the kernels are launched on
     it, delta = h.run(args.steps, -1.0)
-    ev1.record()
+    ev1.record(h.stream)
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
@@ -254,13 +268,9 @@ def main():
     d2h = 8 * (C0.size + T0.size) + 8
 
     # ---- max over ranks
-    if world > 1:
-        t = torch.tensor([ms_total, e2e_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total, e2e_ms = float(t[0]), float(t[1])
-    ms_per_step = ms_total / args.steps
-    value = world * args.steps / (ms_total * 1e-3)
-    e2e_value = world * 1e3 / e2e_ms
+    agg = aggregate_over_ranks(ms_total, e2e_ms, args.steps, world, device="cuda")
+    ms_total, e2e_ms = agg["ms_total"], agg["e2e_ms"]
+    ms_per_step, value, e2e_value = agg["ms_per_step"], agg["value"], agg["e2e_value"]
 
     if rank == 0:
         k4_ms = stage_ms["K4_absorb_a"] / nst

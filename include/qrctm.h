@@ -58,9 +58,12 @@ enum {
   QRCTM_OPT_GEMM_PATH = 4,   /* 0 = FP64 tensor-core (DMMA) tiles [default], 1 = plain DFMA reference kernel */
   QRCTM_OPT_TIME_STAGES = 5, /* 1 = qrctm_run records CUDA events around every stage of every step (default 0) */
   QRCTM_OPT_QR_PATH = 6,     /* 0 = blocked compact-WY QR, cluster panel kernel [default], 1 = level-2 column kernels */
-  QRCTM_OPT_OVERLAP_CHECK = 7 /* 1 [default] = qrctm_run overlaps the convergence check of step k (side stream) with
+  QRCTM_OPT_OVERLAP_CHECK = 7, /* 1 [default] = qrctm_run overlaps the convergence check of step k (side stream) with
                                 K1..K6 of step k+1; results are identical, Q/R/raw buffers then hold the factors of
                                 the last *started* iteration.  0 = strictly serial */
+  QRCTM_OPT_USE_GRAPH = 8    /* 1 [default] = K1..K6 and K7 are captured once into CUDA graphs and replayed by
+                                qrctm_step / qrctm_run (needs a non-default stream); 0 = plain launches, which keep
+                                the per-stage NVTX ranges for profilers */
 };
 
 /* Create a handle for dimensions (d, D, chi); allocates every workspace with

@@ -19,7 +19,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libqrctm.so")
 
 QRCTM_OK = 0
-OPT_CORNER_MODE, OPT_SYMMETRIZE, OPT_CHECK_EVERY, OPT_GEMM_PATH, OPT_TIME_STAGES, OPT_QR_PATH, OPT_OVERLAP_CHECK = 1, 2, 3, 4, 5, 6, 7
+OPT_CORNER_MODE, OPT_SYMMETRIZE, OPT_CHECK_EVERY, OPT_GEMM_PATH, OPT_TIME_STAGES, OPT_QR_PATH, OPT_OVERLAP_CHECK, OPT_USE_GRAPH = 1, 2, 3, 4, 5, 6, 7, 8
 NSTAGE = 7
 STAGE_NAMES = ("K1_reduced_corner", "K2_qr", "K3_half_absorb", "K4_absorb_a", "K5_project",
                "K6_corner", "K7_normalize")
@@ -108,10 +108,13 @@ class QRCTM:
     """Handle of one (d, D, chi) QR-CTMRG problem on the current CUDA device.
 
     Device workspace is a torch uint8 tensor (PyTorch owns device memory); work is
-    enqueued on torch's current stream at construction time.
+    enqueued on `self.stream`, a torch.cuda.Stream owned by the handle (a non-default
+    stream, so that the library can capture the step into CUDA graphs).  Calls that take
+    device tensors first make that stream wait for the caller's current stream; every
+    get_* / run / norm_per_site call synchronises before returning.
     """
 
-    def __init__(self, d: int, D: int, chi: int):
+    def __init__(self, d: int, D: int, chi: int, stream=None):
         import torch
         if not torch.cuda.is_available():
             raise QrctmError("no CUDA device: the QR-CTMRG path has no CPU fallback")
@@ -127,7 +130,9 @@ class QRCTM:
         if rc != QRCTM_OK:
             raise QrctmError(f"qrctm_create_in failed: {rc}")
         self._h = h
-        self._check(self.lib.qrctm_set_stream(h, c_void_p(torch.cuda.current_stream().cuda_stream)))
+        self.stream = stream if stream is not None else torch.cuda.Stream()
+        self.stream.wait_stream(torch.cuda.current_stream())
+        self._check(self.lib.qrctm_set_stream(h, c_void_p(self.stream.cuda_stream)))
 
     # -- plumbing
     def _check(self, rc: int):
@@ -154,15 +159,26 @@ class QRCTM:
         return np.empty(shape, dtype=np.float64)
 
     # -- the C ABI, same names
-    def set_stream(self, cuda_stream: int):
-        self._check(self.lib.qrctm_set_stream(self._h, c_void_p(cuda_stream)))
+    def set_stream(self, stream):
+        """stream: a torch.cuda.Stream"""
+        self.stream = stream
+        self._check(self.lib.qrctm_set_stream(self._h, c_void_p(stream.cuda_stream)))
+
+    def synchronize(self):
+        self.stream.synchronize()
+
+    def _order_after_caller(self):
+        import torch
+        self.stream.wait_stream(torch.cuda.current_stream())
 
     def set_A(self, A):
         assert tuple(A.shape) == (self.d,) + (self.D,) * 4
+        self._order_after_caller()
         self._check(self.lib.qrctm_set_A(self._h, _ptr(A)))
 
     def set_env(self, C, T):
         assert tuple(C.shape) == (self.chi, self.chi) and tuple(T.shape) == (self.chi, self.b, self.chi)
+        self._order_after_caller()
         self._check(self.lib.qrctm_set_env(self._h, _ptr(C), _ptr(T)))
 
     def step(self):

@@ -45,6 +45,9 @@ struct qrctm {
   long long launches;
   cudaEvent_t ev[QRCTM_NSTAGE + 2];
   bool have_ev;
+  cudaGraphExec_t g_front, g_k7;  // captured K1..K6 and K7 (replayed by step/run)
+  long long g_front_n, g_k7_n;    // kernels per replay
+  int use_graph, warm_steps, graph_failed;
   cudaStream_t side;            // high-priority stream for the overlapped convergence check
   cudaEvent_t ev_env, ev_spec;  // environment ready (main) / spectrum done (side)
   int overlap;
@@ -634,6 +637,63 @@ int do_step(qrctm* h, cudaEvent_t* ev /* QRCTM_NSTAGE+1 events or null */, bool 
   return rc;
 }
 
+void invalidate_graphs(qrctm* h) {
+  if (h->g_front) { cudaGraphExecDestroy(h->g_front); h->g_front = nullptr; }
+  if (h->g_k7) { cudaGraphExecDestroy(h->g_k7); h->g_k7 = nullptr; }
+  h->graph_failed = 0;
+}
+
+// Capture `body` (which only enqueues work on h->stream) into an executable graph.
+template <class F>
+bool capture_graph(qrctm* h, F body, cudaGraphExec_t* exec, long long* nlaunch) {
+  const long long l0 = h->launches;
+  if (cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeRelaxed) != cudaSuccess) { cudaGetLastError(); return false; }
+  const int rc = body();
+  cudaGraph_t graph = nullptr;
+  cudaError_t e = cudaStreamEndCapture(h->stream, &graph);
+  *nlaunch = h->launches - l0;
+  h->launches = l0;
+  if (rc != QRCTM_OK || e != cudaSuccess || !graph) { if (graph) cudaGraphDestroy(graph); cudaGetLastError(); return false; }
+  e = cudaGraphInstantiate(exec, graph, 0);
+  cudaGraphDestroy(graph);
+  if (e != cudaSuccess) { *exec = nullptr; cudaGetLastError(); return false; }
+  return true;
+}
+
+// K1..K6 (front) and K7, replayed from CUDA graphs once one ordinary step has run (so that all
+// one-time function attributes are set) -- unless events / NVTX ranges per stage are wanted.
+int run_front(qrctm* h, cudaEvent_t* ev) {
+  const bool can = h->use_graph && !ev && h->stream != nullptr && !h->graph_failed && h->warm_steps >= 1;
+  if (can && !h->g_front) {
+    if (!capture_graph(h, [&] { return do_step(h, nullptr, false); }, &h->g_front, &h->g_front_n)) h->graph_failed = 1;
+  }
+  if (can && h->g_front) {
+    CU(h, cudaGraphLaunch(h->g_front, h->stream));
+    h->launches += h->g_front_n;
+    return QRCTM_OK;
+  }
+  return do_step(h, ev, false);
+}
+
+int run_k7(qrctm* h, cudaEvent_t* ev) {
+  const bool can = h->use_graph && !ev && h->stream != nullptr && !h->graph_failed && h->warm_steps >= 1;
+  if (can && !h->g_k7) {
+    if (!capture_graph(h, [&] { return stage_normalize(h, h->Cn, h->Tn); }, &h->g_k7, &h->g_k7_n)) h->graph_failed = 1;
+  }
+  int rc;
+  if (can && h->g_k7) {
+    CU(h, cudaGraphLaunch(h->g_k7, h->stream));
+    h->launches += h->g_k7_n;
+    rc = QRCTM_OK;
+  } else {
+    if (ev) { nvtxRangePushA("K7_normalize"); cudaEventRecord(ev[6], h->stream); }
+    rc = stage_normalize(h, h->Cn, h->Tn);
+    if (ev) { cudaEventRecord(ev[7], h->stream); nvtxRangePop(); }
+  }
+  if (rc == QRCTM_OK) h->warm_steps += 1;
+  return rc;
+}
+
 int check_flag(qrctm* h) {   // stream must be synchronised by the caller's copy
   CU(h, cudaMemcpyAsync(h->h_flag, h->flag, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
   CU(h, cudaStreamSynchronize(h->stream));
@@ -666,7 +726,7 @@ static int create_common(int d, int D, int chi, void* ws, unsigned long long ws_
   memset(h, 0, sizeof(*h));
   h->d = d; h->D = D; h->b = D * D; h->chi = chi; h->m = (long long)chi * D * D;
   h->L = L; h->stream = 0;
-  h->corner_mode = 0; h->symmetrize = 1; h->check_every = 1; h->gemm_path = 0; h->overlap = 1;
+  h->corner_mode = 0; h->symmetrize = 1; h->check_every = 1; h->gemm_path = 0; h->overlap = 1; h->use_graph = 1;
   if (ws) {
     if (ws_bytes < L.total || (reinterpret_cast<uintptr_t>(ws) & (kAlign - 1)) || !is_device_ptr(ws)) {
       delete h; return QRCTM_ERR_INVALID_ARG;
@@ -712,6 +772,7 @@ int qrctm_create_in(int d, int D, int chi, void* workspace, unsigned long long w
 int qrctm_destroy(qrctm_t* h) {
   if (!h) return QRCTM_ERR_INVALID_ARG;
   cudaStreamSynchronize(h->stream);
+  invalidate_graphs(h);
   if (h->owns_ws && h->base) cudaFree(h->base);
   if (h->h_pinned) cudaFreeHost(h->h_pinned);
   if (h->side) { cudaStreamSynchronize(h->side); cudaStreamDestroy(h->side); cudaEventDestroy(h->ev_env); cudaEventDestroy(h->ev_spec); }
@@ -724,6 +785,7 @@ int qrctm_destroy(qrctm_t* h) {
 int qrctm_set_stream(qrctm_t* h, void* cuda_stream) {
   if (!h) return QRCTM_ERR_INVALID_ARG;
   CU(h, cudaStreamSynchronize(h->stream));
+  invalidate_graphs(h);
   h->stream = static_cast<cudaStream_t>(cuda_stream);
   return QRCTM_OK;
 }
@@ -758,7 +820,9 @@ int qrctm_set_env(qrctm_t* h, const double* C, const double* T) {
 int qrctm_step(qrctm_t* h) {
   if (!h) return QRCTM_ERR_INVALID_ARG;
   if (!h->have_A || !h->have_env) return fail(h, QRCTM_ERR_NOT_READY, "set_A and set_env first");
-  return do_step(h, nullptr);
+  if (!h->use_graph || h->stream == nullptr) { int rc0 = do_step(h, nullptr); if (!rc0) h->warm_steps += 1; return rc0; }
+  int rc = run_front(h, nullptr); if (rc) return rc;
+  return run_k7(h, nullptr);
 }
 
 int qrctm_run(qrctm_t* h, int max_iter, double tol, int* iters_done, double* final_delta) {
@@ -772,7 +836,7 @@ int qrctm_run(qrctm_t* h, int max_iter, double tol, int* iters_done, double* fin
     int done = 0;
     bool pending = false;                       // a spectrum result is in flight on the side stream
     for (int it = 1; it <= max_iter; ++it) {
-      int rc = do_step(h, nullptr, false); if (rc) return rc;
+      int rc = run_front(h, nullptr); if (rc) return rc;
       if (pending) {
         CU(h, cudaEventSynchronize(h->ev_spec));
         pending = false;
@@ -780,7 +844,7 @@ int qrctm_run(qrctm_t* h, int max_iter, double tol, int* iters_done, double* fin
         delta = h->h_pinned[0];
         if (delta < tol) break;                 // converged at step it-1: the half step in flight is discarded
       }
-      rc = stage_normalize(h, h->Cn, h->Tn); if (rc) return rc;
+      rc = run_k7(h, nullptr); if (rc) return rc;
       done = it;
       if (it % h->check_every == 0 || it == max_iter) {
         CU(h, cudaEventRecord(h->ev_env, h->stream));
@@ -811,6 +875,7 @@ int qrctm_run(qrctm_t* h, int max_iter, double tol, int* iters_done, double* fin
   }
   for (it = 1; it <= max_iter; ++it) {
     int rc = do_step(h, h->time_stages ? h->ev : nullptr); if (rc) return rc;
+    h->warm_steps += 1;
     const bool check = (it % h->check_every == 0 || it == max_iter);
     if (check) {
       rc = stage_spectrum(h, h->s, 1, h->stream); if (rc) return rc;
@@ -883,6 +948,8 @@ int qrctm_get_a(qrctm_t* h, double* a) {
 
 int qrctm_set_option(qrctm_t* h, int key, int value) {
   if (!h) return QRCTM_ERR_INVALID_ARG;
+  cudaStreamSynchronize(h->stream);
+  invalidate_graphs(h);
   switch (key) {
     case QRCTM_OPT_CORNER_MODE: if (value != 0 && value != 1) break; h->corner_mode = value; return QRCTM_OK;
     case QRCTM_OPT_SYMMETRIZE:  if (value != 0 && value != 1) break; h->symmetrize = value; return QRCTM_OK;
@@ -890,6 +957,7 @@ int qrctm_set_option(qrctm_t* h, int key, int value) {
     case QRCTM_OPT_GEMM_PATH:   if (value != 0 && value != 1) break; h->gemm_path = value; return QRCTM_OK;
     case QRCTM_OPT_QR_PATH:     if (value != 0 && value != 1) break; h->qr_path = value; return QRCTM_OK;
     case QRCTM_OPT_OVERLAP_CHECK: if (value != 0 && value != 1) break; h->overlap = value; return QRCTM_OK;
+    case QRCTM_OPT_USE_GRAPH:   if (value != 0 && value != 1) break; h->use_graph = value; return QRCTM_OK;
     case QRCTM_OPT_TIME_STAGES: if (value != 0 && value != 1) break; h->time_stages = value; return QRCTM_OK;
     default: break;
   }

@@ -21,6 +21,7 @@ def main():
     a = ap.parse_args()
     A, C0, T0, c = gen_named(a.config)
     h = pkg.QRCTM(c["d"], c["D"], c["chi"])
+    h.set_option(pkg.OPT_USE_GRAPH, 0)          # plain launches keep the NVTX stage ranges
     h.set_A(A)
     h.set_env(C0, T0)
     for _ in range(a.steps):
