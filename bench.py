@@ -234,6 +234,36 @@ def main():
     h.set_option(pkg.OPT_TIME_STAGES, 0)
     assert nst == args.steps
 
+    # ---- NEXT-1 variant: layered absorption, same result up to rounding, own flop count
+    layered = None
+    if chi % 2 == 0:
+        h.set_option(pkg.OPT_ABSORB_MODE, 1)
+        h.set_env(C0, T0)
+        h.run(args.warmup, -1.0)
+        torch.cuda.synchronize()
+        ev0.record(h.stream)
+        h.run(args.steps, -1.0)
+        ev1.record(h.stream)
+        torch.cuda.synchronize()
+        lay_ms = ev0.elapsed_time(ev1) / args.steps
+        h.set_option(pkg.OPT_TIME_STAGES, 1)
+        h.run(1, -1.0)
+        h.get_stage_ms(reset=True)
+        h.run(args.steps, -1.0)
+        lst, ln = h.get_stage_ms(reset=True)
+        h.set_option(pkg.OPT_TIME_STAGES, 0)
+        k4l = lst["K4_absorb_a"] / ln
+        fl_l = 4 * d * chi ** 2 * D ** 6
+        by_l = 8 * ((chi * b) ** 2 * 2 + 2 * d * b * chi * chi * b)      # P read, S written, P1 written + read
+        layered = {"value": 1e3 / lay_ms, "unit": UNIT, "ms_per_step": lay_ms, "k4_ms": k4l,
+                   "k4_algorithmic_gflop": fl_l / 1e9, "k4_tflops": fl_l / (k4l * 1e-3) / 1e12,
+                   "k4_algorithmic_gbytes": by_l / 1e9, "k4_gbs": by_l / (k4l * 1e-3) / 1e9,
+                   "note": "QRCTM_OPT_ABSORB_MODE=1: P contracted with the ket and bra copies of A in turn "
+                           "(4 d chi^2 D^6 flops instead of 2 chi^2 D^8); not the headline path"}
+        h.set_option(pkg.OPT_ABSORB_MODE, 0)
+        h.set_env(C0, T0)
+        h.run(2, -1.0)
+
     # ---- end to end through the C ABI with host buffers (pinned), copies inside the timed region
     Ah = torch.from_numpy(A).pin_memory()
     Ch, Th = torch.from_numpy(C0).pin_memory(), torch.from_numpy(T0).pin_memory()
@@ -301,6 +331,7 @@ def main():
                                         "(MEASURED_PEAKS.json has no FP64 entry; nominal 148 SM x 64 FMA/clk x 1.965 GHz = 37.2)",
                          "dfma_peak": peak_dfma, "algorithmic_flops_per_launch": fl["K4"], "ms_per_launch": k4_ms},
             "stages_ms": {k: v / nst for k, v in stage_ms.items()},
+            "next_1_layered": layered,
             "step_tflops": sum(fl.values()) / (ms_per_step * 1e-3) / 1e12,
             "step_frac_of_fp64_peak": sum(fl.values()) / (ms_per_step * 1e-3) / 1e12 / peak_dmma,
         }

@@ -61,9 +61,12 @@ enum {
   QRCTM_OPT_OVERLAP_CHECK = 7, /* 1 [default] = qrctm_run overlaps the convergence check of step k (side stream) with
                                 K1..K6 of step k+1; results are identical, Q/R/raw buffers then hold the factors of
                                 the last *started* iteration.  0 = strictly serial */
-  QRCTM_OPT_USE_GRAPH = 8    /* 1 [default] = K1..K6 and K7 are captured once into CUDA graphs and replayed by
+  QRCTM_OPT_USE_GRAPH = 8,   /* 1 [default] = K1..K6 and K7 are captured once into CUDA graphs and replayed by
                                 qrctm_step / qrctm_run (needs a non-default stream); 0 = plain launches, which keep
                                 the per-stage NVTX ranges for profilers */
+  QRCTM_OPT_ABSORB_MODE = 9  /* K4: 0 [default] = contract with the explicit double-layer tensor a (2 chi^2 D^8 flops),
+                                1 = layered: contract with the ket and the bra copy of A in turn (4 d chi^2 D^6
+                                flops; same T' up to rounding; needs even chi, otherwise mode 0 is used) */
 };
 
 /* Create a handle for dimensions (d, D, chi); allocates every workspace with

@@ -21,9 +21,15 @@
 
 namespace qk {
 
-struct IndexMap {          // idx -> (idx / div) * hi + (idx % div) * lo
+struct IndexMap {          // idx -> (idx / div) * hi + ((idx % div) / div0) * lo + (idx % div0) * lo0
   int div;
   long long hi, lo;
+  int div0 = 1;            // third level (default: none)
+  long long lo0 = 0;
+  __host__ __device__ long long operator()(int idx) const {
+    const int r = idx % div;
+    return (long long)(idx / div) * hi + (long long)(r / div0) * lo + (long long)(r % div0) * lo0;
+  }
 };
 __host__ __device__ inline IndexMap plain_map(long long ld) { return IndexMap{1, ld, 0}; }
 
@@ -37,6 +43,15 @@ struct GemmArgs {
   long long split_stride;    // elements between partial outputs (split-K only)
   int mode;                  // 0: out = acc, 1: out = out - acc, 2: out = out + acc
   int vecA, vecB;            // 16-byte cp.async legal for A / B
+  // transA = 1 only: logical k-row r of A lives at row ka(r) of the stored matrix (default identity)
+  IndexMap ka = IndexMap{1, 1, 0};
+  // batched launch (gridDim.z = batch, no split-K): A += za(z) elements, out += z * zo elements
+  int batch = 0;
+  IndexMap za = IndexMap{1, 0, 0};
+  long long zo = 0;
+  int nz = 1;                // number of z slices (splits or batches) -- work list of the ws kernel
+  int epi = 0;               // ws kernel epilogue: 0 = fragments straight to global, 1 = staged through shared
+                             // memory so that the 32 lanes of a store run along the column index j
 };
 
 constexpr int BK = 16;
@@ -176,14 +191,14 @@ gemm_f64_dmma(GemmArgs p) {
   for (int i = 0; i < FM; ++i) {
     int r = m0 + wm0 + i * 8 + lr;
     if (r >= p.M) continue;
-    long long roff = (long long)(r / p.ro.div) * p.ro.hi + (long long)(r % p.ro.div) * p.ro.lo;
+    long long roff = p.ro(r);
 #pragma unroll
     for (int j = 0; j < FN; ++j) {
 #pragma unroll
       for (int e = 0; e < 2; ++e) {
         int c = n0 + wn0 + j * 8 + 2 * lc + e;
         if (c < p.N) {
-          long long off = roff + (long long)(c / p.co.div) * p.co.hi + (long long)(c % p.co.div) * p.co.lo;
+          long long off = roff + p.co(c);
           double v = acc[i][j][e];
           if (p.mode == 1) v = out[off] - v;
           else if (p.mode == 2) v = out[off] + v;
@@ -247,12 +262,12 @@ gemm_f64_dmma_ws(GemmArgs p) {
   uint64_t* empty = full + STAGES;
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int m0 = blockIdx.y * BM, n0 = blockIdx.x * BN;
+  // Persistent CTA: work items w = (z, tile_m, tile_n), tile_n fastest; the smem ring and its
+  // mbarrier phases run on across work items, so the producer prefetches the next tile while the
+  // consumers are still storing the previous one.
+  const int tn = (p.N + BN - 1) / BN, tm = (p.M + BM - 1) / BM;
+  const long long nwork = (long long)tn * tm * p.nz;
   const int nkt_total = (p.K + BK - 1) / BK;
-  const int kt_begin = blockIdx.z * p.ktiles_per_split;
-  int kt_end = kt_begin + p.ktiles_per_split;
-  if (kt_end > nkt_total) kt_end = nkt_total;
-  const int nkt = kt_end > kt_begin ? kt_end - kt_begin : 0;
 
   if (tid == 0) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, NCW); }
@@ -262,28 +277,36 @@ gemm_f64_dmma_ws(GemmArgs p) {
 
   if (warp == NCW) {
     // ------------------------------ producer warp
-    int wA = p.M - m0; if (wA > BM) wA = BM; wA = (wA + 1) & ~1;
-    int wB = p.N - n0; if (wB > BN) wB = BN; wB = (wB + 1) & ~1;
     const int row = lane & 15;
     const bool isB = lane >= 16;
-    const double* src = isB ? p.B + (long long)row * p.ldb + n0 : p.A + (long long)row * p.lda + m0;
-    src += (long long)kt_begin * BK * (isB ? p.ldb : p.lda);
-    const long long step = (long long)BK * (isB ? p.ldb : p.lda);
-    const uint32_t bytes = (uint32_t)(isB ? wB : wA) * 8u;
     const int srow = isB ? row * LDB_S : row * LDA_S;
-    for (int kt = 0; kt < nkt; ++kt, src += step) {
-      const int stage = kt % STAGES, round = kt / STAGES;
-      if (round > 0) mbar_wait(empty + stage, (round - 1) & 1);
-      int krows = p.K - (kt_begin + kt) * BK; if (krows > BK) krows = BK;
-      double* dst = (isB ? Bs + stage * B_STAGE : As + stage * A_STAGE) + srow;
-      if (row >= krows) {                         // ragged K: zero rows (last tile only)
-        const int w = isB ? BN : BM;
-        for (int c = 0; c < w; ++c) dst[c] = 0.0;
+    int it = 0;                                   // k-tiles issued so far by this CTA (ring position)
+    for (long long w = blockIdx.x; w < nwork; w += gridDim.x) {
+      const int z = (int)(w / ((long long)tn * tm));
+      const int rem = (int)(w % ((long long)tn * tm));
+      const int m0 = (rem / tn) * BM, n0 = (rem % tn) * BN;
+      const int kt_begin = p.batch ? 0 : z * p.ktiles_per_split;
+      int kt_end = kt_begin + p.ktiles_per_split; if (kt_end > nkt_total) kt_end = nkt_total;
+      const double* Abase = p.A + (p.batch ? p.za(z) : 0);
+      int wA = p.M - m0; if (wA > BM) wA = BM; wA = (wA + 1) & ~1;
+      int wB = p.N - n0; if (wB > BN) wB = BN; wB = (wB + 1) & ~1;
+      const uint32_t bytes = (uint32_t)(isB ? wB : wA) * 8u;
+      for (int kt = kt_begin; kt < kt_end; ++kt, ++it) {
+        const int stage = it % STAGES, round = it / STAGES;
+        if (round > 0) mbar_wait(empty + stage, (round - 1) & 1);
+        const int kr = kt * BK + row;                                 // logical k-row of this lane
+        int krows = p.K - kt * BK; if (krows > BK) krows = BK;
+        const double* src = isB ? p.B + (long long)kr * p.ldb + n0 : Abase + p.ka(kr) * p.lda + m0;
+        double* dst = (isB ? Bs + stage * B_STAGE : As + stage * A_STAGE) + srow;
+        if (row >= krows) {                         // ragged K: zero rows (last tile only)
+          const int wz = isB ? BN : BM;
+          for (int c = 0; c < wz; ++c) dst[c] = 0.0;
+        }
+        __syncwarp();
+        if (lane == 0) mbar_expect_tx(full + stage, (uint32_t)krows * (uint32_t)(wA + wB) * 8u);
+        __syncwarp();
+        if (row < krows) bulk_g2s(dst, src, bytes, full + stage);
       }
-      __syncwarp();
-      if (lane == 0) mbar_expect_tx(full + stage, (uint32_t)krows * (uint32_t)(wA + wB) * 8u);
-      __syncwarp();
-      if (row < krows) bulk_g2s(dst, src, bytes, full + stage);
     }
     return;
   }
@@ -291,66 +314,122 @@ gemm_f64_dmma_ws(GemmArgs p) {
   // -------------------------------- consumer warps
   const int wm0 = (warp / NW_N) * WM, wn0 = (warp % NW_N) * WN;
   const int lr = lane >> 2, lc = lane & 3;
-  double acc[FM][FN][2];
-#pragma unroll
-  for (int i = 0; i < FM; ++i)
-#pragma unroll
-    for (int j = 0; j < FN; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+  int it = 0;
+  for (long long w = blockIdx.x; w < nwork; w += gridDim.x) {
+    const int z = (int)(w / ((long long)tn * tm));
+    const int rem = (int)(w % ((long long)tn * tm));
+    const int m0 = (rem / tn) * BM, n0 = (rem % tn) * BN;
+    const int kt_begin = p.batch ? 0 : z * p.ktiles_per_split;
+    int kt_end = kt_begin + p.ktiles_per_split; if (kt_end > nkt_total) kt_end = nkt_total;
 
-  for (int kt = 0; kt < nkt; ++kt) {
-    const int stage = kt % STAGES, round = kt / STAGES;
-    mbar_wait(full + stage, round & 1);
-    const double* as = As + stage * A_STAGE + wm0 + lr + lc * LDA_S;
-    const double* bs = Bs + stage * B_STAGE + wn0 + lr + lc * LDB_S;
-    int krows = p.K - (kt_begin + kt) * BK;
-    if (krows >= BK) {
+    double acc[FM][FN][2];
 #pragma unroll
-      for (int ks = 0; ks < BK / 4; ++ks) {
-        double af[FM], bf[FN];
+    for (int i = 0; i < FM; ++i)
 #pragma unroll
-        for (int i = 0; i < FM; ++i) af[i] = as[ks * 4 * LDA_S + i * 8];
+      for (int j = 0; j < FN; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+    for (int kt = kt_begin; kt < kt_end; ++kt, ++it) {
+      const int stage = it % STAGES, round = it / STAGES;
+      mbar_wait(full + stage, round & 1);
+      const double* as = As + stage * A_STAGE + wm0 + lr + lc * LDA_S;
+      const double* bs = Bs + stage * B_STAGE + wn0 + lr + lc * LDB_S;
+      const int krows = p.K - kt * BK;
+      if (krows >= BK) {
 #pragma unroll
-        for (int j = 0; j < FN; ++j) bf[j] = bs[ks * 4 * LDB_S + j * 8];
+        for (int ks = 0; ks < BK / 4; ++ks) {
+          double af[FM], bf[FN];
 #pragma unroll
-        for (int i = 0; i < FM; ++i)
+          for (int i = 0; i < FM; ++i) af[i] = as[ks * 4 * LDA_S + i * 8];
 #pragma unroll
-          for (int j = 0; j < FN; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+          for (int j = 0; j < FN; ++j) bf[j] = bs[ks * 4 * LDB_S + j * 8];
+#pragma unroll
+          for (int i = 0; i < FM; ++i)
+#pragma unroll
+            for (int j = 0; j < FN; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+        }
+      } else {
+        const int ksteps = (krows + 3) >> 2;
+        for (int ks = 0; ks < ksteps; ++ks) {
+          double af[FM], bf[FN];
+#pragma unroll
+          for (int i = 0; i < FM; ++i) af[i] = as[ks * 4 * LDA_S + i * 8];
+#pragma unroll
+          for (int j = 0; j < FN; ++j) bf[j] = bs[ks * 4 * LDB_S + j * 8];
+#pragma unroll
+          for (int i = 0; i < FM; ++i)
+#pragma unroll
+            for (int j = 0; j < FN; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+        }
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(empty + stage);
+    }
+
+    double* out = p.out + (p.batch ? (long long)z * p.zo : (long long)z * p.split_stride);
+    if (p.epi == 1) {
+      // staged: 8 rows x WN columns of this warp go through its private shared-memory slab, then every
+      // store instruction writes 32 consecutive columns of one row (coalesced wherever co() is contiguous)
+      constexpr int SP = WN + 4, NCH = (WN + 31) / 32;
+      double* stg = reinterpret_cast<double*>(empty + STAGES) + warp * (8 * SP);
+      long long coffL[NCH];
+#pragma unroll
+      for (int q = 0; q < NCH; ++q) {
+        const int cl = q * 32 + lane, c = n0 + wn0 + cl;
+        coffL[q] = (cl < WN && c < p.N) ? p.co(c) : -1;
+      }
+#pragma unroll
+      for (int i = 0; i < FM; ++i) {
+        const int rbase = m0 + wm0 + i * 8;
+        const long long myro = (lane < 8 && rbase + lane < p.M) ? p.ro(rbase + lane) : -1;
+#pragma unroll
+        for (int j = 0; j < FN; ++j) {
+          double2 v2 = make_double2(acc[i][j][0], acc[i][j][1]);
+          *reinterpret_cast<double2*>(stg + lr * SP + j * 8 + 2 * lc) = v2;
+        }
+        __syncwarp();
+#pragma unroll
+        for (int rr = 0; rr < 8; ++rr) {
+          const long long roff = __shfl_sync(0xffffffffu, myro, rr);
+          if (roff < 0) continue;
+#pragma unroll
+          for (int q = 0; q < NCH; ++q) {
+            if (coffL[q] >= 0) {
+              const long long off = roff + coffL[q];
+              double v = stg[rr * SP + q * 32 + lane];
+              if (p.mode == 1) v = out[off] - v;
+              else if (p.mode == 2) v = out[off] + v;
+              out[off] = v;
+            }
+          }
+        }
+        __syncwarp();
       }
     } else {
-      const int ksteps = (krows + 3) >> 2;
-      for (int ks = 0; ks < ksteps; ++ks) {
-        double af[FM], bf[FN];
+      long long coff[FN][2];
 #pragma unroll
-        for (int i = 0; i < FM; ++i) af[i] = as[ks * 4 * LDA_S + i * 8];
+      for (int j = 0; j < FN; ++j)
 #pragma unroll
-        for (int j = 0; j < FN; ++j) bf[j] = bs[ks * 4 * LDB_S + j * 8];
+        for (int e = 0; e < 2; ++e) {
+          const int c = n0 + wn0 + j * 8 + 2 * lc + e;
+          coff[j][e] = c < p.N ? p.co(c) : -1;
+        }
 #pragma unroll
-        for (int i = 0; i < FM; ++i)
+      for (int i = 0; i < FM; ++i) {
+        const int r = m0 + wm0 + i * 8 + lr;
+        if (r >= p.M) continue;
+        const long long roff = p.ro(r);
 #pragma unroll
-          for (int j = 0; j < FN; ++j) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
-      }
-    }
-    __syncwarp();
-    if (lane == 0) mbar_arrive(empty + stage);
-  }
-
-  double* out = p.out + (long long)blockIdx.z * p.split_stride;
+        for (int j = 0; j < FN; ++j) {
 #pragma unroll
-  for (int i = 0; i < FM; ++i) {
-    int r = m0 + wm0 + i * 8 + lr;
-    if (r >= p.M) continue;
-    long long roff = (long long)(r / p.ro.div) * p.ro.hi + (long long)(r % p.ro.div) * p.ro.lo;
-#pragma unroll
-    for (int j = 0; j < FN; ++j) {
-#pragma unroll
-      for (int e = 0; e < 2; ++e) {
-        int c = n0 + wn0 + j * 8 + 2 * lc + e;
-        if (c < p.N) {
-          long long off = roff + (long long)(c / p.co.div) * p.co.hi + (long long)(c % p.co.div) * p.co.lo;
-          double v = acc[i][j][e];
-          if (p.mode == 1) v = out[off] - v;
-          else if (p.mode == 2) v = out[off] + v;
-          out[off] = v;
+          for (int e = 0; e < 2; ++e) {
+            if (coff[j][e] >= 0) {
+              const long long off = roff + coff[j][e];
+              double v = acc[i][j][e];
+              if (p.mode == 1) v = out[off] - v;
+              else if (p.mode == 2) v = out[off] + v;
+              out[off] = v;
+            }
+          }
         }
       }
     }
@@ -363,16 +442,17 @@ __global__ void gemm_f64_ref(GemmArgs p) {
   long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= (long long)p.M * p.N) return;
   int i = (int)(idx / p.N), j = (int)(idx % p.N);
+  const double* A = p.A + (p.batch ? p.za((int)blockIdx.z) : 0);
+  double* out = p.out + (p.batch ? (long long)blockIdx.z * p.zo : 0);
   double s = 0.0;
   for (int k = 0; k < p.K; ++k) {
-    double a = p.transA ? p.A[(long long)k * p.lda + i] : p.A[(long long)i * p.lda + k];
+    double a = p.transA ? A[p.ka(k) * p.lda + i] : A[(long long)i * p.lda + k];
     s = fma(a, p.B[(long long)k * p.ldb + j], s);
   }
-  long long off = (long long)(i / p.ro.div) * p.ro.hi + (long long)(i % p.ro.div) * p.ro.lo +
-                  (long long)(j / p.co.div) * p.co.hi + (long long)(j % p.co.div) * p.co.lo;
-  if (p.mode == 1) s = p.out[off] - s;
-  else if (p.mode == 2) s = p.out[off] + s;
-  p.out[off] = s;
+  long long off = p.ro(i) + p.co(j);
+  if (p.mode == 1) s = out[off] - s;
+  else if (p.mode == 2) s = out[off] + s;
+  out[off] = s;
 }
 
 // out[ro(i)+co(j)] (op)= sum_z part[z][i][j], z ascending (fixed order).
@@ -391,8 +471,7 @@ __global__ void reduce_splitk(const double* part, long long split_stride, int sp
     for (int u = 0; u < 8; ++u) s += v[u];
   }
   for (; z < splits; ++z) s += part[(long long)z * split_stride + idx];
-  long long off = (long long)(i / ro.div) * ro.hi + (long long)(i % ro.div) * ro.lo +
-                  (long long)(j / co.div) * co.hi + (long long)(j % co.div) * co.lo;
+  long long off = ro(i) + co(j);
   if (mode == 1) s = out[off] - s;
   else if (mode == 2) s = out[off] + s;
   out[off] = s;

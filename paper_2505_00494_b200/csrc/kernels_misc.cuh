@@ -69,6 +69,22 @@ __global__ void build_a_kernel(const double* __restrict__ A, int d, int D, doubl
   }
 }
 
+// Re-laid-out copies of A for the layered absorption (NEXT-1):
+//   B1[(u_k,l_k)][(s,d_k,r_k)] = A[s,u_k,l_k,d_k,r_k]   (D^2 x d D^2, leading dimension ld1)
+//   B2[(s,u_b,l_b)][(d_b,r_b)] = A[s,u_b,l_b,d_b,r_b]   (d D^2 x D^2, leading dimension ld2)
+__global__ void build_layers_kernel(const double* __restrict__ A, int d, int D, double* __restrict__ B1,
+                                    long long ld1, double* __restrict__ B2, long long ld2) {
+  const long long n = (long long)d * D * D * D * D;
+  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < n;
+       idx += (long long)gridDim.x * blockDim.x) {
+    int r = (int)(idx % D), dd = (int)((idx / D) % D), l = (int)((idx / (D * D)) % D),
+        u = (int)((idx / ((long long)D * D * D)) % D), sidx = (int)(idx / ((long long)D * D * D * D));
+    const double v = A[idx];
+    B1[((long long)u * D + l) * ld1 + ((long long)sidx * D + dd) * D + r] = v;
+    B2[(((long long)sidx * D + u) * D + l) * ld2 + (long long)dd * D + r] = v;
+  }
+}
+
 // ---------------------------------------------------------------- K7
 // Pass 1: dst = sym(src) (or copy), per-block partial sums of squares in a fixed
 // order.  C part: n x n matrix.  T part: (chi, b, chi) swapping the chi legs.

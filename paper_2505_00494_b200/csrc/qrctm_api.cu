@@ -25,9 +25,9 @@ constexpr size_t kAlign = 256;
 inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {   // byte offsets into the workspace
-  size_t A, a_mat, C, T, Cn, Tn, X, V, Q, R, tau, P, S, W, E, splitk, partial, scal, flag, Wc, dvec, evec,
+  size_t A, a_mat, B1, B2, P1, C, T, Cn, Tn, X, V, Q, R, tau, P, S, W, E, splitk, partial, scal, flag, Wc, dvec, evec,
       vv, pv, eig, s, s_prev, s_tmp, delta, qrwork, total;
-  long long lda_a;
+  long long lda_a, ld1, ld2;
   size_t splitk_elems, qrwork_bytes;
 };
 
@@ -41,7 +41,7 @@ struct qrctm {
   bool owns_ws;
   Layout L;
   bool have_A, have_env;
-  int corner_mode, symmetrize, check_every, gemm_path, time_stages, qr_path;
+  int corner_mode, symmetrize, check_every, gemm_path, time_stages, qr_path, absorb_mode;
   long long launches;
   cudaEvent_t ev[QRCTM_NSTAGE + 2];
   bool have_ev;
@@ -57,7 +57,7 @@ struct qrctm {
   double* h_pinned;       // [0] delta, [1..] scratch ; pinned host
   int* h_flag;
   // typed views
-  double *A, *a_mat, *C, *T, *Cn, *Tn, *X, *V, *Q, *R, *tau, *P, *S, *W, *E, *splitk, *partial, *scal, *Wc,
+  double *A, *a_mat, *B1, *B2, *P1, *C, *T, *Cn, *Tn, *X, *V, *Q, *R, *tau, *P, *S, *W, *E, *splitk, *partial, *scal, *Wc,
       *dvec, *evec, *vv, *pv, *eig, *s, *s_prev, *s_tmp, *delta;
   int* flag;
   void* qrwork;
@@ -78,6 +78,11 @@ bool make_layout(int d, int D, int chi, Layout* L) {
   const size_t dbl = sizeof(double);
   L->A = take(dbl * d * b2);
   L->a_mat = take(dbl * b2 * L->lda_a);
+  L->ld1 = ((long long)d * b + 15) / 16 * 16;
+  L->ld2 = (b + 15) / 16 * 16;
+  L->B1 = take(dbl * b * L->ld1);
+  L->B2 = take(dbl * d * b * L->ld2);
+  L->P1 = take(dbl * (size_t)d * b * (size_t)chi * chi * b);
   L->C = take(dbl * chi * chi);
   L->T = take(dbl * m * chi);
   L->Cn = take(dbl * chi * chi);
@@ -116,7 +121,7 @@ void bind_views(qrctm* h) {
   char* B = h->base;
   const Layout& L = h->L;
 #define V_(name) h->name = reinterpret_cast<double*>(B + L.name)
-  V_(A); V_(a_mat); V_(C); V_(T); V_(Cn); V_(Tn); V_(X); V_(V); V_(Q); V_(R); V_(tau); V_(P); V_(S); V_(W);
+  V_(A); V_(a_mat); V_(B1); V_(B2); V_(P1); V_(C); V_(T); V_(Cn); V_(Tn); V_(X); V_(V); V_(Q); V_(R); V_(tau); V_(P); V_(S); V_(W);
   V_(E); V_(splitk); V_(partial); V_(scal); V_(Wc); V_(dvec); V_(evec); V_(vv); V_(pv); V_(eig); V_(s);
   V_(s_prev); V_(s_tmp); V_(delta);
 #undef V_
@@ -178,7 +183,8 @@ cudaError_t launch_cfg(cudaStream_t st, const GemmArgs& g, int splits) {
 template <int BM, int BN, int WM, int WN, int STAGES>
 cudaError_t launch_cfg_ws(cudaStream_t st, const GemmArgs& g, int splits) {
   constexpr int NT = ((BM / WM) * (BN / WN) + 1) * 32;
-  constexpr size_t smem = sizeof(double) * STAGES * BK * ((BM + PAD) + (BN + PAD)) + 2 * STAGES * sizeof(uint64_t);
+  constexpr size_t smem = sizeof(double) * STAGES * BK * ((BM + PAD) + (BN + PAD)) + 2 * STAGES * sizeof(uint64_t) +
+                          sizeof(double) * (BM / WM) * (BN / WN) * 8 * (WN + 4);     // + per-warp epilogue slabs
   static bool attr_done = false;
   if (!attr_done) {
     cudaError_t e = cudaFuncSetAttribute(gemm_f64_dmma_ws<BM, BN, WM, WN, STAGES>,
@@ -186,8 +192,20 @@ cudaError_t launch_cfg_ws(cudaStream_t st, const GemmArgs& g, int splits) {
     if (e != cudaSuccess) return e;
     attr_done = true;
   }
-  dim3 grid((g.N + BN - 1) / BN, (g.M + BM - 1) / BM, splits);
-  gemm_f64_dmma_ws<BM, BN, WM, WN, STAGES><<<grid, NT, smem, st>>>(g);
+  static int nslots = 0;
+  if (!nslots) {
+    int dev = 0, nsm = 148, per = 1;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, gemm_f64_dmma_ws<BM, BN, WM, WN, STAGES>, NT, smem);
+    nslots = nsm * (per > 0 ? per : 1);
+  }
+  GemmArgs ga = g;
+  ga.nz = splits;
+  const long long nwork = (long long)((g.N + BN - 1) / BN) * ((g.M + BM - 1) / BM) * splits;
+  (void)nslots;                                  // one work item per CTA: the hardware scheduler balances better
+  const unsigned grid = (unsigned)nwork;         // than a static persistent loop (measured)
+  gemm_f64_dmma_ws<BM, BN, WM, WN, STAGES><<<grid, NT, smem, st>>>(ga);
   return cudaGetLastError();
 }
 
@@ -197,6 +215,11 @@ struct GemmCall {
   double* out; IndexMap ro, co;
   int M, N, K;
   int mode;   // 0 store, 1 out -= , 2 out +=
+  IndexMap ka = IndexMap{1, 1, 0};     // k-row map of A (transA = 1)
+  int batch = 0;                       // > 0: gridDim.z batches, A += za(z), out += z * zo
+  IndexMap za = IndexMap{1, 0, 0};
+  long long zo = 0;
+  int epi = 0;                         // 1: shared-memory staged epilogue (outputs contiguous along the column index)
 };
 
 // Returns number of kernels launched (>0) or -1 on error (err set).
@@ -207,6 +230,7 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
   GemmArgs g;
   g.A = c.A; g.lda = c.lda; g.transA = c.transA; g.B = c.B; g.ldb = c.ldb; g.out = c.out;
   g.ro = c.ro; g.co = c.co; g.M = c.M; g.N = c.N; g.K = c.K; g.mode = c.mode;
+  g.ka = c.ka; g.batch = c.batch > 0 ? 1 : 0; g.za = c.za; g.zo = c.zo; g.epi = c.epi;
   g.vecA = c.transA && (c.lda % 2 == 0) && ((reinterpret_cast<uintptr_t>(c.A) & 15) == 0);
   g.vecB = (c.ldb % 2 == 0) && ((reinterpret_cast<uintptr_t>(c.B) & 15) == 0);
   g.split_stride = 0;
@@ -214,7 +238,7 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
   g.ktiles_per_split = nkt > 0 ? nkt : 1;
   if (path == 1) {
     long long n = (long long)c.M * c.N;
-    gemm_f64_ref<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(g);
+    gemm_f64_ref<<<dim3((unsigned)((n + 255) / 256), 1, c.batch > 0 ? c.batch : 1), 256, 0, st>>>(g);
     *err = cudaGetLastError();
     return *err == cudaSuccess ? 1 : -1;
   }
@@ -224,16 +248,28 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
   const bool ws_ok = g.transA && g.vecA && g.vecB;     // bulk copies need 16-byte aligned rows
   int splits = 1;
   int cfg = 0;          // 0: 64x64 cp.async, 1: 128x128 cp.async, 2: ws 128x128, 3: ws 128x104, 4: ws 128x64 (2 CTA/SM)
-  const bool ws_big = ws_ok && c.M >= 96 && c.N >= 96 && (double)c.M * c.N * c.K > 2.0e8;
+  const bool ws_big = ws_ok && c.M >= 96 && c.N >= 32 && (double)c.M * c.N * c.K > 2.0e8;
+  if (c.batch > 0) {
+    // batched launch (layered absorption): bulk-copy kernel only, one batch per gridDim.z, no split-K
+    if (!ws_ok) { *err = cudaErrorInvalidValue; return -1; }
+    const int pad128 = (c.N + 127) / 128 * 128, pad104 = (c.N + 103) / 104 * 104, pad64 = (c.N + 63) / 64 * 64;
+    if (c.N <= 56) *err = launch_cfg_ws<128, 56, 32, 56, 3>(st, g, c.batch);
+    else if (pad64 <= pad104 && pad64 <= pad128) *err = launch_cfg_ws<128, 64, 64, 32, 4>(st, g, c.batch);
+    else if (pad104 <= pad128) *err = launch_cfg_ws<128, 104, 16, 104, 4>(st, g, c.batch);
+    else *err = launch_cfg_ws<128, 128, 64, 32, 4>(st, g, c.batch);
+    return *err == cudaSuccess ? 1 : -1;
+  }
   if (ws_big) {
     // pick the N tile with the least padding, then split K so that the CTAs fill whole waves
     auto padded = [&](int bn) { return (long long)((c.N + bn - 1) / bn) * bn; };
     int bn = 128; cfg = 2;
-    if (nkt <= 32 && c.N >= 1024) { bn = 64; cfg = 4; }        // short K: two CTAs per SM overlap epilogue and mainloop
+    if (c.N <= 56) { bn = 56; cfg = 5; }                       // narrow N (layered absorption, N = D^2)
+    else if (c.N <= 64) { bn = 64; cfg = 4; }
+    else if (nkt <= 32 && c.N >= 1024) { bn = 64; cfg = 4; }   // short K: two CTAs per SM overlap epilogue and mainloop
     else if (padded(104) * 100 < padded(128) * 97) { bn = 104; cfg = 3; }
     const long long tiles = (long long)((c.M + 127) / 128) * ((c.N + bn - 1) / bn);
-    const int slots = cfg == 4 ? 296 : 148;
-    const double t_kt = 2.1e-6 * bn / 128.0 * (cfg == 4 ? 2.0 : 1.0), t_fix = 4e-6;
+    const int slots = (cfg == 4 || cfg == 5) ? 296 : 148;
+    const double t_kt = 2.1e-6 * bn / 128.0 * ((cfg == 4 || cfg == 5) ? 2.0 : 1.0), t_fix = 4e-6;
     double best = 1e30;
     for (int sp = 1; sp <= 64; ++sp) {
       int per = (nkt + sp - 1) / sp;
@@ -265,6 +301,7 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
     case 2: *err = launch_cfg_ws<128, 128, 64, 32, 4>(st, g, splits); break;
     case 3: *err = launch_cfg_ws<128, 104, 16, 104, 4>(st, g, splits); break;
     case 4: *err = launch_cfg_ws<128, 64, 64, 32, 4>(st, g, splits); break;
+    case 5: *err = launch_cfg_ws<128, 56, 32, 56, 3>(st, g, splits); break;
     case 1: *err = launch_cfg<128, 128, 64, 32, 4>(st, g, splits); break;
     default: *err = launch_cfg<64, 64, 32, 32, 4>(st, g, splits); break;
   }
@@ -512,25 +549,53 @@ int stage_reduced_corner(qrctm* h, const double* C, const double* T, double* X) 
   return QRCTM_OK;
 }
 
-// K3: P'[u,l,m,J] = sum_j Qm[j,u,m] T[j,l,J]        (Qm: chi*b x n viewed chi x b*n)
+// K3: P'[u,l,J,m] = sum_j Qm[j,u,m] T[j,l,J]        (Qm: chi*b x n viewed chi x b*n).  m innermost: the
+// consecutive rows of a K4 tile (M index (J,m)) are then adjacent in K4's outputs.
 int stage_half_absorb(qrctm* h, const double* Qm, const double* T, double* P) {
   const int chi = h->chi, b = h->b; const long long bc = (long long)b * chi, cc = (long long)chi * chi;
-  GemmCall c{Qm, bc, 1, T, bc, P, IndexMap{chi, b * cc, chi}, IndexMap{chi, cc, 1}, (int)bc, (int)bc, chi, 0};
+  GemmCall c{Qm, bc, 1, T, bc, P, IndexMap{chi, b * cc, 1}, IndexMap{chi, cc, chi}, (int)bc, (int)bc, chi, 0};
   GEMM(h, c);
   return QRCTM_OK;
 }
 
-// K4: S[m,J,d,r] = sum_{u,l} P'[(u,l),(m,J)] a[(u,l),(d,r)]
+// K4: S[m,J,d,r] = sum_{u,l} P'[(u,l),(J,m)] a[(u,l),(d,r)]      (GEMM row index i = J*chi + m)
 //   layout 0: S''[J,d,m,r]  (what K5 wants: K x M with K = (J,d))
 //   layout 1: S~ [m,r,J,d]  (what the kappa network wants: K = (m,r))
 //   layout 2: C~[(J,d),(m,r)] natural enlarged-corner matrix == layout 0
 int stage_absorb_a(qrctm* h, const double* P, double* S, int layout) {
   const int chi = h->chi, b = h->b; const long long m = h->m, cc = (long long)chi * chi;
   IndexMap ro, co;
-  if (layout == 0) { ro = IndexMap{chi, b, (long long)b * m}; co = IndexMap{b, m, 1}; }
-  else             { ro = IndexMap{chi, (long long)b * m, b}; co = IndexMap{b, 1, (long long)chi * b}; }
+  if (layout == 0) { ro = IndexMap{chi, (long long)b * m, b}; co = IndexMap{b, m, 1}; }
+  else             { ro = IndexMap{chi, b, (long long)b * m}; co = IndexMap{b, 1, (long long)chi * b}; }
   GemmCall c{P, cc, 1, h->a_mat, h->L.lda_a, S, ro, co, (int)cc, b * b, b * b, 0};
+  c.epi = 1;
   GEMM(h, c);
+  return QRCTM_OK;
+}
+
+// K4 layered (NEXT-1): the same S'' without ever using the double-layer tensor,
+//   P1[(s,u_b,l_b)][J,d_k,m,r_k] = sum_{u_k,l_k} P'[(u_k u_b),(l_k l_b),J,m] A[s,u_k,l_k,d_k,r_k]   (D^2 batched GEMMs, K = D^2)
+//   S''[J,(d_k d_b),m,(r_k r_b)] = sum_{s,u_b,l_b} P1[(s,u_b,l_b)][J,d_k,m,r_k] A[s,u_b,l_b,d_b,r_b]  (K = d D^2)
+// 4 d chi^2 D^6 flops instead of 2 chi^2 D^8.  Needs even chi (16-byte aligned rows for the bulk copies).
+bool layered_ok(const qrctm* h) { return h->chi % 2 == 0; }
+
+int stage_absorb_layered(qrctm* h, const double* P, double* S) {
+  const int chi = h->chi, D = h->D, b = h->b, d = h->d;
+  const long long m = h->m, cc = (long long)chi * chi, M2 = cc * b;
+  GemmCall g1{P, cc, 1, h->B1, h->L.ld1, h->P1,
+              IndexMap{chi, (long long)D * chi * D, D},
+              IndexMap{D * D, (long long)b * M2, (long long)chi * D, D, 1},
+              (int)cc, d * b, b, 0};
+  g1.ka = IndexMap{D, (long long)D * b, D};
+  g1.batch = b;
+  g1.za = IndexMap{D, (long long)b * cc, cc};
+  g1.zo = M2;
+  g1.epi = 1;
+  GEMM(h, g1);
+  GemmCall g2{h->P1, M2, 1, h->B2, h->L.ld2, S, IndexMap{chi * D, (long long)D * m, D}, IndexMap{D, m, 1},
+              (int)M2, b, d * b, 0};
+  g2.epi = 1;
+  GEMM(h, g2);
   return QRCTM_OK;
 }
 
@@ -538,6 +603,7 @@ int stage_absorb_a(qrctm* h, const double* P, double* S, int layout) {
 int stage_project(qrctm* h, const double* S, const double* Qm, double* out) {
   const int chi = h->chi; const long long m = h->m;
   GemmCall c{S, m, 1, Qm, chi, out, plain_map(chi), IndexMap{1, 1, 0}, (int)m, chi, (int)m, 0};
+  c.epi = 1;
   GEMM(h, c);
   return QRCTM_OK;
 }
@@ -628,7 +694,10 @@ int do_step(qrctm* h, cudaEvent_t* ev /* QRCTM_NSTAGE+1 events or null */, bool 
     if (nl < 0) rc = fail(h, QRCTM_ERR_CUDA, "qr", e); else h->launches += nl;
   }
   if (!rc) { mark(2, "K3_half_absorb"); rc = stage_half_absorb(h, h->Q, h->T, h->P); }
-  if (!rc) { mark(3, "K4_absorb_a"); rc = stage_absorb_a(h, h->P, h->S, 0); }
+  if (!rc) {
+    mark(3, "K4_absorb_a");
+    rc = (h->absorb_mode == 1 && layered_ok(h)) ? stage_absorb_layered(h, h->P, h->S) : stage_absorb_a(h, h->P, h->S, 0);
+  }
   if (!rc) { mark(4, "K5_project"); rc = stage_project(h, h->S, h->Q, h->Tn); }
   if (!rc) { mark(5, "K6_corner"); rc = h->corner_mode == 0 ? stage_corner_accel(h) : stage_corner_enlarged(h); }
   if (!rc && !with_k7) { nvtxRangePop(); return rc; }
@@ -798,7 +867,10 @@ int qrctm_set_A(qrctm_t* h, const double* A) {
   long long n = b2 * b2;
   int nb = (int)((n + 255) / 256); if (nb > 148 * 8) nb = 148 * 8;
   build_a_kernel<<<nb, 256, 0, h->stream>>>(h->A, h->d, h->D, h->a_mat, h->L.lda_a);
-  h->launches += 1;
+  CU(h, cudaMemsetAsync(h->B1, 0, sizeof(double) * h->b * h->L.ld1, h->stream));
+  CU(h, cudaMemsetAsync(h->B2, 0, sizeof(double) * h->d * h->b * h->L.ld2, h->stream));
+  build_layers_kernel<<<64, 256, 0, h->stream>>>(h->A, h->d, h->D, h->B1, h->L.ld1, h->B2, h->L.ld2);
+  h->launches += 2;
   CU(h, cudaGetLastError());
   h->have_A = true;
   return QRCTM_OK;
@@ -957,6 +1029,7 @@ int qrctm_set_option(qrctm_t* h, int key, int value) {
     case QRCTM_OPT_GEMM_PATH:   if (value != 0 && value != 1) break; h->gemm_path = value; return QRCTM_OK;
     case QRCTM_OPT_QR_PATH:     if (value != 0 && value != 1) break; h->qr_path = value; return QRCTM_OK;
     case QRCTM_OPT_OVERLAP_CHECK: if (value != 0 && value != 1) break; h->overlap = value; return QRCTM_OK;
+    case QRCTM_OPT_ABSORB_MODE: if (value != 0 && value != 1) break; h->absorb_mode = value; return QRCTM_OK;
     case QRCTM_OPT_USE_GRAPH:   if (value != 0 && value != 1) break; h->use_graph = value; return QRCTM_OK;
     case QRCTM_OPT_TIME_STAGES: if (value != 0 && value != 1) break; h->time_stages = value; return QRCTM_OK;
     default: break;

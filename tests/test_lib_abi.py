@@ -40,7 +40,7 @@ def test_invalid_arguments_rejected(lib):
     assert lib.qrctm_workspace_bytes(2, 2, 0) == 0
     n = lib.qrctm_workspace_bytes(2, 7, 196)
     m = 196 * 49
-    assert 2 * 8 * m * m < n < 2 * 8 * m * m + (1 << 30)      # P and S dominate
+    assert 2 * 8 * m * m < n < 4 * 8 * m * m + (1 << 30)      # P, S (m^2 each) and the layered P1 (2 m^2) dominate
     h = ctypes.c_void_p()
     assert lib.qrctm_create(0, 2, 8, ctypes.byref(h)) == -1
     assert lib.qrctm_create(2, 2, 8, None) == -1
