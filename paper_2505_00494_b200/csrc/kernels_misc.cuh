@@ -185,6 +185,12 @@ __global__ void copy_triu_kernel(const double* __restrict__ X, long long ldx, in
     R[idx] = j >= i ? X[(long long)i * ldx + j] : 0.0;
   }
 }
+__global__ void transpose_small_kernel(const double* __restrict__ Rm, int n, double* __restrict__ Rt) {
+  for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < n * n; idx += gridDim.x * blockDim.x) {
+    int i = idx / n, j = idx % n;
+    Rt[(long long)j * n + i] = Rm[idx];
+  }
+}
 // dot of two arrays with a fixed tree: partial per block, then final by block 0 of a 2nd launch
 __global__ void dot_partial_kernel(const double* __restrict__ x, const double* __restrict__ y, long long n,
                                    double* __restrict__ partial) {

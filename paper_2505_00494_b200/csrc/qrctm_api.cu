@@ -25,7 +25,7 @@ constexpr size_t kAlign = 256;
 inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {   // byte offsets into the workspace
-  size_t A, a_mat, B1, B2, P1, C, T, Cn, Tn, X, V, Q, R, tau, P, S, W, E, splitk, partial, scal, flag, Wc, dvec, evec,
+  size_t A, a_mat, B1, B2, P1, C, T, Cn, Tn, X, V, Q, R, Rt, tau, P, S, W, E, splitk, partial, scal, flag, Wc, dvec, evec,
       vv, pv, eig, s, s_prev, s_tmp, delta, qrwork, total;
   long long lda_a, ld1, ld2;
   size_t splitk_elems, qrwork_bytes;
@@ -57,7 +57,7 @@ struct qrctm {
   double* h_pinned;       // [0] delta, [1..] scratch ; pinned host
   int* h_flag;
   // typed views
-  double *A, *a_mat, *B1, *B2, *P1, *C, *T, *Cn, *Tn, *X, *V, *Q, *R, *tau, *P, *S, *W, *E, *splitk, *partial, *scal, *Wc,
+  double *A, *a_mat, *B1, *B2, *P1, *C, *T, *Cn, *Tn, *X, *V, *Q, *R, *Rt, *tau, *P, *S, *W, *E, *splitk, *partial, *scal, *Wc,
       *dvec, *evec, *vv, *pv, *eig, *s, *s_prev, *s_tmp, *delta;
   int* flag;
   void* qrwork;
@@ -91,6 +91,7 @@ bool make_layout(int d, int D, int chi, Layout* L) {
   L->V = take(dbl * m * chi);
   L->Q = take(dbl * m * chi);
   L->R = take(dbl * chi * chi);
+  L->Rt = take(dbl * chi * chi);
   L->tau = take(dbl * chi);
   L->P = take(dbl * m * m);
   L->S = take(dbl * m * m);
@@ -121,7 +122,7 @@ void bind_views(qrctm* h) {
   char* B = h->base;
   const Layout& L = h->L;
 #define V_(name) h->name = reinterpret_cast<double*>(B + L.name)
-  V_(A); V_(a_mat); V_(B1); V_(B2); V_(P1); V_(C); V_(T); V_(Cn); V_(Tn); V_(X); V_(V); V_(Q); V_(R); V_(tau); V_(P); V_(S); V_(W);
+  V_(A); V_(a_mat); V_(B1); V_(B2); V_(P1); V_(C); V_(T); V_(Cn); V_(Tn); V_(X); V_(V); V_(Q); V_(R); V_(Rt); V_(tau); V_(P); V_(S); V_(W);
   V_(E); V_(splitk); V_(partial); V_(scal); V_(Wc); V_(dvec); V_(evec); V_(vv); V_(pv); V_(eig); V_(s);
   V_(s_prev); V_(s_tmp); V_(delta);
 #undef V_
@@ -542,10 +543,18 @@ namespace {
   } while (0)
 
 // K1 (E1): X[(j,u),k] = sum_i C[j,i] T[i,u,k]       -> out (chi x b*chi == chi*b x chi)
+// Computed transposed, X^T[(u,k), j] = sum_i T[i,(u,k)] C[i,j]^T, so that both operands are K x (M|N)
+// row-major (bulk-copy kernel) and the long index is the GEMM's M; the epilogue writes X itself.
+// Ct is C^T as a K x N matrix: C itself when it is exactly symmetric (SYMMETRIZE = 1).
 int stage_reduced_corner(qrctm* h, const double* C, const double* T, double* X) {
   const int chi = h->chi; const long long bc = (long long)h->b * chi;
-  GemmCall c{C, chi, 0, T, bc, X, plain_map(bc), IndexMap{1, 1, 0}, chi, (int)bc, chi, 0};
-  GEMM(h, c);
+  if (h->symmetrize) {
+    GemmCall c{T, bc, 1, C, chi, X, IndexMap{1, 1, 0}, plain_map(bc), (int)bc, chi, chi, 0};
+    GEMM(h, c);
+  } else {
+    GemmCall c{C, chi, 0, T, bc, X, plain_map(bc), IndexMap{1, 1, 0}, chi, (int)bc, chi, 0};
+    GEMM(h, c);
+  }
   return QRCTM_OK;
 }
 
@@ -611,7 +620,10 @@ int stage_project(qrctm* h, const double* S, const double* Qm, double* out) {
 // K6 (E4): W[m,(r,n)] = sum_k R[m,k] Q[k,(r,n)] ;  C'[p,n] = sum_{(m,r)} T'[(m,r),p] W[(m,r),n]
 int stage_corner_accel(qrctm* h) {
   const int chi = h->chi; const long long bc = (long long)h->b * chi, m = h->m;
-  GemmCall c1{h->R, chi, 0, h->Q, bc, h->W, plain_map(bc), IndexMap{1, 1, 0}, chi, (int)bc, chi, 0};
+  // W^T[(r,n), m] = sum_k Q[k,(r,n)] R^T[k,m]  (long index as M, both operands K-major); writes W
+  transpose_small_kernel<<<(chi * chi + 255) / 256, 256, 0, h->stream>>>(h->R, chi, h->Rt);
+  h->launches += 1;
+  GemmCall c1{h->Q, bc, 1, h->Rt, chi, h->W, IndexMap{1, 1, 0}, plain_map(bc), (int)bc, chi, chi, 0};
   GEMM(h, c1);
   GemmCall c2{h->Tn, chi, 1, h->W, chi, h->Cn, plain_map(chi), IndexMap{1, 1, 0}, chi, chi, (int)m, 0};
   GEMM(h, c2);
