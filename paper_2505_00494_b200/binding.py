@@ -16,7 +16,7 @@ from ctypes import (POINTER, byref, c_char_p, c_double, c_float, c_int, c_longlo
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libqrctm.so")
+LIB_PATH = os.environ.get("QRCTM_LIB", os.path.join(_HERE, "libqrctm.so"))
 
 QRCTM_OK = 0
 OPT_CORNER_MODE, OPT_SYMMETRIZE, OPT_CHECK_EVERY, OPT_GEMM_PATH, OPT_TIME_STAGES, OPT_QR_PATH, OPT_OVERLAP_CHECK, OPT_USE_GRAPH, OPT_ABSORB_MODE = 1, 2, 3, 4, 5, 6, 7, 8, 9

@@ -11,6 +11,7 @@
 
 #include "kernels_misc.cuh"
 
+
 namespace qk {
 
 // One block.  Column k of X (rows k..rows-1): compute the reflector in place.
@@ -441,9 +442,12 @@ qr_panel_reg2_kernel(double* __restrict__ V, long long ld, long long m, int j0, 
   const int rank = CLUSTER ? (int)cluster.block_rank() : 0;
   constexpr int NRG = NT / NB, NW = NT / 32;
   static_assert(NRG >= NB, "diagonal rows must all sit at t = 0");
+  static_assert(RPT % 8 == 0 && NW % 4 == 0, "unrolled accumulators / tree sums");
   __shared__ double exch[2 * 16 * NB];
   __shared__ double rowv[2 * NB];
   __shared__ double red[2 * NW * NB];
+  __shared__ double Gs[NB * NB];               // Gs[a][k] = v_a^T v_k (a < k), filled column by column
+  __shared__ double taus[NB];
   __shared__ double Ts[NB * NB];
 
   const int tid = threadIdx.x, col = tid % NB, rg = tid / NB, warp = tid >> 5, lane = tid & 31;
@@ -461,8 +465,7 @@ qr_panel_reg2_kernel(double* __restrict__ V, long long ld, long long m, int j0, 
     for (int t = 0; t < RPT; ++t, pl += (long long)NRG * ld)
       val[t] = (rg + t * NRG < nloc && col < nbw) ? *pl : 0.0;
   }
-  if (tid < NB * NB) Ts[tid] = 0.0;
-  if (NT < NB * NB) for (int i = tid + NT; i < NB * NB; i += NT) Ts[i] = 0.0;
+  for (int i = tid; i < NB * NB; i += NT) { Ts[i] = 0.0; Gs[i] = 0.0; }
   double my_scale = 0.0;                       // scale of this thread's column once it has been factored
   __syncthreads();
   if (CLUSTER) cluster.sync();
@@ -477,31 +480,54 @@ qr_panel_reg2_kernel(double* __restrict__ V, long long ld, long long m, int j0, 
       if (CLUSTER) { for (int q = 0; q < C; ++q) { double* rr = cluster.map_shared_rank(rowv, q); rr[buf * NB + col] = rvv; } }
       else rowv[buf * NB + col] = rvv;
     }
-    // B. column k of my rows, dot with my column
+    // B. column k of my rows, dot with my column.  FP64 dependent-issue latency is long (~30 cycles),
+    //    so the sum runs on 8 independent accumulators combined by a fixed tree.
     double xs[RPT];
-    double a0 = 0.0, a1 = 0.0;
+    double ac[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) ac[u] = 0.0;
 #pragma unroll
     for (int t = 0; t < RPT; ++t) {
       xs[t] = __shfl_sync(0xffffffffu, val[t], lane_base | k);
-      if (t & 1) a1 = fma(xs[t], val[t], a1); else a0 = fma(xs[t], val[t], a0);
+      ac[t & 7] = fma(xs[t], val[t], ac[t & 7]);
     }
-    double acc = a0 + a1;
+    double acc = ((ac[0] + ac[1]) + (ac[2] + ac[3])) + ((ac[4] + ac[5]) + (ac[6] + ac[7]));
     if (NB == 16) acc += __shfl_xor_sync(0xffffffffu, acc, 16);
     if (lane < NB) red[(buf * NW + warp) * NB + lane] = acc;
     __syncthreads();
     double gk = 0.0, gj = 0.0;
     if (CLUSTER) {
       if (tid < NB) {
-        double g = 0.0;
+        double pg[NW];
 #pragma unroll
-        for (int w = 0; w < NW; ++w) g += red[(buf * NW + w) * NB + tid];
-        for (int q = 0; q < C; ++q) { double* rex = cluster.map_shared_rank(exch, q); rex[(buf * 16 + rank) * NB + tid] = g; }
+        for (int w = 0; w < NW; ++w) pg[w] = red[(buf * NW + w) * NB + tid];
+#pragma unroll
+        for (int st = 1; st < NW; st *= 2)
+#pragma unroll
+          for (int w = 0; w + st < NW; w += 2 * st) pg[w] += pg[w + st];
+        for (int q = 0; q < C; ++q) { double* rex = cluster.map_shared_rank(exch, q); rex[(buf * 16 + rank) * NB + tid] = pg[0]; }
       }
       cluster.sync();
-      for (int q = 0; q < C; ++q) { gk += exch[(buf * 16 + q) * NB + k]; gj += exch[(buf * 16 + q) * NB + col]; }
-    } else {
+      double pk[16], pj[16];
 #pragma unroll
-      for (int w = 0; w < NW; ++w) { gk += red[(buf * NW + w) * NB + k]; gj += red[(buf * NW + w) * NB + col]; }
+      for (int q = 0; q < 16; ++q) {
+        pk[q] = q < C ? exch[(buf * 16 + q) * NB + k] : 0.0;
+        pj[q] = q < C ? exch[(buf * 16 + q) * NB + col] : 0.0;
+      }
+#pragma unroll
+      for (int st = 1; st < 16; st *= 2)
+#pragma unroll
+        for (int q = 0; q + st < 16; q += 2 * st) { pk[q] += pk[q + st]; pj[q] += pj[q + st]; }
+      gk = pk[0]; gj = pj[0];
+    } else {
+      double pk[NW], pj[NW];
+#pragma unroll
+      for (int w = 0; w < NW; ++w) { pk[w] = red[(buf * NW + w) * NB + k]; pj[w] = red[(buf * NW + w) * NB + col]; }
+#pragma unroll
+      for (int st = 1; st < NW; st *= 2)
+#pragma unroll
+        for (int w = 0; w + st < NW; w += 2 * st) { pk[w] += pk[w + st]; pj[w] += pj[w + st]; }
+      gk = pk[0]; gj = pj[0];
     }
     // F. reflector scalars (identical in every thread)
     const double alpha = rowv[buf * NB + k], yrj = rowv[buf * NB + col];
@@ -529,21 +555,10 @@ qr_panel_reg2_kernel(double* __restrict__ V, long long ld, long long m, int j0, 
       V[(long long)(j0 + k) * ld + j0 + col] = vout;
       Vc[(long long)(j0 + k) * ld + j0 + col] = vclean;
     }
-    // I. column k of T (warp 0, lanes a < NB hold col = a): T[a][k] = -tau_k sum_{c=a}^{k-1} T[a][c] G[c][k]
-    if (warp == 0) {
-      const double Gak = my_scale * z;                       // valid for lanes with col < k (rg = 0 half)
-      double s0 = 0.0, s1 = 0.0;
-#pragma unroll
-      for (int c = 0; c < NB; c += 2) {
-        const double g0 = __shfl_sync(0xffffffffu, Gak, c), g1 = __shfl_sync(0xffffffffu, Gak, c + 1);
-        if (lane < NB && c >= lane && c < k) s0 = fma(Ts[lane * NB + c], g0, s0);
-        if (lane < NB && c + 1 >= lane && c + 1 < k) s1 = fma(Ts[lane * NB + c + 1], g1, s1);
-      }
-      if (lane < NB) {
-        if (lane == k) Ts[k * NB + k] = tk;
-        else if (lane < k) Ts[lane * NB + k] = -tk * (s0 + s1);
-      }
-      if (rank == 0 && lane == k) tau[j0 + k] = tk;
+    // I. Gram column k of the reflectors (for the T factor, built after the loop) and tau_k
+    if (rg == 0) {
+      if (col < k) Gs[col * NB + k] = my_scale * z;
+      else if (col == k) { taus[k] = tk; if (rank == 0) tau[j0 + k] = tk; }
     }
     if (col == k) my_scale = scale;
     buf ^= 1;
@@ -562,8 +577,27 @@ qr_panel_reg2_kernel(double* __restrict__ V, long long ld, long long m, int j0, 
       }
     }
   }
-  __syncwarp();
+  // compact-WY factor, forward recurrence (LAPACK dlarft): T[a][k] = -tau_k sum_{c=a}^{k-1} T[a][c] G[c][k]
+  __syncthreads();
   if (rank == 0 && warp == 0) {
+    if (lane < NB) {
+      const int a = lane;
+      for (int k = 0; k < nbw; ++k) {
+        const double tk = taus[k];
+        if (a == k) Ts[k * NB + k] = tk;
+        else if (a < k) {
+          double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+#pragma unroll
+          for (int c = 0; c < NB; c += 4) {
+            if (c >= a && c < k) s0 = fma(Ts[a * NB + c], Gs[c * NB + k], s0);
+            if (c + 1 >= a && c + 1 < k) s1 = fma(Ts[a * NB + c + 1], Gs[(c + 1) * NB + k], s1);
+            if (c + 2 >= a && c + 2 < k) s2 = fma(Ts[a * NB + c + 2], Gs[(c + 2) * NB + k], s2);
+            if (c + 3 >= a && c + 3 < k) s3 = fma(Ts[a * NB + c + 3], Gs[(c + 3) * NB + k], s3);
+          }
+          Ts[a * NB + k] = -tk * ((s0 + s1) + (s2 + s3));
+        }
+      }
+    }
     __syncwarp();
     for (int i = lane; i < NB * NB; i += 32) Tp[i] = Ts[i];
   }

@@ -368,3 +368,44 @@ def test_layered_absorption_matches_oracle_and_explicit(d, D, chi, seed, path):
     assert rel(lay["C"], Co) < 1e-11 and rel(lay["T"], To) < 1e-11
     exp, _, _ = _one_step(d, D, chi, seed, absorb=0, path=path)
     assert rel(lay["raw"][1], exp["raw"][1]) < 1e-12
+
+
+def test_large_chi_fallback_paths():
+    """chi = 300 > 236: the corner spectrum takes the global-memory tridiagonalisation path; D = 1 keeps it cheap.
+    Also a square c~ (m = chi) for the QR (19 panels, the last one ragged)."""
+    d, D, chi = 2, 1, 300
+    A, C0, T0 = gen_config(d, D, chi, 5)
+    h = pkg.QRCTM(d, D, chi)
+    h.set_A(A); h.set_env(C0, T0)
+    C, _ = h.get_env()
+    assert np.max(np.abs(h.get_corner_spectrum() - o.spectrum(C))) < 5e-15 * chi
+    h.step()
+    a = o.build_a(A)
+    Cr, Tr = o.normalize(C0, T0)
+    s = o.qr_step(Cr, Tr, a)
+    Co, To = o.normalize(s["Cn"], s["Tn"])
+    Q, R = h.get_qr()
+    assert np.linalg.norm(Q.T @ Q - np.eye(chi)) < chi * 2e-15 and rel(Q @ R, s["X"]) < 1e-13
+    cond = np.linalg.cond(s["X"])
+    C1, T1 = h.get_env()
+    tol = max(1e-11, 1e-14 * cond)          # a square random c~ is ill-conditioned: Q is only determined to cond * eps
+    assert rel(C1, Co) < tol and rel(T1, To) < tol
+    it, dl = h.run(3, -1.0)
+    assert it == 3 and np.isfinite(dl)
+    h.close()
+
+
+def test_odd_chi_and_d3_run_parity():
+    """Odd chi (no 16-byte aligned rows: cp.async fallback GEMM, layered mode falls back to explicit) and d = 3."""
+    d, D, chi = 3, 2, 9
+    A, C0, T0 = gen_config(d, D, chi, 11)
+    for absorb in (0, 1):
+        h = pkg.QRCTM(d, D, chi)
+        h.set_option(pkg.OPT_ABSORB_MODE, absorb)
+        h.set_A(A); h.set_env(C0, T0)
+        it, dl = h.run(12, -1.0)
+        Co, To, a = _oracle_steps(A, C0, T0, 12)
+        C, T = h.get_env()
+        assert rel(C, Co) < 1e-10 and rel(T, To) < 1e-10
+        assert abs(h.norm_per_site() / o.kappa(Co, To, a) - 1) < 1e-9
+        h.close()
