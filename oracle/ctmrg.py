@@ -334,3 +334,50 @@ def naive_qr_step_tensors(C, T, a, Q, R):
                         acc += R[m, k] * Tn[m, r, p] * Q3[k, r, n]
             Cn[p, n] = acc
     return Cn, Tn
+
+
+# ------------------------------------------------- NEXT-3: nearest-neighbour energy
+def build_a_pair(A, s, sp):
+    """Double-layer tensor with the physical legs left open:
+    a^{s s'}[(u u'),(l l'),(d d'),(r r')] = A[s,u,l,d,r] A[s',u',l',d',r']  (sum_s a^{ss} = a of (E0))."""
+    D = A.shape[1]
+    aa = np.multiply.outer(A[s], A[sp])                       # [u,l,d,r,u',l',d',r']
+    aa = aa.transpose(0, 4, 1, 5, 2, 6, 3, 7)
+    b = D * D
+    return np.ascontiguousarray(aa.reshape(b, b, b, b))
+
+
+def half_network(C, T, a_x):
+    """Left half of the two-site network  C T T C / T a a T / C T T C  cut through the bond between
+    the two sites:  LH[k,x,k'] = sum c~[(j,u),k] T[j,l,J] a_x[u,l,d,x] c~[(J,d),k'],  c~ = C.T (E1),
+    i.e. (E3) with c~ in place of Q.  k / k' are the top / bottom chi legs, x the cut bond."""
+    X = reduced_corner(C, T)
+    return edge_update(X, T, a_x)
+
+
+def rdm2(C, T, A):
+    """Two-site reduced density matrix on a nearest-neighbour bond (un-normalised):
+    rho[s1,s1',s2,s2'] = sum_{k,x,k'} LH^{s1 s1'}[k,x,k'] LH^{s2 s2'}[k,x,k'].
+    The right half is the mirror image of the left one (A is invariant under the l <-> r reflection
+    of C4v), so it is the same tensor with the same leg labels."""
+    d = A.shape[0]
+    LH = [[half_network(C, T, build_a_pair(A, s, sp)) for sp in range(d)] for s in range(d)]
+    rho = np.zeros((d, d, d, d))
+    for s1 in range(d):
+        for s1p in range(d):
+            for s2 in range(d):
+                for s2p in range(d):
+                    rho[s1, s1p, s2, s2p] = np.sum(LH[s1][s1p] * LH[s2][s2p])
+    return rho
+
+
+def energy_nn(C, T, A, H):
+    """<h> on one bond for a two-site operator H[(s1 s2),(s1' s2')] (d^2 x d^2, ket index first):
+    Tr(rho2 h) / Tr(rho2).  PAPER.md:38-40 evaluates the energy per site of nearest-neighbour
+    Hamiltonians this way (the square lattice has two bonds per site; under C4v all bonds are equal)."""
+    d = A.shape[0]
+    rho = rdm2(C, T, A)
+    H4 = np.asarray(H, dtype=np.float64).reshape(d, d, d, d)   # [s1,s2,s1',s2']
+    num = np.einsum("abcd,acbd->", rho, H4)                    # rho[s1,s1',s2,s2'] H[s1,s2,s1',s2']
+    den = np.einsum("aabb->", rho)
+    return float(num / den)

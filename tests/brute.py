@@ -50,3 +50,51 @@ def ising_A(K: float) -> np.ndarray:
     lam, V = np.linalg.eigh(B)
     w = (V * np.sqrt(lam)) @ V.T
     return np.einsum("su,sl,sd,sr->suldr", w, w, w, w)
+
+
+def patch_contract(site, nrows: int, ncols: int, D: int) -> float:
+    """Like patch_norm but with a possibly different double-layer tensor per site: site(r, c) -> a[u,l,d,r]."""
+    b = D * D
+    v = np.eye(D).reshape(b)
+    state = v
+    for _ in range(ncols - 1):
+        state = np.multiply.outer(state, v)
+    state = state.reshape((b,) * ncols)
+    for rr in range(nrows):
+        cur = np.multiply.outer(v, state)
+        for c in range(ncols):
+            cur = np.tensordot(cur, site(rr, c), axes=([1 + c, 0], [0, 1]))
+            nd = cur.ndim
+            order = [nd - 1] + list(range(0, c)) + [nd - 2] + list(range(c, nd - 2))
+            cur = cur.transpose(order)
+        state = np.tensordot(v, cur, axes=([0], [0]))
+    for _ in range(ncols):
+        state = np.tensordot(state, v, axes=([0], [0]))
+    return float(state)
+
+
+def patch_energy_nn(A: np.ndarray, H: np.ndarray, nrows: int, ncols: int, r0: int, c0: int) -> float:
+    """<psi|h|psi>/<psi|psi> for an open nrows x ncols patch of the single-site iPEPS tensor A with the
+    two-site operator H[(s1 s2),(s1' s2')] on the horizontal bond (r0,c0)-(r0,c0+1).  Brute force."""
+    d, D = A.shape[0], A.shape[1]
+    b = D * D
+
+    def pair(s, sp):
+        aa = np.multiply.outer(A[s], A[sp]).transpose(0, 4, 1, 5, 2, 6, 3, 7)
+        return aa.reshape(b, b, b, b)
+
+    a = sum(pair(s, s) for s in range(d))
+    H4 = np.asarray(H).reshape(d, d, d, d)
+    num = 0.0
+    for s1 in range(d):
+        for s1p in range(d):
+            for s2 in range(d):
+                for s2p in range(d):
+                    hv = H4[s1, s2, s1p, s2p]
+                    if hv == 0.0:
+                        continue
+                    t1, t2 = pair(s1, s1p), pair(s2, s2p)
+                    num += hv * patch_contract(
+                        lambda r, c: t1 if (r, c) == (r0, c0) else (t2 if (r, c) == (r0, c0 + 1) else a),
+                        nrows, ncols, D)
+    return num / patch_contract(lambda r, c: a, nrows, ncols, D)

@@ -10,7 +10,7 @@ import pytest
 
 from oracle import ctmrg as o
 from qrctm_inputs import C4V_PERMS, c4v_symmetrize, gen_config
-from tests.brute import ising_A, onsager_ln_kappa, patch_norm
+from tests.brute import ising_A, onsager_ln_kappa, patch_energy_nn, patch_norm
 
 
 def rel(x, y):
@@ -303,3 +303,50 @@ def test_P11_fixed_point(cfg0):
     assert abs(o.kappa(C1, T1, a) / o.kappa(C, T, a) - 1) < 1e-11
     sp = o.spectrum(C)
     assert abs(np.sum(sp ** 2) - 1) < 1e-13 and np.all(np.diff(sp) <= 0)
+
+
+# ---- NEXT-3: nearest-neighbour energy ---------------------------------------------
+def _heisenberg_rotated():
+    """S.S on a bond after the sublattice rotation exp(i pi sigma^y / 2) on one site:
+    -SxSx + SySy - SzSz, real in the sigma^z basis.  Index order [(s1 s2),(s1' s2')]."""
+    sx = np.array([[0, 1], [1, 0]]) / 2; sz = np.array([[1, 0], [0, -1]]) / 2
+    sy_im = np.array([[0, -1], [1, 0]]) / 2          # Sy = i * sy_im
+    return -np.kron(sx, sx) - np.kron(sy_im, sy_im) - np.kron(sz, sz)   # (i sy_im)(i sy_im) = -sy_im x sy_im
+
+
+def test_energy_identity_and_product_state():
+    g = np.random.default_rng(12)
+    A, C0, T0 = gen_config(2, 2, 6, 3)
+    assert abs(o.energy_nn(C0, T0, A, np.eye(4)) - 1.0) < 1e-13
+    phi = g.standard_normal(2); v = g.standard_normal(3)
+    Ap = np.einsum("s,u,l,d,r->suldr", phi, v, v, v, v)
+    _, C1, T1 = gen_config(2, 3, 5, 1)
+    H = g.standard_normal((4, 4)); H = H + H.T
+    want = np.kron(phi, phi) @ H @ np.kron(phi, phi) / (phi @ phi) ** 2
+    assert abs(o.energy_nn(C1, T1, Ap, H) - want) < 1e-12 * max(1.0, abs(want))
+
+
+@pytest.mark.parametrize("n", [0, 1])
+def test_energy_exact_environment_vs_brute_force_patch(n):
+    """bulk_init + n untruncated eigen steps is the exact environment of an open patch (fn.[48]): the CTM energy on
+    the central bond must equal <psi|h|psi>/<psi|psi> of the (2n+3) x (2n+4) patch contracted by brute force."""
+    A, _, _ = gen_config(2, 2, 4, 6)
+    a = o.build_a(A)
+    C, T = o.bulk_init(A)
+    for _ in range(n):
+        e = o.eig_step(C, T, a, chi_new=C.shape[0] * 4)
+        C, T = e["Cn"], e["Tn"]
+    g = np.random.default_rng(2)
+    for H in (_heisenberg_rotated(), (lambda M: M + M.T)(g.standard_normal((4, 4)))):
+        got = o.energy_nn(C, T, A, H)
+        want = patch_energy_nn(A, H, 2 * n + 3, 2 * n + 4, n + 1, n + 1)
+        assert abs(got - want) < 1e-11 * max(1.0, abs(want))
+
+
+def test_rdm2_trace_is_the_two_site_norm_network():
+    A, C0, T0 = gen_config(2, 2, 6, 2)
+    a = o.build_a(A)
+    rho = o.rdm2(C0, T0, A)
+    LH = o.half_network(C0, T0, a)
+    assert abs(np.einsum("aabb->", rho) / np.sum(LH * LH) - 1) < 1e-13
+    assert np.allclose(rho, rho.transpose(2, 3, 0, 1), atol=1e-14 * np.abs(rho).max())   # site exchange
