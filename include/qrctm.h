@@ -141,6 +141,15 @@ int qrctm_get_a(qrctm_t* h, double* a);
  * (reading A8).  HOST pointer.  Synchronises. */
 int qrctm_norm_per_site(qrctm_t* h, double* kappa);
 
+/* NEXT-3.  Expectation value of a two-site operator on a nearest-neighbour bond,
+ *   e_bond = Tr(rho2 H) / Tr(rho2),   rho2[s1,s1',s2,s2'] = sum LH^{s1 s1'}[k,x,k'] LH^{s2 s2'}[k,x,k'],
+ * LH^{ss'} = (E3) with c~ = C.T in place of Q and a^{ss'} = A[s] (x) A[s'] in place of a  (the left half of the network
+ * C T T C / T a a T / C T T C; the right half is its mirror image under C4v).  H is d^2 x d^2 row-major with index
+ * [(s1 s2)][(s1' s2')] (HOST).  The energy per site of H_total = sum_<ij> h_ij on the square lattice is 2 e_bond
+ * (PAPER.md:38-40).  rho_out (HOST, d^4, may be NULL) receives the un-normalised rho2.  d <= 4.  Overwrites the
+ * step scratch (X, P, S); the environment is untouched.  Synchronises. */
+int qrctm_energy_nn(qrctm_t* h, const double* H, double* e_bond, double* rho_out);
+
 /* min_k R_kk / max_k R_kk of the last step: a conditioning diagnostic for the
  * uniqueness of Q (DESIGN.md hazard H1).  HOST pointer.  Synchronises. */
 int qrctm_r_diag_ratio(qrctm_t* h, double* ratio);

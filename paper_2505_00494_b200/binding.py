@@ -30,7 +30,7 @@ SYMBOLS = (
     "qrctm_create", "qrctm_workspace_bytes", "qrctm_create_in", "qrctm_destroy", "qrctm_set_stream",
     "qrctm_set_A", "qrctm_set_env", "qrctm_step", "qrctm_run", "qrctm_get_env",
     "qrctm_get_corner_spectrum", "qrctm_get_qr", "qrctm_get_raw", "qrctm_get_a", "qrctm_norm_per_site",
-    "qrctm_r_diag_ratio", "qrctm_set_option", "qrctm_launch_count", "qrctm_get_stage_ms", "qrctm_profile_step",
+    "qrctm_r_diag_ratio", "qrctm_energy_nn", "qrctm_set_option", "qrctm_launch_count", "qrctm_get_stage_ms", "qrctm_profile_step",
     "qrctm_gemm_f64", "qrctm_qr_work_bytes", "qrctm_qr_f64", "qrctm_probe_fp64", "qrctm_last_error",
     "qrctm_version",
 )
@@ -70,6 +70,7 @@ def load_library() -> ctypes.CDLL:
     lib.qrctm_get_a.argtypes = [P, P]
     lib.qrctm_norm_per_site.argtypes = [P, POINTER(c_double)]
     lib.qrctm_r_diag_ratio.argtypes = [P, POINTER(c_double)]
+    lib.qrctm_energy_nn.argtypes = [P, P, POINTER(c_double), P]
     lib.qrctm_set_option.argtypes = [P, c_int, c_int]
     lib.qrctm_launch_count.argtypes = [P]
     lib.qrctm_launch_count.restype = c_longlong
@@ -221,6 +222,15 @@ class QRCTM:
         k = c_double(0.0)
         self._check(self.lib.qrctm_norm_per_site(self._h, byref(k)))
         return k.value
+
+    def energy_nn(self, H, return_rho: bool = False):
+        """Tr(rho2 H)/Tr(rho2) on a nearest-neighbour bond; H is (d*d, d*d) with index [(s1 s2), (s1' s2')]."""
+        H = np.ascontiguousarray(H, dtype=np.float64)
+        assert H.shape == (self.d * self.d, self.d * self.d)
+        e = c_double(0.0)
+        rho = np.empty((self.d,) * 4, dtype=np.float64) if return_rho else None
+        self._check(self.lib.qrctm_energy_nn(self._h, _ptr(H), byref(e), _ptr(rho)))
+        return (e.value, rho) if return_rho else e.value
 
     def r_diag_ratio(self) -> float:
         k = c_double(0.0)

@@ -69,6 +69,24 @@ __global__ void build_a_kernel(const double* __restrict__ A, int d, int D, doubl
   }
 }
 
+// a^{s s'}[(u u'),(l l'),(d d'),(r r')] = A[s,u,l,d,r] A[s',u',l',d',r']  (physical legs open; NEXT-3 energy),
+// same K x N matrix layout as build_a_kernel.
+__global__ void build_a_pair_kernel(const double* __restrict__ A, int D, int s, int sp, double* __restrict__ a_mat,
+                                    long long lda_a) {
+  const int b = D * D;
+  const long long n = (long long)b * b * b * b;
+  const long long DD = (long long)D * D * D * D;
+  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < n;
+       idx += (long long)gridDim.x * blockDim.x) {
+    int r = (int)(idx % b), dd = (int)((idx / b) % b), l = (int)((idx / ((long long)b * b)) % b),
+        u = (int)(idx / ((long long)b * b * b));
+    int uk = u / D, ub = u % D, lk = l / D, lb = l % D, dk = dd / D, db = dd % D, rk = r / D, rb = r % D;
+    long long ik = (((long long)uk * D + lk) * D + dk) * D + rk;
+    long long ib = (((long long)ub * D + lb) * D + db) * D + rb;
+    a_mat[((long long)u * b + l) * lda_a + (long long)dd * b + r] = A[s * DD + ik] * A[sp * DD + ib];
+  }
+}
+
 // Re-laid-out copies of A for the layered absorption (NEXT-1):
 //   B1[(u_k,l_k)][(s,d_k,r_k)] = A[s,u_k,l_k,d_k,r_k]   (D^2 x d D^2, leading dimension ld1)
 //   B2[(s,u_b,l_b)][(d_b,r_b)] = A[s,u_b,l_b,d_b,r_b]   (d D^2 x D^2, leading dimension ld2)

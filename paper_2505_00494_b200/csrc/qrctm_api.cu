@@ -25,7 +25,7 @@ constexpr size_t kAlign = 256;
 inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {   // byte offsets into the workspace
-  size_t A, a_mat, B1, B2, P1, C, T, Cn, Tn, X, V, Q, R, Rt, tau, P, S, W, E, splitk, partial, scal, flag, Wc, dvec, evec,
+  size_t A, a_mat, a2_mat, LH, rho, B1, B2, P1, C, T, Cn, Tn, X, V, Q, R, Rt, tau, P, S, W, E, splitk, partial, scal, flag, Wc, dvec, evec,
       vv, pv, eig, s, s_prev, s_tmp, delta, qrwork, total;
   long long lda_a, ld1, ld2;
   size_t splitk_elems, qrwork_bytes;
@@ -57,7 +57,7 @@ struct qrctm {
   double* h_pinned;       // [0] delta, [1..] scratch ; pinned host
   int* h_flag;
   // typed views
-  double *A, *a_mat, *B1, *B2, *P1, *C, *T, *Cn, *Tn, *X, *V, *Q, *R, *Rt, *tau, *P, *S, *W, *E, *splitk, *partial, *scal, *Wc,
+  double *A, *a_mat, *a2_mat, *LH, *rho, *B1, *B2, *P1, *C, *T, *Cn, *Tn, *X, *V, *Q, *R, *Rt, *tau, *P, *S, *W, *E, *splitk, *partial, *scal, *Wc,
       *dvec, *evec, *vv, *pv, *eig, *s, *s_prev, *s_tmp, *delta;
   int* flag;
   void* qrwork;
@@ -78,6 +78,9 @@ bool make_layout(int d, int D, int chi, Layout* L) {
   const size_t dbl = sizeof(double);
   L->A = take(dbl * d * b2);
   L->a_mat = take(dbl * b2 * L->lda_a);
+  L->a2_mat = take(dbl * b2 * L->lda_a);
+  L->LH = take(d <= 4 ? dbl * (size_t)d * d * m * chi : 0);
+  L->rho = take(dbl * 256);
   L->ld1 = ((long long)d * b + 15) / 16 * 16;
   L->ld2 = (b + 15) / 16 * 16;
   L->B1 = take(dbl * b * L->ld1);
@@ -122,7 +125,7 @@ void bind_views(qrctm* h) {
   char* B = h->base;
   const Layout& L = h->L;
 #define V_(name) h->name = reinterpret_cast<double*>(B + L.name)
-  V_(A); V_(a_mat); V_(B1); V_(B2); V_(P1); V_(C); V_(T); V_(Cn); V_(Tn); V_(X); V_(V); V_(Q); V_(R); V_(Rt); V_(tau); V_(P); V_(S); V_(W);
+  V_(A); V_(a_mat); V_(a2_mat); V_(LH); V_(rho); V_(B1); V_(B2); V_(P1); V_(C); V_(T); V_(Cn); V_(Tn); V_(X); V_(V); V_(Q); V_(R); V_(Rt); V_(tau); V_(P); V_(S); V_(W);
   V_(E); V_(splitk); V_(partial); V_(scal); V_(Wc); V_(dvec); V_(evec); V_(vv); V_(pv); V_(eig); V_(s);
   V_(s_prev); V_(s_tmp); V_(delta);
 #undef V_
@@ -571,12 +574,12 @@ int stage_half_absorb(qrctm* h, const double* Qm, const double* T, double* P) {
 //   layout 0: S''[J,d,m,r]  (what K5 wants: K x M with K = (J,d))
 //   layout 1: S~ [m,r,J,d]  (what the kappa network wants: K = (m,r))
 //   layout 2: C~[(J,d),(m,r)] natural enlarged-corner matrix == layout 0
-int stage_absorb_a(qrctm* h, const double* P, double* S, int layout) {
+int stage_absorb_a(qrctm* h, const double* P, double* S, int layout, const double* amat = nullptr) {
   const int chi = h->chi, b = h->b; const long long m = h->m, cc = (long long)chi * chi;
   IndexMap ro, co;
   if (layout == 0) { ro = IndexMap{chi, (long long)b * m, b}; co = IndexMap{b, m, 1}; }
   else             { ro = IndexMap{chi, b, (long long)b * m}; co = IndexMap{b, 1, (long long)chi * b}; }
-  GemmCall c{P, cc, 1, h->a_mat, h->L.lda_a, S, ro, co, (int)cc, b * b, b * b, 0};
+  GemmCall c{P, cc, 1, amat ? amat : h->a_mat, h->L.lda_a, S, ro, co, (int)cc, b * b, b * b, 0};
   c.epi = 1;
   GEMM(h, c);
   return QRCTM_OK;
@@ -833,7 +836,7 @@ static int create_common(int d, int D, int chi, void* ws, unsigned long long ws_
       cudaGetLastError(); h->side = nullptr; h->overlap = 0;
     }
   }
-  h->h_flag = reinterpret_cast<int*>(h->h_pinned + 32);
+  h->h_flag = reinterpret_cast<int*>(h->h_pinned + 32);       // [64..319] holds the two-site RDM
   cudaMemsetAsync(h->flag, 0, 4 * sizeof(int), 0);
   cudaMemsetAsync(h->s_prev, 0, sizeof(double) * chi, 0);
   cudaMemsetAsync(h->R, 0, sizeof(double) * chi * chi, 0);
@@ -1116,6 +1119,50 @@ int qrctm_norm_per_site(qrctm_t* h, double* kappa) {
   CU(h, cudaStreamSynchronize(h->stream));
   double Z4 = h->h_pinned[2], Z2 = h->h_pinned[3], Z1 = h->h_pinned[4];
   *kappa = Z1 * Z4 / (Z2 * Z2);
+  return QRCTM_OK;
+}
+
+int qrctm_energy_nn(qrctm_t* h, const double* H, double* e_bond, double* rho_out) {
+  if (!h || !H || !e_bond) return h ? fail(h, QRCTM_ERR_INVALID_ARG, "null argument") : QRCTM_ERR_INVALID_ARG;
+  if (!h->have_A || !h->have_env) return fail(h, QRCTM_ERR_NOT_READY, "set_A and set_env first");
+  const int d = h->d, chi = h->chi;
+  if (d > 4) return fail(h, QRCTM_ERR_INVALID_ARG, "qrctm_energy_nn supports d <= 4");
+  if (is_device_ptr(H) || (rho_out && is_device_ptr(rho_out))) return fail(h, QRCTM_ERR_INVALID_ARG, "H, rho: host pointers");
+  const long long m = h->m, nlh = m * chi;
+  int rc;
+  // half network LH^{ss'} = (E3) with c~ for Q and a^{ss'} for a
+  rc = stage_reduced_corner(h, h->C, h->T, h->X); if (rc) return rc;
+  rc = stage_half_absorb(h, h->X, h->T, h->P); if (rc) return rc;
+  const long long b2 = (long long)h->b * h->b, n = b2 * b2;
+  int nb = (int)((n + 255) / 256); if (nb > 148 * 8) nb = 148 * 8;
+  CU(h, cudaMemsetAsync(h->a2_mat, 0, sizeof(double) * b2 * h->L.lda_a, h->stream));
+  for (int s = 0; s < d; ++s)
+    for (int sp = 0; sp < d; ++sp) {
+      build_a_pair_kernel<<<nb, 256, 0, h->stream>>>(h->A, h->D, s, sp, h->a2_mat, h->L.lda_a);
+      h->launches += 1;
+      rc = stage_absorb_a(h, h->P, h->S, 0, h->a2_mat); if (rc) return rc;
+      rc = stage_project(h, h->S, h->X, h->LH + (size_t)(s * d + sp) * nlh); if (rc) return rc;
+    }
+  // rho[s1,s1',s2,s2'] = <LH^{s1s1'}, LH^{s2s2'}>   (symmetric under exchange of the two pairs)
+  const int d2 = d * d;
+  for (int p = 0; p < d2; ++p)
+    for (int q = p; q < d2; ++q) {
+      rc = reduce_dot(h, h->LH + (size_t)p * nlh, h->LH + (size_t)q * nlh, nlh, h->rho + p * d2 + q); if (rc) return rc;
+    }
+  CU(h, cudaMemcpyAsync(h->h_pinned + 64, h->rho, sizeof(double) * d2 * d2, cudaMemcpyDeviceToHost, h->stream));
+  CU(h, cudaStreamSynchronize(h->stream));
+  const double* r = h->h_pinned + 64;
+  double num = 0.0, den = 0.0;
+  for (int s1 = 0; s1 < d; ++s1) for (int s1p = 0; s1p < d; ++s1p)
+    for (int s2 = 0; s2 < d; ++s2) for (int s2p = 0; s2p < d; ++s2p) {
+      const int p = s1 * d + s1p, q = s2 * d + s2p;
+      const double v = p <= q ? r[p * d2 + q] : r[q * d2 + p];
+      if (rho_out) rho_out[((s1 * d + s1p) * d + s2) * d + s2p] = v;
+      num += v * H[(size_t)(s1 * d + s2) * d2 + (s1p * d + s2p)];
+      if (s1 == s1p && s2 == s2p) den += v;
+    }
+  if (!(den != 0.0)) return fail(h, QRCTM_ERR_NUMERIC, "zero two-site norm");
+  *e_bond = num / den;
   return QRCTM_OK;
 }
 

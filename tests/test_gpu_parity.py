@@ -409,3 +409,24 @@ def test_odd_chi_and_d3_run_parity():
         assert rel(C, Co) < 1e-10 and rel(T, To) < 1e-10
         assert abs(h.norm_per_site() / o.kappa(Co, To, a) - 1) < 1e-9
         h.close()
+
+
+@pytest.mark.parametrize("d,D,chi,seed,steps", [(2, 2, 8, 0, 30), (2, 3, 20, 1, 10), (3, 2, 6, 4, 5), (2, 4, 32, 2, 3)])
+def test_energy_nn_matches_oracle(d, D, chi, seed, steps):
+    """NEXT-3: two-site RDM and bond energy from the GPU half network vs the oracle, same environment."""
+    g = np.random.default_rng(seed + 100)
+    A, C0, T0 = gen_config(d, D, chi, seed)
+    H = g.standard_normal((d * d, d * d)); H = H + H.T
+    h = pkg.QRCTM(d, D, chi)
+    h.set_A(A); h.set_env(C0, T0)
+    h.run(steps, -1.0)
+    C, T = h.get_env()
+    e, rho = h.energy_nn(H, return_rho=True)
+    rho_o = o.rdm2(C, T, A)
+    assert rel(rho, rho_o) < 1e-11
+    assert abs(e - o.energy_nn(C, T, A, H)) < 1e-10 * max(1.0, abs(e))
+    assert abs(h.energy_nn(np.eye(d * d)) - 1.0) < 1e-12
+    C2, T2 = h.get_env()
+    assert np.array_equal(C, C2) and np.array_equal(T, T2)        # the environment is untouched
+    h.step()                                                      # and the step still works afterwards
+    h.close()
