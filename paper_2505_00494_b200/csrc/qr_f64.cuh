@@ -273,157 +273,14 @@ qr_panel_cluster_kernel(double* __restrict__ V, long long ld, long long m, int j
 }
 
 // ------------------------------------------------------------------------------
-// Register-resident panel kernel (default path).  Same algorithm as above, but
-// every thread keeps its RPT rows of its column in REGISTERS and column k is
-// broadcast inside the (half-)warp with shuffles, so a column step costs no
-// shared-memory traffic for the panel itself (the shared-memory version is bound
-// by the 128 B/clk LDS bandwidth: ncu, profiles/).  All NB lanes take part in the
-// dot products: lanes j >= k give the reflector/update terms g_j, lanes a < k give
-// h_a = sum_{i>r} x_a[i] x_k[i], from which the Gram entries of the compact-WY
-// recurrence follow at no extra pass:
-//     G[a][k] = v_a^T v_k = scale_a (scale_k h_a + x_a[r]),
-//     T[a][k] = -tau_k sum_{c=a}^{k-1} T[a][c] G[c][k],  T[k][k] = tau_k.
-// Thread layout: col = tid % NB, row group rg = tid / NB, local rows rg + t*NRG.
-template <int NB, int NT, int RPT>
-__global__ void __launch_bounds__(NT, 1)
-qr_panel_reg_kernel(double* __restrict__ V, long long ld, long long m, int j0, int nbw,
-                    double* __restrict__ Vc, double* __restrict__ tau, double* __restrict__ Tp, long long rpc) {
-  namespace cg = cooperative_groups;
-  cg::cluster_group cluster = cg::this_cluster();
-  const int C = (int)cluster.num_blocks();
-  const int rank = (int)cluster.block_rank();
-  constexpr int NRG = NT / NB, NW = NT / 32;
-  __shared__ double exch[2 * 16 * NB];
-  __shared__ double rowv[2 * NB];
-  __shared__ double red[NW * NB];
-  __shared__ double par[3 * NB];          // scale, beta, tau per column
-  __shared__ double wv[NB + 2];
-  __shared__ double Gcol[NB];
-  __shared__ double Ts[NB * NB];
-
-  const int tid = threadIdx.x, col = tid % NB, rg = tid / NB, warp = tid >> 5, lane = tid & 31;
-  const int lane_base = lane & ~(NB - 1);
-  const long long row_lo = (long long)j0 + (long long)rank * rpc;
-  long long row_hi = row_lo + rpc; if (row_hi > m) row_hi = m;
-  const int nloc = row_hi > row_lo ? (int)(row_hi - row_lo) : 0;
-  double* const gpan = V + row_lo * ld + j0;
-
-  double val[RPT];
-#pragma unroll
-  for (int t = 0; t < RPT; ++t) {
-    const int li = rg + t * NRG;
-    val[t] = (li < nloc && col < nbw) ? gpan[(long long)li * ld + col] : 0.0;
-  }
-  for (int i = tid; i < NB * NB; i += NT) Ts[i] = 0.0;
-  __syncthreads();
-  cluster.sync();
-
-  int buf = 0;
-  for (int k = 0; k < nbw; ++k) {
-    const long long r = (long long)j0 + k;
-    long long lo64 = r + 1 - row_lo; if (lo64 < 0) lo64 = 0; if (lo64 > nloc) lo64 = nloc;
-    const int lo = (int)lo64;
-    const int t0 = lo <= rg ? 0 : (lo - rg + NRG - 1) / NRG;        // first t with row strictly below r
-    const bool owner = (r >= row_lo && r < row_hi);
-    const int lr_ = owner ? (int)(r - row_lo) : -1;
-    const bool mine = owner && (lr_ % NRG) == rg;                   // this thread holds row r of its column
-    const int tr = owner ? lr_ / NRG : -1;
-    double a0 = 0.0, a1 = 0.0, rvv = 0.0;
-    double xs[RPT];                                   // column k of my rows, broadcast once per step
-#pragma unroll
-    for (int t = 0; t < RPT; ++t) {
-      xs[t] = __shfl_sync(0xffffffffu, val[t], lane_base | k);
-      if (t >= t0) { if (t & 1) a1 = fma(xs[t], val[t], a1); else a0 = fma(xs[t], val[t], a0); }
-      if (mine && t == tr) rvv = val[t];
-    }
-    double acc = a0 + a1;
-    if (NB == 16) acc += __shfl_xor_sync(0xffffffffu, acc, 16);
-    if (lane < NB) red[warp * NB + lane] = acc;
-    __syncthreads();
-    if (tid < NB) {
-      double g = 0.0;
-#pragma unroll
-      for (int w = 0; w < NW; ++w) g += red[w * NB + tid];
-      for (int q = 0; q < C; ++q) {
-        double* rex = cluster.map_shared_rank(exch, q);
-        rex[(buf * 16 + rank) * NB + tid] = g;
-      }
-    }
-    if (mine) {
-      for (int q = 0; q < C; ++q) { double* rr = cluster.map_shared_rank(rowv, q); rr[buf * NB + col] = rvv; }
-    }
-    cluster.sync();
-    if (tid < NB) {
-      double gk = 0.0, gj = 0.0;
-      for (int q = 0; q < C; ++q) { gk += exch[(buf * 16 + q) * NB + k]; gj += exch[(buf * 16 + q) * NB + tid]; }
-      const double alpha = rowv[buf * NB + k], yrj = rowv[buf * NB + tid];
-      double tk = 0.0, scale = 0.0, beta = alpha;
-      if (gk > 0.0) {
-        double sigma = sqrt(fma(alpha, alpha, gk));
-        beta = alpha >= 0.0 ? -sigma : sigma;
-        tk = (beta - alpha) / beta;
-        scale = 1.0 / (alpha - beta);
-      }
-      if (tid > k) wv[tid] = tk * fma(scale, gj, yrj);
-      else if (tid < k) Gcol[tid] = par[tid] * fma(scale, gj, yrj);     // G[a][k], a = tid
-      if (tid == 0) { par[k] = scale; par[NB + k] = beta; par[2 * NB + k] = tk; wv[NB] = scale; wv[NB + 1] = tk; }
-    }
-    __syncthreads();
-    const double tk = wv[NB + 1];
-    if (tid < NB) {                                   // column k of T (every CTA keeps an identical copy)
-      if (tid == k) Ts[k * NB + k] = tk;
-      else if (tid < k) {
-        double s0 = 0.0, s1 = 0.0;
-#pragma unroll
-        for (int c = 0; c < NB; c += 2) {
-          if (c >= tid && c < k) s0 = fma(Ts[tid * NB + c], Gcol[c], s0);
-          if (c + 1 >= tid && c + 1 < k) s1 = fma(Ts[tid * NB + c + 1], Gcol[c + 1], s1);
-        }
-        Ts[tid * NB + k] = -tk * (s0 + s1);
-      }
-    }
-    if (tk != 0.0) {
-      const bool upd = col > k && col < nbw;
-      const double w = upd ? wv[col] : 0.0, scale = wv[NB];
-      const double nsw = -scale * w;
-#pragma unroll
-      for (int t = 0; t < RPT; ++t) {
-        if (upd && t >= t0) val[t] = fma(xs[t], nsw, val[t]);
-        if (upd && mine && t == tr) val[t] -= w;
-      }
-    }
-    __syncthreads();
-    buf ^= 1;
-  }
-
-  double* const gvc = Vc + row_lo * ld + j0;
-  if (col < nbw) {
-    const double sc = par[col], be = par[NB + col];
-    const long long rc = (long long)j0 + col;
-#pragma unroll
-    for (int t = 0; t < RPT; ++t) {
-      const int li = rg + t * NRG;
-      if (li < nloc) {
-        const long long gi = row_lo + li;
-        double vout, vclean;
-        if (gi > rc) { vclean = val[t] * sc; vout = vclean; }
-        else if (gi == rc) { vclean = 1.0; vout = be; }
-        else { vclean = 0.0; vout = val[t]; }
-        gpan[(long long)li * ld + col] = vout;
-        gvc[(long long)li * ld + col] = vclean;
-      }
-    }
-  }
-  if (rank == 0) {
-    if (tid < nbw) tau[j0 + tid] = par[2 * NB + tid];
-    for (int i = tid; i < NB * NB; i += NT) Tp[i] = Ts[i];
-  }
-  cluster.sync();      // nobody exits while a peer may still address its shared memory
-}
-
-// ------------------------------------------------------------------------------
-// Register-resident panel kernel, second version (the default).  Differences to
-// qr_panel_reg_kernel: (1) the diagonal row r of step k is taken out of the register
+// Register-resident panel kernel (the default).  Same algorithm as the shared-memory kernel above, but
+// every thread keeps its RPT rows of its column in REGISTERS and column k is broadcast inside the
+// (half-)warp with shuffles, so a column step costs no shared-memory traffic for the panel itself (the
+// shared-memory version is bound by the 128 B/clk LDS bandwidth: ncu, profiles/).  All NB lanes take part
+// in the dot products: lanes j >= k give the reflector/update terms g_j, lanes a < k give
+// h_a = sum_{i>r} x_a[i] x_k[i], from which the Gram entries of the compact-WY recurrence follow at no
+// extra pass:  G[a][k] = v_a^T v_k = scale_a (scale_k h_a + x_a[r]).  Further: (1) the diagonal row r of
+// step k is taken out of the register
 // tile at the START of the step (its values travel through `rowv`, its final R / v
 // entries are written straight to global memory), so the register tile only ever
 // holds rows strictly below the current diagonal and the dot / update loops carry no

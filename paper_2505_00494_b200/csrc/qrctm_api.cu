@@ -25,7 +25,7 @@ constexpr size_t kAlign = 256;
 inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {   // byte offsets into the workspace
-  size_t A, a_mat, a2_mat, LH, rho, B1, B2, P1, C, T, Cn, Tn, X, V, Q, R, Rt, tau, P, S, W, E, splitk, partial, scal, flag, Wc, dvec, evec,
+  size_t A, a_mat, a2_mat, LH, rho, B1, B2, P1, C, T, Cn, Tn, X, Q, R, Rt, P, S, W, E, splitk, partial, scal, flag, Wc, dvec, evec,
       vv, pv, eig, s, s_prev, s_tmp, delta, qrwork, total;
   long long lda_a, ld1, ld2;
   size_t splitk_elems, qrwork_bytes;
@@ -57,7 +57,7 @@ struct qrctm {
   double* h_pinned;       // [0] delta, [1..] scratch ; pinned host
   int* h_flag;
   // typed views
-  double *A, *a_mat, *a2_mat, *LH, *rho, *B1, *B2, *P1, *C, *T, *Cn, *Tn, *X, *V, *Q, *R, *Rt, *tau, *P, *S, *W, *E, *splitk, *partial, *scal, *Wc,
+  double *A, *a_mat, *a2_mat, *LH, *rho, *B1, *B2, *P1, *C, *T, *Cn, *Tn, *X, *Q, *R, *Rt, *P, *S, *W, *E, *splitk, *partial, *scal, *Wc,
       *dvec, *evec, *vv, *pv, *eig, *s, *s_prev, *s_tmp, *delta;
   int* flag;
   void* qrwork;
@@ -91,11 +91,9 @@ bool make_layout(int d, int D, int chi, Layout* L) {
   L->Cn = take(dbl * chi * chi);
   L->Tn = take(dbl * m * chi);
   L->X = take(dbl * m * chi);
-  L->V = take(dbl * m * chi);
   L->Q = take(dbl * m * chi);
   L->R = take(dbl * chi * chi);
   L->Rt = take(dbl * chi * chi);
-  L->tau = take(dbl * chi);
   L->P = take(dbl * m * m);
   L->S = take(dbl * m * m);
   L->W = take(dbl * m * chi);
@@ -125,7 +123,7 @@ void bind_views(qrctm* h) {
   char* B = h->base;
   const Layout& L = h->L;
 #define V_(name) h->name = reinterpret_cast<double*>(B + L.name)
-  V_(A); V_(a_mat); V_(a2_mat); V_(LH); V_(rho); V_(B1); V_(B2); V_(P1); V_(C); V_(T); V_(Cn); V_(Tn); V_(X); V_(V); V_(Q); V_(R); V_(Rt); V_(tau); V_(P); V_(S); V_(W);
+  V_(A); V_(a_mat); V_(a2_mat); V_(LH); V_(rho); V_(B1); V_(B2); V_(P1); V_(C); V_(T); V_(Cn); V_(Tn); V_(X); V_(Q); V_(R); V_(Rt); V_(P); V_(S); V_(W);
   V_(E); V_(splitk); V_(partial); V_(scal); V_(Wc); V_(dvec); V_(evec); V_(vv); V_(pv); V_(eig); V_(s);
   V_(s_prev); V_(s_tmp); V_(delta);
 #undef V_
