@@ -724,6 +724,7 @@ void invalidate_graphs(qrctm* h) {
   if (h->g_front) { cudaGraphExecDestroy(h->g_front); h->g_front = nullptr; }
   if (h->g_k7) { cudaGraphExecDestroy(h->g_k7); h->g_k7 = nullptr; }
   h->graph_failed = 0;
+  h->warm_steps = 0;      // one ordinary step first: newly selected kernels set their attributes outside capture
 }
 
 // Capture `body` (which only enqueues work on h->stream) into an executable graph.
