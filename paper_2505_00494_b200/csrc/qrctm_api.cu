@@ -48,6 +48,7 @@ struct qrctm {
   cudaGraphExec_t g_front, g_k7;  // captured K1..K6 and K7 (replayed by step/run)
   long long g_front_n, g_k7_n;    // kernels per replay
   int use_graph, warm_steps, graph_failed;
+  int need_s0;                    // spectrum of the environment set by set_env not computed yet (lazy)
   cudaStream_t side;            // high-priority stream for the overlapped convergence check
   cudaEvent_t ev_env, ev_spec;  // environment ready (main) / spectrum done (side)
   int overlap;
@@ -899,7 +900,7 @@ int qrctm_set_env(qrctm_t* h, const double* C, const double* T) {
   int rc = stage_normalize(h, h->Cn, h->Tn); if (rc) return rc;
   rc = check_flag(h); if (rc) return rc;
   CU(h, cudaMemsetAsync(h->s_prev, 0, sizeof(double) * h->chi, h->stream));
-  rc = stage_spectrum(h, h->s, 1, h->stream); if (rc) return rc;
+  h->need_s0 = 1;      // s_prev = spectrum(C0) is computed by the next qrctm_run, overlapped with its first step
   h->have_env = true;
   return QRCTM_OK;
 }
@@ -922,8 +923,17 @@ int qrctm_run(qrctm_t* h, int max_iter, double tol, int* iters_done, double* fin
     double delta = INFINITY;
     int done = 0;
     bool pending = false;                       // a spectrum result is in flight on the side stream
+    bool s0_inflight = false;
+    if (h->need_s0 && max_iter > 0) {           // s_prev = spectrum(C0) on the side stream, under step 1's K1..K6
+      CU(h, cudaEventRecord(h->ev_env, h->stream));
+      CU(h, cudaStreamWaitEvent(h->side, h->ev_env, 0));
+      int rc0 = stage_spectrum(h, h->s, 1, h->side); if (rc0) return rc0;
+      CU(h, cudaEventRecord(h->ev_spec, h->side));
+      h->need_s0 = 0; s0_inflight = true;
+    }
     for (int it = 1; it <= max_iter; ++it) {
       int rc = run_front(h, nullptr); if (rc) return rc;
+      if (s0_inflight) { CU(h, cudaStreamWaitEvent(h->stream, h->ev_spec, 0)); s0_inflight = false; }   // K7 overwrites C
       if (pending) {
         CU(h, cudaEventSynchronize(h->ev_spec));
         pending = false;
@@ -954,6 +964,7 @@ int qrctm_run(qrctm_t* h, int max_iter, double tol, int* iters_done, double* fin
     if (final_delta) *final_delta = delta;
     return QRCTM_OK;
   }
+  if (h->need_s0 && max_iter > 0) { int rc0 = stage_spectrum(h, h->s, 1, h->stream); if (rc0) return rc0; h->need_s0 = 0; }
   double delta = INFINITY;
   int it = 0;
   if (h->time_stages && !h->have_ev) {
