@@ -258,6 +258,7 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
     const int pad128 = (c.N + 127) / 128 * 128, pad104 = (c.N + 103) / 104 * 104, pad64 = (c.N + 63) / 64 * 64;
     if (c.N <= 56) *err = launch_cfg_ws<128, 56, 32, 56, 3>(st, g, c.batch);
     else if (pad64 <= pad104 && pad64 <= pad128) *err = launch_cfg_ws<128, 64, 64, 32, 4>(st, g, c.batch);
+    else if (pad104 <= pad128 && nkt <= 6) *err = launch_cfg_ws<64, 104, 16, 104, 3>(st, g, c.batch);   // 2 CTAs/SM
     else if (pad104 <= pad128) *err = launch_cfg_ws<128, 104, 16, 104, 4>(st, g, c.batch);
     else *err = launch_cfg_ws<128, 128, 64, 32, 4>(st, g, c.batch);
     return *err == cudaSuccess ? 1 : -1;
