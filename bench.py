@@ -234,6 +234,34 @@ def main():
     h.set_option(pkg.OPT_TIME_STAGES, 0)
     assert nst == args.steps
 
+    # ---- bandwidth-bound stages (L2-resident at these sizes, reported against the measured HBM copy rate)
+    Ad = torch.from_numpy(A).cuda()
+    for _ in range(2):
+        h.set_A(Ad)
+    torch.cuda.synchronize()
+    ev0.record(h.stream)
+    for _ in range(5):
+        h.set_A(Ad)
+    ev1.record(h.stream)
+    torch.cuda.synchronize()
+    k0_ms = ev0.elapsed_time(ev1) / 5
+    k0_bytes = 8 * (b ** 4) + 8 * 3 * d * D ** 4                  # a written; A read, two layered copies of A written
+    k7_ms = stage_ms["K7_normalize"] / nst
+    k7_bytes = 8 * (chi * chi + chi * b * chi) * 5                 # pass 1: read x2 (symmetrisation partner) + write, pass 2: read + write
+    hbm_peak = None
+    try:
+        hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+    except Exception:
+        hbm_peak = 6650.0                                          # guide fallback
+    hbm_kernels = {
+        "peak_gbs": hbm_peak,
+        "K0_build_a": {"ms": k0_ms, "gbytes": k0_bytes / 1e9, "gbs": k0_bytes / (k0_ms * 1e-3) / 1e9,
+                       "frac": k0_bytes / (k0_ms * 1e-3) / 1e9 / hbm_peak},
+        "K7_normalize": {"ms": k7_ms, "gbytes": k7_bytes / 1e9, "gbs": k7_bytes / (k7_ms * 1e-3) / 1e9,
+                         "frac": k7_bytes / (k7_ms * 1e-3) / 1e9 / hbm_peak,
+                         "note": "two launches over an L2-resident 15 MB working set: launch-latency-bound"},
+    }
+
     # ---- NEXT-1 variant: layered absorption, same result up to rounding, own flop count
     layered = None
     if chi % 2 == 0:
@@ -331,6 +359,7 @@ def main():
                                         "(MEASURED_PEAKS.json has no FP64 entry; nominal 148 SM x 64 FMA/clk x 1.965 GHz = 37.2)",
                          "dfma_peak": peak_dfma, "algorithmic_flops_per_launch": fl["K4"], "ms_per_launch": k4_ms},
             "stages_ms": {k: v / nst for k, v in stage_ms.items()},
+            "hbm_kernels": hbm_kernels,
             "next_1_layered": layered,
             "step_tflops": sum(fl.values()) / (ms_per_step * 1e-3) / 1e12,
             "step_frac_of_fp64_peak": sum(fl.values()) / (ms_per_step * 1e-3) / 1e12 / peak_dmma,

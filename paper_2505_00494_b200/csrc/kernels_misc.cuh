@@ -53,19 +53,20 @@ __device__ __forceinline__ double block_max(double v, double* sh) {
 // (padded so every row is 16-byte aligned for the GEMM's vector loads).
 __global__ void build_a_kernel(const double* __restrict__ A, int d, int D, double* __restrict__ a_mat,
                                long long lda_a) {
-  const int b = D * D;
-  const long long n = (long long)b * b * b * b;
+  // one block per matrix row (u,l); threads run along the contiguous column index (d,r)
+  const int b = D * D, b2 = b * b;
   const long long DD = (long long)D * D * D * D;
-  for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < n;
-       idx += (long long)gridDim.x * blockDim.x) {
-    int r = (int)(idx % b), dd = (int)((idx / b) % b), l = (int)((idx / ((long long)b * b)) % b),
-        u = (int)(idx / ((long long)b * b * b));
-    int uk = u / D, ub = u % D, lk = l / D, lb = l % D, dk = dd / D, db = dd % D, rk = r / D, rb = r % D;
-    long long ik = (((long long)uk * D + lk) * D + dk) * D + rk;
-    long long ib = (((long long)ub * D + lb) * D + db) * D + rb;
+  const int row = blockIdx.x, u = row / b, l = row % b;
+  const int uk = u / D, ub = u % D, lk = l / D, lb = l % D;
+  const long long rk0 = ((long long)uk * D + lk) * D * D, rb0 = ((long long)ub * D + lb) * D * D;
+  double* out = a_mat + (long long)row * lda_a;
+  for (int c = threadIdx.x; c < b2; c += blockDim.x) {
+    const int dd = c / b, r = c % b;
+    const int dk = dd / D, db = dd % D, rk = r / D, rb = r % D;
+    const long long ik = rk0 + dk * D + rk, ib = rb0 + db * D + rb;
     double s = 0.0;
     for (int sidx = 0; sidx < d; ++sidx) s = fma(A[sidx * DD + ik], A[sidx * DD + ib], s);
-    a_mat[((long long)u * b + l) * lda_a + (long long)dd * b + r] = s;
+    out[c] = s;
   }
 }
 

@@ -840,6 +840,13 @@ static int create_common(int d, int D, int chi, void* ws, unsigned long long ws_
   }
   h->h_flag = reinterpret_cast<int*>(h->h_pinned + 32);       // [64..319] holds the two-site RDM
   cudaMemsetAsync(h->flag, 0, 4 * sizeof(int), 0);
+  {   // padded operand matrices: the pad columns are zeroed once and never written again
+    const size_t b2 = (size_t)h->b * h->b;
+    cudaMemsetAsync(h->a_mat, 0, sizeof(double) * b2 * L.lda_a, 0);
+    cudaMemsetAsync(h->a2_mat, 0, sizeof(double) * b2 * L.lda_a, 0);
+    cudaMemsetAsync(h->B1, 0, sizeof(double) * h->b * L.ld1, 0);
+    cudaMemsetAsync(h->B2, 0, sizeof(double) * (size_t)d * h->b * L.ld2, 0);
+  }
   cudaMemsetAsync(h->s_prev, 0, sizeof(double) * chi, 0);
   cudaMemsetAsync(h->R, 0, sizeof(double) * chi * chi, 0);
   cudaMemsetAsync(h->Q, 0, sizeof(double) * h->m * chi, 0);
@@ -880,12 +887,7 @@ int qrctm_set_A(qrctm_t* h, const double* A) {
   if (!h || !A) return h ? fail(h, QRCTM_ERR_INVALID_ARG, "null A") : QRCTM_ERR_INVALID_ARG;
   long long b2 = (long long)h->b * h->b;
   CU(h, copy_in(h->A, A, (size_t)h->d * b2, h->stream));
-  CU(h, cudaMemsetAsync(h->a_mat, 0, sizeof(double) * b2 * h->L.lda_a, h->stream));
-  long long n = b2 * b2;
-  int nb = (int)((n + 255) / 256); if (nb > 148 * 8) nb = 148 * 8;
-  build_a_kernel<<<nb, 256, 0, h->stream>>>(h->A, h->d, h->D, h->a_mat, h->L.lda_a);
-  CU(h, cudaMemsetAsync(h->B1, 0, sizeof(double) * h->b * h->L.ld1, h->stream));
-  CU(h, cudaMemsetAsync(h->B2, 0, sizeof(double) * h->d * h->b * h->L.ld2, h->stream));
+  build_a_kernel<<<(unsigned)b2, 256, 0, h->stream>>>(h->A, h->d, h->D, h->a_mat, h->L.lda_a);
   build_layers_kernel<<<64, 256, 0, h->stream>>>(h->A, h->d, h->D, h->B1, h->L.ld1, h->B2, h->L.ld2);
   h->launches += 2;
   CU(h, cudaGetLastError());
@@ -1147,7 +1149,6 @@ int qrctm_energy_nn(qrctm_t* h, const double* H, double* e_bond, double* rho_out
   rc = stage_half_absorb(h, h->X, h->T, h->P); if (rc) return rc;
   const long long b2 = (long long)h->b * h->b, n = b2 * b2;
   int nb = (int)((n + 255) / 256); if (nb > 148 * 8) nb = 148 * 8;
-  CU(h, cudaMemsetAsync(h->a2_mat, 0, sizeof(double) * b2 * h->L.lda_a, h->stream));
   for (int s = 0; s < d; ++s)
     for (int sp = 0; sp < d; ++sp) {
       build_a_pair_kernel<<<nb, 256, 0, h->stream>>>(h->A, h->D, s, sp, h->a2_mat, h->L.lda_a);
