@@ -35,6 +35,19 @@ def test_P4_c4v_parameter_count(D, count):
         assert 2 * count == 1332          # "1'332 for D=8" (d=2)
 
 
+def test_P4_golden_fixture_from_the_paper():
+    """tests/golden/c4v_parameter_count.txt: the count the paper prints (1332 for D=8, d=2) and
+    fn.[47]'s formula against the rank of the generator's symmetriser (Burnside count)."""
+    import os
+    path = os.path.join(os.path.dirname(__file__), "golden", "c4v_parameter_count.txt")
+    rows = [tuple(int(x) for x in ln.split()) for ln in open(path) if ln.strip() and not ln.startswith("#")]
+    assert (2, 8, 1332) in rows
+    for d, D, n in rows:
+        idx = np.array(list(itertools.product(range(D), repeat=4)))
+        fixed = sum(int(np.all(idx[:, list(p)] == idx, axis=1).sum()) for p in C4V_PERMS)
+        assert d * fixed // 8 == n and (d * fixed) % 8 == 0
+
+
 def test_P4_symmetrizer_is_projector_of_that_rank():
     D = 3
     n = D ** 4
