@@ -289,6 +289,33 @@ qr_panel_cluster_kernel(double* __restrict__ V, long long ld, long long m, int j
 // __syncthreads and (multi-CTA only) ONE cluster barrier; (3) the compact-WY column
 // of T is built by warp 0 with shuffles off the critical path of the other warps.
 // The panel's diagonal rows j0..j0+nbw-1 are the first local rows of rank 0 (t = 0).
+// --- DSMEM exchange primitives: remote store that completes bytes on the destination CTA's mbarrier
+__device__ __forceinline__ uint32_t qr_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ uint32_t qr_mapa(uint32_t addr, uint32_t rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;\n" : "=r"(r) : "r"(addr), "r"(rank));
+  return r;
+}
+__device__ __forceinline__ void qr_st_async(uint32_t remote_addr, double v, uint32_t remote_bar) {
+  asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b64 [%0], %1, [%2];\n"
+               :: "r"(remote_addr), "l"(__double_as_longlong(v)), "r"(remote_bar) : "memory");
+}
+__device__ __forceinline__ void qr_mbar_init(uint64_t* b, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" :: "r"(qr_smem_u32(b)), "r"(count));
+}
+__device__ __forceinline__ void qr_mbar_arm(uint64_t* b, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" :: "r"(qr_smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void qr_mbar_wait(uint64_t* b, uint32_t parity) {
+  asm volatile(
+      "{\n.reg .pred p;\nQRW_%=:\n"
+      "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra QRD_%=;\nbra QRW_%=;\nQRD_%=:\n}\n" :: "r"(qr_smem_u32(b)), "r"(parity) : "memory");
+}
+#ifndef QR_STAMP
+#define QR_STAMP(i) do { } while (0)      // phase time stamps for the measurement harness (profiles/r1_qr_panel_phases.md)
+#endif
+
 template <int NB, int NT, int RPT, bool CLUSTER>
 __global__ void __launch_bounds__(NT, 1)
 qr_panel_reg2_kernel(double* __restrict__ V, long long ld, long long m, int j0, int nbw,
@@ -303,6 +330,7 @@ qr_panel_reg2_kernel(double* __restrict__ V, long long ld, long long m, int j0, 
   __shared__ double exch[2 * 16 * NB];
   __shared__ double rowv[2 * NB];
   __shared__ double red[2 * NW * NB];
+  __shared__ uint64_t xbar[2];                 // per-buffer mbarrier: bytes of all ranks' partials + the diagonal row
   __shared__ double Gs[NB * NB];               // Gs[a][k] = v_a^T v_k (a < k), filled column by column
   __shared__ double taus[NB];
   __shared__ double Ts[NB * NB];
@@ -323,9 +351,14 @@ qr_panel_reg2_kernel(double* __restrict__ V, long long ld, long long m, int j0, 
       val[t] = (rg + t * NRG < nloc && col < nbw) ? *pl : 0.0;
   }
   for (int i = tid; i < NB * NB; i += NT) { Ts[i] = 0.0; Gs[i] = 0.0; }
+  if (CLUSTER && tid == 0) {
+    qr_mbar_init(&xbar[0], 1); qr_mbar_init(&xbar[1], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
   double my_scale = 0.0;                       // scale of this thread's column once it has been factored
   __syncthreads();
   if (CLUSTER) cluster.sync();
+  const uint32_t exch_a = qr_smem_u32(exch), rowv_a = qr_smem_u32(rowv);
 
   int buf = 0;
   for (int k = 0; k < nbw; ++k) {
@@ -334,8 +367,10 @@ qr_panel_reg2_kernel(double* __restrict__ V, long long ld, long long m, int j0, 
     double rvv = 0.0;
     if (mine) {
       rvv = val[0]; val[0] = 0.0;
-      if (CLUSTER) { for (int q = 0; q < C; ++q) { double* rr = cluster.map_shared_rank(rowv, q); rr[buf * NB + col] = rvv; } }
-      else rowv[buf * NB + col] = rvv;
+      if (CLUSTER) {
+        for (int q = 0; q < C; ++q)
+          qr_st_async(qr_mapa(rowv_a + (buf * NB + col) * 8, q), rvv, qr_mapa(qr_smem_u32(&xbar[buf]), q));
+      } else rowv[buf * NB + col] = rvv;
     }
     // B. column k of my rows, dot with my column.  FP64 dependent-issue latency is long (~30 cycles),
     //    so the sum runs on 8 independent accumulators combined by a fixed tree.
@@ -354,17 +389,20 @@ qr_panel_reg2_kernel(double* __restrict__ V, long long ld, long long m, int j0, 
     __syncthreads();
     double gk = 0.0, gj = 0.0;
     if (CLUSTER) {
-      if (tid < NB) {
+      // every thread sums the warps' partials of ITS column (fixed tree), thread (q = tid / NB) sends it to rank q
+      if (tid == 0) qr_mbar_arm(&xbar[buf], (uint32_t)(C * NB + NB) * 8u);
+      {
         double pg[NW];
 #pragma unroll
-        for (int w = 0; w < NW; ++w) pg[w] = red[(buf * NW + w) * NB + tid];
+        for (int w = 0; w < NW; ++w) pg[w] = red[(buf * NW + w) * NB + col];
 #pragma unroll
         for (int st = 1; st < NW; st *= 2)
 #pragma unroll
           for (int w = 0; w + st < NW; w += 2 * st) pg[w] += pg[w + st];
-        for (int q = 0; q < C; ++q) { double* rex = cluster.map_shared_rank(exch, q); rex[(buf * 16 + rank) * NB + tid] = pg[0]; }
+        for (int q = rg; q < C; q += NRG)
+          qr_st_async(qr_mapa(exch_a + ((buf * 16 + rank) * NB + col) * 8, q), pg[0], qr_mapa(qr_smem_u32(&xbar[buf]), q));
       }
-      cluster.sync();
+      qr_mbar_wait(&xbar[buf], (k >> 1) & 1);
       double pk[16], pj[16];
 #pragma unroll
       for (int q = 0; q < 16; ++q) {
