@@ -650,4 +650,73 @@ wy_update_kernel(const double* __restrict__ Vp, long long ldv, double* __restric
   }
 }
 
+// ------------------------------------------------------------------------------
+// Form Q in one shot (K2c).  With all reflectors V (unit lower trapezoidal, m x n) the product of the
+// Householder transformations is  H_1 ... H_n = I - V T V^T,  T^{-1} = D^{-1} + striu(V^T V), D = diag(tau),
+// so  Q = (I - V T V^T) [I;0] = [I;0] - V X,   X = T V_top^T   (V_top = the first n rows of V),
+// i.e. X solves the upper-triangular system (D^{-1} + striu(G)) X = V_top^T with G = V^T V.  The diagonal blocks
+// of that system are inverted already: (D_p^{-1} + striu(G_pp))^{-1} = T_p, the per-panel compact-WY factors.
+// Blocked back substitution, one CTA per 16 right-hand-side columns:  X_p = T_p (Y_p - sum_{q>p} G_pq X_q).
+template <int NB>
+__global__ void __launch_bounds__(NB * NB)
+wy_formq_trsm_kernel(const double* __restrict__ G, const double* __restrict__ Tfac, const double* __restrict__ Vc,
+                     long long ldv, int n, double* __restrict__ X) {
+  extern __shared__ double xs_[];              // X chunk: n x NB
+  __shared__ double rblk[NB * NB];
+  const int a = threadIdx.x / NB, jj = threadIdx.x % NB;   // entry (a, jj) of a 16 x 16 block
+  const int j = blockIdx.x * NB + jj;                       // right-hand-side column
+  const int npan = (n + NB - 1) / NB;
+  double* gs = xs_ + (size_t)npan * NB * NB;                // G row block: NB x (npan * NB)
+  const int ldg = npan * NB;
+  for (int p = npan - 1; p >= 0; --p) {
+    const int ra = p * NB + a;                              // row of the system
+    // stage rows p*NB .. p*NB+NB-1 of G, columns (p+1)*NB .. n-1, coalesced
+    for (int idx = threadIdx.x; idx < NB * ldg; idx += NB * NB) {
+      const int rr = idx / ldg, cc = idx % ldg;
+      const int gr = p * NB + rr;
+      gs[idx] = (gr < n && cc < n && cc >= (p + 1) * NB) ? G[(long long)gr * n + cc] : 0.0;
+    }
+    __syncthreads();
+    double r = 0.0;
+    if (ra < n && j < n) {
+      r = (j >= ra) ? Vc[(long long)j * ldv + ra] : 0.0;    // Y[ra][j] = V[j][ra] (zero above the diagonal of V)
+      double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+      const int c_lo = (p + 1) * NB, c_hi = npan * NB;      // padded columns hold zeros in gs and xs_
+      for (int c = c_lo; c < c_hi; c += 4) {
+        s0 = fma(gs[a * ldg + c], xs_[c * NB + jj], s0);
+        s1 = fma(gs[a * ldg + c + 1], xs_[(c + 1) * NB + jj], s1);
+        s2 = fma(gs[a * ldg + c + 2], xs_[(c + 2) * NB + jj], s2);
+        s3 = fma(gs[a * ldg + c + 3], xs_[(c + 3) * NB + jj], s3);
+      }
+      r -= (s0 + s1) + (s2 + s3);
+    }
+    rblk[a * NB + jj] = r;
+    __syncthreads();
+    double x = 0.0;
+    const double* Tp = Tfac + (size_t)p * NB * NB;
+    if (ra < n) {
+#pragma unroll
+      for (int c = 0; c < NB; ++c) x = fma(Tp[a * NB + c], rblk[c * NB + jj], x);   // T_p upper triangular (zeros below)
+      if (j < n) X[(long long)ra * n + j] = x;
+    }
+    xs_[ra * NB + jj] = x;                                  // padded rows: zero
+    __syncthreads();
+  }
+}
+
+// Vt[c][r] = V[r][c]  (rows x n -> n x rows), 32 x 32 tiles through shared memory
+__global__ void transpose_tall_kernel(const double* __restrict__ V, long long rows, int n, double* __restrict__ Vt) {
+  __shared__ double tile[32][33];
+  const long long r0 = (long long)blockIdx.x * 32; const int c0 = blockIdx.y * 32;
+  for (int i = threadIdx.y; i < 32; i += blockDim.y) {
+    long long r = r0 + i; int c = c0 + threadIdx.x;
+    tile[i][threadIdx.x] = (r < rows && c < n) ? V[r * n + c] : 0.0;
+  }
+  __syncthreads();
+  for (int i = threadIdx.y; i < 32; i += blockDim.y) {
+    int c = c0 + i; long long r = r0 + threadIdx.x;
+    if (c < n && r < rows) Vt[(long long)c * rows + r] = tile[threadIdx.x][i];
+  }
+}
+
 }  // namespace qk

@@ -334,7 +334,7 @@ constexpr int QR_REG_NT = 256, QR_REG_RPT = 40;                       // 640 row
 constexpr int QR_MAX_PARTS = 320;
 
 struct QrWork {     // carved out of the caller's work buffer
-  double *V, *Vc, *tau, *Tfac, *W1, *W2, *splitk, *part;
+  double *V, *Vc, *tau, *Tfac, *W1, *W2, *splitk, *part, *Vct, *Gq, *Xq;
   size_t splitk_elems;
 };
 
@@ -347,12 +347,15 @@ size_t qr_layout(long long rows, int n, char* base, QrWork* w) {
   size_t sk = (size_t)512 * QR_NB * n;
   size_t oS = take(sk);
   size_t oP = take((size_t)QR_MAX_PARTS * QR_NB_REG * n);
+  size_t oVt = take((size_t)rows * n), oG = take((size_t)n * n), oX = take((size_t)n * n);
   if (w) {
     w->V = reinterpret_cast<double*>(base + oV); w->Vc = reinterpret_cast<double*>(base + oVc);
     w->tau = reinterpret_cast<double*>(base + otau); w->Tfac = reinterpret_cast<double*>(base + oT);
     w->W1 = reinterpret_cast<double*>(base + oW1); w->W2 = reinterpret_cast<double*>(base + oW2);
     w->splitk = reinterpret_cast<double*>(base + oS); w->splitk_elems = sk;
     w->part = reinterpret_cast<double*>(base + oP);
+    w->Vct = reinterpret_cast<double*>(base + oVt); w->Gq = reinterpret_cast<double*>(base + oG);
+    w->Xq = reinterpret_cast<double*>(base + oX);
   }
   return off;
 }
@@ -498,6 +501,9 @@ long long qr_factor_blocked_t(cudaStream_t st, long long rows, int n, const doub
   long long launches = 0;
   *err = cudaMemcpyAsync(wk.V, X, sizeof(double) * rows * n, cudaMemcpyDeviceToDevice, st);
   if (*err != cudaSuccess) return -1;
+  // the clean reflectors are zero above their diagonal: rows above a panel are never written by its kernel
+  *err = cudaMemsetAsync(wk.Vc, 0, sizeof(double) * rows * n, st);
+  if (*err != cudaSuccess) return -1;
   const int npan = (n + NB - 1) / NB;
   for (int p = 0; p < npan; ++p) {
     const int j0 = p * NB, nbw = (n - j0 < NB) ? n - j0 : NB, n2 = n - j0 - nbw;
@@ -513,10 +519,31 @@ long long qr_factor_blocked_t(cudaStream_t st, long long rows, int n, const doub
   copy_triu_kernel<<<(n * n + 255) / 256, 256, 0, st>>>(wk.V, n, n, R);
   set_identity_top_kernel<<<296, 256, 0, st>>>(Q, rows, n);
   launches += 2;
-  for (int p = npan - 1; p >= 0; --p) {      // Q2 <- (I - Vp T Vp^T) Q2, back to front
-    const int j0 = p * NB, nbw = (n - j0 < NB) ? n - j0 : NB;
-    launches += apply_block_reflector<NB>(st, wk.Vc + (long long)j0 * n + j0, n, Q + (long long)j0 * n + j0, n,
-                                          rows - j0, n - j0, nbw, wk.Tfac + (size_t)p * NB * NB, 0, wk);
+  if (npan == 1) {
+    launches += apply_block_reflector<NB>(st, wk.Vc, n, Q, n, rows, n, n, wk.Tfac, 0, wk);
+  } else {
+    // Q = [I;0] - V X with X from the global compact-WY system (see wy_formq_trsm_kernel)
+    auto gemm = [&](const GemmCall& c) -> bool {
+      int nl = launch_gemm(st, 0, c, wk.splitk, wk.splitk_elems, err);
+      if (nl < 0) return false;
+      launches += nl;
+      return true;
+    };
+    const IndexMap unit{1, 1, 0};
+    if (!gemm(GemmCall{wk.Vc, n, 1, wk.Vc, n, wk.Gq, plain_map(n), unit, n, n, (int)rows, 0})) return -1;   // G = V^T V
+    {
+      static bool trsm_attr = false;
+      if (!trsm_attr) {
+        *err = cudaFuncSetAttribute(wy_formq_trsm_kernel<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        if (*err != cudaSuccess) return -1;
+        trsm_attr = true;
+      }
+    }
+    wy_formq_trsm_kernel<NB><<<npan, NB * NB, sizeof(double) * (size_t)npan * NB * NB * 2, st>>>(wk.Gq, wk.Tfac, wk.Vc, n, n,
+                                                                                           wk.Xq);
+    transpose_tall_kernel<<<dim3((unsigned)((rows + 31) / 32), (n + 31) / 32), dim3(32, 8), 0, st>>>(wk.Vc, rows, n, wk.Vct);
+    launches += 2;
+    if (!gemm(GemmCall{wk.Vct, rows, 1, wk.Xq, n, Q, plain_map(n), unit, (int)rows, n, n, 1})) return -1;    // Q -= V X
   }
   sign_fix_kernel<<<296, 256, 0, st>>>(Q, rows, n, R);
   sign_fix_R_kernel<<<n, 128, 0, st>>>(R, n);
