@@ -57,7 +57,8 @@ enum {
   QRCTM_OPT_CHECK_EVERY = 3, /* qrctm_run computes the corner spectrum / delta every n steps, default 1 */
   QRCTM_OPT_GEMM_PATH = 4,   /* 0 = FP64 tensor-core (DMMA) tiles [default], 1 = plain DFMA reference kernel */
   QRCTM_OPT_TIME_STAGES = 5, /* 1 = qrctm_run records CUDA events around every stage of every step (default 0) */
-  QRCTM_OPT_QR_PATH = 6,     /* 0 = blocked compact-WY QR, cluster panel kernel [default], 1 = level-2 column kernels */
+  QRCTM_OPT_QR_PATH = 6,     /* 0 = blocked compact-WY QR, cluster panel kernel [default], 1 = one kernel launch per
+                                Householder reflector (slow reference path for cross-checking) */
   QRCTM_OPT_OVERLAP_CHECK = 7, /* 1 [default] = qrctm_run overlaps the convergence check of step k (side stream) with
                                 K1..K6 of step k+1; results are identical, Q/R/raw buffers then hold the factors of
                                 the last *started* iteration.  0 = strictly serial */
@@ -70,9 +71,10 @@ enum {
 };
 
 /* Create a handle for dimensions (d, D, chi); allocates every workspace with
- * cudaMalloc on the current device (about 16*(chi*D*D)^2 bytes for the two
- * m x m intermediates plus 8*D^8 for the double-layer tensor).  *out = NULL on
- * failure. */
+ * cudaMalloc on the current device (about 32*(chi*D*D)^2 bytes: the two m x m
+ * intermediates P and S plus the 2 m^2 intermediate of the layered mode, plus
+ * 16*D^8 for the double-layer tensors; qrctm_workspace_bytes gives the exact
+ * figure).  *out = NULL on failure. */
 int qrctm_create(int d, int D, int chi, qrctm_t** out);
 
 /* Bytes of device workspace a handle for (d, D, chi) needs (for callers that
@@ -157,7 +159,7 @@ int qrctm_r_diag_ratio(qrctm_t* h, double* ratio);
 int qrctm_set_option(qrctm_t* h, int key, int value);
 
 /* Number of kernels this handle has launched so far (for bench.py's
- * gpu_launches), and reset. */
+ * gpu_launches); kernels replayed from a CUDA graph are counted per replay. */
 long long qrctm_launch_count(const qrctm_t* h);
 
 /* Event-timed profile of one step: runs one qrctm_step with CUDA events around
