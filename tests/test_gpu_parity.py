@@ -430,3 +430,45 @@ def test_energy_nn_matches_oracle(d, D, chi, seed, steps):
     assert np.array_equal(C, C2) and np.array_equal(T, T2)        # the environment is untouched
     h.step()                                                      # and the step still works afterwards
     h.close()
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3a"])
+def test_long_run_parity_at_baseline_iteration_counts(name):
+    """BASELINE.json: cfg1 runs to tol 1e-10 or 500 iterations, cfg2 300 iterations.  North-star bar for the run:
+    relative error <= 1e-9 on the norm per site and on the top-10 normalised corner eigenvalues."""
+    c = CONFIGS[name]
+    A, C0, T0 = gen_config(c["d"], c["D"], c["chi"], c["seed"])
+    a = o.build_a(A)
+    h = pkg.QRCTM(c["d"], c["D"], c["chi"])
+    h.set_A(A); h.set_env(C0, T0)
+    it, dl = h.run(c["iters"], c["tol"])
+    Co, To, ito, dlo, hist = o.run(C0, T0, a, "qr", c["iters"], c["tol"])
+    assert abs(it - ito) <= 1
+    if it != ito:                       # delta crossed tol one step apart: bring the oracle to the same count
+        Co, To, _ = _oracle_steps(A, C0, T0, it)
+    s, so = h.get_corner_spectrum(), o.spectrum(Co)
+    assert np.max(np.abs(s[:10] - so[:10]) / so[:10]) < 1e-9
+    k, ko = h.norm_per_site(), o.kappa(Co, To, a)
+    assert abs(k / ko - 1) < 1e-9
+    if it == c["iters"]:                # hit the cap (hazard H2 for cfg1's seed): deltas must agree too
+        assert abs(dl - hist[-1]) <= 1e-9 * max(1.0, abs(hist[-1])) + 1e-12
+    h.close()
+
+
+def test_cfg4_five_iterations_run_parity():
+    """The headline config through qrctm_run (graphs, overlapped check): 5 iterations against the oracle."""
+    c = CONFIGS["cfg4"]
+    A, C0, T0 = gen_config(c["d"], c["D"], c["chi"], c["seed"])
+    h = pkg.QRCTM(c["d"], c["D"], c["chi"])
+    h.set_A(A); h.set_env(C0, T0)
+    it, dl = h.run(5, -1.0)
+    assert it == 5
+    Co, To, a = _oracle_steps(A, C0, T0, 5)
+    C, T = h.get_env()
+    assert rel(C, Co) < 1e-10 and rel(T, To) < 1e-10
+    s, so = h.get_corner_spectrum(), o.spectrum(Co)
+    assert np.max(np.abs(s[:10] - so[:10]) / so[:10]) < 1e-9
+    so_prev = o.spectrum(_oracle_steps(A, C0, T0, 4)[0])
+    assert abs(dl - np.max(np.abs(so - so_prev))) < 1e-12
+    assert abs(h.norm_per_site() / o.kappa(Co, To, a) - 1) < 1e-9
+    h.close()
