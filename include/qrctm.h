@@ -57,8 +57,10 @@ enum {
   QRCTM_OPT_CHECK_EVERY = 3, /* qrctm_run computes the corner spectrum / delta every n steps, default 1 */
   QRCTM_OPT_GEMM_PATH = 4,   /* 0 = FP64 tensor-core (DMMA) tiles [default], 1 = plain DFMA reference kernel */
   QRCTM_OPT_TIME_STAGES = 5, /* 1 = qrctm_run records CUDA events around every stage of every step (default 0) */
-  QRCTM_OPT_QR_PATH = 6,     /* 0 = blocked compact-WY QR, cluster panel kernel [default], 1 = one kernel launch per
-                                Householder reflector (slow reference path for cross-checking) */
+  QRCTM_OPT_QR_PATH = 6,     /* 0 [default] = automatic: whole-matrix register-resident cluster kernel when c~ fits
+                                (chi <= 112, rows <= 16 x 160..384), else blocked compact-WY with the cluster panel
+                                kernel; 1 = one kernel launch per Householder reflector (slow reference path for
+                                cross-checking); 2 = always the blocked path */
   QRCTM_OPT_OVERLAP_CHECK = 7, /* 1 [default] = qrctm_run overlaps the convergence check of step k (side stream) with
                                 K1..K6 of step k+1; results are identical, Q/R/raw buffers then hold the factors of
                                 the last *started* iteration.  0 = strictly serial */

@@ -500,6 +500,220 @@ qr_panel_reg2_kernel(double* __restrict__ V, long long ld, long long m, int j0, 
 }
 
 // ------------------------------------------------------------------------------
+// Whole-matrix register-resident QR (small / medium c~: n <= 16 NCS columns, rows <= 16 RPT per CTA, up to 16 CTAs).
+// Same column step as qr_panel_reg2_kernel, but every thread holds its rows of ALL its NCS column slots
+// (column c = cs*16 + tid%16), so the Householder update of the whole trailing matrix happens in registers:
+// no panel / WY-apply launches at all.  The dots of column k with every other column come out of one reduction:
+// columns j > k feed the update, columns a < k give the Gram entries G[a][k] = v_a^T v_k, i.e. the complete
+// V^T V that the one-shot form-Q (wy_formq_trsm_kernel) needs, plus the per-block T_p.  Outputs: R (upper
+// triangle, rows written as they retire), the clean reflectors Vc, tau, G (n x n) and the T_p blocks.
+template <int NCS, int RPT, bool CLUSTER>
+__global__ void __launch_bounds__(256, 1)
+qr_full_reg_kernel(const double* __restrict__ X, long long ld, long long m, int n, double* __restrict__ Rout,
+                   double* __restrict__ Vc, double* __restrict__ tau, double* __restrict__ Gout,
+                   double* __restrict__ Tfac, long long rpc) {
+  namespace cg = cooperative_groups;
+  cg::cluster_group cluster = cg::this_cluster();
+  const int C = CLUSTER ? (int)cluster.num_blocks() : 1;
+  const int rank = CLUSTER ? (int)cluster.block_rank() : 0;
+  constexpr int NB = 16, NT = 256, NRG = NT / NB, NW = NT / 32, NP = NCS * NB;   // NP: padded column count
+  static_assert(RPT >= NCS, "the diagonal rows of column slot cs sit at t = cs");
+  extern __shared__ __align__(16) double fsm[];
+  double* exch = fsm;                       // [2][16][NP]
+  double* rowv = exch + 2 * 16 * NP;        // [2][NP]
+  double* red = rowv + 2 * NP;              // [2][NW][NP]
+  double* gsum = red + 2 * NW * NP;         // [NP]   cluster-wide sums of the current column step
+  double* Gs = gsum + NP;                   // [NP][NP]
+  double* taus = Gs + NP * NP;              // [NP]
+  double* scl = taus + NP;                  // [NP]   scale of every factored column
+  __shared__ uint64_t xbar[2];
+
+  const int tid = threadIdx.x, col = tid % NB, rg = tid / NB, warp = tid >> 5, lane = tid & 31;
+  const int lane_base = lane & ~(NB - 1);
+  const long long row_lo = (long long)rank * rpc;
+  long long row_hi = row_lo + rpc; if (row_hi > m) row_hi = m;
+  const int nloc = row_hi > row_lo ? (int)(row_hi - row_lo) : 0;
+
+  double val[NCS][RPT];
+#pragma unroll
+  for (int cs = 0; cs < NCS; ++cs)
+#pragma unroll
+    for (int t = 0; t < RPT; ++t) {
+      const int li = rg + t * NRG, c = cs * NB + col;
+      val[cs][t] = (li < nloc && c < n) ? X[(row_lo + li) * ld + c] : 0.0;
+    }
+  for (int i = tid; i < NP * NP; i += NT) Gs[i] = 0.0;
+  for (int i = tid; i < NP; i += NT) { taus[i] = 0.0; scl[i] = 0.0; }
+  if (CLUSTER && tid == 0) {
+    qr_mbar_init(&xbar[0], 1); qr_mbar_init(&xbar[1], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+  }
+  __syncthreads();
+  if (CLUSTER) cluster.sync();
+  const uint32_t exch_a = qr_smem_u32(exch), rowv_a = qr_smem_u32(rowv);
+
+  int buf = 0, kidx = 0;
+#pragma unroll
+  for (int csk = 0; csk < NCS; ++csk) {
+    for (int kk = 0; kk < NB; ++kk, ++kidx) {
+      const int k = csk * NB + kk;
+      if (k >= n) break;
+      // A. retire the diagonal row r = k: rank 0, row group kk, t = csk (static)
+      const bool mine = (rank == 0) && (rg == kk);
+      double rvv[NCS];
+#pragma unroll
+      for (int cs = 0; cs < NCS; ++cs) rvv[cs] = 0.0;
+      if (mine) {
+#pragma unroll
+        for (int cs = 0; cs < NCS; ++cs) {
+          rvv[cs] = val[cs][csk]; val[cs][csk] = 0.0;
+          if (CLUSTER) {
+            for (int q = 0; q < C; ++q)
+              qr_st_async(qr_mapa(rowv_a + (buf * NP + cs * NB + col) * 8, q), rvv[cs], qr_mapa(qr_smem_u32(&xbar[buf]), q));
+          } else rowv[buf * NP + cs * NB + col] = rvv[cs];
+        }
+      }
+      // B. column k of my rows (shuffle broadcast inside the half warp), dots with all my columns
+      double xs[RPT], acc[NCS];
+#pragma unroll
+      for (int cs = 0; cs < NCS; ++cs) acc[cs] = 0.0;
+#pragma unroll
+      for (int t = 0; t < RPT; ++t) {
+        xs[t] = __shfl_sync(0xffffffffu, val[csk][t], lane_base | kk);
+#pragma unroll
+        for (int cs = 0; cs < NCS; ++cs) acc[cs] = fma(xs[t], val[cs][t], acc[cs]);
+      }
+#pragma unroll
+      for (int cs = 0; cs < NCS; ++cs) {
+        acc[cs] += __shfl_xor_sync(0xffffffffu, acc[cs], 16);
+        if (lane < NB) red[(buf * NW + warp) * NP + cs * NB + lane] = acc[cs];
+      }
+      __syncthreads();
+      // C. CTA sums (fixed tree over the warps), then the cluster exchange
+      if (CLUSTER) {
+        if (tid == 0) qr_mbar_arm(&xbar[buf], (uint32_t)(C * NP + NP) * 8u);
+        for (int e = tid; e < NP * 16; e += NT) {              // (destination rank q, column c)
+          const int c = e % NP, q = e / NP;
+          if (q < C) {
+            double pg[NW];
+#pragma unroll
+            for (int w = 0; w < NW; ++w) pg[w] = red[(buf * NW + w) * NP + c];
+#pragma unroll
+            for (int st = 1; st < NW; st *= 2)
+#pragma unroll
+              for (int w = 0; w + st < NW; w += 2 * st) pg[w] += pg[w + st];
+            qr_st_async(qr_mapa(exch_a + ((buf * 16 + rank) * NP + c) * 8, q), pg[0], qr_mapa(qr_smem_u32(&xbar[buf]), q));
+          }
+        }
+        qr_mbar_wait(&xbar[buf], (kidx >> 1) & 1);
+        if (tid < NP) {
+          double pk[16];
+#pragma unroll
+          for (int q = 0; q < 16; ++q) pk[q] = q < C ? exch[(buf * 16 + q) * NP + tid] : 0.0;
+#pragma unroll
+          for (int st = 1; st < 16; st *= 2)
+#pragma unroll
+            for (int q = 0; q + st < 16; q += 2 * st) pk[q] += pk[q + st];
+          gsum[tid] = pk[0];
+        }
+      } else {
+        if (tid < NP) {
+          double pg[NW];
+#pragma unroll
+          for (int w = 0; w < NW; ++w) pg[w] = red[(buf * NW + w) * NP + tid];
+#pragma unroll
+          for (int st = 1; st < NW; st *= 2)
+#pragma unroll
+            for (int w = 0; w + st < NW; w += 2 * st) pg[w] += pg[w + st];
+          gsum[tid] = pg[0];
+        }
+      }
+      __syncthreads();
+      // F. reflector scalars (identical in every thread)
+      const double gk = gsum[k], alpha = rowv[buf * NP + k];
+      double tk = 0.0, scale = 0.0, beta = alpha;
+      if (gk > 0.0) {
+        const double sigma = sqrt(fma(alpha, alpha, gk));
+        beta = alpha >= 0.0 ? -sigma : sigma;
+        tk = (beta - alpha) / beta;
+        scale = 1.0 / (alpha - beta);
+      }
+      // G/H/I. per column slot: update (columns > k), final row-r entries, Gram column (columns < k)
+#pragma unroll
+      for (int cs = 0; cs < NCS; ++cs) {
+        const int c = cs * NB + col;
+        const double z = fma(scale, gsum[c], rowv[buf * NP + c]);
+        const double w = tk * z;
+        if (c > k && c < n && tk != 0.0) {
+          const double nsw = -scale * w;
+#pragma unroll
+          for (int t = 0; t < RPT; ++t) val[cs][t] = fma(xs[t], nsw, val[cs][t]);
+        }
+        if (mine && c < n) {
+          const double sc_c = scl[c];
+          double vclean, rval;
+          if (c < k) { vclean = rvv[cs] * sc_c; rval = 0.0; }
+          else if (c == k) { vclean = 1.0; rval = beta; }
+          else { vclean = 0.0; rval = (tk != 0.0) ? rvv[cs] - w : rvv[cs]; }
+          Vc[(long long)k * ld + c] = vclean;
+          Rout[(long long)k * n + c] = rval;
+        }
+        if (rg == 0 && c < k) Gs[c * NP + k] = scl[c] * z;
+      }
+      __syncthreads();                                   // everyone has read scl / gsum / rowv of this step
+      if (tid == 0) { taus[k] = tk; scl[k] = scale; if (rank == 0) tau[k] = tk; }
+      buf ^= 1;
+    }
+  }
+  __syncthreads();
+
+  // clean reflectors below the diagonal rows
+#pragma unroll
+  for (int cs = 0; cs < NCS; ++cs) {
+    const int c = cs * NB + col;
+    if (c < n) {
+      const double sc_c = scl[c];
+#pragma unroll
+      for (int t = 0; t < RPT; ++t) {
+        const int li = rg + t * NRG;
+        const long long gi = row_lo + li;
+        if (li < nloc && gi >= n) Vc[gi * ld + c] = val[cs][t] * sc_c;     // rows < n were written when they retired
+      }
+    }
+  }
+  if (rank == 0) {
+    // G (strict upper part is what the solve needs) and the per-block compact-WY factors T_p
+    for (int i = tid; i < n * n; i += NT) { const int a = i / n, c = i % n; Gout[i] = Gs[a * NP + c]; }
+    if (warp == 0 && lane < NB) {
+      const int a = lane;
+      for (int p = 0; p * NB < n; ++p) {
+        double Trow[NB];
+#pragma unroll
+        for (int i = 0; i < NB; ++i) Trow[i] = 0.0;
+#pragma unroll
+        for (int i = 0; i < NB; ++i) {
+          const int gi = p * NB + i;
+          if (gi < n) {
+            const double ti = taus[gi];
+            if (a == i) Trow[i] = ti;
+            else if (a < i) {
+              double sacc = 0.0;
+#pragma unroll
+              for (int c = 0; c < NB; ++c)
+                if (c >= a && c < i) sacc = fma(Trow[c], Gs[(p * NB + c) * NP + gi], sacc);
+              Trow[i] = -ti * sacc;
+            }
+          }
+        }
+#pragma unroll
+        for (int i = 0; i < NB; ++i) Tfac[(size_t)p * NB * NB + a * NB + i] = Trow[i];
+      }
+    }
+  }
+  if (CLUSTER) cluster.sync();
+}
+
+// ------------------------------------------------------------------------------
 // Applying a block reflector  Y <- (I - Vp op(T) Vp^T) Y  to Y = rows x nc (ld ldy):
 // three memory-bound kernels (intensity 2*NB flop per 16 bytes of Y, below the
 // FP64 ridge of ~5.7 flop/B even at NB = 32, so plain DFMA with coalesced row

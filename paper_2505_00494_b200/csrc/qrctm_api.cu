@@ -492,6 +492,9 @@ int apply_block_reflector(cudaStream_t st, const double* Vp, long long ldv, doub
   return 3;
 }
 
+template <int NB>
+long long form_q_global(cudaStream_t st, long long rows, int n, const QrWork& wk, double* Q, cudaError_t* err);
+
 // Blocked Householder QR with compact-WY updates (K2a panel / K2b trailing / K2c form Q + sign fix).
 template <int NB, bool REG>
 long long qr_factor_blocked_t(cudaStream_t st, long long rows, int n, const double* X, double* Q, double* R,
@@ -517,33 +520,16 @@ long long qr_factor_blocked_t(cudaStream_t st, long long rows, int n, const doub
                                             n, rows - j0, n2, nbw, Tp, 1, wk);
   }
   copy_triu_kernel<<<(n * n + 255) / 256, 256, 0, st>>>(wk.V, n, n, R);
-  set_identity_top_kernel<<<296, 256, 0, st>>>(Q, rows, n);
-  launches += 2;
-  if (npan == 1) {
-    launches += apply_block_reflector<NB>(st, wk.Vc, n, Q, n, rows, n, n, wk.Tfac, 0, wk);
-  } else {
-    // Q = [I;0] - V X with X from the global compact-WY system (see wy_formq_trsm_kernel)
-    auto gemm = [&](const GemmCall& c) -> bool {
-      int nl = launch_gemm(st, 0, c, wk.splitk, wk.splitk_elems, err);
-      if (nl < 0) return false;
-      launches += nl;
-      return true;
-    };
-    const IndexMap unit{1, 1, 0};
-    if (!gemm(GemmCall{wk.Vc, n, 1, wk.Vc, n, wk.Gq, plain_map(n), unit, n, n, (int)rows, 0})) return -1;   // G = V^T V
-    {
-      static bool trsm_attr = false;
-      if (!trsm_attr) {
-        *err = cudaFuncSetAttribute(wy_formq_trsm_kernel<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        if (*err != cudaSuccess) return -1;
-        trsm_attr = true;
-      }
-    }
-    wy_formq_trsm_kernel<NB><<<npan, NB * NB, sizeof(double) * (size_t)npan * NB * NB * 2, st>>>(wk.Gq, wk.Tfac, wk.Vc, n, n,
-                                                                                           wk.Xq);
-    transpose_tall_kernel<<<dim3((unsigned)((rows + 31) / 32), (n + 31) / 32), dim3(32, 8), 0, st>>>(wk.Vc, rows, n, wk.Vct);
-    launches += 2;
-    if (!gemm(GemmCall{wk.Vct, rows, 1, wk.Xq, n, Q, plain_map(n), unit, (int)rows, n, n, 1})) return -1;    // Q -= V X
+  launches += 1;
+  {
+    // G = V^T V on the DMMA GEMM (split-K), then the one-shot form-Q
+    int nl = launch_gemm(st, 0, GemmCall{wk.Vc, n, 1, wk.Vc, n, wk.Gq, plain_map(n), IndexMap{1, 1, 0}, n, n, (int)rows, 0},
+                         wk.splitk, wk.splitk_elems, err);
+    if (nl < 0) return -1;
+    launches += nl;
+    long long nq = form_q_global<NB>(st, rows, n, wk, Q, err);
+    if (nq < 0) return -1;
+    launches += nq;
   }
   sign_fix_kernel<<<296, 256, 0, st>>>(Q, rows, n, R);
   sign_fix_R_kernel<<<n, 128, 0, st>>>(R, n);
@@ -552,8 +538,84 @@ long long qr_factor_blocked_t(cudaStream_t st, long long rows, int n, const doub
   return *err == cudaSuccess ? launches : -1;
 }
 
-long long qr_factor_blocked(cudaStream_t st, int /*gemm_path*/, long long rows, int n, const double* X, double* Q,
+// Form Q from the clean reflectors Vc, the Gram matrix G = V^T V (strict upper part) and the per-block T_p:
+// Q = [I;0] - V X, (D^-1 + striu(G)) X = V_top^T  (see wy_formq_trsm_kernel).  Returns launches or -1.
+template <int NB>
+long long form_q_global(cudaStream_t st, long long rows, int n, const QrWork& wk, double* Q, cudaError_t* err) {
+  long long launches = 0;
+  const int npan = (n + NB - 1) / NB;
+  static bool trsm_attr = false;
+  if (!trsm_attr) {
+    *err = cudaFuncSetAttribute(wy_formq_trsm_kernel<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    if (*err != cudaSuccess) return -1;
+    trsm_attr = true;
+  }
+  set_identity_top_kernel<<<296, 256, 0, st>>>(Q, rows, n);
+  wy_formq_trsm_kernel<NB><<<npan, NB * NB, sizeof(double) * (size_t)npan * NB * NB * 2, st>>>(wk.Gq, wk.Tfac, wk.Vc, n, n,
+                                                                                             wk.Xq);
+  transpose_tall_kernel<<<dim3((unsigned)((rows + 31) / 32), (n + 31) / 32), dim3(32, 8), 0, st>>>(wk.Vc, rows, n, wk.Vct);
+  launches += 3;
+  int nl = launch_gemm(st, 0, GemmCall{wk.Vct, rows, 1, wk.Xq, n, Q, plain_map(n), IndexMap{1, 1, 0}, (int)rows, n, n, 1},
+                       wk.splitk, wk.splitk_elems, err);                                            // Q -= V X
+  if (nl < 0) return -1;
+  return launches + nl;
+}
+
+// Whole-matrix register-resident QR for small / medium c~ (n <= 112 columns, one cluster).  Returns -2 if it does not fit.
+template <int NCS, int RPT>
+long long qr_factor_fullreg_t(cudaStream_t st, long long rows, int n, const double* X, double* Q, double* R, const QrWork& wk,
+                              cudaError_t* err) {
+  constexpr int NP = NCS * 16, cap = RPT * 16;
+  static int maxc = -1;
+  constexpr size_t smem = sizeof(double) * (2 * 16 * NP + 2 * NP + 2 * 8 * NP + NP + NP * NP + 2 * NP);
+  if (maxc < 0) {
+    *err = cudaFuncSetAttribute(qr_full_reg_kernel<NCS, RPT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (*err != cudaSuccess) return -1;
+    *err = cudaFuncSetAttribute(qr_full_reg_kernel<NCS, RPT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (*err != cudaSuccess) return -1;
+    maxc = cudaFuncSetAttribute(qr_full_reg_kernel<NCS, RPT, true>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) ==
+                   cudaSuccess ? 16 : 8;
+    cudaGetLastError();
+  }
+  int C = 1;
+  while (C < maxc && (rows + C - 1) / C > cap) C *= 2;
+  const long long rpc = (rows + C - 1) / C;
+  if (rpc > cap || (C > 1 && rpc < n)) return -2;           // too tall, or the diagonal rows would leave rank 0
+  if (C == 1) {
+    qr_full_reg_kernel<NCS, RPT, false><<<1, 256, smem, st>>>(X, (long long)n, rows, n, R, wk.Vc, wk.tau, wk.Gq, wk.Tfac, rpc);
+  } else {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(C); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    *err = cudaLaunchKernelEx(&cfg, qr_full_reg_kernel<NCS, RPT, true>, X, (long long)n, rows, n, R, wk.Vc, wk.tau, wk.Gq,
+                              wk.Tfac, rpc);
+    if (*err != cudaSuccess) return -1;
+  }
+  long long launches = 1;
+  long long nq = form_q_global<16>(st, rows, n, wk, Q, err);
+  if (nq < 0) return -1;
+  launches += nq;
+  sign_fix_kernel<<<296, 256, 0, st>>>(Q, rows, n, R);
+  sign_fix_R_kernel<<<n, 128, 0, st>>>(R, n);
+  launches += 2;
+  *err = cudaGetLastError();
+  return *err == cudaSuccess ? launches : -1;
+}
+
+// qr_path: 0 = automatic (whole-matrix register kernel when it fits, else blocked), 2 = always blocked
+long long qr_factor_blocked(cudaStream_t st, int qr_path, long long rows, int n, const double* X, double* Q,
                             double* R, void* work, cudaError_t* err) {
+  if (qr_path == 0 && n <= 112) {
+    QrWork wk;
+    qr_layout(rows, n, static_cast<char*>(work), &wk);
+    long long nl = n <= 32 ? qr_factor_fullreg_t<2, 24>(st, rows, n, X, Q, R, wk, err)
+                 : n <= 64 ? qr_factor_fullreg_t<4, 16>(st, rows, n, X, Q, R, wk, err)
+                           : qr_factor_fullreg_t<7, 10>(st, rows, n, X, Q, R, wk, err);
+    if (nl != -2) return nl;
+  }
   constexpr long long cap = (long long)QR_REG_RPT * (QR_REG_NT / QR_NB_REG);
   if (rows <= cap * reg_panel_max_cluster())
     return qr_factor_blocked_t<QR_NB_REG, true>(st, rows, n, X, Q, R, work, err);
@@ -731,8 +793,8 @@ int do_step(qrctm* h, cudaEvent_t* ev /* QRCTM_NSTAGE+1 events or null */, bool 
   if (!rc) {
     mark(1, "K2_qr");
     cudaError_t e;
-    long long nl = h->qr_path == 0
-        ? qr_factor_blocked(h->stream, h->gemm_path, h->m, h->chi, h->X, h->Q, h->R, h->qrwork, &e)
+    long long nl = h->qr_path != 1
+        ? qr_factor_blocked(h->stream, h->qr_path, h->m, h->chi, h->X, h->Q, h->R, h->qrwork, &e)
         : qr_factor_level2(h->stream, h->m, h->chi, h->X, h->Q, h->R, h->qrwork, &e);
     if (nl < 0) rc = fail(h, QRCTM_ERR_CUDA, "qr", e); else h->launches += nl;
   }
@@ -1083,7 +1145,7 @@ int qrctm_set_option(qrctm_t* h, int key, int value) {
     case QRCTM_OPT_SYMMETRIZE:  if (value != 0 && value != 1) break; h->symmetrize = value; return QRCTM_OK;
     case QRCTM_OPT_CHECK_EVERY: if (value < 1) break; h->check_every = value; return QRCTM_OK;
     case QRCTM_OPT_GEMM_PATH:   if (value != 0 && value != 1) break; h->gemm_path = value; return QRCTM_OK;
-    case QRCTM_OPT_QR_PATH:     if (value != 0 && value != 1) break; h->qr_path = value; return QRCTM_OK;
+    case QRCTM_OPT_QR_PATH:     if (value < 0 || value > 2) break; h->qr_path = value; return QRCTM_OK;
     case QRCTM_OPT_OVERLAP_CHECK: if (value != 0 && value != 1) break; h->overlap = value; return QRCTM_OK;
     case QRCTM_OPT_ABSORB_MODE: if (value != 0 && value != 1) break; h->absorb_mode = value; return QRCTM_OK;
     case QRCTM_OPT_USE_GRAPH:   if (value != 0 && value != 1) break; h->use_graph = value; return QRCTM_OK;
@@ -1244,11 +1306,11 @@ unsigned long long qrctm_qr_work_bytes(int rows, int cols) { return qr_work_byte
 
 int qrctm_qr_f64(void* cuda_stream, int path, int rows, int cols, const double* X, double* Q, double* R,
                  void* work) {
-  if (!X || !Q || !R || !work || rows < 1 || cols < 1 || cols > rows || (path != 0 && path != 1))
+  if (!X || !Q || !R || !work || rows < 1 || cols < 1 || cols > rows || path < 0 || path > 2)
     return QRCTM_ERR_INVALID_ARG;
   cudaError_t e;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  long long nl = path == 0 ? qr_factor_blocked(st, 0, rows, cols, X, Q, R, work, &e)
+  long long nl = path != 1 ? qr_factor_blocked(st, path, rows, cols, X, Q, R, work, &e)
                            : qr_factor_level2(st, rows, cols, X, Q, R, work, &e);
   return nl < 0 ? QRCTM_ERR_CUDA : QRCTM_OK;
 }

@@ -55,9 +55,9 @@ def test_gemm_odd_leading_dimension_views():
 
 
 @pytest.mark.parametrize("rows,cols", [(32, 8), (324, 36), (1024, 64), (50, 50), (7, 1), (333, 17), (16, 16),
-                                       (2500, 100), (40, 33), (9604, 196), (3000, 150),
+                                       (2500, 100), (40, 33), (9604, 196), (3000, 150), (112, 112), (5000, 64), (1792, 112), (4096, 50),
                                        (15000, 24), (40000, 40)])   # 16-CTA cluster; global-memory panel path
-@pytest.mark.parametrize("path", [0, 1])
+@pytest.mark.parametrize("path", [0, 1, 2])
 def test_qr_f64_matches_oracle(rows, cols, path):
     if path == 1 and rows * cols > 200000:
         pytest.skip("level-2 path only checked on small cases")
@@ -77,7 +77,7 @@ def test_qr_f64_matches_oracle(rows, cols, path):
 def test_qr_rank_deficient_is_still_valid():
     g = np.random.default_rng(3)
     X = g.standard_normal((200, 6)) @ g.standard_normal((6, 12))       # rank 6 < 12 (hazard H1)
-    for path in (0, 1):
+    for path in (0, 1, 2):
         Q, R = pkg.qr_f64(torch_dev(X), path=path)
         Q, R = Q.cpu().numpy(), R.cpu().numpy()
         assert np.linalg.norm(Q.T @ Q - np.eye(12)) < 1e-13
