@@ -54,13 +54,15 @@ def test_gemm_odd_leading_dimension_views():
     assert rel(out, A.cpu().numpy().T @ B.cpu().numpy()) < 1e-13
 
 
-@pytest.mark.parametrize("rows,cols", [(32, 8), (324, 36), (1024, 64), (50, 50), (7, 1), (333, 17), (16, 16),
-                                       (2500, 100), (40, 33), (9604, 196), (3000, 150), (112, 112), (5000, 64), (1792, 112), (4096, 50),
-                                       (15000, 24), (40000, 40)])   # 16-CTA cluster; global-memory panel path
-@pytest.mark.parametrize("path", [0, 1, 2])
+_QR_SHAPES = [(32, 8), (324, 36), (1024, 64), (50, 50), (7, 1), (333, 17), (16, 16),
+              (2500, 100), (40, 33), (9604, 196), (3000, 150), (112, 112), (5000, 64), (1792, 112), (4096, 50),
+              (15000, 24), (40000, 40)]   # 16-CTA cluster; global-memory panel path
+# the per-reflector (level-2) path 1 is only checked on small cases
+_QR_CASES = [(r, c, p) for p in (0, 1, 2) for (r, c) in _QR_SHAPES if not (p == 1 and r * c > 200000)]
+
+
+@pytest.mark.parametrize("rows,cols,path", _QR_CASES)
 def test_qr_f64_matches_oracle(rows, cols, path):
-    if path == 1 and rows * cols > 200000:
-        pytest.skip("level-2 path only checked on small cases")
     g = np.random.default_rng(rows + cols)
     X = g.standard_normal((rows, cols))
     Q, R = pkg.qr_f64(torch_dev(X), path=path)
@@ -355,14 +357,15 @@ def test_cfg3a_ten_steps_and_kappa_parity():
     h.close()
 
 
-@pytest.mark.parametrize("d,D,chi,seed", [(2, 2, 8, 0), (2, 3, 36, 1), (3, 2, 6, 7), (2, 4, 64, 2), (2, 5, 100, 3),
-                                          (2, 7, 196, 4), (2, 3, 7, 8)])
-@pytest.mark.parametrize("path", [0, 1])
+_LAYERED_SIZES = [(2, 2, 8, 0), (2, 3, 36, 1), (3, 2, 6, 7), (2, 4, 64, 2), (2, 5, 100, 3), (2, 7, 196, 4), (2, 3, 7, 8)]
+# the reference GEMM (path 1) is only run on the small cases
+_LAYERED_CASES = [sz + (p,) for p in (0, 1) for sz in _LAYERED_SIZES if not (p == 1 and sz[2] > 40)]
+
+
+@pytest.mark.parametrize("d,D,chi,seed,path", _LAYERED_CASES)
 def test_layered_absorption_matches_oracle_and_explicit(d, D, chi, seed, path):
     """NEXT-1: absorbing the ket and bra layers of A one after the other gives the same T' (and C')
     as the explicit double-layer tensor; odd chi silently uses the explicit path."""
-    if path == 1 and chi > 40:
-        pytest.skip("reference GEMM only on small cases")
     lay, s, (Cr, Tr, Co, To) = _one_step(d, D, chi, seed, absorb=1, path=path)
     assert rel(lay["raw"][1], s["Tn"]) < 1e-11 and rel(lay["raw"][0], s["Cn"]) < 1e-11
     assert rel(lay["C"], Co) < 1e-11 and rel(lay["T"], To) < 1e-11
