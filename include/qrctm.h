@@ -192,6 +192,48 @@ unsigned long long qrctm_qr_work_bytes(int rows, int cols);
 int qrctm_qr_f64(void* cuda_stream, int path, int rows, int cols, const double* X, double* Q,
                  double* R, void* work);
 
+/* ---- NEXT-2: the paper's initialisation and warm-up ----
+ * PAPER.md:28 "we start from an initial boundary that is not obtained from a
+ * previous QR-CTMRG run ... the first one to four steps are done with the standard
+ * CTMRG ... bond dimension chi is grown dynamically"; fn.[48] PAPER.md:132.
+ *
+ * qrctm_get_chi: the CURRENT environment bond dimension (below the capacity the
+ *   handle was created with only between qrctm_init_bulk and the end of the
+ *   warm-up) and that capacity.  Either pointer may be NULL.  HOST pointers.
+ * qrctm_init_bulk: C0[(d d'),(r r')] = sum_{s,u,l} A A, T0[(l l'),(d d'),(r r')] =
+ *   sum_{s,u} A A (fn.[48]), normalised (K7); the current chi becomes D^2.
+ *   Needs set_A; QRCTM_ERR_INVALID_ARG if D^2 > capacity.
+ * qrctm_eig_step: one standard CTMRG iteration (Fig. 1(d)):
+ *   C~ (E5) from the current C, T; its chi_new eigenpairs of largest |lambda|
+ *   (ties: ascending eigenvalue order first, reading A9) -> U, sign gauge
+ *   "largest-magnitude component of every column positive"; C' = diag(lambda),
+ *   T' = (E3) with U for Q; K7.  chi_new = 0 keeps chi; otherwise
+ *   1 <= chi_new <= min(capacity, chi D^2).  The eigensolver is the library's own
+ *   (Householder tridiagonalisation, multisection, inverse iteration; csrc/eigh.cuh)
+ *   and needs chi D^2 <= 14000; its workspace is a separate DEVICE allocation owned
+ *   by the handle, made on first use.  The next qrctm_run starts a fresh convergence
+ *   history (s_prev = spectrum of the new C).
+ * qrctm_get_eig: U (rows x cols, row-major) and lambda (cols) of the last
+ *   qrctm_eig_step; rows/cols (HOST, may be NULL) are always written, U / lam
+ *   (HOST or DEVICE, may be NULL) only if non-NULL.  QRCTM_ERR_NOT_READY before
+ *   the first eigen step.
+ * qrctm_warmup: qrctm_init_bulk, then n_eig_steps eigen steps with
+ *   chi <- min(capacity, chi D^2) each. */
+int qrctm_get_chi(const qrctm_t* h, int* chi, int* chi_capacity);
+int qrctm_init_bulk(qrctm_t* h);
+int qrctm_eig_step(qrctm_t* h, int chi_new);
+int qrctm_get_eig(qrctm_t* h, double* U, double* lam, int* rows, int* cols);
+int qrctm_warmup(qrctm_t* h, int n_eig_steps);
+
+/* Stand-alone entry of the eigensolver used by qrctm_eig_step: the k eigenpairs of
+ * largest |lambda| of the symmetric A[n][n] (DEVICE, row-major, DESTROYED):
+ * lam[k] (DEVICE) in decreasing |lambda| (ties: the smaller eigenvalue first),
+ * U[n][k] (DEVICE, row-major) orthonormal, largest-magnitude component of each
+ * column positive.  1 <= k <= n <= 14000.  work: qrctm_eigh_work_bytes(n, k) bytes
+ * (DEVICE); 0 is returned for unsupported sizes. */
+unsigned long long qrctm_eigh_work_bytes(int n, int k);
+int qrctm_eigh_top_f64(void* cuda_stream, int n, int k, double* A, double* lam, double* U, void* work);
+
 /* FP64 issue-rate probe (roofline denominators):
  * kind 0 = DFMA chains, 1 = DMMA m8n8k4 chains.  Returns TFLOP/s measured with
  * CUDA events over `iters` loop trips on every SM.  HOST pointer. */

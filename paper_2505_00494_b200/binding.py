@@ -33,6 +33,8 @@ SYMBOLS = (
     "qrctm_r_diag_ratio", "qrctm_energy_nn", "qrctm_set_option", "qrctm_launch_count", "qrctm_get_stage_ms", "qrctm_profile_step",
     "qrctm_gemm_f64", "qrctm_qr_work_bytes", "qrctm_qr_f64", "qrctm_probe_fp64", "qrctm_last_error",
     "qrctm_version",
+    "qrctm_get_chi", "qrctm_init_bulk", "qrctm_eig_step", "qrctm_get_eig", "qrctm_warmup",
+    "qrctm_eigh_work_bytes", "qrctm_eigh_top_f64",
 )
 
 
@@ -82,6 +84,14 @@ def load_library() -> ctypes.CDLL:
     lib.qrctm_qr_work_bytes.restype = c_ulonglong
     lib.qrctm_qr_f64.argtypes = [P, c_int, c_int, c_int, P, P, P, P]
     lib.qrctm_probe_fp64.argtypes = [c_int, c_int, POINTER(c_double)]
+    lib.qrctm_get_chi.argtypes = [P, POINTER(c_int), POINTER(c_int)]
+    lib.qrctm_init_bulk.argtypes = [P]
+    lib.qrctm_eig_step.argtypes = [P, c_int]
+    lib.qrctm_get_eig.argtypes = [P, P, P, POINTER(c_int), POINTER(c_int)]
+    lib.qrctm_warmup.argtypes = [P, c_int]
+    lib.qrctm_eigh_work_bytes.argtypes = [c_int, c_int]
+    lib.qrctm_eigh_work_bytes.restype = c_ulonglong
+    lib.qrctm_eigh_top_f64.argtypes = [P, c_int, c_int, P, P, P, P]
     lib.qrctm_last_error.argtypes = [P]
     lib.qrctm_last_error.restype = c_char_p
     lib.qrctm_version.restype = c_char_p
@@ -120,7 +130,7 @@ class QRCTM:
         if not torch.cuda.is_available():
             raise QrctmError("no CUDA device: the QR-CTMRG path has no CPU fallback")
         self.lib = load_library()
-        self.d, self.D, self.chi, self.b = d, D, chi, D * D
+        self.d, self.D, self.chi_cap, self.b = d, D, chi, D * D      # self.chi: the current chi (property)
         nbytes = self.lib.qrctm_workspace_bytes(d, D, chi)
         if nbytes == 0:
             raise QrctmError("invalid (d, D, chi)")
@@ -134,6 +144,13 @@ class QRCTM:
         self.stream = stream if stream is not None else torch.cuda.Stream()
         self.stream.wait_stream(torch.cuda.current_stream())
         self._check(self.lib.qrctm_set_stream(h, c_void_p(self.stream.cuda_stream)))
+
+    @property
+    def chi(self) -> int:
+        """Current environment bond dimension (== the capacity except during the NEXT-2 warm-up)."""
+        c = c_int(0)
+        self._check(self.lib.qrctm_get_chi(self._h, byref(c), None))
+        return c.value
 
     # -- plumbing
     def _check(self, rc: int):
@@ -178,7 +195,8 @@ class QRCTM:
         self._check(self.lib.qrctm_set_A(self._h, _ptr(A)))
 
     def set_env(self, C, T):
-        assert tuple(C.shape) == (self.chi, self.chi) and tuple(T.shape) == (self.chi, self.b, self.chi)
+        n = self.chi_cap
+        assert tuple(C.shape) == (n, n) and tuple(T.shape) == (n, self.b, n)
         self._order_after_caller()
         self._check(self.lib.qrctm_set_env(self._h, _ptr(C), _ptr(T)))
 
@@ -191,8 +209,9 @@ class QRCTM:
         return it.value, dl.value
 
     def get_env(self, device: bool = False):
-        C = self._out((self.chi, self.chi), device)
-        T = self._out((self.chi, self.b, self.chi), device)
+        n = self.chi
+        C = self._out((n, n), device)
+        T = self._out((n, self.b, n), device)
         self._check(self.lib.qrctm_get_env(self._h, _ptr(C), _ptr(T)))
         return C, T
 
@@ -202,16 +221,35 @@ class QRCTM:
         return s
 
     def get_qr(self, device: bool = False):
-        Q = self._out((self.chi * self.b, self.chi), device)
-        R = self._out((self.chi, self.chi), device)
+        n = self.chi
+        Q = self._out((n * self.b, n), device)
+        R = self._out((n, n), device)
         self._check(self.lib.qrctm_get_qr(self._h, _ptr(Q), _ptr(R)))
         return Q, R
 
     def get_raw(self, device: bool = False):
-        Cn = self._out((self.chi, self.chi), device)
-        Tn = self._out((self.chi, self.b, self.chi), device)
+        n = self.chi
+        Cn = self._out((n, n), device)
+        Tn = self._out((n, self.b, n), device)
         self._check(self.lib.qrctm_get_raw(self._h, _ptr(Cn), _ptr(Tn)))
         return Cn, Tn
+
+    def init_bulk(self):
+        self._check(self.lib.qrctm_init_bulk(self._h))
+
+    def eig_step(self, chi_new: int = 0):
+        self._check(self.lib.qrctm_eig_step(self._h, chi_new))
+
+    def get_eig(self, device: bool = False):
+        r, c = c_int(0), c_int(0)
+        self._check(self.lib.qrctm_get_eig(self._h, None, None, byref(r), byref(c)))
+        U = self._out((r.value, c.value), device)
+        lam = self._out((c.value,), device)
+        self._check(self.lib.qrctm_get_eig(self._h, _ptr(U), _ptr(lam), None, None))
+        return U, lam
+
+    def warmup(self, n_eig_steps: int):
+        self._check(self.lib.qrctm_warmup(self._h, n_eig_steps))
 
     def get_a(self):
         a = np.empty((self.b,) * 4, dtype=np.float64)
@@ -290,6 +328,27 @@ def qr_f64(X, path: int = 0):
         raise QrctmError(f"qrctm_qr_f64 failed: {rc}")
     torch.cuda.current_stream().synchronize()
     return Q, R
+
+
+def eigh_top_f64(A, k: int):
+    """(lam, U): the k eigenpairs of largest |lambda| of a symmetric torch CUDA float64 matrix through
+    qrctm_eigh_top_f64 (A is copied; the library destroys its input)."""
+    import torch
+    lib = load_library()
+    n = A.shape[0]
+    nbytes = lib.qrctm_eigh_work_bytes(n, k)
+    if nbytes == 0:
+        raise QrctmError("qrctm_eigh_work_bytes: unsupported (n, k)")
+    W = A.contiguous().clone()
+    lam = torch.empty((k,), dtype=torch.float64, device="cuda")
+    U = torch.empty((n, k), dtype=torch.float64, device="cuda")
+    work = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    rc = lib.qrctm_eigh_top_f64(c_void_p(torch.cuda.current_stream().cuda_stream), n, k, _ptr(W), _ptr(lam), _ptr(U),
+                                c_void_p(work.data_ptr()))
+    if rc != QRCTM_OK:
+        raise QrctmError(f"qrctm_eigh_top_f64 failed: {rc}")
+    torch.cuda.current_stream().synchronize()
+    return lam, U
 
 
 def probe_fp64(kind: int, iters: int = 20000) -> float:

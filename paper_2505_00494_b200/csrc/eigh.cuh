@@ -1,0 +1,367 @@
+// NEXT-2: the standard (eigen) CTMRG step needs "the chi eigenvectors with the largest
+// magnitudes" of the symmetric enlarged corner C~ (reading A9).
+// Hand-written symmetric eigensolver for the k largest-|lambda| pairs of an n x n matrix:
+//   1. Householder tridiagonalisation, one reflector per step, all SMs:
+//        eigh_reflector_kernel (one CTA)  : finishes w_{k-1}, brings row k up to date, builds v_k
+//        eigh_pass_kernel      (grid)     : applies the pending rank-2 update of reflector k-1 to
+//                                           the trailing block and, in the same sweep, y = A22 v_k
+//      (one read + one write of the trailing block per step; HBM/L2-bound)
+//   2. all eigenvalues of the tridiagonal by warp multisection (spectrum.cuh)
+//   3. eigh_select_kernel: the k of largest magnitude, stable in ascending-eigenvalue order
+//   4. eigh_invit_kernel: inverse iteration on the tridiagonal, one thread per vector,
+//      partial-pivoting LU recomputed each sweep, random start vectors
+//   5. Householder QR of the n x k vectors (qr_f64.cuh) -- orthonormality to rounding even for
+//      clustered eigenvalues; R's positive diagonal keeps every vector's direction
+//   6. eigh_backtransform_kernel: U = H_0 ... H_{n-3} Z, two columns per CTA held in shared memory
+//   7. eigh_sign_kernel: largest-|.| component of every column made positive (the sign gauge DESIGN.md fixes)
+#pragma once
+#include "kernels_misc.cuh"
+
+namespace qk {
+
+// One CTA.  Step k of the tridiagonalisation of W (n x n, row-major, symmetric; rows/cols >= k live).
+//   k > 0 : y = A22 v_{k-1} (rows k..n-1) is in y[]; forms w_{k-1} = p - (tau/2)(p.v) v, p = tau y
+//   row k brought up to date: r[j] = W[k][j] - v[k] w[j] - w[k] v[j]  (j >= k)
+//   k <= n-3: reflector v_k from r[k+1..], stored in vnew[] and in W[k][k+2..] (v_k[k+1] = 1 implied)
+//   k == n-2: the last 2x2 block: d[n-2], e[n-1], d[n-1]
+// Reflector convention as in K2 (LAPACK dlarfg): beta = -sign(alpha) ||x||, tau = (beta-alpha)/beta.
+__global__ void __launch_bounds__(1024, 1)
+eigh_reflector_kernel(double* __restrict__ W, int n, int k, const double* __restrict__ y,
+                      const double* __restrict__ vprev, double* __restrict__ wv, double* __restrict__ vnew,
+                      double* __restrict__ tauv, double* __restrict__ dvec, double* __restrict__ evec) {
+  __shared__ double sh[33];
+  __shared__ double s_tau, s_scale;
+  const int tid = threadIdx.x;
+  double* Wk = W + (long long)k * n;
+  double vk = 0.0, wk = 0.0;
+  if (k > 0) {
+    const double tau = tauv[k - 1];
+    double acc = 0.0;
+    for (int i = k + tid; i < n; i += blockDim.x) acc = fma(tau * y[i], vprev[i], acc);
+    const double pTv = block_sum(acc, sh);
+    const double coef = 0.5 * tau * pTv;
+    for (int i = k + tid; i < n; i += blockDim.x) wv[i] = fma(-coef, vprev[i], tau * y[i]);
+    __syncthreads();
+    vk = vprev[k]; wk = wv[k];
+  }
+  // r[j], j >= k, kept in place in W[k][j]
+  for (int j = k + tid; j < n; j += blockDim.x) {
+    double x = Wk[j];
+    if (k > 0) { x = fma(-vk, wv[j], x); x = fma(-wk, vprev[j], x); }
+    Wk[j] = x;
+  }
+  __syncthreads();
+  if (k >= n - 2) {            // final block (n >= 2: k = n-2; n == 1: k = 0)
+    if (tid == 0) {
+      dvec[k] = Wk[k];
+      evec[0] = 0.0;
+      if (k + 1 < n) {
+        evec[k + 1] = Wk[k + 1];
+        double x = W[(long long)(k + 1) * n + (k + 1)];
+        if (k > 0) x = fma(-2.0 * vprev[k + 1], wv[k + 1], x);
+        dvec[k + 1] = x;
+      }
+    }
+    return;
+  }
+  double acc = 0.0;
+  for (int j = k + 2 + tid; j < n; j += blockDim.x) { double x = Wk[j]; acc = fma(x, x, acc); }
+  const double tail2 = block_sum(acc, sh);
+  if (tid == 0) {
+    const double alpha = Wk[k + 1];
+    double t = 0.0, scale = 0.0, beta = alpha;
+    if (tail2 > 0.0) {
+      const double sigma = sqrt(fma(alpha, alpha, tail2));
+      beta = alpha >= 0.0 ? -sigma : sigma;
+      t = (beta - alpha) / beta;
+      scale = 1.0 / (alpha - beta);
+    }
+    s_tau = t; s_scale = scale;
+    tauv[k] = t; dvec[k] = Wk[k]; evec[k + 1] = beta;
+  }
+  __syncthreads();
+  const double scale = s_scale;
+  for (int j = k + 1 + tid; j < n; j += blockDim.x) {
+    const double v = (j == k + 1) ? 1.0 : Wk[j] * scale;
+    vnew[j] = v;
+    if (j > k + 1) Wk[j] = v;
+  }
+}
+
+// Grid.  Rows i in [k+1, n), columns j in [k+1, n):  x = W[i][j] - vprev[i] w[j] - w[i] vprev[j]
+// (the pending update of reflector k-1, skipped when k == 0), stored back, and y[i] = sum_j x vnew[j].
+// One warp per ROWS consecutive rows, lanes along the contiguous j.
+template <int ROWS>
+__global__ void __launch_bounds__(256)
+eigh_pass_kernel(double* __restrict__ W, int n, int k, const double* __restrict__ vprev,
+                 const double* __restrict__ wv, const double* __restrict__ vnew, double* __restrict__ y) {
+  const int lane = threadIdx.x & 31;
+  const int gw = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  const int i0 = k + 1 + gw * ROWS;
+  if (i0 >= n) return;
+  const bool pending = k > 0;
+  double vi[ROWS], wi[ROWS], acc[ROWS];
+  double* row[ROWS];
+#pragma unroll
+  for (int r = 0; r < ROWS; ++r) {
+    const int i = min(i0 + r, n - 1);
+    row[r] = W + (long long)i * n;
+    vi[r] = pending ? vprev[i] : 0.0;
+    wi[r] = pending ? wv[i] : 0.0;
+    acc[r] = 0.0;
+  }
+  for (int j = k + 1 + lane; j < n; j += 32) {
+    const double vn = vnew[j];
+    double vj = 0.0, wj = 0.0;
+    if (pending) { vj = vprev[j]; wj = wv[j]; }
+#pragma unroll
+    for (int r = 0; r < ROWS; ++r) {
+      double x = row[r][j];
+      if (pending) {
+        x = fma(-vi[r], wj, x);
+        x = fma(-wi[r], vj, x);
+        if (i0 + r < n) row[r][j] = x;
+      }
+      acc[r] = fma(x, vn, acc[r]);
+    }
+  }
+#pragma unroll
+  for (int r = 0; r < ROWS; ++r) {
+    const double s = warp_sum(acc[r]);
+    if (lane == 0 && i0 + r < n) y[i0 + r] = s;
+  }
+}
+
+// (W + W^T)/2 in place (C~ is symmetric for a C4v state; rounding in the GEMMs that
+// build it breaks that at the 1e-16 level; reading A15).
+__global__ void symmetrize_inplace_kernel(double* __restrict__ W, int n) {
+  const long long total = (long long)n * n;
+  for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
+       idx += (long long)gridDim.x * blockDim.x) {
+    const int i = (int)(idx / n), j = (int)(idx % n);
+    if (j < i) {
+      const double a = W[idx], b = W[(long long)j * n + i];
+      const double s = 0.5 * (a + b);
+      W[idx] = s; W[(long long)j * n + i] = s;
+    }
+  }
+}
+
+// eig[n] ascending -> lamsel[r] = the eigenvalue of rank r in decreasing |lambda| (ties: lower index
+// first, i.e. numpy's stable argsort of -|lambda| on the ascending list), r < k.
+// scal[0] = max_i (|d_i| + |e_i| + |e_{i+1}|), the norm bound used as pivot scale by the inverse iteration.
+__global__ void eigh_select_kernel(const double* __restrict__ eig, int n, int k, double* __restrict__ lamsel,
+                                   const double* __restrict__ dvec, const double* __restrict__ evec,
+                                   double* __restrict__ scal) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) {
+    const double mine = fabs(eig[i]);
+    int rank = 0;
+    for (int j = 0; j < n; ++j) {
+      const double o = fabs(eig[j]);
+      rank += (o > mine) || (o == mine && j < i);
+    }
+    if (rank < k) lamsel[rank] = eig[i];
+  }
+  if (blockIdx.x == 0) {
+    __shared__ double sh[33];
+    double mx = 0.0;
+    for (int t = threadIdx.x; t < n; t += blockDim.x) {
+      const double el = t > 0 ? fabs(evec[t]) : 0.0, er = t + 1 < n ? fabs(evec[t + 1]) : 0.0;
+      mx = fmax(mx, fabs(dvec[t]) + el + er);
+    }
+    mx = block_max(mx, sh);
+    if (threadIdx.x == 0) scal[0] = mx;
+  }
+}
+
+__device__ __forceinline__ double eigh_rnd(unsigned i, unsigned c) {   // counter-based, in (-1, 1)
+  unsigned long long z = ((unsigned long long)i << 32 | c) + 0x9E3779B97F4A7C15ull;
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  z ^= z >> 31;
+  return ((double)(z >> 11) + 0.5) * (2.0 / 9007199254740992.0) - 1.0;
+}
+
+// Inverse iteration for column c: (T - lam_c) x = rhs, `iters` times from a random start, x normalised
+// after every solve.  T - lam = P L U by Gaussian elimination with partial pivoting (two
+// superdiagonals in U); the elimination is replayed on the right-hand side in the same sweep.
+// Z, U0, U1, U2: n x k row-major (threads of a warp touch consecutive addresses).
+__global__ void eigh_invit_kernel(const double* __restrict__ dvec, const double* __restrict__ evec, int n,
+                                  const double* __restrict__ lamsel, int k, const double* __restrict__ scal,
+                                  double* __restrict__ Z, double* __restrict__ U0, double* __restrict__ U1,
+                                  double* __restrict__ U2, int iters) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= k) return;
+  const double lam = lamsel[c];
+  const double tiny = fmax(2.220446049250313e-16 * scal[0], 1e-300);
+  for (int i = 0; i < n; ++i) Z[(long long)i * k + c] = eigh_rnd((unsigned)i, (unsigned)c);
+  for (int it = 0; it < iters; ++it) {
+    double p0 = dvec[0] - lam, p1 = n > 1 ? evec[1] : 0.0, p2 = 0.0;
+    double r = Z[c];
+    for (int i = 0; i + 1 < n; ++i) {
+      const double cc = evec[i + 1], a = dvec[i + 1] - lam, b = i + 2 < n ? evec[i + 2] : 0.0;
+      const double yn = Z[(long long)(i + 1) * k + c];
+      double u0, u1, u2, ri, n0, n1, nr;
+      if (fabs(p0) >= fabs(cc)) {
+        if (fabs(p0) < tiny) p0 = p0 < 0.0 ? -tiny : tiny;
+        const double mlt = cc / p0;
+        u0 = p0; u1 = p1; u2 = p2; ri = r;
+        n0 = fma(-mlt, p1, a); n1 = fma(-mlt, p2, b); nr = fma(-mlt, r, yn);
+      } else {
+        const double mlt = p0 / cc;
+        u0 = cc; u1 = a; u2 = b; ri = yn;
+        n0 = fma(-mlt, a, p1); n1 = fma(-mlt, b, p2); nr = fma(-mlt, yn, r);
+      }
+      const long long o = (long long)i * k + c;
+      U0[o] = u0; U1[o] = u1; U2[o] = u2; Z[o] = ri;
+      p0 = n0; p1 = n1; p2 = 0.0; r = nr;
+    }
+    if (fabs(p0) < tiny) p0 = p0 < 0.0 ? -tiny : tiny;
+    {
+      const long long o = (long long)(n - 1) * k + c;
+      U0[o] = p0; U1[o] = 0.0; U2[o] = 0.0; Z[o] = r;
+    }
+    double x1 = 0.0, x2 = 0.0, mx = 0.0;
+    for (int i = n - 1; i >= 0; --i) {
+      const long long o = (long long)i * k + c;
+      double x = Z[o];
+      x = fma(-U1[o], x1, x);
+      x = fma(-U2[o], x2, x);
+      x /= U0[o];
+      Z[o] = x;
+      x2 = x1; x1 = x;
+      mx = fmax(mx, fabs(x));
+    }
+    const double inv = mx > 0.0 ? 1.0 / mx : 1.0;
+    double ss = 0.0;
+    for (int i = 0; i < n; ++i) { const double x = Z[(long long)i * k + c] * inv; ss = fma(x, x, ss); }
+    const double sc = inv / sqrt(ss);
+    for (int i = 0; i < n; ++i) Z[(long long)i * k + c] *= sc;
+  }
+}
+
+// U = H_0 H_1 ... H_{n-3} U, reflector k = I - tau_k v v^T with v[k+1] = 1, v[j] = W[k][j] (j > k+1).
+// CTA b owns columns 2b, 2b+1 of U (n x ldu) in shared memory; thread t owns rows t, t + 1024, ...
+// for the whole kernel, so only the two dot products need a block-wide exchange per reflector.
+__global__ void __launch_bounds__(1024, 1)
+eigh_backtransform_kernel(const double* __restrict__ W, const double* __restrict__ tauv, int n,
+                          double* __restrict__ U, int ldu, int ncols) {
+  extern __shared__ __align__(16) double bsm[];
+  double* x0 = bsm;
+  double* x1 = bsm + n;
+  double* part = bsm + 2 * n;          // [2][2][32]
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int c0 = 2 * blockIdx.x, c1 = c0 + 1;
+  const bool two = c1 < ncols;
+  for (int i = tid; i < n; i += 1024) {
+    x0[i] = U[(long long)i * ldu + c0];
+    x1[i] = two ? U[(long long)i * ldu + c1] : 0.0;
+  }
+  int buf = 0;
+  for (int k = n - 3; k >= 0; --k) {
+    const double tau = tauv[k];
+    if (tau == 0.0) continue;
+    const double* Wk = W + (long long)k * n;
+    double a0 = 0.0, a1 = 0.0;
+    for (int i = tid; i < n; i += 1024) {
+      if (i > k) {
+        const double v = (i == k + 1) ? 1.0 : Wk[i];
+        a0 = fma(v, x0[i], a0);
+        a1 = fma(v, x1[i], a1);
+      }
+    }
+    a0 = warp_sum(a0); a1 = warp_sum(a1);
+    double* pb = part + buf * 64;
+    if (lane == 0) { pb[warp] = a0; pb[32 + warp] = a1; }
+    __syncthreads();
+    double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+    for (int w = 0; w < 32; ++w) { s0 += pb[w]; s1 += pb[32 + w]; }
+    s0 *= tau; s1 *= tau;
+    for (int i = tid; i < n; i += 1024) {
+      if (i > k) {
+        const double v = (i == k + 1) ? 1.0 : Wk[i];
+        x0[i] = fma(-s0, v, x0[i]);
+        x1[i] = fma(-s1, v, x1[i]);
+      }
+    }
+    buf ^= 1;
+  }
+  for (int i = tid; i < n; i += 1024) {
+    U[(long long)i * ldu + c0] = x0[i];
+    if (two) U[(long long)i * ldu + c1] = x1[i];
+  }
+}
+
+// One CTA per column: the component of largest magnitude (first one on ties, numpy's argmax) is made positive.
+__global__ void __launch_bounds__(256)
+eigh_sign_kernel(double* __restrict__ U, int n, int ldu) {
+  __shared__ double sv[256];
+  __shared__ int si[256];
+  const int c = blockIdx.x, tid = threadIdx.x;
+  double best = -1.0; int bi = 0x7fffffff;
+  for (int i = tid; i < n; i += 256) {
+    const double a = fabs(U[(long long)i * ldu + c]);
+    if (a > best) { best = a; bi = i; }
+  }
+  sv[tid] = best; si[tid] = bi;
+  __syncthreads();
+  for (int s = 128; s > 0; s >>= 1) {
+    if (tid < s) {
+      const double o = sv[tid + s]; const int oi = si[tid + s];
+      if (o > sv[tid] || (o == sv[tid] && oi < si[tid])) { sv[tid] = o; si[tid] = oi; }
+    }
+    __syncthreads();
+  }
+  const bool flip = U[(long long)si[0] * ldu + c] < 0.0;
+  __syncthreads();
+  if (flip)
+    for (int i = tid; i < n; i += 256) U[(long long)i * ldu + c] = -U[(long long)i * ldu + c];
+}
+
+// out (k x k) = diag(lam)
+__global__ void diag_matrix_kernel(const double* __restrict__ lam, int k, double* __restrict__ out) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx < k * k) out[idx] = (idx / k == idx % k) ? lam[idx / k] : 0.0;
+}
+
+// fn.[48] PAPER.md:132: boundary from the bulk tensor, open bra/ket legs contracted:
+//   C0[(d d'),(r r')]        = sum_{s,u,l} A[s,u,l,d,r] A[s,u,l,d',r']
+//   T0[(l l'),(d d'),(r r')] = sum_{s,u}   A[s,u,l,d,r] A[s,u,l',d',r']
+// One thread per output element (b^2 + b^3 elements, d D^2 resp. d D terms each).
+__global__ void bulk_init_kernel(const double* __restrict__ A, int d, int D, double* __restrict__ C0,
+                                 double* __restrict__ T0) {
+  const int b = D * D;
+  const long long nC = (long long)b * b, nT = nC * b;
+  const long long s1 = (long long)D * D * D * D;      // stride of s
+  const long long su = (long long)D * D * D, sl = (long long)D * D;
+  for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < nC + nT;
+       idx += (long long)gridDim.x * blockDim.x) {
+    if (idx < nC) {
+      const int dd = (int)(idx / b), rr = (int)(idx % b);
+      const int dk = dd / D, db = dd % D, rk = rr / D, rb = rr % D;
+      double acc = 0.0;
+      for (int s = 0; s < d; ++s)
+        for (int u = 0; u < D; ++u)
+          for (int l = 0; l < D; ++l) {
+            const double* base = A + s * s1 + u * su + l * sl;
+            acc = fma(base[dk * D + rk], base[db * D + rb], acc);
+          }
+      C0[idx] = acc;
+    } else {
+      const long long t = idx - nC;
+      const int ll = (int)(t / nC), dd = (int)((t / b) % b), rr = (int)(t % b);
+      const int lk = ll / D, lb = ll % D, dk = dd / D, db = dd % D, rk = rr / D, rb = rr % D;
+      double acc = 0.0;
+      for (int s = 0; s < d; ++s)
+        for (int u = 0; u < D; ++u) {
+          const double* base = A + s * s1 + u * su;
+          acc = fma(base[lk * sl + dk * D + rk], base[lb * sl + db * D + rb], acc);
+        }
+      T0[t] = acc;
+    }
+  }
+}
+
+}  // namespace qk

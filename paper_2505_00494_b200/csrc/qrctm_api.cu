@@ -14,6 +14,7 @@
 #include "kernels_misc.cuh"
 #include "qr_f64.cuh"
 #include "spectrum.cuh"
+#include "eigh.cuh"
 
 using namespace qk;
 
@@ -34,8 +35,12 @@ struct Layout {   // byte offsets into the workspace
 }  // namespace
 
 struct qrctm {
-  int d, D, b, chi;
+  int d, D, b, chi;       // chi: current bond dimension (<= chi_cap; below it only during the NEXT-2 warm-up)
+  int chi_cap;            // the chi the workspace was sized for
   long long m;            // chi * b
+  int eig_rows, eig_cols; // shape of U left in Q by the last eigen step (0: none)
+  void* eigwork;          // NEXT-2 eigensolver workspace, allocated by the first qrctm_eig_step
+  size_t eigwork_bytes;
   cudaStream_t stream;
   char* base;             // workspace
   bool owns_ws;
@@ -622,6 +627,87 @@ long long qr_factor_blocked(cudaStream_t st, int qr_path, long long rows, int n,
   return qr_factor_blocked_t<QR_NB, false>(st, rows, n, X, Q, R, work, err);
 }
 
+// ------------------------------------------------------------------ NEXT-2: top-k symmetric eigensolver
+constexpr int EIGH_MAX_N = 14000;     // d, e2 of the multisection / two columns of the back-transform in shared memory
+
+struct EighWork {
+  double *v0, *v1, *w, *y, *tau, *d, *e, *eig, *scal, *Z, *U0, *U1, *U2, *R;
+  void* qr;
+};
+
+size_t eigh_layout(long long n, int k, char* base, EighWork* w) {
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes); return o; };
+  const size_t dbl = sizeof(double);
+  size_t o[14];
+  for (int i = 0; i < 8; ++i) o[i] = take(dbl * n);         // v0 v1 w y tau d e eig
+  o[8] = take(dbl * 16);
+  for (int i = 9; i < 13; ++i) o[i] = take(dbl * n * k);    // Z U0 U1 U2
+  o[13] = take(dbl * (size_t)k * k);
+  size_t oq = take(qr_work_bytes_impl(n, k));
+  if (w) {
+    double** f[14] = {&w->v0, &w->v1, &w->w, &w->y, &w->tau, &w->d, &w->e, &w->eig, &w->scal,
+                      &w->Z, &w->U0, &w->U1, &w->U2, &w->R};
+    for (int i = 0; i < 14; ++i) *f[i] = reinterpret_cast<double*>(base + o[i]);
+    w->qr = base + oq;
+  }
+  return off;
+}
+
+unsigned long long eigh_work_bytes_impl(long long n, int k) {
+  if (n < 1 || k < 1 || k > n || n > EIGH_MAX_N) return 0;
+  return eigh_layout(n, k, nullptr, nullptr);
+}
+
+// W (n x n symmetric, row-major, DEVICE, destroyed) -> lam[k] (largest |lambda| first), U (n x k, ld k).
+// Returns kernels launched or -1.
+long long eigh_top(cudaStream_t st, int n, int k, double* W, double* lam, double* U, void* work, cudaError_t* err) {
+  EighWork wk;
+  eigh_layout(n, k, static_cast<char*>(work), &wk);
+  long long launches = 0;
+  static int attr_done = 0;
+  if (!attr_done) {
+    int dev = 0, max_smem = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    cudaFuncSetAttribute(multisect_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem - 1024);
+    cudaFuncSetAttribute(eigh_backtransform_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem - 1024);
+    attr_done = 1;
+  }
+  constexpr int ROWS = 4;
+  cudaMemsetAsync(wk.tau, 0, sizeof(double) * n, st);
+  for (int k2 = 0; k2 + 2 < n; ++k2) {
+    double* vprev = (k2 & 1) ? wk.v0 : wk.v1;      // v_{k-1}
+    double* vnew = (k2 & 1) ? wk.v1 : wk.v0;       // v_k
+    eigh_reflector_kernel<<<1, 1024, 0, st>>>(W, n, k2, wk.y, vprev, wk.w, vnew, wk.tau, wk.d, wk.e);
+    const int nrows = n - k2 - 1, warps = (nrows + ROWS - 1) / ROWS;
+    eigh_pass_kernel<ROWS><<<(warps + 7) / 8, 256, 0, st>>>(W, n, k2, vprev, wk.w, vnew, wk.y);
+    launches += 2;
+  }
+  {
+    const int kf = n >= 2 ? n - 2 : 0;
+    double* vprev = (kf & 1) ? wk.v0 : wk.v1;
+    eigh_reflector_kernel<<<1, 1024, 0, st>>>(W, n, kf, wk.y, vprev, wk.w, wk.v0, wk.tau, wk.d, wk.e);
+  }
+  multisect_kernel<<<(n + 7) / 8, 256, sizeof(double) * (2 * (size_t)n + 40), st>>>(wk.d, wk.e, n, wk.eig);
+  eigh_select_kernel<<<(n + 255) / 256, 256, 0, st>>>(wk.eig, n, k, lam, wk.d, wk.e, wk.scal);
+  eigh_invit_kernel<<<(k + 31) / 32, 32, 0, st>>>(wk.d, wk.e, n, lam, k, wk.scal, wk.Z, wk.U0, wk.U1, wk.U2, 3);
+  launches += 4;
+  *err = cudaGetLastError();
+  if (*err != cudaSuccess) return -1;
+  long long nq = qr_factor_blocked(st, 0, n, k, wk.Z, U, wk.R, wk.qr, err);
+  if (nq < 0) return -1;
+  launches += nq;
+  if (n >= 3) {
+    eigh_backtransform_kernel<<<(k + 1) / 2, 1024, sizeof(double) * (2 * (size_t)n + 128), st>>>(W, wk.tau, n, U, k, k);
+    launches += 1;
+  }
+  eigh_sign_kernel<<<k, 256, 0, st>>>(U, n, k);
+  launches += 1;
+  *err = cudaGetLastError();
+  return *err == cudaSuccess ? launches : -1;
+}
+
 }  // namespace
 
 // ------------------------------------------------------------------ step stages
@@ -653,9 +739,12 @@ int stage_reduced_corner(qrctm* h, const double* C, const double* T, double* X) 
 
 // K3: P'[u,l,J,m] = sum_j Qm[j,u,m] T[j,l,J]        (Qm: chi*b x n viewed chi x b*n).  m innermost: the
 // consecutive rows of a K4 tile (M index (J,m)) are then adjacent in K4's outputs.
-int stage_half_absorb(qrctm* h, const double* Qm, const double* T, double* P) {
-  const int chi = h->chi, b = h->b; const long long bc = (long long)b * chi, cc = (long long)chi * chi;
-  GemmCall c{Qm, bc, 1, T, bc, P, IndexMap{chi, b * cc, 1}, IndexMap{chi, cc, chi}, (int)bc, (int)bc, chi, 0};
+// co = number of columns of Qm (the new chi) when it differs from the chi of T (eigen step with chi growth).
+int stage_half_absorb(qrctm* h, const double* Qm, const double* T, double* P, int co = 0) {
+  const int ci = h->chi, b = h->b; if (co <= 0) co = ci;
+  const long long cc = (long long)ci * co;
+  GemmCall c{Qm, (long long)b * co, 1, T, (long long)b * ci, P, IndexMap{co, b * cc, 1}, IndexMap{ci, cc, co},
+             b * co, b * ci, ci, 0};
   GEMM(h, c);
   return QRCTM_OK;
 }
@@ -664,8 +753,9 @@ int stage_half_absorb(qrctm* h, const double* Qm, const double* T, double* P) {
 //   layout 0: S''[J,d,m,r]  (what K5 wants: K x M with K = (J,d))
 //   layout 1: S~ [m,r,J,d]  (what the kappa network wants: K = (m,r))
 //   layout 2: C~[(J,d),(m,r)] natural enlarged-corner matrix == layout 0
-int stage_absorb_a(qrctm* h, const double* P, double* S, int layout, const double* amat = nullptr) {
-  const int chi = h->chi, b = h->b; const long long m = h->m, cc = (long long)chi * chi;
+int stage_absorb_a(qrctm* h, const double* P, double* S, int layout, const double* amat = nullptr, int chi_out = 0) {
+  const int ci = h->chi, chi = chi_out > 0 ? chi_out : ci, b = h->b;     // chi: range of the index m
+  const long long m = (long long)chi * b, cc = (long long)ci * chi;
   IndexMap ro, co;
   if (layout == 0) { ro = IndexMap{chi, (long long)b * m, b}; co = IndexMap{b, m, 1}; }
   else             { ro = IndexMap{chi, b, (long long)b * m}; co = IndexMap{b, 1, (long long)chi * b}; }
@@ -702,9 +792,9 @@ int stage_absorb_layered(qrctm* h, const double* P, double* S) {
 }
 
 // K5: out[(m,r),n] = sum_{(J,d)} S''[(J,d),(m,r)] Qm[(J,d),n]
-int stage_project(qrctm* h, const double* S, const double* Qm, double* out) {
-  const int chi = h->chi; const long long m = h->m;
-  GemmCall c{S, m, 1, Qm, chi, out, plain_map(chi), IndexMap{1, 1, 0}, (int)m, chi, (int)m, 0};
+int stage_project(qrctm* h, const double* S, const double* Qm, double* out, int chi_out = 0) {
+  const int chi = chi_out > 0 ? chi_out : h->chi; const long long m = (long long)chi * h->b, mi = h->m;
+  GemmCall c{S, m, 1, Qm, chi, out, plain_map(chi), IndexMap{1, 1, 0}, (int)m, chi, (int)mi, 0};
   c.epi = 1;
   GEMM(h, c);
   return QRCTM_OK;
@@ -818,6 +908,13 @@ void invalidate_graphs(qrctm* h) {
   h->warm_steps = 0;      // one ordinary step first: newly selected kernels set their attributes outside capture
 }
 
+// current bond dimension (NEXT-2 warm-up grows it up to chi_cap); captured graphs hold the old shapes
+void set_chi(qrctm* h, int chi) {
+  if (chi == h->chi) return;
+  invalidate_graphs(h);
+  h->chi = chi; h->m = (long long)chi * h->b;
+}
+
 // Capture `body` (which only enqueues work on h->stream) into an executable graph.
 template <class F>
 bool capture_graph(qrctm* h, F body, cudaGraphExec_t* exec, long long* nlaunch) {
@@ -900,6 +997,7 @@ static int create_common(int d, int D, int chi, void* ws, unsigned long long ws_
   if (!h) return QRCTM_ERR_CUDA;
   memset(h, 0, sizeof(*h));
   h->d = d; h->D = D; h->b = D * D; h->chi = chi; h->m = (long long)chi * D * D;
+  h->chi_cap = chi; h->eigwork = nullptr; h->eigwork_bytes = 0; h->eig_rows = h->eig_cols = 0;
   h->L = L; h->stream = 0;
   h->corner_mode = 0; h->symmetrize = 1; h->check_every = 1; h->gemm_path = 0; h->overlap = 1; h->use_graph = 1;
   if (ws) {
@@ -956,6 +1054,7 @@ int qrctm_destroy(qrctm_t* h) {
   cudaStreamSynchronize(h->stream);
   invalidate_graphs(h);
   if (h->owns_ws && h->base) cudaFree(h->base);
+  if (h->eigwork) cudaFree(h->eigwork);
   if (h->h_pinned) cudaFreeHost(h->h_pinned);
   if (h->side) { cudaStreamSynchronize(h->side); cudaStreamDestroy(h->side); cudaEventDestroy(h->ev_env); cudaEventDestroy(h->ev_spec); }
   if (h->have_ev) for (int i = 0; i < QRCTM_NSTAGE + 2; ++i) cudaEventDestroy(h->ev[i]);
@@ -986,6 +1085,7 @@ int qrctm_set_A(qrctm_t* h, const double* A) {
 
 int qrctm_set_env(qrctm_t* h, const double* C, const double* T) {
   if (!h || !C || !T) return h ? fail(h, QRCTM_ERR_INVALID_ARG, "null C/T") : QRCTM_ERR_INVALID_ARG;
+  if (h->chi != h->chi_cap) { CU(h, cudaStreamSynchronize(h->stream)); set_chi(h, h->chi_cap); }
   CU(h, copy_in(h->Cn, C, (size_t)h->chi * h->chi, h->stream));
   CU(h, copy_in(h->Tn, T, (size_t)h->m * h->chi, h->stream));
   CU(h, cudaMemsetAsync(h->flag, 0, sizeof(int), h->stream));
@@ -1000,6 +1100,7 @@ int qrctm_set_env(qrctm_t* h, const double* C, const double* T) {
 int qrctm_step(qrctm_t* h) {
   if (!h) return QRCTM_ERR_INVALID_ARG;
   if (!h->have_A || !h->have_env) return fail(h, QRCTM_ERR_NOT_READY, "set_A and set_env first");
+  h->eig_rows = 0;          // Q is about to be overwritten by K2
   if (!h->use_graph || h->stream == nullptr) { int rc0 = do_step(h, nullptr); if (!rc0) h->warm_steps += 1; return rc0; }
   int rc = run_front(h, nullptr); if (rc) return rc;
   return run_k7(h, nullptr);
@@ -1008,6 +1109,7 @@ int qrctm_step(qrctm_t* h) {
 int qrctm_run(qrctm_t* h, int max_iter, double tol, int* iters_done, double* final_delta) {
   if (!h) return QRCTM_ERR_INVALID_ARG;
   if (!h->have_A || !h->have_env) return fail(h, QRCTM_ERR_NOT_READY, "set_A and set_env first");
+  h->eig_rows = 0;          // Q is about to be overwritten by K2
   if (max_iter < 0) return fail(h, QRCTM_ERR_INVALID_ARG, "max_iter < 0");
   if (h->overlap && h->side && !h->time_stages) {
     // Overlapped driver: K1..K6 of step it are queued before the host waits for the spectrum of
@@ -1336,6 +1438,127 @@ int qrctm_probe_fp64(int kind, int iters, double* tflops) {
   double flops = kind == 0 ? nthr * iters * 16.0 * 2.0 : (nthr / 32.0) * iters * 8.0 * 512.0;
   *tflops = flops / (ms * 1e-3) / 1e12;
   return QRCTM_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------ NEXT-2: initialisation and eigen step
+namespace {
+
+// K1, K3, K4 with C, T themselves give C~; its chi_new largest-|lambda| eigenpairs give U (for Q) and
+// C' = diag(lambda); T' = (E3) with U for Q  (Fig. 1(d)).
+int stage_eig_step(qrctm* h, int chi_new) {
+  const int ci = h->chi, b = h->b; const long long mi = h->m;
+  const size_t need = eigh_work_bytes_impl(mi, chi_new) + sizeof(double) * (size_t)chi_new + 256;
+  if (h->eigwork_bytes < need) {
+    CU(h, cudaStreamSynchronize(h->stream));
+    if (h->eigwork) { cudaFree(h->eigwork); h->eigwork = nullptr; h->eigwork_bytes = 0; }
+    CU(h, cudaMalloc(&h->eigwork, need));
+    h->eigwork_bytes = need;
+  }
+  double* lam = static_cast<double*>(h->eigwork);
+  void* work = static_cast<char*>(h->eigwork) + align_up(sizeof(double) * (size_t)chi_new);
+  nvtxRangePushA("E1_enlarged_corner");
+  int rc = stage_reduced_corner(h, h->C, h->T, h->X);
+  if (!rc) rc = stage_half_absorb(h, h->X, h->T, h->P);
+  if (!rc) rc = stage_absorb_a(h, h->P, h->S, 0);                        // S = C~[(J,d),(k,r)]
+  nvtxRangePop();
+  if (rc) return rc;
+  symmetrize_inplace_kernel<<<592, 256, 0, h->stream>>>(h->S, (int)mi);
+  h->launches += 1;
+  nvtxRangePushA("E2_eigh");
+  cudaError_t e;
+  long long nl = eigh_top(h->stream, (int)mi, chi_new, h->S, lam, h->Q, work, &e);
+  nvtxRangePop();
+  if (nl < 0) return fail(h, QRCTM_ERR_CUDA, "eigh", e);
+  h->launches += nl;
+  nvtxRangePushA("E3_edge");
+  rc = stage_half_absorb(h, h->Q, h->T, h->P, chi_new);
+  if (!rc) rc = stage_absorb_a(h, h->P, h->S, 0, nullptr, chi_new);
+  if (!rc) rc = stage_project(h, h->S, h->Q, h->Tn, chi_new);
+  nvtxRangePop();
+  if (rc) return rc;
+  diag_matrix_kernel<<<(chi_new * chi_new + 255) / 256, 256, 0, h->stream>>>(lam, chi_new, h->Cn);
+  h->launches += 1;
+  CU(h, cudaGetLastError());
+  h->eig_rows = (int)mi; h->eig_cols = chi_new;
+  set_chi(h, chi_new);
+  (void)ci; (void)b;
+  return stage_normalize(h, h->Cn, h->Tn);
+}
+
+}  // namespace
+
+extern "C" {
+
+int qrctm_get_chi(const qrctm_t* h, int* chi, int* chi_capacity) {
+  if (!h) return QRCTM_ERR_INVALID_ARG;
+  if (chi) *chi = h->chi;
+  if (chi_capacity) *chi_capacity = h->chi_cap;
+  return QRCTM_OK;
+}
+
+int qrctm_init_bulk(qrctm_t* h) {
+  if (!h) return QRCTM_ERR_INVALID_ARG;
+  if (!h->have_A) return fail(h, QRCTM_ERR_NOT_READY, "set_A first");
+  if (h->b > h->chi_cap) return fail(h, QRCTM_ERR_INVALID_ARG, "bulk initialisation needs D^2 <= chi");
+  CU(h, cudaStreamSynchronize(h->stream));
+  set_chi(h, h->b);
+  const long long tot = (long long)h->b * h->b * (1 + h->b);
+  int nb = (int)((tot + 255) / 256); if (nb > 1184) nb = 1184;
+  bulk_init_kernel<<<nb, 256, 0, h->stream>>>(h->A, h->d, h->D, h->Cn, h->Tn);
+  h->launches += 1;
+  CU(h, cudaGetLastError());
+  CU(h, cudaMemsetAsync(h->flag, 0, sizeof(int), h->stream));
+  int rc = stage_normalize(h, h->Cn, h->Tn); if (rc) return rc;
+  rc = check_flag(h); if (rc) return rc;
+  CU(h, cudaMemsetAsync(h->s_prev, 0, sizeof(double) * h->chi_cap, h->stream));
+  h->need_s0 = 1;
+  h->have_env = true;
+  return QRCTM_OK;
+}
+
+int qrctm_eig_step(qrctm_t* h, int chi_new) {
+  if (!h) return QRCTM_ERR_INVALID_ARG;
+  if (!h->have_A || !h->have_env) return fail(h, QRCTM_ERR_NOT_READY, "set_A and set_env / init_bulk first");
+  if (chi_new == 0) chi_new = h->chi;
+  if (chi_new < 1 || chi_new > h->chi_cap || chi_new > h->m) return fail(h, QRCTM_ERR_INVALID_ARG, "chi_new out of range");
+  if (h->m > EIGH_MAX_N) return fail(h, QRCTM_ERR_INVALID_ARG, "eigen step supports chi*D^2 <= 14000");
+  int rc = stage_eig_step(h, chi_new); if (rc) return rc;
+  rc = check_flag(h); if (rc) return rc;
+  CU(h, cudaMemsetAsync(h->s_prev, 0, sizeof(double) * h->chi_cap, h->stream));
+  h->need_s0 = 1;
+  return QRCTM_OK;
+}
+
+int qrctm_get_eig(qrctm_t* h, double* U, double* lam, int* rows, int* cols) {
+  if (!h) return QRCTM_ERR_INVALID_ARG;
+  if (!h->eig_rows || !h->eigwork) return fail(h, QRCTM_ERR_NOT_READY, "no eigen step yet");
+  if (rows) *rows = h->eig_rows;
+  if (cols) *cols = h->eig_cols;
+  if (U) CU(h, copy_out(U, h->Q, (size_t)h->eig_rows * h->eig_cols, h->stream));
+  if (lam) CU(h, copy_out(lam, static_cast<double*>(h->eigwork), (size_t)h->eig_cols, h->stream));
+  return QRCTM_OK;
+}
+
+int qrctm_warmup(qrctm_t* h, int n_eig_steps) {
+  if (!h || n_eig_steps < 0) return h ? fail(h, QRCTM_ERR_INVALID_ARG, "n_eig_steps < 0") : QRCTM_ERR_INVALID_ARG;
+  int rc = qrctm_init_bulk(h); if (rc) return rc;
+  for (int i = 0; i < n_eig_steps; ++i) {
+    long long grown = h->m;                                   // chi * D^2
+    int chi_new = grown > h->chi_cap ? h->chi_cap : (int)grown;
+    rc = qrctm_eig_step(h, chi_new); if (rc) return rc;
+  }
+  return QRCTM_OK;
+}
+
+unsigned long long qrctm_eigh_work_bytes(int n, int k) { return eigh_work_bytes_impl(n, k); }
+
+int qrctm_eigh_top_f64(void* cuda_stream, int n, int k, double* A, double* lam, double* U, void* work) {
+  if (!A || !lam || !U || !work || n < 1 || k < 1 || k > n || n > EIGH_MAX_N) return QRCTM_ERR_INVALID_ARG;
+  cudaError_t e;
+  long long nl = eigh_top(static_cast<cudaStream_t>(cuda_stream), n, k, A, lam, U, work, &e);
+  return nl < 0 ? QRCTM_ERR_CUDA : QRCTM_OK;
 }
 
 }  // extern "C"
