@@ -6,7 +6,7 @@
 //        eigh_pass_kernel      (grid)     : applies the pending rank-2 update of reflector k-1 to
 //                                           the trailing block and, in the same sweep, y = A22 v_k
 //      (one read + one write of the trailing block per step; HBM/L2-bound)
-//   2. all eigenvalues of the tridiagonal by warp multisection (spectrum.cuh)
+//   2. the k smallest and k largest eigenvalues of the tridiagonal by warp multisection (spectrum.cuh)
 //   3. eigh_select_kernel: the k of largest magnitude, stable in ascending-eigenvalue order
 //   4. eigh_invit_kernel: inverse iteration on the tridiagonal, one thread per vector,
 //      partial-pivoting LU recomputed each sweep, random start vectors
@@ -20,115 +20,147 @@
 namespace qk {
 
 // One CTA.  Step k of the tridiagonalisation of W (n x n, row-major, symmetric; rows/cols >= k live).
-//   k > 0 : y = A22 v_{k-1} (rows k..n-1) is in y[]; forms w_{k-1} = p - (tau/2)(p.v) v, p = tau y
+//   k > 0 : y = A22 v_{k-1} (rows k..n-1) = the sum of the pass kernel's per-chunk partials; forms w_{k-1} = p - (tau/2)(p.v) v, p = tau y
 //   row k brought up to date: r[j] = W[k][j] - v[k] w[j] - w[k] v[j]  (j >= k)
 //   k <= n-3: reflector v_k from r[k+1..], stored in vnew[] and in W[k][k+2..] (v_k[k+1] = 1 implied)
 //   k == n-2: the last 2x2 block: d[n-2], e[n-1], d[n-1]
 // Reflector convention as in K2 (LAPACK dlarfg): beta = -sign(alpha) ||x||, tau = (beta-alpha)/beta.
+// Thread t owns columns k + t, k + t + 1024, ... (RMAX of them, n - k <= 1024 RMAX) in registers through all phases.
+template <int RMAX>
 __global__ void __launch_bounds__(1024, 1)
-eigh_reflector_kernel(double* __restrict__ W, int n, int k, const double* __restrict__ y,
+eigh_reflector_kernel(double* __restrict__ W, int n, int k, const double* __restrict__ ypart, int nchunk_prev,
                       const double* __restrict__ vprev, double* __restrict__ wv, double* __restrict__ vnew,
                       double* __restrict__ tauv, double* __restrict__ dvec, double* __restrict__ evec) {
   __shared__ double sh[33];
-  __shared__ double s_tau, s_scale;
+  __shared__ double s_vk, s_wk, s_alpha;
   const int tid = threadIdx.x;
   double* Wk = W + (long long)k * n;
-  double vk = 0.0, wk = 0.0;
-  if (k > 0) {
+  double vp[RMAX], x[RMAX];              // v_{k-1}[i];  w_{k-1}[i], then the updated row entry r[i]
+  const bool pending = k > 0;
+  if (pending) {
     const double tau = tauv[k - 1];
     double acc = 0.0;
-    for (int i = k + tid; i < n; i += blockDim.x) acc = fma(tau * y[i], vprev[i], acc);
+#pragma unroll
+    for (int r = 0; r < RMAX; ++r) {
+      const int i = k + tid + 1024 * r;
+      double yi = 0.0; vp[r] = 0.0;
+      if (i < n) {
+        for (int c = 0; c < nchunk_prev; ++c) yi += ypart[(long long)c * n + i];      // fixed order: deterministic
+        vp[r] = vprev[i];
+      }
+      x[r] = tau * yi;
+      acc = fma(x[r], vp[r], acc);
+    }
     const double pTv = block_sum(acc, sh);
     const double coef = 0.5 * tau * pTv;
-    for (int i = k + tid; i < n; i += blockDim.x) wv[i] = fma(-coef, vprev[i], tau * y[i]);
-    __syncthreads();
-    vk = vprev[k]; wk = wv[k];
-  }
-  // r[j], j >= k, kept in place in W[k][j]
-  for (int j = k + tid; j < n; j += blockDim.x) {
-    double x = Wk[j];
-    if (k > 0) { x = fma(-vk, wv[j], x); x = fma(-wk, vprev[j], x); }
-    Wk[j] = x;
-  }
-  __syncthreads();
-  if (k >= n - 2) {            // final block (n >= 2: k = n-2; n == 1: k = 0)
-    if (tid == 0) {
-      dvec[k] = Wk[k];
-      evec[0] = 0.0;
-      if (k + 1 < n) {
-        evec[k + 1] = Wk[k + 1];
-        double x = W[(long long)(k + 1) * n + (k + 1)];
-        if (k > 0) x = fma(-2.0 * vprev[k + 1], wv[k + 1], x);
-        dvec[k + 1] = x;
-      }
+#pragma unroll
+    for (int r = 0; r < RMAX; ++r) {
+      const int i = k + tid + 1024 * r;
+      x[r] = fma(-coef, vp[r], x[r]);
+      if (i < n) wv[i] = x[r];
     }
+    if (tid == 0) { s_vk = vp[0]; s_wk = x[0]; }
+    __syncthreads();
+  }
+  const double vk = pending ? s_vk : 0.0, wk = pending ? s_wk : 0.0;
+  double acc = 0.0, d1 = 0.0;
+#pragma unroll
+  for (int r = 0; r < RMAX; ++r) {
+    const int i = k + tid + 1024 * r;
+    double xi = i < n ? Wk[i] : 0.0;
+    if (pending) {
+      if (i == k + 1) d1 = -2.0 * vp[r] * x[r];        // correction of W[k+1][k+1] (final block only)
+      xi = fma(-vk, x[r], xi); xi = fma(-wk, vp[r], xi);
+    }
+    x[r] = xi;
+    if (i >= k + 2) acc = fma(xi, xi, acc);
+  }
+  if (tid == 1 && k + 1 < n) s_alpha = x[0];
+  if (k >= n - 2) {            // final block (n >= 2: k = n-2; n == 1: k = 0)
+    if (tid == 0) { dvec[k] = x[0]; evec[0] = 0.0; }
+    if (tid == 1 && k + 1 < n) { evec[k + 1] = x[0]; dvec[k + 1] = W[(long long)(k + 1) * n + (k + 1)] + d1; }
     return;
   }
-  double acc = 0.0;
-  for (int j = k + 2 + tid; j < n; j += blockDim.x) { double x = Wk[j]; acc = fma(x, x, acc); }
   const double tail2 = block_sum(acc, sh);
-  if (tid == 0) {
-    const double alpha = Wk[k + 1];
-    double t = 0.0, scale = 0.0, beta = alpha;
-    if (tail2 > 0.0) {
-      const double sigma = sqrt(fma(alpha, alpha, tail2));
-      beta = alpha >= 0.0 ? -sigma : sigma;
-      t = (beta - alpha) / beta;
-      scale = 1.0 / (alpha - beta);
-    }
-    s_tau = t; s_scale = scale;
-    tauv[k] = t; dvec[k] = Wk[k]; evec[k + 1] = beta;
+  const double alpha = s_alpha;
+  double t = 0.0, scale = 0.0, beta = alpha;
+  if (tail2 > 0.0) {
+    const double sigma = sqrt(fma(alpha, alpha, tail2));
+    beta = alpha >= 0.0 ? -sigma : sigma;
+    t = (beta - alpha) / beta;
+    scale = 1.0 / (alpha - beta);
   }
-  __syncthreads();
-  const double scale = s_scale;
-  for (int j = k + 1 + tid; j < n; j += blockDim.x) {
-    const double v = (j == k + 1) ? 1.0 : Wk[j] * scale;
-    vnew[j] = v;
-    if (j > k + 1) Wk[j] = v;
+  if (tid == 0) { tauv[k] = t; dvec[k] = x[0]; evec[k + 1] = beta; }
+#pragma unroll
+  for (int r = 0; r < RMAX; ++r) {
+    const int i = k + tid + 1024 * r;
+    if (i > k && i < n) {
+      const double v = (i == k + 1) ? 1.0 : x[r] * scale;
+      vnew[i] = v;
+      if (i > k + 1) Wk[i] = v;
+    }
   }
 }
 
-// Grid.  Rows i in [k+1, n), columns j in [k+1, n):  x = W[i][j] - vprev[i] w[j] - w[i] vprev[j]
-// (the pending update of reflector k-1, skipped when k == 0), stored back, and y[i] = sum_j x vnew[j].
-// One warp per ROWS consecutive rows, lanes along the contiguous j.
+// Grid (x: column chunks of cw, y: groups of 8*ROWS rows).  Rows i in [k+1, n), columns j in [k+1, n):
+//   x = W[i][j] - vprev[i] w[j] - w[i] vprev[j]   (the pending update of reflector k-1, skipped when k == 0),
+// stored back, and ypart[chunk][i] = sum_{j in chunk} x vnew[j].  Each warp owns ROWS rows of the chunk, lanes
+// run along the contiguous j; the three vectors of the chunk are staged in shared memory once per CTA.
 template <int ROWS>
 __global__ void __launch_bounds__(256)
-eigh_pass_kernel(double* __restrict__ W, int n, int k, const double* __restrict__ vprev,
-                 const double* __restrict__ wv, const double* __restrict__ vnew, double* __restrict__ y) {
-  const int lane = threadIdx.x & 31;
-  const int gw = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-  const int i0 = k + 1 + gw * ROWS;
-  if (i0 >= n) return;
+eigh_pass_kernel(double* __restrict__ W, int n, int k, int cw, const double* __restrict__ vprev,
+                 const double* __restrict__ wv, const double* __restrict__ vnew, double* __restrict__ ypart) {
+  extern __shared__ __align__(16) double psm[];       // vnew[cw], vprev[cw], w[cw]
+  double* s_vn = psm; double* s_vp = psm + cw; double* s_w = psm + 2 * cw;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const bool pending = k > 0;
+  const int j0 = k + 1 + blockIdx.x * cw;
+  const int jn = min(cw, n - j0);
+  for (int t = threadIdx.x; t < jn; t += 256) {
+    s_vn[t] = vnew[j0 + t];
+    s_vp[t] = pending ? vprev[j0 + t] : 0.0;
+    s_w[t] = pending ? wv[j0 + t] : 0.0;
+  }
+  __syncthreads();
+  const int i0 = k + 1 + (blockIdx.y * 8 + warp) * ROWS;
+  if (i0 >= n) return;
   double vi[ROWS], wi[ROWS], acc[ROWS];
   double* row[ROWS];
 #pragma unroll
   for (int r = 0; r < ROWS; ++r) {
     const int i = min(i0 + r, n - 1);
-    row[r] = W + (long long)i * n;
+    row[r] = W + (long long)i * n + j0;
     vi[r] = pending ? vprev[i] : 0.0;
     wi[r] = pending ? wv[i] : 0.0;
     acc[r] = 0.0;
   }
-  for (int j = k + 1 + lane; j < n; j += 32) {
-    const double vn = vnew[j];
-    double vj = 0.0, wj = 0.0;
-    if (pending) { vj = vprev[j]; wj = wv[j]; }
+  if (pending) {
+#pragma unroll 2
+    for (int t = lane; t < jn; t += 32) {
+      const double vn = s_vn[t], vj = s_vp[t], wj = s_w[t];
+      double x[ROWS];
 #pragma unroll
-    for (int r = 0; r < ROWS; ++r) {
-      double x = row[r][j];
-      if (pending) {
-        x = fma(-vi[r], wj, x);
-        x = fma(-wi[r], vj, x);
-        if (i0 + r < n) row[r][j] = x;
+      for (int r = 0; r < ROWS; ++r) x[r] = row[r][t];
+#pragma unroll
+      for (int r = 0; r < ROWS; ++r) {
+        x[r] = fma(-vi[r], wj, x[r]);
+        x[r] = fma(-wi[r], vj, x[r]);
+        if (i0 + r < n) row[r][t] = x[r];
+        acc[r] = fma(x[r], vn, acc[r]);
       }
-      acc[r] = fma(x, vn, acc[r]);
+    }
+  } else {
+    for (int t = lane; t < jn; t += 32) {
+      const double vn = s_vn[t];
+#pragma unroll
+      for (int r = 0; r < ROWS; ++r) acc[r] = fma(row[r][t], vn, acc[r]);
     }
   }
+  double* yp = ypart + (long long)blockIdx.x * n;
 #pragma unroll
   for (int r = 0; r < ROWS; ++r) {
-    const double s = warp_sum(acc[r]);
-    if (lane == 0 && i0 + r < n) y[i0 + r] = s;
+    const double sm = warp_sum(acc[r]);
+    if (lane == 0 && i0 + r < n) yp[i0 + r] = sm;
   }
 }
 
@@ -147,17 +179,18 @@ __global__ void symmetrize_inplace_kernel(double* __restrict__ W, int n) {
   }
 }
 
-// eig[n] ascending -> lamsel[r] = the eigenvalue of rank r in decreasing |lambda| (ties: lower index
+// eig[nc] ascending (the candidates: all n eigenvalues, or the k smallest followed by the k largest -- an
+// eigenvalue of rank < k in |lambda| is always among those) -> lamsel[r] = the eigenvalue of rank r in decreasing |lambda| (ties: lower index
 // first, i.e. numpy's stable argsort of -|lambda| on the ascending list), r < k.
 // scal[0] = max_i (|d_i| + |e_i| + |e_{i+1}|), the norm bound used as pivot scale by the inverse iteration.
-__global__ void eigh_select_kernel(const double* __restrict__ eig, int n, int k, double* __restrict__ lamsel,
-                                   const double* __restrict__ dvec, const double* __restrict__ evec,
+__global__ void eigh_select_kernel(const double* __restrict__ eig, int nc, int k, double* __restrict__ lamsel,
+                                   const double* __restrict__ dvec, const double* __restrict__ evec, int n,
                                    double* __restrict__ scal) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) {
+  if (i < nc) {
     const double mine = fabs(eig[i]);
     int rank = 0;
-    for (int j = 0; j < n; ++j) {
+    for (int j = 0; j < nc; ++j) {
       const double o = fabs(eig[j]);
       rank += (o > mine) || (o == mine && j < i);
     }
@@ -195,13 +228,14 @@ __global__ void eigh_invit_kernel(const double* __restrict__ dvec, const double*
   if (c >= k) return;
   const double lam = lamsel[c];
   const double tiny = fmax(2.220446049250313e-16 * scal[0], 1e-300);
-  for (int i = 0; i < n; ++i) Z[(long long)i * k + c] = eigh_rnd((unsigned)i, (unsigned)c);
+  // rhs of sweep `it` = sc * (x of sweep it-1); sweep 0: random numbers generated on the fly
+  double sc = 1.0;
   for (int it = 0; it < iters; ++it) {
     double p0 = dvec[0] - lam, p1 = n > 1 ? evec[1] : 0.0, p2 = 0.0;
-    double r = Z[c];
+    double r = it ? sc * Z[c] : eigh_rnd(0u, (unsigned)c);
     for (int i = 0; i + 1 < n; ++i) {
       const double cc = evec[i + 1], a = dvec[i + 1] - lam, b = i + 2 < n ? evec[i + 2] : 0.0;
-      const double yn = Z[(long long)(i + 1) * k + c];
+      const double yn = it ? sc * Z[(long long)(i + 1) * k + c] : eigh_rnd((unsigned)(i + 1), (unsigned)c);
       double u0, u1, u2, ri, n0, n1, nr;
       if (fabs(p0) >= fabs(cc)) {
         if (fabs(p0) < tiny) p0 = p0 < 0.0 ? -tiny : tiny;
@@ -214,43 +248,44 @@ __global__ void eigh_invit_kernel(const double* __restrict__ dvec, const double*
         n0 = fma(-mlt, a, p1); n1 = fma(-mlt, b, p2); nr = fma(-mlt, yn, r);
       }
       const long long o = (long long)i * k + c;
-      U0[o] = u0; U1[o] = u1; U2[o] = u2; Z[o] = ri;
+      if (it == 0) { U0[o] = 1.0 / u0; U1[o] = u1; U2[o] = u2; }      // the factors do not depend on the rhs
+      Z[o] = ri;
       p0 = n0; p1 = n1; p2 = 0.0; r = nr;
     }
     if (fabs(p0) < tiny) p0 = p0 < 0.0 ? -tiny : tiny;
     {
       const long long o = (long long)(n - 1) * k + c;
-      U0[o] = p0; U1[o] = 0.0; U2[o] = 0.0; Z[o] = r;
+      if (it == 0) { U0[o] = 1.0 / p0; U1[o] = 0.0; U2[o] = 0.0; }
+      Z[o] = r;
     }
-    double x1 = 0.0, x2 = 0.0, mx = 0.0;
+    // back substitution; the growth is bounded by 1 / (eps ||T||) per sweep, so the sum of squares cannot overflow
+    double x1 = 0.0, x2 = 0.0, ss = 0.0;
     for (int i = n - 1; i >= 0; --i) {
       const long long o = (long long)i * k + c;
       double x = Z[o];
       x = fma(-U1[o], x1, x);
       x = fma(-U2[o], x2, x);
-      x /= U0[o];
+      x *= U0[o];
       Z[o] = x;
       x2 = x1; x1 = x;
-      mx = fmax(mx, fabs(x));
+      ss = fma(x, x, ss);
     }
-    const double inv = mx > 0.0 ? 1.0 / mx : 1.0;
-    double ss = 0.0;
-    for (int i = 0; i < n; ++i) { const double x = Z[(long long)i * k + c] * inv; ss = fma(x, x, ss); }
-    const double sc = inv / sqrt(ss);
-    for (int i = 0; i < n; ++i) Z[(long long)i * k + c] *= sc;
+    sc = ss > 0.0 ? 1.0 / sqrt(ss) : 1.0;
   }
+  for (int i = 0; i < n; ++i) Z[(long long)i * k + c] *= sc;
 }
 
 // U = H_0 H_1 ... H_{n-3} U, reflector k = I - tau_k v v^T with v[k+1] = 1, v[j] = W[k][j] (j > k+1).
 // CTA b owns columns 2b, 2b+1 of U (n x ldu) in shared memory; thread t owns rows t, t + 1024, ...
-// for the whole kernel, so only the two dot products need a block-wide exchange per reflector.
+// for the whole kernel, so only the two dot products need a block-wide exchange per reflector; the
+// next reflector row is prefetched into L1 while the current one is applied.
 __global__ void __launch_bounds__(1024, 1)
 eigh_backtransform_kernel(const double* __restrict__ W, const double* __restrict__ tauv, int n,
                           double* __restrict__ U, int ldu, int ncols) {
-  extern __shared__ __align__(16) double bsm[];
+  extern __shared__ __align__(16) double bsm[];      // x0[n], x1[n]
+  __shared__ double part[2][2][32];
   double* x0 = bsm;
   double* x1 = bsm + n;
-  double* part = bsm + 2 * n;          // [2][2][32]
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int c0 = 2 * blockIdx.x, c1 = c0 + 1;
   const bool two = c1 < ncols;
@@ -260,31 +295,30 @@ eigh_backtransform_kernel(const double* __restrict__ W, const double* __restrict
   }
   int buf = 0;
   for (int k = n - 3; k >= 0; --k) {
+    const double* Wk = W + (long long)k * n;
+    if (k > 0) {                                     // next reflector row into L1, one request per 128-byte line
+      const double* Wn = Wk - n;
+      for (int i = (k & ~15) + 16 * tid; i < n + 15; i += 16 * 1024)
+        asm volatile("prefetch.global.L1 [%0];" ::"l"(Wn + min(i, n - 1)));
+    }
     const double tau = tauv[k];
     if (tau == 0.0) continue;
-    const double* Wk = W + (long long)k * n;
+    const int ifirst = tid > k ? tid : tid + ((k - tid) / 1024 + 1) * 1024;     // first owned row > k
     double a0 = 0.0, a1 = 0.0;
-    for (int i = tid; i < n; i += 1024) {
-      if (i > k) {
-        const double v = (i == k + 1) ? 1.0 : Wk[i];
-        a0 = fma(v, x0[i], a0);
-        a1 = fma(v, x1[i], a1);
-      }
+    for (int i = ifirst; i < n; i += 1024) {
+      const double v = (i == k + 1) ? 1.0 : Wk[i];
+      a0 = fma(v, x0[i], a0);
+      a1 = fma(v, x1[i], a1);
     }
     a0 = warp_sum(a0); a1 = warp_sum(a1);
-    double* pb = part + buf * 64;
-    if (lane == 0) { pb[warp] = a0; pb[32 + warp] = a1; }
+    if (lane == 0) { part[buf][0][warp] = a0; part[buf][1][warp] = a1; }
     __syncthreads();
-    double s0 = 0.0, s1 = 0.0;
-#pragma unroll
-    for (int w = 0; w < 32; ++w) { s0 += pb[w]; s1 += pb[32 + w]; }
-    s0 *= tau; s1 *= tau;
-    for (int i = tid; i < n; i += 1024) {
-      if (i > k) {
-        const double v = (i == k + 1) ? 1.0 : Wk[i];
-        x0[i] = fma(-s0, v, x0[i]);
-        x1[i] = fma(-s1, v, x1[i]);
-      }
+    double s0 = part[buf][0][lane], s1 = part[buf][1][lane];
+    s0 = warp_sum(s0) * tau; s1 = warp_sum(s1) * tau;
+    for (int i = ifirst; i < n; i += 1024) {
+      const double v = (i == k + 1) ? 1.0 : Wk[i];
+      x0[i] = fma(-s0, v, x0[i]);
+      x1[i] = fma(-s1, v, x1[i]);
     }
     buf ^= 1;
   }

@@ -628,10 +628,11 @@ long long qr_factor_blocked(cudaStream_t st, int qr_path, long long rows, int n,
 }
 
 // ------------------------------------------------------------------ NEXT-2: top-k symmetric eigensolver
-constexpr int EIGH_MAX_N = 14000;     // d, e2 of the multisection / two columns of the back-transform in shared memory
+constexpr int EIGH_MAX_N = 14000;
+constexpr int EIGH_MAX_CHUNKS = 16;   // column chunks of the tridiagonalisation sweep (partial y per chunk)     // d, e2 of the multisection / two columns of the back-transform in shared memory
 
 struct EighWork {
-  double *v0, *v1, *w, *y, *tau, *d, *e, *eig, *scal, *Z, *U0, *U1, *U2, *R;
+  double *v0, *v1, *w, *y, *tau, *d, *e, *eig, *scal, *Z, *U0, *U1, *U2, *R, *ypart;
   void* qr;
 };
 
@@ -644,8 +645,10 @@ size_t eigh_layout(long long n, int k, char* base, EighWork* w) {
   o[8] = take(dbl * 16);
   for (int i = 9; i < 13; ++i) o[i] = take(dbl * n * k);    // Z U0 U1 U2
   o[13] = take(dbl * (size_t)k * k);
+  size_t oy = take(dbl * n * EIGH_MAX_CHUNKS);
   size_t oq = take(qr_work_bytes_impl(n, k));
   if (w) {
+    w->ypart = reinterpret_cast<double*>(base + oy);
     double** f[14] = {&w->v0, &w->v1, &w->w, &w->y, &w->tau, &w->d, &w->e, &w->eig, &w->scal,
                       &w->Z, &w->U0, &w->U1, &w->U2, &w->R};
     for (int i = 0; i < 14; ++i) *f[i] = reinterpret_cast<double*>(base + o[i]);
@@ -676,21 +679,37 @@ long long eigh_top(cudaStream_t st, int n, int k, double* W, double* lam, double
   }
   constexpr int ROWS = 4;
   cudaMemsetAsync(wk.tau, 0, sizeof(double) * n, st);
+  int nchunk_prev = 0;
+#define REFL(k_, vprev_, vnew_)                                                                                  \
+  do {                                                                                                           \
+    const int left_ = n - (k_);                                                                                  \
+    if (left_ <= 2048) eigh_reflector_kernel<2><<<1, 1024, 0, st>>>(W, n, (k_), wk.ypart, nchunk_prev, (vprev_), wk.w, (vnew_), wk.tau, wk.d, wk.e); \
+    else if (left_ <= 6144) eigh_reflector_kernel<6><<<1, 1024, 0, st>>>(W, n, (k_), wk.ypart, nchunk_prev, (vprev_), wk.w, (vnew_), wk.tau, wk.d, wk.e); \
+    else if (left_ <= 10240) eigh_reflector_kernel<10><<<1, 1024, 0, st>>>(W, n, (k_), wk.ypart, nchunk_prev, (vprev_), wk.w, (vnew_), wk.tau, wk.d, wk.e); \
+    else eigh_reflector_kernel<14><<<1, 1024, 0, st>>>(W, n, (k_), wk.ypart, nchunk_prev, (vprev_), wk.w, (vnew_), wk.tau, wk.d, wk.e); \
+  } while (0)
   for (int k2 = 0; k2 + 2 < n; ++k2) {
     double* vprev = (k2 & 1) ? wk.v0 : wk.v1;      // v_{k-1}
     double* vnew = (k2 & 1) ? wk.v1 : wk.v0;       // v_k
-    eigh_reflector_kernel<<<1, 1024, 0, st>>>(W, n, k2, wk.y, vprev, wk.w, vnew, wk.tau, wk.d, wk.e);
-    const int nrows = n - k2 - 1, warps = (nrows + ROWS - 1) / ROWS;
-    eigh_pass_kernel<ROWS><<<(warps + 7) / 8, 256, 0, st>>>(W, n, k2, vprev, wk.w, vnew, wk.y);
+    REFL(k2, vprev, vnew);
+    const int nt = n - k2 - 1;                     // trailing block is nt x nt
+    int cw = 256 * ((nt + 256 * EIGH_MAX_CHUNKS - 1) / (256 * EIGH_MAX_CHUNKS));
+    const int nchunk = (nt + cw - 1) / cw;
+    dim3 grid(nchunk, (nt + 8 * ROWS - 1) / (8 * ROWS));
+    eigh_pass_kernel<ROWS><<<grid, 256, sizeof(double) * 3 * cw, st>>>(W, n, k2, cw, vprev, wk.w, vnew, wk.ypart);
+    nchunk_prev = nchunk;
     launches += 2;
   }
   {
     const int kf = n >= 2 ? n - 2 : 0;
     double* vprev = (kf & 1) ? wk.v0 : wk.v1;
-    eigh_reflector_kernel<<<1, 1024, 0, st>>>(W, n, kf, wk.y, vprev, wk.w, wk.v0, wk.tau, wk.d, wk.e);
+    REFL(kf, vprev, wk.v0);
+    launches += 1;
   }
-  multisect_kernel<<<(n + 7) / 8, 256, sizeof(double) * (2 * (size_t)n + 40), st>>>(wk.d, wk.e, n, wk.eig);
-  eigh_select_kernel<<<(n + 255) / 256, 256, 0, st>>>(wk.eig, n, k, lam, wk.d, wk.e, wk.scal);
+#undef REFL
+  const int nc = 2 * k < n ? 2 * k : n;            // candidates: the k smallest and the k largest eigenvalues
+  multisect_kernel<<<(nc + 7) / 8, 256, sizeof(double) * (2 * (size_t)n + 40), st>>>(wk.d, wk.e, n, wk.eig, k);
+  eigh_select_kernel<<<(nc + 255) / 256, 256, 0, st>>>(wk.eig, nc, k, lam, wk.d, wk.e, n, wk.scal);
   eigh_invit_kernel<<<(k + 31) / 32, 32, 0, st>>>(wk.d, wk.e, n, lam, k, wk.scal, wk.Z, wk.U0, wk.U1, wk.U2, 3);
   launches += 4;
   *err = cudaGetLastError();
@@ -699,7 +718,8 @@ long long eigh_top(cudaStream_t st, int n, int k, double* W, double* lam, double
   if (nq < 0) return -1;
   launches += nq;
   if (n >= 3) {
-    eigh_backtransform_kernel<<<(k + 1) / 2, 1024, sizeof(double) * (2 * (size_t)n + 128), st>>>(W, wk.tau, n, U, k, k);
+    const int nb = (k + 1) / 2;
+    eigh_backtransform_kernel<<<nb, 1024, sizeof(double) * 2 * (size_t)n, st>>>(W, wk.tau, n, U, k, k);
     launches += 1;
   }
   eigh_sign_kernel<<<k, 256, 0, st>>>(U, n, k);

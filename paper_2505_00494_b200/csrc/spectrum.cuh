@@ -240,12 +240,12 @@ tridiag_smem_kernel(const double* __restrict__ Cmat, int n, double* __restrict__
 }
 
 // Eigenvalues of the tridiagonal by warp-multisection: warp w of block B finds
-// eigenvalue number idx = 8 B + w (ascending).  Each iteration the 32 lanes evaluate
+// eigenvalue number idx = 8 B + w (ascending; see `ke` for the partial mode).  Each iteration the 32 lanes evaluate
 // the Sturm count at 32 interior points of [a, b], shrinking the bracket 33-fold
 // (about 11 iterations to the last ulp instead of ~55 bisection steps).
 __global__ void __launch_bounds__(256)
 multisect_kernel(const double* __restrict__ dvec, const double* __restrict__ evec, int n,
-                 double* __restrict__ eig_out) {
+                 double* __restrict__ eig_out, int ke = 0) {
   extern __shared__ double msm[];               // d[n], e2[n], red[33]
   double* d = msm; double* e2 = msm + n; double* red = msm + 2 * n;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -269,8 +269,12 @@ multisect_kernel(const double* __restrict__ dvec, const double* __restrict__ eve
   const double pivmin = fmax(2.2250738585072014e-308 * fmax(1.0, gemax), 1e-300);
   glo -= 2.0 * 2.220446049250313e-16 * bnd * n + 2.0 * pivmin;
   ghi += 2.0 * 2.220446049250313e-16 * bnd * n + 2.0 * pivmin;
-  const int idx = blockIdx.x * 8 + warp;
-  if (idx >= n) return;
+  // ke > 0 (and 2 ke < n): only the ke smallest and the ke largest eigenvalues, written compactly
+  // (slot c < ke: eigenvalue c; slot c >= ke: eigenvalue n - 2 ke + c) -- the eigen step's candidates.
+  const int slot = blockIdx.x * 8 + warp;
+  const bool part = ke > 0 && 2 * ke < n;
+  if (slot >= (part ? 2 * ke : n)) return;
+  const int idx = (part && slot >= ke) ? n - 2 * ke + slot : slot;
   double a = glo, b = ghi;
   for (int it = 0; it < 64; ++it) {
     const double h = (b - a) / 33.0;
@@ -287,7 +291,7 @@ multisect_kernel(const double* __restrict__ dvec, const double* __restrict__ eve
     a = na; b = nb;
     if (!progress || !(b - a > 0.0)) break;
   }
-  if (lane == 0) eig_out[idx] = 0.5 * (a + b);
+  if (lane == 0) eig_out[slot] = 0.5 * (a + b);
 }
 
 // One block, blockDim.x >= n: s = sorted |eig| (descending), delta vs s_prev.

@@ -3,6 +3,9 @@ its NVTX range (K1_reduced_corner ... K7_normalize), e.g.
 
   ncu --set full --nvtx --nvtx-include "K4_absorb_a/" -c 1 \
       python -m paper_2505_00494_b200.profile_stage --config cfg4 --steps 2
+
+--warmup N runs the NEXT-2 warm-up instead (bulk initialisation + N eigen steps, NVTX ranges
+E1_enlarged_corner, E2_eigh, E3_edge); --eig-steps M adds M eigen steps at the final chi.
 """
 import argparse
 import os
@@ -18,12 +21,19 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--config", default="cfg4", choices=sorted(CONFIGS))
     ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--warmup", type=int, default=-1)
+    ap.add_argument("--eig-steps", type=int, default=0)
     a = ap.parse_args()
     A, C0, T0, c = gen_named(a.config)
     h = pkg.QRCTM(c["d"], c["D"], c["chi"])
     h.set_option(pkg.OPT_USE_GRAPH, 0)          # plain launches keep the NVTX stage ranges
     h.set_A(A)
-    h.set_env(C0, T0)
+    if a.warmup >= 0:
+        h.warmup(a.warmup)
+    else:
+        h.set_env(C0, T0)
+    for _ in range(a.eig_steps):
+        h.eig_step()
     for _ in range(a.steps):
         h.step()
     torch.cuda.synchronize()
