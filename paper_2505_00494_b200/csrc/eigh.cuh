@@ -3,9 +3,11 @@
 // Hand-written symmetric eigensolver for the k largest-|lambda| pairs of an n x n matrix:
 //   1. Householder tridiagonalisation, one reflector per step, all SMs:
 //        eigh_reflector_kernel (one CTA)  : finishes w_{k-1}, brings row k up to date, builds v_k
-//        eigh_pass_kernel      (grid)     : applies the pending rank-2 update of reflector k-1 to
-//                                           the trailing block and, in the same sweep, y = A22 v_k
-//      (one read + one write of the trailing block per step; HBM/L2-bound)
+//        eigh_pass_kernel      (grid)     : applies the pending rank-2 update of reflector k-1 to the upper
+//                                           triangle of the trailing block and, in the same sweep, the
+//                                           row and column partial sums of y = A22 v_k
+//        eigh_ysum_kernel      (grid)     : y from the partials, fixed order
+//      (one read + one write of HALF the trailing block per step; HBM/L2-bound)
 //   2. the k smallest and k largest eigenvalues of the tridiagonal by warp multisection (spectrum.cuh)
 //   3. eigh_select_kernel: the k of largest magnitude, stable in ascending-eigenvalue order
 //   4. eigh_invit_kernel: inverse iteration on the tridiagonal, one thread per vector,
@@ -19,8 +21,10 @@
 
 namespace qk {
 
+constexpr int EIGH_CW = 256;      // columns per chunk of the tridiagonalisation sweep
+
 // One CTA.  Step k of the tridiagonalisation of W (n x n, row-major, symmetric; rows/cols >= k live).
-//   k > 0 : y = A22 v_{k-1} (rows k..n-1) = the sum of the pass kernel's per-chunk partials; forms w_{k-1} = p - (tau/2)(p.v) v, p = tau y
+//   k > 0 : y = A22 v_{k-1} (rows k..n-1, from eigh_ysum_kernel, or summed here when rg_prev > 0); forms w_{k-1} = p - (tau/2)(p.v) v, p = tau y
 //   row k brought up to date: r[j] = W[k][j] - v[k] w[j] - w[k] v[j]  (j >= k)
 //   k <= n-3: reflector v_k from r[k+1..], stored in vnew[] and in W[k][k+2..] (v_k[k+1] = 1 implied)
 //   k == n-2: the last 2x2 block: d[n-2], e[n-1], d[n-1]
@@ -28,7 +32,8 @@ namespace qk {
 // Thread t owns columns k + t, k + t + 1024, ... (RMAX of them, n - k <= 1024 RMAX) in registers through all phases.
 template <int RMAX>
 __global__ void __launch_bounds__(1024, 1)
-eigh_reflector_kernel(double* __restrict__ W, int n, int k, const double* __restrict__ ypart, int nchunk_prev,
+eigh_reflector_kernel(double* __restrict__ W, int n, int k, const double* __restrict__ y,
+                      const double* __restrict__ rowpart, const double* __restrict__ colpart, int rg_prev,
                       const double* __restrict__ vprev, double* __restrict__ wv, double* __restrict__ vnew,
                       double* __restrict__ tauv, double* __restrict__ dvec, double* __restrict__ evec) {
   __shared__ double sh[33];
@@ -45,7 +50,13 @@ eigh_reflector_kernel(double* __restrict__ W, int n, int k, const double* __rest
       const int i = k + tid + 1024 * r;
       double yi = 0.0; vp[r] = 0.0;
       if (i < n) {
-        for (int c = 0; c < nchunk_prev; ++c) yi += ypart[(long long)c * n + i];      // fixed order: deterministic
+        if (rg_prev > 0) {          // short tail: sum the sweep's partials here (same order as eigh_ysum_kernel)
+          const int ii = i - k, nch = (n - k + EIGH_CW - 1) / EIGH_CW;
+          for (int c = ii / EIGH_CW; c < nch; ++c) yi += rowpart[(long long)c * n + i];
+          for (int g = 0; g <= ii / rg_prev; ++g) yi += colpart[(long long)g * n + i];
+        } else {
+          yi = y[i];
+        }
         vp[r] = vprev[i];
       }
       x[r] = tau * yi;
@@ -102,66 +113,97 @@ eigh_reflector_kernel(double* __restrict__ W, int n, int k, const double* __rest
   }
 }
 
-// Grid (x: column chunks of cw, y: groups of 8*ROWS rows).  Rows i in [k+1, n), columns j in [k+1, n):
-//   x = W[i][j] - vprev[i] w[j] - w[i] vprev[j]   (the pending update of reflector k-1, skipped when k == 0),
-// stored back, and ypart[chunk][i] = sum_{j in chunk} x vnew[j].  Each warp owns ROWS rows of the chunk, lanes
-// run along the contiguous j; the three vectors of the chunk are staged in shared memory once per CTA.
-template <int ROWS>
-__global__ void __launch_bounds__(256)
-eigh_pass_kernel(double* __restrict__ W, int n, int k, int cw, const double* __restrict__ vprev,
-                 const double* __restrict__ wv, const double* __restrict__ vnew, double* __restrict__ ypart) {
-  extern __shared__ __align__(16) double psm[];       // vnew[cw], vprev[cw], w[cw]
-  double* s_vn = psm; double* s_vp = psm + cw; double* s_w = psm + 2 * cw;
+// Symmetric sweep over the UPPER triangle of the trailing block (rows/cols k+1..n-1; relative index ii = i-(k+1)):
+//   x = W[i][j] - vprev[i] w[j] - w[i] vprev[j]   (pending update of reflector k-1; skipped when k == 0), j >= i,
+// stored back, and the two halves of y = A22 v_k:
+//   rowpart[c][i] = sum_{j in chunk c, j >= i} x_ij vnew[j]        colpart[g][j] = sum_{i in row group g, i < j} x_ij vnew[i]
+// Grid: x = column chunk c (EIGH_CW columns), y = row group g (rg rows, a multiple of 32).  A CTA walks the 32-row blocks
+// of its group that reach the chunk (warp w: rows 4w..4w+3 of the block, lanes along the contiguous j, 8 columns per
+// lane), keeps its column sums in registers, and reduces them over its 8 warps at the end.  Half the bytes of a
+// full-matrix sweep; every partial is written by exactly one CTA and summed later in a fixed order (deterministic).
+__global__ void __launch_bounds__(256, 2)
+eigh_pass_kernel(double* __restrict__ W, int n, int k, int rg, const double* __restrict__ vprev,
+                 const double* __restrict__ wv, const double* __restrict__ vnew, double* __restrict__ rowpart,
+                 double* __restrict__ colpart) {
+  constexpr int QW = EIGH_CW / 32, ROWS = 4;
+  __shared__ double s_col[8][EIGH_CW];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const bool pending = k > 0;
-  const int j0 = k + 1 + blockIdx.x * cw;
-  const int jn = min(cw, n - j0);
-  for (int t = threadIdx.x; t < jn; t += 256) {
-    s_vn[t] = vnew[j0 + t];
-    s_vp[t] = pending ? vprev[j0 + t] : 0.0;
-    s_w[t] = pending ? wv[j0 + t] : 0.0;
+  const int base = k + 1, nt = n - base;
+  const int c = blockIdx.x, g = blockIdx.y;
+  const int jj0 = c * EIGH_CW, jlast = min(jj0 + EIGH_CW, nt) - 1;     // relative column range of the chunk
+  const int ii_begin = g * rg, ii_end = min(ii_begin + rg, nt);
+  if (ii_begin > jlast) return;                                        // group entirely below the diagonal
+  double vn[QW], vp[QW], wj[QW], colacc[QW];
+#pragma unroll
+  for (int q = 0; q < QW; ++q) {
+    const int jj = jj0 + lane + 32 * q;
+    const bool ok = jj < nt;
+    vn[q] = ok ? vnew[base + jj] : 0.0;
+    vp[q] = (ok && pending) ? vprev[base + jj] : 0.0;
+    wj[q] = (ok && pending) ? wv[base + jj] : 0.0;
+    colacc[q] = 0.0;
   }
-  __syncthreads();
-  const int i0 = k + 1 + (blockIdx.y * 8 + warp) * ROWS;
-  if (i0 >= n) return;
-  double vi[ROWS], wi[ROWS], acc[ROWS];
-  double* row[ROWS];
+  double* rp = rowpart + (long long)c * n + base;
+  for (int rb = ii_begin; rb < ii_end && rb <= jlast; rb += 32) {
 #pragma unroll
-  for (int r = 0; r < ROWS; ++r) {
-    const int i = min(i0 + r, n - 1);
-    row[r] = W + (long long)i * n + j0;
-    vi[r] = pending ? vprev[i] : 0.0;
-    wi[r] = pending ? wv[i] : 0.0;
-    acc[r] = 0.0;
-  }
-  if (pending) {
-#pragma unroll 2
-    for (int t = lane; t < jn; t += 32) {
-      const double vn = s_vn[t], vj = s_vp[t], wj = s_w[t];
-      double x[ROWS];
+    for (int r = 0; r < ROWS; ++r) {
+      const int ii = rb + ROWS * warp + r;
+      if (ii >= ii_end || ii > jlast) continue;                       // warp-uniform
+      double* row = W + (long long)(base + ii) * n + base + jj0 + lane;
+      const double vni = vnew[base + ii];
+      const double vi = pending ? vprev[base + ii] : 0.0, wi = pending ? wv[base + ii] : 0.0;
+      double x[QW];
 #pragma unroll
-      for (int r = 0; r < ROWS; ++r) x[r] = row[r][t];
-#pragma unroll
-      for (int r = 0; r < ROWS; ++r) {
-        x[r] = fma(-vi[r], wj, x[r]);
-        x[r] = fma(-wi[r], vj, x[r]);
-        if (i0 + r < n) row[r][t] = x[r];
-        acc[r] = fma(x[r], vn, acc[r]);
+      for (int q = 0; q < QW; ++q) {
+        const int jj = jj0 + lane + 32 * q;
+        x[q] = (jj >= ii && jj < nt) ? row[32 * q] : 0.0;
       }
-    }
-  } else {
-    for (int t = lane; t < jn; t += 32) {
-      const double vn = s_vn[t];
+      double racc = 0.0;
 #pragma unroll
-      for (int r = 0; r < ROWS; ++r) acc[r] = fma(row[r][t], vn, acc[r]);
+      for (int q = 0; q < QW; ++q) {
+        const int jj = jj0 + lane + 32 * q;
+        if (jj >= ii && jj < nt) {
+          if (pending) {
+            x[q] = fma(-vi, wj[q], x[q]);
+            x[q] = fma(-wi, vp[q], x[q]);
+            row[32 * q] = x[q];
+          }
+          racc = fma(x[q], vn[q], racc);
+          if (jj > ii) colacc[q] = fma(x[q], vni, colacc[q]);
+        }
+      }
+      racc = warp_sum(racc);
+      if (lane == 0) rp[ii] = racc;
     }
   }
-  double* yp = ypart + (long long)blockIdx.x * n;
 #pragma unroll
-  for (int r = 0; r < ROWS; ++r) {
-    const double sm = warp_sum(acc[r]);
-    if (lane == 0 && i0 + r < n) yp[i0 + r] = sm;
+  for (int q = 0; q < QW; ++q) s_col[warp][lane + 32 * q] = colacc[q];
+  __syncthreads();
+  {
+    const int t = threadIdx.x, jj = jj0 + t;
+    if (jj < nt) {
+      double sacc = 0.0;
+#pragma unroll
+      for (int w2 = 0; w2 < 8; ++w2) sacc += s_col[w2][t];
+      colpart[(long long)g * n + base + jj] = sacc;
+    }
   }
+}
+
+// y[i] = sum of the sweep's partials in a fixed order: row parts of the chunks from the one holding the diagonal on,
+// column parts of the row groups up to the one holding row i.
+__global__ void __launch_bounds__(256)
+eigh_ysum_kernel(const double* __restrict__ rowpart, const double* __restrict__ colpart, int n, int k, int rg,
+                 double* __restrict__ y) {
+  const int base = k + 1, nt = n - base;
+  const int ii = blockIdx.x * 256 + threadIdx.x;
+  if (ii >= nt) return;
+  const int nch = (nt + EIGH_CW - 1) / EIGH_CW;
+  double acc = 0.0;
+  for (int c = ii / EIGH_CW; c < nch; ++c) acc += rowpart[(long long)c * n + base + ii];
+  for (int g = 0; g <= ii / rg; ++g) acc += colpart[(long long)g * n + base + ii];
+  y[base + ii] = acc;
 }
 
 // (W + W^T)/2 in place (C~ is symmetric for a C4v state; rounding in the GEMMs that

@@ -629,10 +629,10 @@ long long qr_factor_blocked(cudaStream_t st, int qr_path, long long rows, int n,
 
 // ------------------------------------------------------------------ NEXT-2: top-k symmetric eigensolver
 constexpr int EIGH_MAX_N = 14000;
-constexpr int EIGH_MAX_CHUNKS = 16;   // column chunks of the tridiagonalisation sweep (partial y per chunk)     // d, e2 of the multisection / two columns of the back-transform in shared memory
+constexpr int EIGH_MAX_GROUPS = 96;   // row groups of the tridiagonalisation sweep (column partials of y per group)     // d, e2 of the multisection / two columns of the back-transform in shared memory
 
 struct EighWork {
-  double *v0, *v1, *w, *y, *tau, *d, *e, *eig, *scal, *Z, *U0, *U1, *U2, *R, *ypart;
+  double *v0, *v1, *w, *y, *tau, *d, *e, *eig, *scal, *Z, *U0, *U1, *U2, *R, *rowpart, *colpart;
   void* qr;
 };
 
@@ -645,10 +645,12 @@ size_t eigh_layout(long long n, int k, char* base, EighWork* w) {
   o[8] = take(dbl * 16);
   for (int i = 9; i < 13; ++i) o[i] = take(dbl * n * k);    // Z U0 U1 U2
   o[13] = take(dbl * (size_t)k * k);
-  size_t oy = take(dbl * n * EIGH_MAX_CHUNKS);
+  size_t oy = take(dbl * n * ((EIGH_MAX_N + EIGH_CW - 1) / EIGH_CW));
+  size_t oc = take(dbl * n * EIGH_MAX_GROUPS);
   size_t oq = take(qr_work_bytes_impl(n, k));
   if (w) {
-    w->ypart = reinterpret_cast<double*>(base + oy);
+    w->rowpart = reinterpret_cast<double*>(base + oy);
+    w->colpart = reinterpret_cast<double*>(base + oc);
     double** f[14] = {&w->v0, &w->v1, &w->w, &w->y, &w->tau, &w->d, &w->e, &w->eig, &w->scal,
                       &w->Z, &w->U0, &w->U1, &w->U2, &w->R};
     for (int i = 0; i < 14; ++i) *f[i] = reinterpret_cast<double*>(base + o[i]);
@@ -677,28 +679,34 @@ long long eigh_top(cudaStream_t st, int n, int k, double* W, double* lam, double
     cudaFuncSetAttribute(eigh_backtransform_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem - 1024);
     attr_done = 1;
   }
-  constexpr int ROWS = 4;
   cudaMemsetAsync(wk.tau, 0, sizeof(double) * n, st);
-  int nchunk_prev = 0;
 #define REFL(k_, vprev_, vnew_)                                                                                  \
   do {                                                                                                           \
     const int left_ = n - (k_);                                                                                  \
-    if (left_ <= 2048) eigh_reflector_kernel<2><<<1, 1024, 0, st>>>(W, n, (k_), wk.ypart, nchunk_prev, (vprev_), wk.w, (vnew_), wk.tau, wk.d, wk.e); \
-    else if (left_ <= 6144) eigh_reflector_kernel<6><<<1, 1024, 0, st>>>(W, n, (k_), wk.ypart, nchunk_prev, (vprev_), wk.w, (vnew_), wk.tau, wk.d, wk.e); \
-    else if (left_ <= 10240) eigh_reflector_kernel<10><<<1, 1024, 0, st>>>(W, n, (k_), wk.ypart, nchunk_prev, (vprev_), wk.w, (vnew_), wk.tau, wk.d, wk.e); \
-    else eigh_reflector_kernel<14><<<1, 1024, 0, st>>>(W, n, (k_), wk.ypart, nchunk_prev, (vprev_), wk.w, (vnew_), wk.tau, wk.d, wk.e); \
+    if (left_ <= 2048) eigh_reflector_kernel<2><<<1, 1024, 0, st>>>(W, n, (k_), wk.y, wk.rowpart, wk.colpart, rg_prev, (vprev_), wk.w, (vnew_), wk.tau, wk.d, wk.e); \
+    else if (left_ <= 6144) eigh_reflector_kernel<6><<<1, 1024, 0, st>>>(W, n, (k_), wk.y, wk.rowpart, wk.colpart, rg_prev, (vprev_), wk.w, (vnew_), wk.tau, wk.d, wk.e); \
+    else if (left_ <= 10240) eigh_reflector_kernel<10><<<1, 1024, 0, st>>>(W, n, (k_), wk.y, wk.rowpart, wk.colpart, rg_prev, (vprev_), wk.w, (vnew_), wk.tau, wk.d, wk.e); \
+    else eigh_reflector_kernel<14><<<1, 1024, 0, st>>>(W, n, (k_), wk.y, wk.rowpart, wk.colpart, rg_prev, (vprev_), wk.w, (vnew_), wk.tau, wk.d, wk.e); \
   } while (0)
+  int rg_prev = 0;                                 // > 0: the next reflector kernel sums the partials itself
   for (int k2 = 0; k2 + 2 < n; ++k2) {
     double* vprev = (k2 & 1) ? wk.v0 : wk.v1;      // v_{k-1}
     double* vnew = (k2 & 1) ? wk.v1 : wk.v0;       // v_k
     REFL(k2, vprev, vnew);
     const int nt = n - k2 - 1;                     // trailing block is nt x nt
-    int cw = 256 * ((nt + 256 * EIGH_MAX_CHUNKS - 1) / (256 * EIGH_MAX_CHUNKS));
-    const int nchunk = (nt + cw - 1) / cw;
-    dim3 grid(nchunk, (nt + 8 * ROWS - 1) / (8 * ROWS));
-    eigh_pass_kernel<ROWS><<<grid, 256, sizeof(double) * 3 * cw, st>>>(W, n, k2, cw, vprev, wk.w, vnew, wk.ypart);
-    nchunk_prev = nchunk;
-    launches += 2;
+    const int nch = (nt + EIGH_CW - 1) / EIGH_CW;
+    // rows per group: a multiple of 32, about 600 CTAs in the upper triangle, at most EIGH_MAX_GROUPS groups
+    long long G = (long long)nt * nch / (2 * 32 * 600);
+    const long long gmin = (nt + 32LL * EIGH_MAX_GROUPS - 1) / (32LL * EIGH_MAX_GROUPS);
+    if (G < gmin) G = gmin;
+    if (G < 1) G = 1;
+    const int rg = (int)(32 * G), ng = (nt + rg - 1) / rg;
+    eigh_pass_kernel<<<dim3(nch, ng), 256, 0, st>>>(W, n, k2, rg, vprev, wk.w, vnew, wk.rowpart, wk.colpart);
+    if (nt <= 2048) { rg_prev = rg; launches += 2; }       // launch-latency-bound tail: one kernel fewer per step
+    else {
+      eigh_ysum_kernel<<<(nt + 255) / 256, 256, 0, st>>>(wk.rowpart, wk.colpart, n, k2, rg, wk.y);
+      rg_prev = 0; launches += 3;
+    }
   }
   {
     const int kf = n >= 2 ? n - 2 : 0;
