@@ -234,6 +234,31 @@ int qrctm_warmup(qrctm_t* h, int n_eig_steps);
 unsigned long long qrctm_eigh_work_bytes(int n, int k);
 int qrctm_eigh_top_f64(void* cuda_stream, int n, int k, double* A, double* lam, double* U, void* work);
 
+/* ---- NEXT-4 ("the use of multiple GPUs") ----
+ * One iteration sharded over the column index m of Q: K3 -> K4 -> K5 never mix different m
+ * (P[:,m,:,:], S[m,...], T'[m,:,:]), and (E4) is a sum over m.  Every rank holds the same
+ * A, C, T (replicated, as is the cheap K1 + K2), computes the rows m in [m0, m1) of T' and
+ * its partial C', and ONE exchange step assembles them: all-gather of the T' slices
+ * (8 chi^2 D^2 bytes in total), all-reduce of the partial C' (8 chi^2 bytes).  The library
+ * does not link a communication library: the exchange is done by the caller on the DEVICE
+ * buffers qrctm_shard_buffers returns (the Python binding uses torch.distributed / NCCL).
+ *
+ * qrctm_shard_range: this rank's contiguous range [m0, m1) of m (sizes differ by <= 1;
+ *   empty when nranks > chi).  HOST pointers.
+ * qrctm_shard_front: K1, K2, then K3-K5 and the partial (E4) for this rank's range.
+ *   Afterwards Tn (chi x D^2 x chi, rows m) holds this rank's rows and ZEROS elsewhere,
+ *   Cn (chi x chi) the partial corner -- so either an all-gather of the row blocks or a
+ *   plain sum over ranks of the whole buffers assembles T' and C'.  nranks = 1 gives the
+ *   un-normalised result of an ordinary step.
+ * qrctm_shard_buffers: DEVICE pointers of Cn and Tn inside the handle's workspace
+ *   (owned by the handle; valid until qrctm_destroy).
+ * qrctm_shard_finish: K7 on the exchanged Cn, Tn -> the new C, T.  The caller must order
+ *   the exchange before it on the handle's stream. */
+int qrctm_shard_range(int chi, int rank, int nranks, int* m0, int* m1);
+int qrctm_shard_front(qrctm_t* h, int rank, int nranks);
+int qrctm_shard_buffers(qrctm_t* h, double** Cn, double** Tn);
+int qrctm_shard_finish(qrctm_t* h);
+
 /* FP64 issue-rate probe (roofline denominators):
  * kind 0 = DFMA chains, 1 = DMMA m8n8k4 chains.  Returns TFLOP/s measured with
  * CUDA events over `iters` loop trips on every SM.  HOST pointer. */

@@ -35,6 +35,7 @@ SYMBOLS = (
     "qrctm_version",
     "qrctm_get_chi", "qrctm_init_bulk", "qrctm_eig_step", "qrctm_get_eig", "qrctm_warmup",
     "qrctm_eigh_work_bytes", "qrctm_eigh_top_f64",
+    "qrctm_shard_range", "qrctm_shard_front", "qrctm_shard_buffers", "qrctm_shard_finish",
 )
 
 
@@ -92,6 +93,10 @@ def load_library() -> ctypes.CDLL:
     lib.qrctm_eigh_work_bytes.argtypes = [c_int, c_int]
     lib.qrctm_eigh_work_bytes.restype = c_ulonglong
     lib.qrctm_eigh_top_f64.argtypes = [P, c_int, c_int, P, P, P, P]
+    lib.qrctm_shard_range.argtypes = [c_int, c_int, c_int, POINTER(c_int), POINTER(c_int)]
+    lib.qrctm_shard_front.argtypes = [P, c_int, c_int]
+    lib.qrctm_shard_buffers.argtypes = [P, POINTER(P), POINTER(P)]
+    lib.qrctm_shard_finish.argtypes = [P]
     lib.qrctm_last_error.argtypes = [P]
     lib.qrctm_last_error.restype = c_char_p
     lib.qrctm_version.restype = c_char_p
@@ -251,6 +256,36 @@ class QRCTM:
     def warmup(self, n_eig_steps: int):
         self._check(self.lib.qrctm_warmup(self._h, n_eig_steps))
 
+    # -- NEXT-4: one iteration sharded over ranks (one process per GPU)
+    def shard_front(self, rank: int, nranks: int):
+        self._check(self.lib.qrctm_shard_front(self._h, rank, nranks))
+
+    def shard_buffers(self):
+        """(Cn, Tn): torch views of the handle's device buffers the exchange works on."""
+        import torch
+        pc, pt = c_void_p(), c_void_p()
+        self._check(self.lib.qrctm_shard_buffers(self._h, byref(pc), byref(pt)))
+        n, base = self.chi, self._ws.data_ptr()
+
+        def view(ptr, count, shape):
+            off = ptr - base
+            return self._ws[off:off + 8 * count].view(torch.float64).view(shape)
+        return view(pc.value, n * n, (n, n)), view(pt.value, n * self.b * n, (n, self.b * n))
+
+    def shard_finish(self):
+        self._check(self.lib.qrctm_shard_finish(self._h))
+
+    def shard_step(self, rank: int, nranks: int, group=None):
+        """One QR-CTMRG iteration with K3-K5 split over `nranks` processes (torch.distributed must be initialised
+        when nranks > 1); every rank ends with the same new C, T."""
+        import torch
+        self.shard_front(rank, nranks)
+        if nranks > 1:
+            Cn, Tn = self.shard_buffers()
+            with torch.cuda.stream(self.stream):
+                shard_exchange(Cn, Tn, rank, nranks, group)
+        self.shard_finish()
+
     def get_a(self):
         a = np.empty((self.b,) * 4, dtype=np.float64)
         self._check(self.lib.qrctm_get_a(self._h, _ptr(a)))
@@ -328,6 +363,27 @@ def qr_f64(X, path: int = 0):
         raise QrctmError(f"qrctm_qr_f64 failed: {rc}")
     torch.cuda.current_stream().synchronize()
     return Q, R
+
+
+def shard_range(chi: int, rank: int, nranks: int):
+    m0, m1 = c_int(0), c_int(0)
+    if load_library().qrctm_shard_range(chi, rank, nranks, byref(m0), byref(m1)) != QRCTM_OK:
+        raise QrctmError("qrctm_shard_range: invalid arguments")
+    return m0.value, m1.value
+
+
+def shard_exchange(Cn, Tn, rank: int, nranks: int, group=None):
+    """The one exchange step of a sharded iteration (include/qrctm.h, NEXT-4), in place on every rank:
+    Tn (chi rows of D^2 chi doubles; this rank's rows filled, zeros elsewhere) becomes the full T',
+    Cn (partial) the full C'.  Equal slices: all-gather of the row blocks; ragged split: sum over ranks."""
+    import torch.distributed as dist
+    chi = Tn.shape[0]
+    if chi % nranks == 0:
+        mine = Tn.view(nranks, -1)[rank].clone()
+        dist.all_gather_into_tensor(Tn.view(-1), mine, group=group)
+    else:
+        dist.all_reduce(Tn, op=dist.ReduceOp.SUM, group=group)
+    dist.all_reduce(Cn, op=dist.ReduceOp.SUM, group=group)
 
 
 def eigh_top_f64(A, k: int):

@@ -23,6 +23,22 @@ namespace qk {
 
 constexpr int EIGH_CW = 256;      // columns per chunk of the tridiagonalisation sweep
 
+// sum_{t = t0}^{t1 - 1} part[t * stride], added in index order; loads issued eight at a time (the plain loop
+// would wait for every load before issuing the next)
+__device__ __forceinline__ double eigh_strided_sum(const double* __restrict__ part, long long stride, int t0, int t1,
+                                                   double acc) {
+  int t = t0;
+  for (; t + 8 <= t1; t += 8) {
+    double v[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) v[u] = part[(long long)(t + u) * stride];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) acc += v[u];
+  }
+  for (; t < t1; ++t) acc += part[(long long)t * stride];
+  return acc;
+}
+
 // One CTA.  Step k of the tridiagonalisation of W (n x n, row-major, symmetric; rows/cols >= k live).
 //   k > 0 : y = A22 v_{k-1} (rows k..n-1, from eigh_ysum_kernel, or summed here when rg_prev > 0); forms w_{k-1} = p - (tau/2)(p.v) v, p = tau y
 //   row k brought up to date: r[j] = W[k][j] - v[k] w[j] - w[k] v[j]  (j >= k)
@@ -52,8 +68,8 @@ eigh_reflector_kernel(double* __restrict__ W, int n, int k, const double* __rest
       if (i < n) {
         if (rg_prev > 0) {          // short tail: sum the sweep's partials here (same order as eigh_ysum_kernel)
           const int ii = i - k, nch = (n - k + EIGH_CW - 1) / EIGH_CW;
-          for (int c = ii / EIGH_CW; c < nch; ++c) yi += rowpart[(long long)c * n + i];
-          for (int g = 0; g <= ii / rg_prev; ++g) yi += colpart[(long long)g * n + i];
+          yi = eigh_strided_sum(rowpart + i, n, ii / EIGH_CW, nch, yi);
+          yi = eigh_strided_sum(colpart + i, n, 0, ii / rg_prev + 1, yi);
         } else {
           yi = y[i];
         }
@@ -193,16 +209,15 @@ eigh_pass_kernel(double* __restrict__ W, int n, int k, int rg, const double* __r
 
 // y[i] = sum of the sweep's partials in a fixed order: row parts of the chunks from the one holding the diagonal on,
 // column parts of the row groups up to the one holding row i.
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(64)
 eigh_ysum_kernel(const double* __restrict__ rowpart, const double* __restrict__ colpart, int n, int k, int rg,
                  double* __restrict__ y) {
   const int base = k + 1, nt = n - base;
-  const int ii = blockIdx.x * 256 + threadIdx.x;
+  const int ii = blockIdx.x * 64 + threadIdx.x;
   if (ii >= nt) return;
   const int nch = (nt + EIGH_CW - 1) / EIGH_CW;
-  double acc = 0.0;
-  for (int c = ii / EIGH_CW; c < nch; ++c) acc += rowpart[(long long)c * n + base + ii];
-  for (int g = 0; g <= ii / rg; ++g) acc += colpart[(long long)g * n + base + ii];
+  double acc = eigh_strided_sum(rowpart + base + ii, n, ii / EIGH_CW, nch, 0.0);
+  acc = eigh_strided_sum(colpart + base + ii, n, 0, ii / rg + 1, acc);
   y[base + ii] = acc;
 }
 

@@ -210,6 +210,24 @@ __global__ void transpose_small_kernel(const double* __restrict__ Rm, int n, dou
     Rt[(long long)j * n + i] = Rm[idx];
   }
 }
+// NEXT-4 helpers: a column slice of a row-major matrix made contiguous, and the transposed row slice of R.
+//   dst[i][c] = src[i][c0 + c]   (rows x nc, src leading dimension ld)
+__global__ void slice_cols_kernel(const double* __restrict__ src, long long rows, int ld, int c0, int nc,
+                                  double* __restrict__ dst) {
+  const long long total = rows * nc;
+  for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
+       idx += (long long)gridDim.x * blockDim.x) {
+    const long long i = idx / nc; const int c = (int)(idx % nc);
+    dst[idx] = src[i * ld + c0 + c];
+  }
+}
+//   Rt[k][r] = Rm[r0 + r][k]     (n x nr)
+__global__ void transpose_rows_kernel(const double* __restrict__ Rm, int n, int r0, int nr, double* __restrict__ Rt) {
+  for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < n * nr; idx += gridDim.x * blockDim.x) {
+    const int k = idx / nr, r = idx % nr;
+    Rt[idx] = Rm[(long long)(r0 + r) * n + k];
+  }
+}
 // dot of two arrays with a fixed tree: partial per block, then final by block 0 of a 2nd launch
 __global__ void dot_partial_kernel(const double* __restrict__ x, const double* __restrict__ y, long long n,
                                    double* __restrict__ partial) {

@@ -704,7 +704,7 @@ long long eigh_top(cudaStream_t st, int n, int k, double* W, double* lam, double
     eigh_pass_kernel<<<dim3(nch, ng), 256, 0, st>>>(W, n, k2, rg, vprev, wk.w, vnew, wk.rowpart, wk.colpart);
     if (nt <= 2048) { rg_prev = rg; launches += 2; }       // launch-latency-bound tail: one kernel fewer per step
     else {
-      eigh_ysum_kernel<<<(nt + 255) / 256, 256, 0, st>>>(wk.rowpart, wk.colpart, n, k2, rg, wk.y);
+      eigh_ysum_kernel<<<(nt + 63) / 64, 64, 0, st>>>(wk.rowpart, wk.colpart, n, k2, rg, wk.y);
       rg_prev = 0; launches += 3;
     }
   }
@@ -820,9 +820,11 @@ int stage_absorb_layered(qrctm* h, const double* P, double* S) {
 }
 
 // K5: out[(m,r),n] = sum_{(J,d)} S''[(J,d),(m,r)] Qm[(J,d),n]
-int stage_project(qrctm* h, const double* S, const double* Qm, double* out, int chi_out = 0) {
+// chi_out: range of the index m of S'' (rows of out / D^2); ncols: columns of Qm (default: chi_out).
+int stage_project(qrctm* h, const double* S, const double* Qm, double* out, int chi_out = 0, int ncols = 0) {
   const int chi = chi_out > 0 ? chi_out : h->chi; const long long m = (long long)chi * h->b, mi = h->m;
-  GemmCall c{S, m, 1, Qm, chi, out, plain_map(chi), IndexMap{1, 1, 0}, (int)m, chi, (int)mi, 0};
+  const int nq = ncols > 0 ? ncols : chi;
+  GemmCall c{S, m, 1, Qm, nq, out, plain_map(nq), IndexMap{1, 1, 0}, (int)m, nq, (int)mi, 0};
   c.epi = 1;
   GEMM(h, c);
   return QRCTM_OK;
@@ -1587,6 +1589,76 @@ int qrctm_eigh_top_f64(void* cuda_stream, int n, int k, double* A, double* lam, 
   cudaError_t e;
   long long nl = eigh_top(static_cast<cudaStream_t>(cuda_stream), n, k, A, lam, U, work, &e);
   return nl < 0 ? QRCTM_ERR_CUDA : QRCTM_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------ NEXT-4: one iteration sharded over the column index m of Q
+namespace {
+
+void shard_range(int chi, int rank, int nranks, int* m0, int* m1) {      // contiguous, sizes differ by at most one
+  const int q = chi / nranks, r = chi % nranks;
+  *m0 = rank * q + (rank < r ? rank : r);
+  *m1 = *m0 + q + (rank < r ? 1 : 0);
+}
+
+}  // namespace
+
+extern "C" {
+
+int qrctm_shard_range(int chi, int rank, int nranks, int* m0, int* m1) {
+  if (chi < 1 || nranks < 1 || rank < 0 || rank >= nranks || !m0 || !m1) return QRCTM_ERR_INVALID_ARG;
+  shard_range(chi, rank, nranks, m0, m1);
+  return QRCTM_OK;
+}
+
+int qrctm_shard_front(qrctm_t* h, int rank, int nranks) {
+  if (!h) return QRCTM_ERR_INVALID_ARG;
+  if (!h->have_A || !h->have_env) return fail(h, QRCTM_ERR_NOT_READY, "set_A and set_env first");
+  if (nranks < 1 || rank < 0 || rank >= nranks) return fail(h, QRCTM_ERR_INVALID_ARG, "rank / nranks");
+  h->eig_rows = 0;
+  const int chi = h->chi, b = h->b; const long long m = h->m, bc = (long long)b * chi;
+  int m0, m1; shard_range(chi, rank, nranks, &m0, &m1);
+  const int co = m1 - m0;
+  // replicated: K1, K2 (0.3 % of the flops)
+  int rc = stage_reduced_corner(h, h->C, h->T, h->X); if (rc) return rc;
+  cudaError_t e;
+  long long nl = h->qr_path != 1 ? qr_factor_blocked(h->stream, h->qr_path, m, chi, h->X, h->Q, h->R, h->qrwork, &e)
+                                 : qr_factor_level2(h->stream, m, chi, h->X, h->Q, h->R, h->qrwork, &e);
+  if (nl < 0) return fail(h, QRCTM_ERR_CUDA, "qr", e);
+  h->launches += nl;
+  // the other ranks' rows of T' and the partial C' start from zero, so that either an all-gather of the slices or a
+  // plain sum over ranks assembles the full tensors
+  CU(h, cudaMemsetAsync(h->Tn, 0, sizeof(double) * m * chi, h->stream));
+  CU(h, cudaMemsetAsync(h->Cn, 0, sizeof(double) * chi * chi, h->stream));
+  if (co == 0) return QRCTM_OK;
+  // this rank's slice: K3, K4, K5 with the columns [m0, m1) of Q in place of Q on the open leg
+  slice_cols_kernel<<<296, 256, 0, h->stream>>>(h->Q, m, chi, m0, co, h->E);
+  transpose_rows_kernel<<<(chi * co + 255) / 256, 256, 0, h->stream>>>(h->R, chi, m0, co, h->Rt);
+  h->launches += 2;
+  CU(h, cudaGetLastError());
+  rc = stage_half_absorb(h, h->E, h->T, h->P, co); if (rc) return rc;
+  rc = stage_absorb_a(h, h->P, h->S, 0, nullptr, co); if (rc) return rc;
+  double* Tn_slice = h->Tn + (long long)m0 * bc;                       // rows (m, r), m in [m0, m1)
+  rc = stage_project(h, h->S, h->Q, Tn_slice, co, chi); if (rc) return rc;
+  // partial (E4): W[(mo,r),n] = sum_k R[m0+mo,k] Q[k,(r,n)];  C'_part[p,n] = sum_{(mo,r)} T'[(mo,r),p] W[(mo,r),n]
+  GemmCall c1{h->Q, bc, 1, h->Rt, co, h->W, IndexMap{1, 1, 0}, plain_map(bc), (int)bc, co, chi, 0};
+  GEMM(h, c1);
+  GemmCall c2{Tn_slice, chi, 1, h->W, chi, h->Cn, plain_map(chi), IndexMap{1, 1, 0}, chi, chi, co * b, 0};
+  GEMM(h, c2);
+  return QRCTM_OK;
+}
+
+int qrctm_shard_buffers(qrctm_t* h, double** Cn, double** Tn) {
+  if (!h || !Cn || !Tn) return QRCTM_ERR_INVALID_ARG;
+  *Cn = h->Cn; *Tn = h->Tn;
+  return QRCTM_OK;
+}
+
+int qrctm_shard_finish(qrctm_t* h) {
+  if (!h) return QRCTM_ERR_INVALID_ARG;
+  if (!h->have_A || !h->have_env) return fail(h, QRCTM_ERR_NOT_READY, "set_A and set_env first");
+  return stage_normalize(h, h->Cn, h->Tn);
 }
 
 }  // extern "C"
