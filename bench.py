@@ -313,13 +313,35 @@ def main():
             torch.cuda.synchronize()
             es_ms = ev0.elapsed_time(ev1)
             n_e = chi * b
-            tri_bytes = 16.0 * n_e ** 3 / 3.0          # one read + one write of the trailing block per reflector
+            tri_bytes = 8.0 * n_e ** 3 / 3.0           # upper triangle of the trailing block read + written once per reflector
             warm.update({"eig_step_ms": es_ms, "eig_step_n": n_e,
                          "eig_over_qr_step_time": es_ms / (ms_total / args.steps),
                          "tridiag_algorithmic_gbytes": tri_bytes / 1e9,
                          "eig_step_gbs_lower_bound": tri_bytes / (es_ms * 1e-3) / 1e9,
                          "note": "the whole eigen step (C~ build, tridiagonalisation, multisection, inverse iteration, "
                                  "back-transform, T' contraction) divided into the tridiagonalisation's bytes alone"})
+        h.set_env(C0, T0)
+        h.run(2, -1.0)
+
+    # ---- NEXT-4: per-rank compute of the sharded iteration, measured on this one GPU.  The
+    # exchange (all-gather of T' slices + all-reduce of C') needs more than one GPU and is NOT in these numbers.
+    shard = None
+    if rank == 0 and world == 1:
+        shard = {"what": "qrctm_shard_front(rank 0, nranks) on one GPU: K1+K2 replicated, K3-K6 on chi/nranks columns of Q; "
+                         "exchange not included", "front_ms": {}}
+        for nr in (1, 2, 4, 8):
+            if nr > chi:
+                continue
+            for _ in range(2):
+                h.shard_front(0, nr)
+            torch.cuda.synchronize()
+            ev0.record(h.stream)
+            for _ in range(3):
+                h.shard_front(0, nr)
+            ev1.record(h.stream)
+            torch.cuda.synchronize()
+            shard["front_ms"][str(nr)] = ev0.elapsed_time(ev1) / 3
+        shard["exchange_bytes_per_rank"] = {"all_gather_T": 8 * chi * b * chi, "all_reduce_C": 8 * chi * chi}
         h.set_env(C0, T0)
         h.run(2, -1.0)
 
@@ -393,6 +415,7 @@ def main():
             "hbm_kernels": hbm_kernels,
             "next_1_layered": layered,
             "next_2_warmup": warm,
+            "next_4_shard": shard,
             "step_tflops": sum(fl.values()) / (ms_per_step * 1e-3) / 1e12,
             "step_frac_of_fp64_peak": sum(fl.values()) / (ms_per_step * 1e-3) / 1e12 / peak_dmma,
         }
