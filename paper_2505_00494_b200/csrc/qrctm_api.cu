@@ -1478,7 +1478,7 @@ namespace {
 // K1, K3, K4 with C, T themselves give C~; its chi_new largest-|lambda| eigenpairs give U (for Q) and
 // C' = diag(lambda); T' = (E3) with U for Q  (Fig. 1(d)).
 int stage_eig_step(qrctm* h, int chi_new) {
-  const int ci = h->chi, b = h->b; const long long mi = h->m;
+  const long long mi = h->m;
   const size_t need = eigh_work_bytes_impl(mi, chi_new) + sizeof(double) * (size_t)chi_new + 256;
   if (h->eigwork_bytes < need) {
     CU(h, cudaStreamSynchronize(h->stream));
@@ -1513,7 +1513,6 @@ int stage_eig_step(qrctm* h, int chi_new) {
   CU(h, cudaGetLastError());
   h->eig_rows = (int)mi; h->eig_cols = chi_new;
   set_chi(h, chi_new);
-  (void)ci; (void)b;
   return stage_normalize(h, h->Cn, h->Tn);
 }
 

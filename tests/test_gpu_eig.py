@@ -281,3 +281,30 @@ def test_eig_step_argument_errors():
     h.set_env(C0, T0)                      # back to capacity
     assert h.chi == 8
     h.close()
+
+
+def test_observables_follow_the_current_chi():
+    """norm per site, corner spectrum and the bond energy right after the bulk initialisation (chi = D^2 < capacity)
+    and after the warm-up step, against the oracle on the same environments"""
+    d, D, chi, seed = 2, 2, 12, 6
+    A, _, _ = gen_config(d, D, chi, seed)
+    g = np.random.default_rng(3)
+    H = g.standard_normal((d * d, d * d)); H = H + H.T
+    a = o.build_a(A)
+    h = pkg.QRCTM(d, D, chi)
+    h.set_A(A)
+    h.init_bulk()
+    Co, To = o.normalize(*o.bulk_init(A))
+    assert abs(h.norm_per_site() / o.kappa(Co, To, a) - 1) < 1e-11
+    assert abs(h.energy_nn(H) - o.energy_nn(Co, To, A, H)) < 1e-11
+    it, dl = h.run(3, -1.0)                       # QR steps at chi = D^2
+    assert it == 3 and h.chi == D * D
+    C, T = Co, To
+    for _ in range(3):
+        q = o.qr_step(C, T, a)
+        C, T = o.normalize(q["Cn"], q["Tn"])
+    Cg, Tg = h.get_env()
+    cond = np.linalg.cond(o.reduced_corner(C, T))
+    assert rel(Cg, C) < 1e-12 * max(cond, 10) and rel(Tg, T) < 1e-12 * max(cond, 10)
+    assert np.max(np.abs(h.get_corner_spectrum() - o.spectrum(C))) < 1e-11
+    h.close()

@@ -50,6 +50,19 @@ def test_invalid_arguments_rejected(lib):
     t = ctypes.c_double()
     assert lib.qrctm_probe_fp64(7, 10, ctypes.byref(t)) == -1
     assert b"qrctm" in lib.qrctm_version()
+    # NEXT-2 / NEXT-4 entry points: argument checks need no device
+    assert lib.qrctm_eigh_work_bytes(0, 1) == 0 and lib.qrctm_eigh_work_bytes(8, 9) == 0
+    assert lib.qrctm_eigh_work_bytes(14001, 4) == 0 and lib.qrctm_eigh_work_bytes(9604, 196) > 8 * 4 * 9604 * 196
+    assert lib.qrctm_eigh_top_f64(None, 4, 2, None, None, None, None) == -1
+    for f in (lib.qrctm_init_bulk, lib.qrctm_shard_finish):
+        assert f(None) == -1
+    assert lib.qrctm_eig_step(None, 4) == -1 and lib.qrctm_warmup(None, 1) == -1
+    assert lib.qrctm_shard_front(None, 0, 1) == -1
+    m0, m1 = ctypes.c_int(), ctypes.c_int()
+    assert lib.qrctm_shard_range(8, 0, 0, ctypes.byref(m0), ctypes.byref(m1)) == -1
+    assert lib.qrctm_shard_range(8, 3, 3, ctypes.byref(m0), ctypes.byref(m1)) == -1
+    assert lib.qrctm_shard_range(8, 1, 3, ctypes.byref(m0), ctypes.byref(m1)) == 0 and (m0.value, m1.value) == (3, 6)
+    assert lib.qrctm_get_chi(None, None, None) == -1
 
 
 def test_no_cpu_fallback_without_gpu(lib):
