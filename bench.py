@@ -166,6 +166,8 @@ def main():
     ap.add_argument("--config", default="cfg4", choices=sorted(CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-next", action="store_true",
+                    help="skip the side measurements of the NEXT-1/2/4 variants (they are outside the timed region)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -264,7 +266,7 @@ def main():
 
     # ---- NEXT-1 variant: layered absorption, same result up to rounding, own flop count
     layered = None
-    if chi % 2 == 0:
+    if chi % 2 == 0 and not args.no_next:
         h.set_option(pkg.OPT_ABSORB_MODE, 1)
         h.set_env(C0, T0)
         h.run(args.warmup, -1.0)
@@ -295,7 +297,7 @@ def main():
     # ---- NEXT-2: the paper's warm-up -- bulk initialisation + one standard (eigen) step growing
     # chi from D^2 -- and one eigen step at the full chi, for the EIGH-vs-QR step-time ratio.
     warm = None
-    if b <= chi and chi * b <= 14000 and rank == 0:
+    if b <= chi and chi * b <= 14000 and rank == 0 and not args.no_next:
         h.warmup(1)
         torch.cuda.synchronize()
         ev0.record(h.stream)
@@ -326,7 +328,7 @@ def main():
     # ---- NEXT-4: per-rank compute of the sharded iteration, measured on this one GPU.  The
     # exchange (all-gather of T' slices + all-reduce of C') needs more than one GPU and is NOT in these numbers.
     shard = None
-    if rank == 0 and world == 1:
+    if rank == 0 and world == 1 and not args.no_next:
         shard = {"what": "qrctm_shard_front(rank 0, nranks) on one GPU: K1+K2 replicated, K3-K6 on chi/nranks columns of Q; "
                          "exchange not included", "front_ms": {}}
         for nr in (1, 2, 4, 8):
