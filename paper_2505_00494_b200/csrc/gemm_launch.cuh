@@ -1,0 +1,161 @@
+// Host side of the FP64 GEMM: tile-configuration choice, split-K cost model, launches (kernels: gemm_f64.cuh).
+// Part of the single translation unit qrctm_api.cu; included inside its anonymous namespace.
+#pragma once
+
+// ------------------------------------------------------------------ GEMM launcher
+template <int BM, int BN, int WM, int WN, int STAGES>
+cudaError_t launch_cfg(cudaStream_t st, const GemmArgs& g, int splits) {
+  constexpr int NT = (BM / WM) * (BN / WN) * 32;
+  constexpr size_t smem = sizeof(double) * STAGES * BK * ((BM + PAD) + (BN + PAD));
+  static bool attr_done = false;
+  if (!attr_done) {
+    cudaError_t e = cudaFuncSetAttribute(gemm_f64_dmma<BM, BN, WM, WN, STAGES>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    attr_done = true;
+  }
+  dim3 grid((g.N + BN - 1) / BN, (g.M + BM - 1) / BM, splits);
+  gemm_f64_dmma<BM, BN, WM, WN, STAGES><<<grid, NT, smem, st>>>(g);
+  return cudaGetLastError();
+}
+
+template <int BM, int BN, int WM, int WN, int STAGES>
+cudaError_t launch_cfg_ws(cudaStream_t st, const GemmArgs& g, int splits) {
+  constexpr int NT = ((BM / WM) * (BN / WN) + 1) * 32;
+  constexpr size_t smem = sizeof(double) * STAGES * BK * ((BM + PAD) + (BN + PAD)) + 2 * STAGES * sizeof(uint64_t) +
+                          sizeof(double) * (BM / WM) * (BN / WN) * 8 * (WN + 4);     // + per-warp epilogue slabs
+  static bool attr_done = false;
+  if (!attr_done) {
+    cudaError_t e = cudaFuncSetAttribute(gemm_f64_dmma_ws<BM, BN, WM, WN, STAGES>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    attr_done = true;
+  }
+  static int nslots = 0;
+  if (!nslots) {
+    int dev = 0, nsm = 148, per = 1;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, gemm_f64_dmma_ws<BM, BN, WM, WN, STAGES>, NT, smem);
+    nslots = nsm * (per > 0 ? per : 1);
+  }
+  GemmArgs ga = g;
+  ga.nz = splits;
+  const long long nwork = (long long)((g.N + BN - 1) / BN) * ((g.M + BM - 1) / BM) * splits;
+  (void)nslots;                                  // one work item per CTA: the hardware scheduler balances better
+  const unsigned grid = (unsigned)nwork;         // than a static persistent loop (measured)
+  gemm_f64_dmma_ws<BM, BN, WM, WN, STAGES><<<grid, NT, smem, st>>>(ga);
+  return cudaGetLastError();
+}
+
+struct GemmCall {
+  const double* A; long long lda; int transA;
+  const double* B; long long ldb;
+  double* out; IndexMap ro, co;
+  int M, N, K;
+  int mode;   // 0 store, 1 out -= , 2 out +=
+  IndexMap ka = IndexMap{1, 1, 0};     // k-row map of A (transA = 1)
+  int batch = 0;                       // > 0: gridDim.z batches, A += za(z), out += z * zo
+  IndexMap za = IndexMap{1, 0, 0};
+  long long zo = 0;
+  int epi = 0;                         // 1: shared-memory staged epilogue (outputs contiguous along the column index)
+};
+
+// Returns number of kernels launched (>0) or -1 on error (err set).
+int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws, size_t splitk_elems,
+                cudaError_t* err) {
+  *err = cudaSuccess;
+  if (c.M <= 0 || c.N <= 0) return 0;
+  GemmArgs g;
+  g.A = c.A; g.lda = c.lda; g.transA = c.transA; g.B = c.B; g.ldb = c.ldb; g.out = c.out;
+  g.ro = c.ro; g.co = c.co; g.M = c.M; g.N = c.N; g.K = c.K; g.mode = c.mode;
+  g.ka = c.ka; g.batch = c.batch > 0 ? 1 : 0; g.za = c.za; g.zo = c.zo; g.epi = c.epi;
+  g.vecA = c.transA && (c.lda % 2 == 0) && ((reinterpret_cast<uintptr_t>(c.A) & 15) == 0);
+  g.vecB = (c.ldb % 2 == 0) && ((reinterpret_cast<uintptr_t>(c.B) & 15) == 0);
+  g.split_stride = 0;
+  const int nkt = (c.K + BK - 1) / BK;
+  g.ktiles_per_split = nkt > 0 ? nkt : 1;
+  if (path == 1) {
+    long long n = (long long)c.M * c.N;
+    gemm_f64_ref<<<dim3((unsigned)((n + 255) / 256), 1, c.batch > 0 ? c.batch : 1), 256, 0, st>>>(g);
+    *err = cudaGetLastError();
+    return *err == cudaSuccess ? 1 : -1;
+  }
+  const long long t128 = (long long)((c.M + 127) / 128) * ((c.N + 127) / 128);
+  const long long t64 = (long long)((c.M + 63) / 64) * ((c.N + 63) / 64);
+  const bool big = t128 >= 120;
+  const bool ws_ok = g.transA && g.vecA && g.vecB;     // bulk copies need 16-byte aligned rows
+  int splits = 1;
+  int cfg = 0;          // 0: 64x64 cp.async, 1: 128x128 cp.async, 2: ws 128x128, 3: ws 128x104, 4: ws 128x64 (2 CTA/SM)
+  const bool ws_big = ws_ok && c.M >= 96 && c.N >= 32 && (double)c.M * c.N * c.K > 2.0e8;
+  if (c.batch > 0) {
+    // batched launch (layered absorption): bulk-copy kernel only, one batch per gridDim.z, no split-K
+    if (!ws_ok) { *err = cudaErrorInvalidValue; return -1; }
+    const int pad128 = (c.N + 127) / 128 * 128, pad104 = (c.N + 103) / 104 * 104, pad64 = (c.N + 63) / 64 * 64;
+    if (c.N <= 56) *err = launch_cfg_ws<128, 56, 32, 56, 3>(st, g, c.batch);
+    else if (pad64 <= pad104 && pad64 <= pad128) *err = launch_cfg_ws<128, 64, 64, 32, 4>(st, g, c.batch);
+    else if (pad104 <= pad128 && nkt <= 6) *err = launch_cfg_ws<64, 104, 16, 104, 3>(st, g, c.batch);   // 2 CTAs/SM
+    else if (pad104 <= pad128) *err = launch_cfg_ws<128, 104, 16, 104, 4>(st, g, c.batch);
+    else *err = launch_cfg_ws<128, 128, 64, 32, 4>(st, g, c.batch);
+    return *err == cudaSuccess ? 1 : -1;
+  }
+  if (ws_big) {
+    // pick the N tile with the least padding, then split K so that the CTAs fill whole waves
+    auto padded = [&](int bn) { return (long long)((c.N + bn - 1) / bn) * bn; };
+    int bn = 128; cfg = 2;
+    if (c.N <= 56) { bn = 56; cfg = 5; }                       // narrow N (layered absorption, N = D^2)
+    else if (c.N <= 64) { bn = 64; cfg = 4; }
+    else if (c.N >= 1024) { bn = 64; cfg = 4; }                // wide N: two CTAs per SM overlap epilogue and main loop
+                                                               // (K4 at cfg4: 13.10 ms vs 13.20 ms with 128x128, 13.20 with 128x56)
+    else if (padded(104) * 100 < padded(128) * 97) { bn = 104; cfg = 3; }
+    const long long tiles = (long long)((c.M + 127) / 128) * ((c.N + bn - 1) / bn);
+    const int slots = (cfg == 4 || cfg == 5) ? 296 : 148;
+    const double t_kt = 2.1e-6 * bn / 128.0 * ((cfg == 4 || cfg == 5) ? 2.0 : 1.0), t_fix = 4e-6;
+    double best = 1e30;
+    for (int sp = 1; sp <= 64; ++sp) {
+      int per = (nkt + sp - 1) / sp;
+      if (sp > 1 && per < 8) break;
+      int sp_eff = (nkt + per - 1) / per;
+      if (sp_eff != sp) continue;
+      if (sp > 1 && (size_t)c.M * c.N * sp > splitk_elems) break;
+      long long waves = (tiles * sp + slots - 1) / slots;
+      double t = waves * (per * t_kt + t_fix) + (sp > 1 ? 2.0 * sp * c.M * (double)c.N * 8.0 / 4e12 + 4e-6 : 0.0);
+      if (t < best * 0.97) { best = t; splits = sp; }
+    }
+  } else if (big) {
+    cfg = 1;
+  } else if (t64 < 148 && nkt >= 8) {
+    splits = (int)((2 * 148 + t64 - 1) / t64);
+    if (splits > nkt / 2) splits = nkt / 2;
+    size_t per = (size_t)c.M * c.N;
+    if (per * splits > splitk_elems) splits = (int)(splitk_elems / per);
+    if (splits < 1) splits = 1;
+  }
+  int launched = 0;
+  if (splits > 1) {
+    g.ktiles_per_split = (nkt + splits - 1) / splits;
+    splits = (nkt + g.ktiles_per_split - 1) / g.ktiles_per_split;
+    g.out = splitk_ws; g.ro = plain_map(c.N); g.co = IndexMap{1, 1, 0}; g.mode = 0;
+    g.split_stride = (long long)c.M * c.N;
+  }
+  switch (cfg) {
+    case 2: *err = launch_cfg_ws<128, 128, 64, 32, 4>(st, g, splits); break;
+    case 3: *err = launch_cfg_ws<128, 104, 16, 104, 4>(st, g, splits); break;
+    case 4: *err = launch_cfg_ws<128, 64, 64, 32, 4>(st, g, splits); break;
+    case 5: *err = launch_cfg_ws<128, 56, 32, 56, 3>(st, g, splits); break;
+    case 1: *err = launch_cfg<128, 128, 64, 32, 4>(st, g, splits); break;
+    default: *err = launch_cfg<64, 64, 32, 32, 4>(st, g, splits); break;
+  }
+  if (*err != cudaSuccess) return -1;
+  ++launched;
+  if (splits > 1) {
+    long long n = (long long)c.M * c.N;
+    reduce_splitk<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(splitk_ws, g.split_stride, splits, c.M, c.N,
+                                                              c.out, c.ro, c.co, c.mode);
+    *err = cudaGetLastError();
+    if (*err != cudaSuccess) return -1;
+    ++launched;
+  }
+  return launched;
+}
+
