@@ -308,3 +308,42 @@ def test_observables_follow_the_current_chi():
     assert rel(Cg, C) < 1e-12 * max(cond, 10) and rel(Tg, T) < 1e-12 * max(cond, 10)
     assert np.max(np.abs(h.get_corner_spectrum() - o.spectrum(C))) < 1e-11
     h.close()
+
+
+def test_ising_onsager_through_the_papers_flow():
+    """PAPER.md:28 + fn.[48]: bulk initialisation, two eigen steps growing chi 4 -> 16, then QR-CTMRG to convergence;
+    ln(kappa) of the Ising partition function against Onsager's closed form (structured A: the enlarged corner is
+    rank-deficient, so the kept eigenvectors of the zero cluster are arbitrary -- kappa is gauge-invariant)."""
+    from tests.brute import ising_A, onsager_ln_kappa
+    K = 0.3
+    h = pkg.QRCTM(2, 2, 16)
+    h.set_A(ising_A(K))
+    h.warmup(2)
+    assert h.chi == 16
+    it, dl = h.run(300, 1e-13)
+    assert abs(np.log(h.norm_per_site()) - onsager_ln_kappa(K)) < 1e-10
+    h.close()
+
+
+def test_eigen_branch_and_qr_branch_agree_at_convergence():
+    """PAPER.md:8 "without loss of accuracy": iterating the standard step and iterating the QR step from the same
+    start reach the same norm per site and corner spectrum (the GPU's own eigen branch, not the oracle's)."""
+    d, D, chi, seed = 2, 2, 8, 0
+    A, C0, T0 = gen_config(d, D, chi, seed)
+    h = pkg.QRCTM(d, D, chi)
+    h.set_A(A); h.set_env(C0, T0)
+    it, dl = h.run(500, 1e-12)
+    kq, sq = h.norm_per_site(), h.get_corner_spectrum()
+    h.set_env(C0, T0)
+    s_prev = None
+    for n_e in range(200):
+        h.eig_step()
+        s = np.sort(np.abs(np.diag(h.get_env()[0])))[::-1]        # C' = diag(lambda) / ||.||
+        if s_prev is not None and np.max(np.abs(s - s_prev)) < 1e-12:
+            break
+        s_prev = s
+    ke = h.norm_per_site()
+    h.close()
+    assert dl < 1e-12 and n_e < 199 and n_e < it
+    assert abs(kq / ke - 1) < 1e-10
+    assert np.max(np.abs(sq - s)) < 1e-9
