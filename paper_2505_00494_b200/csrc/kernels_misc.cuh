@@ -211,21 +211,22 @@ __global__ void transpose_small_kernel(const double* __restrict__ Rm, int n, dou
   }
 }
 // NEXT-4 helpers: a column slice of a row-major matrix made contiguous, and the transposed row slice of R.
-//   dst[i][c] = src[i][c0 + c]   (rows x nc, src leading dimension ld)
-__global__ void slice_cols_kernel(const double* __restrict__ src, long long rows, int ld, int c0, int nc,
+//   dst[i][c] = src[i][c0 + c] for c < nc, 0 for nc <= c < ldd   (rows x ldd, src leading dimension ld)
+__global__ void slice_cols_kernel(const double* __restrict__ src, long long rows, int ld, int c0, int nc, int ldd,
                                   double* __restrict__ dst) {
-  const long long total = rows * nc;
+  const long long total = rows * ldd;
   for (long long idx = blockIdx.x * (long long)blockDim.x + threadIdx.x; idx < total;
        idx += (long long)gridDim.x * blockDim.x) {
-    const long long i = idx / nc; const int c = (int)(idx % nc);
-    dst[idx] = src[i * ld + c0 + c];
+    const long long i = idx / ldd; const int c = (int)(idx % ldd);
+    dst[idx] = c < nc ? src[i * ld + c0 + c] : 0.0;
   }
 }
-//   Rt[k][r] = Rm[r0 + r][k]     (n x nr)
-__global__ void transpose_rows_kernel(const double* __restrict__ Rm, int n, int r0, int nr, double* __restrict__ Rt) {
-  for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < n * nr; idx += gridDim.x * blockDim.x) {
-    const int k = idx / nr, r = idx % nr;
-    Rt[idx] = Rm[(long long)(r0 + r) * n + k];
+//   Rt[k][r] = Rm[r0 + r][k] for r < nr, 0 for nr <= r < ldt     (n x ldt)
+__global__ void transpose_rows_kernel(const double* __restrict__ Rm, int n, int r0, int nr, int ldt,
+                                      double* __restrict__ Rt) {
+  for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < n * ldt; idx += gridDim.x * blockDim.x) {
+    const int k = idx / ldt, r = idx % ldt;
+    Rt[idx] = r < nr ? Rm[(long long)(r0 + r) * n + k] : 0.0;
   }
 }
 // dot of two arrays with a fixed tree: partial per block, then final by block 0 of a 2nd launch

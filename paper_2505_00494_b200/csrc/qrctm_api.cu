@@ -815,17 +815,19 @@ int qrctm_shard_front(qrctm_t* h, int rank, int nranks) {
   CU(h, cudaMemsetAsync(h->Tn, 0, sizeof(double) * m * chi, h->stream));
   CU(h, cudaMemsetAsync(h->Cn, 0, sizeof(double) * chi * chi, h->stream));
   if (co == 0) return QRCTM_OK;
-  // this rank's slice: K3, K4, K5 with the columns [m0, m1) of Q in place of Q on the open leg
-  slice_cols_kernel<<<296, 256, 0, h->stream>>>(h->Q, m, chi, m0, co, h->E);
-  transpose_rows_kernel<<<(chi * co + 255) / 256, 256, 0, h->stream>>>(h->R, chi, m0, co, h->Rt);
+  // this rank's slice: K3, K4, K5 with the columns [m0, m1) of Q in place of Q on the open leg.  An odd slice width is
+  // padded with one zero column (cop): rows of 16-byte-aligned length keep every GEMM on the bulk-copy kernel.
+  const int cop = (co & 1) && co < chi ? co + 1 : co;         // co == chi (one rank, odd chi): no room, no padding
+  slice_cols_kernel<<<296, 256, 0, h->stream>>>(h->Q, m, chi, m0, co, cop, h->E);
+  transpose_rows_kernel<<<(chi * cop + 255) / 256, 256, 0, h->stream>>>(h->R, chi, m0, co, cop, h->Rt);
   h->launches += 2;
   CU(h, cudaGetLastError());
-  rc = stage_half_absorb(h, h->E, h->T, h->P, co); if (rc) return rc;
-  rc = stage_absorb_a(h, h->P, h->S, 0, nullptr, co); if (rc) return rc;
+  rc = stage_half_absorb(h, h->E, h->T, h->P, cop); if (rc) return rc;
+  rc = stage_absorb_a(h, h->P, h->S, 0, nullptr, cop); if (rc) return rc;
   double* Tn_slice = h->Tn + (long long)m0 * bc;                       // rows (m, r), m in [m0, m1)
-  rc = stage_project(h, h->S, h->Q, Tn_slice, co, chi); if (rc) return rc;
+  rc = stage_project(h, h->S, h->Q, Tn_slice, cop, chi, co); if (rc) return rc;
   // partial (E4): W[(mo,r),n] = sum_k R[m0+mo,k] Q[k,(r,n)];  C'_part[p,n] = sum_{(mo,r)} T'[(mo,r),p] W[(mo,r),n]
-  GemmCall c1{h->Q, bc, 1, h->Rt, co, h->W, IndexMap{1, 1, 0}, plain_map(bc), (int)bc, co, chi, 0};
+  GemmCall c1{h->Q, bc, 1, h->Rt, cop, h->W, IndexMap{1, 1, 0}, plain_map(bc), (int)bc, cop, chi, 0};
   GEMM(h, c1);
   GemmCall c2{Tn_slice, chi, 1, h->W, chi, h->Cn, plain_map(chi), IndexMap{1, 1, 0}, chi, chi, co * b, 0};
   GEMM(h, c2);

@@ -84,10 +84,13 @@ int stage_absorb_layered(qrctm* h, const double* P, double* S) {
 
 // K5: out[(m,r),n] = sum_{(J,d)} S''[(J,d),(m,r)] Qm[(J,d),n]
 // chi_out: range of the index m of S'' (rows of out / D^2); ncols: columns of Qm (default: chi_out).
-int stage_project(qrctm* h, const double* S, const double* Qm, double* out, int chi_out = 0, int ncols = 0) {
+// chi_rows (<= chi_out): only the rows m < chi_rows of out are computed (a zero-padded slice, NEXT-4).
+int stage_project(qrctm* h, const double* S, const double* Qm, double* out, int chi_out = 0, int ncols = 0,
+                  int chi_rows = 0) {
   const int chi = chi_out > 0 ? chi_out : h->chi; const long long m = (long long)chi * h->b, mi = h->m;
   const int nq = ncols > 0 ? ncols : chi;
-  GemmCall c{S, m, 1, Qm, nq, out, plain_map(nq), IndexMap{1, 1, 0}, (int)m, nq, (int)mi, 0};
+  const long long mrows = chi_rows > 0 ? (long long)chi_rows * h->b : m;
+  GemmCall c{S, m, 1, Qm, nq, out, plain_map(nq), IndexMap{1, 1, 0}, (int)mrows, nq, (int)mi, 0};
   c.epi = 1;
   GEMM(h, c);
   return QRCTM_OK;
