@@ -23,6 +23,13 @@ namespace qk {
 
 constexpr int EIGH_CW = 256;      // columns per chunk of the tridiagonalisation sweep
 
+// First statement of the three tridiagonalisation kernels (launched with programmatic stream serialisation): let the
+// next kernel in the stream be set up now, then wait until the previous one has completed and flushed its writes.
+__device__ __forceinline__ void eigh_pdl_sync() {
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
 // sum_{t = t0}^{t1 - 1} part[t * stride], added in index order; loads issued eight at a time (the plain loop
 // would wait for every load before issuing the next)
 __device__ __forceinline__ double eigh_strided_sum(const double* __restrict__ part, long long stride, int t0, int t1,
@@ -54,6 +61,7 @@ eigh_reflector_kernel(double* __restrict__ W, int n, int k, const double* __rest
                       double* __restrict__ tauv, double* __restrict__ dvec, double* __restrict__ evec) {
   __shared__ double sh[33];
   __shared__ double s_vk, s_wk, s_alpha;
+  eigh_pdl_sync();
   const int tid = threadIdx.x;
   double* Wk = W + (long long)k * n;
   double vp[RMAX], x[RMAX];              // v_{k-1}[i];  w_{k-1}[i], then the updated row entry r[i]
@@ -143,6 +151,7 @@ eigh_pass_kernel(double* __restrict__ W, int n, int k, int rg, const double* __r
                  double* __restrict__ colpart) {
   constexpr int QW = EIGH_CW / 32, ROWS = 4;
   __shared__ double s_col[8][EIGH_CW];
+  eigh_pdl_sync();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const bool pending = k > 0;
   const int base = k + 1, nt = n - base;
@@ -212,6 +221,7 @@ eigh_pass_kernel(double* __restrict__ W, int n, int k, int rg, const double* __r
 __global__ void __launch_bounds__(64)
 eigh_ysum_kernel(const double* __restrict__ rowpart, const double* __restrict__ colpart, int n, int k, int rg,
                  double* __restrict__ y) {
+  eigh_pdl_sync();
   const int base = k + 1, nt = n - base;
   const int ii = blockIdx.x * 64 + threadIdx.x;
   if (ii >= nt) return;

@@ -39,6 +39,20 @@ unsigned long long eigh_work_bytes_impl(long long n, int k) {
   return eigh_layout(n, k, nullptr, nullptr);
 }
 
+// Launch with programmatic stream serialisation: the grid may be set up while its predecessor in the stream is still
+// draining; the three tridiagonalisation kernels start with griddepcontrol.wait, which holds them until the
+// predecessor has completed and its writes are visible (eigh.cuh, eigh_pdl_sync).
+template <class... KArgs, class... Args>
+void launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+
 // W (n x n symmetric, row-major, DEVICE, destroyed) -> lam[k] (largest |lambda| first), U (n x k, ld k).
 // Returns kernels launched or -1.
 long long eigh_top(cudaStream_t st, int n, int k, double* W, double* lam, double* U, void* work, cudaError_t* err) {
@@ -58,10 +72,10 @@ long long eigh_top(cudaStream_t st, int n, int k, double* W, double* lam, double
 #define REFL(k_, vprev_, vnew_)                                                                                  \
   do {                                                                                                           \
     const int left_ = n - (k_);                                                                                  \
-    if (left_ <= 2048) eigh_reflector_kernel<2><<<1, 1024, 0, st>>>(W, n, (k_), wk.y, wk.rowpart, wk.colpart, rg_prev, (vprev_), wk.w, (vnew_), wk.tau, wk.d, wk.e); \
-    else if (left_ <= 6144) eigh_reflector_kernel<6><<<1, 1024, 0, st>>>(W, n, (k_), wk.y, wk.rowpart, wk.colpart, rg_prev, (vprev_), wk.w, (vnew_), wk.tau, wk.d, wk.e); \
-    else if (left_ <= 10240) eigh_reflector_kernel<10><<<1, 1024, 0, st>>>(W, n, (k_), wk.y, wk.rowpart, wk.colpart, rg_prev, (vprev_), wk.w, (vnew_), wk.tau, wk.d, wk.e); \
-    else eigh_reflector_kernel<14><<<1, 1024, 0, st>>>(W, n, (k_), wk.y, wk.rowpart, wk.colpart, rg_prev, (vprev_), wk.w, (vnew_), wk.tau, wk.d, wk.e); \
+    if (left_ <= 2048) launch_pdl(eigh_reflector_kernel<2>, dim3(1), dim3(1024), 0, st, W, n, (k_), wk.y, wk.rowpart, wk.colpart, rg_prev, (vprev_), wk.w, (vnew_), wk.tau, wk.d, wk.e); \
+    else if (left_ <= 6144) launch_pdl(eigh_reflector_kernel<6>, dim3(1), dim3(1024), 0, st, W, n, (k_), wk.y, wk.rowpart, wk.colpart, rg_prev, (vprev_), wk.w, (vnew_), wk.tau, wk.d, wk.e); \
+    else if (left_ <= 10240) launch_pdl(eigh_reflector_kernel<10>, dim3(1), dim3(1024), 0, st, W, n, (k_), wk.y, wk.rowpart, wk.colpart, rg_prev, (vprev_), wk.w, (vnew_), wk.tau, wk.d, wk.e); \
+    else launch_pdl(eigh_reflector_kernel<14>, dim3(1), dim3(1024), 0, st, W, n, (k_), wk.y, wk.rowpart, wk.colpart, rg_prev, (vprev_), wk.w, (vnew_), wk.tau, wk.d, wk.e); \
   } while (0)
   int rg_prev = 0;                                 // > 0: the next reflector kernel sums the partials itself
   for (int k2 = 0; k2 + 2 < n; ++k2) {
@@ -76,10 +90,10 @@ long long eigh_top(cudaStream_t st, int n, int k, double* W, double* lam, double
     if (G < gmin) G = gmin;
     if (G < 1) G = 1;
     const int rg = (int)(32 * G), ng = (nt + rg - 1) / rg;
-    eigh_pass_kernel<<<dim3(nch, ng), 256, 0, st>>>(W, n, k2, rg, vprev, wk.w, vnew, wk.rowpart, wk.colpart);
+    launch_pdl(eigh_pass_kernel, dim3(nch, ng), dim3(256), 0, st, W, n, k2, rg, vprev, wk.w, vnew, wk.rowpart, wk.colpart);
     if (nt <= 2048) { rg_prev = rg; launches += 2; }       // launch-latency-bound tail: one kernel fewer per step
     else {
-      eigh_ysum_kernel<<<(nt + 63) / 64, 64, 0, st>>>(wk.rowpart, wk.colpart, n, k2, rg, wk.y);
+      launch_pdl(eigh_ysum_kernel, dim3((nt + 63) / 64), dim3(64), 0, st, wk.rowpart, wk.colpart, n, k2, rg, wk.y);
       rg_prev = 0; launches += 3;
     }
   }
