@@ -298,8 +298,8 @@ gemm_f64_dmma_ws(GemmArgs p) {
         int krows = p.K - kt * BK; if (krows > BK) krows = BK;
         const double* src = isB ? p.B + (long long)kr * p.ldb + n0 : Abase + p.ka(kr) * p.lda + m0;
         double* dst = (isB ? Bs + stage * B_STAGE : As + stage * A_STAGE) + srow;
-        if (row >= krows) {                         // ragged K: zero rows (last tile only)
-          const int wz = isB ? BN : BM;
+        if (row >= krows && row < ((krows + 3) & ~3)) {   // ragged K: zero the rows that complete the last k-step
+          const int wz = isB ? BN : BM;                   // (the consumers stop after ceil(krows / 4) k-steps)
           for (int c = 0; c < wz; ++c) dst[c] = 0.0;
         }
         __syncwarp();
@@ -321,6 +321,18 @@ gemm_f64_dmma_ws(GemmArgs p) {
     const int m0 = (rem / tn) * BM, n0 = (rem % tn) * BN;
     const int kt_begin = p.batch ? 0 : z * p.ktiles_per_split;
     int kt_end = kt_begin + p.ktiles_per_split; if (kt_end > nkt_total) kt_end = nkt_total;
+
+    // Direct epilogue: the output offsets of the tile's BM rows and BN columns (-1 = out of range) are worked out
+    // once per tile by all consumer threads together, while the first operand tiles are still in flight, instead
+    // of 16 index-map evaluations (32 integer divisions) per thread after the main loop.
+    long long* otab = reinterpret_cast<long long*>(empty + STAGES);
+    if (p.epi == 0) {
+      asm volatile("bar.sync 1, %0;\n" ::"n"(NCW * 32) : "memory");       // previous tile's epilogue has read the table
+      for (int t = tid; t < BM + BN; t += NCW * 32) {
+        const int g = t < BM ? m0 + t : n0 + t - BM;
+        otab[t] = t < BM ? (g < p.M ? p.ro(g) : -1) : (g < p.N ? p.co(g) : -1);
+      }
+    }
 
     double acc[FM][FN][2];
 #pragma unroll
@@ -405,30 +417,37 @@ gemm_f64_dmma_ws(GemmArgs p) {
         __syncwarp();
       }
     } else {
+      asm volatile("bar.sync 1, %0;\n" ::"n"(NCW * 32) : "memory");       // offset table complete
       long long coff[FN][2];
 #pragma unroll
-      for (int j = 0; j < FN; ++j)
+      for (int j = 0; j < FN; ++j) {
+        const longlong2 c2 = *reinterpret_cast<const longlong2*>(otab + BM + wn0 + j * 8 + 2 * lc);
+        coff[j][0] = c2.x; coff[j][1] = c2.y;
+      }
+      if (p.mode == 0) {
 #pragma unroll
-        for (int e = 0; e < 2; ++e) {
-          const int c = n0 + wn0 + j * 8 + 2 * lc + e;
-          coff[j][e] = c < p.N ? p.co(c) : -1;
+        for (int i = 0; i < FM; ++i) {
+          const long long roff = otab[wm0 + i * 8 + lr];
+          if (roff < 0) continue;
+          double* orow = out + roff;
+#pragma unroll
+          for (int j = 0; j < FN; ++j) {
+            if (coff[j][0] >= 0) orow[coff[j][0]] = acc[i][j][0];
+            if (coff[j][1] >= 0) orow[coff[j][1]] = acc[i][j][1];
+          }
         }
+      } else {
+        const double sgn = p.mode == 1 ? -1.0 : 1.0;
 #pragma unroll
-      for (int i = 0; i < FM; ++i) {
-        const int r = m0 + wm0 + i * 8 + lr;
-        if (r >= p.M) continue;
-        const long long roff = p.ro(r);
+        for (int i = 0; i < FM; ++i) {
+          const long long roff = otab[wm0 + i * 8 + lr];
+          if (roff < 0) continue;
+          double* orow = out + roff;
 #pragma unroll
-        for (int j = 0; j < FN; ++j) {
+          for (int j = 0; j < FN; ++j) {
 #pragma unroll
-          for (int e = 0; e < 2; ++e) {
-            if (coff[j][e] >= 0) {
-              const long long off = roff + coff[j][e];
-              double v = acc[i][j][e];
-              if (p.mode == 1) v = out[off] - v;
-              else if (p.mode == 2) v = out[off] + v;
-              out[off] = v;
-            }
+            for (int e = 0; e < 2; ++e)
+              if (coff[j][e] >= 0) orow[coff[j][e]] = fma(sgn, acc[i][j][e], orow[coff[j][e]]);
           }
         }
       }

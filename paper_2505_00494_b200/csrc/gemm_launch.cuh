@@ -43,7 +43,8 @@ cudaError_t launch_cfg_ws(cudaStream_t st, const GemmArgs& g, int splits) {
   ga.nz = splits;
   const long long nwork = (long long)((g.N + BN - 1) / BN) * ((g.M + BM - 1) / BM) * splits;
   (void)nslots;                                  // one work item per CTA: the hardware scheduler balances better
-  const unsigned grid = (unsigned)nwork;         // than a static persistent loop (measured)
+  const unsigned grid = (unsigned)nwork;         // than a static persistent loop, with or without a start-up stagger
+                                                 // between the two CTAs of an SM (measured, profiles/r1_gemm_experiments.md)
   gemm_f64_dmma_ws<BM, BN, WM, WN, STAGES><<<grid, NT, smem, st>>>(ga);
   return cudaGetLastError();
 }
