@@ -183,6 +183,13 @@ int qrctm_get_stage_ms(qrctm_t* h, double* ms /* QRCTM_NSTAGE + 1 */, long long*
 int qrctm_gemm_f64(void* cuda_stream, int path, int transA, int M, int N, int K,
                    const double* A, long long lda, const double* B, long long ldb,
                    double* Cmat, long long ldc);
+/* The same with a scratch buffer: work (DEVICE, work_bytes bytes, 16-byte aligned, may be NULL / 0) lets the
+ * launcher use its K-splitting schedules - split-K with a fixed-order reduction, and stream-K for GEMMs whose tiles
+ * fill only a few ragged waves - exactly as the stages of qrctm_step do with the handle's
+ * workspace.  The result does not depend on the schedule beyond the summation order (<= 1e-13 relative). */
+int qrctm_gemm_f64_ws(void* cuda_stream, int path, int transA, int M, int N, int K,
+                      const double* A, long long lda, const double* B, long long ldb,
+                      double* Cmat, long long ldc, void* work, unsigned long long work_bytes);
 
 /* Stand-alone QR entry (K2): factor X[rows][cols] (DEVICE, row-major, cols <=
  * rows) into Q[rows][cols], R[cols][cols] with diag(R) >= 0 (path: see

@@ -31,7 +31,7 @@ SYMBOLS = (
     "qrctm_set_A", "qrctm_set_env", "qrctm_step", "qrctm_run", "qrctm_get_env",
     "qrctm_get_corner_spectrum", "qrctm_get_qr", "qrctm_get_raw", "qrctm_get_a", "qrctm_norm_per_site",
     "qrctm_r_diag_ratio", "qrctm_energy_nn", "qrctm_set_option", "qrctm_launch_count", "qrctm_get_stage_ms", "qrctm_profile_step",
-    "qrctm_gemm_f64", "qrctm_qr_work_bytes", "qrctm_qr_f64", "qrctm_probe_fp64", "qrctm_last_error",
+    "qrctm_gemm_f64", "qrctm_gemm_f64_ws", "qrctm_qr_work_bytes", "qrctm_qr_f64", "qrctm_probe_fp64", "qrctm_last_error",
     "qrctm_version",
     "qrctm_get_chi", "qrctm_init_bulk", "qrctm_eig_step", "qrctm_get_eig", "qrctm_warmup",
     "qrctm_eigh_work_bytes", "qrctm_eigh_top_f64",
@@ -81,6 +81,8 @@ def load_library() -> ctypes.CDLL:
     lib.qrctm_get_stage_ms.argtypes = [P, POINTER(c_double), POINTER(c_longlong), c_int]
     lib.qrctm_gemm_f64.argtypes = [P, c_int, c_int, c_int, c_int, c_int, P, c_longlong, P, c_longlong, P,
                                    c_longlong]
+    lib.qrctm_gemm_f64_ws.argtypes = [P, c_int, c_int, c_int, c_int, c_int, P, c_longlong, P, c_longlong, P,
+                                      c_longlong, P, c_ulonglong]
     lib.qrctm_qr_work_bytes.argtypes = [c_int, c_int]
     lib.qrctm_qr_work_bytes.restype = c_ulonglong
     lib.qrctm_qr_f64.argtypes = [P, c_int, c_int, c_int, P, P, P, P]
@@ -330,8 +332,9 @@ class QRCTM:
 
 
 # -- stand-alone entries (device tensors in, device tensors out)
-def gemm_f64(A, B, transA: bool = False, path: int = 0):
-    """out[M,N] = op(A) @ B on the GPU through qrctm_gemm_f64 (torch CUDA float64 tensors)."""
+def gemm_f64(A, B, transA: bool = False, path: int = 0, work_bytes: int = 0):
+    """out[M,N] = op(A) @ B on the GPU through qrctm_gemm_f64 (torch CUDA float64 tensors);
+    work_bytes > 0: through qrctm_gemm_f64_ws with a scratch buffer of that size (split-K / stream-K schedules)."""
     import torch
     lib = load_library()
     K, N = B.shape
@@ -341,9 +344,15 @@ def gemm_f64(A, B, transA: bool = False, path: int = 0):
         if t.dtype != torch.float64 or not t.is_cuda or t.stride(1) != 1:
             raise QrctmError("gemm_f64 wants CUDA float64 matrices with unit column stride")
     out = torch.empty((M, N), dtype=torch.float64, device="cuda")
-    rc = lib.qrctm_gemm_f64(c_void_p(torch.cuda.current_stream().cuda_stream), path, int(transA), M, N, K,
-                            c_void_p(A.data_ptr()), A.stride(0), c_void_p(B.data_ptr()), B.stride(0),
-                            _ptr(out), N)
+    if work_bytes > 0:
+        work = torch.empty(work_bytes, dtype=torch.uint8, device="cuda")
+        rc = lib.qrctm_gemm_f64_ws(c_void_p(torch.cuda.current_stream().cuda_stream), path, int(transA), M, N, K,
+                                   c_void_p(A.data_ptr()), A.stride(0), c_void_p(B.data_ptr()), B.stride(0),
+                                   _ptr(out), N, c_void_p(work.data_ptr()), work_bytes)
+    else:
+        rc = lib.qrctm_gemm_f64(c_void_p(torch.cuda.current_stream().cuda_stream), path, int(transA), M, N, K,
+                                c_void_p(A.data_ptr()), A.stride(0), c_void_p(B.data_ptr()), B.stride(0),
+                                _ptr(out), N)
     if rc != QRCTM_OK:
         raise QrctmError(f"qrctm_gemm_f64 failed: {rc}")
     return out

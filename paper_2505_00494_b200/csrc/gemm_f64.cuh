@@ -52,7 +52,16 @@ struct GemmArgs {
   int nz = 1;                // number of z slices (splits or batches) -- work list of the ws kernel
   int epi = 0;               // ws kernel epilogue: 0 = fragments straight to global, 1 = staged through shared
                              // memory so that the 32 lanes of a store run along the column index j
+  // stream-K (ws kernel, nz = 1, no batch): the tiles x k-tiles units are dealt out evenly and contiguously to the
+  // gridDim.x CTAs; a CTA that covers only part of a tile's k range writes a plain BM x BN partial tile to slot
+  // 2 * blockIdx.x (its first segment) or 2 * blockIdx.x + 1 (its last) of sk_ws, and streamk_fixup sums the
+  // partial tiles of every split tile in ascending k (fixed order).
+  int sk = 0;
+  double* sk_ws = nullptr;
 };
+
+// first unit of CTA c when `units` units are dealt to `ncta` CTAs
+__host__ __device__ inline long long sk_first_unit(long long c, long long units, long long ncta) { return c * units / ncta; }
 
 constexpr int BK = 16;
 constexpr int PAD = 4;
@@ -247,7 +256,7 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-template <int BM, int BN, int WM, int WN, int STAGES>
+template <int BM, int BN, int WM, int WN, int STAGES, bool SK = false>
 __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 1) * 32, ((BM / WM) * (BN / WN) <= 4 ? 2 : 1))
 gemm_f64_dmma_ws(GemmArgs p) {
   constexpr int NW_M = BM / WM, NW_N = BN / WN, NCW = NW_M * NW_N;
@@ -268,6 +277,8 @@ gemm_f64_dmma_ws(GemmArgs p) {
   const int tn = (p.N + BN - 1) / BN, tm = (p.M + BM - 1) / BM;
   const long long nwork = (long long)tn * tm * p.nz;
   const int nkt_total = (p.K + BK - 1) / BK;
+  const long long w_begin = SK ? sk_first_unit(blockIdx.x, (long long)tn * tm * nkt_total, gridDim.x) : blockIdx.x;
+  const long long w_end = SK ? sk_first_unit(blockIdx.x + 1, (long long)tn * tm * nkt_total, gridDim.x) : nwork;
 
   if (tid == 0) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, NCW); }
@@ -281,12 +292,20 @@ gemm_f64_dmma_ws(GemmArgs p) {
     const bool isB = lane >= 16;
     const int srow = isB ? row * LDB_S : row * LDA_S;
     int it = 0;                                   // k-tiles issued so far by this CTA (ring position)
-    for (long long w = blockIdx.x; w < nwork; w += gridDim.x) {
-      const int z = (int)(w / ((long long)tn * tm));
-      const int rem = (int)(w % ((long long)tn * tm));
+    for (long long w = w_begin; w < w_end;) {
+      int z, rem, kt_begin, kt_end;
+      if (SK) {
+        z = 0; rem = (int)(w / nkt_total); kt_begin = (int)(w % nkt_total);
+        const long long left = w_end - w;
+        kt_end = left < nkt_total - kt_begin ? kt_begin + (int)left : nkt_total;
+        w += kt_end - kt_begin;
+      } else {
+        z = (int)(w / ((long long)tn * tm)); rem = (int)(w % ((long long)tn * tm));
+        kt_begin = p.batch ? 0 : z * p.ktiles_per_split;
+        kt_end = kt_begin + p.ktiles_per_split; if (kt_end > nkt_total) kt_end = nkt_total;
+        w += gridDim.x;
+      }
       const int m0 = (rem / tn) * BM, n0 = (rem % tn) * BN;
-      const int kt_begin = p.batch ? 0 : z * p.ktiles_per_split;
-      int kt_end = kt_begin + p.ktiles_per_split; if (kt_end > nkt_total) kt_end = nkt_total;
       const double* Abase = p.A + (p.batch ? p.za(z) : 0);
       int wA = p.M - m0; if (wA > BM) wA = BM; wA = (wA + 1) & ~1;
       int wB = p.N - n0; if (wB > BN) wB = BN; wB = (wB + 1) & ~1;
@@ -315,18 +334,30 @@ gemm_f64_dmma_ws(GemmArgs p) {
   const int wm0 = (warp / NW_N) * WM, wn0 = (warp % NW_N) * WN;
   const int lr = lane >> 2, lc = lane & 3;
   int it = 0;
-  for (long long w = blockIdx.x; w < nwork; w += gridDim.x) {
-    const int z = (int)(w / ((long long)tn * tm));
-    const int rem = (int)(w % ((long long)tn * tm));
+  for (long long w = w_begin; w < w_end;) {
+    int z, rem, kt_begin, kt_end;
+    bool partial = false;
+    int slot = 0;
+    if (SK) {
+      z = 0; rem = (int)(w / nkt_total); kt_begin = (int)(w % nkt_total);
+      const long long left = w_end - w;
+      kt_end = left < nkt_total - kt_begin ? kt_begin + (int)left : nkt_total;
+      partial = kt_begin != 0 || kt_end != nkt_total;
+      slot = 2 * blockIdx.x + (w == w_begin ? 0 : 1);
+      w += kt_end - kt_begin;
+    } else {
+      z = (int)(w / ((long long)tn * tm)); rem = (int)(w % ((long long)tn * tm));
+      kt_begin = p.batch ? 0 : z * p.ktiles_per_split;
+      kt_end = kt_begin + p.ktiles_per_split; if (kt_end > nkt_total) kt_end = nkt_total;
+      w += gridDim.x;
+    }
     const int m0 = (rem / tn) * BM, n0 = (rem % tn) * BN;
-    const int kt_begin = p.batch ? 0 : z * p.ktiles_per_split;
-    int kt_end = kt_begin + p.ktiles_per_split; if (kt_end > nkt_total) kt_end = nkt_total;
 
     // Direct epilogue: the output offsets of the tile's BM rows and BN columns (-1 = out of range) are worked out
     // once per tile by all consumer threads together, while the first operand tiles are still in flight, instead
     // of 16 index-map evaluations (32 integer divisions) per thread after the main loop.
     long long* otab = reinterpret_cast<long long*>(empty + STAGES);
-    if (p.epi == 0) {
+    if (p.epi == 0 && !(SK && partial)) {
       asm volatile("bar.sync 1, %0;\n" ::"n"(NCW * 32) : "memory");       // previous tile's epilogue has read the table
       for (int t = tid; t < BM + BN; t += NCW * 32) {
         const int g = t < BM ? m0 + t : n0 + t - BM;
@@ -378,7 +409,15 @@ gemm_f64_dmma_ws(GemmArgs p) {
     }
 
     double* out = p.out + (p.batch ? (long long)z * p.zo : (long long)z * p.split_stride);
-    if (p.epi == 1) {
+    if (SK && partial) {
+      // stream-K partial tile: plain BM x BN slab, no maps, no bounds (the fix-up reads the valid part only)
+      double* slab = p.sk_ws + (long long)slot * (BM * BN) + (wm0 + lr) * BN + wn0 + 2 * lc;
+#pragma unroll
+      for (int i = 0; i < FM; ++i)
+#pragma unroll
+        for (int j = 0; j < FN; ++j)
+          *reinterpret_cast<double2*>(slab + i * 8 * BN + j * 8) = make_double2(acc[i][j][0], acc[i][j][1]);
+    } else if (p.epi == 1) {
       // staged: 8 rows x WN columns of this warp go through its private shared-memory slab, then every
       // store instruction writes 32 consecutive columns of one row (coalesced wherever co() is contiguous)
       constexpr int SP = WN + 4, NCH = (WN + 31) / 32;
@@ -494,6 +533,59 @@ __global__ void reduce_splitk(const double* part, long long split_stride, int sp
   if (mode == 1) s = out[off] - s;
   else if (mode == 2) s = out[off] + s;
   out[off] = s;
+}
+
+// Stream-K fix-up: gridDim.x = output tiles, gridDim.y = row slices of a tile.  The CTAs that hold a part of tile t's
+// k range are found from the same arithmetic the GEMM used (thread 0, once per CTA); if one of them covered the whole
+// range the tile was stored directly and nothing is done.
+// out[ro(i)+co(j)] (op)= sum of the partial tiles in ascending k (= ascending CTA index: fixed order).
+constexpr int SK_MAXSEG = 320;
+__global__ void __launch_bounds__(256)
+streamk_fixup(const double* __restrict__ ws, int BM, int BN, int tn, int nkt, long long units, int ncta, int M, int N,
+              double* out, IndexMap ro, IndexMap co, int mode) {
+  __shared__ int slots[SK_MAXSEG];
+  __shared__ int nseg_s;
+  const int t = blockIdx.x;
+  if (threadIdx.x == 0) {
+    const long long ub = (long long)t * nkt, ue = ub + nkt;
+    long long c = ub * ncta / units;
+    while (c + 1 < ncta && sk_first_unit(c + 1, units, ncta) <= ub) ++c;
+    while (c > 0 && sk_first_unit(c, units, ncta) > ub) --c;
+    int nseg = 0;
+    for (; c < ncta && nseg < SK_MAXSEG; ++c) {
+      const long long u0 = sk_first_unit(c, units, ncta), u1 = sk_first_unit(c + 1, units, ncta);
+      if (u0 >= ue) break;
+      if (u0 <= ub && u1 >= ue) { nseg = 0; break; }         // whole tile by one CTA: stored directly
+      if (u1 > u0) slots[nseg++] = (int)(2 * c + (u0 >= ub ? 0 : 1));   // first segment of CTA c, else its last
+    }
+    nseg_s = nseg;
+  }
+  __syncthreads();
+  const int nseg = nseg_s;
+  if (nseg == 0) return;
+  const int m0 = (t / tn) * BM, n0 = (t % tn) * BN;
+  const int hrows = M - m0 < BM ? M - m0 : BM, wcols = N - n0 < BN ? N - n0 : BN;
+  const long long tile = (long long)BM * BN;
+  const int rows_per = (hrows + gridDim.y - 1) / gridDim.y;
+  const int i0 = blockIdx.y * rows_per, i1 = i0 + rows_per < hrows ? i0 + rows_per : hrows;
+  for (int i = i0 + threadIdx.x / 32; i < i1; i += blockDim.x / 32) {
+    const long long roff = ro(m0 + i);
+    for (int j = threadIdx.x % 32; j < wcols; j += 32) {
+      const double* src = ws + (long long)i * BN + j;
+      double s = 0.0;
+      int q = 0;
+      for (; q + 4 <= nseg; q += 4) {
+        const double v0 = src[slots[q] * tile], v1 = src[slots[q + 1] * tile], v2 = src[slots[q + 2] * tile],
+                     v3 = src[slots[q + 3] * tile];
+        s += v0; s += v1; s += v2; s += v3;
+      }
+      for (; q < nseg; ++q) s += src[slots[q] * tile];
+      const long long off = roff + co(n0 + j);
+      if (mode == 1) s = out[off] - s;
+      else if (mode == 2) s = out[off] + s;
+      out[off] = s;
+    }
+  }
 }
 
 }  // namespace qk

@@ -19,8 +19,11 @@ cudaError_t launch_cfg(cudaStream_t st, const GemmArgs& g, int splits) {
   return cudaGetLastError();
 }
 
+// stream-K request: workspace for the partial tiles; `used` is set when the launch went that way (else plain tiles)
+struct StreamK { double* ws; size_t ws_elems; bool used; };
+
 template <int BM, int BN, int WM, int WN, int STAGES>
-cudaError_t launch_cfg_ws(cudaStream_t st, const GemmArgs& g, int splits) {
+cudaError_t launch_cfg_ws(cudaStream_t st, const GemmArgs& g, int splits, StreamK* sk = nullptr) {
   constexpr int NT = ((BM / WM) * (BN / WN) + 1) * 32;
   constexpr size_t smem = sizeof(double) * STAGES * BK * ((BM + PAD) + (BN + PAD)) + 2 * STAGES * sizeof(uint64_t) +
                           sizeof(double) * (BM / WM) * (BN / WN) * 8 * (WN + 4);     // + per-warp epilogue slabs
@@ -42,6 +45,27 @@ cudaError_t launch_cfg_ws(cudaStream_t st, const GemmArgs& g, int splits) {
   GemmArgs ga = g;
   ga.nz = splits;
   const long long nwork = (long long)((g.N + BN - 1) / BN) * ((g.M + BM - 1) / BM) * splits;
+  if (sk) {
+    // stream-K: one CTA per slot, every CTA the same number (+-1) of k-tiles; then the fix-up of the split tiles
+    const int tn = (g.N + BN - 1) / BN, nkt = (g.K + BK - 1) / BK;
+    const long long units = nwork * nkt;
+    const long long ncta = units < nslots ? units : nslots;
+    sk->used = splits == 1 && !g.batch && (size_t)2 * ncta * BM * BN <= sk->ws_elems;
+    if (sk->used) {
+      static bool sk_attr = false;
+      if (!sk_attr) {
+        cudaError_t e = cudaFuncSetAttribute(gemm_f64_dmma_ws<BM, BN, WM, WN, STAGES, true>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        sk_attr = true;
+      }
+      ga.sk = 1; ga.sk_ws = sk->ws;
+      gemm_f64_dmma_ws<BM, BN, WM, WN, STAGES, true><<<(unsigned)ncta, NT, smem, st>>>(ga);
+      streamk_fixup<<<dim3((unsigned)nwork, 8), 256, 0, st>>>(sk->ws, BM, BN, tn, nkt, units, (int)ncta, g.M, g.N, g.out, g.ro,
+                                                    g.co, g.mode);
+      return cudaGetLastError();
+    }
+  }
   (void)nslots;                                  // one work item per CTA: the hardware scheduler balances better
   const unsigned grid = (unsigned)nwork;         // than a static persistent loop, with or without a start-up stagger
                                                  // between the two CTAs of an SM (measured, profiles/r1_gemm_experiments.md)
@@ -87,6 +111,7 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
   const bool big = t128 >= 120;
   const bool ws_ok = g.transA && g.vecA && g.vecB;     // bulk copies need 16-byte aligned rows
   int splits = 1;
+  bool use_sk = false;
   int cfg = 0;          // 0: 64x64 cp.async, 1: 128x128 cp.async, 2: ws 128x128, 3: ws 128x104, 4: ws 128x64 (2 CTA/SM)
   const bool ws_big = ws_ok && c.M >= 96 && c.N >= 32 && (double)c.M * c.N * c.K > 2.0e8;
   if (c.batch > 0) {
@@ -123,6 +148,13 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
       double t = waves * (per * t_kt + t_fix) + (sp > 1 ? 2.0 * sp * c.M * (double)c.N * 8.0 / 4e12 + 4e-6 : 0.0);
       if (t < best * 0.97) { best = t; splits = sp; }
     }
+    // stream-K instead when the tiles fill only a few ragged waves: every CTA gets the same share of k-tiles
+    const double units = (double)tiles * nkt;
+    if (tiles < 6LL * slots && units >= 24.0 * slots && (size_t)2 * slots * 128 * bn <= splitk_elems) {
+      // up to two partial tiles per CTA written and read again, one more launch
+      const double t_sk = ceil(units / slots) * t_kt + 2 * t_fix + 2.0 * (2.0 * slots * 128.0 * bn * 8.0) / 3e12 + 5e-6;
+      if (t_sk < best * 0.97) { use_sk = true; splits = 1; }
+    }
   } else if (big) {
     cfg = 1;
   } else if (t64 < 148 && nkt >= 8) {
@@ -139,16 +171,19 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
     g.out = splitk_ws; g.ro = plain_map(c.N); g.co = IndexMap{1, 1, 0}; g.mode = 0;
     g.split_stride = (long long)c.M * c.N;
   }
+  StreamK skreq{splitk_ws, splitk_elems, false};
+  StreamK* sk = use_sk ? &skreq : nullptr;
   switch (cfg) {
-    case 2: *err = launch_cfg_ws<128, 128, 64, 32, 4>(st, g, splits); break;
-    case 3: *err = launch_cfg_ws<128, 104, 16, 104, 4>(st, g, splits); break;
-    case 4: *err = launch_cfg_ws<128, 64, 64, 32, 4>(st, g, splits); break;
-    case 5: *err = launch_cfg_ws<128, 56, 32, 56, 3>(st, g, splits); break;
+    case 2: *err = launch_cfg_ws<128, 128, 64, 32, 4>(st, g, splits, sk); break;
+    case 3: *err = launch_cfg_ws<128, 104, 16, 104, 4>(st, g, splits, sk); break;
+    case 4: *err = launch_cfg_ws<128, 64, 64, 32, 4>(st, g, splits, sk); break;
+    case 5: *err = launch_cfg_ws<128, 56, 32, 56, 3>(st, g, splits, sk); break;
     case 1: *err = launch_cfg<128, 128, 64, 32, 4>(st, g, splits); break;
     default: *err = launch_cfg<64, 64, 32, 32, 4>(st, g, splits); break;
   }
   if (*err != cudaSuccess) return -1;
   ++launched;
+  if (skreq.used) ++launched;
   if (splits > 1) {
     long long n = (long long)c.M * c.N;
     reduce_splitk<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(splitk_ws, g.split_stride, splits, c.M, c.N,

@@ -618,6 +618,18 @@ int qrctm_gemm_f64(void* cuda_stream, int path, int transA, int M, int N, int K,
   return nl < 0 ? QRCTM_ERR_CUDA : QRCTM_OK;
 }
 
+int qrctm_gemm_f64_ws(void* cuda_stream, int path, int transA, int M, int N, int K, const double* A, long long lda,
+                      const double* B, long long ldb, double* Cmat, long long ldc, void* work,
+                      unsigned long long work_bytes) {
+  if (!A || !B || !Cmat || M < 0 || N < 0 || K < 0 || (path != 0 && path != 1)) return QRCTM_ERR_INVALID_ARG;
+  if ((work == nullptr && work_bytes != 0) || (reinterpret_cast<uintptr_t>(work) & 15)) return QRCTM_ERR_INVALID_ARG;
+  GemmCall c{A, lda, transA ? 1 : 0, B, ldb, Cmat, plain_map(ldc), IndexMap{1, 1, 0}, M, N, K, 0};
+  cudaError_t e;
+  int nl = launch_gemm(static_cast<cudaStream_t>(cuda_stream), path, c, static_cast<double*>(work),
+                       (size_t)(work_bytes / sizeof(double)), &e);
+  return nl < 0 ? QRCTM_ERR_CUDA : QRCTM_OK;
+}
+
 unsigned long long qrctm_qr_work_bytes(int rows, int cols) { return qr_work_bytes_impl(rows, cols); }
 
 int qrctm_qr_f64(void* cuda_stream, int path, int rows, int cols, const double* X, double* Q, double* R,

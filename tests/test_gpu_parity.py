@@ -499,3 +499,25 @@ def test_gemm_randomised_shapes_against_numpy():
         out = pkg.gemm_f64(Ad, Bd, transA=transA).cpu().numpy()
         scale = np.linalg.norm(ref) if np.linalg.norm(ref) > 0 else 1.0
         assert np.linalg.norm(out - ref) / scale < 1e-13, (trial, M, N, K, transA, padA, padB)
+
+
+@pytest.mark.parametrize("M,N,K", [
+    (2000, 100, 4000),     # 16 tiles of 128x104, 250 k-tiles each: stream-K, every tile split over ~9 CTAs
+    (9604, 196, 2401),     # K5's shape with a shorter K: 152 tiles on 148 CTAs
+    (1100, 1030, 1500),    # 128x64 tiles, two CTAs per SM: 153 tiles on 296 CTAs, ragged in M, N and K
+    (700, 260, 9000),      # 128x128 tiles (N pads least there), 18 tiles, K not a multiple of 16
+    (4000, 196, 333),      # short K: split-K / plain tiles chosen by the cost model
+])
+def test_gemm_k_splitting_schedules_against_numpy(M, N, K):
+    """qrctm_gemm_f64_ws: with a scratch buffer the launcher may split K (split-K or stream-K).
+    Result vs NumPy, bitwise reproducibility, and agreement with the unsplit schedule to summation-order rounding."""
+    g = np.random.default_rng(M + 3 * N + 7 * K)
+    A = g.standard_normal((K, M)); B = g.standard_normal((K, N))
+    Ad, Bd = torch_dev(A), torch_dev(B)
+    ref = A.T @ B
+    out1 = pkg.gemm_f64(Ad, Bd, transA=True, work_bytes=256 << 20).cpu().numpy()
+    out2 = pkg.gemm_f64(Ad, Bd, transA=True, work_bytes=256 << 20).cpu().numpy()
+    plain = pkg.gemm_f64(Ad, Bd, transA=True).cpu().numpy()
+    assert np.array_equal(out1, out2)
+    assert rel(out1, ref) < 1e-13
+    assert rel(out1, plain) < 1e-14
