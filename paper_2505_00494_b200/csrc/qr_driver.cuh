@@ -168,6 +168,38 @@ int apply_block_reflector(cudaStream_t st, const double* Vp, long long ldv, doub
   return 3;
 }
 
+// One-launch version (wy_fused_cluster_kernel): clusters of 8 CTAs, one per 16-column slab.  Returns 0 if the
+// shape does not fit it (rows per thread, shared memory), else 1 after launching.
+template <int NB, int RPT>
+int launch_wy_fused(cudaStream_t st, const double* Vp, long long ldv, double* Y, long long ldy, long long rows, int nc,
+                    int nbw, const double* Tp, int transT, cudaError_t* err) {
+  constexpr int CS = 8;
+  const int rows_cta = (int)((rows + CS - 1) / CS);
+  if (rows_cta > 32 * RPT) return 0;
+  const size_t smem = sizeof(double) * ((size_t)rows_cta * (NB + 2) + 8 * 256 + 16 * 256 + 256);
+  static int max_smem = -1;
+  if (max_smem < 0) {
+    int dev = 0; cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+  }
+  if (smem > (size_t)max_smem) return 0;
+  static bool attr = false;
+  if (!attr) {
+    *err = cudaFuncSetAttribute(wy_fused_cluster_kernel<NB, RPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem);
+    if (*err != cudaSuccess) return -1;
+    attr = true;
+  }
+  const int nslab = (nc + NB - 1) / NB;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(nslab * CS); cfg.blockDim = dim3(256); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = CS; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  *err = cudaLaunchKernelEx(&cfg, wy_fused_cluster_kernel<NB, RPT>, Vp, ldv, Y, ldy, rows, nc, nbw, Tp, transT, rows_cta);
+  return *err == cudaSuccess ? 1 : -1;
+}
+
 template <int NB>
 long long form_q_global(cudaStream_t st, long long rows, int n, const QrWork& wk, double* Q, cudaError_t* err);
 
@@ -191,9 +223,18 @@ long long qr_factor_blocked_t(cudaStream_t st, long long rows, int n, const doub
                : launch_panel(st, wk.V, n, rows, j0, nbw, wk.Vc, wk.tau, Tp);
     if (*err != cudaSuccess) return -1;
     ++launches;
-    if (n2 > 0)      // trailing update: A2 <- (I - Vp T^T Vp^T) A2
-      launches += apply_block_reflector<NB>(st, wk.Vc + (long long)j0 * n + j0, n, wk.V + (long long)j0 * n + j0 + nbw,
-                                            n, rows - j0, n2, nbw, Tp, 1, wk);
+    if (n2 > 0) {    // trailing update: A2 <- (I - Vp T^T Vp^T) A2
+      const double* Vp = wk.Vc + (long long)j0 * n + j0;
+      double* A2 = wk.V + (long long)j0 * n + j0 + nbw;
+      // up to 8 x 32 x 20 = 5120 rows: one cluster launch; taller (cfg4): the three streaming kernels (a 40-rows-per-
+      // thread instantiation spills and takes 60 us per panel against their 33, profiles/r1_qr_panel_phases.md)
+      int nf = 0;
+      if (NB == 16) {
+        nf = launch_wy_fused<16, 20>(st, Vp, n, A2, n, rows - j0, n2, nbw, Tp, 1, err);
+        if (nf < 0) return -1;
+      }
+      launches += nf > 0 ? nf : apply_block_reflector<NB>(st, Vp, n, A2, n, rows - j0, n2, nbw, Tp, 1, wk);
+    }
   }
   copy_triu_kernel<<<(n * n + 255) / 256, 256, 0, st>>>(wk.V, n, n, R);
   launches += 1;

@@ -865,6 +865,141 @@ wy_update_kernel(const double* __restrict__ Vp, long long ldv, double* __restric
 }
 
 // ------------------------------------------------------------------------------
+// The same block-reflector application in ONE launch (trailing update of the blocked QR):
+//   Y <- (I - Vp op(T) Vp^T) Y,   Y = rows x nc (ld ldy),  Vp = rows x nbw (ld ldv)
+// A cluster of CS CTAs owns a slab of 16 columns of Y and all its rows (CTA rank r: a contiguous block of
+// rows_cta rows).  Each thread keeps its part of the slab in registers from the one read to the one write
+// (2 columns x RPT rows; thread = (row group rg = tid / 8, column pair ct = tid % 8), rows rg + 32 i); the CTA's
+// rows of Vp sit in shared memory (pitch 18 doubles: the four rows a warp touches fall into different banks).
+//   phase 1: W1 = Vp^T Y     per-thread partial sums -> warp shuffles -> 8 warps (fixed order) -> the cluster's
+//                            CTAs through distributed shared memory (fixed order over the ranks)
+//   phase 2: W2 = op(T) W1   16 x 16, every CTA for itself
+//   phase 3: Y -= Vp W2      from the registers, one coalesced write
+// Y crosses the L2 once in each direction (the three-kernel version reads it twice and goes through `part`), and the
+// two relaunches are gone.  Deterministic: every sum has a fixed order.
+template <int NB, int RPT>
+__global__ void __launch_bounds__(256, 1)
+wy_fused_cluster_kernel(const double* __restrict__ Vp, long long ldv, double* __restrict__ Y, long long ldy,
+                        long long rows, int nc, int nbw, const double* __restrict__ Tp, int transT, int rows_cta) {
+  static_assert(NB == 16, "thread mapping assumes 16-column slabs and 16-wide panels");
+  namespace cg = cooperative_groups;
+  cg::cluster_group cluster = cg::this_cluster();
+  const int CS = (int)cluster.num_blocks(), rank = (int)cluster.block_rank();
+  constexpr int VP = NB + 2;                      // shared-memory pitch of a row of Vp
+  extern __shared__ __align__(16) double wsm[];
+  double* vs = wsm;                               // rows_cta x VP
+  double* red = vs + (size_t)rows_cta * VP;       // 8 warps x 256
+  double* xch = red + 8 * 256;                    // CS ranks x 256   (written by the peers)
+  double* w2s = xch + 16 * 256;                   // 16 x 16
+  const int tid = threadIdx.x, rg = tid >> 3, ct = tid & 7, lane = tid & 31, warp = tid >> 5;
+  const int slab = blockIdx.x / CS;
+  const int jc = slab * NB + ct;                  // this thread's columns: jc, jc + 8
+  const bool c0ok = jc < nc, c1ok = jc + 8 < nc;
+  const long long r0 = (long long)rank * rows_cta;
+  long long rl = rows - r0; if (rl > rows_cta) rl = rows_cta; if (rl < 0) rl = 0;
+  const int nr = (int)rl;                         // rows of this CTA
+
+  // the slab into registers (all loads in flight at once), the rows of Vp into shared memory
+  double y0[RPT], y1[RPT];
+#pragma unroll
+  for (int i = 0; i < RPT; ++i) {
+    const int r = rg + 32 * i;
+    const double* yp = Y + (r0 + r) * ldy + jc;
+    y0[i] = (r < nr && c0ok) ? yp[0] : 0.0;
+    y1[i] = (r < nr && c1ok) ? yp[8] : 0.0;
+  }
+  {
+    const int a = tid & 15;                         // 16 rows per sweep of the CTA, 8 sweeps in flight
+    const double* vp = Vp + r0 * ldv + a;
+    for (int ib = tid >> 4; ib < nr; ib += 128) {
+      double t[8];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) t[u] = (a < nbw && ib + 16 * u < nr) ? vp[(long long)(ib + 16 * u) * ldv] : 0.0;
+#pragma unroll
+      for (int u = 0; u < 8; ++u) if (ib + 16 * u < nr) vs[(ib + 16 * u) * VP + a] = t[u];
+    }
+  }
+  __syncthreads();
+
+  // phase 1
+  double acc0[NB], acc1[NB];
+#pragma unroll
+  for (int a = 0; a < NB; ++a) acc0[a] = acc1[a] = 0.0;
+#pragma unroll
+  for (int i = 0; i < RPT; ++i) {
+    const int r = rg + 32 * i;
+    if (r < nr) {
+      const double2* v2 = reinterpret_cast<const double2*>(vs + r * VP);
+#pragma unroll
+      for (int q = 0; q < NB / 2; ++q) {
+        const double2 v = v2[q];
+        acc0[2 * q] = fma(v.x, y0[i], acc0[2 * q]);         acc1[2 * q] = fma(v.x, y1[i], acc1[2 * q]);
+        acc0[2 * q + 1] = fma(v.y, y0[i], acc0[2 * q + 1]); acc1[2 * q + 1] = fma(v.y, y1[i], acc1[2 * q + 1]);
+      }
+    }
+  }
+  // the four row groups of a warp (lanes ct, ct+8, ct+16, ct+24), then the 8 warps in order
+#pragma unroll
+  for (int a = 0; a < NB; ++a) {
+    acc0[a] += __shfl_xor_sync(0xffffffffu, acc0[a], 8);  acc1[a] += __shfl_xor_sync(0xffffffffu, acc1[a], 8);
+    acc0[a] += __shfl_xor_sync(0xffffffffu, acc0[a], 16); acc1[a] += __shfl_xor_sync(0xffffffffu, acc1[a], 16);
+  }
+  if (lane < 8) {
+#pragma unroll
+    for (int a = 0; a < NB; ++a) {
+      red[warp * 256 + a * NB + ct] = acc0[a];
+      red[warp * 256 + a * NB + ct + 8] = acc1[a];
+    }
+  }
+  __syncthreads();
+  {
+    double t = 0.0;                                // thread tid = entry (a, j) = (tid / 16, tid % 16)
+#pragma unroll
+    for (int w = 0; w < 8; ++w) t += red[w * 256 + tid];
+    for (int q = 0; q < CS; ++q) *cluster.map_shared_rank(xch + rank * 256 + tid, q) = t;
+  }
+  cluster.sync();
+  {
+    double t = 0.0;
+    for (int q = 0; q < CS; ++q) t += xch[q * 256 + tid];
+    red[tid] = t;                                  // W1[a][j]
+  }
+  __syncthreads();
+
+  // phase 2
+  {
+    const int a = tid >> 4, j = tid & 15;
+    double t = 0.0;
+    if (a < nbw)
+      for (int k = 0; k < nbw; ++k) t = fma(transT ? Tp[k * NB + a] : Tp[a * NB + k], red[k * NB + j], t);
+    w2s[tid] = t;
+  }
+  __syncthreads();
+
+  // phase 3
+  double w0[NB], w1[NB];
+#pragma unroll
+  for (int a = 0; a < NB; ++a) { w0[a] = w2s[a * NB + ct]; w1[a] = w2s[a * NB + ct + 8]; }
+#pragma unroll
+  for (int i = 0; i < RPT; ++i) {
+    const int r = rg + 32 * i;
+    if (r < nr) {
+      const double2* v2 = reinterpret_cast<const double2*>(vs + r * VP);
+      double s0 = 0.0, s1 = 0.0, t0 = 0.0, t1 = 0.0;
+#pragma unroll
+      for (int q = 0; q < NB / 2; ++q) {
+        const double2 v = v2[q];
+        s0 = fma(v.x, w0[2 * q], s0);     s1 = fma(v.x, w1[2 * q], s1);
+        t0 = fma(v.y, w0[2 * q + 1], t0); t1 = fma(v.y, w1[2 * q + 1], t1);
+      }
+      double* yp = Y + (r0 + r) * ldy + jc;
+      if (c0ok) yp[0] = y0[i] - (s0 + t0);
+      if (c1ok) yp[8] = y1[i] - (s1 + t1);
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------
 // Form Q in one shot (K2c).  With all reflectors V (unit lower trapezoidal, m x n) the product of the
 // Householder transformations is  H_1 ... H_n = I - V T V^T,  T^{-1} = D^{-1} + striu(V^T V), D = diag(tau),
 // so  Q = (I - V T V^T) [I;0] = [I;0] - V X,   X = T V_top^T   (V_top = the first n rows of V),
