@@ -353,11 +353,11 @@ gemm_f64_dmma_ws(GemmArgs p) {
     }
     const int m0 = (rem / tn) * BM, n0 = (rem % tn) * BN;
 
-    // Direct epilogue: the output offsets of the tile's BM rows and BN columns (-1 = out of range) are worked out
-    // once per tile by all consumer threads together, while the first operand tiles are still in flight, instead
-    // of 16 index-map evaluations (32 integer divisions) per thread after the main loop.
-    long long* otab = reinterpret_cast<long long*>(empty + STAGES);
-    if (p.epi == 0 && !(SK && partial)) {
+    // The output offsets of the tile's BM rows and BN columns (-1 = out of range) are worked out once per tile by
+    // all consumer threads together, while the first operand tiles are still in flight, instead of up to 16
+    // index-map evaluations (32 integer divisions) per thread after the main loop.
+    long long* otab = reinterpret_cast<long long*>(empty + STAGES) + NCW * 8 * (WN + 4);   // behind the staging slabs
+    if (!(SK && partial)) {
       asm volatile("bar.sync 1, %0;\n" ::"n"(NCW * 32) : "memory");       // previous tile's epilogue has read the table
       for (int t = tid; t < BM + BN; t += NCW * 32) {
         const int g = t < BM ? m0 + t : n0 + t - BM;
@@ -422,16 +422,16 @@ gemm_f64_dmma_ws(GemmArgs p) {
       // store instruction writes 32 consecutive columns of one row (coalesced wherever co() is contiguous)
       constexpr int SP = WN + 4, NCH = (WN + 31) / 32;
       double* stg = reinterpret_cast<double*>(empty + STAGES) + warp * (8 * SP);
+      asm volatile("bar.sync 1, %0;\n" ::"n"(NCW * 32) : "memory");       // offset table complete
       long long coffL[NCH];
 #pragma unroll
       for (int q = 0; q < NCH; ++q) {
-        const int cl = q * 32 + lane, c = n0 + wn0 + cl;
-        coffL[q] = (cl < WN && c < p.N) ? p.co(c) : -1;
+        const int cl = q * 32 + lane;
+        coffL[q] = cl < WN ? otab[BM + wn0 + cl] : -1;
       }
 #pragma unroll
       for (int i = 0; i < FM; ++i) {
-        const int rbase = m0 + wm0 + i * 8;
-        const long long myro = (lane < 8 && rbase + lane < p.M) ? p.ro(rbase + lane) : -1;
+        const long long myro = lane < 8 ? otab[wm0 + i * 8 + lane] : -1;
 #pragma unroll
         for (int j = 0; j < FN; ++j) {
           double2 v2 = make_double2(acc[i][j][0], acc[i][j][1]);

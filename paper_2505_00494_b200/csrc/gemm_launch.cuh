@@ -26,7 +26,8 @@ template <int BM, int BN, int WM, int WN, int STAGES>
 cudaError_t launch_cfg_ws(cudaStream_t st, const GemmArgs& g, int splits, StreamK* sk = nullptr) {
   constexpr int NT = ((BM / WM) * (BN / WN) + 1) * 32;
   constexpr size_t smem = sizeof(double) * STAGES * BK * ((BM + PAD) + (BN + PAD)) + 2 * STAGES * sizeof(uint64_t) +
-                          sizeof(double) * (BM / WM) * (BN / WN) * 8 * (WN + 4);     // + per-warp epilogue slabs
+                          sizeof(double) * (BM / WM) * (BN / WN) * 8 * (WN + 4) +     // + per-warp epilogue slabs
+                          sizeof(long long) * (BM + BN);                               // + output-offset table
   static bool attr_done = false;
   if (!attr_done) {
     cudaError_t e = cudaFuncSetAttribute(gemm_f64_dmma_ws<BM, BN, WM, WN, STAGES>,
