@@ -168,12 +168,26 @@ int apply_block_reflector(cudaStream_t st, const double* Vp, long long ldv, doub
   return 3;
 }
 
+constexpr int wy_fused_max_slabs16 = 7;     // 16-CTA clusters co-resident on a B200 (launch__cluster_max_active)
 // One-launch version (wy_fused_cluster_kernel): clusters of 8 CTAs, one per 16-column slab.  Returns 0 if the
 // shape does not fit it (rows per thread, shared memory), else 1 after launching.
 template <int NB, int RPT>
 int launch_wy_fused(cudaStream_t st, const double* Vp, long long ldv, double* Y, long long ldy, long long rows, int nc,
                     int nbw, const double* Tp, int transT, cudaError_t* err) {
-  constexpr int CS = 8;
+  // clusters of 8 (15 of them fit the GPU at once); taller matrices: clusters of 16 (7 at once) while the slabs fit
+  // one wave of them -- beyond that the three streaming kernels are faster
+  static int max16 = -1;
+  if (max16 < 0) {
+    max16 = cudaFuncSetAttribute(wy_fused_cluster_kernel<NB, RPT>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) ==
+                    cudaSuccess ? 1 : 0;
+    cudaGetLastError();
+  }
+  const int nslab_ = (nc + NB - 1) / NB;
+  int CS = 8;
+  if ((rows + CS - 1) / CS > 32 * RPT) {
+    if (!max16 || nslab_ > wy_fused_max_slabs16) return 0;
+    CS = 16;
+  }
   const int rows_cta = (int)((rows + CS - 1) / CS);
   if (rows_cta > 32 * RPT) return 0;
   const size_t smem = sizeof(double) * ((size_t)rows_cta * (NB + 2) + 8 * 256 + 16 * 256 + 256);
