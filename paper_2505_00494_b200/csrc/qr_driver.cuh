@@ -282,8 +282,19 @@ long long form_q_global(cudaStream_t st, long long rows, int n, const QrWork& wk
     trsm_attr = true;
   }
   set_identity_top_kernel<<<296, 256, 0, st>>>(Q, rows, n);
-  wy_formq_trsm_kernel<NB><<<npan, NB * NB, sizeof(double) * (size_t)npan * NB * NB * 2, st>>>(wk.Gq, wk.Tfac, wk.Vc, n, n,
-                                                                                             wk.Xq);
+  if (npan <= 16) {
+    static bool pipe_attr = false;
+    if (!pipe_attr) {
+      *err = cudaFuncSetAttribute(wy_formq_trsm_pipe_kernel<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+      if (*err != cudaSuccess) return -1;
+      pipe_attr = true;
+    }
+    wy_formq_trsm_pipe_kernel<NB><<<npan, NB * NB, sizeof(double) * (size_t)npan * NB * NB * 3, st>>>(wk.Gq, wk.Tfac, wk.Vc,
+                                                                                                    n, n, wk.Xq);
+  } else {
+    wy_formq_trsm_kernel<NB><<<npan, NB * NB, sizeof(double) * (size_t)npan * NB * NB * 2, st>>>(wk.Gq, wk.Tfac, wk.Vc, n,
+                                                                                               n, wk.Xq);
+  }
   transpose_tall_kernel<<<dim3((unsigned)((rows + 31) / 32), (n + 31) / 32), dim3(32, 8), 0, st>>>(wk.Vc, rows, n, wk.Vct);
   launches += 3;
   int nl = launch_gemm(st, 0, GemmCall{wk.Vct, rows, 1, wk.Xq, n, Q, plain_map(n), IndexMap{1, 1, 0}, (int)rows, n, n, 1},
