@@ -51,7 +51,7 @@ cudaError_t launch_cfg_ws(cudaStream_t st, const GemmArgs& g, int splits, Stream
     const int tn = (g.N + BN - 1) / BN, nkt = (g.K + BK - 1) / BK;
     const long long units = nwork * nkt;
     const long long ncta = units < nslots ? units : nslots;
-    sk->used = splits == 1 && !g.batch && (size_t)2 * ncta * BM * BN <= sk->ws_elems;
+    sk->used = splits == 1 && !g.batch && ncta <= SK_MAXSEG && (size_t)2 * ncta * BM * BN <= sk->ws_elems;
     if (sk->used) {
       static bool sk_attr = false;
       if (!sk_attr) {
