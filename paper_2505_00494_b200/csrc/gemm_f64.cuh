@@ -16,6 +16,7 @@
 // * split-K: gridDim.z slices write plain partial tiles; reduce_splitk sums them
 //   in a fixed order (deterministic, no atomics).
 #pragma once
+#include <cuda.h>            // CUtensorMap (type only: the encoder is reached through cudaGetDriverEntryPoint)
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -58,6 +59,13 @@ struct GemmArgs {
   // partial tiles of every split tile in ascending k (fixed order).
   int sk = 0;
   double* sk_ws = nullptr;
+  // ws kernel: tma = 1 -> the operand tiles are fetched with ONE tiled bulk tensor copy each (cp.async.bulk.tensor.2d,
+  // SASS UTMALDG) through these tensor maps instead of one linear bulk copy per k-row.  The box is BK rows of
+  // BM + PAD (BN + PAD) columns, i.e. it is as wide as the padded shared-memory pitch, so the dense box the copy
+  // engine writes IS the conflict-free padded layout (the 4 extra columns are the neighbour tile's, never read);
+  // rows beyond K and columns beyond M / N are zero-filled by the copy engine.
+  int tma = 0;
+  alignas(64) CUtensorMap tmA, tmB;
 };
 
 // first unit of CTA c when `units` units are dealt to `ncta` CTAs
@@ -130,7 +138,7 @@ gemm_f64_dmma(GemmArgs p) {
   constexpr int LDA_S = BM + PAD, LDB_S = BN + PAD;
   constexpr int A_STAGE = BK * LDA_S, B_STAGE = BK * LDB_S;
   constexpr int FM = WM / 8, FN = WN / 8;
-  extern __shared__ __align__(16) double smem[];
+  extern __shared__ __align__(128) double smem[];
   double* As = smem;
   double* Bs = smem + STAGES * A_STAGE;
 
@@ -256,15 +264,20 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
+__device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* tm, int c0, int c1, uint64_t* bar) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];\n"
+               ::"r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(smem_u32(bar)) : "memory");
+}
+
 template <int BM, int BN, int WM, int WN, int STAGES, bool SK = false>
 __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 1) * 32, ((BM / WM) * (BN / WN) <= 4 ? 2 : 1))
-gemm_f64_dmma_ws(GemmArgs p) {
+gemm_f64_dmma_ws(const __grid_constant__ GemmArgs p) {
   constexpr int NW_M = BM / WM, NW_N = BN / WN, NCW = NW_M * NW_N;
   constexpr int LDA_S = BM + PAD, LDB_S = BN + PAD;
   constexpr int A_STAGE = BK * LDA_S, B_STAGE = BK * LDB_S;
   constexpr int FM = WM / 8, FN = WN / 8;
   static_assert(BK == 16, "one copy per lane: 16 A rows + 16 B rows");
-  extern __shared__ __align__(16) double smem[];
+  extern __shared__ __align__(128) double smem[];
   double* As = smem;
   double* Bs = smem + STAGES * A_STAGE;
   uint64_t* full = reinterpret_cast<uint64_t*>(Bs + STAGES * B_STAGE);
@@ -310,6 +323,19 @@ gemm_f64_dmma_ws(GemmArgs p) {
       int wA = p.M - m0; if (wA > BM) wA = BM; wA = (wA + 1) & ~1;
       int wB = p.N - n0; if (wB > BN) wB = BN; wB = (wB + 1) & ~1;
       const uint32_t bytes = (uint32_t)(isB ? wB : wA) * 8u;
+      if (p.tma) {
+        for (int kt = kt_begin; kt < kt_end; ++kt, ++it) {
+          const int stage = it % STAGES, round = it / STAGES;
+          if (round > 0) mbar_wait(empty + stage, (round - 1) & 1);
+          if (lane == 0) {
+            mbar_expect_tx(full + stage, (uint32_t)(BK * (LDA_S + LDB_S)) * 8u);
+            tma_load_2d(As + stage * A_STAGE, &p.tmA, m0, kt * BK, full + stage);
+            tma_load_2d(Bs + stage * B_STAGE, &p.tmB, n0, kt * BK, full + stage);
+          }
+          __syncwarp();
+        }
+        continue;
+      }
       for (int kt = kt_begin; kt < kt_end; ++kt, ++it) {
         const int stage = it % STAGES, round = it / STAGES;
         if (round > 0) mbar_wait(empty + stage, (round - 1) & 1);

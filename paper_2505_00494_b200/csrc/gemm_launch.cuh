@@ -3,6 +3,7 @@
 #pragma once
 
 // ------------------------------------------------------------------ GEMM launcher
+
 template <int BM, int BN, int WM, int WN, int STAGES>
 cudaError_t launch_cfg(cudaStream_t st, const GemmArgs& g, int splits) {
   constexpr int NT = (BM / WM) * (BN / WN) * 32;
@@ -17,6 +18,33 @@ cudaError_t launch_cfg(cudaStream_t st, const GemmArgs& g, int splits) {
   dim3 grid((g.N + BN - 1) / BN, (g.M + BM - 1) / BM, splits);
   gemm_f64_dmma<BM, BN, WM, WN, STAGES><<<grid, NT, smem, st>>>(g);
   return cudaGetLastError();
+}
+
+// Tensor maps for the tiled bulk copies of the ws kernel (the encoder comes from the driver through the runtime, the
+// library links no libcuda).  Returns false if the driver entry point is missing or the shape is refused.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+bool encode_operand_map(CUtensorMap* tm, const double* base, long long ld, int width, int krows, int box_w) {
+  static EncodeTiledFn fn = nullptr;
+  static bool tried = false;
+  if (!tried) {
+    tried = true;
+    void* f = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(f);
+    cudaGetLastError();
+  }
+  if (!fn || width < 1 || krows < 1) return false;
+  const cuuint64_t dims[2] = {(cuuint64_t)width, (cuuint64_t)krows};
+  const cuuint64_t strides[1] = {(cuuint64_t)ld * sizeof(double)};
+  const cuuint32_t box[2] = {(cuuint32_t)box_w, (cuuint32_t)BK};
+  const cuuint32_t estr[2] = {1, 1};
+  return fn(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, const_cast<double*>(base), dims, strides, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 // stream-K request: workspace for the partial tiles; `used` is set when the launch went that way (else plain tiles)
@@ -45,6 +73,11 @@ cudaError_t launch_cfg_ws(cudaStream_t st, const GemmArgs& g, int splits, Stream
   }
   GemmArgs ga = g;
   ga.nz = splits;
+  // tiled bulk tensor copies when the k-rows are the stored rows (no K-row map, no batch offsets)
+  ga.tma = 0;
+  if (!g.batch && g.ka.div == 1 && g.ka.hi == 1 && g.ka.lo == 0)
+    ga.tma = encode_operand_map(&ga.tmA, g.A, g.lda, g.M, g.K, BM + PAD) &&
+             encode_operand_map(&ga.tmB, g.B, g.ldb, g.N, g.K, BN + PAD) ? 1 : 0;
   const long long nwork = (long long)((g.N + BN - 1) / BN) * ((g.M + BM - 1) / BM) * splits;
   if (sk) {
     // stream-K: one CTA per slot, every CTA the same number (+-1) of k-tiles; then the fix-up of the split tiles
