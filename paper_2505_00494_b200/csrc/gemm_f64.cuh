@@ -58,6 +58,7 @@ struct GemmArgs {
   // 2 * blockIdx.x (its first segment) or 2 * blockIdx.x + 1 (its last) of sk_ws, and streamk_fixup sums the
   // partial tiles of every split tile in ascending k (fixed order).
   int sk = 0;
+  int sk_t1 = 0;             // whole-tile CTAs ahead of the stream-K CTAs (hybrid schedule)
   double* sk_ws = nullptr;
   // ws kernel: tma = 1 -> the operand tiles are fetched with ONE tiled bulk tensor copy each (cp.async.bulk.tensor.2d,
   // SASS UTMALDG) through these tensor maps instead of one linear bulk copy per k-row.  The box is BK rows of
@@ -68,8 +69,13 @@ struct GemmArgs {
   alignas(64) CUtensorMap tmA, tmB;
 };
 
-// first unit of CTA c when `units` units are dealt to `ncta` CTAs
-__host__ __device__ inline long long sk_first_unit(long long c, long long units, long long ncta) { return c * units / ncta; }
+// First unit of CTA c.  The first t1 CTAs take one whole tile each (nkt units, stored directly); the remaining
+// ncta - t1 CTAs share the rest of the units evenly.  t1 = 0: pure stream-K.  t1 = whole waves of tiles: only the
+// ragged last wave is dealt out by k-tiles ("data-parallel + stream-K" hybrid).
+__host__ __device__ inline long long sk_first_unit(long long c, long long units, long long ncta, long long t1, long long nkt) {
+  if (c <= t1) return c * nkt;
+  return t1 * nkt + (c - t1) * (units - t1 * nkt) / (ncta - t1);
+}
 
 constexpr int BK = 16;
 constexpr int PAD = 4;
@@ -290,8 +296,8 @@ gemm_f64_dmma_ws(const __grid_constant__ GemmArgs p) {
   const int tn = (p.N + BN - 1) / BN, tm = (p.M + BM - 1) / BM;
   const long long nwork = (long long)tn * tm * p.nz;
   const int nkt_total = (p.K + BK - 1) / BK;
-  const long long w_begin = SK ? sk_first_unit(blockIdx.x, (long long)tn * tm * nkt_total, gridDim.x) : blockIdx.x;
-  const long long w_end = SK ? sk_first_unit(blockIdx.x + 1, (long long)tn * tm * nkt_total, gridDim.x) : nwork;
+  const long long w_begin = SK ? sk_first_unit(blockIdx.x, (long long)tn * tm * nkt_total, gridDim.x, p.sk_t1, nkt_total) : blockIdx.x;
+  const long long w_end = SK ? sk_first_unit(blockIdx.x + 1, (long long)tn * tm * nkt_total, gridDim.x, p.sk_t1, nkt_total) : nwork;
 
   if (tid == 0) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, NCW); }
@@ -369,7 +375,7 @@ gemm_f64_dmma_ws(const __grid_constant__ GemmArgs p) {
       const long long left = w_end - w;
       kt_end = left < nkt_total - kt_begin ? kt_begin + (int)left : nkt_total;
       partial = kt_begin != 0 || kt_end != nkt_total;
-      slot = 2 * blockIdx.x + (w == w_begin ? 0 : 1);
+      slot = 2 * ((int)blockIdx.x - p.sk_t1) + (w == w_begin ? 0 : 1);    // whole-tile CTAs never write a partial tile
       w += kt_end - kt_begin;
     } else {
       z = (int)(w / ((long long)tn * tm)); rem = (int)(w % ((long long)tn * tm));
@@ -567,22 +573,22 @@ __global__ void reduce_splitk(const double* part, long long split_stride, int sp
 // out[ro(i)+co(j)] (op)= sum of the partial tiles in ascending k (= ascending CTA index: fixed order).
 constexpr int SK_MAXSEG = 320;
 __global__ void __launch_bounds__(256)
-streamk_fixup(const double* __restrict__ ws, int BM, int BN, int tn, int nkt, long long units, int ncta, int M, int N,
-              double* out, IndexMap ro, IndexMap co, int mode) {
+streamk_fixup(const double* __restrict__ ws, int BM, int BN, int tn, int nkt, long long units, int ncta, int t1, int M,
+              int N, double* out, IndexMap ro, IndexMap co, int mode) {
   __shared__ int slots[SK_MAXSEG];
   __shared__ int nseg_s;
-  const int t = blockIdx.x;
+  const int t = t1 + blockIdx.x;                             // tiles below t1 were stored directly
   if (threadIdx.x == 0) {
     const long long ub = (long long)t * nkt, ue = ub + nkt;
-    long long c = ub * ncta / units;
-    while (c + 1 < ncta && sk_first_unit(c + 1, units, ncta) <= ub) ++c;
-    while (c > 0 && sk_first_unit(c, units, ncta) > ub) --c;
+    long long c = t1 + (ub - (long long)t1 * nkt) * (ncta - t1) / (units - (long long)t1 * nkt);
+    while (c + 1 < ncta && sk_first_unit(c + 1, units, ncta, t1, nkt) <= ub) ++c;
+    while (c > t1 && sk_first_unit(c, units, ncta, t1, nkt) > ub) --c;
     int nseg = 0;
     for (; c < ncta && nseg < SK_MAXSEG; ++c) {
-      const long long u0 = sk_first_unit(c, units, ncta), u1 = sk_first_unit(c + 1, units, ncta);
+      const long long u0 = sk_first_unit(c, units, ncta, t1, nkt), u1 = sk_first_unit(c + 1, units, ncta, t1, nkt);
       if (u0 >= ue) break;
       if (u0 <= ub && u1 >= ue) { nseg = 0; break; }         // whole tile by one CTA: stored directly
-      if (u1 > u0) slots[nseg++] = (int)(2 * c + (u0 >= ub ? 0 : 1));   // first segment of CTA c, else its last
+      if (u1 > u0) slots[nseg++] = (int)(2 * (c - t1) + (u0 >= ub ? 0 : 1));   // first segment of CTA c, else its last
     }
     nseg_s = nseg;
   }

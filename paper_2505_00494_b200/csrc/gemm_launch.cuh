@@ -48,7 +48,7 @@ bool encode_operand_map(CUtensorMap* tm, const double* base, long long ld, int w
 }
 
 // stream-K request: workspace for the partial tiles; `used` is set when the launch went that way (else plain tiles)
-struct StreamK { double* ws; size_t ws_elems; bool used; };
+struct StreamK { double* ws; size_t ws_elems; bool used; bool hybrid; };
 
 template <int BM, int BN, int WM, int WN, int STAGES>
 cudaError_t launch_cfg_ws(cudaStream_t st, const GemmArgs& g, int splits, StreamK* sk = nullptr) {
@@ -83,8 +83,11 @@ cudaError_t launch_cfg_ws(cudaStream_t st, const GemmArgs& g, int splits, Stream
     // stream-K: one CTA per slot, every CTA the same number (+-1) of k-tiles; then the fix-up of the split tiles
     const int tn = (g.N + BN - 1) / BN, nkt = (g.K + BK - 1) / BK;
     const long long units = nwork * nkt;
-    const long long ncta = units < nslots ? units : nslots;
-    sk->used = splits == 1 && !g.batch && ncta <= SK_MAXSEG && (size_t)2 * ncta * BM * BN <= sk->ws_elems;
+    // hybrid: whole waves of tiles as they are, only the ragged last wave dealt out by k-tiles
+    const long long t1 = sk->hybrid ? nwork / nslots * nslots : 0;
+    const long long nsk = units - t1 * nkt < nslots ? units - t1 * nkt : nslots;      // stream-K CTAs
+    const long long ncta = t1 + nsk;
+    sk->used = splits == 1 && !g.batch && nsk >= 1 && nsk <= SK_MAXSEG && (size_t)2 * nsk * BM * BN <= sk->ws_elems;
     if (sk->used) {
       static bool sk_attr = false;
       if (!sk_attr) {
@@ -93,10 +96,10 @@ cudaError_t launch_cfg_ws(cudaStream_t st, const GemmArgs& g, int splits, Stream
         if (e != cudaSuccess) return e;
         sk_attr = true;
       }
-      ga.sk = 1; ga.sk_ws = sk->ws;
+      ga.sk = 1; ga.sk_ws = sk->ws; ga.sk_t1 = (int)t1;
       gemm_f64_dmma_ws<BM, BN, WM, WN, STAGES, true><<<(unsigned)ncta, NT, smem, st>>>(ga);
-      streamk_fixup<<<dim3((unsigned)nwork, 8), 256, 0, st>>>(sk->ws, BM, BN, tn, nkt, units, (int)ncta, g.M, g.N, g.out, g.ro,
-                                                    g.co, g.mode);
+      streamk_fixup<<<dim3((unsigned)(nwork - t1), 8), 256, 0, st>>>(sk->ws, BM, BN, tn, nkt, units, (int)ncta, (int)t1, g.M,
+                                                                    g.N, g.out, g.ro, g.co, g.mode);
       return cudaGetLastError();
     }
   }
@@ -145,7 +148,7 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
   const bool big = t128 >= 120;
   const bool ws_ok = g.transA && g.vecA && g.vecB;     // bulk copies need 16-byte aligned rows
   int splits = 1;
-  bool use_sk = false;
+  bool use_sk = false, sk_hybrid = false;
   int cfg = 0;          // 0: 64x64 cp.async, 1: 128x128 cp.async, 2: ws 128x128, 3: ws 128x104, 4: ws 128x64 (2 CTA/SM)
   const bool ws_big = ws_ok && c.M >= 96 && c.N >= 32 && (double)c.M * c.N * c.K > 2.0e8;
   if (c.batch > 0) {
@@ -188,6 +191,10 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
       // up to two partial tiles per CTA written and read again, one more launch
       const double t_sk = ceil(units / slots) * t_kt + 2 * t_fix + 2.0 * (2.0 * slots * 128.0 * bn * 8.0) / 3e12 + 5e-6;
       if (t_sk < best * 0.97) { use_sk = true; splits = 1; }
+    } else if (splits == 1 && tiles > slots && (size_t)2 * slots * 128 * bn <= splitk_elems) {
+      // many waves: if the last one is ragged and long enough to be worth splitting, deal it out by k-tiles
+      const long long rem = tiles % slots;
+      if (rem > 0 && rem * 10 < slots * 8 && (double)rem * nkt >= 24.0 * slots) { use_sk = true; sk_hybrid = true; }
     }
   } else if (big) {
     cfg = 1;
@@ -205,7 +212,7 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
     g.out = splitk_ws; g.ro = plain_map(c.N); g.co = IndexMap{1, 1, 0}; g.mode = 0;
     g.split_stride = (long long)c.M * c.N;
   }
-  StreamK skreq{splitk_ws, splitk_elems, false};
+  StreamK skreq{splitk_ws, splitk_elems, false, sk_hybrid};
   StreamK* sk = use_sk ? &skreq : nullptr;
   switch (cfg) {
     case 2: *err = launch_cfg_ws<128, 128, 64, 32, 4>(st, g, splits, sk); break;
