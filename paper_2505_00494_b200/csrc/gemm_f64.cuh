@@ -10,11 +10,14 @@
 //   contractions of (E3) are fused into the epilogue of the producing GEMM:
 //       ro(i) = (i / rdiv) * rs_hi + (i % rdiv) * rs_lo     (same for co)
 // * math: mma.sync.aligned.m8n8k4 f64 (SASS DMMA.8x8x4), the only FP64 tensor
-//   instruction sm_100a has (tcgen05 has no f64 kind).  Operands are staged into
-//   shared memory by a 4-stage cp.async (LDGSTS) ring, zero-filled at the ragged
-//   edges; rows are padded by 4 doubles so both fragment loads are conflict free.
-// * split-K: gridDim.z slices write plain partial tiles; reduce_splitk sums them
-//   in a fixed order (deterministic, no atomics).
+//   instruction sm_100a has (tcgen05 has no f64 kind).  Two kernels: gemm_f64_dmma
+//   (small / unaligned cases: a 4-stage cp.async (LDGSTS) ring, zero-filled at the
+//   ragged edges) and gemm_f64_dmma_ws (every large contraction: a TMA producer warp
+//   feeding an mbarrier ring, see below).  Shared-memory rows are padded by 4 doubles
+//   so both fragment loads are conflict free.
+// * K splitting, all deterministic (fixed summation order, no atomics): split-K
+//   (gridDim.z slices write plain partial outputs, reduce_splitk sums them) and, in
+//   the ws kernel, stream-K / hybrid schedules with streamk_fixup.
 #pragma once
 #include <cuda.h>            // CUtensorMap (type only: the encoder is reached through cudaGetDriverEntryPoint)
 #include <cuda_runtime.h>
@@ -234,21 +237,21 @@ gemm_f64_dmma(GemmArgs p) {
 
 // ------------------------------------------------------------------------------
 // Warp-specialised variant (the hot path for every large contraction, transA = 1):
-//   * ONE producer warp stages the operands with bulk asynchronous copies
-//     (cp.async.bulk global -> shared, SASS UBLKCP: the TMA engine's linear mode),
-//     one copy per k-row of the A tile (lanes 0..15) and of the B tile (lanes
-//     16..31), completion counted in bytes on the stage's `full` mbarrier;
-//   * the consumer warps only do LDS.64 + DMMA and release a stage by arriving on
-//     its `empty` mbarrier -- no CTA-wide barrier and no address arithmetic in the
-//     math warps (ncu on the cp.async kernel: DMMA pipe 71.6 % active, the rest
-//     lost to the in-line producer code and __syncthreads, profiles/).
-// The padded row pitch (BM + 4 doubles) keeps the fragment loads conflict free,
-// which the dense box of a tiled tensor map could not.  Ragged M/N edges: copied
-// widths are clipped (rounded up to 16 bytes), the unwritten columns only feed
-// output rows/columns that are never stored.  Ragged K: the missing k-rows of the
-// last tile are zero-filled by the producer with ordinary stores.
-// Requires even leading dimensions and 16-byte aligned bases (checked on the host;
-// otherwise the cp.async kernel above is used).
+//   * ONE producer warp stages the operands through the TMA engine, completion counted in bytes on the stage's
+//     `full` mbarrier.  Default: one tiled bulk tensor copy per operand tile and k-step (cp.async.bulk.tensor.2d
+//     through a tensor map, SASS UTMALDG, issued by one elected lane).  The box is BK rows of BM + PAD (BN + PAD)
+//     columns - exactly the padded shared-memory pitch - so the dense box the copy engine writes is the padded,
+//     bank-conflict-free layout (a BM-wide dense box would give 4-way conflicts on the 8-byte fragment loads and no
+//     swizzle mode removes them); the PAD extra columns are the neighbour tile's and never read; ragged M / N / K
+//     edges are zero-filled by the copy engine.  Batched launches and K-row maps (layered GEMM1): one linear bulk
+//     copy (cp.async.bulk, SASS UBLKCP) per k-row of the A tile (lanes 0..15) and of the B tile (lanes 16..31),
+//     widths clipped, missing k-rows of the last k-step zero-filled by the producer with ordinary stores.
+//   * the consumer warps only do LDS.64 + DMMA and release a stage by arriving on its `empty` mbarrier -- no
+//     CTA-wide barrier and no address arithmetic in the math warps (ncu history in profiles/r1_k4_gemm_ws_ncu.md:
+//     cp.async kernel 71.6 % DMMA-active -> linear bulk copies 93.3 % -> tensor copies 96.4 %).
+//   * SK = true: stream-K / hybrid schedules (GemmArgs::sk, sk_t1).
+// Requires even leading dimensions and 16-byte aligned bases (checked on the host; otherwise the cp.async kernel
+// above is used).
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* b, int count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(b)), "r"(count));
