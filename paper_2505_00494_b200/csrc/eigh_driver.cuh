@@ -53,21 +53,11 @@ void launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cuda
   cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
 }
 
-// W (n x n symmetric, row-major, DEVICE, destroyed) -> lam[k] (largest |lambda| first), U (n x k, ld k).
-// Returns kernels launched or -1.
-long long eigh_top(cudaStream_t st, int n, int k, double* W, double* lam, double* U, void* work, cudaError_t* err) {
-  EighWork wk;
-  eigh_layout(n, k, static_cast<char*>(work), &wk);
+// Householder tridiagonalisation of W (n x n symmetric, row-major, DEVICE; upper triangle swept, destroyed): diagonal
+// -> wk.d, off-diagonal -> wk.e (e[i] couples i-1 and i), reflectors left in W / wk.tau.  Also K8's path for corner
+// matrices too large for one SM's shared memory.  Returns kernels launched.
+long long eigh_tridiagonalise(cudaStream_t st, int n, double* W, const EighWork& wk) {
   long long launches = 0;
-  static int attr_done = 0;
-  if (!attr_done) {
-    int dev = 0, max_smem = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-    cudaFuncSetAttribute(multisect_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem - 1024);
-    cudaFuncSetAttribute(eigh_backtransform_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem - 1024);
-    attr_done = 1;
-  }
   cudaMemsetAsync(wk.tau, 0, sizeof(double) * n, st);
 #define REFL(k_, vprev_, vnew_)                                                                                  \
   do {                                                                                                           \
@@ -104,6 +94,25 @@ long long eigh_top(cudaStream_t st, int n, int k, double* W, double* lam, double
     launches += 1;
   }
 #undef REFL
+  return launches;
+}
+
+// W (n x n symmetric, row-major, DEVICE, destroyed) -> lam[k] (largest |lambda| first), U (n x k, ld k).
+// Returns kernels launched or -1.
+long long eigh_top(cudaStream_t st, int n, int k, double* W, double* lam, double* U, void* work, cudaError_t* err) {
+  EighWork wk;
+  eigh_layout(n, k, static_cast<char*>(work), &wk);
+  long long launches = 0;
+  static int attr_done = 0;
+  if (!attr_done) {
+    int dev = 0, max_smem = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    cudaFuncSetAttribute(multisect_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem - 1024);
+    cudaFuncSetAttribute(eigh_backtransform_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem - 1024);
+    attr_done = 1;
+  }
+  launches += eigh_tridiagonalise(st, n, W, wk);
   const int nc = 2 * k < n ? 2 * k : n;            // candidates: the k smallest and the k largest eigenvalues
   multisect_kernel<<<(nc + 7) / 8, 256, sizeof(double) * (2 * (size_t)n + 40), st>>>(wk.d, wk.e, n, wk.eig, k);
   eigh_select_kernel<<<(nc + 255) / 256, 256, 0, st>>>(wk.eig, nc, k, lam, wk.d, wk.e, n, wk.scal);

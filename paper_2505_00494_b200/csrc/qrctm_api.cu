@@ -27,9 +27,9 @@ inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {   // byte offsets into the workspace
   size_t A, a_mat, a2_mat, LH, rho, B1, B2, P1, C, T, Cn, Tn, X, Q, R, Rt, P, S, W, E, splitk, partial, scal, flag, Wc, dvec, evec,
-      vv, pv, eig, s, s_prev, s_tmp, delta, qrwork, total;
+      vv, pv, eig, s, s_prev, s_tmp, delta, qrwork, k8work, total;
   long long lda_a, ld1, ld2;
-  size_t splitk_elems, qrwork_bytes;
+  size_t splitk_elems, qrwork_bytes, k8work_bytes;
 };
 
 }  // namespace
@@ -67,11 +67,15 @@ struct qrctm {
       *dvec, *evec, *vv, *pv, *eig, *s, *s_prev, *s_tmp, *delta;
   int* flag;
   void* qrwork;
+  void* k8work;                 // scratch of K8's multi-CTA tridiagonalisation (chi too large for one SM), or null
 };
 
 namespace {
 
 unsigned long long qr_work_bytes_impl(long long rows, int cols);
+struct EighWork;
+size_t eigh_layout(long long n, int k, char* base, EighWork* w);
+constexpr int kK8SmemMaxChi = 200;      // above this chi a scratch area for the multi-CTA tridiagonalisation is carved
 
 bool make_layout(int d, int D, int chi, Layout* L) {
   if (d < 1 || D < 1 || chi < 1) return false;
@@ -121,6 +125,8 @@ bool make_layout(int d, int D, int chi, Layout* L) {
   L->delta = take(dbl * 4);
   L->qrwork_bytes = qr_work_bytes_impl(m, chi);
   L->qrwork = take(L->qrwork_bytes);
+  L->k8work_bytes = chi > kK8SmemMaxChi ? eigh_layout(chi, 1, nullptr, nullptr) : 0;
+  L->k8work = take(L->k8work_bytes);
   L->total = off;
   return true;
 }
@@ -135,6 +141,7 @@ void bind_views(qrctm* h) {
 #undef V_
   h->flag = reinterpret_cast<int*>(B + L.flag);
   h->qrwork = B + L.qrwork;
+  h->k8work = L.k8work_bytes ? B + L.k8work : nullptr;
 }
 
 int fail(qrctm* h, int code, const char* what, cudaError_t e = cudaSuccess) {

@@ -155,6 +155,22 @@ int stage_spectrum(qrctm* h, double* s_out, int update_prev, cudaStream_t st) {
     spectrum_finalize_kernel<<<1, nt, sizeof(double) * (chi + 40), st>>>(h->eig, chi, s_out, h->s_prev,
                                                                                  h->delta, update_prev);
     h->launches += 3;
+  } else if (h->k8work && chi <= 1024) {
+    // corner too large for one SM's shared memory: the eigen step's multi-CTA tridiagonalisation (eigh_driver.cuh)
+    // on a scratch copy, then the same multisection / finalisation as the fast path
+    static bool ms_attr = false;
+    if (!ms_attr) {
+      CU(h, cudaFuncSetAttribute(multisect_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
+      ms_attr = true;
+    }
+    EighWork wk;
+    eigh_layout(chi, 1, static_cast<char*>(h->k8work), &wk);
+    CU(h, cudaMemcpyAsync(h->Wc, h->C, sizeof(double) * chi * chi, cudaMemcpyDeviceToDevice, st));
+    h->launches += eigh_tridiagonalise(st, chi, h->Wc, wk);
+    multisect_kernel<<<(chi + 7) / 8, 256, sizeof(double) * (2 * chi + 40), st>>>(wk.d, wk.e, chi, h->eig);
+    spectrum_finalize_kernel<<<1, nt, sizeof(double) * (chi + 40), st>>>(h->eig, chi, s_out, h->s_prev, h->delta,
+                                                                        update_prev);
+    h->launches += 2;
   } else {
     CU(h, cudaMemcpyAsync(h->Wc, h->C, sizeof(double) * chi * chi, cudaMemcpyDeviceToDevice, st));
     tridiag_kernel<<<1, 1024, 0, st>>>(h->Wc, chi, h->dvec, h->evec, h->vv, h->pv);

@@ -241,7 +241,8 @@ def test_cfg1_fixed_count_and_kappa():
 
 def test_spectrum_kernel_against_lapack():
     import torch
-    for chi, seed in [(1, 0), (2, 1), (8, 2), (36, 3), (100, 4), (196, 5)]:
+    # chi <= 236: shared-memory tridiagonalisation; above: the multi-CTA tridiagonalisation of the eigen step
+    for chi, seed in [(1, 0), (2, 1), (8, 2), (36, 3), (100, 4), (196, 5), (236, 6), (237, 7), (400, 8), (700, 9)]:
         A, C0, T0 = gen_config(2, 1, chi, seed)
         h = pkg.QRCTM(2, 1, chi)
         h.set_A(A); h.set_env(C0, T0)
