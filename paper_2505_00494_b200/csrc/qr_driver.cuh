@@ -7,6 +7,7 @@
 constexpr int QR_NB = 16;        // shared-memory / global panel kernel (fallback for very tall panels)
 constexpr int QR_NB_REG = 16;    // register-resident panel kernel (default)
 constexpr int QR_REG_NT = 256, QR_REG_RPT = 40;                       // 640 rows per CTA
+constexpr int QR_REG_RPT_TALL = 80;                                   // 1280 rows per CTA (column k re-broadcast for the update)
 constexpr int QR_MAX_PARTS = 320;
 
 struct QrWork {     // carved out of the caller's work buffer
@@ -131,6 +132,25 @@ int reg_panel_max_cluster() {
   return maxc;
 }
 
+template <int RPT>
+cudaError_t launch_panel_reg_tall(cudaStream_t st, int C, double* V, long long ld, long long m, int j0, int nbw, double* Vc,
+                                  double* tau, double* Tp, long long rpc) {
+  auto k2 = qr_panel_reg2_kernel<QR_NB_REG, QR_REG_NT, RPT, true, false>;
+  static bool attr2 = false;
+  if (!attr2) {
+    cudaError_t e = cudaFuncSetAttribute(k2, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    if (e != cudaSuccess) return e;
+    attr2 = true;
+  }
+  cudaLaunchConfig_t cfg2 = {};
+  cfg2.gridDim = dim3(C); cfg2.blockDim = dim3(QR_REG_NT); cfg2.dynamicSmemBytes = 0; cfg2.stream = st;
+  cudaLaunchAttribute at2[1];
+  at2[0].id = cudaLaunchAttributeClusterDimension;
+  at2[0].val.clusterDim.x = C; at2[0].val.clusterDim.y = 1; at2[0].val.clusterDim.z = 1;
+  cfg2.attrs = at2; cfg2.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg2, k2, V, ld, m, j0, nbw, Vc, tau, Tp, rpc);
+}
+
 cudaError_t launch_panel_reg(cudaStream_t st, double* V, long long ld, long long m, int j0, int nbw, double* Vc,
                              double* tau, double* Tp) {
   constexpr int cap = QR_REG_RPT * (QR_REG_NT / QR_NB_REG);
@@ -139,7 +159,15 @@ cudaError_t launch_panel_reg(cudaStream_t st, double* V, long long ld, long long
   int C = 1;
   while (C < maxc && (prow + C - 1) / C > cap) C *= 2;
   const long long rpc = (prow + C - 1) / C;
-  if (rpc > cap) return cudaErrorInvalidValue;
+  if (rpc > cap) {
+    // tall panel: more rows per thread (48 / 64 / 80), column k re-broadcast for the update
+    if (maxc < 16) return cudaErrorInvalidValue;
+    constexpr int nrg = QR_REG_NT / QR_NB_REG;
+    if (rpc <= 48 * nrg) return launch_panel_reg_tall<48>(st, C, V, ld, m, j0, nbw, Vc, tau, Tp, rpc);
+    if (rpc <= 64 * nrg) return launch_panel_reg_tall<64>(st, C, V, ld, m, j0, nbw, Vc, tau, Tp, rpc);
+    if (rpc <= QR_REG_RPT_TALL * nrg) return launch_panel_reg_tall<QR_REG_RPT_TALL>(st, C, V, ld, m, j0, nbw, Vc, tau, Tp, rpc);
+    return cudaErrorInvalidValue;
+  }
   if (C == 1) {
     qr_panel_reg2_kernel<QR_NB_REG, QR_REG_NT, QR_REG_RPT, false><<<1, QR_REG_NT, 0, st>>>(V, ld, m, j0, nbw, Vc, tau,
                                                                                           Tp, rpc);
@@ -358,7 +386,7 @@ long long qr_factor_blocked(cudaStream_t st, int qr_path, long long rows, int n,
                            : qr_factor_fullreg_t<7, 10>(st, rows, n, X, Q, R, wk, err);
     if (nl != -2) return nl;
   }
-  constexpr long long cap = (long long)QR_REG_RPT * (QR_REG_NT / QR_NB_REG);
+  constexpr long long cap = (long long)QR_REG_RPT_TALL * (QR_REG_NT / QR_NB_REG);
   if (rows <= cap * reg_panel_max_cluster())
     return qr_factor_blocked_t<QR_NB_REG, true>(st, rows, n, X, Q, R, work, err);
   return qr_factor_blocked_t<QR_NB, false>(st, rows, n, X, Q, R, work, err);

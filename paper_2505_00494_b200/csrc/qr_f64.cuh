@@ -316,7 +316,11 @@ __device__ __forceinline__ void qr_mbar_wait(uint64_t* b, uint32_t parity) {
 #define QR_STAMP(i) do { } while (0)      // phase time stamps for the measurement harness (profiles/r1_qr_panel_phases.md)
 #endif
 
-template <int NB, int NT, int RPT, bool CLUSTER>
+// KEEPX = true: the broadcast column k (xs[]) stays in registers from the dot products to the update (RPT = 40: 640
+// rows per CTA).  KEEPX = false: it is shuffled again for the update instead, which frees the registers for twice the
+// rows per thread (RPT = 80: 1280 rows per CTA, 20480 per 16-CTA cluster) at ~2x the per-column time - still twice as
+// fast as the shared-memory panel kernel that tall panels fell back to.
+template <int NB, int NT, int RPT, bool CLUSTER, bool KEEPX = true>
 __global__ void __launch_bounds__(NT, 1)
 qr_panel_reg2_kernel(double* __restrict__ V, long long ld, long long m, int j0, int nbw,
                      double* __restrict__ Vc, double* __restrict__ tau, double* __restrict__ Tp, long long rpc) {
@@ -374,14 +378,15 @@ qr_panel_reg2_kernel(double* __restrict__ V, long long ld, long long m, int j0, 
     }
     // B. column k of my rows, dot with my column.  FP64 dependent-issue latency is long (~30 cycles),
     //    so the sum runs on 8 independent accumulators combined by a fixed tree.
-    double xs[RPT];
+    double xs[KEEPX ? RPT : 1];
     double ac[8];
 #pragma unroll
     for (int u = 0; u < 8; ++u) ac[u] = 0.0;
 #pragma unroll
     for (int t = 0; t < RPT; ++t) {
-      xs[t] = __shfl_sync(0xffffffffu, val[t], lane_base | k);
-      ac[t & 7] = fma(xs[t], val[t], ac[t & 7]);
+      const double x = __shfl_sync(0xffffffffu, val[t], lane_base | k);
+      if (KEEPX) xs[t] = x;
+      ac[t & 7] = fma(x, val[t], ac[t & 7]);
     }
     double acc = ((ac[0] + ac[1]) + (ac[2] + ac[3])) + ((ac[4] + ac[5]) + (ac[6] + ac[7]));
     if (NB == 16) acc += __shfl_xor_sync(0xffffffffu, acc, 16);
@@ -436,10 +441,21 @@ qr_panel_reg2_kernel(double* __restrict__ V, long long ld, long long m, int j0, 
     const double z = fma(scale, gj, yrj);          // v_k^T y_j (j > k)  or  (x_a[r] + scale h_a) (a < k)
     const double w = tk * z;
     // G. update the trailing panel columns
-    if (col > k && col < nbw && tk != 0.0) {
-      const double nsw = -scale * w;
+    if (KEEPX) {
+      if (col > k && col < nbw && tk != 0.0) {
+        const double nsw = -scale * w;
 #pragma unroll
-      for (int t = 0; t < RPT; ++t) val[t] = fma(xs[t], nsw, val[t]);
+        for (int t = 0; t < RPT; ++t) val[t] = fma(xs[t], nsw, val[t]);
+      }
+    } else {
+      // all lanes take part in the shuffles; column k itself (nsw = 0 there) is not modified, so the values read are
+      // the ones the dot products saw
+      const double nsw = (col > k && col < nbw && tk != 0.0) ? -scale * w : 0.0;
+#pragma unroll
+      for (int t = 0; t < RPT; ++t) {
+        const double x = __shfl_sync(0xffffffffu, val[t], lane_base | k);
+        if (nsw != 0.0) val[t] = fma(x, nsw, val[t]);
+      }
     }
     // H. final entries of row r
     if (mine && col < nbw) {

@@ -57,7 +57,9 @@ def test_gemm_odd_leading_dimension_views():
 _QR_SHAPES = [(32, 8), (324, 36), (1024, 64), (50, 50), (7, 1), (333, 17), (16, 16),
               (2500, 100), (40, 33), (9604, 196), (3000, 150), (112, 112), (5000, 64), (1792, 112), (4096, 50),
               (15000, 24), (40000, 40),   # 16-CTA cluster; global-memory panel path
-              (5120, 130), (5121, 130), (2000, 113)]   # one-launch trailing update: its row limit, one past it, ragged slab
+              (5120, 130), (5121, 130), (2000, 113),   # one-launch trailing update: its row limit, one past it, ragged slab
+              (10241, 40), (12289, 48), (16400, 33), (20480, 20), (20481, 20)]   # tall register panels: 48 / 64 / 80 rows
+                                                                                  # per thread, and one row past them
 # the per-reflector (level-2) path 1 is only checked on small cases
 _QR_CASES = [(r, c, p) for p in (0, 1, 2) for (r, c) in _QR_SHAPES if not (p == 1 and r * c > 200000)]
 
