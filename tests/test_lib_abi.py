@@ -63,6 +63,13 @@ def test_invalid_arguments_rejected(lib):
     assert lib.qrctm_shard_range(8, 3, 3, ctypes.byref(m0), ctypes.byref(m1)) == -1
     assert lib.qrctm_shard_range(8, 1, 3, ctypes.byref(m0), ctypes.byref(m1)) == 0 and (m0.value, m1.value) == (3, 6)
     assert lib.qrctm_get_chi(None, None, None) == -1
+    # stand-alone GEMM with a scratch buffer: null operands, bad path, misaligned / inconsistent scratch
+    P = ctypes.c_void_p
+    fake = P(256)
+    assert lib.qrctm_gemm_f64_ws(None, 0, 1, 4, 4, 4, None, 4, None, 4, None, 4, None, 0) == -1
+    assert lib.qrctm_gemm_f64_ws(None, 5, 1, 4, 4, 4, fake, 4, fake, 4, fake, 4, None, 0) == -1
+    assert lib.qrctm_gemm_f64_ws(None, 0, 1, 4, 4, 4, fake, 4, fake, 4, fake, 4, P(8), 64) == -1
+    assert lib.qrctm_gemm_f64_ws(None, 0, 1, 4, 4, 4, fake, 4, fake, 4, fake, 4, None, 64) == -1
 
 
 def test_no_cpu_fallback_without_gpu(lib):
