@@ -15,6 +15,8 @@ another one.  Inputs are the seeded synthetic tensors of qrctm_inputs.
              2 chi^2 D^8 per launch / its mean CUDA-event duration in the timed run,
              against the FP64 tensor issue rate measured live by qrctm_probe_fp64
   cpu_baseline  the oracle (NumPy) timed on the host cores, rank 0, bounded sample
+  time_to_convergence  the config's own BASELINE.json run (max iterations, tol) from its
+             seeded initial environment: iterations done, final delta, device ms
 
 Multi-GPU: the path is one dependent chain on one GPU:
 "replicas only" -- each rank runs an independent instance, no collective.
@@ -264,6 +266,23 @@ def main():
                          "note": "two launches over an L2-resident 15 MB working set: launch-latency-bound"},
     }
 
+    # ---- time to convergence (north_star: "iterations/s and time-to-convergence"): the config's own run from its seeded
+    # initial environment, qrctm_run(iters, tol) with the default check interval (every step); outside the timed region
+    conv = None
+    if rank == 0:
+        h.set_env(C0, T0)
+        torch.cuda.synchronize()
+        ev0.record(h.stream)
+        its, dl = h.run(int(c["iters"]), float(c["tol"]))
+        ev1.record(h.stream)
+        torch.cuda.synchronize()
+        conv = {"iterations": int(its), "max_iter": int(c["iters"]), "tol": float(c["tol"]), "final_delta": float(dl),
+                "converged": bool(dl < c["tol"]), "ms": ev0.elapsed_time(ev1),
+                "note": "BASELINE.json run of this config: qrctm_run(max_iter, tol) from the seeded C0, T0; "
+                        "delta = max_i |s_i - s_i^prev| of the normalised corner spectrum, checked every step"}
+        h.set_env(C0, T0)
+        h.run(2, -1.0)
+
     # ---- NEXT-1 variant: layered absorption, same result up to rounding, own flop count
     layered = None
     if chi % 2 == 0 and not args.no_next:
@@ -415,6 +434,7 @@ def main():
                          "dfma_peak": peak_dfma, "algorithmic_flops_per_launch": fl["K4"], "ms_per_launch": k4_ms},
             "stages_ms": {k: v / nst for k, v in stage_ms.items()},
             "hbm_kernels": hbm_kernels,
+            "time_to_convergence": conv,
             "next_1_layered": layered,
             "next_2_warmup": warm,
             "next_4_shard": shard,
