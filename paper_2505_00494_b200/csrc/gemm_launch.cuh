@@ -149,7 +149,8 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
   const bool ws_ok = g.transA && g.vecA && g.vecB;     // bulk copies need 16-byte aligned rows
   int splits = 1;
   bool use_sk = false, sk_hybrid = false;
-  int cfg = 0;          // 0: 64x64 cp.async, 1: 128x128 cp.async, 2: ws 128x128, 3: ws 128x104, 4: ws 128x64 (2 CTA/SM)
+  int cfg = 0;          // 0: 64x64 cp.async, 1: 128x128 cp.async, 2: ws 128x128, 3: ws 128x104, 4: ws 128x64 (2 CTA/SM),
+                        // 5: ws 128x56, 6: ws 80x208 (one wave for M <= 148 x 80, N <= 208)
   const bool ws_big = ws_ok && c.M >= 96 && c.N >= 32 && (double)c.M * c.N * c.K > 2.0e8;
   if (c.batch > 0) {
     // batched launch (layered absorption): bulk-copy kernel only, one batch per gridDim.z, no split-K
@@ -196,6 +197,12 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
       const long long rem = tiles % slots;
       if (rem > 0 && rem * 10 < slots * 8 && (double)rem * nkt >= 24.0 * slots) { use_sk = true; sk_hybrid = true; }
     }
+    // N in (104, 208] with just over one wave of 128 x 104 tiles and no K split (K1, K6's first product, the form-Q
+    // GEMM: 152 tiles on 148 SMs = two waves): 80 x 208 tiles cover N in one tile and M in one wave
+    if (cfg == 3 && splits == 1 && !use_sk && c.N > 104 && c.N <= 208 && tiles > slots && tiles <= 2 * slots &&
+        (c.M + 79) / 80 <= slots) {
+      cfg = 6;
+    }
   } else if (big) {
     cfg = 1;
   } else if (t64 < 148 && nkt >= 8) {
@@ -219,6 +226,7 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
     case 3: *err = launch_cfg_ws<128, 104, 16, 104, 4>(st, g, splits, sk); break;
     case 4: *err = launch_cfg_ws<128, 64, 64, 32, 4>(st, g, splits, sk); break;
     case 5: *err = launch_cfg_ws<128, 56, 32, 56, 3>(st, g, splits, sk); break;
+    case 6: *err = launch_cfg_ws<80, 208, 16, 104, 3>(st, g, splits, sk); break;
     case 1: *err = launch_cfg<128, 128, 64, 32, 4>(st, g, splits); break;
     default: *err = launch_cfg<64, 64, 32, 32, 4>(st, g, splits); break;
   }
