@@ -169,7 +169,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-next", action="store_true",
-                    help="skip the side measurements of the NEXT-1/2/4 variants (they are outside the timed region)")
+                    help="skip the side measurements outside the timed region: the NEXT-1/2/4 variants and the "
+                         "time-to-convergence run")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -269,7 +270,7 @@ def main():
     # ---- time to convergence (north_star: "iterations/s and time-to-convergence"): the config's own run from its seeded
     # initial environment, qrctm_run(iters, tol) with the default check interval (every step); outside the timed region
     conv = None
-    if rank == 0:
+    if rank == 0 and not args.no_next:
         h.set_env(C0, T0)
         torch.cuda.synchronize()
         ev0.record(h.stream)
