@@ -32,6 +32,11 @@
  *
  * There is no CPU fallback: without a CUDA device qrctm_create fails with
  * QRCTM_ERR_CUDA.
+ *
+ * Limits of this build: D <= 32, chi <= 800, d <= 64.  ONE DEVICE PER PROCESS: the
+ * one-time kernel attributes (shared-memory opt-in, cluster sizes, occupancy) are
+ * cached per process, so all handles of a process must live on the same device
+ * (the one current at the first call).
  */
 #ifndef QRCTM_H
 #define QRCTM_H
@@ -103,8 +108,10 @@ int qrctm_set_stream(qrctm_t* h, void* cuda_stream);
 int qrctm_set_A(qrctm_t* h, const double* A);
 
 /* Copy an initial environment in, symmetrise (if enabled) and Frobenius-
- * normalise it, reset the convergence history (previous spectrum = spectrum of
- * this C). */
+ * normalise it, reset the convergence history: the previous spectrum becomes the
+ * spectrum of this C (computed by the next qrctm_run under its first step, or by
+ * whichever other entry is the first to overwrite C).  delta is always measured
+ * against the spectrum of the previous check, or of this C before the first one. */
 int qrctm_set_env(qrctm_t* h, const double* C, const double* T);
 
 /* One QR-CTMRG iteration, asynchronous on the stream:
@@ -154,6 +161,13 @@ int qrctm_norm_per_site(qrctm_t* h, double* kappa);
  * step scratch (X, P, S); the environment is untouched.  Synchronises. */
 int qrctm_energy_nn(qrctm_t* h, const double* H, double* e_bond, double* rho_out);
 
+/* K3 -> K4 -> K5 alone (the edge renormalisation of PAPER.md:32, "T' = Q^T (T a) Q"), with an arbitrary matrix U
+ * in place of Q:  Tout[m][r][n] = sum U[(j,u),m] T[j,l,J] a[u,l,d,r] U[(J,d),n]   (E3)
+ * U[chi*b][ncols] row-major (HOST or DEVICE), 1 <= ncols <= chi capacity; Tout[ncols][b][ncols] (HOST or DEVICE).
+ * Uses the current T and a; overwrites the step scratch (P, S); the environment is untouched.  Synchronises.
+ * For the sub-step parity tests (an isometry that is not a QR factor). */
+int qrctm_edge_update(qrctm_t* h, const double* U, int ncols, double* Tout);
+
 /* min_k R_kk / max_k R_kk of the last step: a conditioning diagnostic for the
  * uniqueness of Q (DESIGN.md hazard H1).  HOST pointer.  Synchronises. */
 int qrctm_r_diag_ratio(qrctm_t* h, double* ratio);
@@ -200,9 +214,10 @@ int qrctm_qr_f64(void* cuda_stream, int path, int rows, int cols, const double* 
                  double* R, void* work);
 
 /* ---- NEXT-2: the paper's initialisation and warm-up ----
- * PAPER.md:28 "we start from an initial boundary that is not obtained from a
- * previous QR-CTMRG run ... the first one to four steps are done with the standard
- * CTMRG ... bond dimension chi is grown dynamically"; fn.[48] PAPER.md:132.
+ * PAPER.md:28 "performing only a few (1-4) initial warm-up steps using the standard
+ * CTMRG scheme is sufficient. This warm-up phase also enables chi to be dynamically
+ * increased up to the desired target value."; the initial boundary from the bulk
+ * tensors is fn.[48].
  *
  * qrctm_get_chi: the CURRENT environment bond dimension (below the capacity the
  *   handle was created with only between qrctm_init_bulk and the end of the

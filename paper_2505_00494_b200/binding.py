@@ -30,7 +30,7 @@ SYMBOLS = (
     "qrctm_create", "qrctm_workspace_bytes", "qrctm_create_in", "qrctm_destroy", "qrctm_set_stream",
     "qrctm_set_A", "qrctm_set_env", "qrctm_step", "qrctm_run", "qrctm_get_env",
     "qrctm_get_corner_spectrum", "qrctm_get_qr", "qrctm_get_raw", "qrctm_get_a", "qrctm_norm_per_site",
-    "qrctm_r_diag_ratio", "qrctm_energy_nn", "qrctm_set_option", "qrctm_launch_count", "qrctm_get_stage_ms", "qrctm_profile_step",
+    "qrctm_r_diag_ratio", "qrctm_energy_nn", "qrctm_edge_update", "qrctm_set_option", "qrctm_launch_count", "qrctm_get_stage_ms", "qrctm_profile_step",
     "qrctm_gemm_f64", "qrctm_gemm_f64_ws", "qrctm_qr_work_bytes", "qrctm_qr_f64", "qrctm_probe_fp64", "qrctm_last_error",
     "qrctm_version",
     "qrctm_get_chi", "qrctm_init_bulk", "qrctm_eig_step", "qrctm_get_eig", "qrctm_warmup",
@@ -74,6 +74,7 @@ def load_library() -> ctypes.CDLL:
     lib.qrctm_norm_per_site.argtypes = [P, POINTER(c_double)]
     lib.qrctm_r_diag_ratio.argtypes = [P, POINTER(c_double)]
     lib.qrctm_energy_nn.argtypes = [P, P, POINTER(c_double), P]
+    lib.qrctm_edge_update.argtypes = [P, P, c_int, P]
     lib.qrctm_set_option.argtypes = [P, c_int, c_int]
     lib.qrctm_launch_count.argtypes = [P]
     lib.qrctm_launch_count.restype = c_longlong
@@ -192,19 +193,24 @@ class QRCTM:
     def synchronize(self):
         self.stream.synchronize()
 
-    def _order_after_caller(self):
+    def _order_after_caller(self, *tensors):
+        """The handle's stream waits for the caller's current stream; torch CUDA inputs are recorded on the handle's
+        stream, so that the caching allocator does not reuse them while an asynchronous copy is still pending."""
         import torch
         self.stream.wait_stream(torch.cuda.current_stream())
+        for t in tensors:
+            if isinstance(t, torch.Tensor) and t.is_cuda:
+                t.record_stream(self.stream)
 
     def set_A(self, A):
         assert tuple(A.shape) == (self.d,) + (self.D,) * 4
-        self._order_after_caller()
+        self._order_after_caller(A)
         self._check(self.lib.qrctm_set_A(self._h, _ptr(A)))
 
     def set_env(self, C, T):
         n = self.chi_cap
         assert tuple(C.shape) == (n, n) and tuple(T.shape) == (n, self.b, n)
-        self._order_after_caller()
+        self._order_after_caller(C, T)
         self._check(self.lib.qrctm_set_env(self._h, _ptr(C), _ptr(T)))
 
     def step(self):
@@ -306,6 +312,15 @@ class QRCTM:
         rho = np.empty((self.d,) * 4, dtype=np.float64) if return_rho else None
         self._check(self.lib.qrctm_energy_nn(self._h, _ptr(H), byref(e), _ptr(rho)))
         return (e.value, rho) if return_rho else e.value
+
+    def edge_update(self, U, device: bool = False):
+        """T' = (E3) with the (chi*b, n) matrix U in place of Q, from the current T and a."""
+        n = int(U.shape[1])
+        assert int(U.shape[0]) == self.chi * self.b
+        self._order_after_caller(U)
+        out = self._out((n, self.b, n), device)
+        self._check(self.lib.qrctm_edge_update(self._h, _ptr(U), n, _ptr(out)))
+        return out
 
     def r_diag_ratio(self) -> float:
         k = c_double(0.0)

@@ -21,6 +21,11 @@ using namespace qk;
 namespace {
 
 constexpr int kPartialBlocks = 592;   // 4 x 148 blocks for the reduction kernels
+// pinned host scratch (doubles): [0] delta, [2..6] scalars read back by the observables, [32..] the NaN/zero flag
+// (as int), [kPinRho .. kPinRho + kRhoMax) the two-site RDM of qrctm_energy_nn (d <= kEnergyMaxD)
+constexpr int kPinFlag = 32, kPinRho = 64, kEnergyMaxD = 4;
+constexpr int kRhoMax = kEnergyMaxD * kEnergyMaxD * kEnergyMaxD * kEnergyMaxD;
+constexpr int kPinDoubles = kPinRho + kRhoMax;
 constexpr size_t kAlign = 256;
 
 inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
@@ -75,11 +80,12 @@ namespace {
 unsigned long long qr_work_bytes_impl(long long rows, int cols);
 struct EighWork;
 size_t eigh_layout(long long n, int k, char* base, EighWork* w);
+constexpr int kMaxChi = 800;            // form-Q back substitution keeps chi/16 blocks of 4 KB in shared memory
 constexpr int kK8SmemMaxChi = 200;      // above this chi a scratch area for the multi-CTA tridiagonalisation is carved
 
 bool make_layout(int d, int D, int chi, Layout* L) {
   if (d < 1 || D < 1 || chi < 1) return false;
-  if (D > 32 || chi > 1024 || d > 64) return false;                  // sizes this build supports
+  if (D > 32 || chi > kMaxChi || d > 64) return false;               // sizes this build supports
   long long b = (long long)D * D, m = b * chi;
   long long b2 = b * b;
   L->lda_a = (b2 + 15) / 16 * 16;
@@ -89,8 +95,8 @@ bool make_layout(int d, int D, int chi, Layout* L) {
   L->A = take(dbl * d * b2);
   L->a_mat = take(dbl * b2 * L->lda_a);
   L->a2_mat = take(dbl * b2 * L->lda_a);
-  L->LH = take(d <= 4 ? dbl * (size_t)d * d * m * chi : 0);
-  L->rho = take(dbl * 256);
+  L->LH = take(d <= kEnergyMaxD ? dbl * (size_t)d * d * m * chi : 0);
+  L->rho = take(dbl * kRhoMax);
   L->ld1 = ((long long)d * b + 15) / 16 * 16;
   L->ld2 = (b + 15) / 16 * 16;
   L->B1 = take(dbl * b * L->ld1);
@@ -233,7 +239,7 @@ static int create_common(int d, int D, int chi, void* ws, unsigned long long ws_
   }
   bind_views(h);
   void* hp = nullptr;
-  if (cudaMallocHost(&hp, 64 * sizeof(double)) != cudaSuccess) {
+  if (cudaMallocHost(&hp, kPinDoubles * sizeof(double)) != cudaSuccess) {
     cudaGetLastError(); if (h->owns_ws) cudaFree(h->base); delete h; return QRCTM_ERR_CUDA;
   }
   h->h_pinned = static_cast<double*>(hp);
@@ -246,7 +252,7 @@ static int create_common(int d, int D, int chi, void* ws, unsigned long long ws_
       cudaGetLastError(); h->side = nullptr; h->overlap = 0;
     }
   }
-  h->h_flag = reinterpret_cast<int*>(h->h_pinned + 32);       // [64..319] holds the two-site RDM
+  h->h_flag = reinterpret_cast<int*>(h->h_pinned + kPinFlag);
   cudaMemsetAsync(h->flag, 0, 4 * sizeof(int), 0);
   {   // padded operand matrices: the pad columns are zeroed once and never written again
     const size_t b2 = (size_t)h->b * h->b;
@@ -318,9 +324,19 @@ int qrctm_set_env(qrctm_t* h, const double* C, const double* T) {
   return QRCTM_OK;
 }
 
+// The convergence history of a freshly set environment starts at s_prev = spectrum(C0).  qrctm_run computes it lazily
+// (under its first step); every other entry that is about to overwrite C computes it first.
+static int ensure_s0(qrctm* h) {
+  if (!h->need_s0) return QRCTM_OK;
+  int rc = stage_spectrum(h, h->s, 1, h->stream); if (rc) return rc;
+  h->need_s0 = 0;
+  return QRCTM_OK;
+}
+
 int qrctm_step(qrctm_t* h) {
   if (!h) return QRCTM_ERR_INVALID_ARG;
   if (!h->have_A || !h->have_env) return fail(h, QRCTM_ERR_NOT_READY, "set_A and set_env first");
+  { int rc0 = ensure_s0(h); if (rc0) return rc0; }
   h->eig_rows = 0;          // Q is about to be overwritten by K2
   if (!h->use_graph || h->stream == nullptr) { int rc0 = do_step(h, nullptr); if (!rc0) h->warm_steps += 1; return rc0; }
   int rc = run_front(h, nullptr); if (rc) return rc;
@@ -552,7 +568,8 @@ int qrctm_energy_nn(qrctm_t* h, const double* H, double* e_bond, double* rho_out
   if (!h || !H || !e_bond) return h ? fail(h, QRCTM_ERR_INVALID_ARG, "null argument") : QRCTM_ERR_INVALID_ARG;
   if (!h->have_A || !h->have_env) return fail(h, QRCTM_ERR_NOT_READY, "set_A and set_env first");
   const int d = h->d, chi = h->chi;
-  if (d > 4) return fail(h, QRCTM_ERR_INVALID_ARG, "qrctm_energy_nn supports d <= 4");
+  static_assert(kPinRho + kRhoMax <= kPinDoubles, "pinned RDM area");
+  if (d > kEnergyMaxD) return fail(h, QRCTM_ERR_INVALID_ARG, "qrctm_energy_nn supports d <= 4");
   if (is_device_ptr(H) || (rho_out && is_device_ptr(rho_out))) return fail(h, QRCTM_ERR_INVALID_ARG, "H, rho: host pointers");
   const long long m = h->m, nlh = m * chi;
   int rc;
@@ -574,9 +591,9 @@ int qrctm_energy_nn(qrctm_t* h, const double* H, double* e_bond, double* rho_out
     for (int q = p; q < d2; ++q) {
       rc = reduce_dot(h, h->LH + (size_t)p * nlh, h->LH + (size_t)q * nlh, nlh, h->rho + p * d2 + q); if (rc) return rc;
     }
-  CU(h, cudaMemcpyAsync(h->h_pinned + 64, h->rho, sizeof(double) * d2 * d2, cudaMemcpyDeviceToHost, h->stream));
+  CU(h, cudaMemcpyAsync(h->h_pinned + kPinRho, h->rho, sizeof(double) * d2 * d2, cudaMemcpyDeviceToHost, h->stream));
   CU(h, cudaStreamSynchronize(h->stream));
-  const double* r = h->h_pinned + 64;
+  const double* r = h->h_pinned + kPinRho;
   double num = 0.0, den = 0.0;
   for (int s1 = 0; s1 < d; ++s1) for (int s1p = 0; s1p < d; ++s1p)
     for (int s2 = 0; s2 < d; ++s2) for (int s2p = 0; s2p < d; ++s2p) {
@@ -588,6 +605,19 @@ int qrctm_energy_nn(qrctm_t* h, const double* H, double* e_bond, double* rho_out
     }
   if (!(den != 0.0)) return fail(h, QRCTM_ERR_NUMERIC, "zero two-site norm");
   *e_bond = num / den;
+  return QRCTM_OK;
+}
+
+int qrctm_edge_update(qrctm_t* h, const double* U, int ncols, double* Tout) {
+  if (!h || !U || !Tout) return h ? fail(h, QRCTM_ERR_INVALID_ARG, "null argument") : QRCTM_ERR_INVALID_ARG;
+  if (!h->have_A || !h->have_env) return fail(h, QRCTM_ERR_NOT_READY, "set_A and set_env first");
+  if (ncols < 1 || ncols > h->chi_cap) return fail(h, QRCTM_ERR_INVALID_ARG, "ncols out of range");
+  const long long mo = (long long)ncols * h->b;
+  CU(h, copy_in(h->E, U, (size_t)h->m * ncols, h->stream));
+  int rc = stage_half_absorb(h, h->E, h->T, h->P, ncols); if (rc) return rc;
+  rc = stage_absorb_a(h, h->P, h->S, 0, nullptr, ncols); if (rc) return rc;
+  rc = stage_project(h, h->S, h->E, h->W, ncols); if (rc) return rc;
+  CU(h, copy_out(Tout, h->W, (size_t)mo * ncols, h->stream));
   return QRCTM_OK;
 }
 
@@ -604,6 +634,7 @@ int qrctm_r_diag_ratio(qrctm_t* h, double* ratio) {
 int qrctm_profile_step(qrctm_t* h, float* ms) {
   if (!h || !ms) return QRCTM_ERR_INVALID_ARG;
   if (!h->have_A || !h->have_env) return fail(h, QRCTM_ERR_NOT_READY, "set_A and set_env first");
+  { int rc0 = ensure_s0(h); if (rc0) return rc0; }
   cudaEvent_t ev[QRCTM_NSTAGE + 1];
   for (int i = 0; i <= QRCTM_NSTAGE; ++i) CU(h, cudaEventCreate(&ev[i]));
   int rc = do_step(h, ev);
@@ -641,7 +672,7 @@ unsigned long long qrctm_qr_work_bytes(int rows, int cols) { return qr_work_byte
 
 int qrctm_qr_f64(void* cuda_stream, int path, int rows, int cols, const double* X, double* Q, double* R,
                  void* work) {
-  if (!X || !Q || !R || !work || rows < 1 || cols < 1 || cols > rows || path < 0 || path > 2)
+  if (!X || !Q || !R || !work || rows < 1 || cols < 1 || cols > rows || cols > kMaxChi || path < 0 || path > 2)
     return QRCTM_ERR_INVALID_ARG;
   cudaError_t e;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
@@ -652,9 +683,10 @@ int qrctm_qr_f64(void* cuda_stream, int path, int rows, int cols, const double* 
 
 int qrctm_probe_fp64(int kind, int iters, double* tflops) {
   if (!tflops || iters < 1 || (kind != 0 && kind != 1)) return QRCTM_ERR_INVALID_ARG;
-  cudaDeviceProp p;
-  if (cudaGetDeviceProperties(&p, 0) != cudaSuccess) { cudaGetLastError(); return QRCTM_ERR_CUDA; }
-  const int blocks = p.multiProcessorCount * 2, threads = 256;
+  int dev = 0, nsm = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess ||
+      cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) { cudaGetLastError(); return QRCTM_ERR_CUDA; }
+  const int blocks = nsm * 2, threads = 256;
   double* out = nullptr;
   if (cudaMalloc(&out, sizeof(double) * blocks * threads) != cudaSuccess) { cudaGetLastError(); return QRCTM_ERR_CUDA; }
   cudaEvent_t a, b; cudaEventCreate(&a); cudaEventCreate(&b);
@@ -756,7 +788,8 @@ int qrctm_eig_step(qrctm_t* h, int chi_new) {
   if (chi_new == 0) chi_new = h->chi;
   if (chi_new < 1 || chi_new > h->chi_cap || chi_new > h->m) return fail(h, QRCTM_ERR_INVALID_ARG, "chi_new out of range");
   if (h->m > EIGH_MAX_N) return fail(h, QRCTM_ERR_INVALID_ARG, "eigen step supports chi*D^2 <= 14000");
-  int rc = stage_eig_step(h, chi_new); if (rc) return rc;
+  int rc = ensure_s0(h); if (rc) return rc;
+  rc = stage_eig_step(h, chi_new); if (rc) return rc;
   rc = check_flag(h); if (rc) return rc;
   CU(h, cudaMemsetAsync(h->s_prev, 0, sizeof(double) * h->chi_cap, h->stream));
   h->need_s0 = 1;
@@ -818,6 +851,7 @@ int qrctm_shard_front(qrctm_t* h, int rank, int nranks) {
   if (!h) return QRCTM_ERR_INVALID_ARG;
   if (!h->have_A || !h->have_env) return fail(h, QRCTM_ERR_NOT_READY, "set_A and set_env first");
   if (nranks < 1 || rank < 0 || rank >= nranks) return fail(h, QRCTM_ERR_INVALID_ARG, "rank / nranks");
+  { int rc0 = ensure_s0(h); if (rc0) return rc0; }
   h->eig_rows = 0;
   const int chi = h->chi, b = h->b; const long long m = h->m, bc = (long long)b * chi;
   int m0, m1; shard_range(chi, rank, nranks, &m0, &m1);

@@ -109,12 +109,15 @@ int stage_corner_accel(qrctm* h) {
   return QRCTM_OK;
 }
 
-// K6' (E5)+(E4'): Z = half_absorb(X), C~ = Z.a, Y = C~ Q, C' = Q^T Y
+// K6' (E5)+(E4'): Z = half_absorb(X), C~ = Z.a, Y = C~ Q, C' = Q^T Y.  K4's epilogue writes C~ transposed,
+// S~[(k,r),(J,d)] = C~[(J,d),(k,r)], i.e. as the K x M operand of Y = C~ Q, so that this m x m x chi product runs on
+// the same bulk-tensor-copy kernel (and stream-K schedule) as K5.
 int stage_corner_enlarged(qrctm* h) {
   const int chi = h->chi; const long long m = h->m;
   int rc = stage_half_absorb(h, h->X, h->T, h->P); if (rc) return rc;
-  rc = stage_absorb_a(h, h->P, h->S, 0); if (rc) return rc;          // S = C~[(J,d),(k,r)]
-  GemmCall c1{h->S, m, 0, h->Q, chi, h->W, plain_map(chi), IndexMap{1, 1, 0}, (int)m, chi, (int)m, 0};
+  rc = stage_absorb_a(h, h->P, h->S, 1); if (rc) return rc;          // S = C~^T
+  GemmCall c1{h->S, m, 1, h->Q, chi, h->W, plain_map(chi), IndexMap{1, 1, 0}, (int)m, chi, (int)m, 0};
+  c1.epi = 1;
   GEMM(h, c1);
   GemmCall c2{h->Q, chi, 1, h->W, chi, h->Cn, plain_map(chi), IndexMap{1, 1, 0}, chi, chi, (int)m, 0};
   GEMM(h, c2);

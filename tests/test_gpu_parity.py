@@ -147,9 +147,14 @@ def test_single_step_parity(d, D, chi, seed):
     assert abs(out["ratio"] - d_.min() / d_.max()) < 1e-10
 
 
-@pytest.mark.parametrize("d,D,chi,seed", [(2, 2, 8, 0), (2, 3, 12, 1)])
+@pytest.mark.parametrize("d,D,chi,seed", [(2, 2, 8, 0), (2, 3, 12, 1), (2, 3, 7, 8),
+                                          (2, 4, 64, 2), (2, 5, 100, 3), (2, 7, 196, 4)])   # ... cfg2, cfg3a, cfg4
 def test_single_step_enlarged_corner_mode(d, D, chi, seed):
+    """K6': the enlarged corner C~ (E5) and C' = Q^T C~ Q (E4'), "the standard diagram on the left-hand side" of
+    Fig. 1(f), up to BASELINE.json's full sizes (cfg4: C~ is 9604 x 9604), against the oracle's
+    enlarged-corner branch and against the accelerated update (E4)."""
     out, s, (Cr, Tr, Co, To) = _one_step(d, D, chi, seed, corner_mode=1)
+    assert rel(out["raw"][0], s["Cn"]) < 1e-11 and rel(out["raw"][1], s["Tn"]) < 1e-11
     assert rel(out["C"], Co) < 1e-11 and rel(out["T"], To) < 1e-11
     acc, _, _ = _one_step(d, D, chi, seed, corner_mode=0)
     assert rel(out["raw"][0], acc["raw"][0]) < 1e-12            # Fig. 1(f): (E4) == (E4')
@@ -167,9 +172,27 @@ def test_step_is_deterministic_bitwise():
     assert np.array_equal(a["C"], b["C"]) and np.array_equal(a["T"], b["T"])
 
 
-def test_edge_update_with_arbitrary_isometry():
-    """K3-K5 alone with an isometry that is not a QR factor: feed the
-    library an environment whose c~ has that isometry as its Q."""
+@pytest.mark.parametrize("d,D,chi,ncols,seed", [(2, 2, 6, 6, 3), (2, 3, 36, 36, 1), (2, 3, 20, 14, 2), (3, 2, 9, 5, 4),
+                                                (2, 4, 64, 64, 5), (2, 5, 100, 100, 6)])
+def test_edge_update_with_arbitrary_isometry(d, D, chi, ncols, seed):
+    """K3-K5 alone (qrctm_edge_update) with a seeded random isometry that is NOT a QR factor of c~,
+    square and with fewer columns than chi, against the oracle's (E3)."""
+    A, C0, T0 = gen_config(d, D, chi, seed)
+    U = random_isometry(chi * D * D, ncols, seed + 50)
+    h = pkg.QRCTM(d, D, chi)
+    h.set_A(A); h.set_env(C0, T0)
+    C, T = o.normalize(C0, T0)
+    Tn = h.edge_update(U)
+    assert Tn.shape == (ncols, D * D, ncols)
+    assert rel(Tn, o.edge_update(U, T, o.build_a(A))) < 1e-13
+    Tn2 = h.edge_update(torch_dev(U), device=True).cpu().numpy()          # device pointers
+    assert np.array_equal(Tn, Tn2)
+    C1, T1 = h.get_env()
+    assert rel(C1, C) < 1e-14 and rel(T1, T) < 1e-14                      # environment untouched
+    h.close()
+
+
+def test_gpu_step_edge_is_the_oracle_contraction_of_its_own_q():
     d, D, chi = 2, 2, 6
     A, C0, T0 = gen_config(d, D, chi, 3)
     h = pkg.QRCTM(d, D, chi)
@@ -177,7 +200,7 @@ def test_edge_update_with_arbitrary_isometry():
     Q, R = h.get_qr()
     _, Tn = h.get_raw()
     C, T = o.normalize(C0, T0)
-    assert rel(Tn, o.edge_update(Q, T, o.build_a(A))) < 1e-13   # oracle contraction of the GPU's own Q
+    assert rel(Tn, o.edge_update(Q, T, o.build_a(A))) < 1e-13
     h.close()
 
 
@@ -439,10 +462,11 @@ def test_energy_nn_matches_oracle(d, D, chi, seed, steps):
     h.close()
 
 
-@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3a"])
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3a", "cfg3b", "cfg4"])
 def test_long_run_parity_at_baseline_iteration_counts(name):
-    """BASELINE.json: cfg1 runs to tol 1e-10 or 500 iterations, cfg2 300 iterations.  North-star bar for the run:
-    relative error <= 1e-9 on the norm per site and on the top-10 normalised corner eigenvalues."""
+    """BASELINE.json: cfg1 runs to tol 1e-10 or 500 iterations, cfg2 300, cfg3a/cfg3b 200 each, cfg4 100 iterations
+    (cfg0's run: test_cfg0_*).  North-star bar for the run, on all five configs: relative error <= 1e-9 on the norm
+    per site and on the top-10 normalised corner eigenvalues (iteration until convergence: PAPER.md:26)."""
     c = CONFIGS[name]
     A, C0, T0 = gen_config(c["d"], c["D"], c["chi"], c["seed"])
     a = o.build_a(A)

@@ -363,3 +363,17 @@ def test_rdm2_trace_is_the_two_site_norm_network():
     LH = o.half_network(C0, T0, a)
     assert abs(np.einsum("aabb->", rho) / np.sum(LH * LH) - 1) < 1e-13
     assert np.allclose(rho, rho.transpose(2, 3, 0, 1), atol=1e-14 * np.abs(rho).max())   # site exchange
+
+
+def test_normalize_is_frobenius_and_symmetrising():
+    """Reading A5: after a step C and T are symmetrised and divided by their FROBENIUS norms (P10 alone would pass with
+    any homogeneous norm).  Pinned on generic, non-symmetric inputs against the definitions written out."""
+    g = np.random.default_rng(77)
+    Cn = g.standard_normal((5, 5)); Tn = g.standard_normal((5, 4, 5))
+    C, T = o.normalize(Cn, Tn)
+    assert abs(np.sqrt(np.sum(C * C)) - 1) < 1e-15 and abs(np.sqrt(np.sum(T * T)) - 1) < 1e-15
+    Cs = 0.5 * (Cn + Cn.T); Ts = 0.5 * (Tn + Tn.transpose(2, 1, 0))
+    assert np.allclose(C, Cs / np.sqrt((Cs ** 2).sum()), rtol=0, atol=1e-16)
+    assert np.allclose(T, Ts / np.sqrt((Ts ** 2).sum()), rtol=0, atol=1e-16)
+    # and it is none of the other usual norms: max-abs, spectral, sum-abs
+    assert abs(np.max(np.abs(C)) - 1) > 1e-3 and abs(np.linalg.norm(C, 2) - 1) > 1e-3 and abs(np.abs(T).sum() - 1) > 1e-3
