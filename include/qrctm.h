@@ -62,10 +62,14 @@ enum {
   QRCTM_OPT_CHECK_EVERY = 3, /* qrctm_run computes the corner spectrum / delta every n steps, default 1 */
   QRCTM_OPT_GEMM_PATH = 4,   /* 0 = FP64 tensor-core (DMMA) tiles [default], 1 = plain DFMA reference kernel */
   QRCTM_OPT_TIME_STAGES = 5, /* 1 = qrctm_run records CUDA events around every stage of every step (default 0) */
-  QRCTM_OPT_QR_PATH = 6,     /* 0 [default] = automatic: whole-matrix register-resident cluster kernel when c~ fits
-                                (chi <= 112, rows <= 16 x 160..384), else blocked compact-WY with the cluster panel
-                                kernel; 1 = one kernel launch per Householder reflector (slow reference path for
-                                cross-checking); 2 = always the blocked path */
+  QRCTM_OPT_QR_PATH = 6,     /* 0 [default] = automatic: CholeskyQR2 (two Gram / Cholesky / triangular-inverse passes, the
+                                O(m chi^2) work on the DMMA GEMM) when 48 <= chi <= 208, checked on the device
+                                (||Q1^T Q1 - I||_F <= 1e-4 and no pivot breakdown) and replaced by the Householder path
+                                when the check fails (ill-conditioned or rank-deficient c~); Householder (as 3) outside
+                                that range; 1 = one kernel launch per Householder reflector (slow reference path for
+                                cross-checking); 2 = blocked compact-WY Householder with the cluster panel kernel;
+                                3 = Householder automatic (whole-matrix register-resident cluster kernel when c~ fits:
+                                chi <= 112, rows <= 16 x 160..384, else 2); 4 = CholeskyQR2 for any chi <= 208 */
   QRCTM_OPT_OVERLAP_CHECK = 7, /* 1 [default] = qrctm_run overlaps the convergence check of step k (side stream) with
                                 K1..K6 of step k+1; results are identical, Q/R/raw buffers then hold the factors of
                                 the last *started* iteration.  0 = strictly serial */
@@ -207,11 +211,23 @@ int qrctm_gemm_f64_ws(void* cuda_stream, int path, int transA, int M, int N, int
 
 /* Stand-alone QR entry (K2): factor X[rows][cols] (DEVICE, row-major, cols <=
  * rows) into Q[rows][cols], R[cols][cols] with diag(R) >= 0 (path: see
- * QRCTM_OPT_QR_PATH). work must hold
+ * QRCTM_OPT_QR_PATH; path 0 synchronises the stream once to read the device-side accuracy verdict). work must hold
  * qrctm_qr_work_bytes(rows, cols) bytes (DEVICE). */
 unsigned long long qrctm_qr_work_bytes(int rows, int cols);
 int qrctm_qr_f64(void* cuda_stream, int path, int rows, int cols, const double* X, double* Q,
                  double* R, void* work);
+
+/* Stand-alone entry of the n x n factorisation inside CholeskyQR2 (K2, csrc/cholqr.cuh; for the sub-step parity
+ * tests): G[n][n] symmetric positive definite (DEVICE; its lower triangle is read), n <= 208.
+ *   R[n][n]    = chol(G)^T, upper triangular (G = R^T R), zeros below the diagonal            (DEVICE)
+ *   Rinv[n][n] = R^-1, upper triangular                                                       (DEVICE)
+ *   status[0]  = 1 if a pivot was not positive and finite (the factor is then meaningless)    (DEVICE int)
+ *   dev[0]     = ||G - I||_F                                                                  (DEVICE)
+ *   prof       = NULL, or 8 DEVICE long longs: SM cycles of the kernel's phases (load; diagonal blocks; panels;
+ *                trailing updates; write R; diagonal-block inverses; inverse; write R^-1).
+ * One CTA; asynchronous on the stream. */
+int qrctm_chol_inv_f64(void* cuda_stream, int n, const double* G, double* R, double* Rinv, int* status, double* dev,
+                       long long* prof);
 
 /* ---- NEXT-2: the paper's initialisation and warm-up ----
  * PAPER.md:28 "performing only a few (1-4) initial warm-up steps using the standard

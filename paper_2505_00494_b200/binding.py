@@ -34,7 +34,7 @@ SYMBOLS = (
     "qrctm_gemm_f64", "qrctm_gemm_f64_ws", "qrctm_qr_work_bytes", "qrctm_qr_f64", "qrctm_probe_fp64", "qrctm_last_error",
     "qrctm_version",
     "qrctm_get_chi", "qrctm_init_bulk", "qrctm_eig_step", "qrctm_get_eig", "qrctm_warmup",
-    "qrctm_eigh_work_bytes", "qrctm_eigh_top_f64",
+    "qrctm_eigh_work_bytes", "qrctm_eigh_top_f64", "qrctm_chol_inv_f64",
     "qrctm_shard_range", "qrctm_shard_front", "qrctm_shard_buffers", "qrctm_shard_finish",
 )
 
@@ -88,6 +88,7 @@ def load_library() -> ctypes.CDLL:
     lib.qrctm_qr_work_bytes.restype = c_ulonglong
     lib.qrctm_qr_f64.argtypes = [P, c_int, c_int, c_int, P, P, P, P]
     lib.qrctm_probe_fp64.argtypes = [c_int, c_int, POINTER(c_double)]
+    lib.qrctm_chol_inv_f64.argtypes = [P, c_int, P, P, P, P, P, P]
     lib.qrctm_get_chi.argtypes = [P, POINTER(c_int), POINTER(c_int)]
     lib.qrctm_init_bulk.argtypes = [P]
     lib.qrctm_eig_step.argtypes = [P, c_int]
@@ -387,6 +388,26 @@ def qr_f64(X, path: int = 0):
         raise QrctmError(f"qrctm_qr_f64 failed: {rc}")
     torch.cuda.current_stream().synchronize()
     return Q, R
+
+
+def chol_inv_f64(G, profile: bool = False):
+    """(R, Rinv, status, dev[, cycles]) of a symmetric positive definite torch CUDA float64 matrix (n <= 208) through
+    qrctm_chol_inv_f64: G = R^T R with R upper triangular."""
+    import torch
+    lib = load_library()
+    n = G.shape[0]
+    R = torch.empty((n, n), dtype=torch.float64, device="cuda")
+    Ri = torch.empty((n, n), dtype=torch.float64, device="cuda")
+    st = torch.zeros(1, dtype=torch.int32, device="cuda")
+    dev = torch.zeros(1, dtype=torch.float64, device="cuda")
+    prof = torch.zeros(8, dtype=torch.int64, device="cuda") if profile else None
+    rc = lib.qrctm_chol_inv_f64(c_void_p(torch.cuda.current_stream().cuda_stream), n, _ptr(G.contiguous()), _ptr(R), _ptr(Ri),
+                                c_void_p(st.data_ptr()), _ptr(dev), c_void_p(prof.data_ptr()) if profile else None)
+    if rc != QRCTM_OK:
+        raise QrctmError(f"qrctm_chol_inv_f64 failed: {rc}")
+    torch.cuda.current_stream().synchronize()
+    out = (R, Ri, int(st.item()), float(dev.item()))
+    return out + (prof.cpu().numpy(),) if profile else out
 
 
 def shard_range(chi: int, rank: int, nranks: int):

@@ -120,7 +120,7 @@ long long eigh_top(cudaStream_t st, int n, int k, double* W, double* lam, double
   launches += 4;
   *err = cudaGetLastError();
   if (*err != cudaSuccess) return -1;
-  long long nq = qr_factor_blocked(st, 0, n, k, wk.Z, U, wk.R, wk.qr, err);
+  long long nq = qr_factor_blocked(st, 3, n, k, wk.Z, U, wk.R, wk.qr, err);      // Householder: clusters of near-parallel vectors
   if (nq < 0) return -1;
   launches += nq;
   if (n >= 3) {

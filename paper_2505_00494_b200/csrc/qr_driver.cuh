@@ -13,6 +13,9 @@ constexpr int QR_MAX_PARTS = 320;
 struct QrWork {     // carved out of the caller's work buffer
   double *V, *Vc, *tau, *Tfac, *W1, *W2, *splitk, *part, *Vct, *Gq, *Xq;
   size_t splitk_elems;
+  // CholeskyQR2 (cholqr.cuh): R1 (upper), R1^-1, L2 (lower), R2^-1, deviations, status words
+  double *cR1, *cRi1, *cL2, *cRi2, *cdev;
+  int* cstat;       // [0] pass-1 breakdown, [1] pass-2 breakdown, [2] verdict: 1 = discard, take the Householder path
 };
 
 size_t qr_layout(long long rows, int n, char* base, QrWork* w) {
@@ -25,7 +28,12 @@ size_t qr_layout(long long rows, int n, char* base, QrWork* w) {
   size_t oS = take(sk);
   size_t oP = take((size_t)QR_MAX_PARTS * QR_NB_REG * n);
   size_t oVt = take((size_t)rows * n), oG = take((size_t)n * n), oX = take((size_t)n * n);
+  size_t oc1 = take((size_t)n * n), oc2 = take((size_t)n * n), oc3 = take((size_t)n * n), oc4 = take((size_t)n * n);
+  size_t ocd = take(8), ocs = take(8);
   if (w) {
+    w->cR1 = reinterpret_cast<double*>(base + oc1); w->cRi1 = reinterpret_cast<double*>(base + oc2);
+    w->cL2 = reinterpret_cast<double*>(base + oc3); w->cRi2 = reinterpret_cast<double*>(base + oc4);
+    w->cdev = reinterpret_cast<double*>(base + ocd); w->cstat = reinterpret_cast<int*>(base + ocs);
     w->V = reinterpret_cast<double*>(base + oV); w->Vc = reinterpret_cast<double*>(base + oVc);
     w->tau = reinterpret_cast<double*>(base + otau); w->Tfac = reinterpret_cast<double*>(base + oT);
     w->W1 = reinterpret_cast<double*>(base + oW1); w->W2 = reinterpret_cast<double*>(base + oW2);
@@ -375,9 +383,174 @@ long long qr_factor_fullreg_t(cudaStream_t st, long long rows, int n, const doub
   return *err == cudaSuccess ? launches : -1;
 }
 
-// qr_path: 0 = automatic (whole-matrix register kernel when it fits, else blocked), 2 = always blocked
+// How the caller wants the "CholeskyQR2 not accurate enough -> Householder" decision taken (it is made on the device):
+//   mode 0: never fall back (the verdict word is still written);
+//   mode 1: the host reads the verdict (synchronises the stream) and launches the Householder path if needed;
+//   mode 2: the stream is being captured: the Householder path goes into the body of a conditional IF node of the
+//           capturing graph (captured on the stream `aux`), executed only when the verdict says so;
+//   mode 3: direct launches without a host round trip: a small graph {set condition; IF node with the Householder
+//           path as its body} is built once (captured on `aux`), kept in *cache by the caller, and launched on the
+//           stream after the CholeskyQR2 kernels.
+struct QrFallback { int mode; cudaStream_t aux; cudaGraphExec_t* cache; };
+
+long long qr_factor_householder(cudaStream_t st, int qr_path, long long rows, int n, const double* X, double* Q,
+                                double* R, void* work, cudaError_t* err);
+
+// On the capturing stream s: enqueue the kernel that sets the condition from the verdict word and append an IF node
+// after it; later work captured on s depends on that node.  Returns the (empty) body graph of the IF node.
+cudaError_t cholqr_append_cond(cudaStream_t s, const int* verdict, cudaGraph_t* body) {
+  cudaStreamCaptureStatus cs; cudaGraph_t g = nullptr; const cudaGraphNode_t* deps = nullptr; size_t nd = 0;
+  unsigned long long id = 0;
+  cudaError_t e = cudaStreamGetCaptureInfo(s, &cs, &id, &g, &deps, &nd);
+  if (e != cudaSuccess) return e;
+  if (cs != cudaStreamCaptureStatusActive || !g) return cudaErrorInvalidValue;
+  cudaGraphConditionalHandle hnd;
+  e = cudaGraphConditionalHandleCreate(&hnd, g, 0, cudaGraphCondAssignDefault);
+  if (e != cudaSuccess) return e;
+  cholqr_set_cond_kernel<<<1, 32, 0, s>>>(hnd, verdict);
+  e = cudaStreamGetCaptureInfo(s, &cs, &id, &g, &deps, &nd);
+  if (e != cudaSuccess) return e;
+  cudaGraphNodeParams prm = {};
+  prm.type = cudaGraphNodeTypeConditional;
+  prm.conditional.handle = hnd; prm.conditional.type = cudaGraphCondTypeIf; prm.conditional.size = 1;
+  cudaGraphNode_t cn;
+  e = cudaGraphAddNode(&cn, g, deps, nd, &prm);
+  if (e != cudaSuccess) return e;
+  e = cudaStreamUpdateCaptureDependencies(s, &cn, 1, cudaStreamSetCaptureDependencies);
+  if (e != cudaSuccess) return e;
+  *body = prm.conditional.phGraph_out[0];
+  return cudaSuccess;
+}
+
+// Capture the Householder path into `body` on the stream aux.
+cudaError_t cholqr_capture_body(cudaStream_t aux, cudaGraph_t body, long long rows, int n, const double* X, double* Q,
+                                double* R, void* work) {
+  cudaError_t e = cudaStreamBeginCaptureToGraph(aux, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
+  if (e != cudaSuccess) return e;
+  cudaError_t eh = cudaSuccess;
+  const long long nh = qr_factor_householder(aux, 0, rows, n, X, Q, R, work, &eh);
+  cudaGraph_t tmp = nullptr;
+  e = cudaStreamEndCapture(aux, &tmp);
+  if (nh < 0) return eh != cudaSuccess ? eh : cudaErrorUnknown;
+  return e;
+}
+
+constexpr int kCholqrMinN = 48;
+constexpr double kCholqrDevMax = 1e-4;     // ||Q1^T Q1 - I||_F above this: cond(c~)^2 eps is not small, discard
+
+cudaError_t chol_inv_attr() {
+  static bool attr = false;
+  if (attr) return cudaSuccess;
+  cudaError_t e = cudaFuncSetAttribute(chol_inv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)chol_smem_bytes(CHOL_MAX_N));
+  if (e == cudaSuccess) attr = true;
+  return e;
+}
+
+// CholeskyQR2 (cholqr.cuh).  Returns launches on the main path, -1 on error, -2 if the shape does not fit.
+long long qr_factor_cholqr2(cudaStream_t st, long long rows, int n, const double* X, double* Q, double* R, void* work,
+                            cudaError_t* err, QrFallback fb) {
+  if (n > CHOL_MAX_N || rows < n) return -2;
+  QrWork wk;
+  qr_layout(rows, n, static_cast<char*>(work), &wk);
+  *err = chol_inv_attr();
+  if (*err != cudaSuccess) return -1;
+  const size_t smem = chol_smem_bytes(n);
+  long long launches = 0;
+  int nl;
+  const dim3 tg((unsigned)((rows + 31) / 32), (n + 31) / 32), tb(32, 8);
+  // pass 1
+  nl = launch_gemm(st, 0, GemmCall{X, n, 1, X, n, wk.Gq, plain_map(n), IndexMap{1, 1, 0}, n, n, (int)rows, 0},
+                   wk.splitk, wk.splitk_elems, err);
+  if (nl < 0) return -1;
+  launches += nl;
+  chol_inv_kernel<<<1, CHOL_NT, smem, st>>>(wk.Gq, n, wk.cR1, nullptr, wk.cRi1, wk.cstat, wk.cdev, nullptr, nullptr, 0.0, nullptr);
+  transpose_tall_kernel<<<tg, tb, 0, st>>>(X, rows, n, wk.Vct);
+  launches += 2;
+  nl = launch_gemm(st, 0, GemmCall{wk.Vct, rows, 1, wk.cRi1, n, wk.V, plain_map(n), IndexMap{1, 1, 0}, (int)rows, n, n, 0},
+                   wk.splitk, wk.splitk_elems, err);                                   // Q1 = X R1^-1
+  if (nl < 0) return -1;
+  launches += nl;
+  // pass 2
+  nl = launch_gemm(st, 0, GemmCall{wk.V, n, 1, wk.V, n, wk.Gq, plain_map(n), IndexMap{1, 1, 0}, n, n, (int)rows, 0},
+                   wk.splitk, wk.splitk_elems, err);
+  if (nl < 0) return -1;
+  launches += nl;
+  chol_inv_kernel<<<1, CHOL_NT, smem, st>>>(wk.Gq, n, nullptr, wk.cL2, wk.cRi2, wk.cstat + 1, wk.cdev + 1, wk.cstat,
+                                            wk.cstat + 2, kCholqrDevMax, nullptr);
+  transpose_tall_kernel<<<tg, tb, 0, st>>>(wk.V, rows, n, wk.Vct);
+  launches += 2;
+  nl = launch_gemm(st, 0, GemmCall{wk.Vct, rows, 1, wk.cRi2, n, Q, plain_map(n), IndexMap{1, 1, 0}, (int)rows, n, n, 0},
+                   wk.splitk, wk.splitk_elems, err);                                   // Q = Q1 R2^-1
+  if (nl < 0) return -1;
+  launches += nl;
+  nl = launch_gemm(st, 0, GemmCall{wk.cL2, n, 1, wk.cR1, n, R, plain_map(n), IndexMap{1, 1, 0}, n, n, n, 0},
+                   wk.splitk, wk.splitk_elems, err);                                   // R = R2 R1 = L2^T R1
+  if (nl < 0) return -1;
+  launches += nl;
+  *err = cudaGetLastError();
+  if (*err != cudaSuccess) return -1;
+  if (fb.mode == 1) {
+    int verdict = 0;
+    *err = cudaMemcpyAsync(&verdict, wk.cstat + 2, sizeof(int), cudaMemcpyDeviceToHost, st);
+    if (*err == cudaSuccess) *err = cudaStreamSynchronize(st);
+    if (*err != cudaSuccess) return -1;
+    if (verdict) {
+      long long nh = qr_factor_householder(st, 0, rows, n, X, Q, R, work, err);
+      if (nh < 0) return -1;
+      launches += nh;
+    }
+  } else if (fb.mode == 2) {
+    cudaGraph_t body = nullptr;
+    *err = cholqr_append_cond(st, wk.cstat + 2, &body);
+    if (*err != cudaSuccess) return -1;
+    launches += 1;
+    *err = cholqr_capture_body(fb.aux, body, rows, n, X, Q, R, work);
+    if (*err != cudaSuccess) return -1;
+  } else if (fb.mode == 3) {
+    if (!*fb.cache) {
+      cudaGraph_t g = nullptr, body = nullptr, tmp = nullptr;
+      *err = cudaGraphCreate(&g, 0);
+      if (*err != cudaSuccess) return -1;
+      *err = cudaStreamBeginCaptureToGraph(fb.aux, g, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
+      if (*err == cudaSuccess) {
+        const cudaError_t e1 = cholqr_append_cond(fb.aux, wk.cstat + 2, &body);
+        const cudaError_t e2 = cudaStreamEndCapture(fb.aux, &tmp);
+        *err = e1 != cudaSuccess ? e1 : e2;
+      }
+      if (*err == cudaSuccess) *err = cholqr_capture_body(fb.aux, body, rows, n, X, Q, R, work);
+      if (*err == cudaSuccess) *err = cudaGraphInstantiate(fb.cache, g, 0);
+      cudaGraphDestroy(g);
+      if (*err != cudaSuccess) { *fb.cache = nullptr; return -1; }
+    }
+    *err = cudaGraphLaunch(*fb.cache, st);
+    if (*err != cudaSuccess) return -1;
+    launches += 1;
+  }
+  return launches;
+}
+
+// qr_path: 0 = automatic (CholeskyQR2 when c~ has kCholqrMinN..CHOL_MAX_N columns, Householder when that is discarded
+// or does not fit), 2 = Householder blocked path only, 3 = Householder automatic (whole-matrix register kernel when it
+// fits, else blocked) -- the round-1 default, 4 = CholeskyQR2 whenever it fits (any n <= CHOL_MAX_N)
 long long qr_factor_blocked(cudaStream_t st, int qr_path, long long rows, int n, const double* X, double* Q,
-                            double* R, void* work, cudaError_t* err) {
+                            double* R, void* work, cudaError_t* err, QrFallback fb = QrFallback{1, nullptr, nullptr}) {
+  // below ~48 columns the whole QR is launch-latency bound and the single-launch register-resident Householder
+  // kernel wins (cfg0: 44 us against 71 us, cfg1: 119 against 133; measured, profiles/r2_k2_cholqr2.md)
+  if (qr_path == 0 && n >= kCholqrMinN) {
+    const long long nl = qr_factor_cholqr2(st, rows, n, X, Q, R, work, err, fb);
+    if (nl != -2) return nl;
+  }
+  if (qr_path == 4) {
+    const long long nl = qr_factor_cholqr2(st, rows, n, X, Q, R, work, err, fb);
+    if (nl != -2) return nl;
+  }
+  return qr_factor_householder(st, qr_path == 3 ? 0 : qr_path, rows, n, X, Q, R, work, err);
+}
+
+// Householder paths.  qr_path: 0 = whole-matrix register kernel when it fits, else blocked; 2 = always blocked
+long long qr_factor_householder(cudaStream_t st, int qr_path, long long rows, int n, const double* X, double* Q,
+                                double* R, void* work, cudaError_t* err) {
   if (qr_path == 0 && n <= 112) {
     QrWork wk;
     qr_layout(rows, n, static_cast<char*>(work), &wk);

@@ -13,6 +13,7 @@
 #include "gemm_f64.cuh"
 #include "kernels_misc.cuh"
 #include "qr_f64.cuh"
+#include "cholqr.cuh"
 #include "spectrum.cuh"
 #include "eigh.cuh"
 
@@ -56,9 +57,11 @@ struct qrctm {
   cudaEvent_t ev[QRCTM_NSTAGE + 2];
   bool have_ev;
   cudaGraphExec_t g_front, g_k7;  // captured K1..K6 and K7 (replayed by step/run)
+  cudaGraphExec_t g_qrfb;         // {set condition; IF -> Householder QR}: the device-decided fallback of K2 for direct launches
   long long g_front_n, g_k7_n;    // kernels per replay
   int use_graph, warm_steps, graph_failed;
   int need_s0;                    // spectrum of the environment set by set_env not computed yet (lazy)
+  cudaStream_t cap_aux;         // captures the body of the conditional Householder fallback of K2 (never runs work itself)
   cudaStream_t side;            // high-priority stream for the overlapped convergence check
   cudaEvent_t ev_env, ev_spec;  // environment ready (main) / spectrum done (side)
   int overlap;
@@ -252,6 +255,7 @@ static int create_common(int d, int D, int chi, void* ws, unsigned long long ws_
       cudaGetLastError(); h->side = nullptr; h->overlap = 0;
     }
   }
+  if (cudaStreamCreateWithFlags(&h->cap_aux, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); h->cap_aux = nullptr; }
   h->h_flag = reinterpret_cast<int*>(h->h_pinned + kPinFlag);
   cudaMemsetAsync(h->flag, 0, 4 * sizeof(int), 0);
   {   // padded operand matrices: the pad columns are zeroed once and never written again
@@ -283,6 +287,7 @@ int qrctm_destroy(qrctm_t* h) {
   if (h->owns_ws && h->base) cudaFree(h->base);
   if (h->eigwork) cudaFree(h->eigwork);
   if (h->h_pinned) cudaFreeHost(h->h_pinned);
+  if (h->cap_aux) cudaStreamDestroy(h->cap_aux);
   if (h->side) { cudaStreamSynchronize(h->side); cudaStreamDestroy(h->side); cudaEventDestroy(h->ev_env); cudaEventDestroy(h->ev_spec); }
   if (h->have_ev) for (int i = 0; i < QRCTM_NSTAGE + 2; ++i) cudaEventDestroy(h->ev[i]);
   cudaGetLastError();
@@ -484,7 +489,7 @@ int qrctm_set_option(qrctm_t* h, int key, int value) {
     case QRCTM_OPT_SYMMETRIZE:  if (value != 0 && value != 1) break; h->symmetrize = value; return QRCTM_OK;
     case QRCTM_OPT_CHECK_EVERY: if (value < 1) break; h->check_every = value; return QRCTM_OK;
     case QRCTM_OPT_GEMM_PATH:   if (value != 0 && value != 1) break; h->gemm_path = value; return QRCTM_OK;
-    case QRCTM_OPT_QR_PATH:     if (value < 0 || value > 2) break; h->qr_path = value; return QRCTM_OK;
+    case QRCTM_OPT_QR_PATH:     if (value < 0 || value > 4) break; h->qr_path = value; return QRCTM_OK;
     case QRCTM_OPT_OVERLAP_CHECK: if (value != 0 && value != 1) break; h->overlap = value; return QRCTM_OK;
     case QRCTM_OPT_ABSORB_MODE: if (value != 0 && value != 1) break; h->absorb_mode = value; return QRCTM_OK;
     case QRCTM_OPT_USE_GRAPH:   if (value != 0 && value != 1) break; h->use_graph = value; return QRCTM_OK;
@@ -672,7 +677,7 @@ unsigned long long qrctm_qr_work_bytes(int rows, int cols) { return qr_work_byte
 
 int qrctm_qr_f64(void* cuda_stream, int path, int rows, int cols, const double* X, double* Q, double* R,
                  void* work) {
-  if (!X || !Q || !R || !work || rows < 1 || cols < 1 || cols > rows || cols > kMaxChi || path < 0 || path > 2)
+  if (!X || !Q || !R || !work || rows < 1 || cols < 1 || cols > rows || cols > kMaxChi || path < 0 || path > 4)
     return QRCTM_ERR_INVALID_ARG;
   cudaError_t e;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
@@ -817,6 +822,15 @@ int qrctm_warmup(qrctm_t* h, int n_eig_steps) {
   return QRCTM_OK;
 }
 
+int qrctm_chol_inv_f64(void* cuda_stream, int n, const double* G, double* R, double* Rinv, int* status, double* dev,
+                       long long* prof) {
+  if (!G || !R || !Rinv || !status || !dev || n < 1 || n > CHOL_MAX_N) return QRCTM_ERR_INVALID_ARG;
+  if (chol_inv_attr() != cudaSuccess) { cudaGetLastError(); return QRCTM_ERR_CUDA; }
+  chol_inv_kernel<<<1, CHOL_NT, chol_smem_bytes(n), static_cast<cudaStream_t>(cuda_stream)>>>(
+      G, n, R, nullptr, Rinv, status, dev, nullptr, nullptr, 0.0, prof);
+  return cudaGetLastError() == cudaSuccess ? QRCTM_OK : QRCTM_ERR_CUDA;
+}
+
 unsigned long long qrctm_eigh_work_bytes(int n, int k) { return eigh_work_bytes_impl(n, k); }
 
 int qrctm_eigh_top_f64(void* cuda_stream, int n, int k, double* A, double* lam, double* U, void* work) {
@@ -859,10 +873,7 @@ int qrctm_shard_front(qrctm_t* h, int rank, int nranks) {
   // replicated: K1, K2 (0.3 % of the flops)
   int rc = stage_reduced_corner(h, h->C, h->T, h->X); if (rc) return rc;
   cudaError_t e;
-  long long nl = h->qr_path != 1 ? qr_factor_blocked(h->stream, h->qr_path, m, chi, h->X, h->Q, h->R, h->qrwork, &e)
-                                 : qr_factor_level2(h->stream, m, chi, h->X, h->Q, h->R, h->qrwork, &e);
-  if (nl < 0) return fail(h, QRCTM_ERR_CUDA, "qr", e);
-  h->launches += nl;
+  int rcq = stage_qr(h); if (rcq) return rcq;
   // the other ranks' rows of T' and the partial C' start from zero, so that either an all-gather of the slices or a
   // plain sum over ranks assembles the full tensors
   CU(h, cudaMemsetAsync(h->Tn, 0, sizeof(double) * m * chi, h->stream));

@@ -28,6 +28,30 @@ int stage_reduced_corner(qrctm* h, const double* C, const double* T, double* X) 
   return QRCTM_OK;
 }
 
+// K2 (E2): X = Q R, diag(R) >= 0.  Automatic path: CholeskyQR2, with the Householder path as its fallback -- decided
+// on the device: by the host after a synchronisation when launching directly, by a conditional graph node when the
+// step is being captured (no host round trip in the replayed step).
+int stage_qr(qrctm* h) {
+  cudaError_t e;
+  long long nl;
+  if (h->qr_path == 1) {
+    nl = qr_factor_level2(h->stream, h->m, h->chi, h->X, h->Q, h->R, h->qrwork, &e);
+  } else {
+    QrFallback fb{1, nullptr, nullptr};
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (h->stream && cudaStreamIsCapturing(h->stream, &cs) == cudaSuccess && cs == cudaStreamCaptureStatusActive) {
+      if (!h->cap_aux) return fail(h, QRCTM_ERR_CUDA, "no auxiliary capture stream");
+      fb = QrFallback{2, h->cap_aux, nullptr};
+    } else if (h->cap_aux) {
+      fb = QrFallback{3, h->cap_aux, &h->g_qrfb};       // direct launches: prebuilt {condition; IF Householder} graph
+    }
+    nl = qr_factor_blocked(h->stream, h->qr_path, h->m, h->chi, h->X, h->Q, h->R, h->qrwork, &e, fb);
+  }
+  if (nl < 0) return fail(h, QRCTM_ERR_CUDA, "qr", e);
+  h->launches += nl;
+  return QRCTM_OK;
+}
+
 // K3: P'[u,l,J,m] = sum_j Qm[j,u,m] T[j,l,J]        (Qm: chi*b x n viewed chi x b*n).  m innermost: the
 // consecutive rows of a K4 tile (M index (J,m)) are then adjacent in K4's outputs.
 // co = number of columns of Qm (the new chi) when it differs from the chi of T (eigen step with chi growth).
@@ -197,11 +221,7 @@ int do_step(qrctm* h, cudaEvent_t* ev /* QRCTM_NSTAGE+1 events or null */, bool 
   rc = stage_reduced_corner(h, h->C, h->T, h->X);
   if (!rc) {
     mark(1, "K2_qr");
-    cudaError_t e;
-    long long nl = h->qr_path != 1
-        ? qr_factor_blocked(h->stream, h->qr_path, h->m, h->chi, h->X, h->Q, h->R, h->qrwork, &e)
-        : qr_factor_level2(h->stream, h->m, h->chi, h->X, h->Q, h->R, h->qrwork, &e);
-    if (nl < 0) rc = fail(h, QRCTM_ERR_CUDA, "qr", e); else h->launches += nl;
+    rc = stage_qr(h);
   }
   if (!rc) { mark(2, "K3_half_absorb"); rc = stage_half_absorb(h, h->Q, h->T, h->P); }
   if (!rc) {
@@ -217,6 +237,7 @@ int do_step(qrctm* h, cudaEvent_t* ev /* QRCTM_NSTAGE+1 events or null */, bool 
 }
 
 void invalidate_graphs(qrctm* h) {
+  if (h->g_qrfb) { cudaGraphExecDestroy(h->g_qrfb); h->g_qrfb = nullptr; }
   if (h->g_front) { cudaGraphExecDestroy(h->g_front); h->g_front = nullptr; }
   if (h->g_k7) { cudaGraphExecDestroy(h->g_k7); h->g_k7 = nullptr; }
   h->graph_failed = 0;

@@ -60,8 +60,11 @@ _QR_SHAPES = [(32, 8), (324, 36), (1024, 64), (50, 50), (7, 1), (333, 17), (16, 
               (5120, 130), (5121, 130), (2000, 113),   # one-launch trailing update: its row limit, one past it, ragged slab
               (10241, 40), (12289, 48), (16400, 33), (20480, 20), (20481, 20)]   # tall register panels: 48 / 64 / 80 rows
                                                                                   # per thread, and one row past them
-# the per-reflector (level-2) path 1 is only checked on small cases
-_QR_CASES = [(r, c, p) for p in (0, 1, 2) for (r, c) in _QR_SHAPES if not (p == 1 and r * c > 200000)]
+_QR_SHAPES += [(208, 208), (5000, 207), (3000, 208), (3000, 209), (4000, 177)]   # CholeskyQR2's column limit (208) +- 1, odd n
+# paths: 0 automatic (CholeskyQR2 for 48 <= n <= 208, Householder when its device-side check fails or outside that
+# range), 1 per-reflector (level-2; only on small cases), 2 blocked Householder, 3 Householder automatic,
+# 4 CholeskyQR2 whenever n <= 208
+_QR_CASES = [(r, c, p) for p in (0, 1, 2, 3, 4) for (r, c) in _QR_SHAPES if not (p == 1 and r * c > 200000)]
 
 
 @pytest.mark.parametrize("rows,cols,path", _QR_CASES)
@@ -79,10 +82,28 @@ def test_qr_f64_matches_oracle(rows, cols, path):
     assert rel(Q, Qo) < 1e-14 * max(cond, 10)
 
 
+@pytest.mark.parametrize("n", [1, 2, 7, 16, 17, 36, 100, 150, 196, 207, 208])
+def test_chol_inv_kernel_against_lapack(n):
+    """The n x n factorisation inside CholeskyQR2 (qrctm_chol_inv_f64): R = chol(G)^T, R^-1, ||G - I||_F, breakdown flag."""
+    g = np.random.default_rng(n)
+    X = g.standard_normal((3 * n + 5, n))
+    G = X.T @ X / (3 * n)
+    R, Ri, st, dev = pkg.chol_inv_f64(torch_dev(G))
+    R, Ri = R.cpu().numpy(), Ri.cpu().numpy()
+    Rn = np.linalg.cholesky(G).T
+    cond = np.linalg.cond(Rn)
+    assert st == 0 and abs(dev - np.linalg.norm(G - np.eye(n))) < 1e-12 * max(1.0, dev)
+    assert np.all(np.tril(R, -1) == 0.0) and np.all(np.tril(Ri, -1) == 0.0) and np.all(np.diag(R) > 0)
+    assert rel(R, Rn) < 1e-14 * max(cond, 10)
+    assert np.linalg.norm(Ri @ Rn - np.eye(n)) < 1e-14 * n * max(cond, 10)
+    G[n // 2, n // 2] = -1.0                                # not positive definite: breakdown must be flagged
+    assert pkg.chol_inv_f64(torch_dev(G))[2] == 1
+
+
 def test_qr_rank_deficient_is_still_valid():
     g = np.random.default_rng(3)
     X = g.standard_normal((200, 6)) @ g.standard_normal((6, 12))       # rank 6 < 12 (hazard H1)
-    for path in (0, 1, 2):
+    for path in (0, 1, 2, 3, 4):
         Q, R = pkg.qr_f64(torch_dev(X), path=path)
         Q, R = Q.cpu().numpy(), R.cpu().numpy()
         assert np.linalg.norm(Q.T @ Q - np.eye(12)) < 1e-13
@@ -91,6 +112,51 @@ def test_qr_rank_deficient_is_still_valid():
     Q, R = Q.cpu().numpy(), R.cpu().numpy()
     assert np.linalg.norm(Q.T @ Q - np.eye(12)) < 1e-13
     assert rel(Q @ R, X) < 1e-13 and np.all(np.diag(R) >= 0.0)
+
+
+@pytest.mark.parametrize("expo", [1, 3, 5, 7, 9, 12])
+def test_qr_graded_conditioning_automatic_path(expo):
+    """The automatic path over a range of cond(X) = 10^expo: CholeskyQR2 where its device-side check
+    (||Q1^T Q1 - I||_F <= 1e-4, no pivot breakdown) passes, Householder beyond -- always orthonormal to rounding,
+    residual at rounding level, and Q, R within cond x 1e-14 of the oracle (until cond eps ~ 1)."""
+    g = np.random.default_rng(expo)
+    U, _ = np.linalg.qr(g.standard_normal((3000, 100)))
+    V, _ = np.linalg.qr(g.standard_normal((100, 100)))
+    X = np.ascontiguousarray((U * np.logspace(0, -expo, 100)) @ V.T)
+    Q, R = pkg.qr_f64(torch_dev(X), path=0)
+    Q, R = Q.cpu().numpy(), R.cpu().numpy()
+    assert np.all(np.tril(R, -1) == 0.0) and np.all(np.diag(R) >= 0.0)
+    assert np.linalg.norm(Q.T @ Q - np.eye(100)) < 100 * 2e-15
+    assert rel(Q @ R, X) < 1e-14
+    Qo, Ro = o.qr_pos(X)
+    assert rel(R, Ro) < 1e-14 * 10.0 ** expo
+    if expo <= 9:
+        assert rel(Q, Qo) < 1e-14 * 10.0 ** expo * 10
+
+
+def test_step_with_rank_deficient_corner_takes_the_householder_fallback_inside_the_graph():
+    """A product-state A makes c~ numerically rank-deficient (hazard H1): CholeskyQR2's device-side check fails and the
+    captured step runs the Householder body of its conditional node.  Graph replay, direct launches and the forced
+    Householder path must agree on the gauge-invariant results (kappa exact for a product state, pin P6)."""
+    d, D, chi = 2, 3, 12
+    g = np.random.default_rng(5)
+    phi, v = g.standard_normal(d), g.standard_normal(D)
+    A = np.einsum("s,u,l,d,r->suldr", phi, v, v, v, v).copy()
+    _, C0, T0 = gen_config(d, D, chi, 7)
+    ks = []
+    for qr_path, graph in ((4, 1), (4, 0), (3, 1)):
+        h = pkg.QRCTM(d, D, chi)
+        h.set_option(pkg.OPT_QR_PATH, qr_path)
+        h.set_option(pkg.OPT_USE_GRAPH, graph)
+        h.set_A(A); h.set_env(C0, T0)
+        h.run(25, -1.0)
+        Q, R = h.get_qr()
+        assert np.linalg.norm(Q.T @ Q - np.eye(chi)) < 1e-13
+        ks.append(h.norm_per_site())
+        h.close()
+    exact = (phi @ phi) * (v @ v) ** 4
+    for k in ks:
+        assert abs(k / exact - 1) < 1e-11
 
 
 @pytest.mark.parametrize("d,D,chi,seed", [(2, 2, 8, 0), (2, 3, 36, 1), (3, 2, 5, 4), (2, 3, 7, 5), (1, 1, 4, 2)])
