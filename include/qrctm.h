@@ -76,6 +76,8 @@ enum {
   QRCTM_OPT_USE_GRAPH = 8,   /* 1 [default] = K1..K6 and K7 are captured once into CUDA graphs and replayed by
                                 qrctm_step / qrctm_run (needs a non-default stream); 0 = plain launches, which keep
                                 the per-stage NVTX ranges for profilers */
+  QRCTM_OPT_K8_PATH = 10,    /* K8 tridiagonalisation for chi <= 232: 0 [default] = the thread-per-column kernel (un-
+                                normalised reflectors, 2 barriers per step), 1 = the round-1 kernel (for cross-checks) */
   QRCTM_OPT_ABSORB_MODE = 9  /* K4: 0 [default] = contract with the explicit double-layer tensor a (2 chi^2 D^8 flops),
                                 1 = layered: contract with the ket and the bra copy of A in turn (4 d chi^2 D^6
                                 flops; same T' up to rounding; needs even chi, otherwise mode 0 is used) */
@@ -228,6 +230,12 @@ int qrctm_qr_f64(void* cuda_stream, int path, int rows, int cols, const double* 
  * One CTA; asynchronous on the stream. */
 int qrctm_chol_inv_f64(void* cuda_stream, int n, const double* G, double* R, double* Rinv, int* status, double* dev,
                        long long* prof);
+
+/* Stand-alone entry of K8's tridiagonalisation (csrc/spectrum.cuh; for the sub-step parity tests): the symmetric
+ * C[n][n] (DEVICE; lower triangle read, untouched), n <= 232, is reduced by Householder similarity transforms to the
+ * tridiagonal matrix with diagonal d[n] and sub-diagonal e[1..n-1] (e[0] = 0) (DEVICE).  prof = NULL, or 8 DEVICE
+ * long longs: SM cycles of the kernel's phases.  One CTA; asynchronous on the stream. */
+int qrctm_tridiag_f64(void* cuda_stream, int n, const double* C, double* d, double* e, long long* prof);
 
 /* ---- NEXT-2: the paper's initialisation and warm-up ----
  * PAPER.md:28 "performing only a few (1-4) initial warm-up steps using the standard

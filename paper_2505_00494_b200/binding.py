@@ -19,7 +19,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("QRCTM_LIB", os.path.join(_HERE, "libqrctm.so"))
 
 QRCTM_OK = 0
-OPT_CORNER_MODE, OPT_SYMMETRIZE, OPT_CHECK_EVERY, OPT_GEMM_PATH, OPT_TIME_STAGES, OPT_QR_PATH, OPT_OVERLAP_CHECK, OPT_USE_GRAPH, OPT_ABSORB_MODE = 1, 2, 3, 4, 5, 6, 7, 8, 9
+OPT_CORNER_MODE, OPT_SYMMETRIZE, OPT_CHECK_EVERY, OPT_GEMM_PATH, OPT_TIME_STAGES, OPT_QR_PATH, OPT_OVERLAP_CHECK, OPT_USE_GRAPH, OPT_ABSORB_MODE, OPT_K8_PATH = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10
 NSTAGE = 7
 STAGE_NAMES = ("K1_reduced_corner", "K2_qr", "K3_half_absorb", "K4_absorb_a", "K5_project",
                "K6_corner", "K7_normalize")
@@ -34,7 +34,7 @@ SYMBOLS = (
     "qrctm_gemm_f64", "qrctm_gemm_f64_ws", "qrctm_qr_work_bytes", "qrctm_qr_f64", "qrctm_probe_fp64", "qrctm_last_error",
     "qrctm_version",
     "qrctm_get_chi", "qrctm_init_bulk", "qrctm_eig_step", "qrctm_get_eig", "qrctm_warmup",
-    "qrctm_eigh_work_bytes", "qrctm_eigh_top_f64", "qrctm_chol_inv_f64",
+    "qrctm_eigh_work_bytes", "qrctm_eigh_top_f64", "qrctm_chol_inv_f64", "qrctm_tridiag_f64",
     "qrctm_shard_range", "qrctm_shard_front", "qrctm_shard_buffers", "qrctm_shard_finish",
 )
 
@@ -89,6 +89,7 @@ def load_library() -> ctypes.CDLL:
     lib.qrctm_qr_f64.argtypes = [P, c_int, c_int, c_int, P, P, P, P]
     lib.qrctm_probe_fp64.argtypes = [c_int, c_int, POINTER(c_double)]
     lib.qrctm_chol_inv_f64.argtypes = [P, c_int, P, P, P, P, P, P]
+    lib.qrctm_tridiag_f64.argtypes = [P, c_int, P, P, P, P]
     lib.qrctm_get_chi.argtypes = [P, POINTER(c_int), POINTER(c_int)]
     lib.qrctm_init_bulk.argtypes = [P]
     lib.qrctm_eig_step.argtypes = [P, c_int]
@@ -408,6 +409,22 @@ def chol_inv_f64(G, profile: bool = False):
     torch.cuda.current_stream().synchronize()
     out = (R, Ri, int(st.item()), float(dev.item()))
     return out + (prof.cpu().numpy(),) if profile else out
+
+
+def tridiag_f64(C, profile: bool = False):
+    """(d, e[, cycles]) of a symmetric torch CUDA float64 matrix (n <= 232) through qrctm_tridiag_f64."""
+    import torch
+    lib = load_library()
+    n = C.shape[0]
+    d = torch.empty((n,), dtype=torch.float64, device="cuda")
+    e = torch.empty((n,), dtype=torch.float64, device="cuda")
+    prof = torch.zeros(8, dtype=torch.int64, device="cuda") if profile else None
+    rc = lib.qrctm_tridiag_f64(c_void_p(torch.cuda.current_stream().cuda_stream), n, _ptr(C.contiguous()), _ptr(d), _ptr(e),
+                               c_void_p(prof.data_ptr()) if profile else None)
+    if rc != QRCTM_OK:
+        raise QrctmError(f"qrctm_tridiag_f64 failed: {rc}")
+    torch.cuda.current_stream().synchronize()
+    return (d, e, prof.cpu().numpy()) if profile else (d, e)
 
 
 def shard_range(chi: int, rank: int, nranks: int):

@@ -53,6 +53,7 @@ struct qrctm {
   Layout L;
   bool have_A, have_env;
   int corner_mode, symmetrize, check_every, gemm_path, time_stages, qr_path, absorb_mode;
+  int k8_old;             // 1: K8 on the round-1 tridiagonalisation kernel (QRCTM_OPT_K8_PATH, for cross-checks)
   long long launches;
   cudaEvent_t ev[QRCTM_NSTAGE + 2];
   bool have_ev;
@@ -494,6 +495,7 @@ int qrctm_set_option(qrctm_t* h, int key, int value) {
     case QRCTM_OPT_ABSORB_MODE: if (value != 0 && value != 1) break; h->absorb_mode = value; return QRCTM_OK;
     case QRCTM_OPT_USE_GRAPH:   if (value != 0 && value != 1) break; h->use_graph = value; return QRCTM_OK;
     case QRCTM_OPT_TIME_STAGES: if (value != 0 && value != 1) break; h->time_stages = value; return QRCTM_OK;
+    case QRCTM_OPT_K8_PATH:     if (value != 0 && value != 1) break; h->k8_old = value; return QRCTM_OK;
     default: break;
   }
   return fail(h, QRCTM_ERR_INVALID_ARG, "bad option key/value");
@@ -828,6 +830,18 @@ int qrctm_chol_inv_f64(void* cuda_stream, int n, const double* G, double* R, dou
   if (chol_inv_attr() != cudaSuccess) { cudaGetLastError(); return QRCTM_ERR_CUDA; }
   chol_inv_kernel<<<1, CHOL_NT, chol_smem_bytes(n), static_cast<cudaStream_t>(cuda_stream)>>>(
       G, n, R, nullptr, Rinv, status, dev, nullptr, nullptr, 0.0, prof);
+  return cudaGetLastError() == cudaSuccess ? QRCTM_OK : QRCTM_ERR_CUDA;
+}
+
+int qrctm_tridiag_f64(void* cuda_stream, int n, const double* C, double* d, double* e, long long* prof) {
+  if (!C || !d || !e || n < 1 || n > TRI2_MAX_N) return QRCTM_ERR_INVALID_ARG;
+  static bool attr = false;
+  if (!attr) {
+    if (cudaFuncSetAttribute(tridiag_smem2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)tri2_smem_bytes(TRI2_MAX_N)) != cudaSuccess) { cudaGetLastError(); return QRCTM_ERR_CUDA; }
+    attr = true;
+  }
+  tridiag_smem2_kernel<<<1, TRI2_NT, tri2_smem_bytes(n), static_cast<cudaStream_t>(cuda_stream)>>>(C, n, d, e, prof);
   return cudaGetLastError() == cudaSuccess ? QRCTM_OK : QRCTM_ERR_CUDA;
 }
 

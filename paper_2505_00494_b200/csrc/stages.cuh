@@ -175,7 +175,19 @@ int stage_spectrum(qrctm* h, double* s_out, int update_prev, cudaStream_t st) {
   }
   const size_t tri_bytes = sizeof(double) * ((size_t)chi * (chi + 1) / 2 + 2 * (size_t)chi + 40);
   const int nt = ((chi + 31) / 32 * 32) < 64 ? 64 : (chi + 31) / 32 * 32;
-  if (tri_bytes <= (size_t)max_smem && chi <= 1024) {
+  if (chi <= TRI2_MAX_N && !h->k8_old) {
+    static bool attr2 = false;
+    if (!attr2) {
+      CU(h, cudaFuncSetAttribute(tridiag_smem2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)tri2_smem_bytes(TRI2_MAX_N)));
+      attr2 = true;
+    }
+    tridiag_smem2_kernel<<<1, TRI2_NT, tri2_smem_bytes(chi), st>>>(h->C, chi, h->dvec, h->evec, nullptr);
+    multisect_kernel<<<(chi + 7) / 8, 256, sizeof(double) * (2 * chi + 40), st>>>(h->dvec, h->evec, chi, h->eig);
+    spectrum_finalize_kernel<<<1, nt, sizeof(double) * (chi + 40), st>>>(h->eig, chi, s_out, h->s_prev, h->delta,
+                                                                        update_prev);
+    h->launches += 3;
+  } else if (tri_bytes <= (size_t)max_smem && chi <= 1024) {
     tridiag_smem_kernel<<<1, 1024, tri_bytes, st>>>(h->C, chi, h->dvec, h->evec);
     multisect_kernel<<<(chi + 7) / 8, 256, sizeof(double) * (2 * chi + 40), st>>>(h->dvec, h->evec, chi,
                                                                                          h->eig);

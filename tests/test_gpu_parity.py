@@ -343,6 +343,32 @@ def test_spectrum_kernel_against_lapack():
         h.close()
 
 
+@pytest.mark.parametrize("n", [1, 2, 3, 8, 33, 64, 100, 196, 232])
+def test_tridiag_kernel_preserves_the_spectrum(n):
+    """qrctm_tridiag_f64 (K8's first stage): the tridiagonal (d, e) it returns is orthogonally similar to C, so the
+    eigenvalues agree with LAPACK's to rounding; also on a rank-one matrix (the trailing block is rounding noise)."""
+    g = np.random.default_rng(n)
+    C = g.standard_normal((n, n)); C = C + C.T; C /= np.linalg.norm(C)
+    for M in (C, np.ones((n, n)) / n):
+        d, e = pkg.tridiag_f64(torch_dev(M))
+        d, e = d.cpu().numpy(), e.cpu().numpy()
+        T = np.diag(d) + np.diag(e[1:], 1) + np.diag(e[1:], -1)
+        assert e[0] == 0.0
+        assert np.max(np.abs(np.linalg.eigvalsh(T) - np.linalg.eigvalsh(M))) < 5e-15 * max(n, 4)
+
+
+def test_k8_paths_agree():
+    A, C0, T0 = gen_config(2, 1, 150, 3)
+    out = []
+    for path in (0, 1):
+        h = pkg.QRCTM(2, 1, 150)
+        h.set_option(pkg.OPT_K8_PATH, path)
+        h.set_A(A); h.set_env(C0, T0)
+        out.append(h.get_corner_spectrum())
+        h.close()
+    assert np.max(np.abs(out[0] - out[1])) < 1e-14
+
+
 def test_errors_and_not_ready():
     h = pkg.QRCTM(2, 2, 4)
     with pytest.raises(pkg.QrctmError):
