@@ -136,6 +136,89 @@ def oracle_time_steps(name, max_steps, budget_s):
     return times, cores
 
 
+def oracle_time_one_thread(name, budget_s):
+    """The same oracle iteration with the host BLAS limited to ONE thread."""
+    try:
+        from threadpoolctl import threadpool_limits
+    except Exception:
+        return None
+    with threadpool_limits(limits=1):
+        times, _ = oracle_time_steps(name, 3, budget_s)
+    tt = times[1:] if len(times) > 1 else times
+    return {"ms_per_step": 1e3 * float(np.mean(tt)), "steps": len(tt), "cores": 1}
+
+
+def oracle_time_eig_step(name, reps):
+    """The oracle's standard (eigen) CTMRG step beside its QR step at the same (D, chi): the shape of the paper's claim
+    that the standard step is dominated by the eigendecomposition."""
+    from oracle import ctmrg as o
+    A, C0, T0, c = gen_named(name)
+    a = o.build_a(A)
+    C, T = o.normalize(C0, T0)
+    te, tq = [], []
+    for _ in range(reps):
+        t0 = time.perf_counter(); o.eig_step(C, T, a); te.append(time.perf_counter() - t0)
+        t0 = time.perf_counter(); o.qr_step(C, T, a); tq.append(time.perf_counter() - t0)
+    e, q = 1e3 * float(np.min(te)), 1e3 * float(np.min(tq))
+    return {"eig_step_ms": e, "qr_step_ms": q, "eig_over_qr": e / q, "reps": reps}
+
+
+def file_sha16(*paths):
+    import hashlib
+    h = hashlib.sha256()
+    for p in paths:
+        h.update(open(p, "rb").read())
+    return h.hexdigest()[:16]
+
+
+def bench_config(pkg, torch, name, steps, warmup, peak_dmma, conv=True, corner_mode=0):
+    """it/s, ms/step, per-stage ms, step TFLOP/s and time-to-convergence of one BASELINE.json config on the current
+    device (the side configs of the `configs` block; the headline config is timed in main() with the same calls)."""
+    A, C0, T0, c = gen_named(name)
+    d, D, chi = c["d"], c["D"], c["chi"]
+    b = D * D
+    fl = step_flops(D, chi)
+    if corner_mode == 1:      # K6': the enlarged corner costs a second K3 + K4, then C~ Q and Q^T (C~ Q)
+        m = chi * b
+        fl = dict(fl); fl["K6"] = 2 * m * m * chi + 2 * chi ** 2 * b ** 4 + 2 * m * m * chi + 2 * m * chi * chi
+    h = pkg.QRCTM(d, D, chi)
+    h.set_option(pkg.OPT_CORNER_MODE, corner_mode)
+    h.set_A(A); h.set_env(C0, T0)
+    h.run(warmup + 1, -1.0)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n0 = h.launch_count()
+    torch.cuda.synchronize()
+    ev0.record(h.stream)
+    it, _ = h.run(steps, -1.0)
+    ev1.record(h.stream)
+    torch.cuda.synchronize()
+    ms = ev0.elapsed_time(ev1) / steps
+    launches = h.launch_count() - n0
+    h.set_option(pkg.OPT_TIME_STAGES, 1)
+    h.run(1, -1.0); h.get_stage_ms(reset=True)
+    h.run(steps, -1.0)
+    st, nst = h.get_stage_ms(reset=True)
+    h.set_option(pkg.OPT_TIME_STAGES, 0)
+    out = {"d": d, "D": D, "chi": chi, "value": 1e3 / ms, "unit": UNIT, "ms_per_step": ms, "steps": steps,
+           "gpu_launches_per_step": launches / steps,
+           "stages_ms": {k: v / nst for k, v in st.items()},
+           "algorithmic_gflop_per_step": sum(fl.values()) / 1e9,
+           "step_tflops": sum(fl.values()) / (ms * 1e-3) / 1e12,
+           "step_frac_of_fp64_peak": sum(fl.values()) / (ms * 1e-3) / 1e12 / peak_dmma}
+    if conv:
+        h.set_env(C0, T0)
+        torch.cuda.synchronize()
+        ev0.record(h.stream)
+        its, dl = h.run(int(c["iters"]), float(c["tol"]))
+        ev1.record(h.stream)
+        torch.cuda.synchronize()
+        out["time_to_convergence"] = {"iterations": int(its), "max_iter": int(c["iters"]), "tol": float(c["tol"]),
+                                      "final_delta": float(dl), "converged": bool(dl < c["tol"]),
+                                      "ms": ev0.elapsed_time(ev1)}
+    h.close()
+    return out
+
+
 def run_reference(args, rank, world):
     if rank != 0:
         return
@@ -408,13 +491,21 @@ def main():
     if rank == 0:
         k4_ms = stage_ms["K4_absorb_a"] / nst
         ach = fl["K4"] / (k4_ms * 1e-3) / 1e12
-        traffic = None
-        tpath = os.path.join(ROOT, "profiles", "k4_traffic_bytes.txt")   # from the committed ncu --set full capture
+        # DRAM traffic of the K4 kernel: not measurable inside this process (it needs ncu's dram__bytes counters), so it
+        # is the figure of the committed ncu --set full capture -- reported ONLY while the GEMM sources still hash to
+        # what that capture profiled (profiles/k4_traffic_bytes.txt: config, bytes, sha16 of gemm_f64.cuh+gemm_launch.cuh)
+        traffic, traffic_note = None, "no capture for this config"
+        csrc = os.path.join(ROOT, "paper_2505_00494_b200", "csrc")
+        src_sha = file_sha16(os.path.join(csrc, "gemm_f64.cuh"), os.path.join(csrc, "gemm_launch.cuh"))
+        tpath = os.path.join(ROOT, "profiles", "k4_traffic_bytes.txt")
         if os.path.exists(tpath):
             for ln in open(tpath):
                 f = ln.split()
-                if len(f) == 2 and f[0] == name:
-                    traffic = int(f[1])
+                if len(f) == 3 and f[0] == name:
+                    if f[2] == src_sha:
+                        traffic, traffic_note = int(f[1]), f"profiles/r1_k4_gemm_ws_ncu.md (GEMM sources sha16 {src_sha})"
+                    else:
+                        traffic_note = f"stale: capture was of GEMM sources {f[2]}, now {src_sha}"
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -429,7 +520,7 @@ def main():
             "gpu_launches": int(launches),
             "clocks": clocks,
             "roofline": {"bound": "tensor", "kernel": "gemm_f64_dmma (K4: S = P.a)", "achieved": ach,
-                         "peak": peak_dmma, "unit": "TFLOP/s", "frac": ach / peak_dmma, "traffic": traffic,
+                         "peak": peak_dmma, "unit": "TFLOP/s", "frac": ach / peak_dmma, "traffic": traffic, "traffic_source": traffic_note,
                          "peak_source": "FP64 DMMA issue rate measured live by qrctm_probe_fp64 "
                                         "(MEASURED_PEAKS.json has no FP64 entry; nominal 148 SM x 64 FMA/clk x 1.965 GHz = 37.2)",
                          "dfma_peak": peak_dfma, "algorithmic_flops_per_launch": fl["K4"], "ms_per_launch": k4_ms},
@@ -442,6 +533,13 @@ def main():
             "step_tflops": sum(fl.values()) / (ms_per_step * 1e-3) / 1e12,
             "step_frac_of_fp64_peak": sum(fl.values()) / (ms_per_step * 1e-3) / 1e12 / peak_dmma,
         }
+        if not args.no_next:
+            side = [n_ for n_ in ("cfg0", "cfg1", "cfg2", "cfg3a", "cfg3b", "cfg4") if n_ != name]
+            line["configs"] = {n_: bench_config(pkg, torch, n_, args.steps, args.warmup, peak_dmma) for n_ in side}
+            # K6' (the enlarged-corner route, "the standard diagram on the left-hand side" of Fig. 1(f))
+            # under its own flop count (cfg2 and cfg4)
+            line["corner_mode_1"] = {n_: bench_config(pkg, torch, n_, max(3, args.steps // 4), args.warmup, peak_dmma,
+                                                       conv=False, corner_mode=1) for n_ in ("cfg2", "cfg4")}
         if not args.no_cpu_baseline and world == 1:
             budget = 20.0
             times, cores = oracle_time_steps(name, 50, budget_s=budget)
@@ -452,6 +550,13 @@ def main():
                                               f"NumPy {np.__version__}), first one discarded" if len(times) > 1 else
                                               f"1 iteration of {name}",
                                     "ms_per_step": cms}
+            one = oracle_time_one_thread(name, 25.0)
+            if one:
+                line["cpu_baseline"]["one_thread"] = one
+            line["cpu_baseline"]["eig_step_vs_qr_step"] = {n_: oracle_time_eig_step(n_, 3) for n_ in ("cfg1", "cfg2")}
+            line["cpu_baseline"]["eig_step_vs_qr_step"]["note"] = (
+                "oracle eig_step (enlarged corner + full LAPACK eigh) beside oracle qr_step at the same (D, chi): the "
+                "shape of PAPER.md:40's claim (standard CTMRG dominated by the eigendecomposition)")
         print(json.dumps(line), flush=True)
     h.close()
     if world > 1:
