@@ -184,6 +184,14 @@ int qrctm_set_option(qrctm_t* h, int key, int value);
  * gpu_launches); kernels replayed from a CUDA graph are counted per replay. */
 long long qrctm_launch_count(const qrctm_t* h);
 
+/* Per-iteration history of the current environment (reset by qrctm_set_env / qrctm_init_bulk / qrctm_eig_step), kept on the device
+ * in a ring buffer of 4096 records and written by the step's own kernels (K7, K8) -- nothing is logged on the hot
+ * path.  Record i (4 doubles): delta_i = max_k |s_k - s_k(previous check)| (NaN if that step was not checked),
+ * ||C'||_F and ||T'||_F before normalisation, min_k R_kk / max_k R_kk of the step's QR (hazard H1).
+ * *n_steps = iterations recorded since the reset; out (HOST, 4 * max_records doubles) receives the last
+ * min(n_steps, max_records, 4096) records in chronological order.  Synchronises. */
+int qrctm_get_history(qrctm_t* h, double* out, int max_records, int* n_steps);
+
 /* Event-timed profile of one step: runs one qrctm_step with CUDA events around
  * each stage and returns milliseconds in ms[0..QRCTM_NSTAGE-1]:
  * 0 K1 reduced corner, 1 K2 QR (panel+WY+form Q+sign), 2 K3 half-absorb,

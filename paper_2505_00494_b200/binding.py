@@ -30,7 +30,7 @@ SYMBOLS = (
     "qrctm_create", "qrctm_workspace_bytes", "qrctm_create_in", "qrctm_destroy", "qrctm_set_stream",
     "qrctm_set_A", "qrctm_set_env", "qrctm_step", "qrctm_run", "qrctm_get_env",
     "qrctm_get_corner_spectrum", "qrctm_get_qr", "qrctm_get_raw", "qrctm_get_a", "qrctm_norm_per_site",
-    "qrctm_r_diag_ratio", "qrctm_energy_nn", "qrctm_edge_update", "qrctm_set_option", "qrctm_launch_count", "qrctm_get_stage_ms", "qrctm_profile_step",
+    "qrctm_r_diag_ratio", "qrctm_energy_nn", "qrctm_edge_update", "qrctm_set_option", "qrctm_launch_count", "qrctm_get_history", "qrctm_get_stage_ms", "qrctm_profile_step",
     "qrctm_gemm_f64", "qrctm_gemm_f64_ws", "qrctm_qr_work_bytes", "qrctm_qr_f64", "qrctm_probe_fp64", "qrctm_last_error",
     "qrctm_version",
     "qrctm_get_chi", "qrctm_init_bulk", "qrctm_eig_step", "qrctm_get_eig", "qrctm_warmup",
@@ -75,6 +75,7 @@ def load_library() -> ctypes.CDLL:
     lib.qrctm_r_diag_ratio.argtypes = [P, POINTER(c_double)]
     lib.qrctm_energy_nn.argtypes = [P, P, POINTER(c_double), P]
     lib.qrctm_edge_update.argtypes = [P, P, c_int, P]
+    lib.qrctm_get_history.argtypes = [P, P, c_int, POINTER(c_int)]
     lib.qrctm_set_option.argtypes = [P, c_int, c_int]
     lib.qrctm_launch_count.argtypes = [P]
     lib.qrctm_launch_count.restype = c_longlong
@@ -331,6 +332,13 @@ class QRCTM:
 
     def set_option(self, key: int, value: int):
         self._check(self.lib.qrctm_set_option(self._h, key, value))
+
+    def get_history(self, max_records: int = 4096):
+        """(records, n_steps): records[i] = (delta, ||C'||_F, ||T'||_F, min R_kk / max R_kk) of the last iterations."""
+        out = np.empty((max(max_records, 1), 4), dtype=np.float64)
+        n = c_int(0)
+        self._check(self.lib.qrctm_get_history(self._h, _ptr(out), max_records, byref(n)))
+        return out[:min(n.value, max_records, 4096)].copy(), n.value
 
     def launch_count(self) -> int:
         return int(self.lib.qrctm_launch_count(self._h))

@@ -140,10 +140,21 @@ __global__ void sym_partial_kernel(const double* __restrict__ Cn, const double* 
 
 // Pass 2: every block re-reduces the partials in the same fixed order, then scales.
 // scal[0] = ||C||_F, scal[1] = ||T||_F ; flag set to 1 on NaN/Inf/zero norm.
+// hist != null: this K7 closes an iteration; block 0 appends the record {delta = NaN (filled in by K8 if the step is
+// checked), ||C'||_F, ||T'||_F, min_k R_kk / max_k R_kk} to the ring buffer hist[QRCTM_HIST_CAP][4] and bumps *hist_n.
+constexpr int QRCTM_HIST_CAP = 4096;
 __global__ void scale_kernel(double* __restrict__ C, double* __restrict__ T, int chi, int b,
                              const double* __restrict__ partial, int nbC, int nbT, double* __restrict__ scal,
-                             int* __restrict__ flag) {
+                             int* __restrict__ flag, double* __restrict__ hist = nullptr, int* __restrict__ hist_n = nullptr,
+                             const double* __restrict__ R = nullptr) {
   __shared__ double sh[33];
+  if (hist && blockIdx.x == 0) {
+    double mn = INFINITY, mx = -INFINITY;
+    for (int k = threadIdx.x; k < chi; k += blockDim.x) { const double v = R[(long long)k * chi + k]; mn = fmin(mn, v); mx = fmax(mx, v); }
+    const double gmx = block_max(mx, sh);
+    const double gmn = -block_max(-mn, sh);
+    if (threadIdx.x == 0) scal[8] = gmx != 0.0 ? gmn / gmx : 0.0;
+  }
   double a = 0.0, t = 0.0;
   for (int i = threadIdx.x; i < nbC; i += blockDim.x) a += partial[i];
   for (int i = threadIdx.x; i < nbT; i += blockDim.x) t += partial[nbC + i];
@@ -153,6 +164,12 @@ __global__ void scale_kernel(double* __restrict__ C, double* __restrict__ T, int
   if (blockIdx.x == 0 && threadIdx.x == 0) {
     scal[0] = nc; scal[1] = nt;
     if (!(nc > 0.0) || !(nt > 0.0) || isinf(nc) || isinf(nt)) *flag = 1;
+    if (hist) {
+      const int idx = *hist_n;
+      double* rec = hist + (size_t)(idx % QRCTM_HIST_CAP) * 4;
+      rec[0] = __longlong_as_double(0x7ff8000000000000LL); rec[1] = nc; rec[2] = nt; rec[3] = scal[8];
+      *hist_n = idx + 1;
+    }
   }
   double ic = 1.0 / nc, it = 1.0 / nt;
   long long n1 = (long long)chi * chi, n2 = (long long)chi * b * chi;

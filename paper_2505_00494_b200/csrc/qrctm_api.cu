@@ -32,7 +32,7 @@ constexpr size_t kAlign = 256;
 inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
 struct Layout {   // byte offsets into the workspace
-  size_t A, a_mat, a2_mat, LH, rho, B1, B2, P1, C, T, Cn, Tn, X, Q, R, Rt, P, S, W, E, splitk, partial, scal, flag, Wc, dvec, evec,
+  size_t A, a_mat, a2_mat, LH, rho, B1, B2, P1, C, T, Cn, Tn, X, Q, R, Rt, P, S, W, E, splitk, partial, scal, flag, hist, Wc, dvec, evec,
       vv, pv, eig, s, s_prev, s_tmp, delta, qrwork, k8work, total;
   long long lda_a, ld1, ld2;
   size_t splitk_elems, qrwork_bytes, k8work_bytes;
@@ -72,7 +72,7 @@ struct qrctm {
   double* h_pinned;       // [0] delta, [1..] scratch ; pinned host
   int* h_flag;
   // typed views
-  double *A, *a_mat, *a2_mat, *LH, *rho, *B1, *B2, *P1, *C, *T, *Cn, *Tn, *X, *Q, *R, *Rt, *P, *S, *W, *E, *splitk, *partial, *scal, *Wc,
+  double *A, *a_mat, *a2_mat, *LH, *rho, *B1, *B2, *P1, *C, *T, *Cn, *Tn, *X, *Q, *R, *Rt, *P, *S, *W, *E, *splitk, *partial, *scal, *hist, *Wc,
       *dvec, *evec, *vv, *pv, *eig, *s, *s_prev, *s_tmp, *delta;
   int* flag;
   void* qrwork;
@@ -122,7 +122,8 @@ bool make_layout(int d, int D, int chi, Layout* L) {
   L->splitk = take(dbl * L->splitk_elems);
   L->partial = take(dbl * 4 * kPartialBlocks);
   L->scal = take(dbl * 16);
-  L->flag = take(sizeof(int) * 4);
+  L->flag = take(sizeof(int) * 4);          // [0] NaN/zero-norm flag, [1] number of history records written
+  L->hist = take(dbl * 4 * QRCTM_HIST_CAP);
   L->Wc = take(dbl * chi * chi);
   L->dvec = take(dbl * chi);
   L->evec = take(dbl * chi);
@@ -146,7 +147,7 @@ void bind_views(qrctm* h) {
   const Layout& L = h->L;
 #define V_(name) h->name = reinterpret_cast<double*>(B + L.name)
   V_(A); V_(a_mat); V_(a2_mat); V_(LH); V_(rho); V_(B1); V_(B2); V_(P1); V_(C); V_(T); V_(Cn); V_(Tn); V_(X); V_(Q); V_(R); V_(Rt); V_(P); V_(S); V_(W);
-  V_(E); V_(splitk); V_(partial); V_(scal); V_(Wc); V_(dvec); V_(evec); V_(vv); V_(pv); V_(eig); V_(s);
+  V_(E); V_(splitk); V_(partial); V_(scal); V_(hist); V_(Wc); V_(dvec); V_(evec); V_(vv); V_(pv); V_(eig); V_(s);
   V_(s_prev); V_(s_tmp); V_(delta);
 #undef V_
   h->flag = reinterpret_cast<int*>(B + L.flag);
@@ -321,7 +322,7 @@ int qrctm_set_env(qrctm_t* h, const double* C, const double* T) {
   if (h->chi != h->chi_cap) { CU(h, cudaStreamSynchronize(h->stream)); set_chi(h, h->chi_cap); }
   CU(h, copy_in(h->Cn, C, (size_t)h->chi * h->chi, h->stream));
   CU(h, copy_in(h->Tn, T, (size_t)h->m * h->chi, h->stream));
-  CU(h, cudaMemsetAsync(h->flag, 0, sizeof(int), h->stream));
+  CU(h, cudaMemsetAsync(h->flag, 0, 2 * sizeof(int), h->stream));      // numeric flag and the history counter
   int rc = stage_normalize(h, h->Cn, h->Tn); if (rc) return rc;
   rc = check_flag(h); if (rc) return rc;
   CU(h, cudaMemsetAsync(h->s_prev, 0, sizeof(double) * h->chi, h->stream));
@@ -502,6 +503,24 @@ int qrctm_set_option(qrctm_t* h, int key, int value) {
 }
 
 long long qrctm_launch_count(const qrctm_t* h) { return h ? h->launches : 0; }
+
+int qrctm_get_history(qrctm_t* h, double* out, int max_records, int* n_steps) {
+  if (!h || !n_steps || max_records < 0 || (max_records > 0 && !out)) return h ? fail(h, QRCTM_ERR_INVALID_ARG, "bad argument") : QRCTM_ERR_INVALID_ARG;
+  if (out && is_device_ptr(out)) return fail(h, QRCTM_ERR_INVALID_ARG, "history: host pointer");
+  if (h->side) CU(h, cudaStreamSynchronize(h->side));
+  int n = 0;
+  CU(h, cudaMemcpyAsync(&n, h->flag + 1, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+  CU(h, cudaStreamSynchronize(h->stream));
+  *n_steps = n;
+  int take = n < max_records ? n : max_records;
+  if (take > QRCTM_HIST_CAP) take = QRCTM_HIST_CAP;
+  for (int r = 0; r < take; ++r) {          // chronological: the last `take` records
+    const int idx = (n - take + r) % QRCTM_HIST_CAP;
+    CU(h, cudaMemcpyAsync(out + 4 * (size_t)r, h->hist + 4 * (size_t)idx, 4 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  }
+  CU(h, cudaStreamSynchronize(h->stream));
+  return QRCTM_OK;
+}
 
 int qrctm_get_stage_ms(qrctm_t* h, double* ms, long long* steps, int reset) {
   if (!h) return QRCTM_ERR_INVALID_ARG;
@@ -780,7 +799,7 @@ int qrctm_init_bulk(qrctm_t* h) {
   bulk_init_kernel<<<nb, 256, 0, h->stream>>>(h->A, h->d, h->D, h->Cn, h->Tn);
   h->launches += 1;
   CU(h, cudaGetLastError());
-  CU(h, cudaMemsetAsync(h->flag, 0, sizeof(int), h->stream));
+  CU(h, cudaMemsetAsync(h->flag, 0, 2 * sizeof(int), h->stream));
   int rc = stage_normalize(h, h->Cn, h->Tn); if (rc) return rc;
   rc = check_flag(h); if (rc) return rc;
   CU(h, cudaMemsetAsync(h->s_prev, 0, sizeof(double) * h->chi_cap, h->stream));
@@ -799,6 +818,7 @@ int qrctm_eig_step(qrctm_t* h, int chi_new) {
   rc = stage_eig_step(h, chi_new); if (rc) return rc;
   rc = check_flag(h); if (rc) return rc;
   CU(h, cudaMemsetAsync(h->s_prev, 0, sizeof(double) * h->chi_cap, h->stream));
+  CU(h, cudaMemsetAsync(h->flag + 1, 0, sizeof(int), h->stream));       // a new convergence history starts here
   h->need_s0 = 1;
   return QRCTM_OK;
 }

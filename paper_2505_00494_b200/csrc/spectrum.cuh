@@ -513,7 +513,8 @@ multisect_kernel(const double* __restrict__ dvec, const double* __restrict__ eve
 // One block, blockDim.x >= n: s = sorted |eig| (descending), delta vs s_prev.
 __global__ void spectrum_finalize_kernel(const double* __restrict__ eig, int n, double* __restrict__ s_out,
                                          double* __restrict__ s_prev, double* __restrict__ delta_out,
-                                         int update_prev) {
+                                         int update_prev, double* __restrict__ hist = nullptr,
+                                         const int* __restrict__ hist_n = nullptr) {
   extern __shared__ double fsm[];               // lam[n], red[33]
   double* lam = fsm; double* red = fsm + n;
   const int tid = threadIdx.x;
@@ -532,7 +533,10 @@ __global__ void spectrum_finalize_kernel(const double* __restrict__ eig, int n, 
   double dl = 0.0;
   if (tid < n) dl = fabs(s_out[tid] - s_prev[tid]);
   double dmax = block_max(dl, red);
-  if (tid == 0) delta_out[0] = dmax;
+  if (tid == 0) {
+    delta_out[0] = dmax;
+    if (hist && update_prev && *hist_n > 0) hist[(size_t)((*hist_n - 1) % 4096) * 4] = dmax;   // this step's record
+  }
   __syncthreads();
   if (update_prev && tid < n) s_prev[tid] = s_out[tid];
 }

@@ -149,7 +149,7 @@ int stage_corner_enlarged(qrctm* h) {
 }
 
 // K7: C,T <- sym(Cn,Tn) / ||.||_F
-int stage_normalize(qrctm* h, const double* Cn, const double* Tn) {
+int stage_normalize(qrctm* h, const double* Cn, const double* Tn, bool record = false) {
   const int chi = h->chi, b = h->b;
   long long nT = (long long)chi * b * chi;
   int nbC = (int)(((long long)chi * chi + 255) / 256); if (nbC > 148) nbC = 148;
@@ -157,7 +157,8 @@ int stage_normalize(qrctm* h, const double* Cn, const double* Tn) {
   sym_partial_kernel<<<nbC + nbT, 256, 0, h->stream>>>(Cn, Tn, chi, b, h->symmetrize, h->C, h->T, h->partial,
                                                       nbC, nbT);
   int nb = (int)((nT + (long long)chi * chi + 255) / 256); if (nb > 592) nb = 592;
-  scale_kernel<<<nb, 256, 0, h->stream>>>(h->C, h->T, chi, b, h->partial, nbC, nbT, h->scal, h->flag);
+  scale_kernel<<<nb, 256, 0, h->stream>>>(h->C, h->T, chi, b, h->partial, nbC, nbT, h->scal, h->flag,
+                                          record ? h->hist : nullptr, h->flag + 1, h->R);
   h->launches += 2;
   CU(h, cudaGetLastError());
   return QRCTM_OK;
@@ -185,14 +186,14 @@ int stage_spectrum(qrctm* h, double* s_out, int update_prev, cudaStream_t st) {
     tridiag_smem2_kernel<<<1, TRI2_NT, tri2_smem_bytes(chi), st>>>(h->C, chi, h->dvec, h->evec, nullptr);
     multisect_kernel<<<(chi + 7) / 8, 256, sizeof(double) * (2 * chi + 40), st>>>(h->dvec, h->evec, chi, h->eig);
     spectrum_finalize_kernel<<<1, nt, sizeof(double) * (chi + 40), st>>>(h->eig, chi, s_out, h->s_prev, h->delta,
-                                                                        update_prev);
+                                                                        update_prev, h->hist, h->flag + 1);
     h->launches += 3;
   } else if (tri_bytes <= (size_t)max_smem && chi <= 1024) {
     tridiag_smem_kernel<<<1, 1024, tri_bytes, st>>>(h->C, chi, h->dvec, h->evec);
     multisect_kernel<<<(chi + 7) / 8, 256, sizeof(double) * (2 * chi + 40), st>>>(h->dvec, h->evec, chi,
                                                                                          h->eig);
     spectrum_finalize_kernel<<<1, nt, sizeof(double) * (chi + 40), st>>>(h->eig, chi, s_out, h->s_prev,
-                                                                                 h->delta, update_prev);
+                                                                                 h->delta, update_prev, h->hist, h->flag + 1);
     h->launches += 3;
   } else if (h->k8work && chi <= 1024) {
     // corner too large for one SM's shared memory: the eigen step's multi-CTA tridiagonalisation (eigh_driver.cuh)
@@ -208,7 +209,7 @@ int stage_spectrum(qrctm* h, double* s_out, int update_prev, cudaStream_t st) {
     h->launches += eigh_tridiagonalise(st, chi, h->Wc, wk);
     multisect_kernel<<<(chi + 7) / 8, 256, sizeof(double) * (2 * chi + 40), st>>>(wk.d, wk.e, chi, h->eig);
     spectrum_finalize_kernel<<<1, nt, sizeof(double) * (chi + 40), st>>>(h->eig, chi, s_out, h->s_prev, h->delta,
-                                                                        update_prev);
+                                                                        update_prev, h->hist, h->flag + 1);
     h->launches += 2;
   } else {
     CU(h, cudaMemcpyAsync(h->Wc, h->C, sizeof(double) * chi * chi, cudaMemcpyDeviceToDevice, st));
@@ -243,7 +244,7 @@ int do_step(qrctm* h, cudaEvent_t* ev /* QRCTM_NSTAGE+1 events or null */, bool 
   if (!rc) { mark(4, "K5_project"); rc = stage_project(h, h->S, h->Q, h->Tn); }
   if (!rc) { mark(5, "K6_corner"); rc = h->corner_mode == 0 ? stage_corner_accel(h) : stage_corner_enlarged(h); }
   if (!rc && !with_k7) { nvtxRangePop(); return rc; }
-  if (!rc) { mark(6, "K7_normalize"); rc = stage_normalize(h, h->Cn, h->Tn); }
+  if (!rc) { mark(6, "K7_normalize"); rc = stage_normalize(h, h->Cn, h->Tn, true); }
   if (!rc) mark(7, nullptr); else nvtxRangePop();
   return rc;
 }
@@ -298,7 +299,7 @@ int run_front(qrctm* h, cudaEvent_t* ev) {
 int run_k7(qrctm* h, cudaEvent_t* ev) {
   const bool can = h->use_graph && !ev && h->stream != nullptr && !h->graph_failed && h->warm_steps >= 1;
   if (can && !h->g_k7) {
-    if (!capture_graph(h, [&] { return stage_normalize(h, h->Cn, h->Tn); }, &h->g_k7, &h->g_k7_n)) h->graph_failed = 1;
+    if (!capture_graph(h, [&] { return stage_normalize(h, h->Cn, h->Tn, true); }, &h->g_k7, &h->g_k7_n)) h->graph_failed = 1;
   }
   int rc;
   if (can && h->g_k7) {
@@ -307,7 +308,7 @@ int run_k7(qrctm* h, cudaEvent_t* ev) {
     rc = QRCTM_OK;
   } else {
     if (ev) { nvtxRangePushA("K7_normalize"); cudaEventRecord(ev[6], h->stream); }
-    rc = stage_normalize(h, h->Cn, h->Tn);
+    rc = stage_normalize(h, h->Cn, h->Tn, true);
     if (ev) { cudaEventRecord(ev[7], h->stream); nvtxRangePop(); }
   }
   if (rc == QRCTM_OK) h->warm_steps += 1;

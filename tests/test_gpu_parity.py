@@ -431,6 +431,38 @@ def test_overlapped_check_is_bitwise_identical_to_serial():
         assert np.array_equal(a[i], b[i])
 
 
+def test_history_ring_buffer_matches_oracle_run():
+    """qrctm_get_history: per-iteration delta, ||C'||_F, ||T'||_F, min/max R_kk against the oracle's run history."""
+    A, C0, T0 = gen_config(2, 3, 20, 1)
+    a = o.build_a(A)
+    h = pkg.QRCTM(2, 3, 20)
+    h.set_A(A); h.set_env(C0, T0)
+    it, dl = h.run(12, -1.0)
+    rec, n = h.get_history()
+    assert n == 12 and rec.shape == (12, 4)
+    C, T = o.normalize(C0, T0)
+    s_prev = o.spectrum(C)
+    for k in range(12):
+        st = o.qr_step(C, T, a)
+        d = np.diag(st["R"])
+        assert abs(rec[k, 1] / np.linalg.norm(0.5 * (st["Cn"] + st["Cn"].T)) - 1) < 1e-9
+        assert abs(rec[k, 2] / np.linalg.norm(0.5 * (st["Tn"] + st["Tn"].transpose(2, 1, 0))) - 1) < 1e-9
+        assert abs(rec[k, 3] - d.min() / d.max()) < 1e-9
+        C, T = o.normalize(st["Cn"], st["Tn"])
+        s = o.spectrum(C)
+        assert abs(rec[k, 0] - np.max(np.abs(s - s_prev))) < 1e-11
+        s_prev = s
+    assert rec[-1, 0] == dl
+    h.set_option(pkg.OPT_CHECK_EVERY, 4)
+    h.run(8, -1.0)
+    rec, n = h.get_history(6)
+    assert n == 20 and rec.shape == (6, 4)
+    assert np.isnan(rec[0, 0]) and np.isfinite(rec[1, 0]) and np.isnan(rec[2, 0]) and np.isfinite(rec[5, 0])
+    h.set_env(C0, T0)
+    assert h.get_history()[1] == 0
+    h.close()
+
+
 def test_check_every_option():
     A, C0, T0 = gen_config(2, 2, 8, 0)
     h = pkg.QRCTM(2, 2, 8)
