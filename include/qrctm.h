@@ -219,6 +219,20 @@ int qrctm_gemm_f64_ws(void* cuda_stream, int path, int transA, int M, int N, int
                       const double* A, long long lda, const double* B, long long ldb,
                       double* Cmat, long long ldc, void* work, unsigned long long work_bytes);
 
+/* The same GEMM for callers that cannot allocate (code under CUDA-graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): Cmat[M][N] = op(A) * B as qrctm_gemm_f64_ws (DMMA path), but the K-splitting scratch (split-K
+ * partial outputs / stream-K partial tiles) is a file-scope device array inside the library -- 16 MiB on every GPU
+ * that loads libqrctm.so, held until the process exits.  The call itself allocates nothing (no cudaMalloc / cudaFree,
+ * no allocating library routine); inputs and the output are the caller's DEVICE buffers.
+ * Limit: M * N <= 65536 (e.g. the chi x chi Gram and corner products with long K); larger shapes are rejected with
+ * QRCTM_ERR_INVALID_ARG and a text in qrctm_noalloc_last_error() (thread-local; empty after a successful call).
+ * The scratch is SHARED by every call on that GPU and keeps the last call's contents: nothing in it has to start at
+ * zero (every partial the reduction reads is written by the same call first), but two calls that overlap on the GPU
+ * (different streams, or graphs replayed concurrently) race on it -- serialise them. */
+int qrctm_gemm_f64_noalloc(void* cuda_stream, int transA, int M, int N, int K, const double* A, long long lda,
+                           const double* B, long long ldb, double* Cmat, long long ldc);
+const char* qrctm_noalloc_last_error(void);
+
 /* Stand-alone QR entry (K2): factor X[rows][cols] (DEVICE, row-major, cols <=
  * rows) into Q[rows][cols], R[cols][cols] with diag(R) >= 0 (path: see
  * QRCTM_OPT_QR_PATH; path 0 synchronises the stream once to read the device-side accuracy verdict). work must hold

@@ -31,7 +31,7 @@ SYMBOLS = (
     "qrctm_set_A", "qrctm_set_env", "qrctm_step", "qrctm_run", "qrctm_get_env",
     "qrctm_get_corner_spectrum", "qrctm_get_qr", "qrctm_get_raw", "qrctm_get_a", "qrctm_norm_per_site",
     "qrctm_r_diag_ratio", "qrctm_energy_nn", "qrctm_edge_update", "qrctm_set_option", "qrctm_launch_count", "qrctm_get_history", "qrctm_get_stage_ms", "qrctm_profile_step",
-    "qrctm_gemm_f64", "qrctm_gemm_f64_ws", "qrctm_qr_work_bytes", "qrctm_qr_f64", "qrctm_probe_fp64", "qrctm_last_error",
+    "qrctm_gemm_f64", "qrctm_gemm_f64_ws", "qrctm_gemm_f64_noalloc", "qrctm_noalloc_last_error", "qrctm_qr_work_bytes", "qrctm_qr_f64", "qrctm_probe_fp64", "qrctm_last_error",
     "qrctm_version",
     "qrctm_get_chi", "qrctm_init_bulk", "qrctm_eig_step", "qrctm_get_eig", "qrctm_warmup",
     "qrctm_eigh_work_bytes", "qrctm_eigh_top_f64", "qrctm_chol_inv_f64", "qrctm_tridiag_f64",
@@ -85,6 +85,8 @@ def load_library() -> ctypes.CDLL:
                                    c_longlong]
     lib.qrctm_gemm_f64_ws.argtypes = [P, c_int, c_int, c_int, c_int, c_int, P, c_longlong, P, c_longlong, P,
                                       c_longlong, P, c_ulonglong]
+    lib.qrctm_gemm_f64_noalloc.argtypes = [P, c_int, c_int, c_int, c_int, P, c_longlong, P, c_longlong, P, c_longlong]
+    lib.qrctm_noalloc_last_error.restype = c_char_p
     lib.qrctm_qr_work_bytes.argtypes = [c_int, c_int]
     lib.qrctm_qr_work_bytes.restype = c_ulonglong
     lib.qrctm_qr_f64.argtypes = [P, c_int, c_int, c_int, P, P, P, P]
@@ -380,6 +382,25 @@ def gemm_f64(A, B, transA: bool = False, path: int = 0, work_bytes: int = 0):
                                 _ptr(out), N)
     if rc != QRCTM_OK:
         raise QrctmError(f"qrctm_gemm_f64 failed: {rc}")
+    return out
+
+
+def gemm_f64_noalloc(A, B, out, transA: bool = False):
+    """out[M,N] = op(A) @ B through qrctm_gemm_f64_noalloc: the library allocates nothing (static device scratch);
+    `out` is the caller's CUDA float64 tensor.  M * N <= 65536."""
+    import torch
+    lib = load_library()
+    K, N = B.shape
+    M = A.shape[1] if transA else A.shape[0]
+    assert (A.shape[0] if transA else A.shape[1]) == K and tuple(out.shape) == (M, N)
+    for t in (A, B, out):
+        if t.dtype != torch.float64 or not t.is_cuda or t.stride(1) != 1:
+            raise QrctmError("gemm_f64_noalloc wants CUDA float64 matrices with unit column stride")
+    rc = lib.qrctm_gemm_f64_noalloc(c_void_p(torch.cuda.current_stream().cuda_stream), int(transA), M, N, K,
+                                    c_void_p(A.data_ptr()), A.stride(0), c_void_p(B.data_ptr()), B.stride(0),
+                                    c_void_p(out.data_ptr()), out.stride(0))
+    if rc != QRCTM_OK:
+        raise QrctmError(f"qrctm_gemm_f64_noalloc failed ({rc}): {lib.qrctm_noalloc_last_error().decode()}")
     return out
 
 

@@ -694,6 +694,53 @@ int qrctm_gemm_f64_ws(void* cuda_stream, int path, int transA, int M, int N, int
   return nl < 0 ? QRCTM_ERR_CUDA : QRCTM_OK;
 }
 
+}  // extern "C"
+
+// ---- allocation-free GEMM entry: the K-splitting scratch lives in a file-scope device array (16 MiB on every GPU that
+// loads the library, until exit).  In host code `g_noalloc_scratch` is only a stand-in for the symbol: the device
+// address is looked up once per device with cudaGetSymbolAddress and that pointer is what the kernels get.
+namespace {
+constexpr size_t kNoAllocElems = (size_t)1 << 21;                 // 2 Mi doubles = 16 MiB
+constexpr long long kNoAllocMaxMN = 65536;                        // M * N of one call (32 K-splits of it fit the array)
+constexpr int kNoAllocMaxDev = 64;
+}  // namespace
+static __device__ __align__(256) double g_noalloc_scratch[kNoAllocElems];
+namespace {
+double* g_noalloc_ptr[kNoAllocMaxDev];                            // per device, filled on first use
+thread_local char g_noalloc_err[200] = "";
+int noalloc_fail(int code, const char* what, cudaError_t e = cudaSuccess) {
+  if (e != cudaSuccess) snprintf(g_noalloc_err, sizeof(g_noalloc_err), "%s: %s", what, cudaGetErrorString(e));
+  else snprintf(g_noalloc_err, sizeof(g_noalloc_err), "%s", what);
+  return code;
+}
+}  // namespace
+
+extern "C" {
+
+const char* qrctm_noalloc_last_error(void) { return g_noalloc_err; }
+
+int qrctm_gemm_f64_noalloc(void* cuda_stream, int transA, int M, int N, int K, const double* A, long long lda,
+                           const double* B, long long ldb, double* Cmat, long long ldc) {
+  g_noalloc_err[0] = 0;
+  if (!A || !B || !Cmat || M < 1 || N < 1 || K < 1) return noalloc_fail(QRCTM_ERR_INVALID_ARG, "null pointer or empty shape");
+  if ((long long)M * N > kNoAllocMaxMN)
+    return noalloc_fail(QRCTM_ERR_INVALID_ARG, "qrctm_gemm_f64_noalloc: M * N exceeds 65536 (the static scratch holds 32 K-splits of a 65536-element output); use qrctm_gemm_f64_ws");
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) { cudaGetLastError(); return noalloc_fail(QRCTM_ERR_CUDA, "cudaGetDevice", e); }
+  if (dev < 0 || dev >= kNoAllocMaxDev) return noalloc_fail(QRCTM_ERR_INVALID_ARG, "device index beyond 63");
+  if (!g_noalloc_ptr[dev]) {                                      // once per device, with that device current
+    double* p = nullptr;
+    e = cudaGetSymbolAddress((void**)&p, g_noalloc_scratch);
+    if (e != cudaSuccess || !p) { cudaGetLastError(); return noalloc_fail(QRCTM_ERR_CUDA, "cudaGetSymbolAddress(g_noalloc_scratch)", e); }
+    g_noalloc_ptr[dev] = p;
+  }
+  GemmCall c{A, lda, transA ? 1 : 0, B, ldb, Cmat, plain_map(ldc), IndexMap{1, 1, 0}, M, N, K, 0};
+  int nl = launch_gemm(static_cast<cudaStream_t>(cuda_stream), 0, c, g_noalloc_ptr[dev], kNoAllocElems, &e);
+  if (nl < 0) return noalloc_fail(QRCTM_ERR_CUDA, "gemm launch", e);
+  return QRCTM_OK;
+}
+
 unsigned long long qrctm_qr_work_bytes(int rows, int cols) { return qr_work_bytes_impl(rows, cols); }
 
 int qrctm_qr_f64(void* cuda_stream, int path, int rows, int cols, const double* X, double* Q, double* R,
