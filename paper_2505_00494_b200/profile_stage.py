@@ -23,10 +23,14 @@ def main():
     ap.add_argument("--steps", type=int, default=2)
     ap.add_argument("--warmup", type=int, default=-1)
     ap.add_argument("--eig-steps", type=int, default=0)
+    ap.add_argument("--qr-path", type=int, default=0, help="QRCTM_OPT_QR_PATH (0 automatic / CholeskyQR2, 2 blocked Householder, ...)")
+    ap.add_argument("--absorb-mode", type=int, default=0, help="QRCTM_OPT_ABSORB_MODE")
     a = ap.parse_args()
     A, C0, T0, c = gen_named(a.config)
     h = pkg.QRCTM(c["d"], c["D"], c["chi"])
     h.set_option(pkg.OPT_USE_GRAPH, 0)          # plain launches keep the NVTX stage ranges
+    h.set_option(pkg.OPT_QR_PATH, a.qr_path)
+    h.set_option(pkg.OPT_ABSORB_MODE, a.absorb_mode)
     h.set_A(A)
     if a.warmup >= 0:
         h.warmup(a.warmup)
