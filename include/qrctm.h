@@ -76,7 +76,7 @@ enum {
   QRCTM_OPT_USE_GRAPH = 8,   /* 1 [default] = K1..K6 and K7 are captured once into CUDA graphs and replayed by
                                 qrctm_step / qrctm_run (needs a non-default stream); 0 = plain launches, which keep
                                 the per-stage NVTX ranges for profilers */
-  QRCTM_OPT_K8_PATH = 10,    /* K8 tridiagonalisation for chi <= 232: 0 [default] = the thread-per-column kernel (un-
+  QRCTM_OPT_K8_PATH = 10,    /* K8 tridiagonalisation for chi <= 216: 0 [default] = the thread-per-column kernel (un-
                                 normalised reflectors, 2 barriers per step), 1 = the round-1 kernel (for cross-checks) */
   QRCTM_OPT_ABSORB_MODE = 9  /* K4: 0 [default] = contract with the explicit double-layer tensor a (2 chi^2 D^8 flops),
                                 1 = layered: contract with the ket and the bra copy of A in turn (4 d chi^2 D^6
@@ -254,7 +254,7 @@ int qrctm_chol_inv_f64(void* cuda_stream, int n, const double* G, double* R, dou
                        long long* prof);
 
 /* Stand-alone entry of K8's tridiagonalisation (csrc/spectrum.cuh; for the sub-step parity tests): the symmetric
- * C[n][n] (DEVICE; lower triangle read, untouched), n <= 232, is reduced by Householder similarity transforms to the
+ * C[n][n] (DEVICE; lower triangle read, untouched), n <= 216, is reduced by Householder similarity transforms to the
  * tridiagonal matrix with diagonal d[n] and sub-diagonal e[1..n-1] (e[0] = 0) (DEVICE).  prof = NULL, or 8 DEVICE
  * long longs: SM cycles of the kernel's phases.  One CTA; asynchronous on the stream. */
 int qrctm_tridiag_f64(void* cuda_stream, int n, const double* C, double* d, double* e, long long* prof);

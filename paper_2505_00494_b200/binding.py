@@ -441,7 +441,7 @@ def chol_inv_f64(G, profile: bool = False):
 
 
 def tridiag_f64(C, profile: bool = False):
-    """(d, e[, cycles]) of a symmetric torch CUDA float64 matrix (n <= 232) through qrctm_tridiag_f64."""
+    """(d, e[, cycles]) of a symmetric torch CUDA float64 matrix (n <= 216) through qrctm_tridiag_f64."""
     import torch
     lib = load_library()
     n = C.shape[0]

@@ -255,24 +255,34 @@ tridiag_smem_kernel(const double* __restrict__ Cmat, int n, double* __restrict__
 //     formed on the fly.
 // Two barriers per step.  Output as tridiag_smem_kernel (d, e; e[0] = 0); the similarity transform differs from
 // LAPACK's only in the scaling of u, so the eigenvalues agree to rounding.
-constexpr int TRI2_NT = 1024, TRI2_NA = 256, TRI2_NWA = TRI2_NA / 32, TRI2_MAX_N = 232;
+constexpr int TRI2_NT = 1024, TRI2_MAX_N = 216, TRI2_MAXSUB = 8, TRI2_MAXCG = (TRI2_MAX_N + 31) / 32;
 __host__ __device__ inline size_t tri2_smem_bytes(int n) {
-  return sizeof(double) * ((size_t)n * (n + 1) / 2 + 1 + 4 * (size_t)n + 16 + 8);
+  return sizeof(double) * ((size_t)n * (n + 1) / 2 + 1 + (4 + TRI2_MAXSUB) * (size_t)n + 16);
 }
 
-// 1024 threads.  Threads 0..255 ("group A", one per column) compute the reflector and p = gamma A u; all 32 warps
-// share the rank-2 update: warp w owns the 32 columns of group w & 7 and the rows congruent to (w >> 3) modulo 4
-// below them, so a column's dependent load-FMA-store chain is split four ways and unrolled four deep.
+// 1024 threads = 32 warps, four barriers per step.  What bounds this kernel is the ISSUE rate of one SM (ncu: the
+// matrix-vector and update loops are "not selected" / issue limited once all 32 warps work), so scalar work is done
+// by ONE warp and broadcast through shared memory (a barrier costs ~70 cycles, redundant scalar code in 32 warps
+// ~1000), and the two O(n^2) loops are written for few instructions per element (contiguous row chunks per warp,
+// immediate offsets, incremental triangular offsets):
+//   R  warp 0: reflector scalars of column k (one rsqrt, one reciprocal), u_{k+1} written in place, and the table
+//      that deals the warps out for phase U                                                              -- barrier
+//   M  p = A u: the active column groups (32 columns each) share the warps evenly, the wpg <= 8 warps of a group
+//      take contiguous row chunks and leave partial sums part[sub][j]                                    -- barrier
+//   C  thread j sums the partials in a fixed order: p_j = gamma sum_sub part[sub][j]; p.u                -- barrier
+//   U  rank-2 update of the lower triangle, warps dealt out to the column groups in proportion to the groups'
+//      heights (the first group's columns are n - k rows tall, the last one's a few); the owner of column k+1 also
+//      leaves it as the next u                                                                           -- barrier
 __global__ void __launch_bounds__(TRI2_NT, 1)
 tridiag_smem2_kernel(const double* __restrict__ Cmat, int n, double* __restrict__ dvec, double* __restrict__ evec,
                      long long* __restrict__ prof /* null, or 8 cycle counters of the phases (thread 0) */) {
   extern __shared__ __align__(16) double tsm[];
-  // (u_i, p_i) pairs, double-buffered over the steps: u = column k of the matrix (written by the thread that owns the
-  // column while it updates it in the step before), p = gamma A u (written by thread i in the matrix-vector phase)
-  double2* up0 = reinterpret_cast<double2*>(tsm);               // 2 x n pairs
-  double* red = tsm + 4 * n;                                    // 8: per-warp partial sums of p.u
-  double* sc = red + 8;                                         // 8: [0] gamma of this step (0: nothing to eliminate)
-  double* L = sc + 8;                                           // n(n+1)/2
+  double2* up0 = reinterpret_cast<double2*>(tsm);               // 2 x n pairs (u_i, p_i), double-buffered over the steps
+  double* part = tsm + 4 * n;                                   // TRI2_MAXSUB x n partial sums of A u
+  double* red = part + TRI2_MAXSUB * n;                         // 8: per-warp partial sums of p.u
+  double* sc = red + 8;                                         // [0] gamma (0: nothing to eliminate)
+  double* L = red + 16;                                         // n(n+1)/2
+  __shared__ int tab[32];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   long long tp[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tc = 0;
 #define TRI_TICK(i) do { if (prof && tid == 0) { const long long t_ = clock64(); tp[i] += t_ - tc; tc = t_; } } while (0)
@@ -285,101 +295,179 @@ tridiag_smem2_kernel(const double* __restrict__ Cmat, int n, double* __restrict_
     }
   __syncthreads();
   TRI_TICK(0);
-  const int cg = warp & 7, rph = warp >> 3;     // column group, row phase (rph = 0: group A)
-  const int j = cg * 32 + lane, tj = tri_off(j);               // my column; start of my row
-  const int jlo = cg * 32, jhi = jlo + 32 < n ? jlo + 32 : n;  // the columns of my warp
-  const double* Lj = L + tj;                    // my row: element (j, i), i <= j
-  double* Lc = L + j;                           // my column: element (i, j) at Lc[tri(i)], i >= j
+  const int ncgt = (n + 31) >> 5;
   for (int k = 0; k < n - 2; ++k) {
     double2* up = up0 + (k & 1) * n;
     double2* upn = up0 + ((k + 1) & 1) * n;
-    const bool active = j > k && j < n;
-    const bool wact = jlo < n && jhi > k + 1;    // warp-uniform: some lane of this warp is active
-    if (rph == 0) {
-      // ---- reflector of column k (rows k+1 .. n-1), redundantly in every warp of group A
+    const int c0 = (k + 1) >> 5, ncg = ncgt - c0;
+    // ---- R (warp 0): reflector of column k (rows k+1 .. n-1), warp table of phase U
+    if (warp == 0) {
       double acc = 0.0;
       for (int i = k + 2 + lane; i < n; i += 32) { const double x = up[i].x; acc = fma(x, x, acc); }
       const double tail2 = warp_sum(acc);
       const double alpha = up[k + 1].x;
-      if (tid == 0) dvec[k] = L[tri_off(k) + k];
+      __syncwarp();
       // nothing to eliminate: H = I.  Entries below 1e-140 in magnitude are dropped rather than eliminated: gamma ~
       // 1 / tail2 would overflow, and the perturbation is 120 orders below rounding for ||C|| ~ 1
       if (!(tail2 > 1e-280)) {
-        if (tid == 0) { evec[k + 1] = alpha; sc[0] = 0.0; }
-        for (int i = k + 2 + tid; i < n; i += TRI2_NA) upn[i].x = L[tri_off(i) + k + 1];
+        if (lane == 0) { dvec[k] = L[tri_off(k) + k]; evec[k + 1] = alpha; sc[0] = 0.0; }
       } else {
         const double s2 = fma(alpha, alpha, tail2);
         const double sigma = s2 * rsqrt(s2);                     // 1-2 ulp: only perturbs e_{k+1} at rounding level
         const double beta = alpha >= 0.0 ? -sigma : sigma;
-        const double u1 = alpha - beta;
         const double gamma = __drcp_rn(fma(-alpha, beta, s2));   // 1 / (beta (beta - alpha)),  beta^2 = s2
-        if (tid == 0) { evec[k + 1] = beta; sc[0] = gamma; }
-        TRI_TICK(1);
-        // ---- p_j = gamma sum_{i > k} A_sym[i][j] u_i for my column: rows above my warp's columns come from my row
-        // (per-lane base + uniform offset), rows below them from my column (uniform row start + lane), the <= 32
-        // rows in between are mixed
-        double uj = 0.0, pj = 0.0;
-        if (wact) {
-          const int jc = active ? j : (k + 1 > jlo ? k + 1 : jlo);  // inactive lanes compute a valid column (discarded)
-          const double* Ljc = active ? Lj : L + tri_off(jc);
-          const double* Lcc = L + jc;
-          uj = (jc == k + 1) ? u1 : up[jc].x;
-          double a0 = Ljc[k + 1] * u1, a1 = 0.0;                  // i = k+1: element (jc, k+1)
-          int i = k + 2;
-          const int e1 = jlo < n ? jlo : n;
-          for (; i + 2 <= e1; i += 2) {                           // rows above the warp's columns: my row
-            a0 = fma(Ljc[i], up[i].x, a0);
-            a1 = fma(Ljc[i + 1], up[i + 1].x, a1);
+        if (lane == 0) {
+          dvec[k] = L[tri_off(k) + k]; evec[k + 1] = beta; sc[0] = gamma;
+          up[k + 1].x = alpha - beta;                            // u_{k+1}: H = I - gamma u u^T, u = x - beta e_1
+        }
+      }
+      // every 8 steps: deal the 32 warps out to the active column groups for phase U, in proportion to the groups'
+      // heights h_c = n - max(32 c, k+1) (a table that is up to 7 steps old only balances slightly worse: rows and
+      // columns that have left the active block are skipped by the lanes themselves)
+      if ((k & 7) == 0) {
+        const int c = c0 + lane;                                  // lane <-> active column group
+        const int h = (lane < ncg) ? n - ((c << 5) > k + 1 ? (c << 5) : k + 1) : 0;
+        int cum = h;
+#pragma unroll
+        for (int o = 1; o < 8; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, cum, o); if (lane >= o) cum += v; }
+        const int H = __shfl_sync(0xffffffffu, cum, ncg - 1);
+        int B = (lane == ncg - 1) ? 32 : (int)((float)cum * __fdividef(32.0f, (float)H));
+        int m = B - lane;                                         // at least one warp per group: B_c >= B_c' + (c - c')
+#pragma unroll
+        for (int o = 1; o < 8; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, m, o); if (lane >= o) m = m > v ? m : v; }
+        B = m + lane;
+        const int room = 32 - (ncg - 1 - lane);                   // ... and one left for every later group
+        B = B < room ? B : room;
+        int t = 0xff;
+        for (int cc = 0; cc < ncg; ++cc) {
+          const int hi = __shfl_sync(0xffffffffu, B, cc), lo = cc ? __shfl_sync(0xffffffffu, B, cc - 1) : 0;
+          const int hh = __shfl_sync(0xffffffffu, h, cc);
+          if (lane >= lo && lane < hi) {
+            const int cnt = hi - lo;
+            t = (c0 + cc) | ((lane - lo) << 8) | (((hh + cnt - 1) / cnt) << 16);        // group, sub, rows per warp
           }
+        }
+        tab[lane] = t;
+      }
+    }
+    TRI_TICK(1);
+    __syncthreads();
+    const double gamma = sc[0];
+    if (gamma == 0.0) {
+      for (int i = k + 2 + tid; i < n; i += TRI2_NT) upn[i].x = L[tri_off(i) + k + 1];
+      __syncthreads();
+      continue;
+    }
+    // ---- M: partial sums of A u
+    const int wpg = ncg <= 4 ? 8 : (ncg == 5 ? 6 : (ncg == 6 ? 5 : 4));
+    {
+      const int g = wpg == 8 ? warp >> 3 : (wpg == 6 ? warp / 6 : (wpg == 5 ? warp / 5 : warp >> 2));
+      const int sub = warp - g * wpg;
+      if (g < ncg) {
+        const int jlo = (c0 + g) << 5, jhi = jlo + 32 < n ? jlo + 32 : n;
+        const int j = jlo + lane;
+        const int jc = j < k + 1 ? k + 1 : (j < n ? j : n - 1);  // out-of-range lanes compute a valid column (discarded)
+        const double* Lrow = L + tri_off(jc);                    // element (jc, i), i <= jc
+        const double* Lcol = L + jc;                             // element (i, jc) at Lcol[tri(i)], i >= jc
+        const int na = n - (k + 1);
+        const int chunk = wpg == 8 ? (na + 7) >> 3 : (wpg == 6 ? (na + 5) / 6 : (wpg == 5 ? (na + 4) / 5 : (na + 3) >> 2));
+        const int r0 = k + 1 + sub * chunk, r1 = r0 + chunk < n ? r0 + chunk : n;
+        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+        int i = r0;
+        {                                                        // rows above the group's columns: my row, contiguous
+          const int e = r1 < jlo ? r1 : jlo;
+          for (; i + 4 <= e; i += 4) {
+            a0 = fma(Lrow[i], up[i].x, a0);
+            a1 = fma(Lrow[i + 1], up[i + 1].x, a1);
+            a2 = fma(Lrow[i + 2], up[i + 2].x, a2);
+            a3 = fma(Lrow[i + 3], up[i + 3].x, a3);
+          }
+          for (; i < e; ++i) a0 = fma(Lrow[i], up[i].x, a0);
+        }
+        {                                                        // rows inside the group's columns: row or column
+          const int e = r1 < jhi ? r1 : jhi;
           int off = tri_off(i);
-          for (; i < jhi; ++i) {                                  // mixed rows
-            a0 = fma(i < jc ? Ljc[i] : Lcc[off], up[i].x, a0);
-            off += i + 1;
-          }
-          for (; i + 2 <= n; i += 2) {                            // rows below: my column
-            a0 = fma(Lcc[off], up[i].x, a0);
-            a1 = fma(Lcc[off + i + 1], up[i + 1].x, a1);
+          for (; i + 2 <= e; i += 2) {
+            a1 = fma(i >= jc ? Lcol[off] : Lrow[i], up[i].x, a1);
+            a2 = fma(i + 1 >= jc ? Lcol[off + i + 1] : Lrow[i + 1], up[i + 1].x, a2);
             off += 2 * i + 3;
           }
-          if (i < n) a0 = fma(Lcc[off], up[i].x, a0);
-          pj = active ? gamma * (a0 + a1) : 0.0;
-          if (active) up[j] = make_double2(uj, pj); else uj = 0.0;   // (u_{k+1} = u1 replaces the raw column entry)
+          if (i < e) { a3 = fma(i >= jc ? Lcol[off] : Lrow[i], up[i].x, a3); ++i; }
         }
-        const double q = warp_sum(pj * uj);
-        if (lane == 0) red[warp] = q;
+        if (i < r1) {                                            // rows below: my column, incremental offsets
+          int off = tri_off(i);
+          for (; i + 4 <= r1; i += 4) {
+            const int o1 = off + i + 1, o2 = o1 + i + 2, o3 = o2 + i + 3;
+            a0 = fma(Lcol[off], up[i].x, a0);
+            a1 = fma(Lcol[o1], up[i + 1].x, a1);
+            a2 = fma(Lcol[o2], up[i + 2].x, a2);
+            a3 = fma(Lcol[o3], up[i + 3].x, a3);
+            off = o3 + i + 4;
+          }
+          for (; i < r1; ++i) { a0 = fma(Lcol[off], up[i].x, a0); off += i + 1; }
+        }
+        if (j >= k + 1 && j < n) part[sub * n + j] = (a0 + a1) + (a2 + a3);
       }
     }
     TRI_TICK(2);
     __syncthreads();
+    // ---- C: p_j, p.u
+    if (warp < 8) {
+      double pj = 0.0, uj = 0.0;
+      if (tid < n && tid > k) {
+        double sum = 0.0;
+        for (int q = 0; q < wpg; ++q) sum += part[q * n + tid];
+        pj = gamma * sum;
+        uj = up[tid].x;
+        up[tid].y = pj;
+      }
+      const double q = warp_sum(pj * uj);
+      if (lane == 0) red[warp] = q;
+    }
     TRI_TICK(3);
-    const double gamma = sc[0];
-    // ---- A -= u w^T + w u^T: x = A_ij - u_i (p_j - 2 cf u_j) - p_i u_j,  cf = (gamma/2) p.u
-    if (gamma != 0.0 && wact && active) {
-      double pu = 0.0;
+    __syncthreads();
+    // ---- U: A -= u w^T + w u^T: x = A_ij - u_i (p_j - 2 cf u_j) - p_i u_j,  cf = (gamma/2) p.u
+    {
+      const int t = tab[warp];
+      const int cgm = t & 0xff;
+      if (cgm != 0xff) {
+        const int sub = (t >> 8) & 0xff, chunk = t >> 16;
+        const int jlo = cgm << 5;
+        const int j = jlo + lane;
+        const bool active = j > k && j < n;
+        const int k8 = (k & ~7) + 1;                             // the table was built at step k & ~7
+        const int start = jlo > k8 ? jlo : k8;
+        const int r0 = start + sub * chunk, r1 = r0 + chunk < n ? r0 + chunk : n;
+        if (active) {
+          double pu = 0.0;
 #pragma unroll
-      for (int w = 0; w < TRI2_NWA; ++w) pu += red[w];
-      const double cf = 0.5 * gamma * pu;
-      const double2 mine = up[j];
-      const double aj = fma(-2.0 * cf, mine.x, mine.y), bj = mine.x;
-      const bool nxt = j == k + 1;                              // my column is the next u
-      const int ib = (jlo > k + 1 ? jlo : k + 1) + rph;         // warp-uniform first row of my phase; lanes join at i >= j
-      for (int i = ib; i < n; i += 16) {
-        double2 u[4]; double y[4]; int o[4]; bool ok[4];
-#pragma unroll
-        for (int r = 0; r < 4; ++r) {
-          const int ii = i + 4 * r;
-          ok[r] = ii < n && ii >= j;
-          o[r] = tri_off(ok[r] ? ii : j);
-          u[r] = up[ok[r] ? ii : j];
-          y[r] = Lc[o[r]];
-        }
-#pragma unroll
-        for (int r = 0; r < 4; ++r) y[r] = fma(-u[r].y, bj, fma(-u[r].x, aj, y[r]));
-#pragma unroll
-        for (int r = 0; r < 4; ++r) {
-          if (ok[r]) {
-            Lc[o[r]] = y[r];
-            if (nxt) upn[i + 4 * r].x = y[r];
+          for (int w = 0; w < 8; ++w) pu += red[w];
+          const double cf = 0.5 * gamma * pu;
+          const double2 mine = up[j];
+          const double aj = fma(-2.0 * cf, mine.x, mine.y), bj = mine.x;
+          const bool nxt = j == k + 1;                           // my column is the next u
+          double* Lc = L + j;
+          int i = r0 > j ? r0 : j;                               // rows above my diagonal element are not mine
+          if (i < r1) {
+            int off = tri_off(i);
+            for (; i + 4 <= r1; i += 4) {
+              const int o1 = off + i + 1, o2 = o1 + i + 2, o3 = o2 + i + 3;
+              const double2 u0 = up[i], u1v = up[i + 1], u2 = up[i + 2], u3 = up[i + 3];
+              const double x0 = fma(-u0.y, bj, fma(-u0.x, aj, Lc[off]));
+              const double x1 = fma(-u1v.y, bj, fma(-u1v.x, aj, Lc[o1]));
+              const double x2 = fma(-u2.y, bj, fma(-u2.x, aj, Lc[o2]));
+              const double x3 = fma(-u3.y, bj, fma(-u3.x, aj, Lc[o3]));
+              Lc[off] = x0; Lc[o1] = x1; Lc[o2] = x2; Lc[o3] = x3;
+              if (nxt) { upn[i].x = x0; upn[i + 1].x = x1; upn[i + 2].x = x2; upn[i + 3].x = x3; }
+              off = o3 + i + 4;
+            }
+            for (; i < r1; ++i) {
+              const double2 ui = up[i];
+              const double x = fma(-ui.y, bj, fma(-ui.x, aj, Lc[off]));
+              Lc[off] = x;
+              if (nxt) upn[i].x = x;
+              off += i + 1;
+            }
           }
         }
       }

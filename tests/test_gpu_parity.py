@@ -343,7 +343,7 @@ def test_spectrum_kernel_against_lapack():
         h.close()
 
 
-@pytest.mark.parametrize("n", [1, 2, 3, 8, 33, 64, 100, 196, 232])
+@pytest.mark.parametrize("n", [1, 2, 3, 8, 31, 32, 33, 64, 65, 100, 161, 196, 216])
 def test_tridiag_kernel_preserves_the_spectrum(n):
     """qrctm_tridiag_f64 (K8's first stage): the tridiagonal (d, e) it returns is orthogonally similar to C, so the
     eigenvalues agree with LAPACK's to rounding; also on a rank-one matrix (the trailing block is rounding noise)."""
