@@ -392,7 +392,10 @@ def main():
                    "k4_algorithmic_gflop": fl_l / 1e9, "k4_tflops": fl_l / (k4l * 1e-3) / 1e12,
                    "k4_algorithmic_gbytes": by_l / 1e9, "k4_gbs": by_l / (k4l * 1e-3) / 1e9,
                    "note": "QRCTM_OPT_ABSORB_MODE=1: P contracted with the ket and bra copies of A in turn "
-                           "(4 d chi^2 D^6 flops instead of 2 chi^2 D^8); not the headline path"}
+                           "(4 d chi^2 D^6 flops instead of 2 chi^2 D^8); not the headline path (the north_star's "
+                           "roofline target is quoted on the explicit double-layer tensor); QRCTM_OPT_ABSORB_MODE=2 "
+                           "(automatic) selects it for D >= 6",
+                   "auto_mode_selects": "layered" if D >= 6 and 4 * d <= b else "explicit"}
         h.set_option(pkg.OPT_ABSORB_MODE, 0)
         h.set_env(C0, T0)
         h.run(2, -1.0)

@@ -80,7 +80,9 @@ enum {
                                 normalised reflectors, 2 barriers per step), 1 = the round-1 kernel (for cross-checks) */
   QRCTM_OPT_ABSORB_MODE = 9  /* K4: 0 [default] = contract with the explicit double-layer tensor a (2 chi^2 D^8 flops),
                                 1 = layered: contract with the ket and the bra copy of A in turn (4 d chi^2 D^6
-                                flops; same T' up to rounding; needs even chi, otherwise mode 0 is used) */
+                                flops; same T' up to rounding; needs even chi, otherwise mode 0 is used),
+                                2 = automatic: layered where it was measured faster on a B200: D >= 6 (and 4 d <= D^2,
+                                even chi), explicit otherwise */
 };
 
 /* Create a handle for dimensions (d, D, chi); allocates every workspace with

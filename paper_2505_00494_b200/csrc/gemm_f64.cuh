@@ -55,7 +55,11 @@ struct GemmArgs {
   long long zo = 0;
   int nz = 1;                // number of z slices (splits or batches) -- work list of the ws kernel
   int epi = 0;               // ws kernel epilogue: 0 = fragments straight to global, 1 = staged through shared
-                             // memory so that the 32 lanes of a store run along the column index j
+                             // memory so that the 32 lanes of a store run along the column index j, 2 = dense
+                             // blocks: the columns come in groups of dense_wc whose 8-row blocks are contiguous in
+                             // the output (row stride dense_wc); each block leaves with ONE bulk store from shared
+                             // memory (cp.async.bulk.global.shared::cta, SASS UBLKCP) instead of 8 * dense_wc stores
+  int dense_wc = 0, dense_magic = 0;   // epi 2: group width, ceil(65536 / dense_wc) (c / wc = c * magic >> 16, c < 128)
   // stream-K (ws kernel, nz = 1, no batch): the tiles x k-tiles units are dealt out evenly and contiguously to the
   // gridDim.x CTAs; a CTA that covers only part of a tile's k range writes a plain BM x BN partial tile to slot
   // 2 * blockIdx.x (its first segment) or 2 * blockIdx.x + 1 (its last) of sk_ws, and streamk_fixup sums the
@@ -273,12 +277,25 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
+__device__ __forceinline__ void bulk_s2g(void* gdst, const void* ssrc, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;\n"
+               ::"l"(gdst), "r"(smem_u32(ssrc)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;\n" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;\n" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;\n" ::: "memory"); }
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory"); }
+
 __device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* tm, int c0, int c1, uint64_t* bar) {
   asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];\n"
                ::"r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(smem_u32(bar)) : "memory");
 }
 
-template <int BM, int BN, int WM, int WN, int STAGES, bool SK = false>
+//   * RESB = true ("resident B", short-K GEMMs whose N fits one tile -- the two contractions of the layered absorption,
+//     K = D^2 and d D^2): the whole K x N operand B is fetched ONCE per CTA into its own shared-memory region, the ring
+//     streams only A tiles, and the CTAs are persistent (grid = resident CTA slots, work items dealt round robin), so
+//     the producer warp prefetches the next tile's A rows while the consumers are still storing the previous tile.
+template <int BM, int BN, int WM, int WN, int STAGES, bool SK = false, bool RESB = false>
 __global__ void __launch_bounds__(((BM / WM) * (BN / WN) + 1) * 32, ((BM / WM) * (BN / WN) <= 4 ? 2 : 1))
 gemm_f64_dmma_ws(const __grid_constant__ GemmArgs p) {
   constexpr int NW_M = BM / WM, NW_N = BN / WN, NCW = NW_M * NW_N;
@@ -288,9 +305,12 @@ gemm_f64_dmma_ws(const __grid_constant__ GemmArgs p) {
   static_assert(BK == 16, "one copy per lane: 16 A rows + 16 B rows");
   extern __shared__ __align__(128) double smem[];
   double* As = smem;
-  double* Bs = smem + STAGES * A_STAGE;
-  uint64_t* full = reinterpret_cast<uint64_t*>(Bs + STAGES * B_STAGE);
+  double* Bs = smem + STAGES * A_STAGE;                 // RESB: all ceil(K / BK) k-tiles of B, else the ring's B stages
+  const int nbst = RESB ? (p.K + BK - 1) / BK : STAGES;
+  uint64_t* full = reinterpret_cast<uint64_t*>(Bs + nbst * B_STAGE);
   uint64_t* empty = full + STAGES;
+  uint64_t* bfull = empty + STAGES;                     // RESB: B has landed (one phase per CTA)
+  double* slabs = reinterpret_cast<double*>(empty + STAGES + 2);
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   // Persistent CTA: work items w = (z, tile_m, tile_n), tile_n fastest; the smem ring and its
@@ -304,6 +324,7 @@ gemm_f64_dmma_ws(const __grid_constant__ GemmArgs p) {
 
   if (tid == 0) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(full + s, 1); mbar_init(empty + s, NCW); }
+    mbar_init(bfull, 1);
     asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
   }
   __syncthreads();
@@ -314,6 +335,27 @@ gemm_f64_dmma_ws(const __grid_constant__ GemmArgs p) {
     const bool isB = lane >= 16;
     const int srow = isB ? row * LDB_S : row * LDA_S;
     int it = 0;                                   // k-tiles issued so far by this CTA (ring position)
+    if (RESB && w_begin < w_end) {                // the whole B operand, once (N fits one tile: n0 = 0)
+      int wBr = p.N < BN ? p.N : BN; wBr = (wBr + 1) & ~1;
+      if (p.tma) {
+        if (lane == 0) {
+          mbar_expect_tx(bfull, (uint32_t)(nkt_total * BK * LDB_S) * 8u);
+          for (int kt = 0; kt < nkt_total; ++kt) tma_load_2d(Bs + kt * B_STAGE, &p.tmB, 0, kt * BK, bfull);
+        }
+      } else {
+        const int kz = (p.K + 3) & ~3;            // rows that complete the last k-step are zero-filled
+        for (int kr = p.K + lane; kr < kz; kr += 32) {
+          double* z = Bs + (kr / BK) * B_STAGE + (kr % BK) * LDB_S;
+          for (int c = 0; c < BN; ++c) z[c] = 0.0;
+        }
+        __syncwarp();
+        if (lane == 0) mbar_expect_tx(bfull, (uint32_t)p.K * (uint32_t)wBr * 8u);
+        __syncwarp();
+        for (int kr = lane; kr < p.K; kr += 32)
+          bulk_g2s(Bs + (kr / BK) * B_STAGE + (kr % BK) * LDB_S, p.B + (long long)kr * p.ldb, (uint32_t)wBr * 8u, bfull);
+      }
+      __syncwarp();
+    }
     for (long long w = w_begin; w < w_end;) {
       int z, rem, kt_begin, kt_end;
       if (SK) {
@@ -337,9 +379,9 @@ gemm_f64_dmma_ws(const __grid_constant__ GemmArgs p) {
           const int stage = it % STAGES, round = it / STAGES;
           if (round > 0) mbar_wait(empty + stage, (round - 1) & 1);
           if (lane == 0) {
-            mbar_expect_tx(full + stage, (uint32_t)(BK * (LDA_S + LDB_S)) * 8u);
+            mbar_expect_tx(full + stage, (uint32_t)(BK * (RESB ? LDA_S : LDA_S + LDB_S)) * 8u);
             tma_load_2d(As + stage * A_STAGE, &p.tmA, m0, kt * BK, full + stage);
-            tma_load_2d(Bs + stage * B_STAGE, &p.tmB, n0, kt * BK, full + stage);
+            if (!RESB) tma_load_2d(Bs + stage * B_STAGE, &p.tmB, n0, kt * BK, full + stage);
           }
           __syncwarp();
         }
@@ -351,15 +393,16 @@ gemm_f64_dmma_ws(const __grid_constant__ GemmArgs p) {
         const int kr = kt * BK + row;                                 // logical k-row of this lane
         int krows = p.K - kt * BK; if (krows > BK) krows = BK;
         const double* src = isB ? p.B + (long long)kr * p.ldb + n0 : Abase + p.ka(kr) * p.lda + m0;
-        double* dst = (isB ? Bs + stage * B_STAGE : As + stage * A_STAGE) + srow;
-        if (row >= krows && row < ((krows + 3) & ~3)) {   // ragged K: zero the rows that complete the last k-step
+        double* dst = (isB ? Bs + (RESB ? 0 : stage) * B_STAGE : As + stage * A_STAGE) + srow;
+        const bool mine = !(RESB && isB);                 // RESB: the B lanes have nothing to fetch per stage
+        if (mine && row >= krows && row < ((krows + 3) & ~3)) {   // ragged K: zero the rows that complete the last k-step
           const int wz = isB ? BN : BM;                   // (the consumers stop after ceil(krows / 4) k-steps)
           for (int c = 0; c < wz; ++c) dst[c] = 0.0;
         }
         __syncwarp();
-        if (lane == 0) mbar_expect_tx(full + stage, (uint32_t)krows * (uint32_t)(wA + wB) * 8u);
+        if (lane == 0) mbar_expect_tx(full + stage, (uint32_t)krows * (uint32_t)(RESB ? wA : wA + wB) * 8u);
         __syncwarp();
-        if (row < krows) bulk_g2s(dst, src, bytes, full + stage);
+        if (mine && row < krows) bulk_g2s(dst, src, bytes, full + stage);
       }
     }
     return;
@@ -369,6 +412,7 @@ gemm_f64_dmma_ws(const __grid_constant__ GemmArgs p) {
   const int wm0 = (warp / NW_N) * WM, wn0 = (warp % NW_N) * WN;
   const int lr = lane >> 2, lc = lane & 3;
   int it = 0;
+  if (RESB && w_begin < w_end) mbar_wait(bfull, 0);
   for (long long w = w_begin; w < w_end;) {
     int z, rem, kt_begin, kt_end;
     bool partial = false;
@@ -391,7 +435,7 @@ gemm_f64_dmma_ws(const __grid_constant__ GemmArgs p) {
     // The output offsets of the tile's BM rows and BN columns (-1 = out of range) are worked out once per tile by
     // all consumer threads together, while the first operand tiles are still in flight, instead of up to 16
     // index-map evaluations (32 integer divisions) per thread after the main loop.
-    long long* otab = reinterpret_cast<long long*>(empty + STAGES) + NCW * 8 * (WN + 4);   // behind the staging slabs
+    long long* otab = reinterpret_cast<long long*>(slabs + NCW * 8 * (WN + 4));            // behind the staging slabs
     if (!(SK && partial)) {
       asm volatile("bar.sync 1, %0;\n" ::"n"(NCW * 32) : "memory");       // previous tile's epilogue has read the table
       for (int t = tid; t < BM + BN; t += NCW * 32) {
@@ -410,7 +454,7 @@ gemm_f64_dmma_ws(const __grid_constant__ GemmArgs p) {
       const int stage = it % STAGES, round = it / STAGES;
       mbar_wait(full + stage, round & 1);
       const double* as = As + stage * A_STAGE + wm0 + lr + lc * LDA_S;
-      const double* bs = Bs + stage * B_STAGE + wn0 + lr + lc * LDB_S;
+      const double* bs = Bs + (RESB ? kt : stage) * B_STAGE + wn0 + lr + lc * LDB_S;
       const int krows = p.K - kt * BK;
       if (krows >= BK) {
 #pragma unroll
@@ -452,11 +496,51 @@ gemm_f64_dmma_ws(const __grid_constant__ GemmArgs p) {
 #pragma unroll
         for (int j = 0; j < FN; ++j)
           *reinterpret_cast<double2*>(slab + i * 8 * BN + j * 8) = make_double2(acc[i][j][0], acc[i][j][1]);
+    } else if (p.epi == 2) {
+      // dense blocks: slab layout [group][8 rows][wc]; lane g stores group g's block (split where the rows of the
+      // block are not consecutive in the output: a row-map boundary, or the ragged end of M)
+      const int wc = p.dense_wc, magic = p.dense_magic;
+      double* stg = slabs + warp * (8 * (WN + 4));
+      const int ng = (p.N - wn0 < WN ? p.N - wn0 : WN) / wc;          // column groups of this warp
+      asm volatile("bar.sync 1, %0;\n" ::"n"(NCW * 32) : "memory");       // offset table complete
+#pragma unroll
+      for (int i = 0; i < FM; ++i) {
+        if (lane < ng) bulk_wait_read0();                               // the slab's previous block has been read
+        __syncwarp();
+#pragma unroll
+        for (int j = 0; j < FN; ++j) {
+#pragma unroll
+          for (int e = 0; e < 2; ++e) {
+            const int c = j * 8 + 2 * lc + e;
+            const int g = (c * magic) >> 16;
+            if (g < ng) stg[(g * 8 + lr) * wc + (c - g * wc)] = acc[i][j][e];
+          }
+        }
+        fence_async_smem();
+        __syncwarp();
+        if (lane < ng) {
+          const long long cgo = otab[BM + wn0 + lane * wc];
+          const long long* rt = otab + wm0 + i * 8;
+          const double* src = stg + lane * 8 * wc;
+          int rr = 0;
+          while (rr < 8) {
+            const long long o0 = rt[rr];
+            if (o0 < 0) break;                                          // rows beyond M sit at the end of the tile
+            int len = 1;
+            while (rr + len < 8 && rt[rr + len] == o0 + (long long)len * wc) ++len;
+            bulk_s2g(out + o0 + cgo, src + rr * wc, (uint32_t)(len * wc) * 8u);
+            rr += len;
+          }
+          bulk_commit();
+        }
+      }
+      if (lane < ng) bulk_wait_read0();
+      __syncwarp();
     } else if (p.epi == 1) {
       // staged: 8 rows x WN columns of this warp go through its private shared-memory slab, then every
       // store instruction writes 32 consecutive columns of one row (coalesced wherever co() is contiguous)
       constexpr int SP = WN + 4, NCH = (WN + 31) / 32;
-      double* stg = reinterpret_cast<double*>(empty + STAGES) + warp * (8 * SP);
+      double* stg = slabs + warp * (8 * SP);
       asm volatile("bar.sync 1, %0;\n" ::"n"(NCW * 32) : "memory");       // offset table complete
       long long coffL[NCH];
 #pragma unroll
@@ -527,6 +611,7 @@ gemm_f64_dmma_ws(const __grid_constant__ GemmArgs p) {
       }
     }
   }
+  if (p.epi == 2) bulk_wait0();                   // every bulk store of this thread has completed
 }
 
 // Plain DFMA reference kernel (QRCTM_OPT_GEMM_PATH = 1): one output element per

@@ -53,7 +53,7 @@ struct StreamK { double* ws; size_t ws_elems; bool used; bool hybrid; };
 template <int BM, int BN, int WM, int WN, int STAGES>
 cudaError_t launch_cfg_ws(cudaStream_t st, const GemmArgs& g, int splits, StreamK* sk = nullptr) {
   constexpr int NT = ((BM / WM) * (BN / WN) + 1) * 32;
-  constexpr size_t smem = sizeof(double) * STAGES * BK * ((BM + PAD) + (BN + PAD)) + 2 * STAGES * sizeof(uint64_t) +
+  constexpr size_t smem = sizeof(double) * STAGES * BK * ((BM + PAD) + (BN + PAD)) + (2 * STAGES + 2) * sizeof(uint64_t) +
                           sizeof(double) * (BM / WM) * (BN / WN) * 8 * (WN + 4) +     // + per-warp epilogue slabs
                           sizeof(long long) * (BM + BN);                               // + output-offset table
   static bool attr_done = false;
@@ -110,6 +110,46 @@ cudaError_t launch_cfg_ws(cudaStream_t st, const GemmArgs& g, int splits, Stream
   return cudaGetLastError();
 }
 
+// Resident-B persistent launch (kernel: RESB = true): N <= BN, K short enough for all of B to sit in shared memory.
+// Returns cudaErrorInvalidValue when the shape does not qualify (the caller then takes the ordinary launch).
+template <int BM, int BN, int WM, int WN, int STAGES>
+cudaError_t launch_cfg_ws_resb(cudaStream_t st, const GemmArgs& g, int nz) {
+  constexpr int NT = ((BM / WM) * (BN / WN) + 1) * 32;
+  const int nkt = (g.K + BK - 1) / BK;
+  if (g.N > BN || nkt > 8) return cudaErrorInvalidValue;
+  const size_t smem = sizeof(double) * BK * (STAGES * (BM + PAD) + (size_t)nkt * (BN + PAD)) + (2 * STAGES + 2) * sizeof(uint64_t) +
+                      sizeof(double) * (BM / WM) * (BN / WN) * 8 * (WN + 4) + sizeof(long long) * (BM + BN);
+  auto kern = gemm_f64_dmma_ws<BM, BN, WM, WN, STAGES, false, true>;
+  static bool attr_done = false;
+  static size_t max_smem = 0;
+  if (!attr_done) {
+    int dev = 0, optin = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, optin);
+    if (e != cudaSuccess) return e;
+    max_smem = (size_t)optin;
+    attr_done = true;
+  }
+  if (smem > max_smem) return cudaErrorInvalidValue;
+  static int nsm = 0;
+  if (!nsm) { int dev = 0; cudaGetDevice(&dev); cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev); }
+  int per = 1;
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per, kern, NT, smem);
+  if (per < 1) return cudaErrorInvalidValue;
+  GemmArgs ga = g;
+  ga.nz = nz;
+  ga.tma = 0;
+  if (!g.batch && g.ka.div == 1 && g.ka.hi == 1 && g.ka.lo == 0)
+    ga.tma = encode_operand_map(&ga.tmA, g.A, g.lda, g.M, g.K, BM + PAD) &&
+             encode_operand_map(&ga.tmB, g.B, g.ldb, g.N, g.K, BN + PAD) ? 1 : 0;
+  const long long nwork = (long long)((g.M + BM - 1) / BM) * nz;
+  const long long slots = (long long)nsm * per;
+  const unsigned grid = (unsigned)(nwork < slots ? nwork : slots);
+  kern<<<grid, NT, smem, st>>>(ga);
+  return cudaGetLastError();
+}
+
 struct GemmCall {
   const double* A; long long lda; int transA;
   const double* B; long long ldb;
@@ -121,6 +161,7 @@ struct GemmCall {
   IndexMap za = IndexMap{1, 0, 0};
   long long zo = 0;
   int epi = 0;                         // 1: shared-memory staged epilogue (outputs contiguous along the column index)
+  int resb = 0;                        // 1: short K, N within one tile: prefer the resident-B persistent kernel
 };
 
 // Returns number of kernels launched (>0) or -1 on error (err set).
@@ -132,6 +173,18 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
   g.A = c.A; g.lda = c.lda; g.transA = c.transA; g.B = c.B; g.ldb = c.ldb; g.out = c.out;
   g.ro = c.ro; g.co = c.co; g.M = c.M; g.N = c.N; g.K = c.K; g.mode = c.mode;
   g.ka = c.ka; g.batch = c.batch > 0 ? 1 : 0; g.za = c.za; g.zo = c.zo; g.epi = c.epi;
+  if (c.epi == 2) {
+    // dense-block epilogue: columns in groups of wc with unit stride inside a group, rows with stride wc inside a row
+    // group; every piece a bulk store may start at or cover must be 16-byte aligned: even strides, even M, even row groups
+    const bool c3 = c.co.div0 > 1;
+    const int wc = c3 ? c.co.div0 : c.co.div;
+    const long long cin = c3 ? c.co.lo0 : c.co.lo, rin = c.ro.div0 > 1 ? -1 : c.ro.lo;
+    const bool ok = c.mode == 0 && wc >= 1 && wc < 128 && c.N % wc == 0 && cin == 1 && rin == wc && c.M % 2 == 0 &&
+                    c.ro.div % 2 == 0 && c.ro.hi % 2 == 0 && c.co.hi % 2 == 0 && (!c3 || c.co.lo % 2 == 0) && c.zo % 2 == 0 &&
+                    (reinterpret_cast<uintptr_t>(c.out) & 15) == 0;
+    if (ok) { g.dense_wc = wc; g.dense_magic = (65536 + wc - 1) / wc; }
+    else g.epi = 1;
+  }
   g.vecA = c.transA && (c.lda % 2 == 0) && ((reinterpret_cast<uintptr_t>(c.A) & 15) == 0);
   g.vecB = (c.ldb % 2 == 0) && ((reinterpret_cast<uintptr_t>(c.B) & 15) == 0);
   g.split_stride = 0;
@@ -156,12 +209,24 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
     // batched launch (layered absorption): bulk-copy kernel only, one batch per gridDim.z, no split-K
     if (!ws_ok) { *err = cudaErrorInvalidValue; return -1; }
     const int pad128 = (c.N + 127) / 128 * 128, pad104 = (c.N + 103) / 104 * 104, pad64 = (c.N + 63) / 64 * 64;
+    if (c.resb && c.N > 64 && c.N <= 104) {
+      *err = launch_cfg_ws_resb<64, 104, 16, 104, 3>(st, g, c.batch);
+      if (*err == cudaSuccess) return 1;
+      if (*err != cudaErrorInvalidValue) return -1;
+      cudaGetLastError();
+    }
     if (c.N <= 56) *err = launch_cfg_ws<128, 56, 32, 56, 3>(st, g, c.batch);
     else if (pad64 <= pad104 && pad64 <= pad128) *err = launch_cfg_ws<128, 64, 64, 32, 4>(st, g, c.batch);
     else if (pad104 <= pad128 && nkt <= 6) *err = launch_cfg_ws<64, 104, 16, 104, 3>(st, g, c.batch);   // 2 CTAs/SM
     else if (pad104 <= pad128) *err = launch_cfg_ws<128, 104, 16, 104, 4>(st, g, c.batch);
     else *err = launch_cfg_ws<128, 128, 64, 32, 4>(st, g, c.batch);
     return *err == cudaSuccess ? 1 : -1;
+  }
+  if (ws_big && c.resb && c.N <= 56) {
+    *err = launch_cfg_ws_resb<128, 56, 32, 56, 2>(st, g, 1);
+    if (*err == cudaSuccess) return 1;
+    if (*err != cudaErrorInvalidValue) return -1;
+    cudaGetLastError();
   }
   if (ws_big) {
     // pick the N tile with the least padding, then split K so that the CTAs fill whole waves

@@ -493,7 +493,7 @@ int qrctm_set_option(qrctm_t* h, int key, int value) {
     case QRCTM_OPT_GEMM_PATH:   if (value != 0 && value != 1) break; h->gemm_path = value; return QRCTM_OK;
     case QRCTM_OPT_QR_PATH:     if (value < 0 || value > 4) break; h->qr_path = value; return QRCTM_OK;
     case QRCTM_OPT_OVERLAP_CHECK: if (value != 0 && value != 1) break; h->overlap = value; return QRCTM_OK;
-    case QRCTM_OPT_ABSORB_MODE: if (value != 0 && value != 1) break; h->absorb_mode = value; return QRCTM_OK;
+    case QRCTM_OPT_ABSORB_MODE: if (value < 0 || value > 2) break; h->absorb_mode = value; return QRCTM_OK;
     case QRCTM_OPT_USE_GRAPH:   if (value != 0 && value != 1) break; h->use_graph = value; return QRCTM_OK;
     case QRCTM_OPT_TIME_STAGES: if (value != 0 && value != 1) break; h->time_stages = value; return QRCTM_OK;
     case QRCTM_OPT_K8_PATH:     if (value != 0 && value != 1) break; h->k8_old = value; return QRCTM_OK;

@@ -85,6 +85,15 @@ int stage_absorb_a(qrctm* h, const double* P, double* S, int layout, const doubl
 //   S''[J,(d_k d_b),m,(r_k r_b)] = sum_{s,u_b,l_b} P1[(s,u_b,l_b)][J,d_k,m,r_k] A[s,u_b,l_b,d_b,r_b]  (K = d D^2)
 // 4 d chi^2 D^6 flops instead of 2 chi^2 D^8.  Needs even chi (16-byte aligned rows for the bulk copies).
 bool layered_ok(const qrctm* h) { return h->chi % 2 == 0; }
+// absorb mode 2 (automatic): the layered contraction does 4 d D^6 flops per (J, m) pair against 2 D^8, but as two short-K
+// GEMMs (K = D^2 and d D^2) that reach ~55 % of the DMMA rate at D = 7 and far less below (K = 25 at D = 5 is two
+// k-tiles); measured on a B200 it wins from D = 6 up (K4 at D = 5, chi = 100: 0.48 against 0.29 ms; D = 6, chi = 100: 1.1
+// against 1.8 ms; D = 7, chi = 196: 1.8 against 12.7 ms), so that is the rule, with a 2x flop margin on d
+bool use_layered(const qrctm* h) {
+  if (!layered_ok(h)) return false;
+  if (h->absorb_mode == 1) return true;
+  return h->absorb_mode == 2 && h->D >= 6 && 4 * h->d <= h->b;
+}
 
 int stage_absorb_layered(qrctm* h, const double* P, double* S) {
   const int chi = h->chi, D = h->D, b = h->b, d = h->d;
@@ -97,11 +106,13 @@ int stage_absorb_layered(qrctm* h, const double* P, double* S) {
   g1.batch = b;
   g1.za = IndexMap{D, (long long)b * cc, cc};
   g1.zo = M2;
-  g1.epi = 1;
+  g1.epi = 2;
+  g1.resb = 1;
   GEMM(h, g1);
   GemmCall g2{h->P1, M2, 1, h->B2, h->L.ld2, S, IndexMap{chi * D, (long long)D * m, D}, IndexMap{D, m, 1},
               (int)M2, b, d * b, 0};
-  g2.epi = 1;
+  g2.epi = 2;
+  g2.resb = 1;
   GEMM(h, g2);
   return QRCTM_OK;
 }
@@ -239,7 +250,7 @@ int do_step(qrctm* h, cudaEvent_t* ev /* QRCTM_NSTAGE+1 events or null */, bool 
   if (!rc) { mark(2, "K3_half_absorb"); rc = stage_half_absorb(h, h->Q, h->T, h->P); }
   if (!rc) {
     mark(3, "K4_absorb_a");
-    rc = (h->absorb_mode == 1 && layered_ok(h)) ? stage_absorb_layered(h, h->P, h->S) : stage_absorb_a(h, h->P, h->S, 0);
+    rc = use_layered(h) ? stage_absorb_layered(h, h->P, h->S) : stage_absorb_a(h, h->P, h->S, 0);
   }
   if (!rc) { mark(4, "K5_project"); rc = stage_project(h, h->S, h->Q, h->Tn); }
   if (!rc) { mark(5, "K6_corner"); rc = h->corner_mode == 0 ? stage_corner_accel(h) : stage_corner_enlarged(h); }

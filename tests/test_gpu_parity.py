@@ -524,6 +524,18 @@ def test_layered_absorption_matches_oracle_and_explicit(d, D, chi, seed, path):
     assert rel(lay["raw"][1], exp["raw"][1]) < 1e-12
 
 
+def test_absorb_mode_auto_selects_by_bond_dimension():
+    """QRCTM_OPT_ABSORB_MODE = 2: layered from D = 6 up, explicit below -- bitwise the respective fixed mode."""
+    for (d, D, chi, seed) in ((2, 6, 12, 3), (2, 4, 16, 2)):
+        outs = {}
+        for mode in (0, 1, 2):
+            o_, _, _ = _one_step(d, D, chi, seed, absorb=mode)
+            outs[mode] = o_
+        same = 1 if D >= 6 else 0
+        assert np.array_equal(outs[2]["T"], outs[same]["T"]) and np.array_equal(outs[2]["C"], outs[same]["C"])
+        assert rel(outs[2]["T"], outs[1 - same]["T"]) < 1e-12
+
+
 def test_large_chi_fallback_paths():
     """chi = 300 > 236: the corner spectrum takes the global-memory tridiagonalisation path; D = 1 keeps it cheap.
     Also a square c~ (m = chi) for the QR (19 panels, the last one ragged)."""
