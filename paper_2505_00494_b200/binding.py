@@ -19,7 +19,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("QRCTM_LIB", os.path.join(_HERE, "libqrctm.so"))
 
 QRCTM_OK = 0
-OPT_CORNER_MODE, OPT_SYMMETRIZE, OPT_CHECK_EVERY, OPT_GEMM_PATH, OPT_TIME_STAGES, OPT_QR_PATH, OPT_OVERLAP_CHECK, OPT_USE_GRAPH, OPT_ABSORB_MODE, OPT_K8_PATH = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10
+OPT_CORNER_MODE, OPT_SYMMETRIZE, OPT_CHECK_EVERY, OPT_GEMM_PATH, OPT_TIME_STAGES, OPT_QR_PATH, OPT_OVERLAP_CHECK, OPT_USE_GRAPH, OPT_ABSORB_MODE, OPT_K8_PATH, OPT_SMALL_PATH = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11
 NSTAGE = 7
 STAGE_NAMES = ("K1_reduced_corner", "K2_qr", "K3_half_absorb", "K4_absorb_a", "K5_project",
                "K6_corner", "K7_normalize")

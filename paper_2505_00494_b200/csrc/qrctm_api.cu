@@ -14,6 +14,7 @@
 #include "kernels_misc.cuh"
 #include "qr_f64.cuh"
 #include "cholqr.cuh"
+#include "small_step.cuh"
 #include "spectrum.cuh"
 #include "eigh.cuh"
 
@@ -54,6 +55,8 @@ struct qrctm {
   bool have_A, have_env;
   int corner_mode, symmetrize, check_every, gemm_path, time_stages, qr_path, absorb_mode;
   int k8_old;             // 1: K8 on the round-1 tridiagonalisation kernel (QRCTM_OPT_K8_PATH, for cross-checks)
+  int small_off;          // 1: never use the whole-iteration kernels for tiny problems (QRCTM_OPT_SMALL_PATH)
+  int small_smem;         // opt-in shared memory available to them (0: not queried yet, -1: unavailable)
   long long launches;
   cudaEvent_t ev[QRCTM_NSTAGE + 2];
   bool have_ev;
@@ -497,6 +500,7 @@ int qrctm_set_option(qrctm_t* h, int key, int value) {
     case QRCTM_OPT_USE_GRAPH:   if (value != 0 && value != 1) break; h->use_graph = value; return QRCTM_OK;
     case QRCTM_OPT_TIME_STAGES: if (value != 0 && value != 1) break; h->time_stages = value; return QRCTM_OK;
     case QRCTM_OPT_K8_PATH:     if (value != 0 && value != 1) break; h->k8_old = value; return QRCTM_OK;
+    case QRCTM_OPT_SMALL_PATH:  if (value != 0 && value != 1) break; h->small_off = value; return QRCTM_OK;
     default: break;
   }
   return fail(h, QRCTM_ERR_INVALID_ARG, "bad option key/value");

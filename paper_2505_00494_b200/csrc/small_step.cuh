@@ -1,0 +1,192 @@
+// Whole-iteration kernels for tiny problems: when C, T, c~, Q, a and both m x m
+// intermediates fit in ONE CTA's shared memory (cfg0: d = 2, D = 2, chi = 8, m = 32), K1..K6 run as one launch
+// (small_front_kernel) and K7 as one more (small_k7_kernel) instead of ~18 launches of a few microseconds each.
+// Plain DFMA loops over shared memory -- at these sizes the step is launch-latency-bound, not a tensor-core problem.
+// Same equations and the same Householder QR (dlarfg convention, then diag(R) >= 0) as the large path:
+//   (E1) X[(j,u),k] = sum_i C[j,i] T[i,u,k]
+//   (E2) X = Q R
+//   (E3) P[(u,l),(J,m)] = sum_j Q[(j,u),m] T[j,l,J];  S[(J,d),(m,r)] = sum_(u,l) P[(u,l),(J,m)] a[(u,l),(d,r)];
+//        T'[(m,r),n] = sum_(J,d) S[(J,d),(m,r)] Q[(J,d),n]
+//   (E4) W[(m,r),n] = sum_k R[m,k] Q[(k,r),n];  C'[p,n] = sum_(m,r) T'[(m,r),p] W[(m,r),n]
+// Deterministic (fixed summation orders).
+#pragma once
+#include "kernels_misc.cuh"
+
+namespace qk {
+
+constexpr int SMALL_NT = 512;
+
+__host__ __device__ inline size_t small_front_doubles(int b, int chi) {
+  const size_t m = (size_t)b * chi, b2 = (size_t)b * b;
+  return (size_t)chi * chi * 2 + m * chi * 5 + b2 * b2 + 2 * m * m + 2 * chi + 64;
+}
+
+// Inputs (global): C[chi][chi], T[chi][b][chi], a_mat[b*b][lda].  Outputs (global): X, Q (m x chi), R (chi x chi),
+// Tn (m x chi), Cn (chi x chi) -- the un-normalised C', T' that K7 consumes.
+__global__ void __launch_bounds__(SMALL_NT, 1)
+small_front_kernel(const double* __restrict__ Cg, const double* __restrict__ Tg, const double* __restrict__ ag,
+                   long long lda, int b, int chi, double* __restrict__ Xg, double* __restrict__ Qg,
+                   double* __restrict__ Rg, double* __restrict__ Tng, double* __restrict__ Cng) {
+  extern __shared__ __align__(16) double ssm[];
+  const int m = b * chi, b2 = b * b, mc = m * chi, cc = chi * chi;
+  double* C = ssm;                 // chi^2
+  double* R = C + cc;              // chi^2
+  double* T = R + cc;              // m chi    T[i][u][k]
+  double* X = T + mc;              // m chi    c~, then the reflectors V (below the diagonal) and R (upper)
+  double* Q = X + mc;              // m chi
+  double* Tn = Q + mc;             // m chi
+  double* W = Tn + mc;             // m chi
+  double* a = W + mc;              // b^4      a[(u,l)][(d,r)]
+  double* P = a + (size_t)b2 * b2; // m^2      P[(u,l)][(J,m)]
+  double* S = P + (size_t)m * m;   // m^2      S[(J,d)][(m,r)]
+  double* tau = S + (size_t)m * m; // chi
+  double* wv = tau + chi;          // chi + 64 scratch
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  constexpr int NW = SMALL_NT / 32;
+
+  for (int i = tid; i < cc; i += SMALL_NT) C[i] = Cg[i];
+  for (int i = tid; i < mc; i += SMALL_NT) T[i] = Tg[i];
+  for (int i = tid; i < b2 * b2; i += SMALL_NT) a[i] = ag[(long long)(i / b2) * lda + i % b2];
+  __syncthreads();
+  // (E1) X[(j,u),k]: row (j,u) = j*b+u; T as chi x (b chi) row-major: T[i][(u,k)]
+  for (int o = tid; o < mc; o += SMALL_NT) {
+    const int j = o / (b * chi), uk = o % (b * chi);
+    double s = 0.0;
+    for (int i = 0; i < chi; ++i) s = fma(C[j * chi + i], T[i * b * chi + uk], s);
+    X[o] = s;                                            // o = (j*b+u)*chi + k
+  }
+  __syncthreads();
+  for (int i = tid; i < mc; i += SMALL_NT) Xg[i] = X[i];
+  // (E2) Householder QR, column by column: warp 0 forms the reflector, then one warp per remaining column applies it
+  for (int k = 0; k < chi; ++k) {
+    if (warp == 0) {
+      double acc = 0.0;
+      for (int i = k + 1 + lane; i < m; i += 32) { const double x = X[i * chi + k]; acc = fma(x, x, acc); }
+      const double tail2 = warp_sum(acc);
+      const double alpha = X[k * chi + k];
+      double t = 0.0, scale = 0.0, beta = alpha;
+      if (tail2 > 0.0) {
+        const double sigma = sqrt(fma(alpha, alpha, tail2));
+        beta = alpha >= 0.0 ? -sigma : sigma;
+        t = (beta - alpha) / beta;
+        scale = 1.0 / (alpha - beta);
+      }
+      __syncwarp();
+      for (int i = k + 1 + lane; i < m; i += 32) X[i * chi + k] *= scale;
+      if (lane == 0) { X[k * chi + k] = beta; tau[k] = t; }
+    }
+    __syncthreads();
+    const double t = tau[k];
+    if (t != 0.0) {
+      for (int j = k + 1 + warp; j < chi; j += NW) {
+        double acc = 0.0;
+        for (int i = k + lane; i < m; i += 32) acc = fma(i == k ? 1.0 : X[i * chi + k], X[i * chi + j], acc);
+        const double w = t * warp_sum(acc);
+        for (int i = k + lane; i < m; i += 32) X[i * chi + j] = fma(-(i == k ? 1.0 : X[i * chi + k]), w, X[i * chi + j]);
+      }
+    }
+    __syncthreads();
+  }
+  for (int o = tid; o < cc; o += SMALL_NT) R[o] = (o % chi >= o / chi) ? X[o] : 0.0;      // X's top chi rows
+  for (int o = tid; o < mc; o += SMALL_NT) Q[o] = (o / chi == o % chi) ? 1.0 : 0.0;
+  __syncthreads();
+  for (int k = chi - 1; k >= 0; --k) {                   // Q = H_0 ... H_{chi-1} [I; 0]
+    const double t = tau[k];
+    if (t != 0.0) {
+      for (int j = k + warp; j < chi; j += NW) {
+        double acc = 0.0;
+        for (int i = k + lane; i < m; i += 32) acc = fma(i == k ? 1.0 : X[i * chi + k], Q[i * chi + j], acc);
+        const double w = t * warp_sum(acc);
+        for (int i = k + lane; i < m; i += 32) Q[i * chi + j] = fma(-(i == k ? 1.0 : X[i * chi + k]), w, Q[i * chi + j]);
+      }
+    }
+    __syncthreads();
+  }
+  if (tid < chi) wv[tid] = R[tid * chi + tid] < 0.0 ? -1.0 : 1.0;                         // sign fix: diag(R) >= 0
+  __syncthreads();
+  for (int o = tid; o < mc; o += SMALL_NT) Q[o] *= wv[o % chi];
+  for (int o = tid; o < cc; o += SMALL_NT) R[o] *= wv[o / chi];
+  __syncthreads();
+  for (int o = tid; o < mc; o += SMALL_NT) Qg[o] = Q[o];
+  for (int o = tid; o < cc; o += SMALL_NT) Rg[o] = R[o];
+  // (E3a) P[(u,l),(J,mm)] = sum_j Q[(j,u),mm] T[j,l,J]
+  for (int o = tid; o < m * m; o += SMALL_NT) {
+    const int ul = o / cc, Jm = o % cc, u = ul / b, l = ul % b, J = Jm / chi, mm = Jm % chi;
+    double s = 0.0;
+    for (int j = 0; j < chi; ++j) s = fma(Q[(j * b + u) * chi + mm], T[(j * b + l) * chi + J], s);
+    P[o] = s;
+  }
+  __syncthreads();
+  // (E3b) S[(J,d),(mm,r)] = sum_(u,l) P[(u,l),(J,mm)] a[(u,l),(d,r)]
+  for (int o = tid; o < m * m; o += SMALL_NT) {
+    const int Jd = o / m, mr = o % m, J = Jd / b, d = Jd % b, mm = mr / b, r = mr % b;
+    double s = 0.0;
+    for (int ul = 0; ul < b2; ++ul) s = fma(P[ul * cc + J * chi + mm], a[ul * b2 + d * b + r], s);
+    S[o] = s;
+  }
+  __syncthreads();
+  // (E3c) T'[(mm,r),n] = sum_(J,d) S[(J,d),(mm,r)] Q[(J,d),n];   (E4a) W[(mm,r),n] = sum_k R[mm,k] Q[(k,r),n]
+  for (int o = tid; o < mc; o += SMALL_NT) {
+    const int mr = o / chi, n = o % chi, mm = mr / b, r = mr % b;
+    double s = 0.0;
+    for (int Jd = 0; Jd < m; ++Jd) s = fma(S[Jd * m + mr], Q[Jd * chi + n], s);
+    Tn[o] = s;
+    double w = 0.0;
+    for (int k = mm; k < chi; ++k) w = fma(R[mm * chi + k], Q[(k * b + r) * chi + n], w);    // R upper triangular
+    W[o] = w;
+  }
+  __syncthreads();
+  for (int o = tid; o < mc; o += SMALL_NT) Tng[o] = Tn[o];
+  // (E4b) C'[p,n] = sum_(mm,r) T'[(mm,r),p] W[(mm,r),n]
+  for (int o = tid; o < cc; o += SMALL_NT) {
+    const int p = o / chi, n = o % chi;
+    double s = 0.0;
+    for (int mr = 0; mr < m; ++mr) s = fma(Tn[mr * chi + p], W[mr * chi + n], s);
+    Cng[o] = s;
+  }
+}
+
+// K7 in one CTA: C, T <- sym(C', T') / ||.||_F, the NaN / zero-norm flag, the norms and (hist != null) the history record.
+__global__ void __launch_bounds__(SMALL_NT, 1)
+small_k7_kernel(const double* __restrict__ Cn, const double* __restrict__ Tn, int chi, int b, int symmetrize,
+                double* __restrict__ C, double* __restrict__ T, double* __restrict__ scal, int* __restrict__ flag,
+                double* __restrict__ hist, int* __restrict__ hist_n, const double* __restrict__ R) {
+  __shared__ double sh[33];
+  const int tid = threadIdx.x;
+  const int cc = chi * chi, bc = b * chi, mc = bc * chi;
+  double ac = 0.0, at = 0.0;
+  for (int o = tid; o < cc; o += SMALL_NT) {
+    double v = Cn[o];
+    if (symmetrize) v = 0.5 * (v + Cn[(o % chi) * chi + o / chi]);
+    C[o] = v; ac = fma(v, v, ac);
+  }
+  for (int o = tid; o < mc; o += SMALL_NT) {
+    const int i = o / bc, s = (o / chi) % b, k = o % chi;
+    double v = Tn[o];
+    if (symmetrize) v = 0.5 * (v + Tn[k * bc + s * chi + i]);
+    T[o] = v; at = fma(v, v, at);
+  }
+  const double nc = sqrt(block_sum(ac, sh)), nt = sqrt(block_sum(at, sh));
+  double ratio = 0.0;
+  if (hist) {
+    double mn = INFINITY, mx = -INFINITY;
+    for (int k = tid; k < chi; k += SMALL_NT) { const double v = R[k * chi + k]; mn = fmin(mn, v); mx = fmax(mx, v); }
+    const double gmx = block_max(mx, sh), gmn = -block_max(-mn, sh);
+    ratio = gmx != 0.0 ? gmn / gmx : 0.0;
+  }
+  __syncthreads();                                       // every thread's own C, T elements are written; same thread rescales them
+  for (int o = tid; o < cc; o += SMALL_NT) C[o] = C[o] / nc;
+  for (int o = tid; o < mc; o += SMALL_NT) T[o] = T[o] / nt;
+  if (tid == 0) {
+    scal[0] = nc; scal[1] = nt;
+    if (!(nc > 0.0) || !(nt > 0.0) || isinf(nc) || isinf(nt)) *flag = 1;
+    if (hist) {
+      const int idx = *hist_n;
+      double* rec = hist + (size_t)(idx % QRCTM_HIST_CAP) * 4;
+      rec[0] = __longlong_as_double(0x7ff8000000000000LL); rec[1] = nc; rec[2] = nt; rec[3] = ratio;
+      *hist_n = idx + 1;
+    }
+  }
+}
+
+}  // namespace qk

@@ -7,6 +7,7 @@
 // rank sort.  Bisection gives each eigenvalue to ~2 ulp of ||C|| = 1, which is
 // what the convergence test (tol 1e-10..1e-12 absolute) needs.
 #pragma once
+#include <stdint.h>
 #include "kernels_misc.cuh"
 
 namespace qk {
@@ -273,10 +274,9 @@ __host__ __device__ inline size_t tri2_smem_bytes(int n) {
 //   U  rank-2 update of the lower triangle, warps dealt out to the column groups in proportion to the groups'
 //      heights (the first group's columns are n - k rows tall, the last one's a few); the owner of column k+1 also
 //      leaves it as the next u                                                                           -- barrier
-__global__ void __launch_bounds__(TRI2_NT, 1)
-tridiag_smem2_kernel(const double* __restrict__ Cmat, int n, double* __restrict__ dvec, double* __restrict__ evec,
-                     long long* __restrict__ prof /* null, or 8 cycle counters of the phases (thread 0) */) {
-  extern __shared__ __align__(16) double tsm[];
+__device__ __forceinline__ void
+tridiag_smem2_body(double* tsm, const double* __restrict__ Cmat, int n, double* dvec, double* evec,
+                   long long* __restrict__ prof /* null, or 8 cycle counters of the phases (thread 0) */) {
   double2* up0 = reinterpret_cast<double2*>(tsm);               // 2 x n pairs (u_i, p_i), double-buffered over the steps
   double* part = tsm + 4 * n;                                   // TRI2_MAXSUB x n partial sums of A u
   double* red = part + TRI2_MAXSUB * n;                         // 8: per-warp partial sums of p.u
@@ -488,6 +488,13 @@ tridiag_smem2_kernel(const double* __restrict__ Cmat, int n, double* __restrict_
 #undef TRI_TICK
 }
 
+__global__ void __launch_bounds__(TRI2_NT, 1)
+tridiag_smem2_kernel(const double* __restrict__ Cmat, int n, double* __restrict__ dvec, double* __restrict__ evec,
+                     long long* __restrict__ prof) {
+  extern __shared__ __align__(16) double tsm[];
+  tridiag_smem2_body(tsm, Cmat, n, dvec, evec, prof);
+}
+
 // Sturm count without divisions: number of eigenvalues < x of the tridiagonal whose SCALED entries (all magnitudes
 // <= ~2) are de[i] = (d_i, e_i^2), from the sign changes of the leading principal minors
 //   p_i = (d_i - x) p_{i-1} - e_i^2 p_{i-2}
@@ -543,27 +550,26 @@ __device__ __forceinline__ int sturm_count_minors(const double2* __restrict__ de
 // eigenvalue number idx = 8 B + w (ascending; see `ke` for the partial mode).  Each iteration the 32 lanes evaluate
 // the Sturm count at 32 interior points of [a, b], shrinking the bracket 33-fold
 // (about 11 iterations to the last ulp instead of ~55 bisection steps).
-__global__ void __launch_bounds__(256)
-multisect_kernel(const double* __restrict__ dvec, const double* __restrict__ evec, int n,
-                 double* __restrict__ eig_out, int ke = 0) {
-  extern __shared__ __align__(16) double msm[];               // de[n] = (d_i, e_i^2) scaled, red[33]
-  double2* de = reinterpret_cast<double2*>(msm); double* red = msm + 2 * n;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+// Block-wide set-up of the multisection: de[i] = (d_i, e_i^2) of the problem scaled by an exact power of two so that every
+// entry has magnitude <= 1 (the minors recurrence of sturm_count_minors then grows by at most ~2.5 per row), the
+// Gershgorin interval [glo, ghi] of the scaled problem, and the factor isc that scales eigenvalues back.
+__device__ __forceinline__ void multisect_setup(const double* dvec, const double* evec, int n, double2* de, double* red,
+                                                double& glo, double& ghi, double& isc) {
+  const int tid = threadIdx.x;
   double lo = INFINITY, hi = -INFINITY;
   for (int i = tid; i < n; i += blockDim.x) {                  // Gershgorin bounds
     const double el = i > 0 ? fabs(evec[i]) : 0.0, er = i + 1 < n ? fabs(evec[i + 1]) : 0.0, di = dvec[i];
     lo = fmin(lo, di - el - er);
     hi = fmax(hi, di + el + er);
   }
-  double ghi = block_max(hi, red);
-  double glo = -block_max(-lo, red);
+  ghi = block_max(hi, red);
+  glo = -block_max(-lo, red);
   const double bnd = fmax(fabs(glo), fabs(ghi));
-  // scale the problem by an exact power of two so that every entry has magnitude <= 1 (the minors recurrence of
-  // sturm_count_minors then grows by at most ~2.5 per row); eigenvalues are scaled back at the end
   int ex = 0;
   if (bnd > 0.0 && bnd < INFINITY) { frexp(bnd, &ex); }
   ex = ex > 1000 ? 1000 : (ex < -1000 ? -1000 : ex);
-  const double sc = ldexp(1.0, -ex), isc = ldexp(1.0, ex);
+  const double sc = ldexp(1.0, -ex);
+  isc = ldexp(1.0, ex);
   for (int i = tid; i < n; i += blockDim.x) {
     const double e = i > 0 ? evec[i] * sc : 0.0;
     de[i] = make_double2(dvec[i] * sc, e * e);
@@ -573,12 +579,11 @@ multisect_kernel(const double* __restrict__ dvec, const double* __restrict__ eve
   const double bs = fmax(fabs(glo), fabs(ghi));
   glo -= 2.0 * 2.220446049250313e-16 * bs * n + 0x1p-90;
   ghi += 2.0 * 2.220446049250313e-16 * bs * n + 0x1p-90;
-  // ke > 0 (and 2 ke < n): only the ke smallest and the ke largest eigenvalues, written compactly
-  // (slot c < ke: eigenvalue c; slot c >= ke: eigenvalue n - 2 ke + c) -- the eigen step's candidates.
-  const int slot = blockIdx.x * 8 + warp;
-  const bool part = ke > 0 && 2 * ke < n;
-  if (slot >= (part ? 2 * ke : n)) return;
-  const int idx = (part && slot >= ke) ? n - 2 * ke + slot : slot;
+}
+
+// One warp: eigenvalue number idx (ascending) of the scaled problem by 33-way multisection.
+__device__ __forceinline__ double multisect_warp(const double2* de, int n, int idx, double glo, double ghi) {
+  const int lane = threadIdx.x & 31;
   double a = glo, b = ghi;
   for (int it = 0; it < 64; ++it) {
     const double h = (b - a) / 33.0;
@@ -595,19 +600,34 @@ multisect_kernel(const double* __restrict__ dvec, const double* __restrict__ eve
     a = na; b = nb;
     if (!progress || !(b - a > 0.0)) break;
   }
-  if (lane == 0) eig_out[slot] = 0.5 * (a + b) * isc;
+  return 0.5 * (a + b);
+}
+
+__global__ void __launch_bounds__(256)
+multisect_kernel(const double* __restrict__ dvec, const double* __restrict__ evec, int n,
+                 double* __restrict__ eig_out, int ke = 0) {
+  extern __shared__ __align__(16) double msm[];               // de[n] = (d_i, e_i^2) scaled, red[33]
+  double2* de = reinterpret_cast<double2*>(msm); double* red = msm + 2 * n;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  double glo, ghi, isc;
+  multisect_setup(dvec, evec, n, de, red, glo, ghi, isc);
+  // ke > 0 (and 2 ke < n): only the ke smallest and the ke largest eigenvalues, written compactly
+  // (slot c < ke: eigenvalue c; slot c >= ke: eigenvalue n - 2 ke + c) -- the eigen step's candidates.
+  const int slot = blockIdx.x * 8 + warp;
+  const bool part = ke > 0 && 2 * ke < n;
+  if (slot >= (part ? 2 * ke : n)) return;
+  const int idx = (part && slot >= ke) ? n - 2 * ke + slot : slot;
+  const double lam = multisect_warp(de, n, idx, glo, ghi);
+  if (lane == 0) eig_out[slot] = lam * isc;
 }
 
 // One block, blockDim.x >= n: s = sorted |eig| (descending), delta vs s_prev.
-__global__ void spectrum_finalize_kernel(const double* __restrict__ eig, int n, double* __restrict__ s_out,
-                                         double* __restrict__ s_prev, double* __restrict__ delta_out,
-                                         int update_prev, double* __restrict__ hist = nullptr,
-                                         const int* __restrict__ hist_n = nullptr) {
-  extern __shared__ double fsm[];               // lam[n], red[33]
-  double* lam = fsm; double* red = fsm + n;
+// blockDim.x >= n.  lam[n] (shared): the eigenvalues; s = sorted |lam| (descending), delta vs s_prev.
+__device__ __forceinline__ void spectrum_finalize_body(const double* lam, double* red, int n, double* __restrict__ s_out,
+                                                       double* __restrict__ s_prev, double* __restrict__ delta_out,
+                                                       int update_prev, double* __restrict__ hist,
+                                                       const int* __restrict__ hist_n) {
   const int tid = threadIdx.x;
-  if (tid < n) lam[tid] = eig[tid];
-  __syncthreads();
   if (tid < n) {
     double mine = fabs(lam[tid]);
     int rank = 0;
@@ -627,6 +647,47 @@ __global__ void spectrum_finalize_kernel(const double* __restrict__ eig, int n, 
   }
   __syncthreads();
   if (update_prev && tid < n) s_prev[tid] = s_out[tid];
+}
+
+// One block, blockDim.x >= n: s = sorted |eig| (descending), delta vs s_prev.
+__global__ void spectrum_finalize_kernel(const double* __restrict__ eig, int n, double* __restrict__ s_out,
+                                         double* __restrict__ s_prev, double* __restrict__ delta_out,
+                                         int update_prev, double* __restrict__ hist = nullptr,
+                                         const int* __restrict__ hist_n = nullptr) {
+  extern __shared__ double fsm[];               // lam[n], red[33]
+  double* lam = fsm; double* red = fsm + n;
+  if (threadIdx.x < n) lam[threadIdx.x] = eig[threadIdx.x];
+  __syncthreads();
+  spectrum_finalize_body(lam, red, n, s_out, s_prev, delta_out, update_prev, hist, hist_n);
+}
+
+// K8 in ONE launch for small corners (n <= SPEC_FUSED_MAX_N): tridiagonalisation, multisection (32 warps, n / 32
+// rounds) and finalisation by the same CTA -- at these sizes the three launches cost more than the arithmetic.
+constexpr int SPEC_FUSED_MAX_N = 24;
+__host__ __device__ inline size_t spectrum_fused_smem_bytes(int n) { return tri2_smem_bytes(n) + sizeof(double) * (5 * (size_t)n + 40); }
+
+__global__ void __launch_bounds__(TRI2_NT, 1)
+spectrum_fused_kernel(const double* __restrict__ Cmat, int n, double* __restrict__ eig_out, double* __restrict__ s_out,
+                      double* __restrict__ s_prev, double* __restrict__ delta_out, int update_prev,
+                      double* __restrict__ hist, const int* __restrict__ hist_n) {
+  extern __shared__ __align__(16) double tsm[];
+  double* extra = tsm + tri2_smem_bytes(n) / sizeof(double);
+  double* dv = extra;                            // n
+  double* ev = dv + n;                           // n
+  double2* de = reinterpret_cast<double2*>((reinterpret_cast<uintptr_t>(ev + n) + 15) & ~static_cast<uintptr_t>(15));   // n pairs
+  double* lam = reinterpret_cast<double*>(de + n);              // n
+  double* red = lam + n;                         // 33
+  tridiag_smem2_body(tsm, Cmat, n, dv, ev, nullptr);
+  __syncthreads();
+  double glo, ghi, isc;
+  multisect_setup(dv, ev, n, de, red, glo, ghi, isc);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int idx = warp; idx < n; idx += TRI2_NT / 32) {
+    const double l = multisect_warp(de, n, idx, glo, ghi) * isc;
+    if (lane == 0) { lam[idx] = l; eig_out[idx] = l; }
+  }
+  __syncthreads();
+  spectrum_finalize_body(lam, red, n, s_out, s_prev, delta_out, update_prev, hist, hist_n);
 }
 
 }  // namespace qk

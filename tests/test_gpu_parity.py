@@ -524,6 +524,32 @@ def test_layered_absorption_matches_oracle_and_explicit(d, D, chi, seed, path):
     assert rel(lay["raw"][1], exp["raw"][1]) < 1e-12
 
 
+@pytest.mark.parametrize("d,D,chi,seed", [(2, 2, 8, 0), (3, 2, 5, 7), (2, 3, 7, 8), (2, 2, 20, 4), (2, 1, 3, 9)])
+def test_small_whole_iteration_kernels_match_the_general_path(d, D, chi, seed):
+    """Tiny problems run K1..K6 as one kernel, K7 as one and K8 as one (QRCTM_OPT_SMALL_PATH = 0, the default): same
+    step as the general multi-kernel path to rounding, same iteration count and delta history, far fewer launches."""
+    A, C0, T0 = gen_config(d, D, chi, seed)
+    out = {}
+    for off in (0, 1):
+        h = pkg.QRCTM(d, D, chi)
+        h.set_option(pkg.OPT_SMALL_PATH, off)
+        h.set_A(A); h.set_env(C0, T0)
+        h.step()
+        Q, R = h.get_qr()
+        raw = h.get_raw()
+        n0 = h.launch_count()
+        it, dl = h.run(12, -1.0)
+        out[off] = (Q, R, raw, h.get_env(), h.get_corner_spectrum(), dl, h.launch_count() - n0, h.get_history()[0])
+        h.close()
+    s, g = out[0], out[1]
+    cond = np.linalg.cond(g[1])
+    assert rel(s[0], g[0]) < 1e-14 * max(cond, 10) and rel(s[1], g[1]) < 1e-14 * max(cond, 10)
+    assert rel(s[2][0], g[2][0]) < 1e-12 and rel(s[2][1], g[2][1]) < 1e-12
+    assert rel(s[3][0], g[3][0]) < 1e-10 and rel(s[3][1], g[3][1]) < 1e-10
+    assert np.max(np.abs(s[4] - g[4])) < 1e-11 and abs(s[5] - g[5]) < 1e-10
+    assert np.allclose(s[7][:, 1:], g[7][:, 1:], rtol=1e-9) and s[6] * 3 < g[6]
+
+
 def test_absorb_mode_auto_selects_by_bond_dimension():
     """QRCTM_OPT_ABSORB_MODE = 2: layered from D = 6 up, explicit below -- bitwise the respective fixed mode."""
     for (d, D, chi, seed) in ((2, 6, 12, 3), (2, 4, 16, 2)):
