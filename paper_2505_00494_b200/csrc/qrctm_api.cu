@@ -358,6 +358,33 @@ int qrctm_run(qrctm_t* h, int max_iter, double tol, int* iters_done, double* fin
   if (!h->have_A || !h->have_env) return fail(h, QRCTM_ERR_NOT_READY, "set_A and set_env first");
   h->eig_rows = 0;          // Q is about to be overwritten by K2
   if (max_iter < 0) return fail(h, QRCTM_ERR_INVALID_ARG, "max_iter < 0");
+  if (max_iter > 0 && h->check_every >= 2 && !h->time_stages && !h->k8_old && h->chi <= SPEC_FUSED_MAX_N && small_ok(h)) {
+    // tiny problem, spectrum not wanted after every step: the whole loop in one launch, convergence decided on the
+    // device (small_step.cuh).  With CHECK_EVERY = 1 the pipelined driver below is faster: there K8 of step k runs on
+    // the side stream under step k+1, here the one CTA does them one after the other (measured at cfg0: 46 us per
+    // step against 51)
+    static bool attr = false;
+    if (!attr) {
+      CU(h, cudaFuncSetAttribute(small_run_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, h->small_smem - 2048));
+      attr = true;                                              // (2 KB: the kernel's static shared memory)
+    }
+    const size_t smem = small_run_smem_bytes(h->b, h->chi);
+    if (smem + 2048 <= (size_t)h->small_smem) {
+      small_run_kernel<<<1, SMALL_NT, smem, h->stream>>>(h->C, h->T, h->a_mat, h->L.lda_a, h->b, h->chi, h->symmetrize, h->X,
+                                                         h->Q, h->R, h->Tn, h->Cn, h->scal, h->flag, h->hist, h->flag + 1, h->eig,
+                                                         h->s, h->s_prev, h->delta, h->need_s0, max_iter, tol, h->check_every,
+                                                         h->scal + 10);
+      h->launches += 1;
+      h->need_s0 = 0;
+      CU(h, cudaGetLastError());
+      CU(h, cudaMemcpyAsync(h->h_pinned + 10, h->scal + 10, 2 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+      int rcf = check_flag(h); if (rcf) return rcf;             // synchronises
+      if (iters_done) *iters_done = (int)h->h_pinned[10];
+      if (final_delta) *final_delta = h->h_pinned[11];
+      h->warm_steps += 1;
+      return QRCTM_OK;
+    }
+  }
   if (h->overlap && h->side && !h->time_stages) {
     // Overlapped driver: K1..K6 of step it are queued before the host waits for the spectrum of
     // step it-1 (side stream); K7 of step it (the only stage that overwrites C, T) waits for it.

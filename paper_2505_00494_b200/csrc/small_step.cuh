@@ -11,10 +11,11 @@
 // Deterministic (fixed summation orders).
 #pragma once
 #include "kernels_misc.cuh"
+#include "spectrum.cuh"
 
 namespace qk {
 
-constexpr int SMALL_NT = 512;
+constexpr int SMALL_NT = 1024;       // = TRI2_NT: the fused run kernel calls the K8 body, written for 32 warps
 
 __host__ __device__ inline size_t small_front_doubles(int b, int chi) {
   const size_t m = (size_t)b * chi, b2 = (size_t)b * b;
@@ -23,11 +24,12 @@ __host__ __device__ inline size_t small_front_doubles(int b, int chi) {
 
 // Inputs (global): C[chi][chi], T[chi][b][chi], a_mat[b*b][lda].  Outputs (global): X, Q (m x chi), R (chi x chi),
 // Tn (m x chi), Cn (chi x chi) -- the un-normalised C', T' that K7 consumes.
-__global__ void __launch_bounds__(SMALL_NT, 1)
-small_front_kernel(const double* __restrict__ Cg, const double* __restrict__ Tg, const double* __restrict__ ag,
-                   long long lda, int b, int chi, double* __restrict__ Xg, double* __restrict__ Qg,
-                   double* __restrict__ Rg, double* __restrict__ Tng, double* __restrict__ Cng) {
-  extern __shared__ __align__(16) double ssm[];
+// (no __restrict__ on the bodies: small_run_kernel calls them in a loop in which C, T are rewritten by the K7 body, so
+// their loads must not go through the non-coherent read-only path)
+template <int NT>
+__device__ __forceinline__ void
+small_front_body(double* ssm, const double* Cg, const double* Tg, const double* ag,
+                 long long lda, int b, int chi, double* Xg, double* Qg, double* Rg, double* Tng, double* Cng) {
   const int m = b * chi, b2 = b * b, mc = m * chi, cc = chi * chi;
   double* C = ssm;                 // chi^2
   double* R = C + cc;              // chi^2
@@ -42,21 +44,21 @@ small_front_kernel(const double* __restrict__ Cg, const double* __restrict__ Tg,
   double* tau = S + (size_t)m * m; // chi
   double* wv = tau + chi;          // chi + 64 scratch
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  constexpr int NW = SMALL_NT / 32;
+  constexpr int NW = NT / 32;
 
-  for (int i = tid; i < cc; i += SMALL_NT) C[i] = Cg[i];
-  for (int i = tid; i < mc; i += SMALL_NT) T[i] = Tg[i];
-  for (int i = tid; i < b2 * b2; i += SMALL_NT) a[i] = ag[(long long)(i / b2) * lda + i % b2];
+  for (int i = tid; i < cc; i += NT) C[i] = Cg[i];
+  for (int i = tid; i < mc; i += NT) T[i] = Tg[i];
+  for (int i = tid; i < b2 * b2; i += NT) a[i] = ag[(long long)(i / b2) * lda + i % b2];
   __syncthreads();
   // (E1) X[(j,u),k]: row (j,u) = j*b+u; T as chi x (b chi) row-major: T[i][(u,k)]
-  for (int o = tid; o < mc; o += SMALL_NT) {
+  for (int o = tid; o < mc; o += NT) {
     const int j = o / (b * chi), uk = o % (b * chi);
     double s = 0.0;
     for (int i = 0; i < chi; ++i) s = fma(C[j * chi + i], T[i * b * chi + uk], s);
     X[o] = s;                                            // o = (j*b+u)*chi + k
   }
   __syncthreads();
-  for (int i = tid; i < mc; i += SMALL_NT) Xg[i] = X[i];
+  for (int i = tid; i < mc; i += NT) Xg[i] = X[i];
   // (E2) Householder QR, column by column: warp 0 forms the reflector, then one warp per remaining column applies it
   for (int k = 0; k < chi; ++k) {
     if (warp == 0) {
@@ -87,8 +89,8 @@ small_front_kernel(const double* __restrict__ Cg, const double* __restrict__ Tg,
     }
     __syncthreads();
   }
-  for (int o = tid; o < cc; o += SMALL_NT) R[o] = (o % chi >= o / chi) ? X[o] : 0.0;      // X's top chi rows
-  for (int o = tid; o < mc; o += SMALL_NT) Q[o] = (o / chi == o % chi) ? 1.0 : 0.0;
+  for (int o = tid; o < cc; o += NT) R[o] = (o % chi >= o / chi) ? X[o] : 0.0;      // X's top chi rows
+  for (int o = tid; o < mc; o += NT) Q[o] = (o / chi == o % chi) ? 1.0 : 0.0;
   __syncthreads();
   for (int k = chi - 1; k >= 0; --k) {                   // Q = H_0 ... H_{chi-1} [I; 0]
     const double t = tau[k];
@@ -104,13 +106,13 @@ small_front_kernel(const double* __restrict__ Cg, const double* __restrict__ Tg,
   }
   if (tid < chi) wv[tid] = R[tid * chi + tid] < 0.0 ? -1.0 : 1.0;                         // sign fix: diag(R) >= 0
   __syncthreads();
-  for (int o = tid; o < mc; o += SMALL_NT) Q[o] *= wv[o % chi];
-  for (int o = tid; o < cc; o += SMALL_NT) R[o] *= wv[o / chi];
+  for (int o = tid; o < mc; o += NT) Q[o] *= wv[o % chi];
+  for (int o = tid; o < cc; o += NT) R[o] *= wv[o / chi];
   __syncthreads();
-  for (int o = tid; o < mc; o += SMALL_NT) Qg[o] = Q[o];
-  for (int o = tid; o < cc; o += SMALL_NT) Rg[o] = R[o];
+  for (int o = tid; o < mc; o += NT) Qg[o] = Q[o];
+  for (int o = tid; o < cc; o += NT) Rg[o] = R[o];
   // (E3a) P[(u,l),(J,mm)] = sum_j Q[(j,u),mm] T[j,l,J]
-  for (int o = tid; o < m * m; o += SMALL_NT) {
+  for (int o = tid; o < m * m; o += NT) {
     const int ul = o / cc, Jm = o % cc, u = ul / b, l = ul % b, J = Jm / chi, mm = Jm % chi;
     double s = 0.0;
     for (int j = 0; j < chi; ++j) s = fma(Q[(j * b + u) * chi + mm], T[(j * b + l) * chi + J], s);
@@ -118,7 +120,7 @@ small_front_kernel(const double* __restrict__ Cg, const double* __restrict__ Tg,
   }
   __syncthreads();
   // (E3b) S[(J,d),(mm,r)] = sum_(u,l) P[(u,l),(J,mm)] a[(u,l),(d,r)]
-  for (int o = tid; o < m * m; o += SMALL_NT) {
+  for (int o = tid; o < m * m; o += NT) {
     const int Jd = o / m, mr = o % m, J = Jd / b, d = Jd % b, mm = mr / b, r = mr % b;
     double s = 0.0;
     for (int ul = 0; ul < b2; ++ul) s = fma(P[ul * cc + J * chi + mm], a[ul * b2 + d * b + r], s);
@@ -126,7 +128,7 @@ small_front_kernel(const double* __restrict__ Cg, const double* __restrict__ Tg,
   }
   __syncthreads();
   // (E3c) T'[(mm,r),n] = sum_(J,d) S[(J,d),(mm,r)] Q[(J,d),n];   (E4a) W[(mm,r),n] = sum_k R[mm,k] Q[(k,r),n]
-  for (int o = tid; o < mc; o += SMALL_NT) {
+  for (int o = tid; o < mc; o += NT) {
     const int mr = o / chi, n = o % chi, mm = mr / b, r = mr % b;
     double s = 0.0;
     for (int Jd = 0; Jd < m; ++Jd) s = fma(S[Jd * m + mr], Q[Jd * chi + n], s);
@@ -136,9 +138,9 @@ small_front_kernel(const double* __restrict__ Cg, const double* __restrict__ Tg,
     W[o] = w;
   }
   __syncthreads();
-  for (int o = tid; o < mc; o += SMALL_NT) Tng[o] = Tn[o];
+  for (int o = tid; o < mc; o += NT) Tng[o] = Tn[o];
   // (E4b) C'[p,n] = sum_(mm,r) T'[(mm,r),p] W[(mm,r),n]
-  for (int o = tid; o < cc; o += SMALL_NT) {
+  for (int o = tid; o < cc; o += NT) {
     const int p = o / chi, n = o % chi;
     double s = 0.0;
     for (int mr = 0; mr < m; ++mr) s = fma(Tn[mr * chi + p], W[mr * chi + n], s);
@@ -146,21 +148,30 @@ small_front_kernel(const double* __restrict__ Cg, const double* __restrict__ Tg,
   }
 }
 
+constexpr int SMALL_NT1 = 256;        // stand-alone kernels at the smallest sizes (m <= 40): fewer warps, cheaper barriers
+template <int NT>
+__global__ void __launch_bounds__(NT, 1)
+small_front_kernel(const double* Cg, const double* Tg, const double* ag, long long lda, int b, int chi, double* Xg,
+                   double* Qg, double* Rg, double* Tng, double* Cng) {
+  extern __shared__ __align__(16) double ssm[];
+  small_front_body<NT>(ssm, Cg, Tg, ag, lda, b, chi, Xg, Qg, Rg, Tng, Cng);
+}
+
 // K7 in one CTA: C, T <- sym(C', T') / ||.||_F, the NaN / zero-norm flag, the norms and (hist != null) the history record.
-__global__ void __launch_bounds__(SMALL_NT, 1)
-small_k7_kernel(const double* __restrict__ Cn, const double* __restrict__ Tn, int chi, int b, int symmetrize,
-                double* __restrict__ C, double* __restrict__ T, double* __restrict__ scal, int* __restrict__ flag,
-                double* __restrict__ hist, int* __restrict__ hist_n, const double* __restrict__ R) {
+template <int NT>
+__device__ __forceinline__ void
+small_k7_body(const double* Cn, const double* Tn, int chi, int b, int symmetrize, double* C, double* T, double* scal,
+              int* flag, double* hist, int* hist_n, const double* R) {
   __shared__ double sh[33];
   const int tid = threadIdx.x;
   const int cc = chi * chi, bc = b * chi, mc = bc * chi;
   double ac = 0.0, at = 0.0;
-  for (int o = tid; o < cc; o += SMALL_NT) {
+  for (int o = tid; o < cc; o += NT) {
     double v = Cn[o];
     if (symmetrize) v = 0.5 * (v + Cn[(o % chi) * chi + o / chi]);
     C[o] = v; ac = fma(v, v, ac);
   }
-  for (int o = tid; o < mc; o += SMALL_NT) {
+  for (int o = tid; o < mc; o += NT) {
     const int i = o / bc, s = (o / chi) % b, k = o % chi;
     double v = Tn[o];
     if (symmetrize) v = 0.5 * (v + Tn[k * bc + s * chi + i]);
@@ -170,13 +181,13 @@ small_k7_kernel(const double* __restrict__ Cn, const double* __restrict__ Tn, in
   double ratio = 0.0;
   if (hist) {
     double mn = INFINITY, mx = -INFINITY;
-    for (int k = tid; k < chi; k += SMALL_NT) { const double v = R[k * chi + k]; mn = fmin(mn, v); mx = fmax(mx, v); }
+    for (int k = tid; k < chi; k += NT) { const double v = R[k * chi + k]; mn = fmin(mn, v); mx = fmax(mx, v); }
     const double gmx = block_max(mx, sh), gmn = -block_max(-mn, sh);
     ratio = gmx != 0.0 ? gmn / gmx : 0.0;
   }
   __syncthreads();                                       // every thread's own C, T elements are written; same thread rescales them
-  for (int o = tid; o < cc; o += SMALL_NT) C[o] = C[o] / nc;
-  for (int o = tid; o < mc; o += SMALL_NT) T[o] = T[o] / nt;
+  for (int o = tid; o < cc; o += NT) C[o] = C[o] / nc;
+  for (int o = tid; o < mc; o += NT) T[o] = T[o] / nt;
   if (tid == 0) {
     scal[0] = nc; scal[1] = nt;
     if (!(nc > 0.0) || !(nt > 0.0) || isinf(nc) || isinf(nt)) *flag = 1;
@@ -187,6 +198,49 @@ small_k7_kernel(const double* __restrict__ Cn, const double* __restrict__ Tn, in
       *hist_n = idx + 1;
     }
   }
+}
+
+__global__ void __launch_bounds__(SMALL_NT1, 1)
+small_k7_kernel(const double* Cn, const double* Tn, int chi, int b, int symmetrize, double* C, double* T, double* scal,
+                int* flag, double* hist, int* hist_n, const double* R) {
+  small_k7_body<SMALL_NT1>(Cn, Tn, chi, b, symmetrize, C, T, scal, flag, hist, hist_n, R);
+}
+
+// K9 for tiny problems: the whole run(max_iter, tol) loop in ONE launch of one CTA -- K1..K6, K7, and every
+// check_every steps K8 with the convergence decision delta < tol taken on the device; no host round trip per
+// iteration.  Same semantics as the host drivers (iters = steps executed, delta = last delta or +inf).
+// out[0] = iterations done, out[1] = last delta (doubles, global).
+__host__ __device__ inline size_t small_run_smem_bytes(int b, int chi) {
+  const size_t f = sizeof(double) * small_front_doubles(b, chi), k8 = spectrum_fused_smem_bytes(chi);
+  return f > k8 ? f : k8;
+}
+
+__global__ void __launch_bounds__(SMALL_NT, 1)
+small_run_kernel(double* C, double* T, const double* ag, long long lda, int b, int chi, int symmetrize, double* Xg,
+                 double* Qg, double* Rg, double* Tng, double* Cng, double* scal, int* flag, double* hist, int* hist_n,
+                 double* eig, double* s_out, double* s_prev, double* delta_out, int need_s0, int max_iter, double tol,
+                 int check_every, double* out) {
+  extern __shared__ __align__(16) double dyn[];
+  if (need_s0) {                                 // previous spectrum = spectrum of the environment just set
+    spectrum_fused_body(dyn, C, chi, eig, s_out, s_prev, delta_out, 1, nullptr, nullptr);
+    __syncthreads();
+  }
+  double delta = INFINITY;
+  int it = 1;
+  for (; it <= max_iter; ++it) {
+    small_front_body<SMALL_NT>(dyn, C, T, ag, lda, b, chi, Xg, Qg, Rg, Tng, Cng);
+    __syncthreads();
+    small_k7_body<SMALL_NT>(Cng, Tng, chi, b, symmetrize, C, T, scal, flag, hist, hist_n, Rg);
+    __syncthreads();
+    if (*flag) break;                            // NaN / zero norm: the host reports it
+    if (it % check_every == 0 || it == max_iter) {
+      spectrum_fused_body(dyn, C, chi, eig, s_out, s_prev, delta_out, 1, hist, hist_n);
+      __syncthreads();
+      delta = delta_out[0];
+      if (delta < tol) break;
+    }
+  }
+  if (threadIdx.x == 0) { out[0] = (double)(it <= max_iter ? it : max_iter); out[1] = delta; }
 }
 
 }  // namespace qk

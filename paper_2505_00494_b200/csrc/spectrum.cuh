@@ -275,8 +275,8 @@ __host__ __device__ inline size_t tri2_smem_bytes(int n) {
 //      heights (the first group's columns are n - k rows tall, the last one's a few); the owner of column k+1 also
 //      leaves it as the next u                                                                           -- barrier
 __device__ __forceinline__ void
-tridiag_smem2_body(double* tsm, const double* __restrict__ Cmat, int n, double* dvec, double* evec,
-                   long long* __restrict__ prof /* null, or 8 cycle counters of the phases (thread 0) */) {
+tridiag_smem2_body(double* tsm, const double* Cmat, int n, double* dvec, double* evec,
+                   long long* prof /* null, or 8 cycle counters of the phases (thread 0) */) {
   double2* up0 = reinterpret_cast<double2*>(tsm);               // 2 x n pairs (u_i, p_i), double-buffered over the steps
   double* part = tsm + 4 * n;                                   // TRI2_MAXSUB x n partial sums of A u
   double* red = part + TRI2_MAXSUB * n;                         // 8: per-warp partial sums of p.u
@@ -623,10 +623,9 @@ multisect_kernel(const double* __restrict__ dvec, const double* __restrict__ eve
 
 // One block, blockDim.x >= n: s = sorted |eig| (descending), delta vs s_prev.
 // blockDim.x >= n.  lam[n] (shared): the eigenvalues; s = sorted |lam| (descending), delta vs s_prev.
-__device__ __forceinline__ void spectrum_finalize_body(const double* lam, double* red, int n, double* __restrict__ s_out,
-                                                       double* __restrict__ s_prev, double* __restrict__ delta_out,
-                                                       int update_prev, double* __restrict__ hist,
-                                                       const int* __restrict__ hist_n) {
+__device__ __forceinline__ void spectrum_finalize_body(const double* lam, double* red, int n, double* s_out,
+                                                       double* s_prev, double* delta_out, int update_prev,
+                                                       double* hist, const int* hist_n) {
   const int tid = threadIdx.x;
   if (tid < n) {
     double mine = fabs(lam[tid]);
@@ -666,11 +665,9 @@ __global__ void spectrum_finalize_kernel(const double* __restrict__ eig, int n, 
 constexpr int SPEC_FUSED_MAX_N = 24;
 __host__ __device__ inline size_t spectrum_fused_smem_bytes(int n) { return tri2_smem_bytes(n) + sizeof(double) * (5 * (size_t)n + 40); }
 
-__global__ void __launch_bounds__(TRI2_NT, 1)
-spectrum_fused_kernel(const double* __restrict__ Cmat, int n, double* __restrict__ eig_out, double* __restrict__ s_out,
-                      double* __restrict__ s_prev, double* __restrict__ delta_out, int update_prev,
-                      double* __restrict__ hist, const int* __restrict__ hist_n) {
-  extern __shared__ __align__(16) double tsm[];
+__device__ __forceinline__ void
+spectrum_fused_body(double* tsm, const double* Cmat, int n, double* eig_out, double* s_out, double* s_prev,
+                    double* delta_out, int update_prev, double* hist, const int* hist_n) {
   double* extra = tsm + tri2_smem_bytes(n) / sizeof(double);
   double* dv = extra;                            // n
   double* ev = dv + n;                           // n
@@ -688,6 +685,13 @@ spectrum_fused_kernel(const double* __restrict__ Cmat, int n, double* __restrict
   }
   __syncthreads();
   spectrum_finalize_body(lam, red, n, s_out, s_prev, delta_out, update_prev, hist, hist_n);
+}
+
+__global__ void __launch_bounds__(TRI2_NT, 1)
+spectrum_fused_kernel(const double* Cmat, int n, double* eig_out, double* s_out, double* s_prev, double* delta_out,
+                      int update_prev, double* hist, const int* hist_n) {
+  extern __shared__ __align__(16) double tsm[];
+  spectrum_fused_body(tsm, Cmat, n, eig_out, s_out, s_prev, delta_out, update_prev, hist, hist_n);
 }
 
 }  // namespace qk

@@ -166,7 +166,7 @@ int stage_normalize(qrctm* h, const double* Cn, const double* Tn, bool record = 
   int nbC = (int)(((long long)chi * chi + 255) / 256); if (nbC > 148) nbC = 148;
   int nbT = (int)((nT + 255) / 256); if (nbT > kPartialBlocks) nbT = kPartialBlocks;
   if (!h->small_off && nT + (long long)chi * chi <= 4096) {       // tiny: one CTA does K7 in one launch
-    small_k7_kernel<<<1, SMALL_NT, 0, h->stream>>>(Cn, Tn, chi, b, h->symmetrize, h->C, h->T, h->scal, h->flag,
+    small_k7_kernel<<<1, SMALL_NT1, 0, h->stream>>>(Cn, Tn, chi, b, h->symmetrize, h->C, h->T, h->scal, h->flag,
                                                    record ? h->hist : nullptr, h->flag + 1, h->R);
     h->launches += 1;
     CU(h, cudaGetLastError());
@@ -258,7 +258,9 @@ bool small_ok(qrctm* h) {
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
     h->small_smem = -1;
-    if (optin > 0 && cudaFuncSetAttribute(small_front_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, optin) == cudaSuccess)
+    if (optin > 0 &&
+        cudaFuncSetAttribute(small_front_kernel<SMALL_NT1>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin) == cudaSuccess &&
+        cudaFuncSetAttribute(small_front_kernel<SMALL_NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, optin) == cudaSuccess)
       h->small_smem = optin;
     cudaGetLastError();
   }
@@ -267,8 +269,12 @@ bool small_ok(qrctm* h) {
 
 int stage_small_front(qrctm* h) {
   const size_t smem = sizeof(double) * small_front_doubles(h->b, h->chi);
-  small_front_kernel<<<1, SMALL_NT, smem, h->stream>>>(h->C, h->T, h->a_mat, h->L.lda_a, h->b, h->chi, h->X, h->Q, h->R,
-                                                       h->Tn, h->Cn);
+  if (h->m <= 40)
+    small_front_kernel<SMALL_NT1><<<1, SMALL_NT1, smem, h->stream>>>(h->C, h->T, h->a_mat, h->L.lda_a, h->b, h->chi, h->X, h->Q,
+                                                                   h->R, h->Tn, h->Cn);
+  else
+    small_front_kernel<SMALL_NT><<<1, SMALL_NT, smem, h->stream>>>(h->C, h->T, h->a_mat, h->L.lda_a, h->b, h->chi, h->X, h->Q,
+                                                                 h->R, h->Tn, h->Cn);
   h->launches += 1;
   CU(h, cudaGetLastError());
   return QRCTM_OK;

@@ -550,6 +550,37 @@ def test_small_whole_iteration_kernels_match_the_general_path(d, D, chi, seed):
     assert np.allclose(s[7][:, 1:], g[7][:, 1:], rtol=1e-9) and s[6] * 3 < g[6]
 
 
+@pytest.mark.parametrize("check_every", [2, 3, 7])
+def test_device_side_run_loop_for_tiny_problems(check_every):
+    """Tiny problems with CHECK_EVERY >= 2: qrctm_run is ONE kernel launch, the convergence decision is taken on the
+    device.  Iteration count, delta, environment, history against the oracle's run with the same check interval, and
+    against the pipelined host driver (QRCTM_OPT_SMALL_PATH = 1)."""
+    c = CONFIGS["cfg0"]
+    A, C0, T0 = gen_config(c["d"], c["D"], c["chi"], c["seed"])
+    a = o.build_a(A)
+    res = []
+    for off in (0, 1):
+        h = pkg.QRCTM(c["d"], c["D"], c["chi"])
+        h.set_option(pkg.OPT_SMALL_PATH, off)
+        h.set_option(pkg.OPT_CHECK_EVERY, check_every)
+        h.set_A(A); h.set_env(C0, T0)
+        n0 = h.launch_count()
+        it, dl = h.run(400, 1e-11)
+        res.append((it, dl, h.get_env(), h.launch_count() - n0, h.get_history()[1]))
+        it2, dl2 = h.run(0, 1e-11)
+        assert it2 == 0
+        h.close()
+    (it, dl, (C, T), nl, nh), (itg, dlg, (Cg, Tg), nlg, _) = res
+    assert nl == 1 and nlg > 50 and nh == it
+    assert it == itg and it % check_every == 0 and it < 400 and dl < 1e-11 and abs(dl - dlg) < 1e-13
+    assert rel(C, Cg) < 1e-9 and rel(T, Tg) < 1e-9
+    Co, To, _ = _oracle_steps(A, C0, T0, it)
+    assert rel(C, Co) < 1e-9 and rel(T, To) < 1e-9
+    # the oracle's delta over check_every steps at the stopping point
+    Cp, _, _ = _oracle_steps(A, C0, T0, it - check_every)
+    assert abs(dl - np.max(np.abs(o.spectrum(Co) - o.spectrum(Cp)))) < 1e-12
+
+
 def test_absorb_mode_auto_selects_by_bond_dimension():
     """QRCTM_OPT_ABSORB_MODE = 2: layered from D = 6 up, explicit below -- bitwise the respective fixed mode."""
     for (d, D, chi, seed) in ((2, 6, 12, 3), (2, 4, 16, 2)):
