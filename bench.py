@@ -201,6 +201,8 @@ def bench_config(pkg, torch, name, steps, warmup, peak_dmma, conv=True, corner_m
     h.set_option(pkg.OPT_TIME_STAGES, 0)
     out = {"d": d, "D": D, "chi": chi, "value": 1e3 / ms, "unit": UNIT, "ms_per_step": ms, "steps": steps,
            "gpu_launches_per_step": launches / steps,
+           "path": ("whole-iteration kernels for tiny problems (K1..K6 one launch, K7 one, K8 one; stages_ms below is the "
+                    "general multi-kernel path, timed serially with events)" if launches / steps < 6 else "general"),
            "stages_ms": {k: v / nst for k, v in st.items()},
            "algorithmic_gflop_per_step": sum(fl.values()) / 1e9,
            "step_tflops": sum(fl.values()) / (ms * 1e-3) / 1e12,

@@ -100,6 +100,20 @@ def test_chol_inv_kernel_against_lapack(n):
     assert pkg.chol_inv_f64(torch_dev(G))[2] == 1
 
 
+def test_qr_maximum_column_count():
+    """The build's limit chi <= 800 (form-Q back substitution keeps chi/16 blocks in shared memory): 800 columns work
+    (blocked Householder path, 50 panels), 801 are rejected with QRCTM_ERR_INVALID_ARG instead of failing at launch."""
+    g = np.random.default_rng(800)
+    X = g.standard_normal((1000, 800))
+    Q, R = pkg.qr_f64(torch_dev(X), path=0)
+    Q, R = Q.cpu().numpy(), R.cpu().numpy()
+    assert np.linalg.norm(Q.T @ Q - np.eye(800)) < 800 * 2e-15 and rel(Q @ R, X) < 1e-13
+    assert np.all(np.diag(R) >= 0) and np.all(np.tril(R, -1) == 0)
+    with pytest.raises(pkg.QrctmError):
+        pkg.qr_f64(torch_dev(g.standard_normal((900, 801))), path=0)
+    assert pkg.load_library().qrctm_workspace_bytes(2, 1, 801) == 0 and pkg.load_library().qrctm_workspace_bytes(2, 1, 800) > 0
+
+
 def test_qr_rank_deficient_is_still_valid():
     g = np.random.default_rng(3)
     X = g.standard_normal((200, 6)) @ g.standard_normal((6, 12))       # rank 6 < 12 (hazard H1)
