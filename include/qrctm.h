@@ -36,7 +36,8 @@
  * Limits of this build: D <= 32, chi <= 800, d <= 64.  ONE DEVICE PER PROCESS: the
  * one-time kernel attributes (shared-memory opt-in, cluster sizes, occupancy) are
  * cached per process, so all handles of a process must live on the same device
- * (the one current at the first call).
+ * (the one current at the first call); qrctm_create on a different device returns
+ * QRCTM_ERR_INVALID_ARG.
  */
 #ifndef QRCTM_H
 #define QRCTM_H

@@ -228,6 +228,13 @@ static int create_common(int d, int D, int chi, void* ws, unsigned long long ws_
   if (!make_layout(d, D, chi, &L)) return QRCTM_ERR_INVALID_ARG;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return QRCTM_ERR_CUDA; }
+  {   // one device per process (the one-time kernel attributes are cached per process): fail loudly on a second one
+    static int first_device = -1;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return QRCTM_ERR_CUDA; }
+    if (first_device < 0) first_device = dev;
+    else if (dev != first_device) return QRCTM_ERR_INVALID_ARG;
+  }
   qrctm* h = new (std::nothrow) qrctm();
   if (!h) return QRCTM_ERR_CUDA;
   memset(h, 0, sizeof(*h));
