@@ -64,7 +64,8 @@ enum {
   QRCTM_OPT_GEMM_PATH = 4,   /* 0 = FP64 tensor-core (DMMA) tiles [default], 1 = plain DFMA reference kernel */
   QRCTM_OPT_TIME_STAGES = 5, /* 1 = qrctm_run records CUDA events around every stage of every step (default 0) */
   QRCTM_OPT_QR_PATH = 6,     /* 0 [default] = automatic: CholeskyQR2 (two Gram / Cholesky / triangular-inverse passes, the
-                                O(m chi^2) work on the DMMA GEMM) when 48 <= chi <= 208, checked on the device
+                                O(m chi^2) work on the DMMA GEMM; for chi <= 64 and m chi small enough one cluster launch with the
+                                rows resident in shared memory) when 48 <= chi <= 208 (12 <= chi with the cluster kernel), checked on the device
                                 (||Q1^T Q1 - I||_F <= 1e-4 and no pivot breakdown) and replaced by the Householder path
                                 when the check fails (ill-conditioned or rank-deficient c~); Householder (as 3) outside
                                 that range; 1 = one kernel launch per Householder reflector (slow reference path for

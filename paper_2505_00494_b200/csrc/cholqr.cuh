@@ -23,6 +23,8 @@
 //   * outputs: Rup = L^T (upper, zeros below), Llow = L, Rinv = M^T = R^-1 (upper), status / deviation.
 // Deterministic: fixed summation orders, no atomics.
 #pragma once
+#include <cooperative_groups.h>
+
 #include "gemm_f64.cuh"
 #include "kernels_misc.cuh"
 
@@ -41,12 +43,11 @@ __host__ __device__ inline size_t chol_smem_bytes(int n) {
 // status[0]: 0 ok, 1 = a pivot was not positive / not finite (breakdown).  dev[0] = ||G - I||_F (pass 2: the loss
 // of orthogonality of Q1).  prev_status (may be null): status word of the first pass; verdict (may be null):
 // verdict[0] = 1 when the CholeskyQR2 result must be discarded (either pass broke down or dev > dev_max).
-__global__ void __launch_bounds__(CHOL_NT, 1)
-chol_inv_kernel(const double* __restrict__ G, int n, double* __restrict__ Rup, double* __restrict__ Llow,
-                double* __restrict__ Rinv, int* __restrict__ status, double* __restrict__ dev,
-                const int* __restrict__ prev_status, int* __restrict__ verdict, double dev_max,
-                long long* __restrict__ prof /* null, or 8 cycle counters of the phases (thread 0) */) {
-  extern __shared__ __align__(16) double sm[];
+// (body: CHOL_NT threads of one CTA; sm = chol_smem_bytes(n) of shared memory; every pointer may be global or shared)
+__device__ __forceinline__ void
+chol_inv_body(double* sm, const double* G, int n, double* Rup, double* Llow, double* Rinv, int* status, double* dev,
+              const int* prev_status, int* verdict, double dev_max,
+              long long* prof /* null, or 8 cycle counters of the phases (thread 0) */) {
   const int nb = (n + 15) / 16, np = nb * 16;
   double* rd = sm + chol_base(nb);             // reciprocal diagonal of L
   double* red = rd + 16 * nb;                  // 33 doubles for the block reduction + flags
@@ -55,6 +56,7 @@ chol_inv_kernel(const double* __restrict__ G, int n, double* __restrict__ Rup, d
   const int lr = lane >> 2, lc = lane & 3;
   constexpr int NW = CHOL_NT / 32;
   if (tid == 0) bad = 0;
+  __syncthreads();
   long long tp[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tc = 0;
 #define CHOL_TICK(i) do { if (prof && tid == 0) { const long long t_ = clock64(); tp[i] += t_ - tc; tc = t_; } } while (0)
   if (prof && tid == 0) tc = clock64();
@@ -280,6 +282,167 @@ chol_inv_kernel(const double* __restrict__ G, int n, double* __restrict__ Rup, d
     if (tid == 0) for (int i = 0; i < 8; ++i) prof[i] = tp[i];
   }
 #undef CHOL_TICK
+}
+
+__global__ void __launch_bounds__(CHOL_NT, 1)
+chol_inv_kernel(const double* __restrict__ G, int n, double* __restrict__ Rup, double* __restrict__ Llow,
+                double* __restrict__ Rinv, int* __restrict__ status, double* __restrict__ dev,
+                const int* __restrict__ prev_status, int* __restrict__ verdict, double dev_max,
+                long long* __restrict__ prof) {
+  extern __shared__ __align__(16) double sm[];
+  chol_inv_body(sm, G, n, Rup, Llow, Rinv, status, dev, prev_status, verdict, dev_max, prof);
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// CholeskyQR2 of a small c~ (n <= CHOLC_MAX_N columns, rows <= 16 slabs that fit shared memory: cfg1, cfg2) as ONE
+// launch of one thread-block cluster instead of eleven dependent launches (which cost 10-20 us each at these sizes:
+// K2 was 55 % of the cfg1 / cfg2 step).  The rows of X are dealt out to the CTAs in contiguous slabs that stay in
+// shared memory through both passes; per pass: local Gram matrix of the slab -> fixed-order sum over the cluster
+// through distributed shared memory (every CTA ends with the full G) -> every CTA factors and inverts G redundantly
+// (chol_inv_body) -> slab <- slab R^-1.  Rank 0 writes R = L2^T R1 and the status / verdict words.  Deterministic.
+constexpr int CHOLC_MAX_N = 64;
+__host__ __device__ inline size_t cholqr2_cluster_smem_bytes(int n, int rpc) {
+  return sizeof(double) * ((size_t)4 * n * n + (size_t)2 * rpc * n + 8) + chol_smem_bytes(n);
+}
+
+__global__ void __launch_bounds__(CHOL_NT, 1)
+cholqr2_cluster_kernel(const double* __restrict__ X, long long rows, int n, double* __restrict__ Q, double* __restrict__ R,
+                       int* __restrict__ cstat /* [3] */, double* __restrict__ cdev /* [2] */, double dev_max, int rpc,
+                       long long* __restrict__ prof /* null, or 8 cycle counters of rank 0's phases */) {
+  namespace cg = cooperative_groups;
+  cg::cluster_group cluster = cg::this_cluster();
+  const int C = (int)cluster.num_blocks(), rank = (int)cluster.block_rank();
+  extern __shared__ __align__(16) double csm[];
+  const int nn = n * n;
+  double* Gp = csm;                      // my slab's partial Gram matrix (pass 2: reused for L2 after the sum)
+  double* Gf = Gp + nn;                  // the full Gram matrix (written by all ranks)
+  double* R1 = Gf + nn;                  // R of pass 1
+  double* Ri = R1 + nn;                  // R^-1 of the current pass
+  double* Xs = Ri + nn;                  // rpc x n: my rows of X, then of Q1 after the swap
+  double* Ys = Xs + (size_t)rpc * n;
+  double* sc = Ys + (size_t)rpc * n;     // [0..1] deviations, ints behind
+  int* st = reinterpret_cast<int*>(sc + 4);
+  double* ws = sc + 8;                   // chol_inv_body's workspace
+  const int tid = threadIdx.x;
+  long long tp[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tc = 0;
+#define CQ_TICK(i) do { if (prof && tid == 0 && rank == 0) { const long long t_ = clock64(); tp[i] += t_ - tc; tc = t_; } } while (0)
+  if (prof && tid == 0 && rank == 0) tc = clock64();
+  const long long r0 = (long long)rank * rpc;
+  const int rl = (int)(rows - r0 < 0 ? 0 : (rows - r0 < rpc ? rows - r0 : rpc));      // my rows
+  for (int i = tid; i < rl * n; i += CHOL_NT) Xs[i] = X[r0 * n + i];
+  __syncthreads();
+  CQ_TICK(0);
+  double* src = Xs;
+  double* dst = Ys;
+  for (int pass = 0; pass < 2; ++pass) {
+    // local Gram matrix of the slab, lower block triangle in 4 x 4 register blocks (a plain one-output-per-thread loop
+    // is bound by shared-memory bandwidth: three wavefronts per FMA; here 8 loads feed 16 FMAs)
+    const int nq = (n + 3) >> 2, nblk = nq * (nq + 1) / 2;
+    for (int q = tid; q < nblk; q += CHOL_NT) {
+      int bi = (int)((sqrtf(8.0f * q + 1.0f) - 1.0f) * 0.5f);
+      while ((bi + 1) * (bi + 2) / 2 <= q) ++bi;
+      while (bi * (bi + 1) / 2 > q) --bi;
+      const int bj = q - bi * (bi + 1) / 2, i0 = bi << 2, j0 = bj << 2;
+      double g[4][4];
+#pragma unroll
+      for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) g[a][c] = 0.0;
+      for (int r = 0; r < rl; ++r) {
+        double xi[4], xj[4];
+#pragma unroll
+        for (int a = 0; a < 4; ++a) { xi[a] = i0 + a < n ? src[r * n + i0 + a] : 0.0; xj[a] = j0 + a < n ? src[r * n + j0 + a] : 0.0; }
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+#pragma unroll
+          for (int c = 0; c < 4; ++c) g[a][c] = fma(xi[a], xj[c], g[a][c]);
+      }
+#pragma unroll
+      for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+          if (i0 + a < n && j0 + c < n) Gp[(i0 + a) * n + j0 + c] = g[a][c];
+    }
+    CQ_TICK(1);
+    cluster.sync();
+    CQ_TICK(2);
+    // fixed-order sum over the ranks of the lower block triangle; rank r owns the blocks q = r (mod C) and hands the
+    // sums to everybody; the upper triangle is mirrored locally afterwards
+    for (int w = rank * 16 + C * 16 * (tid >> 4) + (tid & 15); (w >> 4) < nblk; w += C * 16 * (CHOL_NT >> 4)) {
+      const int q = w >> 4, el = w & 15;
+      int bi = (int)((sqrtf(8.0f * q + 1.0f) - 1.0f) * 0.5f);
+      while ((bi + 1) * (bi + 2) / 2 <= q) ++bi;
+      while (bi * (bi + 1) / 2 > q) --bi;
+      const int bj = q - bi * (bi + 1) / 2, i = (bi << 2) + (el >> 2), j = (bj << 2) + (el & 3);
+      if (i < n && j < n) {
+        const int e = i * n + j;
+        double s = 0.0;
+        for (int qq = 0; qq < C; ++qq) s += cluster.map_shared_rank(Gp, qq)[e];
+        for (int qq = 0; qq < C; ++qq) cluster.map_shared_rank(Gf, qq)[e] = s;
+      }
+    }
+    CQ_TICK(3);
+    cluster.sync();
+    CQ_TICK(2);
+    for (int e = tid; e < nn; e += CHOL_NT) {               // mirror: blocks above the block diagonal
+      const int i = e / n, j = e % n;
+      if ((j >> 2) > (i >> 2)) Gf[e] = Gf[j * n + i];
+    }
+    __syncthreads();
+    if (pass == 0) chol_inv_body(ws, Gf, n, R1, nullptr, Ri, st, sc, nullptr, nullptr, 0.0, nullptr);
+    else           chol_inv_body(ws, Gf, n, nullptr, Gp, Ri, st + 1, sc + 1, st, st + 2, dev_max, nullptr);
+    __syncthreads();
+    CQ_TICK(4);
+    // slab <- slab R^-1 (R^-1 upper triangular) in 4 x 4 register blocks: pass 1 into the other buffer, pass 2 to Q
+    {
+      const int nrb = (rl + 3) >> 2;
+      for (int q = tid; q < nrb * nq; q += CHOL_NT) {
+        const int rb = q / nq, cb = q % nq, rr0 = rb << 2, c0 = cb << 2;
+        double y[4][4];
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+#pragma unroll
+          for (int c = 0; c < 4; ++c) y[a][c] = 0.0;
+        const int kend = c0 + 4 < n ? c0 + 4 : n;           // R^-1[k][c] = 0 for k > c
+        for (int k = 0; k < kend; ++k) {
+          double xs[4], rv[4];
+#pragma unroll
+          for (int a = 0; a < 4; ++a) { xs[a] = rr0 + a < rl ? src[(rr0 + a) * n + k] : 0.0; rv[a] = c0 + a < n ? Ri[k * n + c0 + a] : 0.0; }
+#pragma unroll
+          for (int a = 0; a < 4; ++a)
+#pragma unroll
+            for (int c = 0; c < 4; ++c) y[a][c] = fma(xs[a], rv[c], y[a][c]);
+        }
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+#pragma unroll
+          for (int c = 0; c < 4; ++c)
+            if (rr0 + a < rl && c0 + c < n) {
+              const int idx = (rr0 + a) * n + c0 + c;
+              if (pass == 0) dst[idx] = y[a][c]; else Q[r0 * n + idx] = y[a][c];
+            }
+      }
+    }
+    __syncthreads();
+    CQ_TICK(5);
+    double* t = src; src = dst; dst = t;
+  }
+  // R = R2 R1 = L2^T R1 (both triangular: j runs over i..k): every rank holds L2 and R1, rank r writes the rows i = r (mod C)
+  for (int e = tid; e < ((n - rank + C - 1) / C) * n; e += CHOL_NT) {
+    const int i = rank + C * (e / n), k = e % n;
+    double s = 0.0;
+    for (int j = i; j <= k; ++j) s = fma(Gp[j * n + i], R1[j * n + k], s);
+    R[i * n + k] = s;
+  }
+  if (rank == 0) {
+    if (tid == 0) { cstat[0] = st[0]; cstat[1] = st[1]; cstat[2] = st[2]; cdev[0] = sc[0]; cdev[1] = sc[1]; }
+    if (prof) {
+      __syncthreads();
+      CQ_TICK(6);
+      if (tid == 0) for (int i = 0; i < 8; ++i) prof[i] = tp[i];
+    }
+  }
+#undef CQ_TICK
 }
 
 // The conditional-graph hook of the fallback: 1 = run the body (the Householder path).

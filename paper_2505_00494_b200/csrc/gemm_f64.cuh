@@ -87,6 +87,15 @@ __host__ __device__ inline long long sk_first_unit(long long c, long long units,
 constexpr int BK = 16;
 constexpr int PAD = 4;
 
+// Programmatic dependent launch: the kernels of a step are short and strictly dependent, so each one lets its
+// successor in the stream be set up at once (launch_dependents: the successor's CTAs become resident as SM slots free
+// up and run their own prologue) and then waits until its predecessor has completed and flushed its writes (wait).  A
+// no-op for kernels launched without the programmatic-serialisation attribute.
+__device__ __forceinline__ void pdl_sync() {
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
 __device__ __forceinline__ void cp_async16(void* smem, const void* g, int src_bytes) {
   uint32_t s = (uint32_t)__cvta_generic_to_shared(smem);
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(g), "r"(src_bytes));
@@ -171,6 +180,7 @@ gemm_f64_dmma(GemmArgs p) {
   for (int i = 0; i < FM; ++i)
 #pragma unroll
     for (int j = 0; j < FN; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+  pdl_sync();
 
   auto load_stage = [&](int kt, int stage) {
     int k0 = (kt_begin + kt) * BK;
@@ -328,6 +338,7 @@ gemm_f64_dmma_ws(const __grid_constant__ GemmArgs p) {
     asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
   }
   __syncthreads();
+  pdl_sync();
 
   if (warp == NCW) {
     // ------------------------------ producer warp
@@ -636,6 +647,7 @@ __global__ void gemm_f64_ref(GemmArgs p) {
 // out[ro(i)+co(j)] (op)= sum_z part[z][i][j], z ascending (fixed order).
 __global__ void reduce_splitk(const double* part, long long split_stride, int splits, int M, int N,
                               double* out, IndexMap ro, IndexMap co, int mode) {
+  pdl_sync();
   long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= (long long)M * N) return;
   int i = (int)(idx / N), j = (int)(idx % N);
@@ -665,6 +677,7 @@ streamk_fixup(const double* __restrict__ ws, int BM, int BN, int tn, int nkt, lo
               int N, double* out, IndexMap ro, IndexMap co, int mode) {
   __shared__ int slots[SK_MAXSEG];
   __shared__ int nseg_s;
+  pdl_sync();
   const int t = t1 + blockIdx.x;                             // tiles below t1 were stored directly
   if (threadIdx.x == 0) {
     const long long ub = (long long)t * nkt, ue = ub + nkt;

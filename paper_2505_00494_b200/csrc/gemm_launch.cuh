@@ -4,6 +4,18 @@
 
 // ------------------------------------------------------------------ GEMM launcher
 
+// Launch with programmatic stream serialisation (kernels: pdl_sync() in gemm_f64.cuh).
+template <class... KArgs, class... Args>
+cudaError_t pdl_launch(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+
 template <int BM, int BN, int WM, int WN, int STAGES>
 cudaError_t launch_cfg(cudaStream_t st, const GemmArgs& g, int splits) {
   constexpr int NT = (BM / WM) * (BN / WN) * 32;
@@ -16,8 +28,7 @@ cudaError_t launch_cfg(cudaStream_t st, const GemmArgs& g, int splits) {
     attr_done = true;
   }
   dim3 grid((g.N + BN - 1) / BN, (g.M + BM - 1) / BM, splits);
-  gemm_f64_dmma<BM, BN, WM, WN, STAGES><<<grid, NT, smem, st>>>(g);
-  return cudaGetLastError();
+  return pdl_launch(gemm_f64_dmma<BM, BN, WM, WN, STAGES>, grid, dim3(NT), smem, st, g);
 }
 
 // Tensor maps for the tiled bulk copies of the ws kernel (the encoder comes from the driver through the runtime, the
@@ -97,17 +108,16 @@ cudaError_t launch_cfg_ws(cudaStream_t st, const GemmArgs& g, int splits, Stream
         sk_attr = true;
       }
       ga.sk = 1; ga.sk_ws = sk->ws; ga.sk_t1 = (int)t1;
-      gemm_f64_dmma_ws<BM, BN, WM, WN, STAGES, true><<<(unsigned)ncta, NT, smem, st>>>(ga);
-      streamk_fixup<<<dim3((unsigned)(nwork - t1), 8), 256, 0, st>>>(sk->ws, BM, BN, tn, nkt, units, (int)ncta, (int)t1, g.M,
-                                                                    g.N, g.out, g.ro, g.co, g.mode);
-      return cudaGetLastError();
+      cudaError_t e1 = pdl_launch(gemm_f64_dmma_ws<BM, BN, WM, WN, STAGES, true>, dim3((unsigned)ncta), dim3(NT), smem, st, ga);
+      if (e1 != cudaSuccess) return e1;
+      return pdl_launch(streamk_fixup, dim3((unsigned)(nwork - t1), 8), dim3(256), 0, st, (const double*)sk->ws, BM, BN, tn, nkt,
+                        units, (int)ncta, (int)t1, g.M, g.N, g.out, g.ro, g.co, g.mode);
     }
   }
   (void)nslots;                                  // one work item per CTA: the hardware scheduler balances better
   const unsigned grid = (unsigned)nwork;         // than a static persistent loop, with or without a start-up stagger
                                                  // between the two CTAs of an SM (measured, profiles/r1_gemm_experiments.md)
-  gemm_f64_dmma_ws<BM, BN, WM, WN, STAGES><<<grid, NT, smem, st>>>(ga);
-  return cudaGetLastError();
+  return pdl_launch(gemm_f64_dmma_ws<BM, BN, WM, WN, STAGES>, dim3(grid), dim3(NT), smem, st, ga);
 }
 
 // Resident-B persistent launch (kernel: RESB = true): N <= BN, K short enough for all of B to sit in shared memory.
@@ -146,8 +156,7 @@ cudaError_t launch_cfg_ws_resb(cudaStream_t st, const GemmArgs& g, int nz) {
   const long long nwork = (long long)((g.M + BM - 1) / BM) * nz;
   const long long slots = (long long)nsm * per;
   const unsigned grid = (unsigned)(nwork < slots ? nwork : slots);
-  kern<<<grid, NT, smem, st>>>(ga);
-  return cudaGetLastError();
+  return pdl_launch(kern, dim3(grid), dim3(NT), smem, st, ga);
 }
 
 struct GemmCall {
@@ -300,9 +309,8 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
   if (skreq.used) ++launched;
   if (splits > 1) {
     long long n = (long long)c.M * c.N;
-    reduce_splitk<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(splitk_ws, g.split_stride, splits, c.M, c.N,
-                                                              c.out, c.ro, c.co, c.mode);
-    *err = cudaGetLastError();
+    *err = pdl_launch(reduce_splitk, dim3((unsigned)((n + 255) / 256)), dim3(256), 0, st, (const double*)splitk_ws, g.split_stride,
+                      splits, c.M, c.N, c.out, c.ro, c.co, c.mode);
     if (*err != cudaSuccess) return -1;
     ++launched;
   }

@@ -436,6 +436,7 @@ cudaError_t cholqr_capture_body(cudaStream_t aux, cudaGraph_t body, long long ro
 }
 
 constexpr int kCholqrMinN = 48;
+constexpr int kCholqrMinNCluster = 12;    // with the one-launch cluster kernel CholeskyQR2 wins from ~12 columns
 constexpr double kCholqrDevMax = 1e-4;     // ||Q1^T Q1 - I||_F above this: cond(c~)^2 eps is not small, discard
 
 cudaError_t chol_inv_attr() {
@@ -458,7 +459,37 @@ long long qr_factor_cholqr2(cudaStream_t st, long long rows, int n, const double
   const size_t smem = chol_smem_bytes(n);
   long long launches = 0;
   int nl;
+  // small c~: the whole CholeskyQR2 in one cluster launch (cholqr.cuh) when 16 row slabs fit shared memory
+  bool clustered = false;
+  if (n <= CHOLC_MAX_N && rows >= 32) {
+    static int optin = 0, c16 = -1;
+    if (c16 < 0) {
+      int dev = 0; cudaGetDevice(&dev);
+      cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+      c16 = (cudaFuncSetAttribute(cholqr2_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, optin - 1024) == cudaSuccess &&
+             cudaFuncSetAttribute(cholqr2_cluster_kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess) ? 1 : 0;
+      cudaGetLastError();
+    }
+    int C = 16;
+    while (C > 2 && (rows + C / 2 - 1) / (C / 2) <= 48) C /= 2;          // at least ~48 rows per CTA
+    const int rpc = (int)((rows + C - 1) / C);
+    const size_t csm = cholqr2_cluster_smem_bytes(n, rpc);
+    if (c16 == 1 && csm + 1024 <= (size_t)optin) {
+      cudaLaunchConfig_t cfg = {};
+      cfg.gridDim = dim3(C); cfg.blockDim = dim3(CHOL_NT); cfg.dynamicSmemBytes = csm; cfg.stream = st;
+      cudaLaunchAttribute at[1];
+      at[0].id = cudaLaunchAttributeClusterDimension;
+      at[0].val.clusterDim.x = C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+      cfg.attrs = at; cfg.numAttrs = 1;
+      *err = cudaLaunchKernelEx(&cfg, cholqr2_cluster_kernel, X, rows, n, Q, R, wk.cstat, wk.cdev, kCholqrDevMax, rpc,
+                                static_cast<long long*>(nullptr));
+      if (*err != cudaSuccess) return -1;
+      launches += 1;
+      clustered = true;
+    }
+  }
   const dim3 tg((unsigned)((rows + 31) / 32), (n + 31) / 32), tb(32, 8);
+  if (!clustered) {
   // pass 1
   nl = launch_gemm(st, 0, GemmCall{X, n, 1, X, n, wk.Gq, plain_map(n), IndexMap{1, 1, 0}, n, n, (int)rows, 0},
                    wk.splitk, wk.splitk_elems, err);
@@ -488,6 +519,7 @@ long long qr_factor_cholqr2(cudaStream_t st, long long rows, int n, const double
                    wk.splitk, wk.splitk_elems, err);                                   // R = R2 R1 = L2^T R1
   if (nl < 0) return -1;
   launches += nl;
+  }
   *err = cudaGetLastError();
   if (*err != cudaSuccess) return -1;
   if (fb.mode == 1) {
@@ -537,7 +569,8 @@ long long qr_factor_blocked(cudaStream_t st, int qr_path, long long rows, int n,
                             double* R, void* work, cudaError_t* err, QrFallback fb = QrFallback{1, nullptr, nullptr}) {
   // below ~48 columns the whole QR is launch-latency bound and the single-launch register-resident Householder
   // kernel wins (cfg0: 44 us against 71 us, cfg1: 119 against 133; measured, profiles/r2_k2_cholqr2.md)
-  if (qr_path == 0 && n >= kCholqrMinN) {
+  if (qr_path == 0 && (n >= kCholqrMinN || (n >= kCholqrMinNCluster && n <= CHOLC_MAX_N && rows >= 32 &&
+                        cholqr2_cluster_smem_bytes(n, (int)((rows + 15) / 16)) + 2048 <= (size_t)227 * 1024))) {
     const long long nl = qr_factor_cholqr2(st, rows, n, X, Q, R, work, err, fb);
     if (nl != -2) return nl;
   }
