@@ -66,6 +66,8 @@ struct qrctm {
   int use_graph, warm_steps, graph_failed;
   int need_s0;                    // spectrum of the environment set by set_env not computed yet (lazy)
   cudaStream_t cap_aux;         // captures the body of the conditional Householder fallback of K2 (never runs work itself)
+  cudaStream_t branch;          // K6's first product W = R.Q (needs only K2's outputs) runs here beside K3..K5
+  cudaEvent_t ev_fork, ev_join;
   cudaStream_t side;            // high-priority stream for the overlapped convergence check
   cudaEvent_t ev_env, ev_spec;  // environment ready (main) / spectrum done (side)
   int overlap;
@@ -268,6 +270,9 @@ static int create_common(int d, int D, int chi, void* ws, unsigned long long ws_
     }
   }
   if (cudaStreamCreateWithFlags(&h->cap_aux, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); h->cap_aux = nullptr; }
+  if (cudaStreamCreateWithFlags(&h->branch, cudaStreamNonBlocking) != cudaSuccess ||
+      cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+      cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); h->branch = nullptr; }
   h->h_flag = reinterpret_cast<int*>(h->h_pinned + kPinFlag);
   cudaMemsetAsync(h->flag, 0, 4 * sizeof(int), 0);
   {   // padded operand matrices: the pad columns are zeroed once and never written again
@@ -300,6 +305,7 @@ int qrctm_destroy(qrctm_t* h) {
   if (h->eigwork) cudaFree(h->eigwork);
   if (h->h_pinned) cudaFreeHost(h->h_pinned);
   if (h->cap_aux) cudaStreamDestroy(h->cap_aux);
+  if (h->branch) { cudaStreamSynchronize(h->branch); cudaStreamDestroy(h->branch); cudaEventDestroy(h->ev_fork); cudaEventDestroy(h->ev_join); }
   if (h->side) { cudaStreamSynchronize(h->side); cudaStreamDestroy(h->side); cudaEventDestroy(h->ev_env); cudaEventDestroy(h->ev_spec); }
   if (h->have_ev) for (int i = 0; i < QRCTM_NSTAGE + 2; ++i) cudaEventDestroy(h->ev[i]);
   cudaGetLastError();

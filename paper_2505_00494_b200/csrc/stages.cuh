@@ -132,16 +132,28 @@ int stage_project(qrctm* h, const double* S, const double* Qm, double* out, int 
 }
 
 // K6 (E4): W[m,(r,n)] = sum_k R[m,k] Q[k,(r,n)] ;  C'[p,n] = sum_{(m,r)} T'[(m,r),p] W[(m,r),n]
-int stage_corner_accel(qrctm* h) {
-  const int chi = h->chi; const long long bc = (long long)h->b * chi, m = h->m;
+// first half: W = R.Q needs only K2's outputs, so it can run on another stream beside K3..K5 (no scratch: no K split)
+int stage_corner_accel_w(qrctm* h, cudaStream_t st) {
+  const int chi = h->chi; const long long bc = (long long)h->b * chi;
   // W^T[(r,n), m] = sum_k Q[k,(r,n)] R^T[k,m]  (long index as M, both operands K-major); writes W
-  transpose_small_kernel<<<(chi * chi + 255) / 256, 256, 0, h->stream>>>(h->R, chi, h->Rt);
+  transpose_small_kernel<<<(chi * chi + 255) / 256, 256, 0, st>>>(h->R, chi, h->Rt);
   h->launches += 1;
   GemmCall c1{h->Q, bc, 1, h->Rt, chi, h->W, IndexMap{1, 1, 0}, plain_map(bc), (int)bc, chi, chi, 0};
-  GEMM(h, c1);
+  cudaError_t ge;
+  const int nl = launch_gemm(st, h->gemm_path, c1, nullptr, 0, &ge);
+  if (nl < 0) return fail(h, QRCTM_ERR_CUDA, "gemm launch", ge);
+  h->launches += nl;
+  return QRCTM_OK;
+}
+int stage_corner_accel_c(qrctm* h) {
+  const int chi = h->chi; const long long m = h->m;
   GemmCall c2{h->Tn, chi, 1, h->W, chi, h->Cn, plain_map(chi), IndexMap{1, 1, 0}, chi, chi, (int)m, 0};
   GEMM(h, c2);
   return QRCTM_OK;
+}
+int stage_corner_accel(qrctm* h) {
+  int rc = stage_corner_accel_w(h, h->stream); if (rc) return rc;
+  return stage_corner_accel_c(h);
 }
 
 // K6' (E5)+(E4'): Z = half_absorb(X), C~ = Z.a, Y = C~ Q, C' = Q^T Y.  K4's epilogue writes C~ transposed,
@@ -301,13 +313,27 @@ int do_step(qrctm* h, cudaEvent_t* ev /* QRCTM_NSTAGE+1 events or null */, bool 
     mark(1, "K2_qr");
     rc = stage_qr(h);
   }
+  // fork: K6's first product beside K3..K5 (not when per-stage events are wanted: the stage times would overlap)
+  const bool forked = !rc && !ev && h->branch && h->corner_mode == 0 && h->stream != nullptr;
+  if (forked) {
+    if (cudaEventRecord(h->ev_fork, h->stream) != cudaSuccess || cudaStreamWaitEvent(h->branch, h->ev_fork, 0) != cudaSuccess)
+      rc = fail(h, QRCTM_ERR_CUDA, "fork", cudaGetLastError());
+    if (!rc) rc = stage_corner_accel_w(h, h->branch);
+    if (!rc && cudaEventRecord(h->ev_join, h->branch) != cudaSuccess) rc = fail(h, QRCTM_ERR_CUDA, "fork", cudaGetLastError());
+  }
   if (!rc) { mark(2, "K3_half_absorb"); rc = stage_half_absorb(h, h->Q, h->T, h->P); }
   if (!rc) {
     mark(3, "K4_absorb_a");
     rc = use_layered(h) ? stage_absorb_layered(h, h->P, h->S) : stage_absorb_a(h, h->P, h->S, 0);
   }
   if (!rc) { mark(4, "K5_project"); rc = stage_project(h, h->S, h->Q, h->Tn); }
-  if (!rc) { mark(5, "K6_corner"); rc = h->corner_mode == 0 ? stage_corner_accel(h) : stage_corner_enlarged(h); }
+  if (!rc) {
+    mark(5, "K6_corner");
+    if (forked) {
+      if (cudaStreamWaitEvent(h->stream, h->ev_join, 0) != cudaSuccess) rc = fail(h, QRCTM_ERR_CUDA, "join", cudaGetLastError());
+      if (!rc) rc = stage_corner_accel_c(h);
+    } else rc = h->corner_mode == 0 ? stage_corner_accel(h) : stage_corner_enlarged(h);
+  }
   if (!rc && !with_k7) { nvtxRangePop(); return rc; }
   if (!rc) { mark(6, "K7_normalize"); rc = stage_normalize(h, h->Cn, h->Tn, true); }
   if (!rc) mark(7, nullptr); else nvtxRangePop();
