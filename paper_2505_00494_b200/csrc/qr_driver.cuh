@@ -391,7 +391,12 @@ long long qr_factor_fullreg_t(cudaStream_t st, long long rows, int n, const doub
 //   mode 3: direct launches without a host round trip: a small graph {set condition; IF node with the Householder
 //           path as its body} is built once (captured on `aux`), kept in *cache by the caller, and launched on the
 //           stream after the CholeskyQR2 kernels.
-struct QrFallback { int mode; cudaStream_t aux; cudaGraphExec_t* cache; };
+struct QrFallback {
+  int mode; cudaStream_t aux; cudaGraphExec_t* cache;
+  // optional second stream + two events: the independent pieces of CholeskyQR2 (the transposes beside the Gram /
+  // Cholesky chain, R = R2 R1 beside Q = Q1 R2^-1) are forked onto it
+  cudaStream_t br = nullptr; cudaEvent_t e_fork = nullptr, e_join = nullptr;
+};
 
 long long qr_factor_householder(cudaStream_t st, int qr_path, long long rows, int n, const double* X, double* Q,
                                 double* R, void* work, cudaError_t* err);
@@ -489,36 +494,59 @@ long long qr_factor_cholqr2(cudaStream_t st, long long rows, int n, const double
     }
   }
   const dim3 tg((unsigned)((rows + 31) / 32), (n + 31) / 32), tb(32, 8);
+  const bool fork_ok = fb.br != nullptr && fb.e_fork != nullptr && fb.e_join != nullptr && st != nullptr;
   if (!clustered) {
   // pass 1
+  if (fork_ok) {                                   // X^T for the first product, beside Gram matrix and factorisation
+    if (cudaEventRecord(fb.e_fork, st) != cudaSuccess || cudaStreamWaitEvent(fb.br, fb.e_fork, 0) != cudaSuccess) { *err = cudaGetLastError(); return -1; }
+    transpose_tall_kernel<<<tg, tb, 0, fb.br>>>(X, rows, n, wk.Vct);
+    if (cudaEventRecord(fb.e_join, fb.br) != cudaSuccess) { *err = cudaGetLastError(); return -1; }
+  }
   nl = launch_gemm(st, 0, GemmCall{X, n, 1, X, n, wk.Gq, plain_map(n), IndexMap{1, 1, 0}, n, n, (int)rows, 0},
                    wk.splitk, wk.splitk_elems, err);
   if (nl < 0) return -1;
   launches += nl;
   chol_inv_kernel<<<1, CHOL_NT, smem, st>>>(wk.Gq, n, wk.cR1, nullptr, wk.cRi1, wk.cstat, wk.cdev, nullptr, nullptr, 0.0, nullptr);
-  transpose_tall_kernel<<<tg, tb, 0, st>>>(X, rows, n, wk.Vct);
+  if (!fork_ok) transpose_tall_kernel<<<tg, tb, 0, st>>>(X, rows, n, wk.Vct);
+  else if (cudaStreamWaitEvent(st, fb.e_join, 0) != cudaSuccess) { *err = cudaGetLastError(); return -1; }
   launches += 2;
   nl = launch_gemm(st, 0, GemmCall{wk.Vct, rows, 1, wk.cRi1, n, wk.V, plain_map(n), IndexMap{1, 1, 0}, (int)rows, n, n, 0},
                    wk.splitk, wk.splitk_elems, err);                                   // Q1 = X R1^-1
   if (nl < 0) return -1;
   launches += nl;
   // pass 2
+  if (fork_ok) {                                   // Q1^T for the second product, beside Gram matrix and factorisation
+    if (cudaEventRecord(fb.e_fork, st) != cudaSuccess || cudaStreamWaitEvent(fb.br, fb.e_fork, 0) != cudaSuccess) { *err = cudaGetLastError(); return -1; }
+    transpose_tall_kernel<<<tg, tb, 0, fb.br>>>(wk.V, rows, n, wk.Vct);
+    if (cudaEventRecord(fb.e_join, fb.br) != cudaSuccess) { *err = cudaGetLastError(); return -1; }
+  }
   nl = launch_gemm(st, 0, GemmCall{wk.V, n, 1, wk.V, n, wk.Gq, plain_map(n), IndexMap{1, 1, 0}, n, n, (int)rows, 0},
                    wk.splitk, wk.splitk_elems, err);
   if (nl < 0) return -1;
   launches += nl;
   chol_inv_kernel<<<1, CHOL_NT, smem, st>>>(wk.Gq, n, nullptr, wk.cL2, wk.cRi2, wk.cstat + 1, wk.cdev + 1, wk.cstat,
                                             wk.cstat + 2, kCholqrDevMax, nullptr);
-  transpose_tall_kernel<<<tg, tb, 0, st>>>(wk.V, rows, n, wk.Vct);
+  if (!fork_ok) transpose_tall_kernel<<<tg, tb, 0, st>>>(wk.V, rows, n, wk.Vct);
+  else {
+    if (cudaStreamWaitEvent(st, fb.e_join, 0) != cudaSuccess) { *err = cudaGetLastError(); return -1; }
+    // R = R2 R1 = L2^T R1 beside Q = Q1 R2^-1 (no scratch: no K split on the side stream)
+    if (cudaEventRecord(fb.e_fork, st) != cudaSuccess || cudaStreamWaitEvent(fb.br, fb.e_fork, 0) != cudaSuccess) { *err = cudaGetLastError(); return -1; }
+    nl = launch_gemm(fb.br, 0, GemmCall{wk.cL2, n, 1, wk.cR1, n, R, plain_map(n), IndexMap{1, 1, 0}, n, n, n, 0}, nullptr, 0, err);
+    if (nl < 0) return -1;
+    launches += nl;
+    if (cudaEventRecord(fb.e_join, fb.br) != cudaSuccess) { *err = cudaGetLastError(); return -1; }
+  }
   launches += 2;
   nl = launch_gemm(st, 0, GemmCall{wk.Vct, rows, 1, wk.cRi2, n, Q, plain_map(n), IndexMap{1, 1, 0}, (int)rows, n, n, 0},
                    wk.splitk, wk.splitk_elems, err);                                   // Q = Q1 R2^-1
   if (nl < 0) return -1;
   launches += nl;
-  nl = launch_gemm(st, 0, GemmCall{wk.cL2, n, 1, wk.cR1, n, R, plain_map(n), IndexMap{1, 1, 0}, n, n, n, 0},
-                   wk.splitk, wk.splitk_elems, err);                                   // R = R2 R1 = L2^T R1
-  if (nl < 0) return -1;
-  launches += nl;
+  if (!fork_ok) {
+    nl = launch_gemm(st, 0, GemmCall{wk.cL2, n, 1, wk.cR1, n, R, plain_map(n), IndexMap{1, 1, 0}, n, n, n, 0},
+                     wk.splitk, wk.splitk_elems, err);                                 // R = R2 R1 = L2^T R1
+    if (nl < 0) return -1;
+    launches += nl;
+  } else if (cudaStreamWaitEvent(st, fb.e_join, 0) != cudaSuccess) { *err = cudaGetLastError(); return -1; }
   }
   *err = cudaGetLastError();
   if (*err != cudaSuccess) return -1;

@@ -45,6 +45,7 @@ int stage_qr(qrctm* h) {
     } else if (h->cap_aux) {
       fb = QrFallback{3, h->cap_aux, &h->g_qrfb};       // direct launches: prebuilt {condition; IF Householder} graph
     }
+    if (h->branch && h->stream) { fb.br = h->branch; fb.e_fork = h->ev_fork; fb.e_join = h->ev_join; }
     nl = qr_factor_blocked(h->stream, h->qr_path, h->m, h->chi, h->X, h->Q, h->R, h->qrwork, &e, fb);
   }
   if (nl < 0) return fail(h, QRCTM_ERR_CUDA, "qr", e);
