@@ -63,116 +63,137 @@ chol_inv_body(double* sm, const double* G, int n, double* Rup, double* Llow, dou
 
   // ---- load the lower block triangle (identity padding), accumulate ||G - I||_F^2 over the full matrix
   double dsum = 0.0;
-  for (int I = 0; I < nb; ++I) {
-    const int w = 16 * (I + 1), S = chol_stride(I);
-    double* blk = sm + chol_base(I);
-    for (int e = tid; e < 16 * w; e += CHOL_NT) {
-      const int r = e / w, j = e % w, i = 16 * I + r;
-      double v = (i == j) ? 1.0 : 0.0;
-      if (i < n && j < n) {
-        v = G[(long long)i * n + j];
-        if (j <= i) { const double t = v - (i == j ? 1.0 : 0.0); dsum += (i == j ? 1.0 : 2.0) * t * t; }
+  for (int i = warp; i < np; i += NW) {                 // one warp per row, lanes along the row; the row's (up to 7)
+    const int I = i >> 4, w = 16 * (I + 1);             // loads per lane are issued together
+    double* rowp = sm + chol_base(I) + (i & 15) * chol_stride(I);
+    double v[(CHOL_MAX_N + 31) / 32];
+#pragma unroll
+    for (int t = 0; t < (CHOL_MAX_N + 31) / 32; ++t) {
+      const int j = lane + 32 * t;
+      v[t] = (i == j) ? 1.0 : 0.0;
+      if (j < w && i < n && j < n) v[t] = G[(long long)i * n + j];
+    }
+#pragma unroll
+    for (int t = 0; t < (CHOL_MAX_N + 31) / 32; ++t) {
+      const int j = lane + 32 * t;
+      if (j < w) {
+        if (i < n && j <= i) { const double d = v[t] - (i == j ? 1.0 : 0.0); dsum += (i == j ? 1.0 : 2.0) * d * d; }
+        rowp[j] = v[t];
       }
-      blk[r * S + j] = v;
     }
   }
   dsum = block_sum(dsum, red);
   CHOL_TICK(0);
 
-  // ---- blocked right-looking Cholesky
-  for (int J = 0; J < nb; ++J) {
+  // ---- blocked right-looking Cholesky with a one-block look-ahead: after the panel of block column J, warp 0 updates
+  // only the next diagonal block and factors it at once (a chain of 16 dependent rsqrt, ~2 us) while the other warps do
+  // the rest of the trailing update, so the diagonal-block chain is off the critical path
+  auto factor_diag = [&](int J) {                       // warp 0
     const int SJ = chol_stride(J);
     double* dblk = sm + chol_base(J) + 16 * J;          // diagonal block (row stride SJ)
+    const int r = lane & 15;                            // lanes 16..31 mirror lanes 0..15 (keeps the shuffles full-warp)
+    double a[16];
+#pragma unroll
+    for (int c = 0; c < 16; ++c) a[c] = dblk[r * SJ + c];
+    int brk = 0;
+#pragma unroll
+    for (int c = 0; c < 16; ++c) {
+      double dcc = __shfl_sync(0xffffffffu, a[c], c);
+      if (!(dcc > 0.0) || !(dcc < INFINITY)) { brk = 1; dcc = 1.0; }
+      const double rs = rsqrt(dcc);
+      a[c] = (r == c) ? dcc * rs : a[c] * rs;            // l[r][c] for r >= c (rows above: unused)
+      if (lane == c) rd[16 * J + c] = rs;
+#pragma unroll
+      for (int c2 = c + 1; c2 < 16; ++c2) {
+        const double l2 = __shfl_sync(0xffffffffu, a[c], c2);       // l[c2][c]
+        a[c2] = fma(-a[c], l2, a[c2]);                               // a[r][c2] -= l[r][c] l[c2][c]   (used for r >= c2)
+      }
+    }
+    if (lane < 16) {
+#pragma unroll
+      for (int c = 0; c < 16; ++c) dblk[r * SJ + c] = (c <= r) ? a[c] : 0.0;
+    }
+    if (brk && lane == 0) bad = 1;
+  };
+  // C[I2][J2] -= L[I2][J] L[J2][J]^T, block number q of the trailing triangle (row by row), one warp
+  auto update_block = [&](int J, int q) {
+    int ri = (int)((sqrtf(8.0f * q + 1.0f) - 1.0f) * 0.5f);
+    while ((ri + 1) * (ri + 2) / 2 <= q) ++ri;
+    while (ri * (ri + 1) / 2 > q) --ri;
+    const int cj = q - ri * (ri + 1) / 2;
+    const int I2 = J + 1 + ri, J2 = J + 1 + cj;
+    const int SI = chol_stride(I2), S2 = chol_stride(J2);
+    const double* ap = sm + chol_base(I2) + lr * SI + 16 * J + lc;
+    const double* bp = sm + chol_base(J2) + lr * S2 + 16 * J + lc;
+    double* cp = sm + chol_base(I2) + lr * SI + 16 * J2 + 2 * lc;
+    double acc[2][2][2];
+#pragma unroll
+    for (int mi = 0; mi < 2; ++mi)
+#pragma unroll
+      for (int ni = 0; ni < 2; ++ni) {
+        const double2 t = *reinterpret_cast<const double2*>(cp + mi * 8 * SI + ni * 8);
+        acc[mi][ni][0] = t.x; acc[mi][ni][1] = t.y;
+      }
+#pragma unroll
+    for (int ks = 0; ks < 4; ++ks) {
+      const double a0 = -ap[ks * 4], a1 = -ap[8 * SI + ks * 4];
+      const double b0 = bp[ks * 4], b1 = bp[8 * S2 + ks * 4];
+      dmma884(acc[0][0][0], acc[0][0][1], a0, b0);
+      dmma884(acc[0][1][0], acc[0][1][1], a0, b1);
+      dmma884(acc[1][0][0], acc[1][0][1], a1, b0);
+      dmma884(acc[1][1][0], acc[1][1][1], a1, b1);
+    }
+#pragma unroll
+    for (int mi = 0; mi < 2; ++mi)
+#pragma unroll
+      for (int ni = 0; ni < 2; ++ni)
+        *reinterpret_cast<double2*>(cp + mi * 8 * SI + ni * 8) = make_double2(acc[mi][ni][0], acc[mi][ni][1]);
+  };
+  for (int J = -1; J < nb; ++J) {                       // J = -1: only the first diagonal block
+    if (J >= 0) {
+      const int SJ = chol_stride(J);
+      const double* dblk = sm + chol_base(J) + 16 * J;
+      // panel below the diagonal block: row i solves x L_JJ^T = a  (one thread per row)
+      const int nrow = np - 16 * (J + 1);
+      if (tid < nrow) {
+        const int i = 16 * (J + 1) + tid, I = i >> 4;
+        double* row = sm + chol_base(I) + (i & 15) * chol_stride(I) + 16 * J;
+        double x[16];
+#pragma unroll
+        for (int c = 0; c < 16; c += 2) { const double2 t = *reinterpret_cast<const double2*>(row + c); x[c] = t.x; x[c + 1] = t.y; }
+#pragma unroll
+        for (int c = 0; c < 16; ++c) {
+          x[c] *= rd[16 * J + c];
+#pragma unroll
+          for (int c2 = c + 1; c2 < 16; ++c2) x[c2] = fma(-x[c], dblk[c2 * SJ + c], x[c2]);
+        }
+#pragma unroll
+        for (int c = 0; c < 16; c += 2) *reinterpret_cast<double2*>(row + c) = make_double2(x[c], x[c + 1]);
+      }
+      __syncthreads();
+      CHOL_TICK(2);
+    }
+    const int nr = nb - J - 1, nt = J >= 0 ? nr * (nr + 1) / 2 : 0;
     if (warp == 0) {
-      const int r = lane & 15;                          // lanes 16..31 mirror lanes 0..15 (keeps the shuffles full-warp)
-      double a[16];
-#pragma unroll
-      for (int c = 0; c < 16; ++c) a[c] = dblk[r * SJ + c];
-      int brk = 0;
-#pragma unroll
-      for (int c = 0; c < 16; ++c) {
-        double dcc = __shfl_sync(0xffffffffu, a[c], c);
-        if (!(dcc > 0.0) || !(dcc < INFINITY)) { brk = 1; dcc = 1.0; }
-        const double rs = rsqrt(dcc);
-        a[c] = (r == c) ? dcc * rs : a[c] * rs;          // l[r][c] for r >= c (rows above: unused)
-        if (lane == c) rd[16 * J + c] = rs;
-#pragma unroll
-        for (int c2 = c + 1; c2 < 16; ++c2) {
-          const double l2 = __shfl_sync(0xffffffffu, a[c], c2);     // l[c2][c]
-          a[c2] = fma(-a[c], l2, a[c2]);                             // a[r][c2] -= l[r][c] l[c2][c]   (used for r >= c2)
-        }
+      if (J < 0 || nt > 0) {
+        if (J >= 0) update_block(J, 0);
+        __syncwarp();
+        factor_diag(J + 1);
       }
-      if (lane < 16) {
-#pragma unroll
-        for (int c = 0; c < 16; ++c) dblk[r * SJ + c] = (c <= r) ? a[c] : 0.0;
-      }
-      if (brk && lane == 0) bad = 1;
-    }
-    __syncthreads();
-    CHOL_TICK(1);
-    // panel below the diagonal block: row i solves x L_JJ^T = a  (one thread per row)
-    const int nrow = np - 16 * (J + 1);
-    if (tid < nrow) {
-      const int i = 16 * (J + 1) + tid, I = i >> 4;
-      double* row = sm + chol_base(I) + (i & 15) * chol_stride(I) + 16 * J;
-      double x[16];
-#pragma unroll
-      for (int c = 0; c < 16; c += 2) { const double2 t = *reinterpret_cast<const double2*>(row + c); x[c] = t.x; x[c + 1] = t.y; }
-#pragma unroll
-      for (int c = 0; c < 16; ++c) {
-        x[c] *= rd[16 * J + c];
-#pragma unroll
-        for (int c2 = c + 1; c2 < 16; ++c2) x[c2] = fma(-x[c], dblk[c2 * SJ + c], x[c2]);
-      }
-#pragma unroll
-      for (int c = 0; c < 16; c += 2) *reinterpret_cast<double2*>(row + c) = make_double2(x[c], x[c + 1]);
-    }
-    __syncthreads();
-    CHOL_TICK(2);
-    // trailing update: C[I2][J2] -= L[I2][J] L[J2][J]^T for J < J2 <= I2 < nb, one 16 x 16 block per warp
-    const int nr = nb - J - 1, nt = nr * (nr + 1) / 2;
-    for (int q = warp; q < nt; q += NW) {
-      int ri = (int)((sqrtf(8.0f * q + 1.0f) - 1.0f) * 0.5f);
-      while ((ri + 1) * (ri + 2) / 2 <= q) ++ri;
-      while (ri * (ri + 1) / 2 > q) --ri;
-      const int cj = q - ri * (ri + 1) / 2;
-      const int I2 = J + 1 + ri, J2 = J + 1 + cj;
-      const int SI = chol_stride(I2), S2 = chol_stride(J2);
-      const double* ap = sm + chol_base(I2) + lr * SI + 16 * J + lc;
-      const double* bp = sm + chol_base(J2) + lr * S2 + 16 * J + lc;
-      double* cp = sm + chol_base(I2) + lr * SI + 16 * J2 + 2 * lc;
-      double acc[2][2][2];
-#pragma unroll
-      for (int mi = 0; mi < 2; ++mi)
-#pragma unroll
-        for (int ni = 0; ni < 2; ++ni) {
-          const double2 t = *reinterpret_cast<const double2*>(cp + mi * 8 * SI + ni * 8);
-          acc[mi][ni][0] = t.x; acc[mi][ni][1] = t.y;
-        }
-#pragma unroll
-      for (int ks = 0; ks < 4; ++ks) {
-        const double a0 = -ap[ks * 4], a1 = -ap[8 * SI + ks * 4];
-        const double b0 = bp[ks * 4], b1 = bp[8 * S2 + ks * 4];
-        dmma884(acc[0][0][0], acc[0][0][1], a0, b0);
-        dmma884(acc[0][1][0], acc[0][1][1], a0, b1);
-        dmma884(acc[1][0][0], acc[1][0][1], a1, b0);
-        dmma884(acc[1][1][0], acc[1][1][1], a1, b1);
-      }
-#pragma unroll
-      for (int mi = 0; mi < 2; ++mi)
-#pragma unroll
-        for (int ni = 0; ni < 2; ++ni)
-          *reinterpret_cast<double2*>(cp + mi * 8 * SI + ni * 8) = make_double2(acc[mi][ni][0], acc[mi][ni][1]);
+    } else {
+      for (int q = warp; q < nt; q += NW - 1) update_block(J, q);
     }
     __syncthreads();
     CHOL_TICK(3);
   }
 
   // ---- write L (lower) and R = L^T (upper)
-  for (int idx = tid; idx < n * n; idx += CHOL_NT) {
-    const int i = idx / n, j = idx % n;
-    if (Llow) Llow[idx] = j <= i ? sm[chol_base(i >> 4) + (i & 15) * chol_stride(i >> 4) + j] : 0.0;
-    if (Rup) Rup[idx] = i <= j ? sm[chol_base(j >> 4) + (j & 15) * chol_stride(j >> 4) + i] : 0.0;
+  for (int i = warp; i < n; i += NW) {                  // one warp per row, coalesced stores; R[i][j] = L[j][i]
+    const double* Li = sm + chol_base(i >> 4) + (i & 15) * chol_stride(i >> 4);
+    for (int j = lane; j < n; j += 32) {
+      if (Llow) Llow[i * n + j] = j <= i ? Li[j] : 0.0;
+      if (Rup) Rup[i * n + j] = j >= i ? sm[chol_base(j >> 4) + (j & 15) * chol_stride(j >> 4) + i] : 0.0;
+    }
   }
   if (tid == 0) {
     status[0] = bad;
@@ -272,10 +293,9 @@ chol_inv_body(double* sm, const double* G, int n, double* Rup, double* Llow, dou
   __syncthreads();
   CHOL_TICK(6);
   // ---- R^-1 = M^T (upper)
-  for (int idx = tid; idx < n * n; idx += CHOL_NT) {
-    const int r = idx / n, c = idx % n;
-    Rinv[idx] = r <= c ? sm[chol_base(c >> 4) + (c & 15) * chol_stride(c >> 4) + r] : 0.0;
-  }
+  for (int r = warp; r < n; r += NW)                    // R^-1[r][c] = M[c][r], M = L^-1
+    for (int c = lane; c < n; c += 32)
+      Rinv[r * n + c] = c >= r ? sm[chol_base(c >> 4) + (c & 15) * chol_stride(c >> 4) + r] : 0.0;
   if (prof) {
     __syncthreads();
     CHOL_TICK(7);
