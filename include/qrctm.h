@@ -80,10 +80,11 @@ enum {
                                 the per-stage NVTX ranges for profilers */
   QRCTM_OPT_K8_PATH = 10,    /* K8 tridiagonalisation for chi <= 216: 0 [default] = the thread-per-column kernel (un-
                                 normalised reflectors, 2 barriers per step), 1 = the round-1 kernel (for cross-checks) */
-  QRCTM_OPT_SMALL_PATH = 11, /* 0 [default] = problems whose whole working set fits one CTA's shared memory (2 m^2 + D^8 +
-                                5 m chi doubles <= ~200 KB, e.g. D = 2, chi <= 24; cfg0) run K1..K6 as ONE kernel and K7
-                                as one more (plain DFMA loops, Householder QR) when the default modes are selected;
-                                1 = always the general multi-kernel path */
+  QRCTM_OPT_SMALL_PATH = 11, /* 0 [default] = problems with chi <= 8 whose whole working set fits one CTA's shared memory
+                                (2 m^2 + D^8 + 5 m chi doubles <= ~200 KB; cfg0) run K1..K6 as ONE kernel and K7 as one
+                                more (plain DFMA loops, Householder QR) when the default modes are selected;
+                                1 = always the general multi-kernel path; 2 = the one-kernel path whenever the working
+                                set fits (e.g. D = 2, chi <= 24), also where the general path was measured faster */
   QRCTM_OPT_ABSORB_MODE = 9  /* K4: 0 [default] = contract with the explicit double-layer tensor a (2 chi^2 D^8 flops),
                                 1 = layered: contract with the ket and the bra copy of A in turn (4 d chi^2 D^6
                                 flops; same T' up to rounding; needs even chi, otherwise mode 0 is used),

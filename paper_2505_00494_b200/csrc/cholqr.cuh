@@ -100,14 +100,17 @@ chol_inv_body(double* sm, const double* G, int n, double* Rup, double* Llow, dou
     for (int c = 0; c < 16; ++c) {
       double dcc = __shfl_sync(0xffffffffu, a[c], c);
       if (!(dcc > 0.0) || !(dcc < INFINITY)) { brk = 1; dcc = 1.0; }
+      // the trailing columns take the UNSCALED column c times 1 / d_cc, so that their shuffles and products do not
+      // wait for the reciprocal square root: the dependent chain per column is shuffle -> rsqrt -> square -> one FMA
+      double t[16];
+#pragma unroll
+      for (int c2 = c + 1; c2 < 16; ++c2) t[c2] = a[c] * __shfl_sync(0xffffffffu, a[c], c2);   // a[r][c] a[c2][c]
       const double rs = rsqrt(dcc);
+      const double rs2 = rs * rs;
+#pragma unroll
+      for (int c2 = c + 1; c2 < 16; ++c2) a[c2] = fma(-t[c2], rs2, a[c2]);   // a[r][c2] -= l[r][c] l[c2][c]   (used for r >= c2)
       a[c] = (r == c) ? dcc * rs : a[c] * rs;            // l[r][c] for r >= c (rows above: unused)
       if (lane == c) rd[16 * J + c] = rs;
-#pragma unroll
-      for (int c2 = c + 1; c2 < 16; ++c2) {
-        const double l2 = __shfl_sync(0xffffffffu, a[c], c2);       // l[c2][c]
-        a[c2] = fma(-a[c], l2, a[c2]);                               // a[r][c2] -= l[r][c] l[c2][c]   (used for r >= c2)
-      }
     }
     if (lane < 16) {
 #pragma unroll

@@ -195,6 +195,15 @@ gemm_f64_dmma(GemmArgs p) {
     if (s < nkt) load_stage(s, s);
     cp_async_commit();
   }
+  // output offsets of the tile's rows and columns, one map evaluation per thread while the first copies are in flight
+  // (a map costs two integer divisions; per fragment element they made the epilogue of a three-k-tile GEMM several
+  // microseconds long)
+  __shared__ long long row_off[BM], col_off[BN];
+  for (int t = tid; t < BM + BN; t += NT) {
+    if (t < BM) row_off[t] = (m0 + t < p.M) ? p.ro(m0 + t) : 0;
+    else col_off[t - BM] = (n0 + t - BM < p.N) ? p.co(n0 + t - BM) : 0;
+  }
+  __syncthreads();
 
   for (int kt = 0; kt < nkt; ++kt) {
     cp_async_wait<STAGES - 2>();
@@ -231,14 +240,14 @@ gemm_f64_dmma(GemmArgs p) {
   for (int i = 0; i < FM; ++i) {
     int r = m0 + wm0 + i * 8 + lr;
     if (r >= p.M) continue;
-    long long roff = p.ro(r);
+    long long roff = row_off[wm0 + i * 8 + lr];
 #pragma unroll
     for (int j = 0; j < FN; ++j) {
 #pragma unroll
       for (int e = 0; e < 2; ++e) {
         int c = n0 + wn0 + j * 8 + 2 * lc + e;
         if (c < p.N) {
-          long long off = roff + p.co(c);
+          long long off = roff + col_off[wn0 + j * 8 + 2 * lc + e];
           double v = acc[i][j][e];
           if (p.mode == 1) v = out[off] - v;
           else if (p.mode == 2) v = out[off] + v;

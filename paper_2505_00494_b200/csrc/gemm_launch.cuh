@@ -302,7 +302,7 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
     case 5: *err = launch_cfg_ws<128, 56, 32, 56, 3>(st, g, splits, sk); break;
     case 6: *err = launch_cfg_ws<80, 208, 16, 104, 3>(st, g, splits, sk); break;
     case 1: *err = launch_cfg<128, 128, 64, 32, 4>(st, g, splits); break;
-    default: *err = launch_cfg<64, 64, 32, 32, 4>(st, g, splits); break;
+    default: *err = launch_cfg<64, 64, 32, 16, 4>(st, g, splits); break;
   }
   if (*err != cudaSuccess) return -1;
   ++launched;

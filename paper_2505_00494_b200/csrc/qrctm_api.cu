@@ -56,6 +56,7 @@ struct qrctm {
   int corner_mode, symmetrize, check_every, gemm_path, time_stages, qr_path, absorb_mode;
   int k8_old;             // 1: K8 on the round-1 tridiagonalisation kernel (QRCTM_OPT_K8_PATH, for cross-checks)
   int small_off;          // 1: never use the whole-iteration kernels for tiny problems (QRCTM_OPT_SMALL_PATH)
+  int small_force;        // 1: use them whenever the working set fits (QRCTM_OPT_SMALL_PATH = 2), not only for chi <= 8
   int small_smem;         // opt-in shared memory available to them (0: not queried yet, -1: unavailable)
   long long launches;
   cudaEvent_t ev[QRCTM_NSTAGE + 2];
@@ -540,7 +541,7 @@ int qrctm_set_option(qrctm_t* h, int key, int value) {
     case QRCTM_OPT_USE_GRAPH:   if (value != 0 && value != 1) break; h->use_graph = value; return QRCTM_OK;
     case QRCTM_OPT_TIME_STAGES: if (value != 0 && value != 1) break; h->time_stages = value; return QRCTM_OK;
     case QRCTM_OPT_K8_PATH:     if (value != 0 && value != 1) break; h->k8_old = value; return QRCTM_OK;
-    case QRCTM_OPT_SMALL_PATH:  if (value != 0 && value != 1) break; h->small_off = value; return QRCTM_OK;
+    case QRCTM_OPT_SMALL_PATH:  if (value < 0 || value > 2) break; h->small_off = value == 1; h->small_force = value == 2; return QRCTM_OK;
     default: break;
   }
   return fail(h, QRCTM_ERR_INVALID_ARG, "bad option key/value");

@@ -266,6 +266,10 @@ int stage_spectrum(qrctm* h, double* s_out, int update_prev, cudaStream_t st) {
 // Tiny problems: K1..K6 in one CTA (small_step.cuh).  Only with the default modes and when no per-stage events are wanted.
 bool small_ok(qrctm* h) {
   if (h->small_off || h->gemm_path != 0 || h->corner_mode != 0 || h->absorb_mode == 1 || h->qr_path != 0) return false;
+  // one CTA walks the chi dependent Householder columns and everything else of the step; from chi ~ 10 the general path
+  // (CholeskyQR2 cluster kernel, small DMMA GEMMs, K8 beside the next step) is faster: measured per step at
+  // (D, chi) = (2, 16) 98 us against 87, (3, 10) 96 / 82, (2, 24) 108 / 108, but (3, 7) 57 / 74, (2, 8) 47 / 60
+  if (!h->small_force && h->chi > 8) return false;
   if (h->small_smem == 0) {
     int dev = 0, optin = 0;
     cudaGetDevice(&dev);

@@ -540,13 +540,14 @@ def test_layered_absorption_matches_oracle_and_explicit(d, D, chi, seed, path):
 
 @pytest.mark.parametrize("d,D,chi,seed", [(2, 2, 8, 0), (3, 2, 5, 7), (2, 3, 7, 8), (2, 2, 20, 4), (2, 1, 3, 9)])
 def test_small_whole_iteration_kernels_match_the_general_path(d, D, chi, seed):
-    """Tiny problems run K1..K6 as one kernel, K7 as one and K8 as one (QRCTM_OPT_SMALL_PATH = 0, the default): same
-    step as the general multi-kernel path to rounding, same iteration count and delta history, far fewer launches."""
+    """Tiny problems run K1..K6 as one kernel, K7 as one and K8 as one (QRCTM_OPT_SMALL_PATH = 2; the default takes
+    this path for chi <= 8): same step as the general multi-kernel path to rounding, same iteration count and delta
+    history, far fewer launches."""
     A, C0, T0 = gen_config(d, D, chi, seed)
     out = {}
     for off in (0, 1):
         h = pkg.QRCTM(d, D, chi)
-        h.set_option(pkg.OPT_SMALL_PATH, off)
+        h.set_option(pkg.OPT_SMALL_PATH, 1 if off else 2)
         h.set_A(A); h.set_env(C0, T0)
         h.step()
         Q, R = h.get_qr()
@@ -562,6 +563,20 @@ def test_small_whole_iteration_kernels_match_the_general_path(d, D, chi, seed):
     assert rel(s[3][0], g[3][0]) < 1e-10 and rel(s[3][1], g[3][1]) < 1e-10
     assert np.max(np.abs(s[4] - g[4])) < 1e-11 and abs(s[5] - g[5]) < 1e-10
     assert np.allclose(s[7][:, 1:], g[7][:, 1:], rtol=1e-9) and s[6] * 3 < g[6]
+
+
+def test_small_path_default_is_by_measured_crossover():
+    """QRCTM_OPT_SMALL_PATH = 0: the one-kernel path up to chi = 8, the general path above (where it is faster)."""
+    for chi, small in ((8, True), (16, False)):
+        A, C0, T0 = gen_config(2, 2, chi, 1)
+        h = pkg.QRCTM(2, 2, chi)
+        h.set_A(A); h.set_env(C0, T0)
+        h.run(3, -1.0)
+        n0 = h.launch_count()
+        h.run(10, -1.0)
+        per_step = (h.launch_count() - n0) / 10
+        h.close()
+        assert (per_step <= 3.5) == small, (chi, per_step)
 
 
 @pytest.mark.parametrize("check_every", [2, 3, 7])
