@@ -114,7 +114,7 @@ long long eigh_top(cudaStream_t st, int n, int k, double* W, double* lam, double
   }
   launches += eigh_tridiagonalise(st, n, W, wk);
   const int nc = 2 * k < n ? 2 * k : n;            // candidates: the k smallest and the k largest eigenvalues
-  multisect_kernel<<<(nc + 7) / 8, 256, sizeof(double) * (2 * (size_t)n + 40), st>>>(wk.d, wk.e, n, wk.eig, k);
+  multisect_kernel<<<(nc + 3) / 4, 128, sizeof(double) * (2 * (size_t)n + 40), st>>>(wk.d, wk.e, n, wk.eig, k);
   eigh_select_kernel<<<(nc + 255) / 256, 256, 0, st>>>(wk.eig, nc, k, lam, wk.d, wk.e, n, wk.scal);
   eigh_invit_kernel<<<(k + 31) / 32, 32, 0, st>>>(wk.d, wk.e, n, lam, k, wk.scal, wk.Z, wk.U0, wk.U1, wk.U2, 3);
   launches += 4;

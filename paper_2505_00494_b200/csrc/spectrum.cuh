@@ -504,30 +504,46 @@ tridiag_smem2_kernel(const double* __restrict__ Cmat, int n, double* __restrict_
 // an exact power of two every 4 rows (magnitudes then stay within 2^+-600 of 1).  d_i - x == 0 is replaced by 2^-100
 // (a perturbation of x far below rounding at this scaling); an exact zero minor counts as a sign change.
 __device__ __forceinline__ int sturm_count_minors(const double2* __restrict__ de, int n, double x) {
+  // Few instructions per row (the count is issue-bound as soon as two warps share a scheduler): the sign changes are
+  // counted on the sign words (an exact zero counts as positive: the row after it has the sign opposite to the row
+  // before it, so a zero adds one change whichever sign it is given); d_i - x = 0 is moved to 2^-100 by an addition
+  // instead of a compare-and-select, so that a decoupled row (e = 0) cannot zero the sequence.
   double p0 = 1.0;
-  double t = de[0].x - x;
-  t = (t == 0.0) ? 0x1p-100 : t;
-  double p1 = t;
-  int neg1 = p1 < 0.0;                         // sign of p_{i-1} as used by the count (zero: opposite to its predecessor)
-  int cnt = neg1;
+  double p1 = (de[0].x - x) + 0x1p-100;
+  int sprev = __double2hiint(p1);
+  int cnt = (int)((unsigned)sprev >> 31);
   int i = 1;
-  for (; i + 4 <= n; i += 4) {
+  // rows in groups of eight: the group's (d_i - x, -e_i^2) are formed ahead of the dependent chain (one FMA per row),
+  // and the next group's rows are fetched from shared memory before the chain of the current one starts
+  double2 w[8];
+  if (i + 8 <= n) {
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
-      const double2 v = de[i + u];
-      double tt = v.x - x;
-      tt = (tt == 0.0) ? 0x1p-100 : tt;
-      const double pn = fma(tt, p1, -v.y * p0);
-      const int negn = (pn == 0.0) ? !neg1 : (pn < 0.0);
-      cnt += negn != neg1;
-      neg1 = negn; p0 = p1; p1 = pn;
+    for (int u = 0; u < 8; ++u) w[u] = de[i + u];
+  }
+  for (; i + 8 <= n; i += 8) {
+    double tt[8], ne[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) { tt[u] = (w[u].x - x) + 0x1p-100; ne[u] = -w[u].y; }
+    if (i + 16 <= n) {
+#pragma unroll
+      for (int u = 0; u < 8; ++u) w[u] = de[i + 8 + u];
     }
-    // renormalise by 2^-e, e = exponent of max(|p0|, |p1|)
-    const double m = fmax(fabs(p0), fabs(p1));
-    const int e = ((__double2hiint(m) >> 20) & 0x7ff) - 1023;
-    if (e > 64 || e < -64) {
-      if (m == 0.0) { p1 = neg1 ? -1.0 : 1.0; }                         // decoupled block: restart the sequence
+    asm volatile("" ::: "memory");               // keeps the loads above ahead of the chain below
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const double pn = fma(tt[u], p1, ne[u] * p0);
+      const int sn = __double2hiint(pn);
+      cnt += (int)((unsigned)(sn ^ sprev) >> 31);
+      sprev = sn; p0 = p1; p1 = pn;
+    }
+    // renormalise by 2^-e, e = the larger exponent of p0, p1 (growth per row <= 3, shrinkage per row can be ~1e-17
+    // in a block of tiny rows: eight rows stay far from overflow and underflow); integer test on the exponent fields
+    const int e0 = __double2hiint(p0) & 0x7ff00000, e1 = __double2hiint(p1) & 0x7ff00000;
+    const int em = e0 > e1 ? e0 : e1;
+    if ((unsigned)(em - ((1023 - 64) << 20)) > (unsigned)(128 << 20)) {
+      if (em == 0) { p0 = 0.0; p1 = sprev < 0 ? -1.0 : 1.0; }           // both zero (or denormal): decoupled block, restart
       else {
+        const int e = (em >> 20) - 1023;
         const int ee = e > 1000 ? 1000 : (e < -1000 ? -1000 : e);
         const double sc = __hiloint2double((1023 - ee) << 20, 0);
         p0 *= sc; p1 *= sc;
@@ -536,12 +552,11 @@ __device__ __forceinline__ int sturm_count_minors(const double2* __restrict__ de
   }
   for (; i < n; ++i) {
     const double2 v = de[i];
-    double tt = v.x - x;
-    tt = (tt == 0.0) ? 0x1p-100 : tt;
+    const double tt = (v.x - x) + 0x1p-100;
     const double pn = fma(tt, p1, -v.y * p0);
-    const int negn = (pn == 0.0) ? !neg1 : (pn < 0.0);
-    cnt += negn != neg1;
-    neg1 = negn; p0 = p1; p1 = pn;
+    const int sn = __double2hiint(pn);
+    cnt += (int)((unsigned)(sn ^ sprev) >> 31);
+    sprev = sn; p0 = p1; p1 = pn;
   }
   return cnt;
 }
@@ -582,10 +597,14 @@ __device__ __forceinline__ void multisect_setup(const double* dvec, const double
 }
 
 // One warp: eigenvalue number idx (ascending) of the scaled problem by 33-way multisection.
+// Stops when the bracket is narrower than 2^-54 of the spectrum's bound (the scaled problem has |lambda| <= 1): the
+// tridiagonalisation's own backward error is n eps ||C||, so resolving the tiny eigenvalues to full RELATIVE accuracy
+// (up to twice as many rounds) buys nothing for s, delta or the inverse-iteration shifts.
 __device__ __forceinline__ double multisect_warp(const double2* de, int n, int idx, double glo, double ghi) {
   const int lane = threadIdx.x & 31;
   double a = glo, b = ghi;
   for (int it = 0; it < 64; ++it) {
+    if (b - a <= 0x1p-54) break;
     const double h = (b - a) / 33.0;
     const double x = a + (lane + 1) * h;
     const bool inside = x > a && x < b;
@@ -613,7 +632,7 @@ multisect_kernel(const double* __restrict__ dvec, const double* __restrict__ eve
   multisect_setup(dvec, evec, n, de, red, glo, ghi, isc);
   // ke > 0 (and 2 ke < n): only the ke smallest and the ke largest eigenvalues, written compactly
   // (slot c < ke: eigenvalue c; slot c >= ke: eigenvalue n - 2 ke + c) -- the eigen step's candidates.
-  const int slot = blockIdx.x * 8 + warp;
+  const int slot = blockIdx.x * (blockDim.x >> 5) + warp;
   const bool part = ke > 0 && 2 * ke < n;
   if (slot >= (part ? 2 * ke : n)) return;
   const int idx = (part && slot >= ke) ? n - 2 * ke + slot : slot;

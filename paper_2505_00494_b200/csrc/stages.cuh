@@ -225,13 +225,13 @@ int stage_spectrum(qrctm* h, double* s_out, int update_prev, cudaStream_t st) {
       attr2 = true;
     }
     tridiag_smem2_kernel<<<1, TRI2_NT, tri2_smem_bytes(chi), st>>>(h->C, chi, h->dvec, h->evec, nullptr);
-    multisect_kernel<<<(chi + 7) / 8, 256, sizeof(double) * (2 * chi + 40), st>>>(h->dvec, h->evec, chi, h->eig);
+    multisect_kernel<<<(chi + 3) / 4, 128, sizeof(double) * (2 * chi + 40), st>>>(h->dvec, h->evec, chi, h->eig);
     spectrum_finalize_kernel<<<1, nt, sizeof(double) * (chi + 40), st>>>(h->eig, chi, s_out, h->s_prev, h->delta,
                                                                         update_prev, h->hist, h->flag + 1);
     h->launches += 3;
   } else if (tri_bytes <= (size_t)max_smem && chi <= 1024) {
     tridiag_smem_kernel<<<1, 1024, tri_bytes, st>>>(h->C, chi, h->dvec, h->evec);
-    multisect_kernel<<<(chi + 7) / 8, 256, sizeof(double) * (2 * chi + 40), st>>>(h->dvec, h->evec, chi,
+    multisect_kernel<<<(chi + 3) / 4, 128, sizeof(double) * (2 * chi + 40), st>>>(h->dvec, h->evec, chi,
                                                                                          h->eig);
     spectrum_finalize_kernel<<<1, nt, sizeof(double) * (chi + 40), st>>>(h->eig, chi, s_out, h->s_prev,
                                                                                  h->delta, update_prev, h->hist, h->flag + 1);
@@ -248,7 +248,7 @@ int stage_spectrum(qrctm* h, double* s_out, int update_prev, cudaStream_t st) {
     eigh_layout(chi, 1, static_cast<char*>(h->k8work), &wk);
     CU(h, cudaMemcpyAsync(h->Wc, h->C, sizeof(double) * chi * chi, cudaMemcpyDeviceToDevice, st));
     h->launches += eigh_tridiagonalise(st, chi, h->Wc, wk);
-    multisect_kernel<<<(chi + 7) / 8, 256, sizeof(double) * (2 * chi + 40), st>>>(wk.d, wk.e, chi, h->eig);
+    multisect_kernel<<<(chi + 3) / 4, 128, sizeof(double) * (2 * chi + 40), st>>>(wk.d, wk.e, chi, h->eig);
     spectrum_finalize_kernel<<<1, nt, sizeof(double) * (chi + 40), st>>>(h->eig, chi, s_out, h->s_prev, h->delta,
                                                                         update_prev, h->hist, h->flag + 1);
     h->launches += 2;
