@@ -282,7 +282,7 @@ tridiag_smem2_body(double* tsm, const double* Cmat, int n, double* dvec, double*
   double* red = part + TRI2_MAXSUB * n;                         // 8: per-warp partial sums of p.u
   double* sc = red + 8;                                         // [0] gamma (0: nothing to eliminate)
   double* L = red + 16;                                         // n(n+1)/2
-  __shared__ int tab[32];
+  __shared__ int tab[2][32];                                    // warp table of phase U, rebuilt every 8 steps (two copies)
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   long long tp[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tc = 0;
 #define TRI_TICK(i) do { if (prof && tid == 0) { const long long t_ = clock64(); tp[i] += t_ - tc; tc = t_; } } while (0)
@@ -296,65 +296,75 @@ tridiag_smem2_body(double* tsm, const double* Cmat, int n, double* dvec, double*
   __syncthreads();
   TRI_TICK(0);
   const int ncgt = (n + 31) >> 5;
+  // ---- R (warp 0): reflector of column k (rows k+1 .. n-1) from the column left in up0 + (k & 1) n, and every 8 steps
+  // the warp table of phase U.  Runs one step AHEAD: R(k+1) beside the rank-2 update of step k (U2 below), so the scalar
+  // chain (norm -> rsqrt -> reciprocal, ~1 us) is off the critical path.
+  auto reflector = [&](int k) {
+    double2* up = up0 + (k & 1) * n;
+    const int c0 = (k + 1) >> 5, ncg = ncgt - c0;
+    double acc = 0.0;
+    for (int i = k + 2 + lane; i < n; i += 32) { const double x = up[i].x; acc = fma(x, x, acc); }
+    const double tail2 = warp_sum(acc);
+    const double alpha = up[k + 1].x;
+    __syncwarp();
+    // nothing to eliminate: H = I.  Entries below 1e-140 in magnitude are dropped rather than eliminated: gamma ~
+    // 1 / tail2 would overflow, and the perturbation is 120 orders below rounding for ||C|| ~ 1
+    if (!(tail2 > 1e-280)) {
+      if (lane == 0) { dvec[k] = L[tri_off(k) + k]; evec[k + 1] = alpha; sc[0] = 0.0; }
+    } else {
+      const double s2 = fma(alpha, alpha, tail2);
+      const double sigma = s2 * rsqrt(s2);                     // 1-2 ulp: only perturbs e_{k+1} at rounding level
+      const double beta = alpha >= 0.0 ? -sigma : sigma;
+      const double gamma = __drcp_rn(fma(-alpha, beta, s2));   // 1 / (beta (beta - alpha)),  beta^2 = s2
+      if (lane == 0) {
+        dvec[k] = L[tri_off(k) + k]; evec[k + 1] = beta; sc[0] = gamma;
+        up[k + 1].x = alpha - beta;                            // u_{k+1}: H = I - gamma u u^T, u = x - beta e_1
+      }
+    }
+    // every 8 steps: deal warps 1..31 out to the active column groups for phase U2, in proportion to the groups'
+    // heights h_c = n - max(32 c, k+1) (a table that is up to 7 steps old only balances slightly worse: rows and
+    // columns that have left the active block are skipped by the lanes themselves)
+    if ((k & 7) == 0) {
+      const int c = c0 + lane;                                  // lane <-> active column group
+      const int h = (lane < ncg) ? n - ((c << 5) > k + 1 ? (c << 5) : k + 1) : 0;
+      int cum = h;
+#pragma unroll
+      for (int o = 1; o < 8; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, cum, o); if (lane >= o) cum += v; }
+      const int H = __shfl_sync(0xffffffffu, cum, ncg - 1);
+      int B = (lane == ncg - 1) ? 31 : (int)((float)cum * __fdividef(31.0f, (float)H));
+      int m = B - lane;                                         // at least one warp per group: B_c >= B_c' + (c - c')
+#pragma unroll
+      for (int o = 1; o < 8; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, m, o); if (lane >= o) m = m > v ? m : v; }
+      B = m + lane;
+      const int room = 31 - (ncg - 1 - lane);                   // ... and one left for every later group
+      B = B < room ? B : room;
+      int t = 0xff;
+      for (int cc = 0; cc < ncg; ++cc) {
+        const int hi = __shfl_sync(0xffffffffu, B, cc), lo = cc ? __shfl_sync(0xffffffffu, B, cc - 1) : 0;
+        const int hh = __shfl_sync(0xffffffffu, h, cc);
+        if (lane >= lo && lane < hi) {
+          const int cnt = hi - lo;
+          t = (c0 + cc) | ((lane - lo) << 8) | (((hh + cnt - 1) / cnt) << 16);        // group, sub, rows per warp
+        }
+      }
+      tab[(k >> 3) & 1][lane] = t;                              // slot s <-> warp s + 1
+    }
+  };
+  if (n > 2) {
+    if (warp == 0) reflector(0);
+    __syncthreads();
+  }
+  TRI_TICK(1);
   for (int k = 0; k < n - 2; ++k) {
     double2* up = up0 + (k & 1) * n;
     double2* upn = up0 + ((k + 1) & 1) * n;
     const int c0 = (k + 1) >> 5, ncg = ncgt - c0;
-    // ---- R (warp 0): reflector of column k (rows k+1 .. n-1), warp table of phase U
-    if (warp == 0) {
-      double acc = 0.0;
-      for (int i = k + 2 + lane; i < n; i += 32) { const double x = up[i].x; acc = fma(x, x, acc); }
-      const double tail2 = warp_sum(acc);
-      const double alpha = up[k + 1].x;
-      __syncwarp();
-      // nothing to eliminate: H = I.  Entries below 1e-140 in magnitude are dropped rather than eliminated: gamma ~
-      // 1 / tail2 would overflow, and the perturbation is 120 orders below rounding for ||C|| ~ 1
-      if (!(tail2 > 1e-280)) {
-        if (lane == 0) { dvec[k] = L[tri_off(k) + k]; evec[k + 1] = alpha; sc[0] = 0.0; }
-      } else {
-        const double s2 = fma(alpha, alpha, tail2);
-        const double sigma = s2 * rsqrt(s2);                     // 1-2 ulp: only perturbs e_{k+1} at rounding level
-        const double beta = alpha >= 0.0 ? -sigma : sigma;
-        const double gamma = __drcp_rn(fma(-alpha, beta, s2));   // 1 / (beta (beta - alpha)),  beta^2 = s2
-        if (lane == 0) {
-          dvec[k] = L[tri_off(k) + k]; evec[k + 1] = beta; sc[0] = gamma;
-          up[k + 1].x = alpha - beta;                            // u_{k+1}: H = I - gamma u u^T, u = x - beta e_1
-        }
-      }
-      // every 8 steps: deal the 32 warps out to the active column groups for phase U, in proportion to the groups'
-      // heights h_c = n - max(32 c, k+1) (a table that is up to 7 steps old only balances slightly worse: rows and
-      // columns that have left the active block are skipped by the lanes themselves)
-      if ((k & 7) == 0) {
-        const int c = c0 + lane;                                  // lane <-> active column group
-        const int h = (lane < ncg) ? n - ((c << 5) > k + 1 ? (c << 5) : k + 1) : 0;
-        int cum = h;
-#pragma unroll
-        for (int o = 1; o < 8; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, cum, o); if (lane >= o) cum += v; }
-        const int H = __shfl_sync(0xffffffffu, cum, ncg - 1);
-        int B = (lane == ncg - 1) ? 32 : (int)((float)cum * __fdividef(32.0f, (float)H));
-        int m = B - lane;                                         // at least one warp per group: B_c >= B_c' + (c - c')
-#pragma unroll
-        for (int o = 1; o < 8; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, m, o); if (lane >= o) m = m > v ? m : v; }
-        B = m + lane;
-        const int room = 32 - (ncg - 1 - lane);                   // ... and one left for every later group
-        B = B < room ? B : room;
-        int t = 0xff;
-        for (int cc = 0; cc < ncg; ++cc) {
-          const int hi = __shfl_sync(0xffffffffu, B, cc), lo = cc ? __shfl_sync(0xffffffffu, B, cc - 1) : 0;
-          const int hh = __shfl_sync(0xffffffffu, h, cc);
-          if (lane >= lo && lane < hi) {
-            const int cnt = hi - lo;
-            t = (c0 + cc) | ((lane - lo) << 8) | (((hh + cnt - 1) / cnt) << 16);        // group, sub, rows per warp
-          }
-        }
-        tab[lane] = t;
-      }
-    }
-    TRI_TICK(1);
-    __syncthreads();
+    const bool more = k + 1 < n - 2;                             // there is a next step
     const double gamma = sc[0];
     if (gamma == 0.0) {
       for (int i = k + 2 + tid; i < n; i += TRI2_NT) upn[i].x = L[tri_off(i) + k + 1];
+      __syncthreads();
+      if (more && warp == 0) reflector(k + 1);
       __syncthreads();
       continue;
     }
@@ -427,25 +437,41 @@ tridiag_smem2_body(double* tsm, const double* Cmat, int n, double* dvec, double*
     TRI_TICK(3);
     __syncthreads();
     // ---- U: A -= u w^T + w u^T: x = A_ij - u_i (p_j - 2 cf u_j) - p_i u_j,  cf = (gamma/2) p.u
+    double pu = 0.0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) pu += red[w];
+    const double cf = 0.5 * gamma * pu;
+    // U1: column k+1 first (one element per thread): it is the next step's u
     {
-      const int t = tab[warp];
+      const int i = k + 1 + tid;
+      if (i < n) {
+        const double2 mine = up[k + 1], ui = up[i];
+        const double aj = fma(-2.0 * cf, mine.x, mine.y), bj = mine.x;
+        double* e = L + tri_off(i) + k + 1;
+        const double x = fma(-ui.y, bj, fma(-ui.x, aj, *e));
+        *e = x;
+        upn[i].x = x;
+      }
+    }
+    __syncthreads();
+    TRI_TICK(4);
+    // U2 (warps 1..31): the columns right of k+1;  R (warp 0): the reflector of the next step
+    if (warp == 0) {
+      if (more) reflector(k + 1);
+    } else {
+      const int t = tab[(k >> 3) & 1][warp - 1];
       const int cgm = t & 0xff;
       if (cgm != 0xff) {
         const int sub = (t >> 8) & 0xff, chunk = t >> 16;
         const int jlo = cgm << 5;
         const int j = jlo + lane;
-        const bool active = j > k && j < n;
+        const bool active = j > k + 1 && j < n;
         const int k8 = (k & ~7) + 1;                             // the table was built at step k & ~7
         const int start = jlo > k8 ? jlo : k8;
         const int r0 = start + sub * chunk, r1 = r0 + chunk < n ? r0 + chunk : n;
         if (active) {
-          double pu = 0.0;
-#pragma unroll
-          for (int w = 0; w < 8; ++w) pu += red[w];
-          const double cf = 0.5 * gamma * pu;
           const double2 mine = up[j];
           const double aj = fma(-2.0 * cf, mine.x, mine.y), bj = mine.x;
-          const bool nxt = j == k + 1;                           // my column is the next u
           double* Lc = L + j;
           int i = r0 > j ? r0 : j;                               // rows above my diagonal element are not mine
           if (i < r1) {
@@ -458,14 +484,12 @@ tridiag_smem2_body(double* tsm, const double* Cmat, int n, double* dvec, double*
               const double x2 = fma(-u2.y, bj, fma(-u2.x, aj, Lc[o2]));
               const double x3 = fma(-u3.y, bj, fma(-u3.x, aj, Lc[o3]));
               Lc[off] = x0; Lc[o1] = x1; Lc[o2] = x2; Lc[o3] = x3;
-              if (nxt) { upn[i].x = x0; upn[i + 1].x = x1; upn[i + 2].x = x2; upn[i + 3].x = x3; }
               off = o3 + i + 4;
             }
             for (; i < r1; ++i) {
               const double2 ui = up[i];
               const double x = fma(-ui.y, bj, fma(-ui.x, aj, Lc[off]));
               Lc[off] = x;
-              if (nxt) upn[i].x = x;
               off += i + 1;
             }
           }
