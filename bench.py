@@ -508,7 +508,7 @@ def main():
                 f = ln.split()
                 if len(f) == 3 and f[0] == name:
                     if f[2] == src_sha:
-                        traffic, traffic_note = int(f[1]), f"profiles/r1_k4_gemm_ws_ncu.md (GEMM sources sha16 {src_sha})"
+                        traffic, traffic_note = int(f[1]), f"profiles/r2_k4_gemm_ws_ncu.md (GEMM sources sha16 {src_sha})"
                     else:
                         traffic_note = f"stale: capture was of GEMM sources {f[2]}, now {src_sha}"
         line = {

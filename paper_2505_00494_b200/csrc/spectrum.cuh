@@ -527,6 +527,9 @@ tridiag_smem2_kernel(const double* __restrict__ Cmat, int n, double* __restrict_
 // minor of a matrix with relatively perturbed entries (backward stable); only signs are used, so p is renormalised by
 // an exact power of two every 4 rows (magnitudes then stay within 2^+-600 of 1).  d_i - x == 0 is replaced by 2^-100
 // (a perturbation of x far below rounding at this scaling); an exact zero minor counts as a sign change.
+// LEAN = true (the 1024-thread kernels, 64 registers per thread): groups of four rows without the look-ahead fetch -- the
+// eight-row version's 64 staging registers would spill there.
+template <bool LEAN = false>
 __device__ __forceinline__ int sturm_count_minors(const double2* __restrict__ de, int n, double x) {
   // Few instructions per row (the count is issue-bound as soon as two warps share a scheduler): the sign changes are
   // counted on the sign words (an exact zero counts as positive: the row after it has the sign opposite to the row
@@ -539,12 +542,38 @@ __device__ __forceinline__ int sturm_count_minors(const double2* __restrict__ de
   int i = 1;
   // rows in groups of eight: the group's (d_i - x, -e_i^2) are formed ahead of the dependent chain (one FMA per row),
   // and the next group's rows are fetched from shared memory before the chain of the current one starts
+  if (LEAN) {
+    for (; i + 4 <= n; i += 4) {
+      double2 v[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) v[u] = de[i + u];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const double tt = (v[u].x - x) + 0x1p-100;
+        const double pn = fma(tt, p1, -v[u].y * p0);
+        const int sn = __double2hiint(pn);
+        cnt += (int)((unsigned)(sn ^ sprev) >> 31);
+        sprev = sn; p0 = p1; p1 = pn;
+      }
+      const int e0 = __double2hiint(p0) & 0x7ff00000, e1 = __double2hiint(p1) & 0x7ff00000;
+      const int em = e0 > e1 ? e0 : e1;
+      if ((unsigned)(em - ((1023 - 64) << 20)) > (unsigned)(128 << 20)) {
+        if (em == 0) { p0 = 0.0; p1 = sprev < 0 ? -1.0 : 1.0; }
+        else {
+          const int e = (em >> 20) - 1023;
+          const int ee = e > 1000 ? 1000 : (e < -1000 ? -1000 : e);
+          const double sc = __hiloint2double((1023 - ee) << 20, 0);
+          p0 *= sc; p1 *= sc;
+        }
+      }
+    }
+  }
   double2 w[8];
-  if (i + 8 <= n) {
+  if (!LEAN && i + 8 <= n) {
 #pragma unroll
     for (int u = 0; u < 8; ++u) w[u] = de[i + u];
   }
-  for (; i + 8 <= n; i += 8) {
+  for (; !LEAN && i + 8 <= n; i += 8) {
     double tt[8], ne[8];
 #pragma unroll
     for (int u = 0; u < 8; ++u) { tt[u] = (w[u].x - x) + 0x1p-100; ne[u] = -w[u].y; }
@@ -624,6 +653,7 @@ __device__ __forceinline__ void multisect_setup(const double* dvec, const double
 // Stops when the bracket is narrower than 2^-54 of the spectrum's bound (the scaled problem has |lambda| <= 1): the
 // tridiagonalisation's own backward error is n eps ||C||, so resolving the tiny eigenvalues to full RELATIVE accuracy
 // (up to twice as many rounds) buys nothing for s, delta or the inverse-iteration shifts.
+template <bool LEAN = false>
 __device__ __forceinline__ double multisect_warp(const double2* de, int n, int idx, double glo, double ghi) {
   const int lane = threadIdx.x & 31;
   double a = glo, b = ghi;
@@ -632,7 +662,7 @@ __device__ __forceinline__ double multisect_warp(const double2* de, int n, int i
     const double h = (b - a) / 33.0;
     const double x = a + (lane + 1) * h;
     const bool inside = x > a && x < b;
-    int cnt = inside ? sturm_count_minors(de, n, x) : (x >= b ? n : 0);
+    int cnt = inside ? sturm_count_minors<LEAN>(de, n, x) : (x >= b ? n : 0);
     const unsigned m = __ballot_sync(0xffffffffu, cnt >= idx + 1);
     const int f = m ? __ffs(m) - 1 : 32;                       // first point with count >= idx+1
     const double xb = __shfl_sync(0xffffffffu, x, f < 32 ? f : 31);
@@ -723,7 +753,7 @@ spectrum_fused_body(double* tsm, const double* Cmat, int n, double* eig_out, dou
   multisect_setup(dv, ev, n, de, red, glo, ghi, isc);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   for (int idx = warp; idx < n; idx += TRI2_NT / 32) {
-    const double l = multisect_warp(de, n, idx, glo, ghi) * isc;
+    const double l = multisect_warp<true>(de, n, idx, glo, ghi) * isc;
     if (lane == 0) { lam[idx] = l; eig_out[idx] = l; }
   }
   __syncthreads();
