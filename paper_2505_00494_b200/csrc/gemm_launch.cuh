@@ -212,7 +212,7 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
   int splits = 1;
   bool use_sk = false, sk_hybrid = false;
   int cfg = 0;          // 0: 64x64 cp.async, 1: 128x128 cp.async, 2: ws 128x128, 3: ws 128x104, 4: ws 128x64 (2 CTA/SM),
-                        // 5: ws 128x56, 6: ws 80x208 (one wave for M <= 148 x 80, N <= 208)
+                        // 5: ws 128x56, 6: ws 80x208 (one wave for M <= 148 x 80, N <= 208), 7: ws 64x160
   const bool ws_big = ws_ok && c.M >= 96 && c.N >= 32 && (double)c.M * c.N * c.K > 2.0e8;
   if (c.batch > 0) {
     // batched launch (layered absorption): bulk-copy kernel only, one batch per gridDim.z, no split-K
@@ -246,9 +246,14 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
     else if (c.N >= 1024) { bn = 64; cfg = 4; }                // wide N: two CTAs per SM overlap epilogue and main loop
                                                                // (K4 at cfg4: 13.10 ms vs 13.20 ms with 128x128, 13.20 with 128x56)
     else if (padded(104) * 100 < padded(128) * 97) { bn = 104; cfg = 3; }
-    const long long tiles = (long long)((c.M + 127) / 128) * ((c.N + bn - 1) / bn);
+    // 128 < N <= 160 (K5, chi = 150: 208 or 256 padded columns otherwise): 64 x 160 tiles, eight warps of 32 x 40
+    // (a 128 x 160 tile needs 160 accumulator registers per thread with eight warps -- a 288-thread CTA gets 168 -- and
+    // spills with sixteen warps at 96)
+    if ((cfg == 2 || cfg == 3) && c.N > 128 && padded(160) * 100 < padded(bn) * 90) { bn = 160; cfg = 7; }
+    const int bm = cfg == 7 ? 64 : 128;
+    const long long tiles = (long long)((c.M + bm - 1) / bm) * ((c.N + bn - 1) / bn);
     const int slots = (cfg == 4 || cfg == 5) ? 296 : 148;
-    const double t_kt = 2.1e-6 * bn / 128.0 * ((cfg == 4 || cfg == 5) ? 2.0 : 1.0), t_fix = 4e-6;
+    const double t_kt = 2.1e-6 * bn / 128.0 * bm / 128.0 * ((cfg == 4 || cfg == 5) ? 2.0 : 1.0), t_fix = 4e-6;
     double best = 1e30;
     for (int sp = 1; sp <= 64; ++sp) {
       int per = (nkt + sp - 1) / sp;
@@ -301,6 +306,7 @@ int launch_gemm(cudaStream_t st, int path, const GemmCall& c, double* splitk_ws,
     case 4: *err = launch_cfg_ws<128, 64, 64, 32, 4>(st, g, splits, sk); break;
     case 5: *err = launch_cfg_ws<128, 56, 32, 56, 3>(st, g, splits, sk); break;
     case 6: *err = launch_cfg_ws<80, 208, 16, 104, 3>(st, g, splits, sk); break;
+    case 7: *err = launch_cfg_ws<64, 160, 32, 40, 4>(st, g, splits, sk); break;
     case 1: *err = launch_cfg<128, 128, 64, 32, 4>(st, g, splits); break;
     default: *err = launch_cfg<64, 64, 32, 16, 4>(st, g, splits); break;
   }

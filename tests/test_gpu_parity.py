@@ -757,6 +757,8 @@ def test_gemm_randomised_shapes_against_numpy():
     (1100, 1030, 1500),    # 128x64 tiles, two CTAs per SM: 153 tiles on 296 CTAs, ragged in M, N and K
     (700, 260, 9000),      # 128x128 tiles (N pads least there), 18 tiles, K not a multiple of 16
     (4000, 196, 333),      # short K: split-K / plain tiles chosen by the cost model
+    (3750, 150, 3750),     # K5 at cfg3b: one 160-wide tile column (128 x 160 tiles, warps of 64 x 40), stream-K
+    (3000, 290, 700),      # two 160-wide tile columns, ragged in N
 ])
 def test_gemm_k_splitting_schedules_against_numpy(M, N, K):
     """qrctm_gemm_f64_ws: with a scratch buffer the launcher may split K (split-K or stream-K).
