@@ -428,9 +428,12 @@ int qrctm_run(qrctm_t* h, int max_iter, double tol, int* iters_done, double* fin
       if (it % h->check_every == 0 || it == max_iter) {
         CU(h, cudaEventRecord(h->ev_env, h->stream));
         CU(h, cudaStreamWaitEvent(h->side, h->ev_env, 0));
-        rc = stage_spectrum(h, h->s, 1, h->side); if (rc) return rc;
-        CU(h, cudaMemcpyAsync(h->h_pinned, h->delta, sizeof(double), cudaMemcpyDeviceToHost, h->side));
-        CU(h, cudaMemcpyAsync(h->h_flag, h->flag, sizeof(int), cudaMemcpyDeviceToHost, h->side));
+        bool wrote = false;
+        rc = stage_spectrum(h, h->s, 1, h->side, true, &wrote); if (rc) return rc;
+        if (!wrote) {       // paths whose last kernel does not write the mapped host words itself
+          CU(h, cudaMemcpyAsync(h->h_pinned, h->delta, sizeof(double), cudaMemcpyDeviceToHost, h->side));
+          CU(h, cudaMemcpyAsync(h->h_flag, h->flag, sizeof(int), cudaMemcpyDeviceToHost, h->side));
+        }
         CU(h, cudaEventRecord(h->ev_spec, h->side));
         // (the next K7, the only writer of C, is enqueued after the host has seen ev_spec complete)
         pending = true;

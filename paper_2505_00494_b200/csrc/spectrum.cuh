@@ -659,7 +659,7 @@ __device__ __forceinline__ double multisect_warp(const double2* de, int n, int i
   double a = glo, b = ghi;
   for (int it = 0; it < 64; ++it) {
     if (b - a <= 0x1p-54) break;
-    const double h = (b - a) / 33.0;
+    const double h = (b - a) * (1.0 / 33.0);                    // (any interior points do: no division in the round)
     const double x = a + (lane + 1) * h;
     const bool inside = x > a && x < b;
     int cnt = inside ? sturm_count_minors<LEAN>(de, n, x) : (x >= b ? n : 0);
@@ -696,9 +696,12 @@ multisect_kernel(const double* __restrict__ dvec, const double* __restrict__ eve
 
 // One block, blockDim.x >= n: s = sorted |eig| (descending), delta vs s_prev.
 // blockDim.x >= n.  lam[n] (shared): the eigenvalues; s = sorted |lam| (descending), delta vs s_prev.
+// host_delta / host_flag (may be null): mapped pinned host words that receive delta and the NaN / zero-norm flag of K7
+// (dev_flag) straight from the kernel, so that the overlapped run driver needs no copies after K8.
 __device__ __forceinline__ void spectrum_finalize_body(const double* lam, double* red, int n, double* s_out,
                                                        double* s_prev, double* delta_out, int update_prev,
-                                                       double* hist, const int* hist_n) {
+                                                       double* hist, const int* hist_n, double* host_delta = nullptr,
+                                                       int* host_flag = nullptr, const int* dev_flag = nullptr) {
   const int tid = threadIdx.x;
   if (tid < n) {
     double mine = fabs(lam[tid]);
@@ -715,6 +718,7 @@ __device__ __forceinline__ void spectrum_finalize_body(const double* lam, double
   double dmax = block_max(dl, red);
   if (tid == 0) {
     delta_out[0] = dmax;
+    if (host_delta) { host_delta[0] = dmax; host_flag[0] = dev_flag[0]; }
     if (hist && update_prev && *hist_n > 0) hist[(size_t)((*hist_n - 1) % 4096) * 4] = dmax;   // this step's record
   }
   __syncthreads();
@@ -725,30 +729,94 @@ __device__ __forceinline__ void spectrum_finalize_body(const double* lam, double
 __global__ void spectrum_finalize_kernel(const double* __restrict__ eig, int n, double* __restrict__ s_out,
                                          double* __restrict__ s_prev, double* __restrict__ delta_out,
                                          int update_prev, double* __restrict__ hist = nullptr,
-                                         const int* __restrict__ hist_n = nullptr) {
+                                         const int* __restrict__ hist_n = nullptr, double* host_delta = nullptr,
+                                         int* host_flag = nullptr, const int* dev_flag = nullptr) {
   extern __shared__ double fsm[];               // lam[n], red[33]
   double* lam = fsm; double* red = fsm + n;
   if (threadIdx.x < n) lam[threadIdx.x] = eig[threadIdx.x];
   __syncthreads();
-  spectrum_finalize_body(lam, red, n, s_out, s_prev, delta_out, update_prev, hist, hist_n);
+  spectrum_finalize_body(lam, red, n, s_out, s_prev, delta_out, update_prev, hist, hist_n, host_delta, host_flag, dev_flag);
 }
 
-// K8 in ONE launch for small corners (n <= SPEC_FUSED_MAX_N): tridiagonalisation, multisection (32 warps, n / 32
-// rounds) and finalisation by the same CTA -- at these sizes the three launches cost more than the arithmetic.
+// Householder tridiagonalisation of a tiny matrix (n <= 32) by ONE warp, lane j <-> column j of the full symmetric matrix
+// in shared memory (pitch n + 1: conflict-free rows).  No block barrier inside the loop: a step is ~0.7 us where the
+// 1024-thread kernel above pays ~2 us for its four barriers and broadcast phases alone.  Same reflector conventions
+// (u = x - beta e_1, H = I - gamma u u^T, entries with |tail|^2 <= 1e-280 dropped), so d, e agree to rounding.
+// S: n (n + 1) + 2 n doubles.  All threads of the CTA load; warp 0 works; ends with a block barrier.
+__host__ __device__ inline size_t tri_warp_smem_bytes(int n) { return sizeof(double) * ((size_t)n * (n + 1) + 2 * (size_t)n + 2); }
+__device__ __forceinline__ void tridiag_warp_body(double* S, const double* Cmat, int n, double* dvec, double* evec) {
+  const int LD = n + 1;
+  double* us = S + n * LD;
+  double* ps = us + n;
+  const int tid = threadIdx.x, lane = tid & 31;
+  for (int e = tid; e < n * n; e += blockDim.x) {
+    const int i = e / n, j = e - i * n;
+    S[i * LD + j] = i >= j ? Cmat[(long long)i * n + j] : Cmat[(long long)j * n + i];     // lower triangle, mirrored
+  }
+  __syncthreads();
+  if (tid < 32) {
+    const int j = lane;
+    const bool col = j < n;
+    for (int k = 0; k < n - 2; ++k) {
+      const double x = (col && j > k) ? S[k * LD + j] : 0.0;
+      const double tail2 = warp_sum(j > k + 1 ? x * x : 0.0);
+      const double alpha = __shfl_sync(0xffffffffu, x, k + 1);
+      if (!(tail2 > 1e-280)) {
+        if (lane == 0) { dvec[k] = S[k * LD + k]; evec[k + 1] = alpha; }
+        continue;
+      }
+      const double s2 = fma(alpha, alpha, tail2);
+      const double sigma = s2 * rsqrt(s2);
+      const double beta = alpha >= 0.0 ? -sigma : sigma;
+      const double gamma = __drcp_rn(fma(-alpha, beta, s2));
+      const double u = j == k + 1 ? alpha - beta : x;            // 0 for j <= k and j >= n
+      if (col) us[j] = u;
+      __syncwarp();
+      double a0 = 0.0, a1 = 0.0;
+      if (col && j > k) {
+        int i = k + 1;
+        for (; i + 2 <= n; i += 2) { a0 = fma(S[i * LD + j], us[i], a0); a1 = fma(S[(i + 1) * LD + j], us[i + 1], a1); }
+        if (i < n) a0 = fma(S[i * LD + j], us[i], a0);
+      }
+      const double p = gamma * (a0 + a1);
+      const double cf = 0.5 * gamma * warp_sum(p * u);
+      if (col) ps[j] = p;
+      __syncwarp();
+      if (col && j > k) {
+        const double aj = fma(-2.0 * cf, u, p), bj = u;
+        for (int i = k + 1; i < n; ++i) S[i * LD + j] = fma(-ps[i], bj, fma(-us[i], aj, S[i * LD + j]));
+      }
+      if (lane == 0) { dvec[k] = S[k * LD + k]; evec[k + 1] = beta; }
+      __syncwarp();
+    }
+    if (lane == 0) {
+      if (n >= 2) { dvec[n - 2] = S[(n - 2) * LD + n - 2]; evec[n - 1] = S[(n - 1) * LD + n - 2]; }
+      dvec[n - 1] = S[(n - 1) * LD + n - 1];
+      evec[0] = 0.0;
+    }
+  }
+  __syncthreads();
+}
+
+// K8 in ONE launch for small corners (n <= SPEC_FUSED_MAX_N): tridiagonalisation (one warp), multisection (32 warps,
+// n / 32 rounds) and finalisation by the same CTA -- at these sizes the three launches cost more than the arithmetic.
 constexpr int SPEC_FUSED_MAX_N = 24;
-__host__ __device__ inline size_t spectrum_fused_smem_bytes(int n) { return tri2_smem_bytes(n) + sizeof(double) * (5 * (size_t)n + 40); }
+__host__ __device__ inline size_t spectrum_fused_smem_bytes(int n) {
+  const size_t a = tri2_smem_bytes(n), b = tri_warp_smem_bytes(n);
+  return (a > b ? a : b) + sizeof(double) * (5 * (size_t)n + 40);
+}
 
 __device__ __forceinline__ void
 spectrum_fused_body(double* tsm, const double* Cmat, int n, double* eig_out, double* s_out, double* s_prev,
-                    double* delta_out, int update_prev, double* hist, const int* hist_n) {
-  double* extra = tsm + tri2_smem_bytes(n) / sizeof(double);
+                    double* delta_out, int update_prev, double* hist, const int* hist_n, double* host_delta = nullptr,
+                    int* host_flag = nullptr, const int* dev_flag = nullptr) {
+  double* extra = tsm + (spectrum_fused_smem_bytes(n) - sizeof(double) * (5 * (size_t)n + 40)) / sizeof(double);
   double* dv = extra;                            // n
   double* ev = dv + n;                           // n
   double2* de = reinterpret_cast<double2*>((reinterpret_cast<uintptr_t>(ev + n) + 15) & ~static_cast<uintptr_t>(15));   // n pairs
   double* lam = reinterpret_cast<double*>(de + n);              // n
   double* red = lam + n;                         // 33
-  tridiag_smem2_body(tsm, Cmat, n, dv, ev, nullptr);
-  __syncthreads();
+  tridiag_warp_body(tsm, Cmat, n, dv, ev);
   double glo, ghi, isc;
   multisect_setup(dv, ev, n, de, red, glo, ghi, isc);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -757,14 +825,15 @@ spectrum_fused_body(double* tsm, const double* Cmat, int n, double* eig_out, dou
     if (lane == 0) { lam[idx] = l; eig_out[idx] = l; }
   }
   __syncthreads();
-  spectrum_finalize_body(lam, red, n, s_out, s_prev, delta_out, update_prev, hist, hist_n);
+  spectrum_finalize_body(lam, red, n, s_out, s_prev, delta_out, update_prev, hist, hist_n, host_delta, host_flag, dev_flag);
 }
 
 __global__ void __launch_bounds__(TRI2_NT, 1)
 spectrum_fused_kernel(const double* Cmat, int n, double* eig_out, double* s_out, double* s_prev, double* delta_out,
-                      int update_prev, double* hist, const int* hist_n) {
+                      int update_prev, double* hist, const int* hist_n, double* host_delta = nullptr,
+                      int* host_flag = nullptr, const int* dev_flag = nullptr) {
   extern __shared__ __align__(16) double tsm[];
-  spectrum_fused_body(tsm, Cmat, n, eig_out, s_out, s_prev, delta_out, update_prev, hist, hist_n);
+  spectrum_fused_body(tsm, Cmat, n, eig_out, s_out, s_prev, delta_out, update_prev, hist, hist_n, host_delta, host_flag, dev_flag);
 }
 
 }  // namespace qk

@@ -196,7 +196,12 @@ int stage_normalize(qrctm* h, const double* Cn, const double* Tn, bool record = 
 }
 
 // K8: spectrum of h->C into s_out (+ delta against s_prev, optional update)
-int stage_spectrum(qrctm* h, double* s_out, int update_prev, cudaStream_t st) {
+// to_host: the finalising kernel also writes delta and K7's flag word into the mapped pinned words h_pinned[0] / h_flag
+// (the overlapped run driver then needs no copies after K8); *wrote_host says whether the selected path did.
+int stage_spectrum(qrctm* h, double* s_out, int update_prev, cudaStream_t st, bool to_host = false, bool* wrote_host = nullptr) {
+  double* hd = to_host ? h->h_pinned : nullptr;
+  int* hf = to_host ? h->h_flag : nullptr;
+  if (wrote_host) *wrote_host = false;
   const int chi = h->chi;
   static int max_smem = -1;
   if (max_smem < 0) {
@@ -215,7 +220,8 @@ int stage_spectrum(qrctm* h, double* s_out, int update_prev, cudaStream_t st) {
       attrf = true;
     }
     spectrum_fused_kernel<<<1, TRI2_NT, spectrum_fused_smem_bytes(chi), st>>>(h->C, chi, h->eig, s_out, h->s_prev, h->delta,
-                                                                           update_prev, h->hist, h->flag + 1);
+                                                                           update_prev, h->hist, h->flag + 1, hd, hf, h->flag);
+    if (wrote_host) *wrote_host = to_host;
     h->launches += 1;
   } else if (chi <= TRI2_MAX_N && !h->k8_old) {
     static bool attr2 = false;
@@ -227,7 +233,8 @@ int stage_spectrum(qrctm* h, double* s_out, int update_prev, cudaStream_t st) {
     tridiag_smem2_kernel<<<1, TRI2_NT, tri2_smem_bytes(chi), st>>>(h->C, chi, h->dvec, h->evec, nullptr);
     multisect_kernel<<<(chi + 3) / 4, 128, sizeof(double) * (2 * chi + 40), st>>>(h->dvec, h->evec, chi, h->eig);
     spectrum_finalize_kernel<<<1, nt, sizeof(double) * (chi + 40), st>>>(h->eig, chi, s_out, h->s_prev, h->delta,
-                                                                        update_prev, h->hist, h->flag + 1);
+                                                                        update_prev, h->hist, h->flag + 1, hd, hf, h->flag);
+    if (wrote_host) *wrote_host = to_host;
     h->launches += 3;
   } else if (tri_bytes <= (size_t)max_smem && chi <= 1024) {
     tridiag_smem_kernel<<<1, 1024, tri_bytes, st>>>(h->C, chi, h->dvec, h->evec);
