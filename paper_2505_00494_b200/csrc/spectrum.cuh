@@ -738,12 +738,14 @@ __global__ void spectrum_finalize_kernel(const double* __restrict__ eig, int n, 
   spectrum_finalize_body(lam, red, n, s_out, s_prev, delta_out, update_prev, hist, hist_n, host_delta, host_flag, dev_flag);
 }
 
-// Householder tridiagonalisation of a tiny matrix (n <= 32) by ONE warp, lane j <-> column j of the full symmetric matrix
-// in shared memory (pitch n + 1: conflict-free rows).  No block barrier inside the loop: a step is ~0.7 us where the
-// 1024-thread kernel above pays ~2 us for its four barriers and broadcast phases alone.  Same reflector conventions
-// (u = x - beta e_1, H = I - gamma u u^T, entries with |tail|^2 <= 1e-280 dropped), so d, e agree to rounding.
-// S: n (n + 1) + 2 n doubles.  All threads of the CTA load; warp 0 works; ends with a block barrier.
+// Householder tridiagonalisation of a small matrix (n <= 32 NC) by ONE warp, lane l <-> columns l, l + 32 (NC = 2) of
+// the full symmetric matrix in shared memory (pitch n + 1: conflict-free rows).  No block barrier inside the loop: a
+// step is 0.7-1.1 us where the 1024-thread kernel above pays ~2 us for its four barriers and broadcast phases alone.
+// Same reflector conventions (u = x - beta e_1, H = I - gamma u u^T, entries with |tail|^2 <= 1e-280 dropped), so d, e
+// agree to rounding.  S: n (n + 1) + 2 n doubles.  All threads of the CTA load; warp 0 works; ends with a block barrier.
+constexpr int TRIW_MAX_N = 40;      // measured: K8 at n = 36 105 us against 116 with the 1024-thread kernel, at n = 64 209 against 187
 __host__ __device__ inline size_t tri_warp_smem_bytes(int n) { return sizeof(double) * ((size_t)n * (n + 1) + 2 * (size_t)n + 2); }
+template <int NC>
 __device__ __forceinline__ void tridiag_warp_body(double* S, const double* Cmat, int n, double* dvec, double* evec) {
   const int LD = n + 1;
   double* us = S + n * LD;
@@ -755,12 +757,17 @@ __device__ __forceinline__ void tridiag_warp_body(double* S, const double* Cmat,
   }
   __syncthreads();
   if (tid < 32) {
-    const int j = lane;
-    const bool col = j < n;
     for (int k = 0; k < n - 2; ++k) {
-      const double x = (col && j > k) ? S[k * LD + j] : 0.0;
-      const double tail2 = warp_sum(j > k + 1 ? x * x : 0.0);
-      const double alpha = __shfl_sync(0xffffffffu, x, k + 1);
+      double x[NC], u[NC], p[NC];
+      double t2 = 0.0;
+#pragma unroll
+      for (int c = 0; c < NC; ++c) {
+        const int j = lane + 32 * c;
+        x[c] = (j < n && j > k) ? S[k * LD + j] : 0.0;
+        t2 += j > k + 1 ? x[c] * x[c] : 0.0;
+      }
+      const double tail2 = warp_sum(t2);
+      const double alpha = S[k * LD + k + 1];
       if (!(tail2 > 1e-280)) {
         if (lane == 0) { dvec[k] = S[k * LD + k]; evec[k + 1] = alpha; }
         continue;
@@ -769,22 +776,80 @@ __device__ __forceinline__ void tridiag_warp_body(double* S, const double* Cmat,
       const double sigma = s2 * rsqrt(s2);
       const double beta = alpha >= 0.0 ? -sigma : sigma;
       const double gamma = __drcp_rn(fma(-alpha, beta, s2));
-      const double u = j == k + 1 ? alpha - beta : x;            // 0 for j <= k and j >= n
-      if (col) us[j] = u;
-      __syncwarp();
-      double a0 = 0.0, a1 = 0.0;
-      if (col && j > k) {
-        int i = k + 1;
-        for (; i + 2 <= n; i += 2) { a0 = fma(S[i * LD + j], us[i], a0); a1 = fma(S[(i + 1) * LD + j], us[i + 1], a1); }
-        if (i < n) a0 = fma(S[i * LD + j], us[i], a0);
+#pragma unroll
+      for (int c = 0; c < NC; ++c) {
+        const int j = lane + 32 * c;
+        u[c] = j == k + 1 ? alpha - beta : x[c];                  // 0 for j <= k and j >= n
+        if (j < n) us[j] = u[c];
       }
-      const double p = gamma * (a0 + a1);
-      const double cf = 0.5 * gamma * warp_sum(p * u);
-      if (col) ps[j] = p;
       __syncwarp();
-      if (col && j > k) {
-        const double aj = fma(-2.0 * cf, u, p), bj = u;
-        for (int i = k + 1; i < n; ++i) S[i * LD + j] = fma(-ps[i], bj, fma(-us[i], aj, S[i * LD + j]));
+      double acc[NC][4];
+#pragma unroll
+      for (int c = 0; c < NC; ++c) acc[c][0] = acc[c][1] = acc[c][2] = acc[c][3] = 0.0;
+      int jo[NC];                                                   // column offsets; lanes / columns beyond n - 1 read a
+#pragma unroll                                                      // valid column (results discarded)
+      for (int c = 0; c < NC; ++c) jo[c] = (lane + 32 * c < n) ? lane + 32 * c : 0;
+      {
+        int i = k + 1;
+        for (; i + 4 <= n; i += 4) {                                // four rows in flight per column
+          const double u0 = us[i], u1 = us[i + 1], u2 = us[i + 2], u3 = us[i + 3];
+          const double* r0 = S + i * LD;
+#pragma unroll
+          for (int c = 0; c < NC; ++c) {
+            acc[c][0] = fma(r0[jo[c]], u0, acc[c][0]);
+            acc[c][1] = fma(r0[LD + jo[c]], u1, acc[c][1]);
+            acc[c][2] = fma(r0[2 * LD + jo[c]], u2, acc[c][2]);
+            acc[c][3] = fma(r0[3 * LD + jo[c]], u3, acc[c][3]);
+          }
+        }
+        for (; i < n; ++i) {
+          const double u0 = us[i];
+#pragma unroll
+          for (int c = 0; c < NC; ++c) acc[c][0] = fma(S[i * LD + jo[c]], u0, acc[c][0]);
+        }
+      }
+      double pu = 0.0;
+#pragma unroll
+      for (int c = 0; c < NC; ++c) {
+        const int j = lane + 32 * c;
+        p[c] = (j < n && j > k) ? gamma * ((acc[c][0] + acc[c][1]) + (acc[c][2] + acc[c][3])) : 0.0;
+        pu = fma(p[c], u[c], pu);
+        if (j < n) ps[j] = p[c];
+      }
+      const double cf = 0.5 * gamma * warp_sum(pu);
+      __syncwarp();
+      {
+        double aj[NC], bj[NC];
+        bool on[NC];
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+          const int j = lane + 32 * c;
+          aj[c] = fma(-2.0 * cf, u[c], p[c]); bj[c] = u[c];
+          on[c] = j < n && j > k;
+        }
+        int i = k + 1;
+        for (; i + 4 <= n; i += 4) {                                // four rows in flight per column
+          const double u0 = us[i], u1 = us[i + 1], u2 = us[i + 2], u3 = us[i + 3];
+          const double p0 = ps[i], p1 = ps[i + 1], p2 = ps[i + 2], p3 = ps[i + 3];
+          double* r0 = S + i * LD;
+#pragma unroll
+          for (int c = 0; c < NC; ++c) {
+            if (on[c]) {
+              double* e = r0 + jo[c];
+              const double v0 = e[0], v1 = e[LD], v2 = e[2 * LD], v3 = e[3 * LD];
+              e[0] = fma(-p0, bj[c], fma(-u0, aj[c], v0));
+              e[LD] = fma(-p1, bj[c], fma(-u1, aj[c], v1));
+              e[2 * LD] = fma(-p2, bj[c], fma(-u2, aj[c], v2));
+              e[3 * LD] = fma(-p3, bj[c], fma(-u3, aj[c], v3));
+            }
+          }
+        }
+        for (; i < n; ++i) {
+          const double u0 = us[i], p0 = ps[i];
+#pragma unroll
+          for (int c = 0; c < NC; ++c)
+            if (on[c]) { double* e = S + i * LD + jo[c]; e[0] = fma(-p0, bj[c], fma(-u0, aj[c], e[0])); }
+        }
       }
       if (lane == 0) { dvec[k] = S[k * LD + k]; evec[k + 1] = beta; }
       __syncwarp();
@@ -796,6 +861,14 @@ __device__ __forceinline__ void tridiag_warp_body(double* S, const double* Cmat,
     }
   }
   __syncthreads();
+}
+
+// 24 < n <= TRIW_MAX_N (cfg1): the one-warp tridiagonalisation as a kernel of its own (128 threads load, warp 0 works).
+__global__ void __launch_bounds__(128)
+tridiag_warp_kernel(const double* Cmat, int n, double* dvec, double* evec) {
+  extern __shared__ __align__(16) double wsm[];
+  if (n <= 32) tridiag_warp_body<1>(wsm, Cmat, n, dvec, evec);
+  else tridiag_warp_body<2>(wsm, Cmat, n, dvec, evec);
 }
 
 // K8 in ONE launch for small corners (n <= SPEC_FUSED_MAX_N): tridiagonalisation (one warp), multisection (32 warps,
@@ -816,7 +889,7 @@ spectrum_fused_body(double* tsm, const double* Cmat, int n, double* eig_out, dou
   double2* de = reinterpret_cast<double2*>((reinterpret_cast<uintptr_t>(ev + n) + 15) & ~static_cast<uintptr_t>(15));   // n pairs
   double* lam = reinterpret_cast<double*>(de + n);              // n
   double* red = lam + n;                         // 33
-  tridiag_warp_body(tsm, Cmat, n, dv, ev);
+  tridiag_warp_body<1>(tsm, Cmat, n, dv, ev);
   double glo, ghi, isc;
   multisect_setup(dv, ev, n, de, red, glo, ghi, isc);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
