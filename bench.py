@@ -204,6 +204,8 @@ def bench_config(pkg, torch, name, steps, warmup, peak_dmma, conv=True, corner_m
            "path": ("whole-iteration kernels for tiny problems (K1..K6 one launch, K7 one, K8 one; stages_ms below is the "
                     "general multi-kernel path, timed serially with events)" if launches / steps < 6 else "general"),
            "stages_ms": {k: v / nst for k, v in st.items()},
+           "stages_tflops": {k: fl[k.split("_")[0]] / (v / nst * 1e-3) / 1e12 for k, v in st.items()
+                             if k.split("_")[0] in fl and v > 0},
            "algorithmic_gflop_per_step": sum(fl.values()) / 1e9,
            "step_tflops": sum(fl.values()) / (ms * 1e-3) / 1e12,
            "step_frac_of_fp64_peak": sum(fl.values()) / (ms * 1e-3) / 1e12 / peak_dmma}
@@ -530,6 +532,8 @@ def main():
                                         "(MEASURED_PEAKS.json has no FP64 entry; nominal 148 SM x 64 FMA/clk x 1.965 GHz = 37.2)",
                          "dfma_peak": peak_dfma, "algorithmic_flops_per_launch": fl["K4"], "ms_per_launch": k4_ms},
             "stages_ms": {k: v / nst for k, v in stage_ms.items()},
+            "stages_tflops": {k: fl[k.split("_")[0]] / (v / nst * 1e-3) / 1e12 for k, v in stage_ms.items()
+                              if k.split("_")[0] in fl and v > 0},
             "hbm_kernels": hbm_kernels,
             "time_to_convergence": conv,
             "next_1_layered": layered,
