@@ -44,10 +44,13 @@ __host__ __device__ inline size_t chol_smem_bytes(int n) {
 // of orthogonality of Q1).  prev_status (may be null): status word of the first pass; verdict (may be null):
 // verdict[0] = 1 when the CholeskyQR2 result must be discarded (either pass broke down or dev > dev_max).
 // (body: CHOL_NT threads of one CTA; sm = chol_smem_bytes(n) of shared memory; every pointer may be global or shared)
+constexpr double kCholFastDsum = 1e-18;   // ||Q1^T Q1 - I||_F^2 below which pass 2 takes the first-order factor
+
 __device__ __forceinline__ void
 chol_inv_body(double* sm, const double* G, int n, double* Rup, double* Llow, double* Rinv, int* status, double* dev,
               const int* prev_status, int* verdict, double dev_max,
-              long long* prof /* null, or 8 cycle counters of the phases (thread 0) */) {
+              long long* prof /* null, or 8 cycle counters of the phases (thread 0) */,
+              double fast_dsum = 0.0 /* > 0: first-order factor when ||G - I||_F^2 <= fast_dsum (see below) */) {
   const int nb = (n + 15) / 16, np = nb * 16;
   double* rd = sm + chol_base(nb);             // reciprocal diagonal of L
   double* red = rd + 16 * nb;                  // 33 doubles for the block reduction + flags
@@ -84,6 +87,29 @@ chol_inv_body(double* sm, const double* G, int n, double* Rup, double* Llow, dou
   }
   dsum = block_sum(dsum, red);
   CHOL_TICK(0);
+
+  // ---- second pass of CholeskyQR2: G = Q1^T Q1 = I + E with ||E||_F ~ cond(X)^2 eps (1e-15 ... 1e-11 on the step's c~).
+  // For ||E||_F <= 1e-9 the first-order factor R = I + U, R^-1 = I - U, U = striu(E) + diag(E) / 2 (U + U^T = E) is the
+  // Cholesky factor to rounding -- the neglected terms are O(||E||^2) <= 1e-18 -- so the serial factorisation and
+  // inversion below (most of this kernel's time) are skipped.  The branch is uniform (dsum is a block-wide sum).
+  if (fast_dsum > 0.0 && dsum <= fast_dsum) {
+    for (int i = warp; i < n; i += NW)
+      for (int j = lane; j < n; j += 32) {
+        const int hi = i > j ? i : j, lo = i > j ? j : i;        // the stored lower triangle holds G[hi][lo]
+        const double g = sm[chol_base(hi >> 4) + (hi & 15) * chol_stride(hi >> 4) + lo];
+        const double u = i == j ? 0.5 * (g - 1.0) : g;
+        if (Llow) Llow[i * n + j] = j < i ? u : (j == i ? 1.0 + u : 0.0);
+        if (Rup) Rup[i * n + j] = j > i ? u : (j == i ? 1.0 + u : 0.0);
+        Rinv[i * n + j] = j > i ? -u : (j == i ? 1.0 - u : 0.0);
+      }
+    if (tid == 0) {
+      status[0] = 0;
+      dev[0] = sqrt(dsum);
+      if (verdict) verdict[0] = (prev_status && prev_status[0]) ? 1 : 0;
+      if (prof) for (int i = 0; i < 8; ++i) prof[i] = tp[i];
+    }
+    return;
+  }
 
   // ---- blocked right-looking Cholesky with a one-block look-ahead: after the panel of block column J, warp 0 updates
   // only the next diagonal block and factors it at once (a chain of 16 dependent rsqrt, ~2 us) while the other warps do
@@ -311,9 +337,9 @@ __global__ void __launch_bounds__(CHOL_NT, 1)
 chol_inv_kernel(const double* __restrict__ G, int n, double* __restrict__ Rup, double* __restrict__ Llow,
                 double* __restrict__ Rinv, int* __restrict__ status, double* __restrict__ dev,
                 const int* __restrict__ prev_status, int* __restrict__ verdict, double dev_max,
-                long long* __restrict__ prof) {
+                long long* __restrict__ prof, double fast_dsum = 0.0) {
   extern __shared__ __align__(16) double sm[];
-  chol_inv_body(sm, G, n, Rup, Llow, Rinv, status, dev, prev_status, verdict, dev_max, prof);
+  chol_inv_body(sm, G, n, Rup, Llow, Rinv, status, dev, prev_status, verdict, dev_max, prof, fast_dsum);
 }
 
 // ------------------------------------------------------------------------------------------------------------------
@@ -413,7 +439,7 @@ cholqr2_cluster_kernel(const double* __restrict__ X, long long rows, int n, doub
     }
     __syncthreads();
     if (pass == 0) chol_inv_body(ws, Gf, n, R1, nullptr, Ri, st, sc, nullptr, nullptr, 0.0, nullptr);
-    else           chol_inv_body(ws, Gf, n, nullptr, Gp, Ri, st + 1, sc + 1, st, st + 2, dev_max, nullptr);
+    else           chol_inv_body(ws, Gf, n, nullptr, Gp, Ri, st + 1, sc + 1, st, st + 2, dev_max, nullptr, kCholFastDsum);
     __syncthreads();
     CQ_TICK(4);
     // slab <- slab R^-1 (R^-1 upper triangular) in 4 x 4 register blocks: pass 1 into the other buffer, pass 2 to Q

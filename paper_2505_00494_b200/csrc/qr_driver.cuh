@@ -525,7 +525,7 @@ long long qr_factor_cholqr2(cudaStream_t st, long long rows, int n, const double
   if (nl < 0) return -1;
   launches += nl;
   chol_inv_kernel<<<1, CHOL_NT, smem, st>>>(wk.Gq, n, nullptr, wk.cL2, wk.cRi2, wk.cstat + 1, wk.cdev + 1, wk.cstat,
-                                            wk.cstat + 2, kCholqrDevMax, nullptr);
+                                            wk.cstat + 2, kCholqrDevMax, nullptr, kCholFastDsum);
   if (!fork_ok) transpose_tall_kernel<<<tg, tb, 0, st>>>(wk.V, rows, n, wk.Vct);
   else {
     if (cudaStreamWaitEvent(st, fb.e_join, 0) != cudaSuccess) { *err = cudaGetLastError(); return -1; }
