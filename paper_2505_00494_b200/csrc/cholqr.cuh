@@ -350,8 +350,12 @@ chol_inv_kernel(const double* __restrict__ G, int n, double* __restrict__ Rup, d
 // through distributed shared memory (every CTA ends with the full G) -> every CTA factors and inverts G redundantly
 // (chol_inv_body) -> slab <- slab R^-1.  Rank 0 writes R = L2^T R1 and the status / verdict words.  Deterministic.
 constexpr int CHOLC_MAX_N = 64;
+// slab pitch: >= n, = 4 (mod 16) doubles, so that the m8n8k4 fragment loads of both products are conflict-free (as in the
+// Cholesky kernel's block rows); slab rows padded to a multiple of 8 (zero rows: they complete the last fragments)
+__host__ __device__ inline int cholqr2_slab_pitch(int n) { return ((n + 11) / 16) * 16 + 4; }
 __host__ __device__ inline size_t cholqr2_cluster_smem_bytes(int n, int rpc) {
-  return sizeof(double) * ((size_t)4 * n * n + (size_t)2 * rpc * n + 8) + chol_smem_bytes(n);
+  const size_t rp = (size_t)((rpc + 7) & ~7);
+  return sizeof(double) * ((size_t)4 * n * n + 2 * rp * cholqr2_slab_pitch(n) + 8) + chol_smem_bytes(n);
 }
 
 __global__ void __launch_bounds__(CHOL_NT, 1)
@@ -367,51 +371,65 @@ cholqr2_cluster_kernel(const double* __restrict__ X, long long rows, int n, doub
   double* Gf = Gp + nn;                  // the full Gram matrix (written by all ranks)
   double* R1 = Gf + nn;                  // R of pass 1
   double* Ri = R1 + nn;                  // R^-1 of the current pass
-  double* Xs = Ri + nn;                  // rpc x n: my rows of X, then of Q1 after the swap
-  double* Ys = Xs + (size_t)rpc * n;
-  double* sc = Ys + (size_t)rpc * n;     // [0..1] deviations, ints behind
+  const int P = cholqr2_slab_pitch(n), rp = (rpc + 7) & ~7;
+  double* Xs = Ri + nn;                  // rp x P: my rows of X, then of Q1 after the swap (pad rows / columns zero)
+  double* Ys = Xs + (size_t)rp * P;
+  double* sc = Ys + (size_t)rp * P;      // [0..1] deviations, ints behind
   int* st = reinterpret_cast<int*>(sc + 4);
   double* ws = sc + 8;                   // chol_inv_body's workspace
-  const int tid = threadIdx.x;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int lr = lane >> 2, lc = lane & 3;
+  constexpr int NW = CHOL_NT / 32;
   long long tp[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tc = 0;
 #define CQ_TICK(i) do { if (prof && tid == 0 && rank == 0) { const long long t_ = clock64(); tp[i] += t_ - tc; tc = t_; } } while (0)
   if (prof && tid == 0 && rank == 0) tc = clock64();
   const long long r0 = (long long)rank * rpc;
   const int rl = (int)(rows - r0 < 0 ? 0 : (rows - r0 < rpc ? rows - r0 : rpc));      // my rows
-  for (int i = tid; i < rl * n; i += CHOL_NT) Xs[i] = X[r0 * n + i];
+  for (int i = tid; i < rp * P; i += CHOL_NT) {
+    const int r = i / P, c = i - r * P;
+    Xs[i] = (r < rl && c < n) ? X[(r0 + r) * n + c] : 0.0;
+    Ys[i] = 0.0;
+  }
   __syncthreads();
   CQ_TICK(0);
   double* src = Xs;
   double* dst = Ys;
+  const int nf = (n + 7) >> 3;             // 8-wide fragment columns
+  const int nrf = (rl + 7) >> 3;           // 8-row fragments of my slab
   for (int pass = 0; pass < 2; ++pass) {
-    // local Gram matrix of the slab, lower block triangle in 4 x 4 register blocks (a plain one-output-per-thread loop
-    // is bound by shared-memory bandwidth: three wavefronts per FMA; here 8 loads feed 16 FMAs)
-    const int nq = (n + 3) >> 2, nblk = nq * (nq + 1) / 2;
-    for (int q = tid; q < nblk; q += CHOL_NT) {
-      int bi = (int)((sqrtf(8.0f * q + 1.0f) - 1.0f) * 0.5f);
-      while ((bi + 1) * (bi + 2) / 2 <= q) ++bi;
-      while (bi * (bi + 1) / 2 > q) --bi;
-      const int bj = q - bi * (bi + 1) / 2, i0 = bi << 2, j0 = bj << 2;
-      double g[4][4];
+    // local Gram matrix of the slab as DMMA tiles straight from shared memory: 8 x 8 output fragments of the lower
+    // fragment triangle, up to three per warp in flight; G[i][j] = sum_r X[r][i] X[r][j]: both operands are read as
+    // src[(r + lc) * P + col + lr] (conflict-free for P = 4 mod 16); the pad rows are zero
+    {
+      const int nfr = nf * (nf + 1) / 2;
+      for (int q0 = warp; q0 < nfr; q0 += 3 * NW) {
+        int i0[3], j0[3];
+        double acc[3][2];
 #pragma unroll
-      for (int a = 0; a < 4; ++a)
+        for (int t = 0; t < 3; ++t) {
+          int q = q0 + t * NW; if (q >= nfr) q = q0;           // a duplicate of the first fragment (not stored)
+          int fi = (int)((sqrtf(8.0f * q + 1.0f) - 1.0f) * 0.5f);
+          while ((fi + 1) * (fi + 2) / 2 <= q) ++fi;
+          while (fi * (fi + 1) / 2 > q) --fi;
+          i0[t] = fi << 3; j0[t] = (q - fi * (fi + 1) / 2) << 3;
+          acc[t][0] = acc[t][1] = 0.0;
+        }
+        const double* sp = src + lc * P + lr;
+        for (int r = 0; r < 8 * nrf; r += 4) {
 #pragma unroll
-        for (int c = 0; c < 4; ++c) g[a][c] = 0.0;
-      for (int r = 0; r < rl; ++r) {
-        double xi[4], xj[4];
+          for (int t = 0; t < 3; ++t) dmma884(acc[t][0], acc[t][1], sp[r * P + i0[t]], sp[r * P + j0[t]]);
+        }
 #pragma unroll
-        for (int a = 0; a < 4; ++a) { xi[a] = i0 + a < n ? src[r * n + i0 + a] : 0.0; xj[a] = j0 + a < n ? src[r * n + j0 + a] : 0.0; }
-#pragma unroll
-        for (int a = 0; a < 4; ++a)
-#pragma unroll
-          for (int c = 0; c < 4; ++c) g[a][c] = fma(xi[a], xj[c], g[a][c]);
+        for (int t = 0; t < 3; ++t) {
+          if (q0 + t * NW < nfr) {
+            const int i = i0[t] + lr, j = j0[t] + 2 * lc;
+            if (i < n && j < n) Gp[i * n + j] = acc[t][0];
+            if (i < n && j + 1 < n) Gp[i * n + j + 1] = acc[t][1];
+          }
+        }
       }
-#pragma unroll
-      for (int a = 0; a < 4; ++a)
-#pragma unroll
-        for (int c = 0; c < 4; ++c)
-          if (i0 + a < n && j0 + c < n) Gp[(i0 + a) * n + j0 + c] = g[a][c];
     }
+    const int nq = (n + 3) >> 2, nblk = nq * (nq + 1) / 2;
     CQ_TICK(1);
     cluster.sync();
     CQ_TICK(2);
@@ -442,34 +460,32 @@ cholqr2_cluster_kernel(const double* __restrict__ X, long long rows, int n, doub
     else           chol_inv_body(ws, Gf, n, nullptr, Gp, Ri, st + 1, sc + 1, st, st + 2, dev_max, nullptr, kCholFastDsum);
     __syncthreads();
     CQ_TICK(4);
-    // slab <- slab R^-1 (R^-1 upper triangular) in 4 x 4 register blocks: pass 1 into the other buffer, pass 2 to Q
+    // slab <- slab R^-1 (R^-1 upper triangular: k <= c) as DMMA tiles: a work item is one fragment column and up to four
+    // row fragments, the B fragment of a k-step is loaded once for the four; pass 1 into the other buffer, pass 2 to Q
     {
-      const int nrb = (rl + 3) >> 2;
-      for (int q = tid; q < nrb * nq; q += CHOL_NT) {
-        const int rb = q / nq, cb = q % nq, rr0 = rb << 2, c0 = cb << 2;
-        double y[4][4];
+      const int nrg = (nrf + 3) >> 2;
+      for (int it = warp; it < nf * nrg; it += NW) {
+        const int cf = it / nrg, rg = it - cf * nrg, c0 = cf << 3, rf0 = rg << 2;
+        double acc[4][2];
 #pragma unroll
-        for (int a = 0; a < 4; ++a)
+        for (int t = 0; t < 4; ++t) acc[t][0] = acc[t][1] = 0.0;
+        const int kend = c0 + 8 < n ? c0 + 8 : n;           // R^-1[k][c] = 0 for k > c
+        const double* ap = src + (size_t)(rf0 * 8 + lr) * P + lc;
+        for (int k = 0; k < kend; k += 4) {
+          const int kk = k + lc, cc = c0 + lr;
+          const double bv = (kk < n && cc < n) ? Ri[kk * n + cc] : 0.0;
 #pragma unroll
-          for (int c = 0; c < 4; ++c) y[a][c] = 0.0;
-        const int kend = c0 + 4 < n ? c0 + 4 : n;           // R^-1[k][c] = 0 for k > c
-        for (int k = 0; k < kend; ++k) {
-          double xs[4], rv[4];
-#pragma unroll
-          for (int a = 0; a < 4; ++a) { xs[a] = rr0 + a < rl ? src[(rr0 + a) * n + k] : 0.0; rv[a] = c0 + a < n ? Ri[k * n + c0 + a] : 0.0; }
-#pragma unroll
-          for (int a = 0; a < 4; ++a)
-#pragma unroll
-            for (int c = 0; c < 4; ++c) y[a][c] = fma(xs[a], rv[c], y[a][c]);
+          for (int t = 0; t < 4; ++t)
+            if (rf0 + t < nrf) dmma884(acc[t][0], acc[t][1], ap[(size_t)t * 8 * P + k], bv);
         }
 #pragma unroll
-        for (int a = 0; a < 4; ++a)
-#pragma unroll
-          for (int c = 0; c < 4; ++c)
-            if (rr0 + a < rl && c0 + c < n) {
-              const int idx = (rr0 + a) * n + c0 + c;
-              if (pass == 0) dst[idx] = y[a][c]; else Q[r0 * n + idx] = y[a][c];
-            }
+        for (int t = 0; t < 4; ++t) {
+          const int r = (rf0 + t) * 8 + lr, c = c0 + 2 * lc;
+          if (rf0 + t < nrf && r < rl) {
+            if (pass == 0) { if (c < n) dst[r * P + c] = acc[t][0]; if (c + 1 < n) dst[r * P + c + 1] = acc[t][1]; }
+            else { if (c < n) Q[(r0 + r) * n + c] = acc[t][0]; if (c + 1 < n) Q[(r0 + r) * n + c + 1] = acc[t][1]; }
+          }
+        }
       }
     }
     __syncthreads();
