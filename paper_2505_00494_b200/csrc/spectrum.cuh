@@ -743,7 +743,6 @@ __global__ void spectrum_finalize_kernel(const double* __restrict__ eig, int n, 
 // step is 0.7-1.1 us where the 1024-thread kernel above pays ~2 us for its four barriers and broadcast phases alone.
 // Same reflector conventions (u = x - beta e_1, H = I - gamma u u^T, entries with |tail|^2 <= 1e-280 dropped), so d, e
 // agree to rounding.  S: n (n + 1) + 2 n doubles.  All threads of the CTA load; warp 0 works; ends with a block barrier.
-constexpr int TRIW_MAX_N = 40;      // measured: K8 at n = 36 105 us against 116 with the 1024-thread kernel, at n = 64 209 against 187
 __host__ __device__ inline size_t tri_warp_smem_bytes(int n) { return sizeof(double) * ((size_t)n * (n + 1) + 2 * (size_t)n + 2); }
 template <int NC>
 __device__ __forceinline__ void tridiag_warp_body(double* S, const double* Cmat, int n, double* dvec, double* evec) {
@@ -863,12 +862,107 @@ __device__ __forceinline__ void tridiag_warp_body(double* S, const double* Cmat,
   __syncthreads();
 }
 
-// 24 < n <= TRIW_MAX_N (cfg1): the one-warp tridiagonalisation as a kernel of its own (128 threads load, warp 0 works).
-__global__ void __launch_bounds__(128)
-tridiag_warp_kernel(const double* Cmat, int n, double* dvec, double* evec) {
-  extern __shared__ __align__(16) double wsm[];
-  if (n <= 32) tridiag_warp_body<1>(wsm, Cmat, n, dvec, evec);
-  else tridiag_warp_body<2>(wsm, Cmat, n, dvec, evec);
+// n <= 128: the matrix lives in REGISTERS.  NCG x NRG warps: warp w holds the columns j = lane + 32 (w % NCG), rows
+// i = w / NCG + NRG t, t = 0..15 of the full symmetric matrix (16 doubles per thread), so the rank-2 update touches no
+// shared memory but u and p, and the matrix-vector product is 16 FMAs per thread + one NRG-way combine.  Three block
+// barriers per step; the reflector scalars and the two warp reductions are computed redundantly by every warp.  Same
+// reflector conventions as the kernels above.  Used as <2, 4>: 256 threads, n <= 64, u of the thread's rows kept in
+// registers (K8 through the API at n = 36 / 64: 70 / 103 us against 105 / 187 with the shared-memory kernels).  The
+// <4, 8> instantiation (1024 threads, 64 registers each, u re-read from shared memory in the update, n <= 128) measured
+// SLOWER than tridiag_smem2_kernel (n = 100: 415 against 316 us) and is not used.
+constexpr int TRIR_MAX_N = 64;
+template <int NCG, int NRG>
+__global__ void __launch_bounds__(32 * NCG * NRG)
+tridiag_reg_kernel(const double* __restrict__ Cmat, int n, double* __restrict__ dvec, double* __restrict__ evec) {
+  constexpr int NC = 32 * NCG;                                   // columns held (>= n), 16 NRG >= n rows
+  constexpr bool KEEPU = NCG * NRG <= 8;
+  __shared__ double us[NC], pb[NC], part[NRG][NC];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int cg = warp % NCG, rg = warp / NCG;
+  const int j = lane + 32 * cg;
+  const bool colv = j < n;
+  double a[16];
+#pragma unroll
+  for (int t = 0; t < 16; ++t) {
+    const int i = rg + NRG * t;
+    a[t] = (colv && i < n) ? (i >= j ? Cmat[(long long)i * n + j] : Cmat[(long long)j * n + i]) : 0.0;   // lower triangle, mirrored
+  }
+  if (tid == 0) evec[0] = 0.0;
+  for (int k = 0; k < n - 2; ++k) {
+    // row k (= column k) from its owners' registers
+    if (rg == k % NRG) {
+      const int tk = k / NRG;
+      double x = a[0];
+#pragma unroll
+      for (int t = 1; t < 16; ++t) x = (tk == t) ? a[t] : x;
+      us[j] = (colv && j > k) ? x : 0.0;
+      if (j == k) dvec[k] = x;
+    }
+    __syncthreads();
+    double xl[NCG], t2 = 0.0;
+#pragma unroll
+    for (int c = 0; c < NCG; ++c) { xl[c] = us[lane + 32 * c]; t2 += lane + 32 * c > k + 1 ? xl[c] * xl[c] : 0.0; }
+    const double tail2 = warp_sum(t2);
+    const double alpha = us[k + 1];
+    if (!(tail2 > 1e-280)) {                                      // uniform: every warp reduces the same numbers
+      if (tid == 0) evec[k + 1] = alpha;
+      __syncthreads();                                           // us is rewritten by the next step
+      continue;
+    }
+    const double s2 = fma(alpha, alpha, tail2);
+    const double sigma = s2 * rsqrt(s2);
+    const double beta = alpha >= 0.0 ? -sigma : sigma;
+    const double gamma = __drcp_rn(fma(-alpha, beta, s2));
+    const double u1 = alpha - beta;
+    double ui[KEEPU ? 16 : 1];
+    const double uj = j == k + 1 ? u1 : us[j];
+    double p0 = 0.0, p1 = 0.0, p2 = 0.0, p3 = 0.0;
+#pragma unroll
+    for (int t = 0; t < 16; t += 4) {
+      double u[4];
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const int i = rg + NRG * (t + q);
+        u[q] = i == k + 1 ? u1 : us[i];                            // us[i] = 0 for i <= k and i >= n
+        if (KEEPU) ui[t + q] = u[q];
+      }
+      p0 = fma(a[t], u[0], p0); p1 = fma(a[t + 1], u[1], p1);
+      p2 = fma(a[t + 2], u[2], p2); p3 = fma(a[t + 3], u[3], p3);
+    }
+    part[rg][j] = (p0 + p1) + (p2 + p3);
+    __syncthreads();
+    if (rg == 0) {
+      double sum = 0.0;
+#pragma unroll
+      for (int r = 0; r < NRG; r += 2) sum += part[r][j] + part[r + 1][j];
+      pb[j] = (colv && j > k) ? gamma * sum : 0.0;
+    }
+    __syncthreads();
+    double pu = 0.0;
+#pragma unroll
+    for (int c = 0; c < NCG; ++c) pu = fma(pb[lane + 32 * c], lane + 32 * c == k + 1 ? u1 : xl[c], pu);
+    const double cf = 0.5 * gamma * warp_sum(pu);
+    const double pj = pb[j];
+    const double aj = fma(-2.0 * cf, uj, pj), bj = uj;           // both 0 for j <= k: rows and columns <= k stay as they are
+#pragma unroll
+    for (int t = 0; t < 16; ++t) {
+      const int i = rg + NRG * t;
+      const double u = KEEPU ? ui[t] : (i == k + 1 ? u1 : us[i]);
+      a[t] = fma(-pb[i], bj, fma(-u, aj, a[t]));
+    }
+    if (tid == 0) evec[k + 1] = beta;
+  }
+  // the last 2 x 2 block
+  {
+    const int i1 = n - 1, i2 = n - 2;
+#pragma unroll
+    for (int t = 0; t < 16; ++t) {
+      const int i = rg + NRG * t;
+      if (n >= 2 && i == i2 && j == i2) dvec[i2] = a[t];
+      if (n >= 2 && i == i1 && j == i2) evec[i1] = a[t];
+      if (i == i1 && j == i1) dvec[i1] = a[t];
+    }
+  }
 }
 
 // K8 in ONE launch for small corners (n <= SPEC_FUSED_MAX_N): tridiagonalisation (one warp), multisection (32 warps,

@@ -346,10 +346,10 @@ def test_cfg1_fixed_count_and_kappa():
 
 def test_spectrum_kernel_against_lapack():
     import torch
-    # chi <= 24: one fused kernel (one-warp tridiagonalisation); <= 40: the one-warp kernel, one / two columns per lane;
-    # <= 216 / 236: shared-memory tridiagonalisations; above: the multi-CTA tridiagonalisation of the eigen step
-    for chi, seed in [(1, 0), (2, 1), (3, 10), (8, 2), (24, 11), (25, 12), (32, 13), (33, 14), (36, 3), (40, 15), (41, 16),
-                      (100, 4), (196, 5), (236, 6), (237, 7), (400, 8), (700, 9)]:
+    # chi <= 24: one fused kernel (one-warp tridiagonalisation); <= 64: the register-resident kernel; <= 216 / 236:
+    # shared-memory tridiagonalisations; above: the multi-CTA tridiagonalisation of the eigen step
+    for chi, seed in [(1, 0), (2, 1), (3, 10), (8, 2), (24, 11), (25, 12), (31, 17), (32, 13), (33, 14), (36, 3), (40, 15),
+                      (41, 16), (63, 18), (64, 19), (65, 20), (100, 4), (196, 5), (236, 6), (237, 7), (400, 8), (700, 9)]:
         A, C0, T0 = gen_config(2, 1, chi, seed)
         h = pkg.QRCTM(2, 1, chi)
         h.set_A(A); h.set_env(C0, T0)
@@ -373,10 +373,12 @@ def test_tridiag_kernel_preserves_the_spectrum(n):
         assert np.max(np.abs(np.linalg.eigvalsh(T) - np.linalg.eigvalsh(M))) < 5e-15 * max(n, 4)
 
 
-@pytest.mark.parametrize("name,n", [("identity", 30), ("diag", 37), ("block", 32), ("ones", 33), ("rank2", 40), ("zero_tail", 20)])
+@pytest.mark.parametrize("name,n", [("identity", 30), ("diag", 37), ("block", 32), ("ones", 33), ("rank2", 40), ("zero_tail", 20),
+                                    ("identity", 64), ("block", 56), ("ones", 16), ("rank2", 61), ("zero_tail", 50), ("diag", 12)])
 def test_spectrum_small_structured_matrices(name, n):
-    """The one-warp tridiagonalisation (n <= 40) on matrices whose reflectors vanish or whose trailing block is rounding
-    noise: identity, diagonal, block-diagonal of all-ones blocks, all ones, rank two, a matrix with an exactly zero tail."""
+    """The small tridiagonalisations (one warp for n <= 24, registers for n <= 64) on matrices whose reflectors vanish or
+    whose trailing block is rounding noise: identity, diagonal, block-diagonal of all-ones blocks, all ones, rank two, a
+    matrix with an exactly zero tail."""
     g = np.random.default_rng(n)
     if name == "identity": C = np.eye(n)
     elif name == "diag": C = np.diag(np.arange(1.0, n + 1))
