@@ -866,24 +866,31 @@ __device__ __forceinline__ void tridiag_warp_body(double* S, const double* Cmat,
 // i = w / NCG + NRG t, t = 0..15 of the full symmetric matrix (16 doubles per thread), so the rank-2 update touches no
 // shared memory but u and p, and the matrix-vector product is 16 FMAs per thread + one NRG-way combine.  Three block
 // barriers per step; the reflector scalars and the two warp reductions are computed redundantly by every warp.  Same
-// reflector conventions as the kernels above.  Used as <2, 4>: 256 threads, n <= 64, u of the thread's rows kept in
-// registers (K8 through the API at n = 36 / 64: 70 / 103 us against 105 / 187 with the shared-memory kernels).  The
-// <4, 8> instantiation (1024 threads, 64 registers each, u re-read from shared memory in the update, n <= 128) measured
-// SLOWER than tridiag_smem2_kernel (n = 100: 415 against 316 us) and is not used.
-constexpr int TRIR_MAX_N = 64;
-template <int NCG, int NRG>
+// reflector conventions as the kernels above.  <2, 4, 16>: 256 threads, n <= 64, u of the thread's rows kept in registers
+// (K8 through the API at n = 36 / 64: 70 / 103 us against 105 / 187 with the shared-memory kernels).  <4, 4, 32>: 512
+// threads x 32 elements, n <= 128; (x_i, p_i) re-read from shared memory as one double2 in the update, rows and column
+// groups that have been eliminated are skipped (n = 100 / 128: 254 / 325 us against 316 / 440).  A 1024-thread variant
+// (64 registers per thread, 32 warps repeating the scalar chain) measured slower than tridiag_smem2_kernel.
+constexpr int TRIR_MAX_N = 64, TRIR_MAX_N2 = 128;
+template <int NCG, int NRG, int NE>
 __global__ void __launch_bounds__(32 * NCG * NRG)
 tridiag_reg_kernel(const double* __restrict__ Cmat, int n, double* __restrict__ dvec, double* __restrict__ evec) {
-  constexpr int NC = 32 * NCG;                                   // columns held (>= n), 16 NRG >= n rows
-  constexpr bool KEEPU = NCG * NRG <= 8;
-  __shared__ double us[NC], pb[NC], part[NRG][NC];
+  constexpr int NC = 32 * NCG;                                   // columns held (>= n), NE NRG >= n rows
+  constexpr bool KEEPU = NE <= 16;
+  // row k (x) and p: the small variant keeps two plain arrays (its u stays in registers, and the 16-byte stride of an
+  // interleaved array costs it bank conflicts on the per-lane reads); the large one reads (x_i, p_i) as one double2
+  __shared__ double2 up[KEEPU ? 1 : NC];
+  __shared__ double us[KEEPU ? NC : 1], pb[KEEPU ? NC : 1];
+  __shared__ double part[NRG][NC];
+  auto X = [&](int i) -> double& { return KEEPU ? us[i] : up[i].x; };
+  auto Pv = [&](int i) -> double& { return KEEPU ? pb[i] : up[i].y; };
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int cg = warp % NCG, rg = warp / NCG;
   const int j = lane + 32 * cg;
   const bool colv = j < n;
-  double a[16];
+  double a[NE];
 #pragma unroll
-  for (int t = 0; t < 16; ++t) {
+  for (int t = 0; t < NE; ++t) {
     const int i = rg + NRG * t;
     a[t] = (colv && i < n) ? (i >= j ? Cmat[(long long)i * n + j] : Cmat[(long long)j * n + i]) : 0.0;   // lower triangle, mirrored
   }
@@ -894,19 +901,19 @@ tridiag_reg_kernel(const double* __restrict__ Cmat, int n, double* __restrict__ 
       const int tk = k / NRG;
       double x = a[0];
 #pragma unroll
-      for (int t = 1; t < 16; ++t) x = (tk == t) ? a[t] : x;
-      us[j] = (colv && j > k) ? x : 0.0;
+      for (int t = 1; t < NE; ++t) x = (tk == t) ? a[t] : x;
+      X(j) = (colv && j > k) ? x : 0.0;
       if (j == k) dvec[k] = x;
     }
     __syncthreads();
     double xl[NCG], t2 = 0.0;
 #pragma unroll
-    for (int c = 0; c < NCG; ++c) { xl[c] = us[lane + 32 * c]; t2 += lane + 32 * c > k + 1 ? xl[c] * xl[c] : 0.0; }
+    for (int c = 0; c < NCG; ++c) { xl[c] = X(lane + 32 * c); t2 += lane + 32 * c > k + 1 ? xl[c] * xl[c] : 0.0; }
     const double tail2 = warp_sum(t2);
-    const double alpha = us[k + 1];
+    const double alpha = X(k + 1);
     if (!(tail2 > 1e-280)) {                                      // uniform: every warp reduces the same numbers
       if (tid == 0) evec[k + 1] = alpha;
-      __syncthreads();                                           // us is rewritten by the next step
+      __syncthreads();                                           // up is rewritten by the next step
       continue;
     }
     const double s2 = fma(alpha, alpha, tail2);
@@ -914,41 +921,59 @@ tridiag_reg_kernel(const double* __restrict__ Cmat, int n, double* __restrict__ 
     const double beta = alpha >= 0.0 ? -sigma : sigma;
     const double gamma = __drcp_rn(fma(-alpha, beta, s2));
     const double u1 = alpha - beta;
-    double ui[KEEPU ? 16 : 1];
-    const double uj = j == k + 1 ? u1 : us[j];
-    double p0 = 0.0, p1 = 0.0, p2 = 0.0, p3 = 0.0;
+    // a warp whose 32 columns have all been eliminated, and groups of four rows that have been or lie beyond n, do
+    // nothing: their u, p are zero (uniform branches)
+    const bool wact = KEEPU || 32 * cg + 31 > k;                   // (the small variant skips nothing: the tests cost more)
+    double ui[KEEPU ? NE : 1];
+    const double uj = j == k + 1 ? u1 : X(j);
+    if (wact) {
+      double p0 = 0.0, p1 = 0.0, p2 = 0.0, p3 = 0.0;
 #pragma unroll
-    for (int t = 0; t < 16; t += 4) {
-      double u[4];
+      for (int t = 0; t < NE; t += 4) {
+        if (KEEPU || (rg + NRG * (t + 3) > k && rg + NRG * t < n)) {
+          double u[4];
 #pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        const int i = rg + NRG * (t + q);
-        u[q] = i == k + 1 ? u1 : us[i];                            // us[i] = 0 for i <= k and i >= n
-        if (KEEPU) ui[t + q] = u[q];
+          for (int q = 0; q < 4; ++q) {
+            const int i = rg + NRG * (t + q);
+            u[q] = i == k + 1 ? u1 : X(i);                         // x_i = 0 for i <= k and i >= n
+            if (KEEPU) ui[t + q] = u[q];
+          }
+          p0 = fma(a[t], u[0], p0); p1 = fma(a[t + 1], u[1], p1);
+          p2 = fma(a[t + 2], u[2], p2); p3 = fma(a[t + 3], u[3], p3);
+        }
       }
-      p0 = fma(a[t], u[0], p0); p1 = fma(a[t + 1], u[1], p1);
-      p2 = fma(a[t + 2], u[2], p2); p3 = fma(a[t + 3], u[3], p3);
+      part[rg][j] = (p0 + p1) + (p2 + p3);
     }
-    part[rg][j] = (p0 + p1) + (p2 + p3);
     __syncthreads();
     if (rg == 0) {
       double sum = 0.0;
+      if (wact) {
 #pragma unroll
-      for (int r = 0; r < NRG; r += 2) sum += part[r][j] + part[r + 1][j];
-      pb[j] = (colv && j > k) ? gamma * sum : 0.0;
+        for (int r = 0; r < NRG; r += 2) sum += part[r][j] + part[r + 1][j];
+      }
+      Pv(j) = (colv && j > k) ? gamma * sum : 0.0;
     }
     __syncthreads();
     double pu = 0.0;
 #pragma unroll
-    for (int c = 0; c < NCG; ++c) pu = fma(pb[lane + 32 * c], lane + 32 * c == k + 1 ? u1 : xl[c], pu);
+    for (int c = 0; c < NCG; ++c) pu = fma(Pv(lane + 32 * c), lane + 32 * c == k + 1 ? u1 : xl[c], pu);
     const double cf = 0.5 * gamma * warp_sum(pu);
-    const double pj = pb[j];
-    const double aj = fma(-2.0 * cf, uj, pj), bj = uj;           // both 0 for j <= k: rows and columns <= k stay as they are
+    if (wact) {
+      const double pj = Pv(j);
+      const double aj = fma(-2.0 * cf, uj, pj), bj = uj;         // both 0 for j <= k: columns <= k stay as they are
 #pragma unroll
-    for (int t = 0; t < 16; ++t) {
-      const int i = rg + NRG * t;
-      const double u = KEEPU ? ui[t] : (i == k + 1 ? u1 : us[i]);
-      a[t] = fma(-pb[i], bj, fma(-u, aj, a[t]));
+      for (int t = 0; t < NE; t += 4) {
+        if (KEEPU || (rg + NRG * (t + 3) > k && rg + NRG * t < n)) {
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            const int i = rg + NRG * (t + q);
+            double u, pi;                                         // (x_i, p_i): both 0 for i <= k and i >= n
+            if (KEEPU) { u = ui[t + q]; pi = pb[i]; }
+            else { const double2 w = up[i]; u = i == k + 1 ? u1 : w.x; pi = w.y; }
+            a[t + q] = fma(-pi, bj, fma(-u, aj, a[t + q]));
+          }
+        }
+      }
     }
     if (tid == 0) evec[k + 1] = beta;
   }
@@ -956,7 +981,7 @@ tridiag_reg_kernel(const double* __restrict__ Cmat, int n, double* __restrict__ 
   {
     const int i1 = n - 1, i2 = n - 2;
 #pragma unroll
-    for (int t = 0; t < 16; ++t) {
+    for (int t = 0; t < NE; ++t) {
       const int i = rg + NRG * t;
       if (n >= 2 && i == i2 && j == i2) dvec[i2] = a[t];
       if (n >= 2 && i == i1 && j == i2) evec[i1] = a[t];

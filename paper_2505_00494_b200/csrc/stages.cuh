@@ -230,7 +230,8 @@ int stage_spectrum(qrctm* h, double* s_out, int update_prev, cudaStream_t st, bo
                                  (int)tri2_smem_bytes(TRI2_MAX_N)));
       attr2 = true;
     }
-    if (chi <= TRIR_MAX_N) tridiag_reg_kernel<2, 4><<<1, 256, 0, st>>>(h->C, chi, h->dvec, h->evec);
+    if (chi <= TRIR_MAX_N) tridiag_reg_kernel<2, 4, 16><<<1, 256, 0, st>>>(h->C, chi, h->dvec, h->evec);
+    else if (chi <= TRIR_MAX_N2) tridiag_reg_kernel<4, 4, 32><<<1, 512, 0, st>>>(h->C, chi, h->dvec, h->evec);
     else tridiag_smem2_kernel<<<1, TRI2_NT, tri2_smem_bytes(chi), st>>>(h->C, chi, h->dvec, h->evec, nullptr);
     multisect_kernel<<<(chi + 3) / 4, 128, sizeof(double) * (2 * chi + 40), st>>>(h->dvec, h->evec, chi, h->eig);
     spectrum_finalize_kernel<<<1, nt, sizeof(double) * (chi + 40), st>>>(h->eig, chi, s_out, h->s_prev, h->delta,

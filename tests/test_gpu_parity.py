@@ -346,10 +346,11 @@ def test_cfg1_fixed_count_and_kappa():
 
 def test_spectrum_kernel_against_lapack():
     import torch
-    # chi <= 24: one fused kernel (one-warp tridiagonalisation); <= 64: the register-resident kernel; <= 216 / 236:
-    # shared-memory tridiagonalisations; above: the multi-CTA tridiagonalisation of the eigen step
+    # chi <= 24: one fused kernel (one-warp tridiagonalisation); <= 64 / 128: the register-resident kernels (256 / 512
+    # threads); <= 216 / 236: shared-memory tridiagonalisations; above: the multi-CTA tridiagonalisation of the eigen step
     for chi, seed in [(1, 0), (2, 1), (3, 10), (8, 2), (24, 11), (25, 12), (31, 17), (32, 13), (33, 14), (36, 3), (40, 15),
-                      (41, 16), (63, 18), (64, 19), (65, 20), (100, 4), (196, 5), (236, 6), (237, 7), (400, 8), (700, 9)]:
+                      (41, 16), (63, 18), (64, 19), (65, 20), (100, 4), (127, 21), (128, 22), (129, 23), (196, 5), (236, 6), (237, 7),
+                      (400, 8), (700, 9)]:
         A, C0, T0 = gen_config(2, 1, chi, seed)
         h = pkg.QRCTM(2, 1, chi)
         h.set_A(A); h.set_env(C0, T0)
@@ -374,10 +375,11 @@ def test_tridiag_kernel_preserves_the_spectrum(n):
 
 
 @pytest.mark.parametrize("name,n", [("identity", 30), ("diag", 37), ("block", 32), ("ones", 33), ("rank2", 40), ("zero_tail", 20),
-                                    ("identity", 64), ("block", 56), ("ones", 16), ("rank2", 61), ("zero_tail", 50), ("diag", 12)])
+                                    ("identity", 64), ("block", 56), ("ones", 16), ("rank2", 61), ("zero_tail", 50), ("diag", 12),
+                                    ("identity", 100), ("block", 128), ("ones", 90), ("rank2", 113), ("zero_tail", 70), ("diag", 77)])
 def test_spectrum_small_structured_matrices(name, n):
     """The small tridiagonalisations (one warp for n <= 24, registers for n <= 64) on matrices whose reflectors vanish or
-    whose trailing block is rounding noise: identity, diagonal, block-diagonal of all-ones blocks, all ones, rank two, a
+    whose trailing block is rounding noise (n <= 128: 512-thread register kernel): identity, diagonal, block-diagonal of all-ones blocks, all ones, rank two, a
     matrix with an exactly zero tail."""
     g = np.random.default_rng(n)
     if name == "identity": C = np.eye(n)
