@@ -79,7 +79,7 @@ enum {
                                 qrctm_step / qrctm_run (needs a non-default stream); 0 = plain launches, which keep
                                 the per-stage NVTX ranges for profilers */
   QRCTM_OPT_K8_PATH = 10,    /* K8 tridiagonalisation for chi <= 216: 0 [default] = the round-2 kernels (chi <= 24 fused
-                                into one launch, chi <= 64 register-resident kernel, else thread-per-column kernel with un-
+                                into one launch, chi <= 128 register-resident kernels, else thread-per-column kernel with un-
                                 normalised reflectors), 1 = the round-1 kernel (for cross-checks) */
   QRCTM_OPT_SMALL_PATH = 11, /* 0 [default] = problems with chi <= 8 whose whole working set fits one CTA's shared memory
                                 (2 m^2 + D^8 + 5 m chi doubles <= ~200 KB; cfg0) run K1..K6 as ONE kernel and K7 as one
