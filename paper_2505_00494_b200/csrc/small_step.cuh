@@ -26,6 +26,116 @@ __host__ __device__ inline size_t small_front_doubles(int b, int chi) {
 // Tn (m x chi), Cn (chi x chi) -- the un-normalised C', T' that K7 consumes.
 // (no __restrict__ on the bodies: small_run_kernel calls them in a loop in which C, T are rewritten by the K7 body, so
 // their loads must not go through the non-coherent read-only path)
+// Householder QR of a tiny c~ (chi <= 8 columns, m <= 32 RPL rows) by ONE warp: lane l holds the rows l + 32 r in registers,
+// no block barrier per column, the dot products of a reflector with all columns are reduced together.  Same reflectors
+// (dlarfg convention) and sign fix (diag(R) >= 0) as the column loop in small_front_body.  X (m x chi) -> Q, R, all in
+// shared memory.
+template <int RPL>
+__device__ __forceinline__ void small_qr_warp(const double* X, double* Q, double* R, int m, int chi, int lane) {
+  double x[RPL][8], q[RPL][8], tauv[8];
+#pragma unroll
+  for (int r = 0; r < RPL; ++r)
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+      const int i = lane + 32 * r;
+      x[r][c] = (i < m && c < chi) ? X[i * chi + c] : 0.0;
+      q[r][c] = (i == c) ? 1.0 : 0.0;
+    }
+#pragma unroll
+  for (int k = 0; k < 8; ++k) {
+    tauv[k] = 0.0;
+    if (k < chi) {
+      double acc = 0.0;
+#pragma unroll
+      for (int r = 0; r < RPL; ++r) { const int i = lane + 32 * r; if (i > k) acc = fma(x[r][k], x[r][k], acc); }
+      const double tail2 = warp_sum(acc);
+      const double alpha = __shfl_sync(0xffffffffu, x[0][k], k);
+      double t = 0.0, scale = 0.0, beta = alpha;
+      if (tail2 > 0.0) {                                            // one rsqrt and two independent reciprocals instead of
+        const double s2 = fma(alpha, alpha, tail2);                 // sqrt and two divisions (~250 cycles less per column)
+        const double sigma = s2 * rsqrt(s2);
+        beta = alpha >= 0.0 ? -sigma : sigma;
+        t = (beta - alpha) * __drcp_rn(beta);
+        scale = __drcp_rn(alpha - beta);
+      }
+      double v[RPL];
+#pragma unroll
+      for (int r = 0; r < RPL; ++r) {
+        const int i = lane + 32 * r;
+        v[r] = i > k ? x[r][k] * scale : (i == k ? 1.0 : 0.0);
+        x[r][k] = i > k ? v[r] : (i == k ? beta : x[r][k]);          // reflector below the diagonal, R on and above it
+      }
+      tauv[k] = t;
+      if (t != 0.0) {
+        double d[8];
+#pragma unroll
+        for (int c = 0; c < 8; ++c) { double acc2 = 0.0;
+          if (c > k) {
+#pragma unroll
+            for (int r = 0; r < RPL; ++r) acc2 = fma(v[r], x[r][c], acc2);
+          }
+          d[c] = acc2; }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+          for (int c = 0; c < 8; ++c) if (c > k) d[c] += __shfl_xor_sync(0xffffffffu, d[c], o);
+#pragma unroll
+        for (int c = 0; c < 8; ++c)
+          if (c > k) {
+            const double w = t * d[c];
+#pragma unroll
+            for (int r = 0; r < RPL; ++r) x[r][c] = fma(-v[r], w, x[r][c]);
+          }
+      }
+    }
+  }
+#pragma unroll
+  for (int k = 7; k >= 0; --k) {                                  // Q = H_0 ... H_{chi-1} [I; 0]
+    if (k < chi && tauv[k] != 0.0) {
+      double v[RPL];
+#pragma unroll
+      for (int r = 0; r < RPL; ++r) { const int i = lane + 32 * r; v[r] = i > k ? x[r][k] : (i == k ? 1.0 : 0.0); }
+      double d[8];
+#pragma unroll
+      for (int c = 0; c < 8; ++c) { double acc2 = 0.0;
+        if (c >= k) {
+#pragma unroll
+          for (int r = 0; r < RPL; ++r) acc2 = fma(v[r], q[r][c], acc2);
+        }
+        d[c] = acc2; }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+        for (int c = 0; c < 8; ++c) if (c >= k) d[c] += __shfl_xor_sync(0xffffffffu, d[c], o);
+#pragma unroll
+      for (int c = 0; c < 8; ++c)
+        if (c >= k) {
+          const double w = tauv[k] * d[c];
+#pragma unroll
+          for (int r = 0; r < RPL; ++r) q[r][c] = fma(-v[r], w, q[r][c]);
+        }
+    }
+  }
+  // sign fix: diag(R) >= 0; R's row k is held by lane k (k < 8 <= 32)
+  double sg[8];
+#pragma unroll
+  for (int c = 0; c < 8; ++c) sg[c] = __shfl_sync(0xffffffffu, x[0][c], c) < 0.0 ? -1.0 : 1.0;
+  double mys = 1.0;
+#pragma unroll
+  for (int c = 0; c < 8; ++c) mys = lane == c ? sg[c] : mys;
+#pragma unroll
+  for (int r = 0; r < RPL; ++r)
+#pragma unroll
+    for (int c = 0; c < 8; ++c) {
+      const int i = lane + 32 * r;
+      if (i < m && c < chi) Q[i * chi + c] = q[r][c] * sg[c];
+    }
+  if (lane < chi) {
+#pragma unroll
+    for (int c = 0; c < 8; ++c) if (c < chi) R[lane * chi + c] = c >= lane ? x[0][c] * mys : 0.0;
+  }
+}
+
 template <int NT>
 __device__ __forceinline__ void
 small_front_body(double* ssm, const double* Cg, const double* Tg, const double* ag,
@@ -59,56 +169,65 @@ small_front_body(double* ssm, const double* Cg, const double* Tg, const double* 
   }
   __syncthreads();
   for (int i = tid; i < mc; i += NT) Xg[i] = X[i];
-  // (E2) Householder QR, column by column: warp 0 forms the reflector, then one warp per remaining column applies it
-  for (int k = 0; k < chi; ++k) {
+  // (E2) Householder QR: by one warp in registers where the matrix is small enough (small_qr_warp), else column by column
+  if (chi <= 8 && m <= (NT <= 256 ? 96 : 32)) {       // (the 1024-thread kernels have 64 registers per thread: one row per lane)
     if (warp == 0) {
-      double acc = 0.0;
-      for (int i = k + 1 + lane; i < m; i += 32) { const double x = X[i * chi + k]; acc = fma(x, x, acc); }
-      const double tail2 = warp_sum(acc);
-      const double alpha = X[k * chi + k];
-      double t = 0.0, scale = 0.0, beta = alpha;
-      if (tail2 > 0.0) {
-        const double sigma = sqrt(fma(alpha, alpha, tail2));
-        beta = alpha >= 0.0 ? -sigma : sigma;
-        t = (beta - alpha) / beta;
-        scale = 1.0 / (alpha - beta);
-      }
-      __syncwarp();
-      for (int i = k + 1 + lane; i < m; i += 32) X[i * chi + k] *= scale;
-      if (lane == 0) { X[k * chi + k] = beta; tau[k] = t; }
+      if (m <= 32) small_qr_warp<1>(X, Q, R, m, chi, lane);
+      else if (NT <= 256) small_qr_warp<3>(X, Q, R, m, chi, lane);
     }
     __syncthreads();
-    const double t = tau[k];
-    if (t != 0.0) {
-      for (int j = k + 1 + warp; j < chi; j += NW) {
+  } else {
+    // (E2) Householder QR, column by column: warp 0 forms the reflector, then one warp per remaining column applies it
+    for (int k = 0; k < chi; ++k) {
+      if (warp == 0) {
         double acc = 0.0;
-        for (int i = k + lane; i < m; i += 32) acc = fma(i == k ? 1.0 : X[i * chi + k], X[i * chi + j], acc);
-        const double w = t * warp_sum(acc);
-        for (int i = k + lane; i < m; i += 32) X[i * chi + j] = fma(-(i == k ? 1.0 : X[i * chi + k]), w, X[i * chi + j]);
+        for (int i = k + 1 + lane; i < m; i += 32) { const double x = X[i * chi + k]; acc = fma(x, x, acc); }
+        const double tail2 = warp_sum(acc);
+        const double alpha = X[k * chi + k];
+        double t = 0.0, scale = 0.0, beta = alpha;
+        if (tail2 > 0.0) {
+          const double sigma = sqrt(fma(alpha, alpha, tail2));
+          beta = alpha >= 0.0 ? -sigma : sigma;
+          t = (beta - alpha) / beta;
+          scale = 1.0 / (alpha - beta);
+        }
+        __syncwarp();
+        for (int i = k + 1 + lane; i < m; i += 32) X[i * chi + k] *= scale;
+        if (lane == 0) { X[k * chi + k] = beta; tau[k] = t; }
       }
+      __syncthreads();
+      const double t = tau[k];
+      if (t != 0.0) {
+        for (int j = k + 1 + warp; j < chi; j += NW) {
+          double acc = 0.0;
+          for (int i = k + lane; i < m; i += 32) acc = fma(i == k ? 1.0 : X[i * chi + k], X[i * chi + j], acc);
+          const double w = t * warp_sum(acc);
+          for (int i = k + lane; i < m; i += 32) X[i * chi + j] = fma(-(i == k ? 1.0 : X[i * chi + k]), w, X[i * chi + j]);
+        }
+      }
+      __syncthreads();
     }
+    for (int o = tid; o < cc; o += NT) R[o] = (o % chi >= o / chi) ? X[o] : 0.0;      // X's top chi rows
+    for (int o = tid; o < mc; o += NT) Q[o] = (o / chi == o % chi) ? 1.0 : 0.0;
+    __syncthreads();
+    for (int k = chi - 1; k >= 0; --k) {                   // Q = H_0 ... H_{chi-1} [I; 0]
+      const double t = tau[k];
+      if (t != 0.0) {
+        for (int j = k + warp; j < chi; j += NW) {
+          double acc = 0.0;
+          for (int i = k + lane; i < m; i += 32) acc = fma(i == k ? 1.0 : X[i * chi + k], Q[i * chi + j], acc);
+          const double w = t * warp_sum(acc);
+          for (int i = k + lane; i < m; i += 32) Q[i * chi + j] = fma(-(i == k ? 1.0 : X[i * chi + k]), w, Q[i * chi + j]);
+        }
+      }
+      __syncthreads();
+    }
+    if (tid < chi) wv[tid] = R[tid * chi + tid] < 0.0 ? -1.0 : 1.0;                         // sign fix: diag(R) >= 0
+    __syncthreads();
+    for (int o = tid; o < mc; o += NT) Q[o] *= wv[o % chi];
+    for (int o = tid; o < cc; o += NT) R[o] *= wv[o / chi];
     __syncthreads();
   }
-  for (int o = tid; o < cc; o += NT) R[o] = (o % chi >= o / chi) ? X[o] : 0.0;      // X's top chi rows
-  for (int o = tid; o < mc; o += NT) Q[o] = (o / chi == o % chi) ? 1.0 : 0.0;
-  __syncthreads();
-  for (int k = chi - 1; k >= 0; --k) {                   // Q = H_0 ... H_{chi-1} [I; 0]
-    const double t = tau[k];
-    if (t != 0.0) {
-      for (int j = k + warp; j < chi; j += NW) {
-        double acc = 0.0;
-        for (int i = k + lane; i < m; i += 32) acc = fma(i == k ? 1.0 : X[i * chi + k], Q[i * chi + j], acc);
-        const double w = t * warp_sum(acc);
-        for (int i = k + lane; i < m; i += 32) Q[i * chi + j] = fma(-(i == k ? 1.0 : X[i * chi + k]), w, Q[i * chi + j]);
-      }
-    }
-    __syncthreads();
-  }
-  if (tid < chi) wv[tid] = R[tid * chi + tid] < 0.0 ? -1.0 : 1.0;                         // sign fix: diag(R) >= 0
-  __syncthreads();
-  for (int o = tid; o < mc; o += NT) Q[o] *= wv[o % chi];
-  for (int o = tid; o < cc; o += NT) R[o] *= wv[o / chi];
-  __syncthreads();
   for (int o = tid; o < mc; o += NT) Qg[o] = Q[o];
   for (int o = tid; o < cc; o += NT) Rg[o] = R[o];
   // (E3a) P[(u,l),(J,mm)] = sum_j Q[(j,u),mm] T[j,l,J]
