@@ -1012,7 +1012,7 @@ spectrum_fused_body(double* tsm, const double* Cmat, int n, double* eig_out, dou
   double glo, ghi, isc;
   multisect_setup(dv, ev, n, de, red, glo, ghi, isc);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  for (int idx = warp; idx < n; idx += TRI2_NT / 32) {
+  for (int idx = warp; idx < n; idx += (int)(blockDim.x >> 5)) {
     const double l = multisect_warp<true>(de, n, idx, glo, ghi) * isc;
     if (lane == 0) { lam[idx] = l; eig_out[idx] = l; }
   }

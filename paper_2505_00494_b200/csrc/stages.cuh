@@ -219,7 +219,8 @@ int stage_spectrum(qrctm* h, double* s_out, int update_prev, cudaStream_t st, bo
                                  (int)spectrum_fused_smem_bytes(SPEC_FUSED_MAX_N)));
       attrf = true;
     }
-    spectrum_fused_kernel<<<1, TRI2_NT, spectrum_fused_smem_bytes(chi), st>>>(h->C, chi, h->eig, s_out, h->s_prev, h->delta,
+    // one warp per eigenvalue: 8 warps do for chi <= 8 (a 1024-thread CTA costs more to launch, to synchronise and to retire)
+    spectrum_fused_kernel<<<1, chi <= 8 ? 256 : TRI2_NT, spectrum_fused_smem_bytes(chi), st>>>(h->C, chi, h->eig, s_out, h->s_prev, h->delta,
                                                                            update_prev, h->hist, h->flag + 1, hd, hf, h->flag);
     if (wrote_host) *wrote_host = to_host;
     h->launches += 1;
